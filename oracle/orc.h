@@ -1,0 +1,86 @@
+/* orc.h -- C ABI of the CPU ORACLE of the longitudinal multi-bunch tracker.
+ *
+ * TEST INFRASTRUCTURE ONLY.  This is the plain, slow, single-threaded fp64
+ * restatement of the per-turn method of arXiv:1809.00391 that the
+ * CUDA library (include/mbt.h) is checked against.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may load it.  It shares no code, header, table or helper with the CUDA path.
+ *
+ * All pointers are HOST pointers.  All arrays passed in are copied.
+ * Every function returns 0 on success or a negative ORC_E* code; the text of
+ * the last error is returned by orc_last_error().
+ *
+ * Passages followed (P:l.N = /root/reference/PAPER.md line N):
+ *   P:l.63-71  Eqs.(1),(2)  energy kick and drift
+ *   P:l.83-92  Eq.(5) line 1 radiation damping + quantum excitation
+ *   P:l.94     list of additional harmonic cavities
+ *   P:l.98-115 bins, wake on each bin, kick Eq.(6a)
+ *   P:l.123-125 per-bunch mean / rms statistics
+ *   P:l.229-237 HOM-driven coupled-bunch motion (long-range resonator wake)
+ * plus the readings D1..D30 of DESIGN.md where the paper is silent.
+ */
+#ifndef ORC_H
+#define ORC_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ORC_EINVAL (-1)
+#define ORC_ENOMEM (-2)
+#define ORC_ESTATE (-3)
+
+#define ORC_RES_SR 1u /* resonator enters the short-range table  */
+#define ORC_RES_LR 2u /* resonator enters the long-range sum     */
+
+typedef struct orc_handle orc_handle;
+
+typedef struct { double E0_eV, T0_s, alpha_c, U0_eV; int32_t h; } orc_ring;
+typedef struct { double V_volt; int32_t m; double phase_rad; } orc_cavity;
+typedef struct { int32_t enable; double sigma_delta, damping_turns; } orc_radiation;
+typedef struct {
+  int32_t n_bunches; const int32_t *bucket; const double *charge_C;
+  int64_t n_per_bunch; double sigma_tau0_s, sigma_delta0;
+} orc_fill;
+typedef struct { double Rs_ohm, fr_Hz, Q; uint32_t flags; } orc_resonator;
+typedef struct {
+  int32_t n_bins; double tau_lo_s, tau_hi_s; int32_t gather_order;
+  int32_t n_res; const orc_resonator *res; int32_t history_turns;
+  int32_t n_table; const double *sr_table;
+} orc_wake;
+typedef struct {
+  orc_ring ring; int32_t n_cav; const orc_cavity *cav; orc_radiation rad;
+  orc_fill fill; orc_wake wake; uint64_t seed; int64_t log_capacity_turns;
+  int32_t lr_mode; /* 0: pairwise sum (THE definition); 1: O(M+K) recurrence (long runs) */
+} orc_params;
+
+int orc_create(const orc_params *p, orc_handle **out);
+int orc_track(orc_handle *h, int64_t n_turns);
+int orc_moments(orc_handle *h, double *out /* [M][6]: n_in n_out mean_tau mean_delta rms_tau rms_delta */);
+int orc_destroy(orc_handle *h);
+int orc_get_particles(orc_handle *h, double *tau, double *delta);
+int orc_set_particles(orc_handle *h, const double *tau, const double *delta, int64_t turn);
+int orc_get_histogram(orc_handle *h, uint32_t *out /* [M][n_bins] */);
+int orc_get_wake(orc_handle *h, double *total, double *sr_only, double *lr_only /* each [M][n_bins] or NULL */);
+int orc_get_moment_log(orc_handle *h, int64_t first_turn, int64_t n, double *out /* [n][M][6] */);
+/* source phasors a[b][n'][r] of the last K turns, oldest first: [K][M][R_lr][2] (re, im) */
+int orc_get_lr_history(orc_handle *h, double *out);
+int orc_set_lr_history(orc_handle *h, const double *in);
+int64_t orc_turn(const orc_handle *h);
+double orc_phi_s(const orc_handle *h);
+const char *orc_last_error(void);
+
+/* ---- unit-level entry points used by the pins (tests/) ------------------- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* the two uniforms and the Box-Muller pair of one Philox call */
+void orc_normal_pair(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                     double *u1, double *u2, double *z_c, double *z_s);
+double orc_resonator_wake(double Rs_ohm, double fr_Hz, double Q, double t_s);
+void orc_sr_convolve(int32_t n_bins, const double *w, const double *q, double *V);
+/* one application of the single-particle map (steps 1-3) without wake, z given */
+void orc_map_one(const orc_handle *h, double *tau, double *delta, double z);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

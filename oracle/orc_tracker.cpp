@@ -1,0 +1,630 @@
+// orc_tracker.cpp -- CPU ORACLE (test infrastructure, see orc.h).
+//
+// Plain single-threaded fp64 restatement of the per-turn longitudinal
+// multi-bunch tracking method of arXiv:1809.00391, written step by step in the
+// paper's order.  No blocking, fusion or reordering.  Build with
+//     g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC
+// (no FMA contraction: every product and sum below rounds separately).
+//
+// Turn n, for every bunch b and particle i:
+//   1. RF kick + synchronous loss        P:l.65 Eq.(1), l.94 (harmonic-cavity list)
+//   2. radiation damping + excitation    P:l.85 Eq.(5) line 1
+//   3. drift with the UPDATED delta      P:l.67-69 Eq.(2) + the sentence before it (D1)
+//   4. bin assignment + per-bin count    P:l.98, l.109-111
+//   5. short-range wake on the bins      P:l.98 "excitation of this wake on each bin"
+//   6. long-range resonator wake         P:l.229-237 (formula: reading D14)
+//   7. wake kick                         P:l.102 Eq.(6a) (reading D9: delta -= V/E0)
+//   8. per-bunch mean / rms              P:l.123-125
+//
+// PINS (tests/test_oracle_*.py, all run without a GPU):
+//   philox4x32_10   Random123 known-answer vectors + cuRAND's host-callable Philox header
+//   normal_pair     moments / KS test against scipy.stats.norm
+//   resonator_wake  numerical inverse Fourier transform of the resonator impedance,
+//                   loss factor of a binned Gaussian vs (1/pi) int Re Z exp(-w^2 s^2) dw
+//   map (1,3)       small-amplitude synchrotron tune (FFT), Jacobian determinant 1
+//   radiation (2)   centroid damping time, equilibrium energy spread
+//   histogram (4)   numpy sort-and-count, sum + n_out = N_p, edge cases
+//   SR wake (5)     numpy O(n^2) brute force, single occupied bin, energy bookkeeping
+//   LR wake (6)     numpy brute-force pairwise sum, geometric-series closed form,
+//                   lr_mode 1 (recurrence) against lr_mode 0 (definition)
+//   whole loop      coupled-bunch growth rate vs the analytic uniform-fill formula, Eq.(7)
+//   moments (8)     numpy mean / std
+#include "orc.h"
+
+#include <cmath>
+#include <complex>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+namespace {
+
+typedef std::complex<double> cplx;
+typedef long double ldbl;
+
+thread_local std::string g_err = "";
+
+int fail(int code, const std::string &msg) {
+  g_err = msg;
+  return code;
+}
+
+const ldbl PI_L = 3.141592653589793238462643383279502884L;
+const double PI_D = 3.14159265358979323846;
+
+// ---------------------------------------------------------------- Philox4x32-10
+// Salmon, Moraes, Dror, Shaw, "Parallel random numbers: as easy as 1, 2, 3", SC'11.
+// Round: (hi0:lo0) = M0*c0, (hi1:lo1) = M1*c2;  c <- (hi1^c1^k0, lo1, hi0^c3^k1, lo0);
+// the key is bumped by the Weyl constants AFTER each round's use.
+void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+  uint32_t k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    uint64_t p0 = (uint64_t)M0 * (uint64_t)c0;
+    uint64_t p1 = (uint64_t)M1 * (uint64_t)c2;
+    uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    uint32_t n0 = hi1 ^ c1 ^ k0;
+    uint32_t n1 = lo1;
+    uint32_t n2 = hi0 ^ c3 ^ k1;
+    uint32_t n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += W0;
+    k1 += W1;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Reading D8: key = (seed mod 2^32, seed >> 32); the two uniforms use the
+// top 52 bits of each 64-bit half, u = (k + 1/2) 2^-52, exactly representable and
+// strictly inside (0,1); Box-Muller gives the pair (z_c, z_s).
+void normal_pair(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                 double *u1o, double *u2o, double *zc, double *zs) {
+  uint32_t ctr[4] = {c0, c1, c2, c3};
+  uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32)};
+  uint32_t x[4];
+  philox4x32_10(ctr, key, x);
+  uint64_t w1 = ((uint64_t)x[1] << 32) | (uint64_t)x[0];
+  uint64_t w2 = ((uint64_t)x[3] << 32) | (uint64_t)x[2];
+  double u1 = ((double)(w1 >> 12) + 0.5) * 0x1p-52;
+  double u2 = ((double)(w2 >> 12) + 0.5) * 0x1p-52;
+  double r = std::sqrt(-2.0 * std::log(u1));
+  double theta = 2.0 * PI_D * u2;
+  *zc = r * std::cos(theta);
+  *zs = r * std::sin(theta);
+  if (u1o) *u1o = u1;
+  if (u2o) *u2o = u2;
+}
+
+enum { TAG_EXCITATION = 0, TAG_INITIAL = 1 };
+
+// ---------------------------------------------------------------- resonator
+struct Resonator {
+  double Rs, fr, Q;
+  uint32_t flags;
+  // derived (reading D10): w_r = 2 pi f_r, alpha = w_r/(2Q), wbar = sqrt(w_r^2 - alpha^2)
+  ldbl alpha_l, wbar_l;
+  double alpha, wbar;
+  cplx C;  // 2 alpha Rs (1 + i alpha / wbar):  W(t>0) = Re[C exp(lambda t)]
+};
+
+void derive(Resonator &r) {
+  ldbl wr = 2.0L * PI_L * (ldbl)r.fr;
+  r.alpha_l = wr / (2.0L * (ldbl)r.Q);
+  r.wbar_l = sqrtl(wr * wr - r.alpha_l * r.alpha_l);
+  r.alpha = (double)r.alpha_l;
+  r.wbar = (double)r.wbar_l;
+  r.C = cplx(2.0 * r.alpha * r.Rs, 2.0 * r.alpha * r.Rs * (r.alpha / r.wbar));
+}
+
+// W(t) [V/C]: causal resonator wake, W(0) = alpha Rs = W(0+)/2 (beam-loading theorem), W(t<0) = 0.
+double resonator_wake(const Resonator &r, double t) {
+  if (t < 0.0) return 0.0;
+  if (t == 0.0) return r.alpha * r.Rs;
+  return 2.0 * r.alpha * r.Rs * std::exp(-r.alpha * t) *
+         (std::cos(r.wbar * t) - (r.alpha / r.wbar) * std::sin(r.wbar * t));
+}
+
+// exp(lambda * dt), lambda = -alpha + i wbar, for dt up to K turns: the phase wbar*dt reaches
+// 1e5..1e6 rad, so it is formed and reduced in extended precision, then rounded to fp64.
+cplx exp_lambda(const Resonator &r, ldbl dt) {
+  ldbl mag = expl(-r.alpha_l * dt);
+  ldbl ph = r.wbar_l * dt;
+  return cplx((double)(mag * cosl(ph)), (double)(mag * sinl(ph)));
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------- handle
+struct orc_handle {
+  // parameters
+  orc_ring ring;
+  std::vector<orc_cavity> cav;
+  orc_radiation rad;
+  int M = 0;
+  int64_t Np = 0;
+  std::vector<int32_t> bucket;
+  std::vector<double> charge;
+  double sigma_tau0 = 0, sigma_delta0 = 0;
+  int nb = 0;
+  double tau_lo = 0, tau_hi = 0;
+  int gather = 1;
+  std::vector<Resonator> res_lr;
+  int K = 0;
+  uint64_t seed = 0;
+  int lr_mode = 0;
+  int64_t log_cap = 0;
+  // derived
+  double omega_rf = 0, T_rf = 0, phi_s = 0, D_E = 0, A_q = 0, drift = 0, Delta = 0, invDelta = 0;
+  std::vector<double> centre;  // c_j
+  std::vector<double> w;       // SR table w_k = sum_r W_r(k Delta)
+  bool have_sr = false;
+  // state
+  int64_t turn = 0;
+  std::vector<double> tau, delta, tpos;
+  std::vector<uint32_t> hist;
+  std::vector<int64_t> n_out;
+  std::vector<double> Vsr, Vlr, V;
+  std::vector<cplx> ring_a;  // [(K+1)][M][R]: source phasors a[b][n'][r], slot n' % (K+1)
+  std::vector<double> mom;   // [M][6]
+  std::vector<double> log;   // [log_cap][M][6]
+  // lr_mode 1 tables
+  std::vector<cplx> g_step;  // [M-1][R] exp(lambda (s_{j+1}-s_j) T_rf)
+  std::vector<cplx> g_hist;  // [K][R]   exp(lambda (k T0 - (s_{M-1}-s_0) T_rf)), k = 1..K
+  std::vector<cplx> g_tail;  // [M][R]   exp(lambda (s_{M-1}-s_j) T_rf)
+  std::vector<cplx> ring_A;  // [(K+1)][R] per-turn aggregates A_{n'}
+
+  int R() const { return (int)res_lr.size(); }
+  cplx &a_at(int64_t n, int b, int r) { return ring_a[((size_t)(n % (K + 1)) * M + b) * R() + r]; }
+};
+
+namespace {
+
+ldbl dt_between(const orc_handle *h, int64_t dn, int ds) {
+  ldbl T0 = (ldbl)h->ring.T0_s;
+  return (ldbl)dn * T0 + (ldbl)ds * (T0 / (ldbl)h->ring.h);
+}
+
+// steps 1-3 for one particle; z is the unit normal of step 2
+inline void map_one(const orc_handle *h, double &tau, double &delta, double z) {
+  // 1. delta += sum_c (V_c/E0) sin(m_c w_rf tau + phi_c) - U0/E0   (terms left to right)
+  const double E0 = h->ring.E0_eV;
+  for (size_t c = 0; c < h->cav.size(); ++c) {
+    const orc_cavity &cv = h->cav[c];
+    delta += (cv.V_volt / E0) * std::sin((double)cv.m * h->omega_rf * tau + cv.phase_rad);
+  }
+  delta -= h->ring.U0_eV / E0;
+  // 2. delta = delta (1 - D_E) + sigma_delta sqrt(2 D_E) z
+  if (h->rad.enable) delta = delta * (1.0 - h->D_E) + h->A_q * z;
+  // 3. tau += alpha_c T0 delta  (the delta just updated, reading D1)
+  tau += h->drift * delta;
+}
+
+void compute_moments(orc_handle *h) {
+  // 8. population mean / rms over ALL particles of the bunch, two passes (reading D22)
+  for (int b = 0; b < h->M; ++b) {
+    const double *t = &h->tau[(size_t)b * h->Np];
+    const double *d = &h->delta[(size_t)b * h->Np];
+    double st = 0, sd = 0;
+    for (int64_t i = 0; i < h->Np; ++i) { st += t[i]; sd += d[i]; }
+    double mt = st / (double)h->Np, md = sd / (double)h->Np;
+    double vt = 0, vd = 0;
+    for (int64_t i = 0; i < h->Np; ++i) {
+      vt += (t[i] - mt) * (t[i] - mt);
+      vd += (d[i] - md) * (d[i] - md);
+    }
+    double *m = &h->mom[(size_t)b * 6];
+    m[0] = (double)(h->Np - h->n_out[b]);
+    m[1] = (double)h->n_out[b];
+    m[2] = mt;
+    m[3] = md;
+    m[4] = std::sqrt(vt / (double)h->Np);
+    m[5] = std::sqrt(vd / (double)h->Np);
+  }
+}
+
+// step 4 for the current coordinates (also used after set_particles so that n_in / n_out and the
+// histogram describe the uploaded state)
+void bin_all(orc_handle *h) {
+  std::fill(h->hist.begin(), h->hist.end(), 0u);
+  std::fill(h->n_out.begin(), h->n_out.end(), (int64_t)0);
+  for (int b = 0; b < h->M; ++b)
+    for (int64_t i = 0; i < h->Np; ++i) {
+      size_t p = (size_t)b * h->Np + i;
+      // 4. t = (tau - tau_lo) * invDelta; in-window iff 0 <= t < n_b; j = floor(t)
+      double t = (h->tau[p] - h->tau_lo) * h->invDelta;
+      h->tpos[p] = t;
+      if (t >= 0.0 && t < (double)h->nb) {
+        int j = (int)std::floor(t);
+        h->hist[(size_t)b * h->nb + j] += 1u;
+      } else {
+        h->n_out[b] += 1;
+      }
+    }
+}
+
+void one_turn(orc_handle *h) {
+  const int M = h->M, nb = h->nb, R = h->R(), K = h->K;
+  const int64_t Np = h->Np;
+  const int64_t n = h->turn + 1;
+  // 1-3: single-particle map
+  for (int b = 0; b < M; ++b)
+    for (int64_t i = 0; i < Np; ++i) {
+      size_t p = (size_t)b * Np + i;
+      double z = 0.0;
+      if (h->rad.enable) {
+        double zc, zs;
+        normal_pair(h->seed, (uint32_t)(i >> 1), (uint32_t)b, (uint32_t)n, TAG_EXCITATION, nullptr, nullptr, &zc, &zs);
+        z = (i & 1) ? zs : zc;
+      }
+      map_one(h, h->tau[p], h->delta[p], z);
+    }
+  // 4: bins
+  bin_all(h);
+  // 5: short-range wake, V_SR[b][j] = sum_{k<=j} w[j-k] q[b][k], q = (Q_b/N_p) hist
+  std::vector<double> q((size_t)nb);
+  for (int b = 0; b < M; ++b) {
+    double qm = h->charge[b] / (double)Np;
+    for (int k = 0; k < nb; ++k) q[k] = qm * (double)h->hist[(size_t)b * nb + k];
+    double *Vs = &h->Vsr[(size_t)b * nb];
+    if (h->have_sr)
+      orc_sr_convolve(nb, h->w.data(), q.data(), Vs);
+    else
+      for (int j = 0; j < nb; ++j) Vs[j] = 0.0;
+  }
+  // 6: long-range resonator wake
+  std::fill(h->Vlr.begin(), h->Vlr.end(), 0.0);
+  if (R > 0) {
+    // source phasors a[b][n][r] = sum_k q[b][k] exp(-lambda_r c_k)
+    for (int b = 0; b < M; ++b) {
+      double qm = h->charge[b] / (double)Np;
+      for (int r = 0; r < R; ++r) {
+        const Resonator &rs = h->res_lr[r];
+        cplx lam(-rs.alpha, rs.wbar);
+        cplx a(0.0, 0.0);
+        for (int k = 0; k < nb; ++k) {
+          double qk = qm * (double)h->hist[(size_t)b * nb + k];
+          a += qk * std::exp(-lam * h->centre[k]);
+        }
+        h->a_at(n, b, r) = a;
+      }
+    }
+    std::vector<cplx> P((size_t)M * R, cplx(0, 0));
+    if (h->lr_mode == 0) {
+      // THE definition: pairwise sum over H(b,n)
+      for (int b = 0; b < M; ++b)
+        for (int r = 0; r < R; ++r) {
+          const Resonator &rs = h->res_lr[r];
+          cplx acc(0, 0);
+          int64_t first = (n - K > 1) ? (n - K) : 1;
+          for (int64_t np = first; np <= n - 1; ++np)
+            for (int bp = 0; bp < M; ++bp)
+              acc += h->a_at(np, bp, r) * exp_lambda(rs, dt_between(h, n - np, h->bucket[b] - h->bucket[bp]));
+          for (int bp = 0; bp < M; ++bp)
+            if (h->bucket[bp] < h->bucket[b])
+              acc += h->a_at(n, bp, r) * exp_lambda(rs, dt_between(h, 0, h->bucket[b] - h->bucket[bp]));
+          P[(size_t)b * R + r] = acc;
+        }
+    } else {
+      // equivalent O(M+K) form; only decaying factors occur
+      for (int r = 0; r < R; ++r) {
+        cplx G(0, 0);
+        for (int k = 1; k <= K && n - k >= 1; ++k)
+          G += h->ring_A[(size_t)((n - k) % (K + 1)) * R + r] * h->g_hist[(size_t)(k - 1) * R + r];
+        cplx Pj = G, own(0, 0);
+        for (int j = 0; j < M; ++j) {
+          P[(size_t)j * R + r] = Pj;
+          own += h->a_at(n, j, r) * h->g_tail[(size_t)j * R + r];
+          if (j + 1 < M) Pj = (Pj + h->a_at(n, j, r)) * h->g_step[(size_t)j * R + r];
+        }
+        h->ring_A[(size_t)(n % (K + 1)) * R + r] = own;
+      }
+    }
+    // V_LR[b][j] = sum_r Re[C_r exp(lambda_r c_j) P[b][r]]
+    for (int b = 0; b < M; ++b)
+      for (int j = 0; j < nb; ++j) {
+        double v = 0.0;
+        for (int r = 0; r < R; ++r) {
+          const Resonator &rs = h->res_lr[r];
+          cplx lam(-rs.alpha, rs.wbar);
+          v += std::real(rs.C * std::exp(lam * h->centre[j]) * P[(size_t)b * R + r]);
+        }
+        h->Vlr[(size_t)b * nb + j] = v;
+      }
+  }
+  for (size_t x = 0; x < h->V.size(); ++x) h->V[x] = h->Vsr[x] + h->Vlr[x];
+  // 7: wake kick on in-window particles, delta -= v/E0 (reading D9)
+  for (int b = 0; b < M; ++b) {
+    const double *Vb = &h->V[(size_t)b * nb];
+    for (int64_t i = 0; i < Np; ++i) {
+      size_t p = (size_t)b * Np + i;
+      double t = h->tpos[p];
+      if (!(t >= 0.0 && t < (double)nb)) continue;
+      double v;
+      if (h->gather == 0) {
+        v = Vb[(int)std::floor(t)];  // nearest grid point: the paper's "kick given to every particle in the bin"
+      } else {
+        double u = t - 0.5;  // linear between bin centres, held constant in the outer half bins (reading D12)
+        if (u <= 0.0) v = Vb[0];
+        else if (u >= (double)(nb - 1)) v = Vb[nb - 1];
+        else {
+          int j0 = (int)std::floor(u);
+          double f = u - (double)j0;
+          v = Vb[j0] + f * (Vb[j0 + 1] - Vb[j0]);
+        }
+      }
+      h->delta[p] -= v / h->ring.E0_eV;
+    }
+  }
+  // 8: statistics
+  compute_moments(h);
+  h->turn = n;
+  if (n - 1 < h->log_cap) std::memcpy(&h->log[(size_t)(n - 1) * M * 6], h->mom.data(), sizeof(double) * M * 6);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *orc_last_error(void) { return g_err.c_str(); }
+
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) { philox4x32_10(ctr, key, out); }
+
+void orc_normal_pair(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, double *u1, double *u2,
+                     double *z_c, double *z_s) {
+  normal_pair(seed, c0, c1, c2, c3, u1, u2, z_c, z_s);
+}
+
+double orc_resonator_wake(double Rs, double fr, double Q, double t) {
+  Resonator r{Rs, fr, Q, 0u, 0, 0, 0, 0, cplx()};
+  derive(r);
+  return resonator_wake(r, t);
+}
+
+// V[j] = sum_{k=0..j} w[j-k] q[k], k ascending -- the definition of the discrete causal convolution
+void orc_sr_convolve(int32_t nb, const double *w, const double *q, double *V) {
+  for (int j = 0; j < nb; ++j) {
+    double acc = 0.0;
+    for (int k = 0; k <= j; ++k) acc += w[j - k] * q[k];
+    V[j] = acc;
+  }
+}
+
+void orc_map_one(const orc_handle *h, double *tau, double *delta, double z) { map_one(h, *tau, *delta, z); }
+
+int orc_create(const orc_params *p, orc_handle **out) {
+  if (!p || !out) return fail(ORC_EINVAL, "null argument");
+  *out = nullptr;
+  const orc_ring &rg = p->ring;
+  if (!(rg.E0_eV > 0) || !(rg.T0_s > 0) || rg.h < 1 || !std::isfinite(rg.alpha_c) || rg.alpha_c == 0.0 ||
+      !std::isfinite(rg.U0_eV))
+    return fail(ORC_EINVAL, "ring: need E0 > 0, T0 > 0, h >= 1, alpha_c != 0");
+  if (p->n_cav < 1 || !p->cav) return fail(ORC_EINVAL, "need at least the main cavity");
+  if (p->fill.n_bunches < 1 || !p->fill.bucket || !p->fill.charge_C || p->fill.n_per_bunch < 1 ||
+      p->fill.n_per_bunch > 0xFFFFFFFFll)
+    return fail(ORC_EINVAL, "fill: need n_bunches >= 1, 1 <= n_per_bunch < 2^32");
+  for (int b = 0; b < p->fill.n_bunches; ++b) {
+    if (p->fill.bucket[b] < 0 || p->fill.bucket[b] >= rg.h) return fail(ORC_EINVAL, "bucket out of [0,h)");
+    if (b > 0 && p->fill.bucket[b] <= p->fill.bucket[b - 1]) return fail(ORC_EINVAL, "buckets not strictly increasing");
+    if (!std::isfinite(p->fill.charge_C[b])) return fail(ORC_EINVAL, "charge not finite");
+  }
+  const orc_wake &wk = p->wake;
+  if (wk.n_bins < 2) return fail(ORC_EINVAL, "n_bins < 2");
+  if (!(wk.tau_hi_s > wk.tau_lo_s) || !((wk.tau_hi_s - wk.tau_lo_s) < rg.T0_s / rg.h))
+    return fail(ORC_EINVAL, "window must satisfy 0 < tau_hi - tau_lo < T_rf");
+  if (wk.gather_order != 0 && wk.gather_order != 1) return fail(ORC_EINVAL, "gather_order must be 0 or 1");
+  if (wk.n_res < 0 || (wk.n_res > 0 && !wk.res)) return fail(ORC_EINVAL, "resonator list");
+  if (wk.n_table < 0 || (wk.n_table > 0 && !wk.sr_table)) return fail(ORC_EINVAL, "sr_table");
+  if (p->rad.enable && (!(p->rad.damping_turns > 0) || !(p->rad.sigma_delta >= 0)))
+    return fail(ORC_EINVAL, "radiation: need damping_turns > 0, sigma_delta >= 0");
+  if (p->log_capacity_turns < 0) return fail(ORC_EINVAL, "log_capacity_turns < 0");
+
+  orc_handle *h = new (std::nothrow) orc_handle();
+  if (!h) return fail(ORC_ENOMEM, "out of memory");
+  try {
+    h->ring = rg;
+    h->cav.assign(p->cav, p->cav + p->n_cav);
+    h->rad = p->rad;
+    h->M = p->fill.n_bunches;
+    h->Np = p->fill.n_per_bunch;
+    h->bucket.assign(p->fill.bucket, p->fill.bucket + h->M);
+    h->charge.assign(p->fill.charge_C, p->fill.charge_C + h->M);
+    h->sigma_tau0 = p->fill.sigma_tau0_s;
+    h->sigma_delta0 = p->fill.sigma_delta0;
+    h->nb = wk.n_bins;
+    h->tau_lo = wk.tau_lo_s;
+    h->tau_hi = wk.tau_hi_s;
+    h->gather = wk.gather_order;
+    h->seed = p->seed;
+    h->lr_mode = p->lr_mode;
+    h->log_cap = p->log_capacity_turns;
+
+    // derived constants
+    h->omega_rf = 2.0 * PI_D * (double)rg.h / rg.T0_s;
+    h->T_rf = rg.T0_s / (double)rg.h;
+    h->D_E = p->rad.enable ? 2.0 / p->rad.damping_turns : 0.0;
+    h->A_q = p->rad.enable ? p->rad.sigma_delta * std::sqrt(2.0 * h->D_E) : 0.0;
+    h->drift = rg.alpha_c * rg.T0_s;
+    h->Delta = (h->tau_hi - h->tau_lo) / (double)h->nb;
+    h->invDelta = (double)h->nb / (h->tau_hi - h->tau_lo);
+    h->centre.resize(h->nb);
+    for (int j = 0; j < h->nb; ++j) h->centre[j] = h->tau_lo + ((double)j + 0.5) * h->Delta;
+
+    // synchronous phase (reading D3): V1 sin(phi_s) = U0 - sum_h V_h sin(phi_h), on the stable side
+    for (int c = 1; c < p->n_cav; ++c)
+      if (std::isnan(h->cav[c].phase_rad)) { delete h; return fail(ORC_EINVAL, "only cavity 0 may leave its phase open"); }
+    if (std::isnan(h->cav[0].phase_rad)) {
+      double u_eff = rg.U0_eV;
+      for (int c = 1; c < p->n_cav; ++c) u_eff -= h->cav[c].V_volt * std::sin(h->cav[c].phase_rad);
+      double s = u_eff / h->cav[0].V_volt;
+      if (!(std::fabs(s) <= 1.0)) { delete h; return fail(ORC_EINVAL, "U0 exceeds the RF voltage: no synchronous phase"); }
+      h->cav[0].phase_rad = (rg.alpha_c > 0.0) ? PI_D - std::asin(s) : std::asin(s);
+    }
+    h->phi_s = h->cav[0].phase_rad;
+
+    // wake sources
+    h->w.assign(h->nb, 0.0);
+    for (int r = 0; r < wk.n_res; ++r) {
+      const orc_resonator &in = wk.res[r];
+      if (!(in.Q > 0.5) || !(in.fr_Hz > 0) || !std::isfinite(in.Rs_ohm)) { delete h; return fail(ORC_EINVAL, "resonator: need Q > 1/2, fr > 0"); }
+      Resonator rr{in.Rs_ohm, in.fr_Hz, in.Q, in.flags, 0, 0, 0, 0, cplx()};
+      derive(rr);
+      if (in.flags & ORC_RES_SR) {
+        h->have_sr = true;
+        for (int k = 0; k < h->nb; ++k) h->w[k] += resonator_wake(rr, (double)k * h->Delta);
+      }
+      if (in.flags & ORC_RES_LR) h->res_lr.push_back(rr);
+    }
+    if (wk.n_table > 0) {  // user-sampled wake at lag k*Delta, added to the resonator table
+      h->have_sr = true;
+      for (int k = 0; k < h->nb && k < wk.n_table; ++k) h->w[k] += wk.sr_table[k];
+    }
+    h->K = wk.history_turns;
+    if (h->R() > 0 && h->K < 0) { delete h; return fail(ORC_EINVAL, "history_turns < 0"); }
+    if (h->R() == 0) h->K = 0;
+
+    // state
+    size_t N = (size_t)h->M * (size_t)h->Np;
+    h->tau.resize(N); h->delta.resize(N); h->tpos.resize(N);
+    h->hist.assign((size_t)h->M * h->nb, 0u);
+    h->n_out.assign(h->M, 0);
+    h->Vsr.assign((size_t)h->M * h->nb, 0.0);
+    h->Vlr.assign((size_t)h->M * h->nb, 0.0);
+    h->V.assign((size_t)h->M * h->nb, 0.0);
+    h->ring_a.assign((size_t)(h->K + 1) * h->M * (h->R() ? h->R() : 1), cplx(0, 0));
+    h->mom.assign((size_t)h->M * 6, 0.0);
+    h->log.assign((size_t)h->log_cap * h->M * 6, 0.0);
+    if (h->R() > 0) {
+      int R = h->R(), M = h->M, K = h->K;
+      h->g_step.assign((size_t)M * R, cplx(0, 0));
+      h->g_tail.assign((size_t)M * R, cplx(0, 0));
+      h->g_hist.assign((size_t)(K ? K : 1) * R, cplx(0, 0));
+      h->ring_A.assign((size_t)(K + 1) * R, cplx(0, 0));
+      int span = h->bucket[M - 1] - h->bucket[0];
+      for (int r = 0; r < R; ++r) {
+        for (int j = 0; j + 1 < M; ++j)
+          h->g_step[(size_t)j * R + r] = exp_lambda(h->res_lr[r], dt_between(h, 0, h->bucket[j + 1] - h->bucket[j]));
+        for (int j = 0; j < M; ++j)
+          h->g_tail[(size_t)j * R + r] = exp_lambda(h->res_lr[r], dt_between(h, 0, h->bucket[M - 1] - h->bucket[j]));
+        for (int k = 1; k <= K; ++k) h->g_hist[(size_t)(k - 1) * R + r] = exp_lambda(h->res_lr[r], dt_between(h, k, -span));
+      }
+    }
+
+    // initial distribution (reading D20): Philox stream 1, counter (i, b, 0, 1); tau = s_tau0 z_c, delta = s_delta0 z_s
+    for (int b = 0; b < h->M; ++b)
+      for (int64_t i = 0; i < h->Np; ++i) {
+        double zc, zs;
+        normal_pair(h->seed, (uint32_t)i, (uint32_t)b, 0u, TAG_INITIAL, nullptr, nullptr, &zc, &zs);
+        h->tau[(size_t)b * h->Np + i] = h->sigma_tau0 * zc;
+        h->delta[(size_t)b * h->Np + i] = h->sigma_delta0 * zs;
+      }
+    bin_all(h);
+    compute_moments(h);
+  } catch (const std::bad_alloc &) {
+    delete h;
+    return fail(ORC_ENOMEM, "out of memory");
+  }
+  *out = h;
+  return 0;
+}
+
+int orc_track(orc_handle *h, int64_t n_turns) {
+  if (!h || n_turns < 0) return fail(ORC_EINVAL, "bad argument");
+  if (h->turn + n_turns > 0xFFFFFFFFll) return fail(ORC_EINVAL, "turn counter would exceed 2^32");
+  for (int64_t t = 0; t < n_turns; ++t) one_turn(h);
+  return 0;
+}
+
+int orc_moments(orc_handle *h, double *out) {
+  if (!h || !out) return fail(ORC_EINVAL, "null argument");
+  std::memcpy(out, h->mom.data(), sizeof(double) * h->mom.size());
+  return 0;
+}
+
+int orc_destroy(orc_handle *h) {
+  delete h;
+  return 0;
+}
+
+int orc_get_particles(orc_handle *h, double *tau, double *delta) {
+  if (!h || !tau || !delta) return fail(ORC_EINVAL, "null argument");
+  std::memcpy(tau, h->tau.data(), sizeof(double) * h->tau.size());
+  std::memcpy(delta, h->delta.data(), sizeof(double) * h->delta.size());
+  return 0;
+}
+
+int orc_set_particles(orc_handle *h, const double *tau, const double *delta, int64_t turn) {
+  if (!h || !tau || !delta || turn < 0) return fail(ORC_EINVAL, "bad argument");
+  std::memcpy(h->tau.data(), tau, sizeof(double) * h->tau.size());
+  std::memcpy(h->delta.data(), delta, sizeof(double) * h->delta.size());
+  h->turn = turn;
+  bin_all(h);
+  compute_moments(h);
+  return 0;
+}
+
+int orc_get_histogram(orc_handle *h, uint32_t *out) {
+  if (!h || !out) return fail(ORC_EINVAL, "null argument");
+  std::memcpy(out, h->hist.data(), sizeof(uint32_t) * h->hist.size());
+  return 0;
+}
+
+int orc_get_wake(orc_handle *h, double *total, double *sr, double *lr) {
+  if (!h) return fail(ORC_EINVAL, "null argument");
+  size_t bytes = sizeof(double) * h->V.size();
+  if (total) std::memcpy(total, h->V.data(), bytes);
+  if (sr) std::memcpy(sr, h->Vsr.data(), bytes);
+  if (lr) std::memcpy(lr, h->Vlr.data(), bytes);
+  return 0;
+}
+
+int orc_get_moment_log(orc_handle *h, int64_t first_turn, int64_t n, double *out) {
+  if (!h || !out || first_turn < 1 || n < 0) return fail(ORC_EINVAL, "bad argument");
+  if (first_turn - 1 + n > h->log_cap || first_turn - 1 + n > h->turn) return fail(ORC_ESTATE, "turns not in the log");
+  std::memcpy(out, &h->log[(size_t)(first_turn - 1) * h->M * 6], sizeof(double) * (size_t)n * h->M * 6);
+  return 0;
+}
+
+int orc_get_lr_history(orc_handle *h, double *out) {
+  if (!h || !out) return fail(ORC_EINVAL, "null argument");
+  int R = h->R(), M = h->M, K = h->K;
+  for (int k = 0; k < K; ++k) {
+    int64_t t = h->turn - K + 1 + k;
+    for (int b = 0; b < M; ++b)
+      for (int r = 0; r < R; ++r) {
+        cplx a = (t >= 1) ? h->a_at(t, b, r) : cplx(0, 0);
+        double *o = &out[(((size_t)k * M + b) * R + r) * 2];
+        o[0] = a.real();
+        o[1] = a.imag();
+      }
+  }
+  return 0;
+}
+
+int orc_set_lr_history(orc_handle *h, const double *in) {
+  if (!h || !in) return fail(ORC_EINVAL, "null argument");
+  int R = h->R(), M = h->M, K = h->K;
+  for (int k = 0; k < K; ++k) {
+    int64_t t = h->turn - K + 1 + k;
+    if (t < 1) continue;
+    cplx A(0, 0);
+    for (int r = 0; r < R; ++r) {
+      cplx agg(0, 0);
+      for (int b = 0; b < M; ++b) {
+        const double *i2 = &in[(((size_t)k * M + b) * R + r) * 2];
+        h->a_at(t, b, r) = cplx(i2[0], i2[1]);
+        agg += h->a_at(t, b, r) * h->g_tail[(size_t)b * R + r];
+      }
+      h->ring_A[(size_t)(t % (K + 1)) * R + r] = agg;
+    }
+  }
+  return 0;
+}
+
+int64_t orc_turn(const orc_handle *h) { return h ? h->turn : -1; }
+double orc_phi_s(const orc_handle *h) { return h ? h->phi_s : NAN; }
+
+}  // extern "C"
