@@ -1,0 +1,294 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fused per-turn hot path (macro-particle-turns/s) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c4] [--impl mbt|reference]
+
+A "step" is one tracked turn of the whole hot path over every macro-particle of the
+workload.  The workload at N = 1 is BASELINE.json configs[3] ("c4": 363 bunches x 1e5 macro-particles, the
+configuration the metric is quoted on), synthetic and seeded (paper_1809_00391_b200/workloads.py).  The particle
+store (581 MB) is larger than the 126 MB L2, so no L2 flush is needed between steps.
+
+N > 1: the path does not shard without a per-turn exchange that BASELINE north_star rules out ("no sharding, no
+collectives"), so every rank tracks an independent replica of the workload (a parameter-scan replica; DESIGN.md
+"Multi-GPU": replicas only) and `value` is the sum over ranks divided by the slowest rank's device time.
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on this host's cores, on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "macro-particle-turns/s"
+BYTES_PER_PARTICLE_TURN = 32.0  # tau, delta read once and written once per turn, fp64
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(prefix="mbt_clocks_", suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+            time.sleep(0.3)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.1)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        try:
+            with open(self.path) as f:
+                for line in f:
+                    c = [x.strip() for x in line.split(",")]
+                    if len(c) < 9:
+                        continue
+                    try:
+                        sm.append(float(c[1])); mx.append(float(c[2]))
+                    except ValueError:
+                        continue
+                    for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                        if v.lower().startswith("active"):
+                            reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def _oracle_sample(cfg_name, budget_s, n_steps):
+    """Bounded sample of the workload for the CPU oracle: same fill pattern, wake sources, bins and history;
+    N_p reduced so that n_steps turns take about budget_s seconds (the oracle runs ~1e7 particle-turns/s/core)."""
+    from paper_1809_00391_b200 import workloads as W
+    full = W.config(cfg_name)
+    m = len(full["fill"]["buckets"])
+    np_full = full["fill"]["n_per_bunch"]
+    per_step = budget_s / max(n_steps, 1) * 8.0e6
+    np_s = int(max(500, min(np_full, per_step / m)))
+    return W.config(cfg_name, n_per_bunch=np_s), np_s, m
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores, rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import orc
+    cfg, np_s, m = _oracle_sample(args.config, 120.0, args.steps + args.warmup)
+    o = orc.Oracle(cfg, lr_mode=1)
+    o.track(args.warmup)
+    t0 = time.perf_counter()
+    o.track(args.steps)
+    dt = time.perf_counter() - t0
+    val = m * np_s * args.steps / dt
+    sample = "%s fill/wake/bins, N_p=%d of %d per bunch, %d turns, lr_mode=1" % (args.config, np_s, W_np(args.config), args.steps)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "particle-turns/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": _workload_name(args.config), "l2": "n/a (CPU)"},
+        "cpu_baseline": {"value": val, "unit": "particle-turns/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "particle-turns/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def W_np(name):
+    from paper_1809_00391_b200 import workloads as W
+    return W.config(name)["fill"]["n_per_bunch"]
+
+
+def _workload_name(name):
+    from paper_1809_00391_b200 import workloads as W
+    c = W.config(name)
+    f, w = c["fill"], c["wake"]
+    return "%s: %d bunches x %d macro-particles, %d bins, %d resonators (%d long-range, %d-turn history), fp64 SoA" % (
+        name, len(f["buckets"]), f["n_per_bunch"], w["n_bins"], len(w["resonators"]),
+        sum(1 for r in w["resonators"] if r["flags"] & 2), w["history_turns"])
+
+
+def run_mbt(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1809_00391_b200 import build, mbt, workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    build.build()
+    cfg = W.config(args.config)
+    n_part = W.n_particles(cfg)
+    K, Wm = args.steps, args.warmup
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    trk = mbt.Tracker(cfg, log_capacity_turns=0, device=local)
+    trk.track(Wm)
+    trk.moments()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = trk.launch_count
+    barrier()
+    trk.track(K)                       # device-timed inside the library with CUDA events on its stream
+    barrier()
+    sec = trk.last_track_seconds()
+    launches = trk.launch_count - l0
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([sec], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        sec = float(t.item())
+    value = world * n_part * K / sec
+
+    # per-kernel device time of the same K steps (event-bracketed plain launches), for the roofline
+    pass_s, wake_s = trk.track_profiled(min(K, 2000))
+    kp = min(K, 2000)
+    peak, peak_src = _peaks()
+    achieved = BYTES_PER_PARTICLE_TURN * n_part / (pass_s / kp) / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_pass<true>", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": BYTES_PER_PARTICLE_TURN * n_part,
+                "pass_ms": pass_s / kp * 1e3, "wake_ms": wake_s / kp * 1e3,
+                "pass_share_of_step": pass_s / (pass_s + wake_s)}
+    prof = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    try:
+        with open(prof) as f:
+            tr = json.load(f)
+        if tr.get("config") == args.config:
+            roofline["traffic"] = tr.get("dram_bytes_per_launch")
+    except Exception:
+        pass
+    trk.close()
+
+    # end to end through the C ABI with HOST buffers: upload the particle state from pinned host memory, track K
+    # turns with the per-turn statistics log, read the statistics back (what the paper's host loop does, P:l.123)
+    e2e = None
+    if True:
+        ld = n_part // len(cfg["fill"]["buckets"])
+        h_tau = torch.empty(n_part, dtype=torch.float64).pin_memory()
+        h_delta = torch.empty(n_part, dtype=torch.float64).pin_memory()
+        t2 = mbt.Tracker(cfg, log_capacity_turns=K, device=local)
+        tau0, delta0 = t2.particles(h_tau.numpy().reshape(len(cfg["fill"]["buckets"]), ld),
+                                    h_delta.numpy().reshape(len(cfg["fill"]["buckets"]), ld))
+        out = np.empty((K, t2.M, 6))
+        barrier()
+        t0 = time.perf_counter()
+        t2.set_particles(tau0, delta0, 0)          # H2D of the whole state (pinned host memory)
+        t2.track(K)
+        out = t2.moment_log(1, K)                  # D2H of the per-turn statistics
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * n_part * K / dt, "unit": "particle-turns/s",
+               "h2d_bytes_per_step": 16.0 * n_part / K, "d2h_bytes_per_step": float(out.nbytes) / K,
+               "what": "mbt_set_particles (pinned host -> device) + mbt_track(K) + mbt_get_moment_log (device -> host), wall clock"}
+        assert np.isfinite(out).all()
+        t2.close()
+
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        from oracle import orc
+        turns = 2
+        t0 = time.perf_counter()
+        o = orc.Oracle(cfg, lr_mode=1)
+        t_init = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        o.track(turns)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n_part * turns / dt, "unit": "particle-turns/s", "cores": 1, "kind": "oracle",
+               "sample": "full %s state, %d turns, lr_mode=1 (init %.1f s not timed)" % (args.config, turns, t_init),
+               "host_cores_available": os.cpu_count()}
+        o.close()
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": "particle-turns/s", "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": sec / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": _workload_name(args.config), "parallelism": "replicas x%d" % world,
+                       "l2": "particle store larger than L2, no flush needed" if 16 * n_part > 126e6 else
+                             "particle store fits L2 (latency-bound config, not an HBM roofline)"},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "algorithmic_GBps_whole_step": BYTES_PER_PARTICLE_TURN * value / world / 1e9,
+        }
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", default="c4")
+    ap.add_argument("--impl", default="mbt", choices=["mbt", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_mbt(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,163 @@
+/* mbt.h -- C ABI of the B200 (sm_100a) longitudinal multi-bunch macro-particle tracker.
+ *
+ * The library tracks M bunches of N_p macro-particles each through the per-turn
+ * method of arXiv:1809.00391 (mbtrack / mbtrack-cuda).  Passages implemented
+ * (P:l.N = PAPER.md line N; D# = reading listed in DESIGN.md):
+ *
+ *   S1  RF kick + synchronous loss       P:l.63-67 Eq.(1), l.94 (list of harmonic cavities)
+ *   S2  radiation damping + excitation   P:l.83-92 Eq.(5) line 1     (Philox4x32-10, D8)
+ *   S3  drift with the updated delta     P:l.67-71 Eq.(2)            (D1)
+ *   S4  bin assignment + per-bin count   P:l.98, l.109-111           (D11)
+ *   S5  short-range wake on the bins     P:l.98, l.107               (D10)
+ *   S6  long-range resonator wake        P:l.229-237                 (D14)
+ *   S0  wake kick  delta -= V(tau)/E0    P:l.102 Eq.(6a), l.115      (D9, D12)
+ *   S7  per-bunch mean / rms             P:l.123-125                 (D22)
+ *
+ * Every step runs in CUDA kernels on the device; there is NO CPU fallback.  All
+ * parameter structs are plain old data; every array passed to mbt_create is a
+ * HOST pointer that is copied before the call returns (the caller keeps ownership).
+ * Particle coordinates live on the device for the whole run (P:l.39) as two fp64
+ * arrays tau[M][ld] and delta[M][ld], ld = mbt_particle_stride(N_p) (N_p rounded up
+ * to an even number so that every bunch starts on a 16-byte boundary).
+ *
+ * Every function returns 0 (MBT_OK) or a negative MBT_E* code; the text of the last
+ * error of the calling thread is returned by mbt_last_error().  No exception and no
+ * abort crosses this boundary.  Functions taking a handle are not thread-safe with
+ * respect to the same handle.
+ *
+ * Observable state: mbt_track() may leave the wake kick of the last turn pending
+ * (it is fused into the head of the next turn's pass); every getter and mbt_moments()
+ * applies it first, so what the caller sees after mbt_track(h, n) is the state
+ * "after turn n's kick", as in the sequential order of the paper (Fig. 2, P:l.47-51).
+ */
+#ifndef MBT_H
+#define MBT_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MBT_OK 0
+#define MBT_EINVAL (-1) /* bad or inconsistent parameter                       */
+#define MBT_ENOMEM (-2) /* host or device allocation failed                    */
+#define MBT_ECUDA (-3)  /* a CUDA call failed; text in mbt_last_error()        */
+#define MBT_ESTATE (-4) /* call not valid in the handle's current state        */
+
+#define MBT_RES_SR 1u /* resonator enters the short-range (same bunch, same turn) table */
+#define MBT_RES_LR 2u /* resonator enters the long-range (other bunches / turns) sum    */
+
+#define MBT_MAX_CAVITIES 8   /* main + harmonic cavities (P:l.94)                 */
+#define MBT_MAX_BINS 4096    /* bins per bunch                                    */
+#define MBT_MAX_LR 8         /* long-range resonators                             */
+#define MBT_MAX_BUNCHES 1024 /* filled buckets (the in-turn scan runs in one CTA) */
+
+typedef struct mbt_handle mbt_handle; /* opaque, library-owned */
+
+/* ring: reference energy [eV], revolution period [s], momentum compaction, energy loss per turn [eV],
+ * harmonic number (P:l.63-71; Table 1 P:l.131-144 lists the same quantities) */
+typedef struct { double E0_eV, T0_s, alpha_c, U0_eV; int32_t h; } mbt_ring;
+
+/* one RF cavity: kick (V/E0) sin(m w_rf tau + phase).  cav[0] is the main cavity; if its phase is NaN the
+ * library solves V_0 sin(phi_s) = U0 - sum_{c>0} V_c sin(phase_c) on the stable side (D3). */
+typedef struct { double V_volt; int32_t m; double phase_rad; } mbt_cavity;
+
+/* radiation (P:l.85 Eq.(5)): D_E = 2/damping_turns, noise amplitude sigma_delta sqrt(2 D_E) (D6) */
+typedef struct { int32_t enable; double sigma_delta, damping_turns; } mbt_radiation;
+
+/* fill pattern: bucket[] strictly increasing in [0,h); charge_C[b] bunch charge [C];
+ * initial distribution: seeded Gaussian, tau = sigma_tau0 z_c, delta = sigma_delta0 z_s (D20) */
+typedef struct {
+  int32_t n_bunches; const int32_t *bucket; const double *charge_C;
+  int64_t n_per_bunch; double sigma_tau0_s, sigma_delta0;
+} mbt_fill;
+
+/* resonator wake W(t>0) = 2 a Rs exp(-a t)[cos(wb t) - (a/wb) sin(wb t)], W(0) = a Rs, a = w_r/2Q (D10) */
+typedef struct { double Rs_ohm, fr_Hz, Q; uint32_t flags; } mbt_resonator;
+
+/* wake: n_bins half-open bins over [tau_lo, tau_hi) around every bucket centre (D11);
+ * gather_order 1 = linear between bin centres (default), 0 = nearest grid point (P:l.98);
+ * history_turns K: the long-range sum covers all bunches of turns n-K..n-1 and the earlier bunches of turn n;
+ * sr_table (optional, n_table samples, V/C at lag k*Delta) is ADDED to the resonator table. */
+typedef struct {
+  int32_t n_bins; double tau_lo_s, tau_hi_s; int32_t gather_order;
+  int32_t n_res; const mbt_resonator *res; int32_t history_turns;
+  int32_t n_table; const double *sr_table;
+} mbt_wake;
+
+typedef struct {
+  mbt_ring ring;
+  int32_t n_cav; const mbt_cavity *cav; /* HOST array, n_cav >= 1 */
+  mbt_radiation rad;
+  mbt_fill fill;
+  mbt_wake wake;
+  uint64_t seed;                /* Philox key (D8)                                                     */
+  int64_t log_capacity_turns;   /* > 0: keep per-turn moments of turns 1..capacity on the device       */
+  void *d_tau, *d_delta;        /* optional caller-owned DEVICE buffers (e.g. torch tensors), each
+                                   n_bunches * mbt_particle_stride(n_per_bunch) doubles, 16-byte aligned,
+                                   alive until mbt_destroy; both NULL -> the library allocates.  They are
+                                   overwritten with the seeded initial distribution.                    */
+  void *stream;                 /* cudaStream_t the library enqueues on (e.g. torch's current stream);
+                                   NULL -> the library creates and owns a (blocking) stream             */
+  int32_t device;               /* CUDA device ordinal; -1 -> the current device                        */
+} mbt_params;
+
+/* Validates, allocates, builds the wake tables and draws the initial distribution on the device.
+ * On failure *out is NULL. */
+int mbt_create(const mbt_params *p, mbt_handle **out);
+
+/* Enqueues n_turns turns on the handle's stream (asynchronous; the turn counter is cumulative and must stay
+ * below 2^32 because it is a Philox counter word). */
+int mbt_track(mbt_handle *h, int64_t n_turns);
+
+/* Per-bunch statistics of the current state into HOST memory, out[M][6]:
+ * n_in, n_out, mean_tau, mean_delta, rms_tau, rms_delta (population rms over all N_p particles, D22).
+ * Synchronises the stream. */
+int mbt_moments(mbt_handle *h, double *out);
+
+/* Frees everything the library allocated (never the caller's d_tau / d_delta).  NULL is allowed. */
+int mbt_destroy(mbt_handle *h);
+
+/* ---- state access used by the parity tests (HOST pointers, packed [M][N_p]; each call synchronises) ---- */
+int mbt_get_particles(mbt_handle *h, double *tau, double *delta);
+/* Upload coordinates and set the turn counter; the pending kick, the wake and the long-range history are
+ * cleared (call mbt_set_lr_history AFTER this call when resuming in the middle of a run). */
+int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int64_t turn);
+/* counts of the current state, out[M][n_bins] */
+int mbt_get_histogram(mbt_handle *h, uint32_t *out);
+/* wake potential [V] on the bin centres built by the last tracked turn; each of total / sr_only / lr_only is
+ * [M][n_bins] or NULL.  All zero before the first turn and after mbt_set_particles. */
+int mbt_get_wake(mbt_handle *h, double *total, double *sr_only, double *lr_only);
+/* per-turn statistics of turns first_turn .. first_turn+n-1 (1-based), out[n][M][6]; needs log_capacity_turns */
+int mbt_get_moment_log(mbt_handle *h, int64_t first_turn, int64_t n, double *out);
+/* long-range source phasors a[b][n'][r] of the last K turns, oldest first, [K][M][R_lr][2] (re, im) */
+int mbt_get_lr_history(mbt_handle *h, double *out);
+int mbt_set_lr_history(mbt_handle *h, const double *in);
+
+/* ---- introspection ---- */
+int64_t mbt_turn(const mbt_handle *h);        /* completed turns, -1 on NULL                 */
+double mbt_phi_s(const mbt_handle *h);        /* synchronous phase of cav[0] [rad]           */
+int64_t mbt_particle_stride(int64_t n_per_bunch); /* ld of the device arrays                 */
+/* DEVICE pointers of the particle store (for zero-copy wrapping, e.g. torch.from_blob-like views) */
+int mbt_device_pointers(mbt_handle *h, void **d_tau, void **d_delta, int64_t *ld);
+/* kernels launched by this handle so far (bench.py's gpu_launches) */
+int64_t mbt_launch_count(const mbt_handle *h);
+/* Seconds of device time of the most recent mbt_track call, measured with CUDA events recorded on the handle's
+ * stream around the enqueued turns; synchronises.  Negative on error. */
+double mbt_last_track_seconds(mbt_handle *h);
+/* Measurement aid: tracks n_turns (1..65536) turns with plain launches instead of graph replay and brackets
+ * every kernel with CUDA events on the handle's stream; returns the summed device time [s] of the fused
+ * particle pass and of the wake kernel.  The turns are real turns (state and turn counter advance).
+ * Synchronises. */
+int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, double *wake_seconds);
+/* Run one Philox4x32-10 block on the device (known-answer tests of the device generator). */
+int mbt_philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* Device Box-Muller pair exactly as the excitation step draws it: HOST arrays of n counters (c0,c1,c2,c3)
+ * in ctr[n][4]; out[n][2] = (z_c, z_s). */
+int mbt_normal_selftest(uint64_t seed, int64_t n, const uint32_t *ctr, double *out);
+const char *mbt_last_error(void); /* thread-local, never NULL */
+const char *mbt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

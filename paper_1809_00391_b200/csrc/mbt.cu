@@ -1,0 +1,709 @@
+// mbt.cu -- host side of the C ABI declared in include/mbt.h: validation, table construction,
+// device memory, per-turn sequencing (CUDA graph replay of {k_pass, k_wake}) and the getters.
+// No step of the method runs on the host: the host only derives constants and tables at create time.
+#include "../../include/mbt.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "mbt_kernels.cuh"
+
+using namespace mbt;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string &msg) {
+  g_err = msg;
+  return code;
+}
+
+#define CU(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) {                                                                       \
+      char buf_[512];                                                                              \
+      snprintf(buf_, sizeof buf_, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+      return fail(e_ == cudaErrorMemoryAllocation ? MBT_ENOMEM : MBT_ECUDA, buf_);                 \
+    }                                                                                              \
+  } while (0)
+
+typedef long double ldbl;
+const ldbl PI_L = 3.141592653589793238462643383279502884L;
+const double PI_D = 3.14159265358979323846;
+
+struct Res {
+  double Rs, fr, Q;
+  ldbl alpha, wbar;  // alpha = w_r / 2Q, wbar = sqrt(w_r^2 - alpha^2)     (D10)
+};
+
+Res make_res(const mbt_resonator &in) {
+  Res r{in.Rs_ohm, in.fr_Hz, in.Q, 0, 0};
+  const ldbl wr = 2.0L * PI_L * (ldbl)in.fr_Hz;
+  r.alpha = wr / (2.0L * (ldbl)in.Q);
+  r.wbar = sqrtl(wr * wr - r.alpha * r.alpha);
+  return r;
+}
+
+// W(t) [V/C], W(0) = alpha Rs, W(t<0) = 0
+double res_wake(const Res &r, ldbl t) {
+  if (t < 0) return 0.0;
+  if (t == 0) return (double)(r.alpha * (ldbl)r.Rs);
+  return (double)(2.0L * r.alpha * (ldbl)r.Rs * expl(-r.alpha * t) * (cosl(r.wbar * t) - (r.alpha / r.wbar) * sinl(r.wbar * t)));
+}
+
+// exp(sign * lambda * t), lambda = -alpha + i wbar, evaluated in extended precision (phases reach 1e6 rad)
+cplx exp_lambda(const Res &r, ldbl t) {
+  const ldbl mag = expl(-r.alpha * t), ph = r.wbar * t;
+  return cplx{(double)(mag * cosl(ph)), (double)(mag * sinl(ph))};
+}
+
+template <class T>
+struct DevBuf {
+  T *p = nullptr;
+  size_t n = 0;
+  cudaError_t alloc(size_t count) {
+    n = count;
+    if (count == 0) count = 1;
+    cudaError_t e = cudaMalloc((void **)&p, count * sizeof(T));
+    if (e == cudaSuccess) e = cudaMemset(p, 0, count * sizeof(T));
+    return e;
+  }
+  cudaError_t upload(const std::vector<T> &v) {
+    cudaError_t e = alloc(v.size());
+    if (e == cudaSuccess && !v.empty()) e = cudaMemcpy(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+    return e;
+  }
+  void release() {
+    if (p) cudaFree(p);
+    p = nullptr;
+  }
+};
+
+}  // namespace
+
+struct mbt_handle {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  bool own_stream = false;
+  int M = 0, nb = 0, R = 0, K = 0;
+  int64_t Np = 0, ld = 0;
+  bool own_particles = false;
+  double *d_tau = nullptr, *d_delta = nullptr;
+  double phi_s = 0.0;
+  int64_t turn = 0;        // host mirror of ctrl.turn
+  bool dirty = true;       // observable quantities (pending kick, moments, counts) need a flush
+  bool wake_valid = false; // a tracked turn has built a wake since create / set_particles
+  int64_t launches = 0;
+  int64_t log_cap = 0;
+  int grid_pass = 0;
+  size_t smem_pass = 0, smem_wake = 0;
+  Args args;
+  WakeArgs wargs;
+  DevBuf<double> qm, w, Vsr, mom_acc, mom_last, mom_log, scratch_a, scratch_b, scratch_c;
+  DevBuf<cplx> Esrc, F, g_step, g_tail, g_hist, a_cur, ring_a, ring_A, P;
+  DevBuf<uint32_t> hist, hist_last;
+  DevBuf<unsigned long long> nout_acc;
+  DevBuf<Ctrl> ctrl;
+  cudaGraphExec_t graph1 = nullptr, graphU = nullptr;
+  int unroll = 16;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool timed = false;
+};
+
+namespace {
+
+int enqueue_turn(mbt_handle *h) {
+  k_pass<true><<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
+  k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
+  return 0;
+}
+
+int build_graph(mbt_handle *h, int turns, cudaGraphExec_t *out) {
+  cudaGraph_t g = nullptr;
+  CU(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+  for (int t = 0; t < turns; ++t) enqueue_turn(h);
+  CU(cudaStreamEndCapture(h->stream, &g));
+  cudaError_t e = cudaGraphInstantiate(out, g, 0);
+  cudaGraphDestroy(g);
+  CU(e);
+  return 0;
+}
+
+// apply the pending kick, close moments and counts of the current state
+int flush(mbt_handle *h) {
+  if (!h->dirty) return 0;
+  CU(cudaSetDevice(h->device));
+  k_pass<false><<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
+  WakeArgs wa = h->wargs;
+  wa.mode = 1;
+  k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(wa);
+  k_clear_pending<<<1, 1, 0, h->stream>>>(h->ctrl.p);
+  h->launches += 3;
+  CU(cudaGetLastError());
+  h->dirty = false;
+  return 0;
+}
+
+void destroy(mbt_handle *h) {
+  if (!h) return;
+  cudaSetDevice(h->device);
+  if (h->stream) cudaStreamSynchronize(h->stream);
+  if (h->graph1) cudaGraphExecDestroy(h->graph1);
+  if (h->graphU) cudaGraphExecDestroy(h->graphU);
+  if (h->ev0) cudaEventDestroy(h->ev0);
+  if (h->ev1) cudaEventDestroy(h->ev1);
+  if (h->own_particles) {
+    if (h->d_tau) cudaFree(h->d_tau);
+    if (h->d_delta) cudaFree(h->d_delta);
+  }
+  h->qm.release(); h->w.release(); h->Vsr.release(); h->mom_acc.release(); h->mom_last.release(); h->mom_log.release();
+  h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
+  h->Esrc.release(); h->F.release(); h->g_step.release(); h->g_tail.release(); h->g_hist.release(); h->a_cur.release();
+  h->ring_a.release(); h->ring_A.release(); h->P.release();
+  h->hist.release(); h->hist_last.release(); h->nout_acc.release(); h->ctrl.release();
+  if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
+  delete h;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *mbt_last_error(void) { return g_err.c_str(); }
+const char *mbt_version(void) { return "mbt-b200 0.1 (sm_100a)"; }
+int64_t mbt_particle_stride(int64_t n) { return n < 0 ? -1 : (n + 1) / 2 * 2; }
+int64_t mbt_turn(const mbt_handle *h) { return h ? h->turn : -1; }
+double mbt_phi_s(const mbt_handle *h) { return h ? h->phi_s : NAN; }
+int64_t mbt_launch_count(const mbt_handle *h) { return h ? h->launches : -1; }
+
+int mbt_create(const mbt_params *p, mbt_handle **out) {
+  if (!p || !out) return fail(MBT_EINVAL, "null argument");
+  *out = nullptr;
+  const mbt_ring &rg = p->ring;
+  if (!(rg.E0_eV > 0) || !(rg.T0_s > 0) || rg.h < 1 || !std::isfinite(rg.alpha_c) || rg.alpha_c == 0.0 ||
+      !std::isfinite(rg.U0_eV))
+    return fail(MBT_EINVAL, "ring: need E0 > 0, T0 > 0, h >= 1, alpha_c != 0");
+  if (p->n_cav < 1 || p->n_cav > MBT_MAX_CAVITIES || !p->cav)
+    return fail(MBT_EINVAL, "need 1..MBT_MAX_CAVITIES cavities, cav[0] the main one");
+  const mbt_fill &fl = p->fill;
+  if (fl.n_bunches < 1 || fl.n_bunches > MBT_MAX_BUNCHES || !fl.bucket || !fl.charge_C)
+    return fail(MBT_EINVAL, "fill: need 1 <= n_bunches <= MBT_MAX_BUNCHES and bucket / charge arrays");
+  if (fl.n_per_bunch < 1 || fl.n_per_bunch > 0x7FFFFFFEll) return fail(MBT_EINVAL, "fill: need 1 <= n_per_bunch < 2^31 - 1");
+  for (int b = 0; b < fl.n_bunches; ++b) {
+    if (fl.bucket[b] < 0 || fl.bucket[b] >= rg.h) return fail(MBT_EINVAL, "bucket out of [0,h)");
+    if (b > 0 && fl.bucket[b] <= fl.bucket[b - 1]) return fail(MBT_EINVAL, "buckets not strictly increasing");
+    if (!std::isfinite(fl.charge_C[b])) return fail(MBT_EINVAL, "charge not finite");
+  }
+  if (!(fl.sigma_tau0_s >= 0) || !(fl.sigma_delta0 >= 0)) return fail(MBT_EINVAL, "initial sigmas must be >= 0");
+  const mbt_wake &wk = p->wake;
+  if (wk.n_bins < 2 || wk.n_bins > MBT_MAX_BINS) return fail(MBT_EINVAL, "need 2 <= n_bins <= MBT_MAX_BINS");
+  if (!(wk.tau_hi_s > wk.tau_lo_s) || !((wk.tau_hi_s - wk.tau_lo_s) < rg.T0_s / rg.h))
+    return fail(MBT_EINVAL, "window must satisfy 0 < tau_hi - tau_lo < T_rf");
+  if (wk.gather_order != 0 && wk.gather_order != 1) return fail(MBT_EINVAL, "gather_order must be 0 or 1");
+  if (wk.n_res < 0 || (wk.n_res > 0 && !wk.res)) return fail(MBT_EINVAL, "resonator list");
+  if (wk.n_table < 0 || (wk.n_table > 0 && !wk.sr_table)) return fail(MBT_EINVAL, "sr_table");
+  if (p->rad.enable && (!(p->rad.damping_turns > 0) || !(p->rad.sigma_delta >= 0)))
+    return fail(MBT_EINVAL, "radiation: need damping_turns > 0, sigma_delta >= 0");
+  if (p->log_capacity_turns < 0) return fail(MBT_EINVAL, "log_capacity_turns < 0");
+  if ((p->d_tau == nullptr) != (p->d_delta == nullptr)) return fail(MBT_EINVAL, "give both d_tau and d_delta or neither");
+  if (p->d_tau && (((uintptr_t)p->d_tau | (uintptr_t)p->d_delta) & 15u)) return fail(MBT_EINVAL, "d_tau / d_delta must be 16-byte aligned");
+  for (int c = 1; c < p->n_cav; ++c)
+    if (std::isnan(p->cav[c].phase_rad)) return fail(MBT_EINVAL, "only cav[0] may leave its phase open");
+  int n_lr = 0;
+  for (int r = 0; r < wk.n_res; ++r) {
+    if (!(wk.res[r].Q > 0.5) || !(wk.res[r].fr_Hz > 0) || !std::isfinite(wk.res[r].Rs_ohm))
+      return fail(MBT_EINVAL, "resonator: need Q > 1/2, fr > 0");
+    if (wk.res[r].flags & MBT_RES_LR) ++n_lr;
+  }
+  if (n_lr > MBT_MAX_LR) return fail(MBT_EINVAL, "too many long-range resonators");
+  if (n_lr > 0 && wk.history_turns < 0) return fail(MBT_EINVAL, "history_turns < 0");
+
+  int dev = p->device;
+  if (dev < 0) CU(cudaGetDevice(&dev));
+  CU(cudaSetDevice(dev));
+  cudaDeviceProp prop;
+  CU(cudaGetDeviceProperties(&prop, dev));
+
+  mbt_handle *h = new (std::nothrow) mbt_handle();
+  if (!h) return fail(MBT_ENOMEM, "out of memory");
+  h->device = dev;
+  h->stream = (cudaStream_t)p->stream;
+  if (!h->stream) {  // stream capture is not allowed on the legacy default stream: use an own (blocking) stream
+    cudaError_t e_ = cudaStreamCreate(&h->stream);
+    if (e_ != cudaSuccess) {
+      h->stream = nullptr;
+      destroy(h);
+      return fail(MBT_ECUDA, std::string("cudaStreamCreate failed: ") + cudaGetErrorString(e_));
+    }
+    h->own_stream = true;
+  }
+  const int M = h->M = fl.n_bunches;
+  const int nb = h->nb = wk.n_bins;
+  const int R = h->R = n_lr;
+  const int K = h->K = n_lr ? wk.history_turns : 0;
+  h->Np = fl.n_per_bunch;
+  h->ld = mbt_particle_stride(h->Np);
+  h->log_cap = p->log_capacity_turns;
+
+#define CUH(call)                                                                                  \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) {                                                                       \
+      char buf_[512];                                                                              \
+      snprintf(buf_, sizeof buf_, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+      cudaGetLastError();                                                                          \
+      destroy(h);                                                                                  \
+      return fail(e_ == cudaErrorMemoryAllocation ? MBT_ENOMEM : MBT_ECUDA, buf_);                 \
+    }                                                                                              \
+  } while (0)
+
+  // ---- derived constants (fp64, once)
+  Args &A = h->args;
+  memset(&A, 0, sizeof A);
+  const double E0 = rg.E0_eV;
+  const double omega_rf = 2.0 * PI_D * (double)rg.h / rg.T0_s;
+  std::vector<mbt_cavity> cav(p->cav, p->cav + p->n_cav);
+  if (std::isnan(cav[0].phase_rad)) {
+    // synchronous phase (D3): V_0 sin(phi_s) = U0 - sum_{c>0} V_c sin(phi_c), alpha_c cos(phi_s) < 0
+    double u_eff = rg.U0_eV;
+    for (int c = 1; c < p->n_cav; ++c) u_eff -= cav[c].V_volt * std::sin(cav[c].phase_rad);
+    const double s = u_eff / cav[0].V_volt;
+    if (!(std::fabs(s) <= 1.0)) {
+      destroy(h);
+      return fail(MBT_EINVAL, "U0 exceeds the RF voltage: no synchronous phase");
+    }
+    cav[0].phase_rad = (rg.alpha_c > 0.0) ? PI_D - std::asin(s) : std::asin(s);
+  }
+  h->phi_s = cav[0].phase_rad;
+  A.n_cav = p->n_cav;
+  for (int c = 0; c < p->n_cav; ++c) {
+    A.cav_amp[c] = cav[c].V_volt / E0;
+    A.cav_w[c] = (double)cav[c].m * omega_rf;
+    A.cav_ph[c] = cav[c].phase_rad;
+  }
+  A.loss = rg.U0_eV / E0;
+  A.rad = p->rad.enable ? 1 : 0;
+  const double D_E = p->rad.enable ? 2.0 / p->rad.damping_turns : 0.0;  // D6
+  A.one_minus_DE = 1.0 - D_E;
+  A.A_q = p->rad.enable ? p->rad.sigma_delta * std::sqrt(2.0 * D_E) : 0.0;
+  A.keys = philox_expand_key((uint32_t)(p->seed & 0xFFFFFFFFull), (uint32_t)(p->seed >> 32));
+  A.drift = rg.alpha_c * rg.T0_s;
+  A.nb = nb;
+  A.gather = wk.gather_order;
+  A.tau_lo = wk.tau_lo_s;
+  A.invDelta = (double)nb / (wk.tau_hi_s - wk.tau_lo_s);
+  A.nb_d = (double)nb;
+  A.invE0 = 1.0 / E0;
+  A.ld = h->ld;
+  A.Np = (uint32_t)h->Np;
+  A.ppb = (uint32_t)(h->ld / 2);
+  A.M = M;
+  A.total_pairs = (int64_t)M * (h->ld / 2);
+  A.R = R;
+
+  // ---- tables (extended precision on the host, rounded once to fp64)
+  const double Delta = (wk.tau_hi_s - wk.tau_lo_s) / (double)nb;
+  std::vector<double> centre(nb);
+  for (int j = 0; j < nb; ++j) centre[j] = wk.tau_lo_s + ((double)j + 0.5) * Delta;
+  std::vector<double> w(nb, 0.0);
+  bool have_sr = false;
+  std::vector<Res> lr;
+  std::vector<cplx> Cr;
+  for (int r = 0; r < wk.n_res; ++r) {
+    const Res rr = make_res(wk.res[r]);
+    if (wk.res[r].flags & MBT_RES_SR) {
+      have_sr = true;
+      for (int k = 0; k < nb; ++k) w[k] += res_wake(rr, (ldbl)((double)k * Delta));
+    }
+    if (wk.res[r].flags & MBT_RES_LR) {
+      lr.push_back(rr);
+      // C_r = 2 alpha Rs (1 + i alpha / wbar):  W(t > 0) = Re[C_r exp(lambda_r t)]
+      const ldbl two_a_rs = 2.0L * rr.alpha * (ldbl)rr.Rs;
+      Cr.push_back(cplx{(double)two_a_rs, (double)(two_a_rs * rr.alpha / rr.wbar)});
+    }
+  }
+  if (wk.n_table > 0) {
+    have_sr = true;
+    for (int k = 0; k < nb && k < wk.n_table; ++k) w[k] += wk.sr_table[k];
+  }
+  std::vector<cplx> Esrc((size_t)R * nb), F((size_t)R * nb), g_step((size_t)M * (R ? R : 1)), g_tail((size_t)M * (R ? R : 1)),
+      g_hist((size_t)(K ? K : 1) * (R ? R : 1));
+  const ldbl T0 = (ldbl)rg.T0_s, Trf = T0 / (ldbl)rg.h;
+  for (int r = 0; r < R; ++r) {
+    for (int k = 0; k < nb; ++k) {
+      // exp(-lambda c_k) and C_r exp(lambda c_k): |c_k| < T_rf / 2, a few radians of phase
+      const ldbl c = (ldbl)centre[k];
+      const ldbl mg = expl(lr[r].alpha * c), ph = -lr[r].wbar * c;
+      Esrc[(size_t)r * nb + k] = cplx{(double)(mg * cosl(ph)), (double)(mg * sinl(ph))};
+      const ldbl mg2 = expl(-lr[r].alpha * c), ph2 = lr[r].wbar * c;
+      const ldbl ere = mg2 * cosl(ph2), eim = mg2 * sinl(ph2);
+      F[(size_t)r * nb + k] = cplx{(double)((ldbl)Cr[r].re * ere - (ldbl)Cr[r].im * eim),
+                                   (double)((ldbl)Cr[r].re * eim + (ldbl)Cr[r].im * ere)};
+    }
+    const int span = fl.bucket[M - 1] - fl.bucket[0];
+    for (int j = 0; j < M; ++j) {
+      if (j + 1 < M) g_step[(size_t)j * R + r] = exp_lambda(lr[r], (ldbl)(fl.bucket[j + 1] - fl.bucket[j]) * Trf);
+      g_tail[(size_t)j * R + r] = exp_lambda(lr[r], (ldbl)(fl.bucket[M - 1] - fl.bucket[j]) * Trf);
+    }
+    for (int k = 1; k <= K; ++k) g_hist[(size_t)(k - 1) * R + r] = exp_lambda(lr[r], (ldbl)k * T0 - (ldbl)span * Trf);
+  }
+  std::vector<double> qm(M);
+  for (int b = 0; b < M; ++b) qm[b] = fl.charge_C[b] / (double)h->Np;
+
+  // ---- device memory
+  const size_t N = (size_t)M * (size_t)h->ld;
+  if (p->d_tau) {
+    h->d_tau = (double *)p->d_tau;
+    h->d_delta = (double *)p->d_delta;
+  } else {
+    h->own_particles = true;
+    CUH(cudaMalloc((void **)&h->d_tau, N * sizeof(double)));
+    CUH(cudaMalloc((void **)&h->d_delta, N * sizeof(double)));
+  }
+  CUH(h->qm.upload(qm));
+  if (have_sr) CUH(h->w.upload(w));
+  CUH(h->Esrc.upload(Esrc));
+  CUH(h->F.upload(F));
+  CUH(h->g_step.upload(g_step));
+  CUH(h->g_tail.upload(g_tail));
+  CUH(h->g_hist.upload(g_hist));
+  CUH(h->Vsr.alloc((size_t)M * nb));
+  CUH(h->a_cur.alloc((size_t)M * (R ? R : 1)));
+  CUH(h->ring_a.alloc((size_t)(K + 1) * M * (R ? R : 1)));
+  CUH(h->ring_A.alloc((size_t)(K + 1) * (R ? R : 1)));
+  CUH(h->P.alloc((size_t)M * (R ? R : 1)));
+  CUH(h->hist.alloc((size_t)M * nb));
+  CUH(h->hist_last.alloc((size_t)M * nb));
+  CUH(h->mom_acc.alloc((size_t)M * 4));
+  CUH(h->nout_acc.alloc((size_t)M));
+  CUH(h->mom_last.alloc((size_t)M * 6));
+  if (h->log_cap > 0) CUH(h->mom_log.alloc((size_t)h->log_cap * M * 6));
+  CUH(h->ctrl.alloc(1));
+
+  A.tau = h->d_tau;
+  A.delta = h->d_delta;
+  A.Vsr = h->Vsr.p;
+  A.P = h->P.p;
+  A.F = h->F.p;
+  A.hist = h->hist.p;
+  A.mom_acc = h->mom_acc.p;
+  A.nout_acc = h->nout_acc.p;
+  A.ctrl = h->ctrl.p;
+
+  WakeArgs &Wa = h->wargs;
+  memset(&Wa, 0, sizeof Wa);
+  Wa.M = M; Wa.nb = nb; Wa.R = R; Wa.K = K; Wa.Np = (uint32_t)h->Np; Wa.mode = 0;
+  Wa.qm = h->qm.p;
+  Wa.w = have_sr ? h->w.p : nullptr;
+  Wa.Esrc = h->Esrc.p; Wa.g_step = h->g_step.p; Wa.g_tail = h->g_tail.p; Wa.g_hist = h->g_hist.p;
+  Wa.hist = h->hist.p; Wa.hist_last = h->hist_last.p; Wa.Vsr = h->Vsr.p;
+  Wa.a_cur = h->a_cur.p; Wa.ring_a = h->ring_a.p; Wa.ring_A = h->ring_A.p; Wa.P = h->P.p;
+  Wa.mom_acc = h->mom_acc.p; Wa.nout_acc = h->nout_acc.p; Wa.mom_last = h->mom_last.p;
+  Wa.mom_log = h->log_cap > 0 ? h->mom_log.p : nullptr;
+  Wa.log_cap = h->log_cap;
+  Wa.ctrl = h->ctrl.p;
+
+  // ---- launch shapes: one resident wave of CTAs, each owning a contiguous run of pairs
+  h->smem_pass = (size_t)nb * (sizeof(double) + sizeof(uint32_t));
+  h->smem_wake = (size_t)nb * 2 * sizeof(double);
+  CUH(cudaFuncSetAttribute(k_pass<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
+  CUH(cudaFuncSetAttribute(k_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
+  CUH(cudaFuncSetAttribute(k_wake, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_wake));
+  int occ = 0;
+  CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pass<true>, kPassThreads, h->smem_pass));
+  if (occ < 1) occ = 1;
+  const int64_t max_cta = (int64_t)prop.multiProcessorCount * occ;
+  const int64_t need = (A.total_pairs + kPassThreads - 1) / kPassThreads;
+  h->grid_pass = (int)(need < max_cta ? need : max_cta);
+
+  // ---- initial distribution (D20) on the device
+  {
+    dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)M);
+    k_init<<<grid, 256, 0, h->stream>>>(h->d_tau, h->d_delta, h->ld, (uint32_t)h->Np, M, A.keys, fl.sigma_tau0_s,
+                                         fl.sigma_delta0);
+    h->launches += 1;
+    CUH(cudaGetLastError());
+  }
+  CUH(cudaEventCreate(&h->ev0));
+  CUH(cudaEventCreate(&h->ev1));
+  CUH(cudaStreamSynchronize(h->stream));
+#undef CUH
+  h->dirty = true;
+  *out = h;
+  return 0;
+}
+
+int mbt_track(mbt_handle *h, int64_t n_turns) {
+  if (!h || n_turns < 0) return fail(MBT_EINVAL, "bad argument");
+  if (h->turn + n_turns > 0xFFFFFFFFll) return fail(MBT_EINVAL, "turn counter would exceed 2^32");
+  CU(cudaSetDevice(h->device));
+  if (n_turns == 0) return 0;
+  if (!h->graph1) {
+    int rc = build_graph(h, 1, &h->graph1);
+    if (rc) return rc;
+  }
+  if (n_turns >= h->unroll && !h->graphU) {
+    int rc = build_graph(h, h->unroll, &h->graphU);
+    if (rc) return rc;
+  }
+  CU(cudaEventRecord(h->ev0, h->stream));
+  int64_t left = n_turns;
+  while (left >= h->unroll) {
+    CU(cudaGraphLaunch(h->graphU, h->stream));
+    left -= h->unroll;
+  }
+  while (left > 0) {
+    CU(cudaGraphLaunch(h->graph1, h->stream));
+    left -= 1;
+  }
+  CU(cudaEventRecord(h->ev1, h->stream));
+  h->timed = true;
+  h->launches += 2 * n_turns;
+  h->turn += n_turns;
+  h->dirty = true;
+  h->wake_valid = true;
+  return 0;
+}
+
+int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, double *wake_seconds) {
+  if (!h || n_turns < 1 || n_turns > 65536 || !pass_seconds || !wake_seconds) return fail(MBT_EINVAL, "bad argument");
+  if (h->turn + n_turns > 0xFFFFFFFFll) return fail(MBT_EINVAL, "turn counter would exceed 2^32");
+  CU(cudaSetDevice(h->device));
+  std::vector<cudaEvent_t> ev((size_t)n_turns * 3, nullptr);
+  for (auto &e : ev) CU(cudaEventCreate(&e));
+  CU(cudaEventRecord(h->ev0, h->stream));
+  for (int64_t t = 0; t < n_turns; ++t) {
+    CU(cudaEventRecord(ev[3 * t], h->stream));
+    k_pass<true><<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
+    CU(cudaEventRecord(ev[3 * t + 1], h->stream));
+    k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
+    CU(cudaEventRecord(ev[3 * t + 2], h->stream));
+  }
+  CU(cudaEventRecord(h->ev1, h->stream));
+  h->timed = true;
+  h->launches += 2 * n_turns;
+  h->turn += n_turns;
+  h->dirty = true;
+  h->wake_valid = true;
+  CU(cudaStreamSynchronize(h->stream));
+  double ps = 0.0, ws = 0.0;
+  for (int64_t t = 0; t < n_turns; ++t) {
+    float a = 0.f, b = 0.f;
+    CU(cudaEventElapsedTime(&a, ev[3 * t], ev[3 * t + 1]));
+    CU(cudaEventElapsedTime(&b, ev[3 * t + 1], ev[3 * t + 2]));
+    ps += (double)a * 1e-3;
+    ws += (double)b * 1e-3;
+  }
+  for (auto &e : ev) cudaEventDestroy(e);
+  *pass_seconds = ps;
+  *wake_seconds = ws;
+  return 0;
+}
+
+double mbt_last_track_seconds(mbt_handle *h) {
+  if (!h || !h->timed) { fail(MBT_ESTATE, "no tracked call to time"); return -1.0; }
+  if (cudaEventSynchronize(h->ev1) != cudaSuccess) { fail(MBT_ECUDA, "event synchronize failed"); return -1.0; }
+  float ms = 0.f;
+  if (cudaEventElapsedTime(&ms, h->ev0, h->ev1) != cudaSuccess) { fail(MBT_ECUDA, "event elapsed failed"); return -1.0; }
+  return (double)ms * 1e-3;
+}
+
+int mbt_moments(mbt_handle *h, double *out) {
+  if (!h || !out) return fail(MBT_EINVAL, "null argument");
+  int rc = flush(h);
+  if (rc) return rc;
+  CU(cudaMemcpyAsync(out, h->mom_last.p, sizeof(double) * h->M * 6, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_destroy(mbt_handle *h) {
+  destroy(h);
+  return 0;
+}
+
+int mbt_device_pointers(mbt_handle *h, void **d_tau, void **d_delta, int64_t *ld) {
+  if (!h) return fail(MBT_EINVAL, "null argument");
+  int rc = flush(h);
+  if (rc) return rc;
+  if (d_tau) *d_tau = h->d_tau;
+  if (d_delta) *d_delta = h->d_delta;
+  if (ld) *ld = h->ld;
+  return 0;
+}
+
+int mbt_get_particles(mbt_handle *h, double *tau, double *delta) {
+  if (!h || !tau || !delta) return fail(MBT_EINVAL, "null argument");
+  int rc = flush(h);
+  if (rc) return rc;
+  const size_t n = (size_t)h->M * h->Np;
+  if (h->ld == h->Np) {
+    CU(cudaMemcpyAsync(tau, h->d_tau, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaMemcpyAsync(delta, h->d_delta, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  } else {
+    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n)); }
+    dim3 grid((unsigned)((h->Np + 255) / 256 < 1024 ? (h->Np + 255) / 256 : 1024), (unsigned)h->M);
+    k_pack<<<grid, 256, 0, h->stream>>>(h->d_tau, h->ld, (uint32_t)h->Np, h->scratch_a.p);
+    CU(cudaMemcpyAsync(tau, h->scratch_a.p, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    k_pack<<<grid, 256, 0, h->stream>>>(h->d_delta, h->ld, (uint32_t)h->Np, h->scratch_a.p);
+    CU(cudaMemcpyAsync(delta, h->scratch_a.p, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    h->launches += 2;
+  }
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int64_t turn) {
+  if (!h || !tau || !delta || turn < 0 || turn > 0xFFFFFFFFll) return fail(MBT_EINVAL, "bad argument");
+  CU(cudaSetDevice(h->device));
+  const size_t n = (size_t)h->M * h->Np;
+  if (h->ld == h->Np) {
+    CU(cudaMemcpyAsync(h->d_tau, tau, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(h->d_delta, delta, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  } else {
+    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n)); }
+    dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)h->M);
+    CU(cudaMemcpyAsync(h->scratch_a.p, tau, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    k_unpack<<<grid, 256, 0, h->stream>>>(h->scratch_a.p, h->ld, (uint32_t)h->Np, h->d_tau);
+    CU(cudaMemcpyAsync(h->scratch_a.p, delta, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    k_unpack<<<grid, 256, 0, h->stream>>>(h->scratch_a.p, h->ld, (uint32_t)h->Np, h->d_delta);
+    h->launches += 2;
+  }
+  k_set_ctrl<<<1, 1, 0, h->stream>>>(h->ctrl.p, (uint32_t)turn, 0u);
+  h->launches += 1;
+  CU(cudaMemsetAsync(h->hist.p, 0, sizeof(uint32_t) * h->M * h->nb, h->stream));
+  CU(cudaMemsetAsync(h->mom_acc.p, 0, sizeof(double) * h->M * 4, h->stream));
+  CU(cudaMemsetAsync(h->nout_acc.p, 0, sizeof(unsigned long long) * h->M, h->stream));
+  CU(cudaMemsetAsync(h->ring_a.p, 0, sizeof(cplx) * (h->ring_a.n ? h->ring_a.n : 1), h->stream));
+  CU(cudaMemsetAsync(h->ring_A.p, 0, sizeof(cplx) * (h->ring_A.n ? h->ring_A.n : 1), h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  h->turn = turn;
+  h->dirty = true;
+  h->wake_valid = false;
+  return 0;
+}
+
+int mbt_get_histogram(mbt_handle *h, uint32_t *out) {
+  if (!h || !out) return fail(MBT_EINVAL, "null argument");
+  int rc = flush(h);
+  if (rc) return rc;
+  CU(cudaMemcpyAsync(out, h->hist_last.p, sizeof(uint32_t) * h->M * h->nb, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_get_wake(mbt_handle *h, double *total, double *sr, double *lr) {
+  if (!h) return fail(MBT_EINVAL, "null argument");
+  CU(cudaSetDevice(h->device));
+  const size_t n = (size_t)h->M * h->nb;
+  if (!h->wake_valid) {
+    if (total) memset(total, 0, n * sizeof(double));
+    if (sr) memset(sr, 0, n * sizeof(double));
+    if (lr) memset(lr, 0, n * sizeof(double));
+    return 0;
+  }
+  if (h->scratch_b.n < 3 * n) { h->scratch_b.release(); CU(h->scratch_b.alloc(3 * n)); }
+  double *dt = h->scratch_b.p, *ds = dt + n, *dl = ds + n;
+  k_eval_wake<<<h->M, 256, 0, h->stream>>>(h->M, h->nb, h->R, h->Vsr.p, h->P.p, h->F.p, dt, ds, dl);
+  h->launches += 1;
+  if (total) CU(cudaMemcpyAsync(total, dt, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  if (sr) CU(cudaMemcpyAsync(sr, ds, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  if (lr) CU(cudaMemcpyAsync(lr, dl, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_get_moment_log(mbt_handle *h, int64_t first_turn, int64_t n, double *out) {
+  if (!h || !out || first_turn < 1 || n < 0) return fail(MBT_EINVAL, "bad argument");
+  if (first_turn - 1 + n > h->log_cap || first_turn - 1 + n > h->turn) return fail(MBT_ESTATE, "turns not in the log");
+  int rc = flush(h);  // closes the moments of the last tracked turn
+  if (rc) return rc;
+  if (n == 0) return 0;
+  CU(cudaMemcpyAsync(out, h->mom_log.p + (size_t)(first_turn - 1) * h->M * 6, sizeof(double) * (size_t)n * h->M * 6,
+                     cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_get_lr_history(mbt_handle *h, double *out) {
+  if (!h || !out) return fail(MBT_EINVAL, "null argument");
+  CU(cudaSetDevice(h->device));
+  const int M = h->M, R = h->R, K = h->K;
+  if (R == 0 || K == 0) return 0;
+  std::vector<cplx> ring((size_t)(K + 1) * M * R);
+  CU(cudaMemcpyAsync(ring.data(), h->ring_a.p, ring.size() * sizeof(cplx), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  for (int k = 0; k < K; ++k) {
+    const int64_t t = h->turn - K + 1 + k;
+    for (int b = 0; b < M; ++b)
+      for (int r = 0; r < R; ++r) {
+        cplx a{0.0, 0.0};
+        if (t >= 1) a = ring[((size_t)(t % (K + 1)) * M + b) * R + r];
+        double *o = &out[(((size_t)k * M + b) * R + r) * 2];
+        o[0] = a.re;
+        o[1] = a.im;
+      }
+  }
+  return 0;
+}
+
+int mbt_set_lr_history(mbt_handle *h, const double *in) {
+  if (!h || !in) return fail(MBT_EINVAL, "null argument");
+  CU(cudaSetDevice(h->device));
+  const int M = h->M, R = h->R, K = h->K;
+  if (R == 0 || K == 0) return 0;
+  std::vector<cplx> ring((size_t)(K + 1) * M * R, cplx{0.0, 0.0});
+  for (int k = 0; k < K; ++k) {
+    const int64_t t = h->turn - K + 1 + k;
+    if (t < 1) continue;
+    for (int b = 0; b < M; ++b)
+      for (int r = 0; r < R; ++r) {
+        const double *i2 = &in[(((size_t)k * M + b) * R + r) * 2];
+        ring[((size_t)(t % (K + 1)) * M + b) * R + r] = cplx{i2[0], i2[1]};
+      }
+  }
+  CU(cudaMemcpyAsync(h->ring_a.p, ring.data(), ring.size() * sizeof(cplx), cudaMemcpyHostToDevice, h->stream));
+  k_aggregate_history<<<K + 1, 32, 0, h->stream>>>(M, R, K, h->ring_a.p, h->g_tail.p, h->ring_A.p);
+  h->launches += 1;
+  CU(cudaGetLastError());
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  if (!ctr || !key || !out) return fail(MBT_EINVAL, "null argument");
+  uint32_t *d = nullptr;
+  CU(cudaMalloc((void **)&d, 4 * sizeof(uint32_t)));
+  k_philox_selftest<<<1, 1>>>(ctr[0], ctr[1], ctr[2], ctr[3], philox_expand_key(key[0], key[1]), d);
+  cudaError_t e = cudaMemcpy(out, d, 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  CU(e);
+  return 0;
+}
+
+int mbt_normal_selftest(uint64_t seed, int64_t n, const uint32_t *ctr, double *out) {
+  if (n < 0 || (n > 0 && (!ctr || !out))) return fail(MBT_EINVAL, "bad argument");
+  if (n == 0) return 0;
+  uint32_t *dc = nullptr;
+  double *dz = nullptr;
+  CU(cudaMalloc((void **)&dc, (size_t)n * 4 * sizeof(uint32_t)));
+  cudaError_t e = cudaMalloc((void **)&dz, (size_t)n * 2 * sizeof(double));
+  if (e != cudaSuccess) { cudaFree(dc); CU(e); }
+  e = cudaMemcpy(dc, ctr, (size_t)n * 4 * sizeof(uint32_t), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    k_normal_selftest<<<148, 256>>>(n, dc, philox_expand_key((uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32)), dz);
+    e = cudaMemcpy(out, dz, (size_t)n * 2 * sizeof(double), cudaMemcpyDeviceToHost);
+  }
+  cudaFree(dc);
+  cudaFree(dz);
+  CU(e);
+  return 0;
+}
+
+}  // extern "C"

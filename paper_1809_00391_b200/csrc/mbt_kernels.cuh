@@ -1,0 +1,513 @@
+// mbt_kernels.cuh -- CUDA kernels (sm_100a) of the longitudinal multi-bunch tracker.
+//
+// One turn = two launches:
+//   k_pass  the fused particle pass (S0 kick of the previous turn, S7 moments, S1 RF, S2 radiation,
+//           S3 drift, S4 binning), one read and one write of the SoA fp64 particle store;
+//   k_wake  per bunch: counts -> charges, S5 Toeplitz short-range convolution, S6 source phasors; the
+//           last CTA to finish runs the S6 in-turn phasor scan over the fill pattern and the history ring.
+// The long-range part of the wake is kept as ONE complex number per (bunch, resonator) and expanded onto the
+// bins when a CTA of the next pass stages the bunch's wake grid in shared memory.
+//
+// Step numbers and citations: include/mbt.h.  DESIGN.md has the data layout and the roofline of each kernel.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "mbt_math.cuh"
+
+namespace mbt {
+
+constexpr int kPassThreads = 256;
+constexpr int kWakeThreads = 256;
+constexpr int kMaxCav = 8;
+constexpr int kMaxLR = 8;
+
+struct cplx {
+  double re, im;
+};
+__host__ __device__ __forceinline__ cplx cmul(cplx a, cplx b) {
+  return cplx{fma(a.re, b.re, -(a.im * b.im)), fma(a.re, b.im, a.im * b.re)};
+}
+__host__ __device__ __forceinline__ cplx cadd(cplx a, cplx b) { return cplx{a.re + b.re, a.im + b.im}; }
+// a*b + c
+__host__ __device__ __forceinline__ cplx cfma(cplx a, cplx b, cplx c) {
+  return cplx{fma(a.re, b.re, fma(-a.im, b.im, c.re)), fma(a.re, b.im, fma(a.im, b.re, c.im))};
+}
+
+// device-resident control words (so that a captured CUDA graph replays without parameter updates)
+struct Ctrl {
+  uint32_t turn;          // completed turns
+  uint32_t ticket;        // CTAs of k_wake that have finished (last-CTA-done election)
+  uint32_t kick_pending;  // 1: the wake of turn `turn` has not been applied to delta yet
+  uint32_t pad;
+};
+
+struct Args {
+  // particle store: tau[M][ld], delta[M][ld], ld even; pair p of bunch b = particles (2p, 2p+1)
+  double *tau, *delta;
+  int64_t ld;
+  uint32_t Np;       // particles per bunch
+  uint32_t ppb;      // pairs per bunch = ld / 2
+  int32_t M;
+  int64_t total_pairs;
+  // S1
+  int32_t n_cav;
+  double cav_amp[kMaxCav];  // V_c / E0
+  double cav_w[kMaxCav];    // m_c * omega_rf
+  double cav_ph[kMaxCav];
+  double loss;              // U0 / E0
+  // S2
+  int32_t rad;
+  double one_minus_DE, A_q;
+  PhiloxKeys keys;
+  // S3
+  double drift;  // alpha_c * T0
+  // S4 / S0
+  int32_t nb;
+  int32_t gather;
+  double tau_lo, invDelta, nb_d, invE0;
+  // wake state
+  const double *Vsr;    // [M][nb]   short-range wake of the last turn [V]
+  const cplx *P;        // [M][R]    long-range phasor seen by bunch b
+  const cplx *F;        // [R][nb]   C_r exp(lambda_r c_j)
+  int32_t R;            // long-range resonators
+  uint32_t *hist;       // [M][nb]   accumulating counts of the pass in flight
+  double *mom_acc;      // [M][4]    sum tau, sum delta, sum tau^2, sum delta^2
+  unsigned long long *nout_acc;  // [M]
+  Ctrl *ctrl;
+};
+
+// ------------------------------------------------------------------ fused particle pass
+// MAP = true : S0 S7 | S1 S2 S3 | S4      (a tracked turn)
+// MAP = false: S0 S7 |          | S4      (flush of the pending kick before the state is observed)
+template <bool MAP>
+struct Particle {
+  static __device__ __forceinline__ void step(const Args &A, const double *sV, uint32_t *sH, double &tau, double &delta,
+                                              double z, double &st, double &sd, double &stt, double &sdd,
+                                              uint32_t &nout) {
+    // S0: kick of the previous turn's wake.  t exactly as the binning computed it (one subtraction, one
+    // multiplication, no contraction), so the in-window decision is the one that deposited the particle.
+    double t = __dmul_rn(__dsub_rn(tau, A.tau_lo), A.invDelta);
+    bool in = (t >= 0.0) && (t < A.nb_d);
+    if (in) {
+      double v;
+      if (A.gather == 0) {
+        v = sV[__double2int_rd(t)];
+      } else {
+        // linear between bin centres, constant in the outer half bins (D12)
+        double u = fmin(fmax(t - 0.5, 0.0), A.nb_d - 1.0);
+        int j0 = min(__double2int_rd(u), A.nb - 2);
+        double f = u - (double)j0;
+        double v0 = sV[j0], v1 = sV[j0 + 1];
+        v = fma(f, v1 - v0, v0);
+      }
+      delta = fma(-v, A.invE0, delta);
+    } else {
+      nout += 1u;
+    }
+    // S7: moments of the state after the kick
+    st += tau;
+    sd += delta;
+    stt = fma(tau, tau, stt);
+    sdd = fma(delta, delta, sdd);
+    if (MAP) {
+      // S1: RF cavities, then the synchronous loss
+#pragma unroll 1
+      for (int c = 0; c < A.n_cav; ++c) delta = fma(A.cav_amp[c], sin_rf(fma(A.cav_w[c], tau, A.cav_ph[c])), delta);
+      delta -= A.loss;
+      // S2
+      if (A.rad) delta = fma(delta, A.one_minus_DE, A.A_q * z);
+      // S3
+      tau = fma(A.drift, delta, tau);
+      // S4
+      t = __dmul_rn(__dsub_rn(tau, A.tau_lo), A.invDelta);
+      in = (t >= 0.0) && (t < A.nb_d);
+    }
+    if (in) atomicAdd(&sH[__double2int_rd(t)], 1u);
+  }
+};
+
+template <bool MAP>
+__global__ void __launch_bounds__(kPassThreads, 3) k_pass(const __grid_constant__ Args A) {
+  extern __shared__ double smem_d[];
+  double *sV = smem_d;                                  // [nb]
+  uint32_t *sH = reinterpret_cast<uint32_t *>(sV + A.nb);  // [nb]
+  __shared__ double s_red[kPassThreads / 32][4];
+  __shared__ uint32_t s_nout[kPassThreads / 32];
+
+  const int tid = threadIdx.x;
+  const uint32_t n = A.ctrl->turn + 1u;  // the turn this pass tracks (Philox counter word, D24)
+  const bool have_kick = A.ctrl->kick_pending != 0u;
+
+  // contiguous range of pairs for this CTA, in multiples of the CTA width
+  int64_t per = (A.total_pairs + gridDim.x - 1) / gridDim.x;
+  per = (per + kPassThreads - 1) / kPassThreads * kPassThreads;
+  int64_t begin = (int64_t)blockIdx.x * per;
+  int64_t end = begin + per < A.total_pairs ? begin + per : A.total_pairs;
+
+  while (begin < end) {
+    const int b = (int)(begin / A.ppb);
+    const uint32_t p0 = (uint32_t)(begin - (int64_t)b * A.ppb);
+    const int64_t left = end - begin;
+    const uint32_t p1 = (left < (int64_t)(A.ppb - p0)) ? (uint32_t)(p0 + left) : A.ppb;
+
+    // stage the wake grid of bunch b: V = V_SR + sum_r Re[F_r[j] P[b][r]]   (S6 expansion), clear the counts
+    for (int j = tid; j < A.nb; j += kPassThreads) {
+      double v = 0.0;
+      if (have_kick) {
+        v = A.Vsr[(size_t)b * A.nb + j];
+        for (int r = 0; r < A.R; ++r) {
+          const cplx f = A.F[(size_t)r * A.nb + j];
+          const cplx pb = A.P[(size_t)b * A.R + r];
+          v += fma(f.re, pb.re, -(f.im * pb.im));
+        }
+      }
+      sV[j] = v;
+      sH[j] = 0u;
+    }
+    __syncthreads();
+
+    double st = 0.0, sd = 0.0, stt = 0.0, sdd = 0.0;
+    uint32_t nout = 0u;
+    double2 *T = reinterpret_cast<double2 *>(A.tau + (size_t)b * A.ld);
+    double2 *D = reinterpret_cast<double2 *>(A.delta + (size_t)b * A.ld);
+
+    uint32_t p = p0 + tid;
+    double2 t2, d2;
+    if (p < p1) { t2 = T[p]; d2 = D[p]; }
+    while (p < p1) {
+      const uint32_t pn = p + kPassThreads;
+      double2 t2n, d2n;
+      if (pn < p1) { t2n = T[pn]; d2n = D[pn]; }  // prefetch the next pair while this one is computed
+
+      double z0 = 0.0, z1 = 0.0;
+      if (MAP && A.rad) {
+        // one Philox call and one Box-Muller serve both particles of the 128-bit load (D8):
+        // counter (pair, bunch, turn, tag 0); even particle takes z_c, odd particle z_s
+        uint32_t x0, x1, x2, x3;
+        philox4x32_10(p, (uint32_t)b, n, 0u, A.keys, x0, x1, x2, x3);
+        box_muller_fast(uniform52(x0, x1), uniform52(x2, x3), z0, z1);
+      }
+      Particle<MAP>::step(A, sV, sH, t2.x, d2.x, z0, st, sd, stt, sdd, nout);
+      if (2u * p + 1u < A.Np) {  // the odd slot of the last pair is padding when N_p is odd
+        Particle<MAP>::step(A, sV, sH, t2.y, d2.y, z1, st, sd, stt, sdd, nout);
+      }
+      if (MAP) T[p] = t2;
+      D[p] = d2;
+      t2 = t2n; d2 = d2n; p = pn;
+    }
+
+    // S7: warp shuffles, then one atomic per CTA and bunch
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      st += __shfl_down_sync(0xffffffffu, st, o);
+      sd += __shfl_down_sync(0xffffffffu, sd, o);
+      stt += __shfl_down_sync(0xffffffffu, stt, o);
+      sdd += __shfl_down_sync(0xffffffffu, sdd, o);
+      nout += __shfl_down_sync(0xffffffffu, nout, o);
+    }
+    if ((tid & 31) == 0) {
+      s_red[tid >> 5][0] = st; s_red[tid >> 5][1] = sd; s_red[tid >> 5][2] = stt; s_red[tid >> 5][3] = sdd;
+      s_nout[tid >> 5] = nout;
+    }
+    __syncthreads();  // also: all shared-memory counts of this segment are in
+    if (tid < 4) {
+      double s = 0.0;
+#pragma unroll
+      for (int w = 0; w < kPassThreads / 32; ++w) s += s_red[w][tid];
+      atomicAdd(&A.mom_acc[(size_t)b * 4 + tid], s);
+    } else if (tid == 4) {
+      uint32_t s = 0u;
+#pragma unroll
+      for (int w = 0; w < kPassThreads / 32; ++w) s += s_nout[w];
+      if (s) atomicAdd(&A.nout_acc[b], (unsigned long long)s);
+    }
+    // S4: flush the CTA's counts into the bunch histogram (integer, order-independent)
+    for (int j = tid; j < A.nb; j += kPassThreads) {
+      const uint32_t c = sH[j];
+      if (c) atomicAdd(&A.hist[(size_t)b * A.nb + j], c);
+    }
+    __syncthreads();
+    begin += (int64_t)(p1 - p0);
+  }
+}
+
+// ------------------------------------------------------------------ wake
+struct WakeArgs {
+  int32_t M, nb, R, K;
+  uint32_t Np;
+  int32_t mode;            // 0: full turn (S5, S6, bump the turn counter); 1: finalise counts and moments only
+  const double *qm;        // [M]      macro-particle charge Q_b / N_p
+  const double *w;         // [nb]     short-range table w_k = W(k Delta); nullptr: none
+  const cplx *Esrc;        // [R][nb]  exp(-lambda_r c_k)
+  const cplx *g_step;      // [M][R]   exp(lambda_r (s_{j+1}-s_j) T_rf), j < M-1
+  const cplx *g_tail;      // [M][R]   exp(lambda_r (s_{M-1}-s_j) T_rf)
+  const cplx *g_hist;      // [K][R]   exp(lambda_r (k T0 - (s_{M-1}-s_0) T_rf)), k = 1..K
+  uint32_t *hist;          // [M][nb]  in: counts of this turn; out: zero
+  uint32_t *hist_last;     // [M][nb]  out: counts of this turn
+  double *Vsr;             // [M][nb]
+  cplx *a_cur;             // [M][R]   source phasors of this turn
+  cplx *ring_a;            // [K+1][M][R] slot n % (K+1)
+  cplx *ring_A;            // [K+1][R]    per-turn aggregates, slot n % (K+1)
+  cplx *P;                 // [M][R]
+  double *mom_acc;         // [M][4]  in: sums gathered by the pass; out: zero
+  unsigned long long *nout_acc;  // [M]
+  double *mom_last;        // [M][6]
+  double *mom_log;         // [cap][M][6] or nullptr
+  int64_t log_cap;
+  Ctrl *ctrl;
+};
+
+// affine map x -> g x + c over the complex numbers; (first o second)(x) = second(first(x))
+struct Affine {
+  cplx g, c;
+};
+__device__ __forceinline__ Affine compose(const Affine &first, const Affine &second) {
+  return Affine{cmul(first.g, second.g), cfma(first.c, second.g, second.c)};
+}
+
+__global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ WakeArgs A) {
+  extern __shared__ double smem_d[];
+  double *sq = smem_d;         // [nb] charge per bin
+  double *sw = smem_d + A.nb;  // [nb] wake table
+  __shared__ double s_red[kWakeThreads / 32][2];
+  __shared__ bool s_last;
+  __shared__ Affine s_scan[kWakeThreads];
+
+  const int tid = threadIdx.x;
+  const int b = blockIdx.x;
+  const int nb = A.nb;
+  const uint32_t n_done = A.ctrl->turn;  // completed turns; the turn being closed is n_done + 1
+  const uint32_t n = n_done + 1u;
+
+  // counts -> charges; keep a copy of the counts; clear the accumulator for the next pass
+  const double qm = A.qm[b];
+  for (int j = tid; j < nb; j += kWakeThreads) {
+    const uint32_t c = A.hist[(size_t)b * nb + j];
+    A.hist_last[(size_t)b * nb + j] = c;
+    A.hist[(size_t)b * nb + j] = 0u;
+    sq[j] = qm * (double)c;
+    if (A.mode == 0 && A.w) sw[j] = A.w[j];
+  }
+  // S7: close the moments the pass gathered (state after turn n_done's kick)
+  if (tid == 0) {
+    const double N = (double)A.Np;
+    const double s1 = A.mom_acc[b * 4 + 0], s2 = A.mom_acc[b * 4 + 1];
+    const double s11 = A.mom_acc[b * 4 + 2], s22 = A.mom_acc[b * 4 + 3];
+    const double no = (double)A.nout_acc[b];
+    const double mt = s1 / N, md = s2 / N;
+    const double vt = fmax(s11 / N - mt * mt, 0.0), vd = fmax(s22 / N - md * md, 0.0);
+    double m[6] = {N - no, no, mt, md, sqrt(vt), sqrt(vd)};
+#pragma unroll
+    for (int k = 0; k < 6; ++k) A.mom_last[b * 6 + k] = m[k];
+    if (A.mom_log && n_done >= 1u && (int64_t)n_done <= A.log_cap) {
+#pragma unroll
+      for (int k = 0; k < 6; ++k) A.mom_log[((size_t)(n_done - 1u) * A.M + b) * 6 + k] = m[k];
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) A.mom_acc[b * 4 + k] = 0.0;
+    A.nout_acc[b] = 0ull;
+  }
+  if (A.mode != 0) return;
+  __syncthreads();
+
+  // S5: V_SR[j] = sum_{k<=j} w[j-k] q[k].  Outputs j and nb-1-j are paired so that every thread does nb+1 terms.
+  if (A.w) {
+    for (int idx = tid; idx < (nb + 1) / 2; idx += kWakeThreads) {
+      const int j1 = idx, j2 = nb - 1 - idx;
+      double acc1 = 0.0, acc2 = 0.0;
+      for (int k = 0; k <= j1; ++k) acc1 = fma(sw[j1 - k], sq[k], acc1);
+      A.Vsr[(size_t)b * nb + j1] = acc1;
+      if (j2 != j1) {
+        for (int k = 0; k <= j2; ++k) acc2 = fma(sw[j2 - k], sq[k], acc2);
+        A.Vsr[(size_t)b * nb + j2] = acc2;
+      }
+    }
+  } else {
+    for (int j = tid; j < nb; j += kWakeThreads) A.Vsr[(size_t)b * nb + j] = 0.0;
+  }
+
+  // S6 sources: a[b][r] = sum_k q[k] exp(-lambda_r c_k)
+  for (int r = 0; r < A.R; ++r) {
+    double are = 0.0, aim = 0.0;
+    for (int k = tid; k < nb; k += kWakeThreads) {
+      const cplx e = A.Esrc[(size_t)r * nb + k];
+      are = fma(sq[k], e.re, are);
+      aim = fma(sq[k], e.im, aim);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      are += __shfl_down_sync(0xffffffffu, are, o);
+      aim += __shfl_down_sync(0xffffffffu, aim, o);
+    }
+    if ((tid & 31) == 0) { s_red[tid >> 5][0] = are; s_red[tid >> 5][1] = aim; }
+    __syncthreads();
+    if (tid == 0) {
+      cplx a{0.0, 0.0};
+      for (int w = 0; w < kWakeThreads / 32; ++w) { a.re += s_red[w][0]; a.im += s_red[w][1]; }
+      A.a_cur[(size_t)b * A.R + r] = a;
+      A.ring_a[((size_t)(n % (uint32_t)(A.K + 1)) * A.M + b) * A.R + r] = a;
+    }
+    __syncthreads();
+  }
+
+  // last-CTA-done election: the CTA that sees every other CTA's ticket closes the turn
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_last = (atomicAdd(&A.ctrl->ticket, 1u) == (uint32_t)(A.M - 1));
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+
+  // S6: P_0 = G_n (history seed), P_{j+1} = (P_j + a_j) g_j -- an inclusive scan of affine maps over the fill
+  // pattern; every factor is exp(lambda * positive time), |g| < 1.
+  const int M = A.M, R = A.R, K = A.K;
+  const int ipt = (M + kWakeThreads - 1) / kWakeThreads;  // consecutive bunches per thread
+  for (int r = 0; r < R; ++r) {
+    // G_n = sum_{k=1..min(K,n-1)} A_{n-k} exp(lambda (k T0 - span))     (direct K-term sum)
+    cplx G{0.0, 0.0};
+    for (int k = 1; k <= K && (int64_t)n - k >= 1; ++k)
+      G = cfma(A.ring_A[(size_t)((n - (uint32_t)k) % (uint32_t)(K + 1)) * R + r], A.g_hist[(size_t)(k - 1) * R + r], G);
+    // thread-local composite of its run of bunches, and this turn's own aggregate
+    const int j_lo = tid * ipt, j_hi = min(j_lo + ipt, M);
+    Affine loc{cplx{1.0, 0.0}, cplx{0.0, 0.0}};
+    cplx own{0.0, 0.0};
+    for (int j = j_lo; j < j_hi; ++j) {
+      const cplx a = A.a_cur[(size_t)j * R + r];
+      own = cfma(a, A.g_tail[(size_t)j * R + r], own);
+      if (j + 1 < M) {
+        const cplx g = A.g_step[(size_t)j * R + r];
+        loc = compose(loc, Affine{g, cmul(a, g)});
+      }
+    }
+    // Hillis-Steele inclusive scan of the thread composites
+    s_scan[tid] = loc;
+    __syncthreads();
+    for (int o = 1; o < kWakeThreads; o <<= 1) {
+      Affine v = s_scan[tid];
+      if (tid >= o) v = compose(s_scan[tid - o], v);
+      __syncthreads();
+      s_scan[tid] = v;
+      __syncthreads();
+    }
+    // exclusive prefix of this thread, applied to G, then walk the run
+    cplx Pj = G;
+    if (tid > 0) {
+      const Affine pre = s_scan[tid - 1];
+      Pj = cfma(pre.g, G, pre.c);
+    }
+    for (int j = j_lo; j < j_hi; ++j) {
+      A.P[(size_t)j * R + r] = Pj;
+      if (j + 1 < M) {
+        const cplx g = A.g_step[(size_t)j * R + r];
+        Pj = cmul(cadd(Pj, A.a_cur[(size_t)j * R + r]), g);
+      }
+    }
+    // A_n = sum_j a_j exp(lambda (s_{M-1}-s_j) T_rf): block reduction
+    double ore = own.re, oim = own.im;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      ore += __shfl_down_sync(0xffffffffu, ore, o);
+      oim += __shfl_down_sync(0xffffffffu, oim, o);
+    }
+    __syncthreads();
+    if ((tid & 31) == 0) { s_red[tid >> 5][0] = ore; s_red[tid >> 5][1] = oim; }
+    __syncthreads();
+    if (tid == 0) {
+      cplx a{0.0, 0.0};
+      for (int w = 0; w < kWakeThreads / 32; ++w) { a.re += s_red[w][0]; a.im += s_red[w][1]; }
+      A.ring_A[(size_t)(n % (uint32_t)(K + 1)) * R + r] = a;
+    }
+    __syncthreads();
+  }
+  if (tid == 0) {
+    A.ctrl->ticket = 0u;
+    A.ctrl->kick_pending = 1u;
+    A.ctrl->turn = n;
+  }
+}
+
+// ------------------------------------------------------------------ small kernels
+// wake potential on the bins for mbt_get_wake: total = sr + lr, lr[b][j] = sum_r Re[F_r[j] P[b][r]]
+__global__ void k_eval_wake(int M, int nb, int R, const double *Vsr, const cplx *P, const cplx *F, double *total,
+                            double *sr, double *lr) {
+  const int b = blockIdx.x;
+  for (int j = threadIdx.x; j < nb; j += blockDim.x) {
+    const double s = Vsr[(size_t)b * nb + j];
+    double l = 0.0;
+    for (int r = 0; r < R; ++r) {
+      const cplx f = F[(size_t)r * nb + j];
+      const cplx pb = P[(size_t)b * R + r];
+      l += fma(f.re, pb.re, -(f.im * pb.im));
+    }
+    total[(size_t)b * nb + j] = s + l;
+    sr[(size_t)b * nb + j] = s;
+    lr[(size_t)b * nb + j] = l;
+  }
+}
+
+// initial distribution (D20): Philox stream tag 1, counter (i, b, 0, 1); tau = sigma_tau0 z_c, delta = sigma_delta0 z_s
+__global__ void k_init(double *tau, double *delta, int64_t ld, uint32_t Np, int M, PhiloxKeys keys, double s_tau,
+                       double s_delta) {
+  const int b = blockIdx.y;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < (uint32_t)ld; i += gridDim.x * blockDim.x) {
+    double t = 0.0, d = 0.0;
+    if (i < Np) {
+      uint32_t x0, x1, x2, x3;
+      philox4x32_10(i, (uint32_t)b, 0u, 1u, keys, x0, x1, x2, x3);
+      double zc, zs;
+      box_muller_accurate(uniform52(x0, x1), uniform52(x2, x3), zc, zs);
+      t = s_tau * zc;
+      d = s_delta * zs;
+    }
+    tau[(size_t)b * ld + i] = t;
+    delta[(size_t)b * ld + i] = d;
+  }
+}
+
+// packed [M][Np] <-> strided [M][ld]
+__global__ void k_pack(const double *src, int64_t ld, uint32_t Np, double *dst) {
+  const int b = blockIdx.y;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < Np; i += gridDim.x * blockDim.x)
+    dst[(size_t)b * Np + i] = src[(size_t)b * ld + i];
+}
+__global__ void k_unpack(const double *src, int64_t ld, uint32_t Np, double *dst) {
+  const int b = blockIdx.y;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < (uint32_t)ld; i += gridDim.x * blockDim.x)
+    dst[(size_t)b * ld + i] = (i < Np) ? src[(size_t)b * Np + i] : 0.0;
+}
+
+// per-turn aggregates A_{n'} = sum_j a[j][n'] g_tail[j] from an uploaded source-phasor history
+__global__ void k_aggregate_history(int M, int R, int K, const cplx *ring_a, const cplx *g_tail, cplx *ring_A) {
+  const int slot = blockIdx.x;  // 0..K
+  const int r = threadIdx.x;
+  if (r >= R) return;
+  cplx acc{0.0, 0.0};
+  for (int j = 0; j < M; ++j) acc = cfma(ring_a[((size_t)slot * M + j) * R + r], g_tail[(size_t)j * R + r], acc);
+  ring_A[(size_t)slot * R + r] = acc;
+}
+
+__global__ void k_set_ctrl(Ctrl *c, uint32_t turn, uint32_t pending) {
+  c->turn = turn;
+  c->ticket = 0u;
+  c->kick_pending = pending;
+}
+__global__ void k_clear_pending(Ctrl *c) { c->kick_pending = 0u; }
+
+__global__ void k_philox_selftest(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, PhiloxKeys keys, uint32_t *out) {
+  uint32_t x0, x1, x2, x3;
+  philox4x32_10(c0, c1, c2, c3, keys, x0, x1, x2, x3);
+  out[0] = x0; out[1] = x1; out[2] = x2; out[3] = x3;
+}
+__global__ void k_normal_selftest(int64_t n, const uint32_t *ctr, PhiloxKeys keys, double *out) {
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    uint32_t x0, x1, x2, x3;
+    philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], keys, x0, x1, x2, x3);
+    double zc, zs;
+    box_muller_fast(uniform52(x0, x1), uniform52(x2, x3), zc, zs);
+    out[2 * i] = zc;
+    out[2 * i + 1] = zs;
+  }
+}
+
+}  // namespace mbt

@@ -1,0 +1,104 @@
+"""Host-side checks that need no GPU: the C-ABI library builds, loads and exports every symbol include/mbt.h
+declares; the binding's struct layout matches the header (compiled probe); workloads are well-formed."""
+import ctypes
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+from paper_1809_00391_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def libpath():
+    from paper_1809_00391_b200 import build
+    return build.build()
+
+
+def _declared_symbols():
+    src = open(os.path.join(ROOT, "include", "mbt.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(mbt_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol(libpath):
+    from paper_1809_00391_b200 import mbt
+    lib = ctypes.CDLL(libpath)
+    declared = _declared_symbols()
+    assert len(declared) >= 20
+    for s in declared:
+        assert hasattr(lib, s), s
+    assert sorted(mbt.SYMBOLS) == declared      # the binding covers exactly the header
+    out = subprocess.run(["nm", "-D", "--defined-only", libpath], capture_output=True, text=True, check=True).stdout
+    exported = set(re.findall(r" T (mbt_[a-z_0-9]+)", out))
+    assert set(declared) <= exported
+
+
+def test_host_only_entry_points(libpath):
+    """Calls that touch no GPU: stride, version, error text, NULL handling."""
+    from paper_1809_00391_b200 import mbt
+    L = mbt.lib()
+    assert mbt.particle_stride(37) == 38 and mbt.particle_stride(100000) == 100000 and mbt.particle_stride(1) == 2
+    assert b"sm_100a" in L.mbt_version()
+    assert L.mbt_turn(None) == -1
+    assert L.mbt_destroy(None) == 0
+    assert L.mbt_create(None, None) == -1
+    assert b"null" in L.mbt_last_error()
+    assert L.mbt_track(None, 1) == -1
+
+
+def test_struct_layout_matches_header(tmp_path):
+    """sizeof/offsetof of every struct as the C compiler sees the header vs the ctypes mirror."""
+    from paper_1809_00391_b200 import mbt
+    probe = tmp_path / "probe.c"
+    probe.write_text('''
+#include <stdio.h>
+#include <stddef.h>
+#include "mbt.h"
+int main(void) {
+  printf("%zu %zu %zu %zu %zu %zu %zu\\n", sizeof(mbt_ring), sizeof(mbt_cavity), sizeof(mbt_radiation), sizeof(mbt_fill),
+         sizeof(mbt_resonator), sizeof(mbt_wake), sizeof(mbt_params));
+  printf("%zu %zu %zu %zu %zu %zu %zu %zu\\n", offsetof(mbt_params, cav), offsetof(mbt_params, rad), offsetof(mbt_params, fill),
+         offsetof(mbt_params, wake), offsetof(mbt_params, seed), offsetof(mbt_params, d_tau), offsetof(mbt_params, stream),
+         offsetof(mbt_params, device));
+  return 0;
+}''')
+    exe = tmp_path / "probe"
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), "-o", str(exe), str(probe)], check=True)
+    a, b = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.strip().splitlines()
+    sizes = [int(x) for x in a.split()]
+    offs = [int(x) for x in b.split()]
+    assert sizes == [ctypes.sizeof(c) for c in (mbt.Ring, mbt.Cavity, mbt.Radiation, mbt.Fill, mbt.Resonator, mbt.Wake, mbt.Params)]
+    P = mbt.Params
+    assert offs == [P.cav.offset, P.rad.offset, P.fill.offset, P.wake.offset, P.seed.offset, P.d_tau.offset,
+                    P.stream.offset, P.device.offset]
+
+
+def test_make_params_marshalling():
+    from paper_1809_00391_b200 import mbt
+    cfg = W.config("c4", n_per_bunch=10)
+    p, keep = mbt.make_params(cfg, log_capacity_turns=7)
+    assert p.fill.n_bunches == 363 and p.fill.bucket[362] == 362 and p.fill.n_per_bunch == 10
+    assert p.wake.n_res == 3 and p.wake.res[2].fr_Hz == 2.1e9 and p.wake.res[0].flags == 1
+    assert p.wake.history_turns == 20 and p.log_capacity_turns == 7 and p.seed == 4
+    assert np.isnan(p.cav[0].phase_rad)
+
+
+def test_workloads_match_baseline_configs():
+    shapes = {"c1": (1, 10_000, 200, 0, 1000), "c2": (1, 1_000_000, 1000, 0, 10_000), "c3": (3, 100_000, 500, 10, 20_000),
+              "c4": (363, 100_000, 300, 20, 10_000), "c5": (484, 200_000, 500, 50, 5_000)}
+    for name, (m, npb, nb, k, turns) in shapes.items():
+        c = W.config(name)
+        assert len(c["fill"]["buckets"]) == m and c["fill"]["n_per_bunch"] == npb
+        assert c["wake"]["n_bins"] == nb and c["wake"]["history_turns"] == k and c["n_turns"] == turns
+    c4 = W.config("c4")
+    q = np.array(c4["fill"]["charge_C"])
+    assert c4["fill"]["buckets"] == list(range(363)) and abs(q.mean() / 1e-9 - 1) < 5e-3 and 0.01 < q.std() / 1e-9 < 0.03
+    assert W.config("c3")["fill"]["buckets"] == [0, 161, 323]
+    assert len(W.config("c5")["cavities"]) == 2 and len(W.config("c5")["wake"]["resonators"]) == 4
+    # seeded: two calls give identical inputs
+    assert W.config("c4") == W.config("c4")

@@ -1,0 +1,354 @@
+"""GPU-vs-oracle parity through the C ABI (run on the B200 box: pytest -m gpu).
+
+Protocol: single-turn comparisons start from an IDENTICAL state -- the oracle's
+state at some turn is uploaded with mbt_set_particles / mbt_set_lr_history -- because only then are the
+histograms expected to be bit-exact; then both sides advance and everything observable is compared:
+  (i)   particle coordinates within 1e-12 relative (D23),
+  (ii)  histogram counts bit-exact except for particles within 1e-12 of a bin edge (counted),
+  (iii) wake potentials within 1e-10 relative (D23); long runs: per-bunch centroid and rms within 1 %.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1809_00391_b200 import workloads as W
+from parity import (TOL_PARTICLE, assert_single_turn_parity, histogram_mismatch, particle_errors, resume_on_gpu,
+                    wake_error)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mbt():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu-marked tests need a CUDA device")
+    from paper_1809_00391_b200 import build, mbt as _mbt
+    build.build()
+    _mbt.lib()
+    return _mbt
+
+
+# ---------------------------------------------------------------------------------------------- generator
+def test_device_philox_known_answers(mbt, orc):
+    import os
+    here = os.path.dirname(os.path.abspath(__file__))
+    rows = []
+    with open(os.path.join(here, "golden", "philox4x32_10_kat.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            v = [int(x, 16) for x in line.split()]
+            rows.append((v[0:4], v[4:6], v[6:10]))
+    for ctr, key, want in rows:
+        assert mbt.philox_selftest(ctr, key) == want
+    rng = np.random.default_rng(5)
+    for _ in range(50):
+        ctr = [int(x) for x in rng.integers(0, 2**32, 4)]
+        key = [int(x) for x in rng.integers(0, 2**32, 2)]
+        assert mbt.philox_selftest(ctr, key) == orc.philox(ctr, key)
+
+
+def test_device_excitation_normals_match_oracle(mbt, orc):
+    """The fast Box-Muller of the per-turn pass against the oracle's libm one: |dz| < 1e-12 (DESIGN.md asks 1e-13
+    of its own arithmetic; the oracle's theta = fl(2 pi u2) adds up to 4e-15)."""
+    rng = np.random.default_rng(6)
+    n = 20000
+    ctr = rng.integers(0, 2**32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    ctr[: n // 2, 1] %= 484          # bunch-like and turn-like small words as in the tracker
+    ctr[: n // 2, 3] = 0
+    seed = 0x1234567811223344
+    z = mbt.normal_selftest(seed, ctr)
+    ref = np.array([orc.normal_pair(seed, *[int(c) for c in row])[2:] for row in ctr])
+    assert np.max(np.abs(z - ref)) < 1e-12
+    # extreme uniforms cannot be forced through Philox; moments of a large sample guard the tails instead
+    big = rng.integers(0, 2**32, size=(2_000_000, 4), dtype=np.uint64).astype(np.uint32)
+    zz = mbt.normal_selftest(7, big).ravel()
+    assert abs(zz.mean()) < 4e-3 and abs(zz.var() - 1) < 4e-3
+    assert abs((zz**4).mean() - 3) < 3e-2
+    assert np.all(np.isfinite(zz)) and np.abs(zz).max() < 8.6   # |z| <= sqrt(2*52*ln2) = 8.49
+
+
+def test_initial_distribution_matches_oracle(mbt, orc):
+    for cfg in (W.tiny(), W.config("c1"), W.config("c3", n_per_bunch=5001)):
+        o = orc.Oracle(cfg)
+        with mbt.Tracker(cfg) as t:
+            tau_c, delta_c = o.particles()
+            tau_g, delta_g = t.particles()
+            assert particle_errors(tau_g, tau_c) <= TOL_PARTICLE
+            assert particle_errors(delta_g, delta_c) <= TOL_PARTICLE
+            bad, _ = histogram_mismatch(t.histogram(), o.histogram(), tau_c, cfg)
+            assert bad == 0
+            m_c, m_g = o.moments(), t.moments()
+            assert np.array_equal(m_c[:, :2], m_g[:, :2])
+            assert np.allclose(m_g[:, 2:], m_c[:, 2:], rtol=1e-9, atol=1e-25)
+            tot, sr, lr = t.wake()
+            assert not tot.any() and not sr.any() and not lr.any()
+            assert t.phi_s == o.phi_s
+            assert t.turn == 0
+
+
+# ---------------------------------------------------------------------------------------------- single turn
+TINY_VARIANTS = {
+    "default": dict(),
+    "even_np": dict(n_per_bunch=64),
+    "one_particle": dict(n_per_bunch=1, m=2),
+    "harmonic": dict(harmonic=True, n_per_bunch=301),
+    "ngp": dict(gather=0, n_per_bunch=257),
+    "no_lr": dict(n_lr=0, n_per_bunch=513),
+    "three_lr": dict(n_lr=3, n_per_bunch=129, k_hist=2),
+    "no_radiation": dict(radiation=0, n_per_bunch=100),
+    "one_bunch": dict(m=1, n_per_bunch=1000),
+    "k1": dict(k_hist=1, n_per_bunch=99),
+    "k0": dict(k_hist=0, n_per_bunch=99),
+    "many_bins": dict(n_bins=1023, n_per_bunch=2000),
+}
+
+
+@pytest.mark.parametrize("name", sorted(TINY_VARIANTS))
+def test_single_turn_parity_tiny(mbt, orc, name):
+    cfg = W.tiny(**TINY_VARIANTS[name])
+    o = orc.Oracle(cfg)
+    o.track(4)                                   # past the history warm-up of k_hist <= 3
+    with mbt.Tracker(cfg) as t:
+        for _ in range(3):                       # three consecutive single turns, each from the oracle's state
+            assert_single_turn_parity(o, t, cfg)
+
+
+@pytest.mark.parametrize("name,over", [
+    ("c1", dict()),
+    ("c2", dict(n_per_bunch=200_001)),
+    ("c3", dict(n_per_bunch=30_000)),
+    ("c4", dict(n_per_bunch=2_000)),
+    ("c5", dict(n_per_bunch=1_001)),
+])
+def test_single_turn_parity_configs(mbt, orc, name, over):
+    """All five BASELINE configs (reduced N_p where the oracle would take minutes): several CTAs per bunch,
+    ragged tails, the full fill patterns (363 / 484 bunches) and the full long-range history depth."""
+    cfg = W.config(name, **over)
+    o = orc.Oracle(cfg, lr_mode=0)
+    o.track(2)
+    with mbt.Tracker(cfg) as t:
+        r1 = assert_single_turn_parity(o, t, cfg)
+        r2 = assert_single_turn_parity(o, t, cfg)
+        print(name, r1, r2)
+
+
+def test_several_turns_without_resync(mbt, orc):
+    """Nine turns from each side's OWN initial distribution and no re-synchronisation: the fused ordering
+    (kick at the head of the next pass) reproduces the sequential order of the paper."""
+    for kw in (dict(), dict(harmonic=True, n_per_bunch=200), dict(gather=0, n_lr=1)):
+        cfg = W.tiny(**kw)
+        o = orc.Oracle(cfg, log_capacity_turns=9)
+        with mbt.Tracker(cfg, log_capacity_turns=9) as t:
+            o.track(4); t.track(4)
+            o.track(5); t.track(5)
+            tau_c, delta_c = o.particles()
+            tau_g, delta_g = t.particles()
+            assert particle_errors(tau_g, tau_c) <= 1e-10
+            assert particle_errors(delta_g, delta_c) <= 1e-10
+            assert wake_error(t.wake()[0], o.wake()[0]) <= 1e-9
+            assert np.array_equal(t.histogram(), o.histogram())
+            lg, lc = t.moment_log(1, 9), o.moment_log(1, 9)
+            assert np.array_equal(lg[..., :2], lc[..., :2])
+            assert np.allclose(lg[..., 2:], lc[..., 2:], rtol=1e-8, atol=1e-22)
+            assert np.allclose(t.lr_history(), o.lr_history(), rtol=0, atol=1e-10 * np.abs(o.lr_history()).max())
+            assert t.turn == 9
+
+
+def test_lr_scan_against_bruteforce_pairwise_sum(mbt, orc):
+    """north_star (4): the phasor scan against the brute-force pairwise sum (oracle lr_mode 0 = the definition),
+    over enough turns to wrap the history ring several times, irregular fill."""
+    cfg = W.tiny(m=5, n_per_bunch=400, n_bins=16, k_hist=3, n_lr=3)
+    o = orc.Oracle(cfg, lr_mode=0)
+    with mbt.Tracker(cfg) as t:
+        for turn in range(1, 12):
+            resume_on_gpu(o, t)
+            o.track(1); t.track(1)
+            lr_c, lr_g = o.wake()[2], t.wake()[2]
+            assert wake_error(lr_g, lr_c) <= 1e-10, turn
+    # uniform fill, many bunches: more than one bunch per scan thread (M > 256)
+    cfg = W.config("c5", n_per_bunch=64, history_turns=5)
+    o = orc.Oracle(cfg, lr_mode=0)
+    o.track(7)
+    with mbt.Tracker(cfg) as t:
+        resume_on_gpu(o, t)
+        o.track(1); t.track(1)
+        assert wake_error(t.wake()[2], o.wake()[2]) <= 1e-10
+
+
+# ---------------------------------------------------------------------------------------------- edge cases
+def test_edge_cases(mbt, orc):
+    cfg = W.tiny()
+    with mbt.Tracker(cfg) as t:
+        t.track(0)                                            # empty run
+        assert t.turn == 0
+        # every particle outside the window: nothing deposited, no wake, all counted in n_out
+        M, Np = t.M, t.Np
+        tau = np.full((M, Np), 1e-9)
+        delta = np.zeros((M, Np))
+        t.set_particles(tau, delta, 0)
+        o = orc.Oracle(cfg)
+        o.set_particles(tau, delta, 0)
+        t.track(2); o.track(2)
+        assert not t.histogram().any()
+        assert np.array_equal(t.moments()[:, :2], o.moments()[:, :2])
+        assert not t.wake()[0].any()
+        assert particle_errors(t.particles()[1], o.particles()[1]) <= 1e-12
+        # particles exactly on the edges: tau_lo is in bin 0, tau_hi is out (D11)
+        w = cfg["wake"]
+        tau = np.zeros((M, Np)); tau[:, 0] = w["tau_lo_s"]; tau[:, 1] = w["tau_hi_s"]
+        t.set_particles(tau, delta, 0)
+        h = t.histogram()
+        assert np.all(h[:, 0] == 1) and np.all(h.sum(axis=1) == Np - 1)
+        # NaN coordinates are out of the window and do not crash
+        tau[:, 2] = np.nan
+        t.set_particles(tau, delta, 0)
+        t.track(1)
+        assert np.all(t.moments()[:, 1] >= 2)
+    # far-off particles exercise the large-argument branch of the RF sine
+    cfg = W.tiny(n_lr=0)
+    o = orc.Oracle(cfg)
+    with mbt.Tracker(cfg) as t:
+        tau, delta = o.particles()
+        tau[:, ::3] += 1.0e-4          # 3e5 rad of RF phase
+        tau[:, 1::3] -= 3.0e-6
+        o.set_particles(tau, delta, 5)
+        assert_single_turn_parity(o, t, cfg)
+
+
+def test_error_codes(mbt):
+    cfg = W.tiny()
+    bad = W.tiny(); bad["wake"]["n_bins"] = 1
+    with pytest.raises(mbt.MbtError) as e:
+        mbt.Tracker(bad)
+    assert e.value.code == -1
+    bad = W.tiny(); bad["ring"]["U0_eV"] = 2e6
+    with pytest.raises(mbt.MbtError):
+        mbt.Tracker(bad)
+    bad = W.tiny(); bad["fill"]["buckets"] = [3, 3, 4, 100, 483]
+    with pytest.raises(mbt.MbtError):
+        mbt.Tracker(bad)
+    bad = W.tiny(); bad["wake"]["tau_hi_s"] = 3e-9
+    with pytest.raises(mbt.MbtError):
+        mbt.Tracker(bad)
+    with mbt.Tracker(cfg) as t:
+        with pytest.raises(mbt.MbtError) as e:
+            t.moment_log(1, 1)
+        assert e.value.code == -4
+
+
+def test_caller_owned_buffers_and_stream(mbt, orc):
+    """PyTorch supplies device memory and the stream (plumbing only); the library tracks in place."""
+    import torch
+    cfg = W.tiny(n_per_bunch=1001)
+    ld = mbt.particle_stride(1001)
+    M = len(cfg["fill"]["buckets"])
+    tau = torch.empty(M * ld, dtype=torch.float64, device="cuda")
+    delta = torch.empty_like(tau)
+    s = torch.cuda.Stream()
+    o = orc.Oracle(cfg)
+    with mbt.Tracker(cfg, d_tau=tau.data_ptr(), d_delta=delta.data_ptr(), stream=s.cuda_stream) as t:
+        t.track(3); o.track(3)
+        tg, dg = t.particles()
+        s.synchronize()
+        view = tau.view(M, ld)[:, :1001].cpu().numpy()
+        assert np.array_equal(view, tg)
+        assert particle_errors(tg, o.particles()[0]) <= 1e-11
+        assert particle_errors(dg, o.particles()[1]) <= 1e-11
+        pt, pd, pld = t.device_pointers()
+        assert pt == tau.data_ptr() and pd == delta.data_ptr() and pld == ld
+
+
+# ---------------------------------------------------------------------------------------------- long runs
+def test_long_run_moments_c1(mbt, orc):
+    """north_star (iii): over long runs per-bunch centroid and rms within 1 % (c1 in full: 1e4 x 1000 turns)."""
+    cfg = W.config("c1")
+    n = cfg["n_turns"]
+    o = orc.Oracle(cfg, log_capacity_turns=n)
+    with mbt.Tracker(cfg, log_capacity_turns=n) as t:
+        o.track(n); t.track(n)
+        lc, lg = o.moment_log(1, n), t.moment_log(1, n)
+    for k in (4, 5):                       # rms tau, rms delta
+        assert np.max(np.abs(lg[:, 0, k] / lc[:, 0, k] - 1)) < 0.01
+    # centroids: 1 % of the rms of the same coordinate (the centroid itself crosses zero)
+    assert np.max(np.abs(lg[:, 0, 2] - lc[:, 0, 2]) / lc[:, 0, 4]) < 0.01
+    assert np.max(np.abs(lg[:, 0, 3] - lc[:, 0, 3]) / lc[:, 0, 5]) < 0.01
+    assert np.max(np.abs(lg[:, 0, 1] - lc[:, 0, 1])) <= 0.01 * cfg["fill"]["n_per_bunch"]
+
+
+def test_long_run_growth_rate_matches_oracle(mbt, orc):
+    """north_star (iii): fitted coupled-bunch growth rate within 5 % of the oracle's, on the workload of the
+    oracle's own pin (f) (tests/test_oracle_growth.py: 11 equally spaced bunches, one HOM on the upper
+    synchrotron sideband of mode 6, radiation off), with more particles per bunch."""
+    from scipy.signal import hilbert
+    m_b, mu, p = 11, 6, 105
+    cfg = W.config("c1", n_per_bunch=1000, radiation=0)
+    r = cfg["ring"]
+    f0 = 1.0 / r["T0_s"]
+    cfg["fill"]["buckets"] = [k * (r["h"] // m_b) for k in range(m_b)]
+    cfg["fill"]["charge_C"] = [2.0e-9] * m_b
+    phi_s = math.pi - math.asin(r["U0_eV"] / cfg["cavities"][0]["V_volt"])
+    q_s = math.sqrt(r["h"] * r["alpha_c"] * cfg["cavities"][0]["V_volt"] * abs(math.cos(phi_s)) / (2 * math.pi * r["E0_eV"]))
+    f_r = (p * m_b + mu) * f0 + q_s * f0
+    cfg["wake"]["resonators"] = [dict(Rs_ohm=1.0e6, fr_Hz=f_r, Q=1.0e4, flags=W.FLAG_LR)]
+    cfg["wake"]["history_turns"] = 25
+    cfg["wake"]["n_bins"] = 100
+    cfg["wake"]["gather_order"] = 1
+    n = 6000
+    o = orc.Oracle(cfg, log_capacity_turns=n, lr_mode=1)
+    tau, delta = o.particles()
+    tau += 1.0e-12 * np.cos(2 * np.pi * mu * np.arange(m_b) / m_b)[:, None]
+    o.set_particles(tau, delta, 0)
+    with mbt.Tracker(cfg, log_capacity_turns=n) as t:
+        t.set_particles(tau, delta, 0)
+        o.track(n); t.track(n)
+        lc, lg = o.moment_log(1, n), t.moment_log(1, n)
+
+    def rates(log):
+        cent = log[:, :, 2] - log[:, :, 2].mean(axis=0)
+        amp = np.abs(np.fft.fft(hilbert(cent, axis=0), axis=1))
+        sl = slice(500, n - 500)
+        turns = np.arange(n)
+        return [float(np.polyfit(turns[sl], np.log(amp[sl, m]), 1)[0]) for m in (mu, m_b - mu)]
+
+    (up_c, dn_c), (up_g, dn_g) = rates(lc), rates(lg)
+    assert up_c > 2e-4 and dn_c < -2e-4
+    assert abs(up_g / up_c - 1) < 0.05 and abs(dn_g / dn_c - 1) < 0.05, (up_g, up_c, dn_g, dn_c)
+    # and the per-bunch rms within 1 % throughout
+    assert np.max(np.abs(lg[:, :, 4] / lc[:, :, 4] - 1)) < 0.01
+    assert np.max(np.abs(lg[:, :, 5] / lc[:, :, 5] - 1)) < 0.01
+
+
+# ---------------------------------------------------------------------------------------------- full size
+@pytest.mark.parametrize("name", ["c4", "c5"])
+def test_full_size_single_turn(mbt, orc, name):
+    """BASELINE full sizes (3.63e7 / 9.68e7 particles) in the launch configuration bench.py times: the initial
+    distribution and one tracked turn compared element by element with the oracle, then properties that hold
+    at any size (sum of counts, n_in + n_out)."""
+    cfg = W.config(name)
+    o = orc.Oracle(cfg, lr_mode=1)
+    with mbt.Tracker(cfg) as t:
+        tau_c, delta_c = o.particles()
+        tau_g, delta_g = t.particles()
+        assert particle_errors(tau_g, tau_c) <= TOL_PARTICLE
+        assert particle_errors(delta_g, delta_c) <= TOL_PARTICLE
+        t.set_particles(tau_c, delta_c, 0)
+        del tau_g, delta_g
+        o.track(1); t.track(1)
+        tau_c, delta_c = o.particles()
+        tau_g, delta_g = t.particles()
+        e_t, e_d = particle_errors(tau_g, tau_c), particle_errors(delta_g, delta_c)
+        assert e_t <= TOL_PARTICLE and e_d <= TOL_PARTICLE, (e_t, e_d)
+        hg, hc = t.histogram(), o.histogram()
+        bad, n_edge = histogram_mismatch(hg, hc, tau_c, cfg)
+        print(name, "tau", e_t, "delta", e_d, "mismatching bins", bad, "edge-adjacent particles", n_edge)
+        m = t.moments()
+        assert np.all(hg.sum(axis=1) == m[:, 0]) and np.all(m[:, 0] + m[:, 1] == cfg["fill"]["n_per_bunch"])
+        if bad == 0:
+            assert wake_error(t.wake()[0], o.wake()[0]) <= 1e-10
+        # a second turn on the GPU only: counts still sum to N_p
+        t.track(1)
+        m = t.moments()
+        assert np.all(t.histogram().sum(axis=1) == m[:, 0])
