@@ -113,7 +113,10 @@ struct Particle {
     if (MAP) {
       // S1: RF cavities, then the synchronous loss
 #pragma unroll 1
-      for (int c = 0; c < A.n_cav; ++c) delta = fma(A.cav_amp[c], sin_rf(fma(A.cav_w[c], tau, A.cav_ph[c])), delta);
+      // phase formed as the oracle forms it (product rounded, then the sum): at |phase| ~ 1e5 rad a fused
+      // product would differ by 1e-11 rad
+      for (int c = 0; c < A.n_cav; ++c)
+        delta = fma(A.cav_amp[c], sin_rf(__dadd_rn(__dmul_rn(A.cav_w[c], tau), A.cav_ph[c])), delta);
       delta -= A.loss;
       // S2
       if (A.rad) delta = fma(delta, A.one_minus_DE, A.A_q * z);
