@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -110,6 +111,10 @@ struct mbt_handle {
   DevBuf<uint32_t> hist, hist_last;
   DevBuf<unsigned long long> nout_acc;
   DevBuf<Ctrl> ctrl;
+  void (*fn_map)(const Args) = nullptr;    // k_pass<true, ...> chosen for this handle's effects
+  void (*fn_flush)(const Args) = nullptr;  // k_pass<false, ...>
+  int npair = 1;
+  DevBuf<LogTabEntry> logtab;
   cudaGraphExec_t graph1 = nullptr, graphU = nullptr;
   int unroll = 16;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -118,8 +123,25 @@ struct mbt_handle {
 
 namespace {
 
+// ---- the instantiations of the fused pass and their selection at create time
+typedef void (*pass_fn)(const Args);
+
+template <int NPAIR>
+pass_fn select_map(bool rad, int gather, int n_cav) {
+#define MBT_SEL_(R, G)                                                    \
+  (n_cav == 1 ? (pass_fn)k_pass<true, R, G, 1, NPAIR>                      \
+              : n_cav == 2 ? (pass_fn)k_pass<true, R, G, 2, NPAIR> : (pass_fn)k_pass<true, R, G, 0, NPAIR>)
+  if (rad) return gather ? MBT_SEL_(true, 1) : MBT_SEL_(true, 0);
+  return gather ? MBT_SEL_(false, 1) : MBT_SEL_(false, 0);
+#undef MBT_SEL_
+}
+template <int NPAIR>
+pass_fn select_flush(int gather) {
+  return gather ? (pass_fn)k_pass<false, false, 1, 0, NPAIR> : (pass_fn)k_pass<false, false, 0, 0, NPAIR>;
+}
+
 int enqueue_turn(mbt_handle *h) {
-  k_pass<true><<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
+  h->fn_map<<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
   k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
   return 0;
 }
@@ -139,7 +161,7 @@ int build_graph(mbt_handle *h, int turns, cudaGraphExec_t *out) {
 int flush(mbt_handle *h) {
   if (!h->dirty) return 0;
   CU(cudaSetDevice(h->device));
-  k_pass<false><<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
+  h->fn_flush<<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
   WakeArgs wa = h->wargs;
   wa.mode = 1;
   k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(wa);
@@ -165,7 +187,7 @@ void destroy(mbt_handle *h) {
   h->qm.release(); h->w.release(); h->Vsr.release(); h->mom_acc.release(); h->mom_last.release(); h->mom_log.release();
   h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
   h->Esrc.release(); h->F.release(); h->g_step.release(); h->g_tail.release(); h->g_hist.release(); h->a_cur.release();
-  h->ring_a.release(); h->ring_A.release(); h->P.release();
+  h->ring_a.release(); h->ring_A.release(); h->P.release(); h->logtab.release();
   h->hist.release(); h->hist_last.release(); h->nout_acc.release(); h->ctrl.release();
   if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
   delete h;
@@ -385,6 +407,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   CUH(h->mom_last.alloc((size_t)M * 6));
   if (h->log_cap > 0) CUH(h->mom_log.alloc((size_t)h->log_cap * M * 6));
   CUH(h->ctrl.alloc(1));
+  CUH(h->logtab.upload(std::vector<LogTabEntry>(kLogTabHost, kLogTabHost + 128)));
 
   A.tau = h->d_tau;
   A.delta = h->d_delta;
@@ -395,6 +418,8 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   A.mom_acc = h->mom_acc.p;
   A.nout_acc = h->nout_acc.p;
   A.ctrl = h->ctrl.p;
+  A.logtab = h->logtab.p;
+  A.mt = make_math_tab();
 
   WakeArgs &Wa = h->wargs;
   memset(&Wa, 0, sizeof Wa);
@@ -410,16 +435,21 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   Wa.ctrl = h->ctrl.p;
 
   // ---- launch shapes: one resident wave of CTAs, each owning a contiguous run of pairs
-  h->smem_pass = (size_t)nb * (sizeof(double) + sizeof(uint32_t));
+  h->npair = kDefaultNPair;
+  if (const char *e = getenv("MBT_NPAIR")) h->npair = (atoi(e) == 2) ? 2 : 1;  // measurement knob
+  const bool rad_on = p->rad.enable != 0;
+  h->fn_map = h->npair == 2 ? select_map<2>(rad_on, wk.gather_order, p->n_cav) : select_map<1>(rad_on, wk.gather_order, p->n_cav);
+  h->fn_flush = h->npair == 2 ? select_flush<2>(wk.gather_order) : select_flush<1>(wk.gather_order);
+  h->smem_pass = pass_smem_bytes(nb);
   h->smem_wake = (size_t)nb * 2 * sizeof(double);
-  CUH(cudaFuncSetAttribute(k_pass<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
-  CUH(cudaFuncSetAttribute(k_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
+  CUH(cudaFuncSetAttribute((const void *)h->fn_map, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
+  CUH(cudaFuncSetAttribute((const void *)h->fn_flush, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
   CUH(cudaFuncSetAttribute(k_wake, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_wake));
   int occ = 0;
-  CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pass<true>, kPassThreads, h->smem_pass));
+  CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)h->fn_map, kPassThreads, h->smem_pass));
   if (occ < 1) occ = 1;
   const int64_t max_cta = (int64_t)prop.multiProcessorCount * occ;
-  const int64_t need = (A.total_pairs + kPassThreads - 1) / kPassThreads;
+  const int64_t need = (A.total_pairs + (int64_t)kPassThreads * h->npair - 1) / ((int64_t)kPassThreads * h->npair);
   h->grid_pass = (int)(need < max_cta ? need : max_cta);
 
   // ---- initial distribution (D20) on the device
@@ -480,7 +510,7 @@ int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, dou
   CU(cudaEventRecord(h->ev0, h->stream));
   for (int64_t t = 0; t < n_turns; ++t) {
     CU(cudaEventRecord(ev[3 * t], h->stream));
-    k_pass<true><<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
+    h->fn_map<<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
     CU(cudaEventRecord(ev[3 * t + 1], h->stream));
     k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
     CU(cudaEventRecord(ev[3 * t + 2], h->stream));
@@ -692,16 +722,20 @@ int mbt_normal_selftest(uint64_t seed, int64_t n, const uint32_t *ctr, double *o
   if (n == 0) return 0;
   uint32_t *dc = nullptr;
   double *dz = nullptr;
+  LogTabEntry *dl = nullptr;
+  CU(cudaMalloc((void **)&dl, sizeof kLogTabHost));
+  CU(cudaMemcpy(dl, kLogTabHost, sizeof kLogTabHost, cudaMemcpyHostToDevice));
   CU(cudaMalloc((void **)&dc, (size_t)n * 4 * sizeof(uint32_t)));
   cudaError_t e = cudaMalloc((void **)&dz, (size_t)n * 2 * sizeof(double));
   if (e != cudaSuccess) { cudaFree(dc); CU(e); }
   e = cudaMemcpy(dc, ctr, (size_t)n * 4 * sizeof(uint32_t), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) {
-    k_normal_selftest<<<148, 256>>>(n, dc, philox_expand_key((uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32)), dz);
+    k_normal_selftest<<<148, 256>>>(n, dc, philox_expand_key((uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32)), dl, make_math_tab(), dz);
     e = cudaMemcpy(out, dz, (size_t)n * 2 * sizeof(double), cudaMemcpyDeviceToHost);
   }
   cudaFree(dc);
   cudaFree(dz);
+  cudaFree(dl);
   CU(e);
   return 0;
 }

@@ -21,6 +21,7 @@ constexpr int kPassThreads = 256;
 constexpr int kWakeThreads = 256;
 constexpr int kMaxCav = 8;
 constexpr int kMaxLR = 8;
+constexpr int kDefaultNPair = 1;  // pairs per thread and iteration of the pass (1 or 2)
 
 struct cplx {
   double re, im;
@@ -75,78 +76,54 @@ struct Args {
   double *mom_acc;      // [M][4]    sum tau, sum delta, sum tau^2, sum delta^2
   unsigned long long *nout_acc;  // [M]
   Ctrl *ctrl;
+  const LogTabEntry *logtab;  // [128] device copy of the log table
+  MathTab mt;
 };
+
+// shared-memory layout of one CTA of the pass (dynamic): wake table, staging copy of V, counts, log table
+struct WakeCell {
+  double mid, dif;  // v(f) = mid + f * dif, f in [-1/2, 1/2] around the cell boundary (linear gather)
+};
+__host__ __device__ inline size_t pass_smem_bytes(int nb) {
+  return (size_t)(nb + 2) * sizeof(WakeCell) + (size_t)nb * sizeof(double) + (size_t)nb * sizeof(uint32_t) +
+         128 * sizeof(LogTabEntry) + 16;
+}
 
 // ------------------------------------------------------------------ fused particle pass
 // MAP = true : S0 S7 | S1 S2 S3 | S4      (a tracked turn)
 // MAP = false: S0 S7 |          | S4      (flush of the pending kick before the state is observed)
-template <bool MAP>
-struct Particle {
-  static __device__ __forceinline__ void step(const Args &A, const double *sV, uint32_t *sH, double &tau, double &delta,
-                                              double z, double &st, double &sd, double &stt, double &sdd,
-                                              uint32_t &nout) {
-    // S0: kick of the previous turn's wake.  t exactly as the binning computed it (one subtraction, one
-    // multiplication, no contraction), so the in-window decision is the one that deposited the particle.
-    double t = __dmul_rn(__dsub_rn(tau, A.tau_lo), A.invDelta);
-    bool in = (t >= 0.0) && (t < A.nb_d);
-    if (in) {
-      double v;
-      if (A.gather == 0) {
-        v = sV[__double2int_rd(t)];
-      } else {
-        // linear between bin centres, constant in the outer half bins (D12)
-        double u = fmin(fmax(t - 0.5, 0.0), A.nb_d - 1.0);
-        int j0 = min(__double2int_rd(u), A.nb - 2);
-        double f = u - (double)j0;
-        double v0 = sV[j0], v1 = sV[j0 + 1];
-        v = fma(f, v1 - v0, v0);
-      }
-      delta = fma(-v, A.invE0, delta);
-    } else {
-      nout += 1u;
-    }
-    // S7: moments of the state after the kick
-    st += tau;
-    sd += delta;
-    stt = fma(tau, tau, stt);
-    sdd = fma(delta, delta, sdd);
-    if (MAP) {
-      // S1: RF cavities, then the synchronous loss
-#pragma unroll 1
-      // phase formed as the oracle forms it (product rounded, then the sum): at |phase| ~ 1e5 rad a fused
-      // product would differ by 1e-11 rad
-      for (int c = 0; c < A.n_cav; ++c)
-        delta = fma(A.cav_amp[c], sin_rf(__dadd_rn(__dmul_rn(A.cav_w[c], tau), A.cav_ph[c])), delta);
-      delta -= A.loss;
-      // S2
-      if (A.rad) delta = fma(delta, A.one_minus_DE, A.A_q * z);
-      // S3
-      tau = fma(A.drift, delta, tau);
-      // S4
-      t = __dmul_rn(__dsub_rn(tau, A.tau_lo), A.invDelta);
-      in = (t >= 0.0) && (t < A.nb_d);
-    }
-    if (in) atomicAdd(&sH[__double2int_rd(t)], 1u);
-  }
-};
-
-template <bool MAP>
-__global__ void __launch_bounds__(kPassThreads, 3) k_pass(const __grid_constant__ Args A) {
-  extern __shared__ double smem_d[];
-  double *sV = smem_d;                                  // [nb]
-  uint32_t *sH = reinterpret_cast<uint32_t *>(sV + A.nb);  // [nb]
+// RAD: radiation on; GATHER: 1 linear, 0 nearest grid point; NCAV: 1 or 2 cavities unrolled, 0 = loop over n_cav.
+// NPAIR pairs (2 NPAIR particles) are advanced together per thread and iteration, in lock step and without
+// branches, so that every coefficient load serves all of them and their dependency chains interleave.
+//
+// Wake gather (S0, D12): with kk = rint(t) the particle sits between the centres of bins kk-1 and kk, at
+// f = t - kk in [-1/2, 1/2] from their midpoint: v = mid[kk] + f dif[kk], mid = (V[kk-1]+V[kk])/2,
+// dif = V[kk]-V[kk-1], with V[-1] := V[0] and V[nb] := V[nb-1] (constant outer half bins).  Cell nb+1 is zero and
+// serves every particle outside the window (no kick, D11), which keeps the step branch-free.
+template <bool MAP, bool RAD, int GATHER, int NCAV, int NPAIR>
+__global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const __grid_constant__ Args A) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  WakeCell *sW = reinterpret_cast<WakeCell *>(smem_raw);                        // [nb+2]
+  double *sV = reinterpret_cast<double *>(sW + (A.nb + 2));                     // [nb]
+  LogTabEntry *sL = reinterpret_cast<LogTabEntry *>(sV + A.nb);                 // [128]
+  uint32_t *sH = reinterpret_cast<uint32_t *>(sL + 128);                        // [nb]
   __shared__ double s_red[kPassThreads / 32][4];
   __shared__ uint32_t s_nout[kPassThreads / 32];
+  constexpr int NP = 2 * NPAIR;               // particles per thread and iteration
+  constexpr uint32_t STRIDE = kPassThreads * NPAIR;  // pairs per CTA and iteration
 
   const int tid = threadIdx.x;
   const uint32_t n = A.ctrl->turn + 1u;  // the turn this pass tracks (Philox counter word, D24)
   const bool have_kick = A.ctrl->kick_pending != 0u;
+  const int nb = A.nb;
+  if (MAP && RAD)
+    for (int i = tid; i < 128; i += kPassThreads) sL[i] = A.logtab[i];
 
-  // contiguous range of pairs for this CTA, in multiples of the CTA width
+  // contiguous range of pairs for this CTA, in multiples of the CTA's stride
   int64_t per = (A.total_pairs + gridDim.x - 1) / gridDim.x;
-  per = (per + kPassThreads - 1) / kPassThreads * kPassThreads;
+  per = (per + STRIDE - 1) / STRIDE * STRIDE;
   int64_t begin = (int64_t)blockIdx.x * per;
-  int64_t end = begin + per < A.total_pairs ? begin + per : A.total_pairs;
+  const int64_t end = begin + per < A.total_pairs ? begin + per : A.total_pairs;
 
   while (begin < end) {
     const int b = (int)(begin / A.ppb);
@@ -154,19 +131,33 @@ __global__ void __launch_bounds__(kPassThreads, 3) k_pass(const __grid_constant_
     const int64_t left = end - begin;
     const uint32_t p1 = (left < (int64_t)(A.ppb - p0)) ? (uint32_t)(p0 + left) : A.ppb;
 
-    // stage the wake grid of bunch b: V = V_SR + sum_r Re[F_r[j] P[b][r]]   (S6 expansion), clear the counts
-    for (int j = tid; j < A.nb; j += kPassThreads) {
+    // stage the wake of bunch b: V = V_SR + sum_r Re[F_r[j] P[b][r]] (S6 expansion), then the gather cells
+    for (int j = tid; j < nb; j += kPassThreads) {
       double v = 0.0;
       if (have_kick) {
-        v = A.Vsr[(size_t)b * A.nb + j];
+        v = A.Vsr[(size_t)b * nb + j];
         for (int r = 0; r < A.R; ++r) {
-          const cplx f = A.F[(size_t)r * A.nb + j];
+          const cplx f = A.F[(size_t)r * nb + j];
           const cplx pb = A.P[(size_t)b * A.R + r];
           v += fma(f.re, pb.re, -(f.im * pb.im));
         }
       }
       sV[j] = v;
       sH[j] = 0u;
+    }
+    __syncthreads();
+    for (int k = tid; k < nb + 2; k += kPassThreads) {
+      WakeCell c{0.0, 0.0};
+      if (GATHER == 1) {
+        if (k <= nb) {
+          const double lo = sV[k > 0 ? k - 1 : 0], hi = sV[k < nb ? k : nb - 1];
+          c.mid = 0.5 * (lo + hi);
+          c.dif = hi - lo;
+        }
+      } else if (k < nb) {
+        c.mid = sV[k];
+      }
+      sW[k] = c;
     }
     __syncthreads();
 
@@ -176,28 +167,121 @@ __global__ void __launch_bounds__(kPassThreads, 3) k_pass(const __grid_constant_
     double2 *D = reinterpret_cast<double2 *>(A.delta + (size_t)b * A.ld);
 
     uint32_t p = p0 + tid;
-    double2 t2, d2;
-    if (p < p1) { t2 = T[p]; d2 = D[p]; }
+    double2 t2[NPAIR], d2[NPAIR], t2n[NPAIR], d2n[NPAIR];
+#pragma unroll
+    for (int q = 0; q < NPAIR; ++q)
+      if (p + q * kPassThreads < p1) { t2[q] = T[p + q * kPassThreads]; d2[q] = D[p + q * kPassThreads]; }
     while (p < p1) {
-      const uint32_t pn = p + kPassThreads;
-      double2 t2n, d2n;
-      if (pn < p1) { t2n = T[pn]; d2n = D[pn]; }  // prefetch the next pair while this one is computed
+      const uint32_t pn = p + STRIDE;
+#pragma unroll
+      for (int q = 0; q < NPAIR; ++q)  // prefetch the next iteration while this one is computed
+        if (pn + q * kPassThreads < p1) { t2n[q] = T[pn + q * kPassThreads]; d2n[q] = D[pn + q * kPassThreads]; }
 
-      double z0 = 0.0, z1 = 0.0;
-      if (MAP && A.rad) {
-        // one Philox call and one Box-Muller serve both particles of the 128-bit load (D8):
-        // counter (pair, bunch, turn, tag 0); even particle takes z_c, odd particle z_s
-        uint32_t x0, x1, x2, x3;
-        philox4x32_10(p, (uint32_t)b, n, 0u, A.keys, x0, x1, x2, x3);
-        box_muller_fast(uniform52(x0, x1), uniform52(x2, x3), z0, z1);
+      double tau[NP], del[NP], z[NP];
+      bool live[NP];
+#pragma unroll
+      for (int q = 0; q < NPAIR; ++q) {
+        const uint32_t pq = p + q * kPassThreads;
+        tau[2 * q] = t2[q].x; tau[2 * q + 1] = t2[q].y;
+        del[2 * q] = d2[q].x; del[2 * q + 1] = d2[q].y;
+        live[2 * q] = pq < p1;                              // a whole pair may be past the end when NPAIR = 2
+        live[2 * q + 1] = live[2 * q] && (2u * pq + 1u < A.Np);  // odd slot of the last pair is padding if N_p is odd
+        z[2 * q] = z[2 * q + 1] = 0.0;
+        if (MAP && RAD) {
+          // one Philox call and one Box-Muller serve both particles of the 128-bit load (D8):
+          // counter (pair, bunch, turn, tag 0); even particle takes z_c, odd particle z_s
+          uint32_t x0, x1, x2, x3;
+          philox4x32_10(pq, (uint32_t)b, n, 0u, A.keys, x0, x1, x2, x3);
+          box_muller_fast(A.mt, sL, x0, x1, x2, x3, A.A_q, z[2 * q], z[2 * q + 1]);
+        }
       }
-      Particle<MAP>::step(A, sV, sH, t2.x, d2.x, z0, st, sd, stt, sdd, nout);
-      if (2u * p + 1u < A.Np) {  // the odd slot of the last pair is padding when N_p is odd
-        Particle<MAP>::step(A, sV, sH, t2.y, d2.y, z1, st, sd, stt, sdd, nout);
+      // S0: kick of the previous turn's wake.  t exactly as the binning computed it (one subtraction, one
+      // multiplication, no contraction), so the in-window decision is the one that deposited the particle.
+      double t[NP];
+      bool in[NP];
+#pragma unroll
+      for (int i = 0; i < NP; ++i) {
+        t[i] = __dmul_rn(__dsub_rn(tau[i], A.tau_lo), A.invDelta);
+        in[i] = live[i] && (t[i] >= 0.0) && (t[i] < A.nb_d);
+        int kk;
+        double f;
+        if (GATHER == 1) {
+          const double km = t[i] + A.mt.magic;
+          kk = __double2loint(km);
+          f = t[i] - (km - A.mt.magic);
+        } else {
+          kk = __double2int_rd(t[i]);
+          f = 0.0;
+        }
+        kk = in[i] ? kk : nb + 1;
+        const WakeCell c = sW[kk];
+        del[i] = fma(-fma(f, c.dif, c.mid), A.invE0, del[i]);
+        if (!in[i] && live[i]) nout += 1u;
       }
-      if (MAP) T[p] = t2;
-      D[p] = d2;
-      t2 = t2n; d2 = d2n; p = pn;
+      // S7: moments of the state after the kick
+#pragma unroll
+      for (int i = 0; i < NP; ++i)
+        if (live[i]) {
+          st += tau[i];
+          sd += del[i];
+          stt = fma(tau[i], tau[i], stt);
+          sdd = fma(del[i], del[i], sdd);
+        }
+      if (MAP) {
+        // S1: RF cavities.  The phase is formed as the oracle forms it (product rounded, then the sum).
+        constexpr int NC = NCAV > 0 ? NCAV : 1;
+        bool fast = true;
+        if (NCAV > 0) {
+          double y[NP][NC];
+#pragma unroll
+          for (int i = 0; i < NP; ++i)
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+              y[i][c] = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
+              fast = fast && (fabs(y[i][c]) < 65536.0);
+            }
+          if (__builtin_expect(fast, 1)) {
+#pragma unroll
+            for (int c = 0; c < NC; ++c)
+#pragma unroll
+              for (int i = 0; i < NP; ++i) del[i] = fma(A.cav_amp[c], sin_rf_fast(A.mt, y[i][c]), del[i]);
+          } else {  // a particle long lost from the bucket (or not finite): library sine, same order of the sum
+#pragma unroll 1
+            for (int i = 0; i < NP; ++i)
+#pragma unroll 1
+              for (int c = 0; c < NC; ++c) del[i] = fma(A.cav_amp[c], sin(y[i][c]), del[i]);
+          }
+        } else {
+#pragma unroll 1
+          for (int c = 0; c < A.n_cav; ++c)
+#pragma unroll 1
+            for (int i = 0; i < NP; ++i) {
+              const double y = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
+              del[i] = fma(A.cav_amp[c], fabs(y) < 65536.0 ? sin_rf_fast(A.mt, y) : sin(y), del[i]);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < NP; ++i) {
+          del[i] -= A.loss;
+          if (RAD) del[i] = fma(del[i], A.one_minus_DE, z[i]);  // S2 (z already scaled by sigma_delta sqrt(2 D_E))
+          tau[i] = fma(A.drift, del[i], tau[i]);                // S3
+          t[i] = __dmul_rn(__dsub_rn(tau[i], A.tau_lo), A.invDelta);  // S4
+          in[i] = live[i] && (t[i] >= 0.0) && (t[i] < A.nb_d);
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < NP; ++i)
+        if (in[i]) atomicAdd(&sH[__double2int_rd(t[i])], 1u);
+#pragma unroll
+      for (int q = 0; q < NPAIR; ++q)
+        if (live[2 * q]) {
+          const uint32_t pq = p + q * kPassThreads;
+          if (MAP) T[pq] = make_double2(tau[2 * q], tau[2 * q + 1]);
+          D[pq] = make_double2(del[2 * q], del[2 * q + 1]);
+        }
+#pragma unroll
+      for (int q = 0; q < NPAIR; ++q) { t2[q] = t2n[q]; d2[q] = d2n[q]; }
+      p = pn;
     }
 
     // S7: warp shuffles, then one atomic per CTA and bunch
@@ -226,9 +310,9 @@ __global__ void __launch_bounds__(kPassThreads, 3) k_pass(const __grid_constant_
       if (s) atomicAdd(&A.nout_acc[b], (unsigned long long)s);
     }
     // S4: flush the CTA's counts into the bunch histogram (integer, order-independent)
-    for (int j = tid; j < A.nb; j += kPassThreads) {
+    for (int j = tid; j < nb; j += kPassThreads) {
       const uint32_t c = sH[j];
-      if (c) atomicAdd(&A.hist[(size_t)b * A.nb + j], c);
+      if (c) atomicAdd(&A.hist[(size_t)b * nb + j], c);
     }
     __syncthreads();
     begin += (int64_t)(p1 - p0);
@@ -502,12 +586,16 @@ __global__ void k_philox_selftest(uint32_t c0, uint32_t c1, uint32_t c2, uint32_
   philox4x32_10(c0, c1, c2, c3, keys, x0, x1, x2, x3);
   out[0] = x0; out[1] = x1; out[2] = x2; out[3] = x3;
 }
-__global__ void k_normal_selftest(int64_t n, const uint32_t *ctr, PhiloxKeys keys, double *out) {
+__global__ void k_normal_selftest(int64_t n, const uint32_t *ctr, PhiloxKeys keys, const LogTabEntry *logtab, MathTab mt,
+                                  double *out) {
+  __shared__ LogTabEntry sL[128];
+  for (int i = threadIdx.x; i < 128; i += blockDim.x) sL[i] = logtab[i];
+  __syncthreads();
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
     uint32_t x0, x1, x2, x3;
     philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], keys, x0, x1, x2, x3);
     double zc, zs;
-    box_muller_fast(uniform52(x0, x1), uniform52(x2, x3), zc, zs);
+    box_muller_fast(mt, sL, x0, x1, x2, x3, 1.0, zc, zs);
     out[2 * i] = zc;
     out[2 * i + 1] = zs;
   }
