@@ -163,19 +163,23 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
 
     double st = 0.0, sd = 0.0, stt = 0.0, sdd = 0.0;
     uint32_t nout = 0u;
-    double2 *T = reinterpret_cast<double2 *>(A.tau + (size_t)b * A.ld);
-    double2 *D = reinterpret_cast<double2 *>(A.delta + (size_t)b * A.ld);
-
+    // one running pointer per thread: tau pair at T[q * kPassThreads], delta pair at the constant byte distance d_off
     uint32_t p = p0 + tid;
+    double2 *T = reinterpret_cast<double2 *>(A.tau + (size_t)b * A.ld) + p;
+    const ptrdiff_t d_off = reinterpret_cast<const char *>(A.delta) - reinterpret_cast<const char *>(A.tau);
+#define MBT_D(ptr) reinterpret_cast<double2 *>(reinterpret_cast<char *>(ptr) + d_off)
     double2 t2[NPAIR], d2[NPAIR], t2n[NPAIR], d2n[NPAIR];
 #pragma unroll
     for (int q = 0; q < NPAIR; ++q)
-      if (p + q * kPassThreads < p1) { t2[q] = T[p + q * kPassThreads]; d2[q] = D[p + q * kPassThreads]; }
+      if (p + q * kPassThreads < p1) { t2[q] = T[q * kPassThreads]; d2[q] = *MBT_D(T + q * kPassThreads); }
     while (p < p1) {
       const uint32_t pn = p + STRIDE;
 #pragma unroll
       for (int q = 0; q < NPAIR; ++q)  // prefetch the next iteration while this one is computed
-        if (pn + q * kPassThreads < p1) { t2n[q] = T[pn + q * kPassThreads]; d2n[q] = D[pn + q * kPassThreads]; }
+        if (pn + q * kPassThreads < p1) {
+          t2n[q] = T[STRIDE + q * kPassThreads];
+          d2n[q] = *MBT_D(T + STRIDE + q * kPassThreads);
+        }
 
       double tau[NP], del[NP], z[NP];
       bool live[NP];
@@ -206,9 +210,9 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
         int kk;
         double f;
         if (GATHER == 1) {
-          const double km = t[i] + A.mt.magic;
+          const double km = t[i] + MBT_MAGIC;
           kk = __double2loint(km);
-          f = t[i] - (km - A.mt.magic);
+          f = t[i] - (km - MBT_MAGIC);
         } else {
           kk = __double2int_rd(t[i]);
           f = 0.0;
@@ -228,37 +232,31 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
           sdd = fma(del[i], del[i], sdd);
         }
       if (MAP) {
-        // S1: RF cavities.  The phase is formed as the oracle forms it (product rounded, then the sum).
-        constexpr int NC = NCAV > 0 ? NCAV : 1;
-        bool fast = true;
+        // S1: RF cavities.  The phase is formed as the oracle forms it (product rounded, then the sum).  A particle
+        // long lost from the bucket (|y| >= 2^16, or not finite) takes the library sine in a cold out-of-line call;
+        // every index below is a compile-time constant, so tau[] / del[] stay in registers (no local memory).
         if (NCAV > 0) {
-          double y[NP][NC];
 #pragma unroll
-          for (int i = 0; i < NP; ++i)
+          for (int c = 0; c < NCAV; ++c)
 #pragma unroll
-            for (int c = 0; c < NC; ++c) {
-              y[i][c] = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
-              fast = fast && (fabs(y[i][c]) < 65536.0);
-            }
-          if (__builtin_expect(fast, 1)) {
-#pragma unroll
-            for (int c = 0; c < NC; ++c)
-#pragma unroll
-              for (int i = 0; i < NP; ++i) del[i] = fma(A.cav_amp[c], sin_rf_fast(A.mt, y[i][c]), del[i]);
-          } else {  // a particle long lost from the bucket (or not finite): library sine, same order of the sum
-#pragma unroll 1
-            for (int i = 0; i < NP; ++i)
-#pragma unroll 1
-              for (int c = 0; c < NC; ++c) del[i] = fma(A.cav_amp[c], sin(y[i][c]), del[i]);
-          }
-        } else {
-#pragma unroll 1
-          for (int c = 0; c < A.n_cav; ++c)
-#pragma unroll 1
             for (int i = 0; i < NP; ++i) {
               const double y = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
-              del[i] = fma(A.cav_amp[c], fabs(y) < 65536.0 ? sin_rf_fast(A.mt, y) : sin(y), del[i]);
+              double s = sin_rf_fast(A.mt, y);
+              if (__builtin_expect(!(fabs(y) < 65536.0), 0)) s = sin_rf_slow(y);
+              del[i] = fma(A.cav_amp[c], s, del[i]);
             }
+        } else {
+#pragma unroll 1
+          for (int c = 0; c < A.n_cav; ++c) {
+            const double cw = A.cav_w[c], cp = A.cav_ph[c], ca = A.cav_amp[c];
+#pragma unroll
+            for (int i = 0; i < NP; ++i) {
+              const double y = __dadd_rn(__dmul_rn(cw, tau[i]), cp);
+              double s = sin_rf_fast(A.mt, y);
+              if (__builtin_expect(!(fabs(y) < 65536.0), 0)) s = sin_rf_slow(y);
+              del[i] = fma(ca, s, del[i]);
+            }
+          }
         }
 #pragma unroll
         for (int i = 0; i < NP; ++i) {
@@ -275,14 +273,15 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
 #pragma unroll
       for (int q = 0; q < NPAIR; ++q)
         if (live[2 * q]) {
-          const uint32_t pq = p + q * kPassThreads;
-          if (MAP) T[pq] = make_double2(tau[2 * q], tau[2 * q + 1]);
-          D[pq] = make_double2(del[2 * q], del[2 * q + 1]);
+          if (MAP) T[q * kPassThreads] = make_double2(tau[2 * q], tau[2 * q + 1]);
+          *MBT_D(T + q * kPassThreads) = make_double2(del[2 * q], del[2 * q + 1]);
         }
 #pragma unroll
       for (int q = 0; q < NPAIR; ++q) { t2[q] = t2n[q]; d2[q] = d2n[q]; }
       p = pn;
+      T += STRIDE;
     }
+#undef MBT_D
 
     // S7: warp shuffles, then one atomic per CTA and bunch
 #pragma unroll
