@@ -141,7 +141,7 @@ pass_fn select_flush(int gather) {
 }
 
 int enqueue_turn(mbt_handle *h) {
-  h->fn_map<<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
+  h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
   k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
   return 0;
 }
@@ -161,7 +161,7 @@ int build_graph(mbt_handle *h, int turns, cudaGraphExec_t *out) {
 int flush(mbt_handle *h) {
   if (!h->dirty) return 0;
   CU(cudaSetDevice(h->device));
-  h->fn_flush<<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
+  h->fn_flush<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
   WakeArgs wa = h->wargs;
   wa.mode = 1;
   k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(wa);
@@ -318,7 +318,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   A.drift = rg.alpha_c * rg.T0_s;
   A.nb = nb;
   A.gather = wk.gather_order;
-  A.tau_lo = wk.tau_lo_s;
+  A.tau_lo = (wk.tau_lo_s == 0.0) ? -0.0 : wk.tau_lo_s;  // see in_window()
   A.invDelta = (double)nb / (wk.tau_hi_s - wk.tau_lo_s);
   A.nb_d = (double)nb;
   A.invE0 = 1.0 / E0;
@@ -440,17 +440,23 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   const bool rad_on = p->rad.enable != 0;
   h->fn_map = h->npair == 2 ? select_map<2>(rad_on, wk.gather_order, p->n_cav) : select_map<1>(rad_on, wk.gather_order, p->n_cav);
   h->fn_flush = h->npair == 2 ? select_flush<2>(wk.gather_order) : select_flush<1>(wk.gather_order);
-  h->smem_pass = pass_smem_bytes(nb);
+  h->smem_pass = pass_smem_bytes(nb, h->npair);
   h->smem_wake = (size_t)nb * 2 * sizeof(double);
   CUH(cudaFuncSetAttribute((const void *)h->fn_map, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
   CUH(cudaFuncSetAttribute((const void *)h->fn_flush, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
   CUH(cudaFuncSetAttribute(k_wake, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_wake));
-  int occ = 0;
-  CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)h->fn_map, kPassThreads, h->smem_pass));
-  if (occ < 1) occ = 1;
-  const int64_t max_cta = (int64_t)prop.multiProcessorCount * occ;
-  const int64_t need = (A.total_pairs + (int64_t)kPassThreads * h->npair - 1) / ((int64_t)kPassThreads * h->npair);
-  h->grid_pass = (int)(need < max_cta ? need : max_cta);
+  // tiles: ~16 iterations per CTA; fewer when the whole grid would not fill two waves of the device
+  {
+    int occ = 0;
+    CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)h->fn_map, kPassThreads, h->smem_pass));
+    if (occ < 1) occ = 1;
+    const int64_t stride = (int64_t)kPassThreads * h->npair, ppb = h->ld / 2;
+    int64_t iters = 16;
+    if (const char *e = getenv("MBT_TILE_ITERS")) iters = atoi(e) > 0 ? atoi(e) : 16;  // measurement knob
+    while (iters > 1 && (int64_t)M * ((ppb + iters * stride - 1) / (iters * stride)) < 2ll * prop.multiProcessorCount * occ) iters /= 2;
+    A.tile_pairs = (uint32_t)(iters * stride);
+    h->grid_pass = (int)((ppb + A.tile_pairs - 1) / A.tile_pairs);
+  }
 
   // ---- initial distribution (D20) on the device
   {
@@ -510,7 +516,7 @@ int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, dou
   CU(cudaEventRecord(h->ev0, h->stream));
   for (int64_t t = 0; t < n_turns; ++t) {
     CU(cudaEventRecord(ev[3 * t], h->stream));
-    h->fn_map<<<h->grid_pass, kPassThreads, h->smem_pass, h->stream>>>(h->args);
+    h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
     CU(cudaEventRecord(ev[3 * t + 1], h->stream));
     k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
     CU(cudaEventRecord(ev[3 * t + 2], h->stream));

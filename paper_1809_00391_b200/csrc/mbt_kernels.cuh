@@ -13,6 +13,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "mbt_math.cuh"
 
 namespace mbt {
@@ -51,6 +53,7 @@ struct Args {
   uint32_t ppb;      // pairs per bunch = ld / 2
   int32_t M;
   int64_t total_pairs;
+  uint32_t tile_pairs;  // pairs per CTA of the pass (a multiple of kPassThreads * NPAIR)
   // S1
   int32_t n_cav;
   double cav_amp[kMaxCav];  // V_c / E0
@@ -84,10 +87,62 @@ struct Args {
 struct WakeCell {
   double mid, dif;  // v(f) = mid + f * dif, f in [-1/2, 1/2] around the cell boundary (linear gather)
 };
-__host__ __device__ inline size_t pass_smem_bytes(int nb) {
-  return (size_t)(nb + 2) * sizeof(WakeCell) + (size_t)nb * sizeof(double) + (size_t)nb * sizeof(uint32_t) +
-         128 * sizeof(LogTabEntry) + 16;
+// Particle staging: a CTA owns kStages shared-memory stages of kPassThreads*NPAIR pairs (tau block, then delta
+// block), filled by cp.async.bulk (TMA, global -> shared) kStages-1 iterations ahead of their use.  full[stage]
+// completes when both blocks have landed (expect_tx); empty[stage] completes when all warps have read the stage
+// (one arrival per warp).  Thread 0 is the producer.  Bytes in flight are bounded by shared memory, not registers.
+#ifndef MBT_STAGES
+#define MBT_STAGES 4
+#endif
+constexpr int kStages = MBT_STAGES;
+__host__ __device__ inline size_t pass_stage_bytes(int npair) {
+  return (size_t)kStages * 2 * kPassThreads * npair * 16;
 }
+__host__ __device__ inline size_t pass_smem_bytes(int nb, int npair) {
+  return pass_stage_bytes(npair) + (size_t)(nb + 2) * sizeof(WakeCell) + (size_t)nb * sizeof(double) +
+         (size_t)(nb + 1) * sizeof(uint32_t) + 128 * sizeof(LogTabEntry) + 16;
+}
+
+// ---- mbarrier / bulk-copy primitives (PTX; SASS: SYNCS / UBLKCP)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ double2 lds_double2(uint32_t addr) {  // volatile: the stage is rewritten by the async proxy
+  double2 v;
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "MBT_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra MBT_DONE;\n"
+      "bra MBT_WAIT;\n"
+      "MBT_DONE:\n"
+      "}" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+
+// 0 <= t < nb decided on the high word of t: nb < 2^21 is an integer, so the low word of (double)nb is zero and
+// t >= nb  <=>  hi(t) >= hi(nb) for t >= +0; a negative t (sign bit) or a NaN compares above hi(nb) as unsigned.
+// t = -0.0 cannot occur: the host stores tau_lo = 0 as -0.0, so that (-0.0) - tau_lo = +0.0 (in the window, bin 0,
+// as the oracle's t >= 0 decides) and every other difference is unchanged.
+__device__ __forceinline__ bool in_window(double t, uint32_t hi_nb) { return (uint32_t)__double2hiint(t) < hi_nb; }
 
 // ------------------------------------------------------------------ fused particle pass
 // MAP = true : S0 S7 | S1 S2 S3 | S4      (a tracked turn)
@@ -101,35 +156,67 @@ __host__ __device__ inline size_t pass_smem_bytes(int nb) {
 // dif = V[kk]-V[kk-1], with V[-1] := V[0] and V[nb] := V[nb-1] (constant outer half bins).  Cell nb+1 is zero and
 // serves every particle outside the window (no kick, D11), which keeps the step branch-free.
 template <bool MAP, bool RAD, int GATHER, int NCAV, int NPAIR>
-__global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const __grid_constant__ Args A) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  WakeCell *sW = reinterpret_cast<WakeCell *>(smem_raw);                        // [nb+2]
+#ifndef MBT_MINB1
+#define MBT_MINB1 3
+#endif
+#ifndef MBT_MINB2
+#define MBT_MINB2 2
+#endif
+__global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? MBT_MINB1 : MBT_MINB2) k_pass(const __grid_constant__ Args A) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int NP = 2 * NPAIR;                       // particles per thread and iteration
+  constexpr uint32_t STRIDE = kPassThreads * NPAIR;   // pairs per CTA and iteration (one stage)
+  constexpr uint32_t STAGE_BYTES = 2 * STRIDE * 16;   // tau block + delta block
+  constexpr int NWARP = kPassThreads / 32;
+  unsigned char *sStage = smem_raw;                   // [stage]{double2 tau[STRIDE]; double2 delta[STRIDE]}
+  WakeCell *sW = reinterpret_cast<WakeCell *>(smem_raw + kStages * STAGE_BYTES);  // [nb+2]
   double *sV = reinterpret_cast<double *>(sW + (A.nb + 2));                     // [nb]
   LogTabEntry *sL = reinterpret_cast<LogTabEntry *>(sV + A.nb);                 // [128]
-  uint32_t *sH = reinterpret_cast<uint32_t *>(sL + 128);                        // [nb]
-  __shared__ double s_red[kPassThreads / 32][4];
-  __shared__ uint32_t s_nout[kPassThreads / 32];
-  constexpr int NP = 2 * NPAIR;               // particles per thread and iteration
-  constexpr uint32_t STRIDE = kPassThreads * NPAIR;  // pairs per CTA and iteration
+  uint32_t *sH = reinterpret_cast<uint32_t *>(sL + 128);                        // [nb + 1], bin nb is a sink
+  __shared__ double s_red[NWARP][4];
+  __shared__ uint32_t s_nout[NWARP];
+  __shared__ __align__(8) uint64_t s_bar[2 * kStages];  // full[kStages], then empty[kStages]
 
   const int tid = threadIdx.x;
+  const int lane = tid & 31;
   const uint32_t n = A.ctrl->turn + 1u;  // the turn this pass tracks (Philox counter word, D24)
   const bool have_kick = A.ctrl->kick_pending != 0u;
   const int nb = A.nb;
+  const uint32_t hi_nb = (uint32_t)__double2hiint(A.nb_d);
+  if (tid < kStages) {
+    mbar_init(smem_u32(&s_bar[tid]), 1u);
+    mbar_init(smem_u32(&s_bar[kStages + tid]), (uint32_t)NWARP);
+  }
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   if (MAP && RAD)
     for (int i = tid; i < 128; i += kPassThreads) sL[i] = A.logtab[i];
+  __syncthreads();
+  const uint32_t stage0 = smem_u32(sStage), full0 = smem_u32(&s_bar[0]), empty0 = full0 + kStages * 8u;
 
-  // contiguous range of pairs for this CTA, in multiples of the CTA's stride
-  int64_t per = (A.total_pairs + gridDim.x - 1) / gridDim.x;
-  per = (per + STRIDE - 1) / STRIDE * STRIDE;
-  int64_t begin = (int64_t)blockIdx.x * per;
-  const int64_t end = begin + per < A.total_pairs ? begin + per : A.total_pairs;
+  // one CTA = one tile of one bunch: pairs [p0, p1) of bunch b (grid = tiles per bunch x bunches).  Many small
+  // CTAs in address order, placed by the hardware scheduler, stream HBM measurably faster than one resident wave of
+  // persistent CTAs with a fixed range each (6.7 vs 5.5 TB/s for a bare read-modify-write of this store).
+  {
+    const int b = (int)blockIdx.y;
+    const uint32_t p0 = blockIdx.x * A.tile_pairs;
+    const uint32_t p1 = (A.ppb - p0 < A.tile_pairs) ? A.ppb : p0 + A.tile_pairs;
 
-  while (begin < end) {
-    const int b = (int)(begin / A.ppb);
-    const uint32_t p0 = (uint32_t)(begin - (int64_t)b * A.ppb);
-    const int64_t left = end - begin;
-    const uint32_t p1 = (left < (int64_t)(A.ppb - p0)) ? (uint32_t)(p0 + left) : A.ppb;
+    // chunk k of the tile = pairs [p0 + k STRIDE, + STRIDE) clipped to p1; it lives in stage k % kStages
+    const uint32_t n_it = (p1 - p0 + STRIDE - 1u) / STRIDE;
+    const double2 *gT = reinterpret_cast<const double2 *>(A.tau + (size_t)b * A.ld);
+    const double2 *gD = reinterpret_cast<const double2 *>(A.delta + (size_t)b * A.ld);
+    auto issue = [&](uint32_t k) {  // producer thread: fill the stage of chunk k once every warp has released it
+      const uint32_t c = k, stage = c % kStages;
+      if (c >= (uint32_t)kStages) mbar_wait(empty0 + stage * 8u, ((c / kStages) + 1u) & 1u);
+      const uint32_t pc = p0 + k * STRIDE;
+      const uint32_t bytes = ((p1 - pc < STRIDE) ? p1 - pc : STRIDE) * 16u;
+      const uint32_t bar = full0 + stage * 8u, dst = stage0 + stage * STAGE_BYTES;
+      mbar_expect_tx(bar, 2u * bytes);
+      bulk_g2s(dst, gT + pc, bytes, bar);
+      bulk_g2s(dst + STRIDE * 16u, gD + pc, bytes, bar);
+    };
+    if (tid == 0)
+      for (uint32_t k = 0; k + 1u < (uint32_t)kStages && k < n_it; ++k) issue(k);
 
     // stage the wake of bunch b: V = V_SR + sum_r Re[F_r[j] P[b][r]] (S6 expansion), then the gather cells
     for (int j = tid; j < nb; j += kPassThreads) {
@@ -168,18 +255,43 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
     double2 *T = reinterpret_cast<double2 *>(A.tau + (size_t)b * A.ld) + p;
     const ptrdiff_t d_off = reinterpret_cast<const char *>(A.delta) - reinterpret_cast<const char *>(A.tau);
 #define MBT_D(ptr) reinterpret_cast<double2 *>(reinterpret_cast<char *>(ptr) + d_off)
-    double2 t2[NPAIR], d2[NPAIR], t2n[NPAIR], d2n[NPAIR];
+    // chunk this thread will issue next (lane 0 of warp w issues the chunks c = w mod NWARP, c >= kStages - 1:
+    // the producer role rotates over the warps, so no warp carries it on its critical path); ~0: none
+    uint32_t next_issue = ~0u;
+    if (lane == 0) {
+      uint32_t c = (uint32_t)(tid >> 5);
+      while (c + 1u < (uint32_t)kStages) c += NWARP;
+      if (c < n_it) next_issue = c;
+    }
+    // a full tile has no ragged end and no padding slot: the `live` logic drops out of its loop
+    const bool full_tile = (p1 - p0 == n_it * STRIDE) && !((A.Np & 1u) && p1 == A.ppb);
+    auto run = [&](auto full_tag) {
+    constexpr bool FULL = decltype(full_tag)::value;
+    // running shared-memory addresses of the stage in use: full barrier (empty barrier kStages * 8 bytes above it)
+    // and this thread's slot; they wrap every kStages iterations, where the mbarrier parity flips
+    uint32_t bar_a = full0, slot_a = stage0 + (uint32_t)tid * 16u, parity = 0u, until_wrap = kStages;
+    for (uint32_t k = 0; k < n_it; ++k) {
+      mbar_wait(bar_a, parity);
+      double2 t2[NPAIR], d2[NPAIR];
 #pragma unroll
-    for (int q = 0; q < NPAIR; ++q)
-      if (p + q * kPassThreads < p1) { t2[q] = T[q * kPassThreads]; d2[q] = *MBT_D(T + q * kPassThreads); }
-    while (p < p1) {
-      const uint32_t pn = p + STRIDE;
-#pragma unroll
-      for (int q = 0; q < NPAIR; ++q)  // prefetch the next iteration while this one is computed
-        if (pn + q * kPassThreads < p1) {
-          t2n[q] = T[STRIDE + q * kPassThreads];
-          d2n[q] = *MBT_D(T + STRIDE + q * kPassThreads);
-        }
+      for (int q = 0; q < NPAIR; ++q) {
+        t2[q] = lds_double2(slot_a + q * kPassThreads * 16u);
+        d2[q] = lds_double2(slot_a + (STRIDE + q * kPassThreads) * 16u);
+      }
+      __syncwarp();  // every lane of the warp has read the stage
+      if (lane == 0) mbar_arrive(bar_a + kStages * 8u);
+      if (k + (uint32_t)kStages - 1u == next_issue) {
+        issue(next_issue);
+        next_issue = (next_issue + NWARP < n_it) ? next_issue + NWARP : ~0u;
+      }
+      bar_a += 8u;
+      slot_a += STAGE_BYTES;
+      if (--until_wrap == 0u) {
+        until_wrap = kStages;
+        bar_a = full0;
+        slot_a -= kStages * STAGE_BYTES;
+        parity ^= 1u;
+      }
 
       double tau[NP], del[NP], z[NP];
       bool live[NP];
@@ -188,8 +300,8 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
         const uint32_t pq = p + q * kPassThreads;
         tau[2 * q] = t2[q].x; tau[2 * q + 1] = t2[q].y;
         del[2 * q] = d2[q].x; del[2 * q + 1] = d2[q].y;
-        live[2 * q] = pq < p1;                              // a whole pair may be past the end when NPAIR = 2
-        live[2 * q + 1] = live[2 * q] && (2u * pq + 1u < A.Np);  // odd slot of the last pair is padding if N_p is odd
+        live[2 * q] = FULL || pq < p1;                      // past the end of the tile: stale stage contents, ignored
+        live[2 * q + 1] = FULL || (live[2 * q] && (2u * pq + 1u < A.Np));  // odd slot of the last pair is padding if N_p is odd
         z[2 * q] = z[2 * q + 1] = 0.0;
         if (MAP && RAD) {
           // one Philox call and one Box-Muller serve both particles of the 128-bit load (D8):
@@ -201,12 +313,13 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
       }
       // S0: kick of the previous turn's wake.  t exactly as the binning computed it (one subtraction, one
       // multiplication, no contraction), so the in-window decision is the one that deposited the particle.
+      // In-window test 0 <= t < nb on the high word of t alone (in_window()): an integer compare, off the fp64 pipe.
       double t[NP];
       bool in[NP];
 #pragma unroll
       for (int i = 0; i < NP; ++i) {
         t[i] = __dmul_rn(__dsub_rn(tau[i], A.tau_lo), A.invDelta);
-        in[i] = live[i] && (t[i] >= 0.0) && (t[i] < A.nb_d);
+        in[i] = live[i] && in_window(t[i], hi_nb);
         int kk;
         double f;
         if (GATHER == 1) {
@@ -225,26 +338,45 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
       // S7: moments of the state after the kick
 #pragma unroll
       for (int i = 0; i < NP; ++i)
+#ifndef MBT_EXP_NOMOM
         if (live[i]) {
           st += tau[i];
           sd += del[i];
           stt = fma(tau[i], tau[i], stt);
           sdd = fma(del[i], del[i], sdd);
         }
+#else
+        ;
+#endif
       if (MAP) {
-        // S1: RF cavities.  The phase is formed as the oracle forms it (product rounded, then the sum).  A particle
-        // long lost from the bucket (|y| >= 2^16, or not finite) takes the library sine in a cold out-of-line call;
-        // every index below is a compile-time constant, so tau[] / del[] stay in registers (no local memory).
+        // S1: RF cavities.  The phase is formed as the oracle forms it (product rounded, then the sum).  All fast sines
+        // of the iteration are evaluated first, in ONE basic block together with the Box-Muller above, so that the
+        // independent polynomial chains interleave (DFMA latency is 8 cycles); a particle long lost from the bucket
+        // (|y| >= 2^16, or not finite) is then patched with the library sine in a single cold branch.
         if (NCAV > 0) {
+          double sn[NCAV > 0 ? NCAV : 1][NP];
+          uint32_t worst = 0u;
 #pragma unroll
           for (int c = 0; c < NCAV; ++c)
 #pragma unroll
             for (int i = 0; i < NP; ++i) {
               const double y = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
-              double s = sin_rf_fast(A.mt, y);
-              if (__builtin_expect(!(fabs(y) < 65536.0), 0)) s = sin_rf_slow(y);
-              del[i] = fma(A.cav_amp[c], s, del[i]);
+              sn[c][i] = sin_rf_fast(A.mt, y);
+              worst = max(worst, (uint32_t)__double2hiint(y) & 0x7FFFFFFFu);
             }
+          if (__builtin_expect(worst >= 0x40F00000u, 0)) {  // some |y| >= 65536, inf or NaN
+#pragma unroll
+            for (int c = 0; c < NCAV; ++c)
+#pragma unroll
+              for (int i = 0; i < NP; ++i) {
+                const double y = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
+                if (!(fabs(y) < 65536.0)) sn[c][i] = sin_rf_slow(y);
+              }
+          }
+#pragma unroll
+          for (int c = 0; c < NCAV; ++c)
+#pragma unroll
+            for (int i = 0; i < NP; ++i) del[i] = fma(A.cav_amp[c], sn[c][i], del[i]);
         } else {
 #pragma unroll 1
           for (int c = 0; c < A.n_cav; ++c) {
@@ -252,9 +384,9 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
 #pragma unroll
             for (int i = 0; i < NP; ++i) {
               const double y = __dadd_rn(__dmul_rn(cw, tau[i]), cp);
-              double s = sin_rf_fast(A.mt, y);
-              if (__builtin_expect(!(fabs(y) < 65536.0), 0)) s = sin_rf_slow(y);
-              del[i] = fma(ca, s, del[i]);
+              double sv = sin_rf_fast(A.mt, y);
+              if (__builtin_expect(!(fabs(y) < 65536.0), 0)) sv = sin_rf_slow(y);
+              del[i] = fma(ca, sv, del[i]);
             }
           }
         }
@@ -264,23 +396,23 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
           if (RAD) del[i] = fma(del[i], A.one_minus_DE, z[i]);  // S2 (z already scaled by sigma_delta sqrt(2 D_E))
           tau[i] = fma(A.drift, del[i], tau[i]);                // S3
           t[i] = __dmul_rn(__dsub_rn(tau[i], A.tau_lo), A.invDelta);  // S4
-          in[i] = live[i] && (t[i] >= 0.0) && (t[i] < A.nb_d);
+          in[i] = live[i] && in_window(t[i], hi_nb);
         }
       }
+      // S4: deposit.  Branch-free: a particle outside the window (or a padding slot) counts into the spare bin nb.
 #pragma unroll
-      for (int i = 0; i < NP; ++i)
-        if (in[i]) atomicAdd(&sH[__double2int_rd(t[i])], 1u);
+      for (int i = 0; i < NP; ++i) atomicAdd(&sH[in[i] ? __double2int_rd(t[i]) : nb], 1u);
 #pragma unroll
       for (int q = 0; q < NPAIR; ++q)
         if (live[2 * q]) {
           if (MAP) T[q * kPassThreads] = make_double2(tau[2 * q], tau[2 * q + 1]);
           *MBT_D(T + q * kPassThreads) = make_double2(del[2 * q], del[2 * q + 1]);
         }
-#pragma unroll
-      for (int q = 0; q < NPAIR; ++q) { t2[q] = t2n[q]; d2[q] = d2n[q]; }
-      p = pn;
+      p += STRIDE;
       T += STRIDE;
     }
+    };  // run
+    if (full_tile) run(std::true_type{}); else run(std::false_type{});
 #undef MBT_D
 
     // S7: warp shuffles, then one atomic per CTA and bunch
@@ -313,8 +445,6 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
       const uint32_t c = sH[j];
       if (c) atomicAdd(&A.hist[(size_t)b * nb + j], c);
     }
-    __syncthreads();
-    begin += (int64_t)(p1 - p0);
   }
 }
 
@@ -344,6 +474,12 @@ struct WakeArgs {
   Ctrl *ctrl;
 };
 
+// L2 load of a complex number written earlier in this kernel by another CTA (never through a stale L1 line)
+__device__ __forceinline__ cplx __ldcg_cplx(const cplx *p) {
+  const double2 v = __ldcg(reinterpret_cast<const double2 *>(p));
+  return cplx{v.x, v.y};
+}
+
 // affine map x -> g x + c over the complex numbers; (first o second)(x) = second(first(x))
 struct Affine {
   cplx g, c;
@@ -358,7 +494,6 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   double *sw = smem_d + A.nb;  // [nb] wake table
   __shared__ double s_red[kWakeThreads / 32][2];
   __shared__ bool s_last;
-  __shared__ Affine s_scan[kWakeThreads];
 
   const int tid = threadIdx.x;
   const int b = blockIdx.x;
@@ -446,66 +581,59 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   __threadfence();
 
   // S6: P_0 = G_n (history seed), P_{j+1} = (P_j + a_j) g_j -- an inclusive scan of affine maps over the fill
-  // pattern; every factor is exp(lambda * positive time), |g| < 1.
+  // pattern; every factor is exp(lambda * positive time), |g| < 1.  One WARP per resonator, all resonators at once,
+  // shuffles only (no block barrier inside): this tail runs alone on the device, so its latency is the turn's.
   const int M = A.M, R = A.R, K = A.K;
-  const int ipt = (M + kWakeThreads - 1) / kWakeThreads;  // consecutive bunches per thread
-  for (int r = 0; r < R; ++r) {
-    // G_n = sum_{k=1..min(K,n-1)} A_{n-k} exp(lambda (k T0 - span))     (direct K-term sum)
+  const int lane = tid & 31;
+  const int run = (M + 31) / 32;  // consecutive bunches per lane
+  for (int r = tid >> 5; r < R; r += kWakeThreads / 32) {
+    // G_n = sum_{k=1..min(K,n-1)} A_{n-k} exp(lambda (k T0 - span)): lanes take k = lane+1, lane+33, ...
     cplx G{0.0, 0.0};
-    for (int k = 1; k <= K && (int64_t)n - k >= 1; ++k)
-      G = cfma(A.ring_A[(size_t)((n - (uint32_t)k) % (uint32_t)(K + 1)) * R + r], A.g_hist[(size_t)(k - 1) * R + r], G);
-    // thread-local composite of its run of bunches, and this turn's own aggregate
-    const int j_lo = tid * ipt, j_hi = min(j_lo + ipt, M);
+    for (int k = lane + 1; k <= K && (int64_t)n - k >= 1; k += 32)
+      G = cfma(__ldcg_cplx(&A.ring_A[(size_t)((n - (uint32_t)k) % (uint32_t)(K + 1)) * R + r]), A.g_hist[(size_t)(k - 1) * R + r], G);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      G.re += __shfl_xor_sync(0xffffffffu, G.re, o);
+      G.im += __shfl_xor_sync(0xffffffffu, G.im, o);
+    }
+    // lane-local composite of its run of bunches, and this turn's own aggregate
+    const int j_lo = lane * run, j_hi = min(j_lo + run, M);
     Affine loc{cplx{1.0, 0.0}, cplx{0.0, 0.0}};
     cplx own{0.0, 0.0};
     for (int j = j_lo; j < j_hi; ++j) {
-      const cplx a = A.a_cur[(size_t)j * R + r];
+      const cplx a = __ldcg_cplx(&A.a_cur[(size_t)j * R + r]);
       own = cfma(a, A.g_tail[(size_t)j * R + r], own);
       if (j + 1 < M) {
         const cplx g = A.g_step[(size_t)j * R + r];
         loc = compose(loc, Affine{g, cmul(a, g)});
       }
     }
-    // Hillis-Steele inclusive scan of the thread composites
-    s_scan[tid] = loc;
-    __syncthreads();
-    for (int o = 1; o < kWakeThreads; o <<= 1) {
-      Affine v = s_scan[tid];
-      if (tid >= o) v = compose(s_scan[tid - o], v);
-      __syncthreads();
-      s_scan[tid] = v;
-      __syncthreads();
+    // inclusive warp scan of the lane composites (Kogge-Stone on shuffles), then the exclusive prefix applied to G
+    Affine inc = loc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      Affine up;
+      up.g.re = __shfl_up_sync(0xffffffffu, inc.g.re, o); up.g.im = __shfl_up_sync(0xffffffffu, inc.g.im, o);
+      up.c.re = __shfl_up_sync(0xffffffffu, inc.c.re, o); up.c.im = __shfl_up_sync(0xffffffffu, inc.c.im, o);
+      if (lane >= o) inc = compose(up, inc);
     }
-    // exclusive prefix of this thread, applied to G, then walk the run
-    cplx Pj = G;
-    if (tid > 0) {
-      const Affine pre = s_scan[tid - 1];
-      Pj = cfma(pre.g, G, pre.c);
-    }
+    Affine pre;
+    pre.g.re = __shfl_up_sync(0xffffffffu, inc.g.re, 1); pre.g.im = __shfl_up_sync(0xffffffffu, inc.g.im, 1);
+    pre.c.re = __shfl_up_sync(0xffffffffu, inc.c.re, 1); pre.c.im = __shfl_up_sync(0xffffffffu, inc.c.im, 1);
+    cplx Pj = (lane > 0) ? cfma(pre.g, G, pre.c) : G;
     for (int j = j_lo; j < j_hi; ++j) {
       A.P[(size_t)j * R + r] = Pj;
-      if (j + 1 < M) {
-        const cplx g = A.g_step[(size_t)j * R + r];
-        Pj = cmul(cadd(Pj, A.a_cur[(size_t)j * R + r]), g);
-      }
+      if (j + 1 < M) Pj = cmul(cadd(Pj, __ldcg_cplx(&A.a_cur[(size_t)j * R + r])), A.g_step[(size_t)j * R + r]);
     }
-    // A_n = sum_j a_j exp(lambda (s_{M-1}-s_j) T_rf): block reduction
-    double ore = own.re, oim = own.im;
+    // A_n = sum_j a_j exp(lambda (s_{M-1}-s_j) T_rf)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-      ore += __shfl_down_sync(0xffffffffu, ore, o);
-      oim += __shfl_down_sync(0xffffffffu, oim, o);
+      own.re += __shfl_xor_sync(0xffffffffu, own.re, o);
+      own.im += __shfl_xor_sync(0xffffffffu, own.im, o);
     }
-    __syncthreads();
-    if ((tid & 31) == 0) { s_red[tid >> 5][0] = ore; s_red[tid >> 5][1] = oim; }
-    __syncthreads();
-    if (tid == 0) {
-      cplx a{0.0, 0.0};
-      for (int w = 0; w < kWakeThreads / 32; ++w) { a.re += s_red[w][0]; a.im += s_red[w][1]; }
-      A.ring_A[(size_t)(n % (uint32_t)(K + 1)) * R + r] = a;
-    }
-    __syncthreads();
+    if (lane == 0) A.ring_A[(size_t)(n % (uint32_t)(K + 1)) * R + r] = own;
   }
+  __syncthreads();
   if (tid == 0) {
     A.ctrl->ticket = 0u;
     A.ctrl->kick_pending = 1u;
