@@ -75,6 +75,9 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 /* the two uniforms and the Box-Muller pair of one Philox call */
 void orc_normal_pair(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
                      double *u1, double *u2, double *z_c, double *z_s);
+/* Excitation stream (reading D8): one Philox block -> four normals; u[4] (may be NULL) and z[4]:
+ * (z[0], z[1]) = Box-Muller of the 32-bit uniforms of words (x0, x1), (z[2], z[3]) of (x2, x3). */
+void orc_normal_quad(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, double *u, double *z);
 double orc_resonator_wake(double Rs_ohm, double fr_Hz, double Q, double t_s);
 void orc_sr_convolve(int32_t n_bins, const double *w, const double *q, double *V);
 /* one application of the single-particle map (steps 1-3) without wake, z given */

@@ -94,6 +94,8 @@ def lib():
         L.orc_philox4x32_10.restype = None
         L.orc_normal_pair.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, dp, dp, dp, dp]
         L.orc_normal_pair.restype = None
+        L.orc_normal_quad.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, dp, dp]
+        L.orc_normal_quad.restype = None
         L.orc_resonator_wake.argtypes = [C.c_double] * 4
         L.orc_resonator_wake.restype = C.c_double
         L.orc_sr_convolve.argtypes = [C.c_int32, dp, dp, dp]
@@ -118,6 +120,14 @@ def philox(ctr, key):
     o = (C.c_uint32 * 4)()
     lib().orc_philox4x32_10(c, k, o)
     return [int(x) for x in o]
+
+
+def normal_quad(seed, c0, c1, c2, c3):
+    """Excitation stream: (u[4], z[4]) of one Philox block (reading D8)."""
+    u = (C.c_double * 4)()
+    z = (C.c_double * 4)()
+    lib().orc_normal_quad(seed, c0, c1, c2, c3, u, z)
+    return list(u), list(z)
 
 
 def normal_pair(seed, c0, c1, c2, c3):

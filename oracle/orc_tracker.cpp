@@ -78,8 +78,8 @@ void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// Reading D8: key = (seed mod 2^32, seed >> 32); the two uniforms use the
-// top 52 bits of each 64-bit half, u = (k + 1/2) 2^-52, exactly representable and
+// Reading D8: key = (seed mod 2^32, seed >> 32).  Initial-distribution stream (tag 1): the two
+// uniforms use the top 52 bits of each 64-bit half, u = (k + 1/2) 2^-52, exactly representable and
 // strictly inside (0,1); Box-Muller gives the pair (z_c, z_s).
 void normal_pair(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
                  double *u1o, double *u2o, double *zc, double *zs) {
@@ -97,6 +97,26 @@ void normal_pair(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t 
   *zs = r * std::sin(theta);
   if (u1o) *u1o = u1;
   if (u2o) *u2o = u2;
+}
+
+// Reading D8, excitation stream (tag 0): one Philox block serves FOUR consecutive particles of a bunch.  Each of
+// its 32-bit words gives one uniform u = (x + 1/2) 2^-32 (exactly representable, strictly inside (0,1)); the
+// words (x0, x1) are (u1, u2) of the Box-Muller pair (z[0], z[1]) of particles 4j, 4j+1 and (x2, x3) those of
+// (z[2], z[3]) of particles 4j+2, 4j+3.
+void normal_quad(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, double *uo, double *z) {
+  uint32_t ctr[4] = {c0, c1, c2, c3};
+  uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32)};
+  uint32_t x[4];
+  philox4x32_10(ctr, key, x);
+  for (int h = 0; h < 2; ++h) {
+    double u1 = ((double)x[2 * h] + 0.5) * 0x1p-32;
+    double u2 = ((double)x[2 * h + 1] + 0.5) * 0x1p-32;
+    double r = std::sqrt(-2.0 * std::log(u1));
+    double theta = 2.0 * PI_D * u2;
+    z[2 * h] = r * std::cos(theta);
+    z[2 * h + 1] = r * std::sin(theta);
+    if (uo) { uo[2 * h] = u1; uo[2 * h + 1] = u2; }
+  }
 }
 
 enum { TAG_EXCITATION = 0, TAG_INITIAL = 1 };
@@ -252,16 +272,19 @@ void one_turn(orc_handle *h) {
   const int64_t n = h->turn + 1;
   // 1-3: single-particle map
   for (int b = 0; b < M; ++b)
+  {
+    double zq[4] = {0.0, 0.0, 0.0, 0.0};
     for (int64_t i = 0; i < Np; ++i) {
       size_t p = (size_t)b * Np + i;
       double z = 0.0;
       if (h->rad.enable) {
-        double zc, zs;
-        normal_pair(h->seed, (uint32_t)(i >> 1), (uint32_t)b, (uint32_t)n, TAG_EXCITATION, nullptr, nullptr, &zc, &zs);
-        z = (i & 1) ? zs : zc;
+        // one block per four particles: counter (i >> 2, b, n, tag 0), particle i takes z[i & 3]
+        if ((i & 3) == 0) normal_quad(h->seed, (uint32_t)(i >> 2), (uint32_t)b, (uint32_t)n, TAG_EXCITATION, nullptr, zq);
+        z = zq[i & 3];
       }
       map_one(h, h->tau[p], h->delta[p], z);
     }
+  }
   // 4: bins
   bin_all(h);
   // 5: short-range wake, V_SR[b][j] = sum_{k<=j} w[j-k] q[b][k], q = (Q_b/N_p) hist
@@ -376,6 +399,10 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 void orc_normal_pair(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, double *u1, double *u2,
                      double *z_c, double *z_s) {
   normal_pair(seed, c0, c1, c2, c3, u1, u2, z_c, z_s);
+}
+
+void orc_normal_quad(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, double *u, double *z) {
+  normal_quad(seed, c0, c1, c2, c3, u, z);
 }
 
 double orc_resonator_wake(double Rs, double fr, double Q, double t) {

@@ -167,8 +167,8 @@ def test_excitation_stream_layout(orc):
     o2 = orc.Oracle(cfg)
     for b in range(2):
         for i in range(5):
-            _, _, zc, zs = orc.normal_pair(cfg["seed"], i >> 1, b, 1, 0)
-            t, d = o2.map_one(tau0[b, i], del0[b, i], zs if i & 1 else zc)
+            _, z = orc.normal_quad(cfg["seed"], i >> 2, b, 1, 0)   # one block per four particles (D8)
+            t, d = o2.map_one(tau0[b, i], del0[b, i], z[i & 3])
             assert t == tau1[b, i] and d == del1[b, i]
     # initial distribution: counter (i, b, 0, 1), tau = sigma_tau0 z_c, delta = sigma_delta0 z_s
     _, _, zc, zs = orc.normal_pair(cfg["seed"], 3, 1, 0, 1)

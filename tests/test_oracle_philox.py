@@ -63,26 +63,48 @@ def test_uniforms_are_top_52_bits_plus_half(orc):
         assert abs(float(r * np.sin(th)) - zs) < 1e-14
 
 
+def test_excitation_uniforms_are_32_bit_words_plus_half(orc):
+    # excitation stream (reading D8): u_k = (x_k + 1/2) 2^-32 for each word of the block, exact in fp64, in (0,1);
+    # (z0, z1) is the Box-Muller pair of (u0, u1), (z2, z3) that of (u2, u3)
+    from fractions import Fraction
+    for seed, c in [(1, (0, 0, 1, 0)), (0xDEADBEEF12345678, (7, 3, 99, 0)), (2**64 - 1, (2**32 - 1,) * 4)]:
+        x = orc.philox(list(c), [seed & 0xFFFFFFFF, seed >> 32])
+        u, z = orc.normal_quad(seed, *c)
+        for k in range(4):
+            assert Fraction(u[k]) == Fraction(2 * x[k] + 1, 2**33)
+            assert 0.0 < u[k] < 1.0
+        for h in range(2):
+            r = np.sqrt(-2.0 * np.log(np.longdouble(u[2 * h])))
+            th = 2.0 * np.pi * np.longdouble(u[2 * h + 1])
+            assert abs(float(r * np.cos(th)) - z[2 * h]) < 1e-14
+            assert abs(float(r * np.sin(th)) - z[2 * h + 1]) < 1e-14
+
+
 def test_normals_are_standard_normal(orc):
-    n = 200_000
-    z = np.empty(2 * n)
-    for i in range(n):
-        _, _, zc, zs = orc.normal_pair(12345, i, 2, 7, 0)
-        z[2 * i] = zc
-        z[2 * i + 1] = zs
-    assert abs(z.mean()) < 4.0 / np.sqrt(2 * n)
-    assert abs(z.var() - 1.0) < 4.0 * np.sqrt(2.0 / (2 * n))
-    assert abs(stats.kurtosis(z)) < 4.0 * np.sqrt(24.0 / (2 * n))
-    assert abs(stats.skew(z)) < 4.0 * np.sqrt(6.0 / (2 * n))
-    assert stats.kstest(z, "norm").pvalue > 1e-3
-    # the two members of a pair are uncorrelated
-    assert abs(np.corrcoef(z[0::2], z[1::2])[0, 1]) < 4.0 / np.sqrt(n)
+    n = 100_000
+    for draw in ("quad", "pair"):
+        if draw == "quad":   # excitation stream: four normals per block
+            z = np.array([orc.normal_quad(12345, i, 2, 7, 0)[1] for i in range(n // 2)]).ravel()
+        else:                # initial-distribution stream: two normals per block
+            z = np.array([orc.normal_pair(12345, i, 2, 0, 1)[2:] for i in range(n)]).ravel()
+        m = z.size
+        assert abs(z.mean()) < 4.0 / np.sqrt(m)
+        assert abs(z.var() - 1.0) < 4.0 * np.sqrt(2.0 / m)
+        assert abs(stats.kurtosis(z)) < 4.0 * np.sqrt(24.0 / m)
+        assert abs(stats.skew(z)) < 4.0 * np.sqrt(6.0 / m)
+        assert stats.kstest(z, "norm").pvalue > 1e-3
+        # the members of a block are uncorrelated
+        assert abs(np.corrcoef(z[0::2], z[1::2])[0, 1]) < 4.0 / np.sqrt(m / 2)
+        if draw == "quad":
+            assert abs(np.corrcoef(z[0::4], z[2::4])[0, 1]) < 4.0 / np.sqrt(m / 4)
+            assert abs(np.corrcoef(z[1::4], z[3::4])[0, 1]) < 4.0 / np.sqrt(m / 4)
 
 
 def test_streams_differ_by_tag_turn_bunch(orc):
-    base = orc.normal_pair(1, 5, 0, 1, 0)
-    assert orc.normal_pair(1, 5, 0, 1, 1) != base   # tag
-    assert orc.normal_pair(1, 5, 0, 2, 0) != base   # turn
-    assert orc.normal_pair(1, 5, 1, 1, 0) != base   # bunch
-    assert orc.normal_pair(2, 5, 0, 1, 0) != base   # seed
-    assert orc.normal_pair(1 << 32, 5, 0, 1, 0) != orc.normal_pair(0, 5, 0, 1, 0)  # high key word is used
+    for draw in (orc.normal_pair, orc.normal_quad):
+        base = draw(1, 5, 0, 1, 0)
+        assert draw(1, 5, 0, 1, 1) != base   # tag
+        assert draw(1, 5, 0, 2, 0) != base   # turn
+        assert draw(1, 5, 1, 1, 0) != base   # bunch
+        assert draw(2, 5, 0, 1, 0) != base   # seed
+        assert draw(1 << 32, 5, 0, 1, 0) != draw(0, 5, 0, 1, 0)  # high key word is used
