@@ -18,7 +18,7 @@
  * HOST pointer that is copied before the call returns (the caller keeps ownership).
  * Particle coordinates live on the device for the whole run (P:l.39) as two fp64
  * arrays tau[M][ld] and delta[M][ld], ld = mbt_particle_stride(N_p) (N_p rounded up
- * to an even number so that every bunch starts on a 16-byte boundary).
+ * to a multiple of 4 so that every bunch starts on a 32-byte boundary).
  *
  * Every function returns 0 (MBT_OK) or a negative MBT_E* code; the text of the last
  * error of the calling thread is returned by mbt_last_error().  No exception and no
@@ -93,7 +93,7 @@ typedef struct {
   uint64_t seed;                /* Philox key (D8)                                                     */
   int64_t log_capacity_turns;   /* > 0: keep per-turn moments of turns 1..capacity on the device       */
   void *d_tau, *d_delta;        /* optional caller-owned DEVICE buffers (e.g. torch tensors), each
-                                   n_bunches * mbt_particle_stride(n_per_bunch) doubles, 16-byte aligned,
+                                   n_bunches * mbt_particle_stride(n_per_bunch) doubles, 32-byte aligned,
                                    alive until mbt_destroy; both NULL -> the library allocates.  They are
                                    overwritten with the seeded initial distribution.                    */
   void *stream;                 /* cudaStream_t the library enqueues on (e.g. torch's current stream);
@@ -151,8 +151,9 @@ double mbt_last_track_seconds(mbt_handle *h);
 int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, double *wake_seconds);
 /* Run one Philox4x32-10 block on the device (known-answer tests of the device generator). */
 int mbt_philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
-/* Device Box-Muller pair exactly as the excitation step draws it: HOST arrays of n counters (c0,c1,c2,c3)
- * in ctr[n][4]; out[n][2] = (z_c, z_s). */
+/* Device normals exactly as the excitation step draws them (reading D8: one Philox block serves four consecutive
+ * particles): HOST arrays of n counters (c0,c1,c2,c3) in ctr[n][4]; out[n][4]: (out[0], out[1]) = Box-Muller pair of
+ * the 32-bit uniforms of words (x0, x1), (out[2], out[3]) that of (x2, x3). */
 int mbt_normal_selftest(uint64_t seed, int64_t n, const uint32_t *ctr, double *out);
 const char *mbt_last_error(void); /* thread-local, never NULL */
 const char *mbt_version(void);

@@ -107,6 +107,8 @@ struct mbt_handle {
   Args args;
   WakeArgs wargs;
   DevBuf<double> qm, w, Vsr, mom_acc, mom_last, mom_log, scratch_a, scratch_b, scratch_c;
+  DevBuf<WakeCell> cellSR;
+  DevBuf<CellF> cellF;
   DevBuf<cplx> Esrc, F, g_step, g_tail, g_hist, a_cur, ring_a, ring_A, P;
   DevBuf<uint32_t> hist, hist_last;
   DevBuf<unsigned long long> nout_acc;
@@ -186,6 +188,7 @@ void destroy(mbt_handle *h) {
   }
   h->qm.release(); h->w.release(); h->Vsr.release(); h->mom_acc.release(); h->mom_last.release(); h->mom_log.release();
   h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
+  h->cellSR.release(); h->cellF.release();
   h->Esrc.release(); h->F.release(); h->g_step.release(); h->g_tail.release(); h->g_hist.release(); h->a_cur.release();
   h->ring_a.release(); h->ring_A.release(); h->P.release(); h->logtab.release();
   h->hist.release(); h->hist_last.release(); h->nout_acc.release(); h->ctrl.release();
@@ -199,7 +202,7 @@ extern "C" {
 
 const char *mbt_last_error(void) { return g_err.c_str(); }
 const char *mbt_version(void) { return "mbt-b200 0.1 (sm_100a)"; }
-int64_t mbt_particle_stride(int64_t n) { return n < 0 ? -1 : (n + 1) / 2 * 2; }
+int64_t mbt_particle_stride(int64_t n) { return n < 0 ? -1 : (n + 3) / 4 * 4; }
 int64_t mbt_turn(const mbt_handle *h) { return h ? h->turn : -1; }
 double mbt_phi_s(const mbt_handle *h) { return h ? h->phi_s : NAN; }
 int64_t mbt_launch_count(const mbt_handle *h) { return h ? h->launches : -1; }
@@ -234,7 +237,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     return fail(MBT_EINVAL, "radiation: need damping_turns > 0, sigma_delta >= 0");
   if (p->log_capacity_turns < 0) return fail(MBT_EINVAL, "log_capacity_turns < 0");
   if ((p->d_tau == nullptr) != (p->d_delta == nullptr)) return fail(MBT_EINVAL, "give both d_tau and d_delta or neither");
-  if (p->d_tau && (((uintptr_t)p->d_tau | (uintptr_t)p->d_delta) & 15u)) return fail(MBT_EINVAL, "d_tau / d_delta must be 16-byte aligned");
+  if (p->d_tau && (((uintptr_t)p->d_tau | (uintptr_t)p->d_delta) & 31u)) return fail(MBT_EINVAL, "d_tau / d_delta must be 32-byte aligned");
   for (int c = 1; c < p->n_cav; ++c)
     if (std::isnan(p->cav[c].phase_rad)) return fail(MBT_EINVAL, "only cav[0] may leave its phase open");
   int n_lr = 0;
@@ -392,6 +395,25 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   if (have_sr) CUH(h->w.upload(w));
   CUH(h->Esrc.upload(Esrc));
   CUH(h->F.upload(F));
+  {  // gather cells of the constant tables F_r (same cell definition as k_wake applies to V_SR)
+    std::vector<CellF> cf((size_t)(R ? R : 1) * (nb + 2), CellF{cplx{0, 0}, cplx{0, 0}});
+    for (int r = 0; r < R; ++r)
+      for (int k = 0; k < nb + 2; ++k) {
+        CellF c{cplx{0, 0}, cplx{0, 0}};
+        if (wk.gather_order == 1) {
+          if (k <= nb) {
+            const cplx lo = F[(size_t)r * nb + (k > 0 ? k - 1 : 0)], hi = F[(size_t)r * nb + (k < nb ? k : nb - 1)];
+            c.mid = cplx{0.5 * (lo.re + hi.re), 0.5 * (lo.im + hi.im)};
+            c.dif = cplx{hi.re - lo.re, hi.im - lo.im};
+          }
+        } else if (k < nb) {
+          c.mid = F[(size_t)r * nb + k];
+        }
+        cf[(size_t)r * (nb + 2) + k] = c;
+      }
+    CUH(h->cellF.upload(cf));
+  }
+  CUH(h->cellSR.alloc((size_t)M * (nb + 2)));
   CUH(h->g_step.upload(g_step));
   CUH(h->g_tail.upload(g_tail));
   CUH(h->g_hist.upload(g_hist));
@@ -414,6 +436,8 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   A.Vsr = h->Vsr.p;
   A.P = h->P.p;
   A.F = h->F.p;
+  A.cellSR = h->cellSR.p;
+  A.cellF = h->cellF.p;
   A.hist = h->hist.p;
   A.mom_acc = h->mom_acc.p;
   A.nout_acc = h->nout_acc.p;
@@ -428,6 +452,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   Wa.w = have_sr ? h->w.p : nullptr;
   Wa.Esrc = h->Esrc.p; Wa.g_step = h->g_step.p; Wa.g_tail = h->g_tail.p; Wa.g_hist = h->g_hist.p;
   Wa.hist = h->hist.p; Wa.hist_last = h->hist_last.p; Wa.Vsr = h->Vsr.p;
+  Wa.cellSR = h->cellSR.p; Wa.gather = wk.gather_order;
   Wa.a_cur = h->a_cur.p; Wa.ring_a = h->ring_a.p; Wa.ring_A = h->ring_A.p; Wa.P = h->P.p;
   Wa.mom_acc = h->mom_acc.p; Wa.nout_acc = h->nout_acc.p; Wa.mom_last = h->mom_last.p;
   Wa.mom_log = h->log_cap > 0 ? h->mom_log.p : nullptr;
@@ -435,13 +460,15 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   Wa.ctrl = h->ctrl.p;
 
   // ---- launch shapes: one resident wave of CTAs, each owning a contiguous run of pairs
-  h->npair = kDefaultNPair;
+  // two pairs per thread (twice the independent arithmetic per warp, 2 CTAs/SM) pay off except for small
+  // two-cavity workloads, where the four sine chains per thread cost more registers than they hide latency
+  h->npair = kDefaultNPair ? kDefaultNPair : ((p->n_cav == 1 || (int64_t)M * h->Np >= 10000000ll) ? 2 : 1);
   if (const char *e = getenv("MBT_NPAIR")) h->npair = (atoi(e) == 2) ? 2 : 1;  // measurement knob
   const bool rad_on = p->rad.enable != 0;
   h->fn_map = h->npair == 2 ? select_map<2>(rad_on, wk.gather_order, p->n_cav) : select_map<1>(rad_on, wk.gather_order, p->n_cav);
   h->fn_flush = h->npair == 2 ? select_flush<2>(wk.gather_order) : select_flush<1>(wk.gather_order);
   h->smem_pass = pass_smem_bytes(nb, h->npair);
-  h->smem_wake = (size_t)nb * 2 * sizeof(double);
+  h->smem_wake = (size_t)nb * 3 * sizeof(double);
   CUH(cudaFuncSetAttribute((const void *)h->fn_map, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
   CUH(cudaFuncSetAttribute((const void *)h->fn_flush, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
   CUH(cudaFuncSetAttribute(k_wake, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_wake));
@@ -732,12 +759,12 @@ int mbt_normal_selftest(uint64_t seed, int64_t n, const uint32_t *ctr, double *o
   CU(cudaMalloc((void **)&dl, sizeof kLogTabHost));
   CU(cudaMemcpy(dl, kLogTabHost, sizeof kLogTabHost, cudaMemcpyHostToDevice));
   CU(cudaMalloc((void **)&dc, (size_t)n * 4 * sizeof(uint32_t)));
-  cudaError_t e = cudaMalloc((void **)&dz, (size_t)n * 2 * sizeof(double));
+  cudaError_t e = cudaMalloc((void **)&dz, (size_t)n * 4 * sizeof(double));
   if (e != cudaSuccess) { cudaFree(dc); CU(e); }
   e = cudaMemcpy(dc, ctr, (size_t)n * 4 * sizeof(uint32_t), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) {
     k_normal_selftest<<<148, 256>>>(n, dc, philox_expand_key((uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32)), dl, make_math_tab(), dz);
-    e = cudaMemcpy(out, dz, (size_t)n * 2 * sizeof(double), cudaMemcpyDeviceToHost);
+    e = cudaMemcpy(out, dz, (size_t)n * 4 * sizeof(double), cudaMemcpyDeviceToHost);
   }
   cudaFree(dc);
   cudaFree(dz);

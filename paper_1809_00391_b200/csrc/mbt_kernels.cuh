@@ -23,7 +23,7 @@ constexpr int kPassThreads = 256;
 constexpr int kWakeThreads = 256;
 constexpr int kMaxCav = 8;
 constexpr int kMaxLR = 8;
-constexpr int kDefaultNPair = 1;  // pairs per thread and iteration of the pass (1 or 2)
+constexpr int kDefaultNPair = 0;  // pairs per thread and iteration of the pass: 1, 2, or 0 = chosen from the workload at create
 
 struct cplx {
   double re, im;
@@ -43,6 +43,16 @@ struct Ctrl {
   uint32_t ticket;        // CTAs of k_wake that have finished (last-CTA-done election)
   uint32_t kick_pending;  // 1: the wake of turn `turn` has not been applied to delta yet
   uint32_t pad;
+};
+
+// gather cell k of a wake grid V[0..nb) (D12): linear gather: the particle with rint(t) = k sits between the centres
+// of bins k-1 and k, v(f) = mid + f dif, f = t - k in [-1/2, 1/2], mid = (V[k-1] + V[k]) / 2, dif = V[k] - V[k-1],
+// with V[-1] := V[0], V[nb] := V[nb-1]; nearest grid point: mid = V[k], dif = 0.  Cell nb+1 is zero.
+struct WakeCell {
+  double mid, dif;
+};
+struct CellF {  // the same cell of the complex table F_r
+  cplx mid, dif;
 };
 
 struct Args {
@@ -74,6 +84,8 @@ struct Args {
   const double *Vsr;    // [M][nb]   short-range wake of the last turn [V]
   const cplx *P;        // [M][R]    long-range phasor seen by bunch b
   const cplx *F;        // [R][nb]   C_r exp(lambda_r c_j)
+  const WakeCell *cellSR;   // [M][nb+2] gather cells of the short-range wake of the last turn (k_wake)
+  const CellF *cellF;       // [R][nb+2] gather cells of F_r: cell(V_SR + sum_r Re[F_r P_r]) = cellSR + sum_r Re[cellF_r P_r]
   int32_t R;            // long-range resonators
   uint32_t *hist;       // [M][nb]   accumulating counts of the pass in flight
   double *mom_acc;      // [M][4]    sum tau, sum delta, sum tau^2, sum delta^2
@@ -83,10 +95,6 @@ struct Args {
   MathTab mt;
 };
 
-// shared-memory layout of one CTA of the pass (dynamic): wake table, staging copy of V, counts, log table
-struct WakeCell {
-  double mid, dif;  // v(f) = mid + f * dif, f in [-1/2, 1/2] around the cell boundary (linear gather)
-};
 // Particle staging: a CTA owns kStages shared-memory stages of kPassThreads*NPAIR pairs (tau block, then delta
 // block), filled by cp.async.bulk (TMA, global -> shared) kStages-1 iterations ahead of their use.  full[stage]
 // completes when both blocks have landed (expect_tx); empty[stage] completes when all warps have read the stage
@@ -99,8 +107,8 @@ __host__ __device__ inline size_t pass_stage_bytes(int npair) {
   return (size_t)kStages * 2 * kPassThreads * npair * 16;
 }
 __host__ __device__ inline size_t pass_smem_bytes(int nb, int npair) {
-  return pass_stage_bytes(npair) + (size_t)(nb + 2) * sizeof(WakeCell) + (size_t)nb * sizeof(double) +
-         (size_t)(nb + 1) * sizeof(uint32_t) + 128 * sizeof(LogTabEntry) + 16;
+  return pass_stage_bytes(npair) + (size_t)(nb + 2) * sizeof(WakeCell) + (size_t)(nb + 1) * sizeof(uint32_t) +
+         128 * sizeof(LogTabEntry) + 16;
 }
 
 // ---- mbarrier / bulk-copy primitives (PTX; SASS: SYNCS / UBLKCP)
@@ -123,6 +131,9 @@ __device__ __forceinline__ double2 lds_double2(uint32_t addr) {  // volatile: th
   double2 v;
   asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
   return v;
+}
+__device__ __forceinline__ void stg_double4(void *p, double a, double b, double c, double d) {  // STG.E.256 (sm_100)
+  asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
@@ -170,8 +181,7 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? MBT_MINB1 : MBT_MIN
   constexpr int NWARP = kPassThreads / 32;
   unsigned char *sStage = smem_raw;                   // [stage]{double2 tau[STRIDE]; double2 delta[STRIDE]}
   WakeCell *sW = reinterpret_cast<WakeCell *>(smem_raw + kStages * STAGE_BYTES);  // [nb+2]
-  double *sV = reinterpret_cast<double *>(sW + (A.nb + 2));                     // [nb]
-  LogTabEntry *sL = reinterpret_cast<LogTabEntry *>(sV + A.nb);                 // [128]
+  LogTabEntry *sL = reinterpret_cast<LogTabEntry *>(sW + (A.nb + 2));          // [128]
   uint32_t *sH = reinterpret_cast<uint32_t *>(sL + 128);                        // [nb + 1], bin nb is a sink
   __shared__ double s_red[NWARP][4];
   __shared__ uint32_t s_nout[NWARP];
@@ -218,40 +228,29 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? MBT_MINB1 : MBT_MIN
     if (tid == 0)
       for (uint32_t k = 0; k + 1u < (uint32_t)kStages && k < n_it; ++k) issue(k);
 
-    // stage the wake of bunch b: V = V_SR + sum_r Re[F_r[j] P[b][r]] (S6 expansion), then the gather cells
-    for (int j = tid; j < nb; j += kPassThreads) {
-      double v = 0.0;
-      if (have_kick) {
-        v = A.Vsr[(size_t)b * nb + j];
-        for (int r = 0; r < A.R; ++r) {
-          const cplx f = A.F[(size_t)r * nb + j];
-          const cplx pb = A.P[(size_t)b * A.R + r];
-          v += fma(f.re, pb.re, -(f.im * pb.im));
-        }
-      }
-      sV[j] = v;
-      sH[j] = 0u;
-    }
-    __syncthreads();
+    // stage the gather cells of bunch b's wake: cellSR + sum_r Re[cellF_r P[b][r]] (S6 expansion); clear the counts
     for (int k = tid; k < nb + 2; k += kPassThreads) {
       WakeCell c{0.0, 0.0};
-      if (GATHER == 1) {
-        if (k <= nb) {
-          const double lo = sV[k > 0 ? k - 1 : 0], hi = sV[k < nb ? k : nb - 1];
-          c.mid = 0.5 * (lo + hi);
-          c.dif = hi - lo;
+      if (have_kick) {
+        c = A.cellSR[(size_t)b * (nb + 2) + k];
+#pragma unroll 1
+        for (int r = 0; r < A.R; ++r) {
+          const CellF f = A.cellF[(size_t)r * (nb + 2) + k];
+          const cplx pb = A.P[(size_t)b * A.R + r];
+          c.mid += fma(f.mid.re, pb.re, -(f.mid.im * pb.im));
+          c.dif += fma(f.dif.re, pb.re, -(f.dif.im * pb.im));
         }
-      } else if (k < nb) {
-        c.mid = sV[k];
       }
       sW[k] = c;
+      if (k < nb) sH[k] = 0u;
     }
     __syncthreads();
 
     double st = 0.0, sd = 0.0, stt = 0.0, sdd = 0.0;
     uint32_t nout = 0u;
-    // one running pointer per thread: tau pair at T[q * kPassThreads], delta pair at the constant byte distance d_off
-    uint32_t p = p0 + tid;
+    // a thread owns NPAIR consecutive pairs (NPAIR = 2: one quad of four particles, 32 bytes per array, one 256-bit
+    // store); one running pointer per thread: tau at T[q], delta at the constant byte distance d_off
+    uint32_t p = p0 + (uint32_t)tid * NPAIR;
     double2 *T = reinterpret_cast<double2 *>(A.tau + (size_t)b * A.ld) + p;
     const ptrdiff_t d_off = reinterpret_cast<const char *>(A.delta) - reinterpret_cast<const char *>(A.tau);
 #define MBT_D(ptr) reinterpret_cast<double2 *>(reinterpret_cast<char *>(ptr) + d_off)
@@ -264,19 +263,19 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? MBT_MINB1 : MBT_MIN
       if (c < n_it) next_issue = c;
     }
     // a full tile has no ragged end and no padding slot: the `live` logic drops out of its loop
-    const bool full_tile = (p1 - p0 == n_it * STRIDE) && !((A.Np & 1u) && p1 == A.ppb);
+    const bool full_tile = (p1 - p0 == n_it * STRIDE) && !(A.Np != 2u * A.ppb && p1 == A.ppb);
     auto run = [&](auto full_tag) {
     constexpr bool FULL = decltype(full_tag)::value;
     // running shared-memory addresses of the stage in use: full barrier (empty barrier kStages * 8 bytes above it)
     // and this thread's slot; they wrap every kStages iterations, where the mbarrier parity flips
-    uint32_t bar_a = full0, slot_a = stage0 + (uint32_t)tid * 16u, parity = 0u, until_wrap = kStages;
+    uint32_t bar_a = full0, slot_a = stage0 + (uint32_t)tid * (16u * NPAIR), parity = 0u, until_wrap = kStages;
     for (uint32_t k = 0; k < n_it; ++k) {
       mbar_wait(bar_a, parity);
       double2 t2[NPAIR], d2[NPAIR];
 #pragma unroll
       for (int q = 0; q < NPAIR; ++q) {
-        t2[q] = lds_double2(slot_a + q * kPassThreads * 16u);
-        d2[q] = lds_double2(slot_a + (STRIDE + q * kPassThreads) * 16u);
+        t2[q] = lds_double2(slot_a + q * 16u);
+        d2[q] = lds_double2(slot_a + (STRIDE + q) * 16u);
       }
       __syncwarp();  // every lane of the warp has read the stage
       if (lane == 0) mbar_arrive(bar_a + kStages * 8u);
@@ -295,20 +294,25 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? MBT_MINB1 : MBT_MIN
 
       double tau[NP], del[NP], z[NP];
       bool live[NP];
+      BmState bm[NPAIR];
+      uint32_t xs[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
       for (int q = 0; q < NPAIR; ++q) {
-        const uint32_t pq = p + q * kPassThreads;
+        const uint32_t pq = p + q;
         tau[2 * q] = t2[q].x; tau[2 * q + 1] = t2[q].y;
         del[2 * q] = d2[q].x; del[2 * q + 1] = d2[q].y;
-        live[2 * q] = FULL || pq < p1;                      // past the end of the tile: stale stage contents, ignored
-        live[2 * q + 1] = FULL || (live[2 * q] && (2u * pq + 1u < A.Np));  // odd slot of the last pair is padding if N_p is odd
+        live[2 * q] = FULL || (pq < p1 && 2u * pq < A.Np);  // past the end of the tile: stale stage contents, ignored;
+        live[2 * q + 1] = FULL || (live[2 * q] && (2u * pq + 1u < A.Np));  // the slots from N_p up to ld are padding
         z[2 * q] = z[2 * q + 1] = 0.0;
         if (MAP && RAD) {
-          // one Philox call and one Box-Muller serve both particles of the 128-bit load (D8):
-          // counter (pair, bunch, turn, tag 0); even particle takes z_c, odd particle z_s
-          uint32_t x0, x1, x2, x3;
-          philox4x32_10(pq, (uint32_t)b, n, 0u, A.keys, x0, x1, x2, x3);
-          box_muller_fast(A.mt, sL, x0, x1, x2, x3, A.A_q, z[2 * q], z[2 * q + 1]);
+          // one Philox block serves FOUR consecutive particles (D8): counter (particle >> 2, bunch, turn, tag 0);
+          // its words (x0, x1) give the Box-Muller pair of particles 4j, 4j+1, (x2, x3) that of 4j+2, 4j+3; the even
+          // particle of a pair takes z_c, the odd one z_s.  A thread that owns the whole quad (NPAIR = 2) calls it once.
+          if (q == 0 || NPAIR == 1) philox4x32_10(pq >> 1, (uint32_t)b, n, 0u, A.keys, xs[0], xs[1], xs[2], xs[3]);
+          const bool hi_half = (NPAIR == 2) ? (q == 1) : ((pq & 1u) != 0u);  // with NPAIR = 2 the thread's first pair is even
+          const double u1 = uniform32(A.mt, hi_half ? xs[2] : xs[0]), u2 = uniform32(A.mt, hi_half ? xs[3] : xs[1]);
+          if (NCAV > 0) bm[q] = box_muller_head(A.mt, sL, u1, u2, A.A_q);  // polynomials: lock step with S1's
+          else box_muller_fast(A.mt, sL, u1, u2, A.A_q, z[2 * q], z[2 * q + 1]);
         }
       }
       // S0: kick of the previous turn's wake.  t exactly as the binning computed it (one subtraction, one
@@ -354,16 +358,33 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? MBT_MINB1 : MBT_MIN
         // independent polynomial chains interleave (DFMA latency is 8 cycles); a particle long lost from the bucket
         // (|y| >= 2^16, or not finite) is then patched with the library sine in a single cold branch.
         if (NCAV > 0) {
-          double sn[NCAV > 0 ? NCAV : 1][NP];
+          constexpr int NS = (NCAV > 0 ? NCAV : 1) * NP;
+          constexpr int NB = RAD ? NPAIR : 0;
+          SinState ss[NS];
+          constexpr int NB1 = NB > 0 ? NB : 1;
+          double zz[NS], pp[NS], f2[NB1], ps[NB1], pc[NB1];
           uint32_t worst = 0u;
 #pragma unroll
           for (int c = 0; c < NCAV; ++c)
 #pragma unroll
             for (int i = 0; i < NP; ++i) {
               const double y = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
-              sn[c][i] = sin_rf_fast(A.mt, y);
+              ss[c * NP + i] = sin_rf_head(A.mt, y);
+              zz[c * NP + i] = ss[c * NP + i].z;
               worst = max(worst, (uint32_t)__double2hiint(y) & 0x7FFFFFFFu);
             }
+#pragma unroll
+          for (int q = 0; q < NB; ++q) f2[q] = bm[q].f2;
+          horner7_lockstep<NS, NB>(A.mt, zz, pp, f2, ps, pc);
+          double sn[NCAV > 0 ? NCAV : 1][NP];
+#pragma unroll
+          for (int c = 0; c < NCAV; ++c)
+#pragma unroll
+            for (int i = 0; i < NP; ++i) sn[c][i] = sin_rf_tail(ss[c * NP + i], pp[c * NP + i]);
+          if (RAD) {
+#pragma unroll
+            for (int q = 0; q < NB; ++q) box_muller_tail(A.mt, bm[q], ps[q], pc[q], z[2 * q], z[2 * q + 1]);
+          }
           if (__builtin_expect(worst >= 0x40F00000u, 0)) {  // some |y| >= 65536, inf or NaN
 #pragma unroll
             for (int c = 0; c < NCAV; ++c)
@@ -402,12 +423,15 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? MBT_MINB1 : MBT_MIN
       // S4: deposit.  Branch-free: a particle outside the window (or a padding slot) counts into the spare bin nb.
 #pragma unroll
       for (int i = 0; i < NP; ++i) atomicAdd(&sH[in[i] ? __double2int_rd(t[i]) : nb], 1u);
-#pragma unroll
-      for (int q = 0; q < NPAIR; ++q)
-        if (live[2 * q]) {
-          if (MAP) T[q * kPassThreads] = make_double2(tau[2 * q], tau[2 * q + 1]);
-          *MBT_D(T + q * kPassThreads) = make_double2(del[2 * q], del[2 * q + 1]);
+      if (FULL || p < p1) {  // p and p1 are even when NPAIR = 2: the thread's pairs are inside the tile together
+        if (NPAIR == 2) {
+          if (MAP) stg_double4(T, tau[0], tau[1], tau[NP - 2], tau[NP - 1]);
+          stg_double4(MBT_D(T), del[0], del[1], del[NP - 2], del[NP - 1]);
+        } else {
+          if (MAP) T[0] = make_double2(tau[0], tau[1]);
+          *MBT_D(T) = make_double2(del[0], del[1]);
         }
+      }
       p += STRIDE;
       T += STRIDE;
     }
@@ -462,6 +486,8 @@ struct WakeArgs {
   uint32_t *hist;          // [M][nb]  in: counts of this turn; out: zero
   uint32_t *hist_last;     // [M][nb]  out: counts of this turn
   double *Vsr;             // [M][nb]
+  WakeCell *cellSR;        // [M][nb+2] gather cells of Vsr (what the pass stages)
+  int32_t gather;          // 1 linear, 0 nearest grid point
   cplx *a_cur;             // [M][R]   source phasors of this turn
   cplx *ring_a;            // [K+1][M][R] slot n % (K+1)
   cplx *ring_A;            // [K+1][R]    per-turn aggregates, slot n % (K+1)
@@ -492,7 +518,7 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   extern __shared__ double smem_d[];
   double *sq = smem_d;         // [nb] charge per bin
   double *sw = smem_d + A.nb;  // [nb] wake table
-  __shared__ double s_red[kWakeThreads / 32][2];
+  double *sv = smem_d + 2 * A.nb;  // [nb] V_SR of this bunch
   __shared__ bool s_last;
 
   const int tid = threadIdx.x;
@@ -510,14 +536,18 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
     sq[j] = qm * (double)c;
     if (A.mode == 0 && A.w) sw[j] = A.w[j];
   }
+  __syncthreads();
   // S7: close the moments the pass gathered (state after turn n_done's kick)
-  if (tid == 0) {
+  // by the last thread of the CTA: its warp has no convolution work unless nb > 448, so this serial stretch
+  // (a division, two square roots) runs beside the convolution instead of ahead of it
+  if (tid == kWakeThreads - 1) {
     const double N = (double)A.Np;
     const double s1 = A.mom_acc[b * 4 + 0], s2 = A.mom_acc[b * 4 + 1];
     const double s11 = A.mom_acc[b * 4 + 2], s22 = A.mom_acc[b * 4 + 3];
     const double no = (double)A.nout_acc[b];
-    const double mt = s1 / N, md = s2 / N;
-    const double vt = fmax(s11 / N - mt * mt, 0.0), vd = fmax(s22 / N - md * md, 0.0);
+    const double iN = 1.0 / N;
+    const double mt = s1 * iN, md = s2 * iN;
+    const double vt = fmax(s11 * iN - mt * mt, 0.0), vd = fmax(s22 * iN - md * md, 0.0);
     double m[6] = {N - no, no, mt, md, sqrt(vt), sqrt(vd)};
 #pragma unroll
     for (int k = 0; k < 6; ++k) A.mom_last[b * 6 + k] = m[k];
@@ -530,46 +560,72 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
     A.nout_acc[b] = 0ull;
   }
   if (A.mode != 0) return;
-  __syncthreads();
+#ifndef MBT_EXP_WAKE
+#define MBT_EXP_WAKE 0
+#endif
+  if (MBT_EXP_WAKE == 4) { if (tid == 0 && b == 0) { A.ctrl->kick_pending = 1u; A.ctrl->turn = n; } return; }
 
-  // S5: V_SR[j] = sum_{k<=j} w[j-k] q[k].  Outputs j and nb-1-j are paired so that every thread does nb+1 terms.
-  if (A.w) {
-    for (int idx = tid; idx < (nb + 1) / 2; idx += kWakeThreads) {
-      const int j1 = idx, j2 = nb - 1 - idx;
-      double acc1 = 0.0, acc2 = 0.0;
-      for (int k = 0; k <= j1; ++k) acc1 = fma(sw[j1 - k], sq[k], acc1);
-      A.Vsr[(size_t)b * nb + j1] = acc1;
-      if (j2 != j1) {
-        for (int k = 0; k <= j2; ++k) acc2 = fma(sw[j2 - k], sq[k], acc2);
-        A.Vsr[(size_t)b * nb + j2] = acc2;
-      }
-    }
-  } else {
-    for (int j = tid; j < nb; j += kWakeThreads) A.Vsr[(size_t)b * nb + j] = 0.0;
-  }
-
-  // S6 sources: a[b][r] = sum_k q[k] exp(-lambda_r c_k)
-  for (int r = 0; r < A.R; ++r) {
+  // S6 sources: a[b][r] = sum_k q[k] exp(-lambda_r c_k).  One warp per resonator (shuffles only, no block
+  // barrier); the other warps go straight to the convolution.
+  for (int r = tid >> 5; r < A.R && MBT_EXP_WAKE != 3; r += kWakeThreads / 32) {
     double are = 0.0, aim = 0.0;
-    for (int k = tid; k < nb; k += kWakeThreads) {
+    for (int k = tid & 31; k < nb; k += 32) {
       const cplx e = A.Esrc[(size_t)r * nb + k];
       are = fma(sq[k], e.re, are);
       aim = fma(sq[k], e.im, aim);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-      are += __shfl_down_sync(0xffffffffu, are, o);
-      aim += __shfl_down_sync(0xffffffffu, aim, o);
+      are += __shfl_xor_sync(0xffffffffu, are, o);
+      aim += __shfl_xor_sync(0xffffffffu, aim, o);
     }
-    if ((tid & 31) == 0) { s_red[tid >> 5][0] = are; s_red[tid >> 5][1] = aim; }
-    __syncthreads();
-    if (tid == 0) {
-      cplx a{0.0, 0.0};
-      for (int w = 0; w < kWakeThreads / 32; ++w) { a.re += s_red[w][0]; a.im += s_red[w][1]; }
+    if ((tid & 31) == 0) {
+      const cplx a{are, aim};
       A.a_cur[(size_t)b * A.R + r] = a;
       A.ring_a[((size_t)(n % (uint32_t)(A.K + 1)) * A.M + b) * A.R + r] = a;
     }
-    __syncthreads();
+  }
+
+  // S5: V_SR[j] = sum_{k<=j} w[j-k] q[k].  Outputs j and nb-1-j are paired so that every thread does nb+1 terms;
+  // each sum runs on four interleaved accumulators (k mod 4), so that the 8-cycle DFMA latency and the
+  // shared-memory loads of consecutive terms overlap.
+  if (A.w && MBT_EXP_WAKE != 1) {
+    for (int idx = tid; idx < (nb + 1) / 2; idx += kWakeThreads) {
+      const int j1 = idx, j2 = nb - 1 - idx;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int j = h ? j2 : j1;
+        if (h && j2 == j1) break;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        int k = 0;
+        for (; k + 3 <= j; k += 4) {
+          a0 = fma(sw[j - k], sq[k], a0);
+          a1 = fma(sw[j - k - 1], sq[k + 1], a1);
+          a2 = fma(sw[j - k - 2], sq[k + 2], a2);
+          a3 = fma(sw[j - k - 3], sq[k + 3], a3);
+        }
+        for (; k <= j; ++k) a0 = fma(sw[j - k], sq[k], a0);
+        const double v = (a0 + a1) + (a2 + a3);
+        A.Vsr[(size_t)b * nb + j] = v;
+        sv[j] = v;
+      }
+    }
+  } else {
+    for (int j = tid; j < nb; j += kWakeThreads) { A.Vsr[(size_t)b * nb + j] = 0.0; sv[j] = 0.0; }
+  }
+  __syncthreads();
+  for (int k = tid; k < nb + 2; k += kWakeThreads) {
+    WakeCell c{0.0, 0.0};
+    if (A.gather == 1) {
+      if (k <= nb) {
+        const double lo = sv[k > 0 ? k - 1 : 0], hi = sv[k < nb ? k : nb - 1];
+        c.mid = 0.5 * (lo + hi);
+        c.dif = hi - lo;
+      }
+    } else if (k < nb) {
+      c.mid = sv[k];
+    }
+    A.cellSR[(size_t)b * (nb + 2) + k] = c;
   }
 
   // last-CTA-done election: the CTA that sees every other CTA's ticket closes the turn
@@ -586,7 +642,7 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   const int M = A.M, R = A.R, K = A.K;
   const int lane = tid & 31;
   const int run = (M + 31) / 32;  // consecutive bunches per lane
-  for (int r = tid >> 5; r < R; r += kWakeThreads / 32) {
+  for (int r = tid >> 5; r < R && MBT_EXP_WAKE != 2; r += kWakeThreads / 32) {
     // G_n = sum_{k=1..min(K,n-1)} A_{n-k} exp(lambda (k T0 - span)): lanes take k = lane+1, lane+33, ...
     cplx G{0.0, 0.0};
     for (int k = lane + 1; k <= K && (int64_t)n - k >= 1; k += 32)
@@ -596,16 +652,27 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
       G.re += __shfl_xor_sync(0xffffffffu, G.re, o);
       G.im += __shfl_xor_sync(0xffffffffu, G.im, o);
     }
-    // lane-local composite of its run of bunches, and this turn's own aggregate
+    // lane-local composite of its run of bunches, and this turn's own aggregate.  The run is walked four bunches
+    // at a time with all of a chunk's loads issued before its arithmetic: each chunk costs one L2 round trip.
     const int j_lo = lane * run, j_hi = min(j_lo + run, M);
     Affine loc{cplx{1.0, 0.0}, cplx{0.0, 0.0}};
     cplx own{0.0, 0.0};
-    for (int j = j_lo; j < j_hi; ++j) {
-      const cplx a = __ldcg_cplx(&A.a_cur[(size_t)j * R + r]);
-      own = cfma(a, A.g_tail[(size_t)j * R + r], own);
-      if (j + 1 < M) {
-        const cplx g = A.g_step[(size_t)j * R + r];
-        loc = compose(loc, Affine{g, cmul(a, g)});
+    for (int j0 = j_lo; j0 < j_hi; j0 += 4) {
+      cplx a[4], gt[4], gs[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int j = min(j0 + u, M - 1);
+        a[u] = __ldcg_cplx(&A.a_cur[(size_t)j * R + r]);
+        gt[u] = A.g_tail[(size_t)j * R + r];
+        gs[u] = A.g_step[(size_t)j * R + r];
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int j = j0 + u;
+        if (j < j_hi) {
+          own = cfma(a[u], gt[u], own);
+          if (j + 1 < M) loc = compose(loc, Affine{gs[u], cmul(a[u], gs[u])});
+        }
       }
     }
     // inclusive warp scan of the lane composites (Kogge-Stone on shuffles), then the exclusive prefix applied to G
@@ -621,9 +688,22 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
     pre.g.re = __shfl_up_sync(0xffffffffu, inc.g.re, 1); pre.g.im = __shfl_up_sync(0xffffffffu, inc.g.im, 1);
     pre.c.re = __shfl_up_sync(0xffffffffu, inc.c.re, 1); pre.c.im = __shfl_up_sync(0xffffffffu, inc.c.im, 1);
     cplx Pj = (lane > 0) ? cfma(pre.g, G, pre.c) : G;
-    for (int j = j_lo; j < j_hi; ++j) {
-      A.P[(size_t)j * R + r] = Pj;
-      if (j + 1 < M) Pj = cmul(cadd(Pj, __ldcg_cplx(&A.a_cur[(size_t)j * R + r])), A.g_step[(size_t)j * R + r]);
+    for (int j0 = j_lo; j0 < j_hi; j0 += 4) {
+      cplx a[4], gs[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int j = min(j0 + u, M - 1);
+        a[u] = __ldcg_cplx(&A.a_cur[(size_t)j * R + r]);
+        gs[u] = A.g_step[(size_t)j * R + r];
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int j = j0 + u;
+        if (j < j_hi) {
+          A.P[(size_t)j * R + r] = Pj;
+          if (j + 1 < M) Pj = cmul(cadd(Pj, a[u]), gs[u]);
+        }
+      }
     }
     // A_n = sum_j a_j exp(lambda (s_{M-1}-s_j) T_rf)
 #pragma unroll
@@ -721,10 +801,8 @@ __global__ void k_normal_selftest(int64_t n, const uint32_t *ctr, PhiloxKeys key
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
     uint32_t x0, x1, x2, x3;
     philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], keys, x0, x1, x2, x3);
-    double zc, zs;
-    box_muller_fast(mt, sL, x0, x1, x2, x3, 1.0, zc, zs);
-    out[2 * i] = zc;
-    out[2 * i + 1] = zs;
+    box_muller_fast(mt, sL, uniform32(mt, x0), uniform32(mt, x1), 1.0, out[4 * i], out[4 * i + 1]);
+    box_muller_fast(mt, sL, uniform32(mt, x2), uniform32(mt, x3), 1.0, out[4 * i + 2], out[4 * i + 3]);
   }
 }
 

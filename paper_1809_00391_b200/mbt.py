@@ -129,7 +129,7 @@ def philox_selftest(ctr, key):
 
 def normal_selftest(seed, ctr):
     ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
-    out = np.empty((ctr.shape[0], 2))
+    out = np.empty((ctr.shape[0], 4))
     _ck(lib().mbt_normal_selftest(int(seed), ctr.shape[0], ctr.ctypes.data_as(C.POINTER(C.c_uint32)), _dp(out)))
     return out
 

@@ -42,7 +42,7 @@ def test_host_only_entry_points(libpath):
     """Calls that touch no GPU: stride, version, error text, NULL handling."""
     from paper_1809_00391_b200 import mbt
     L = mbt.lib()
-    assert mbt.particle_stride(37) == 38 and mbt.particle_stride(100000) == 100000 and mbt.particle_stride(1) == 2
+    assert mbt.particle_stride(37) == 40 and mbt.particle_stride(100000) == 100000 and mbt.particle_stride(1) == 4
     assert b"sm_100a" in L.mbt_version()
     assert L.mbt_turn(None) == -1
     assert L.mbt_destroy(None) == 0
