@@ -204,12 +204,12 @@ def run_mbt(args):
                 "algorithmic_bytes_per_launch": BYTES_PER_PARTICLE_TURN * n_part,
                 "pass_ms": pass_s / kp * 1e3, "wake_ms": wake_s / kp * 1e3,
                 "pass_share_of_step": pass_s / (pass_s + wake_s)}
-    prof = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    # DRAM bytes of one launch from the committed `ncu --set full` capture of this workload (profiles/traffic_<cfg>.txt)
     try:
-        with open(prof) as f:
-            tr = json.load(f)
-        if tr.get("config") == args.config:
-            roofline["traffic"] = tr.get("dram_bytes_per_launch")
+        with open(os.path.join(ROOT, "profiles", "traffic_%s.txt" % args.config)) as f:
+            for ln in f:
+                if ln.startswith("dram_bytes_per_launch"):
+                    roofline["traffic"] = float(ln.split()[1])
     except Exception:
         pass
     trk.close()
