@@ -135,6 +135,22 @@ def test_single_turn_parity_configs(mbt, orc, name, over):
         print(name, r1, r2)
 
 
+@pytest.mark.parametrize("npair", [1, 2])
+@pytest.mark.parametrize("n_per_bunch", [1, 2, 3, 4, 5, 7, 255, 257, 511, 513, 1023, 1025, 2049, 8191, 8193, 16387])
+def test_ragged_sizes_both_kernel_variants(mbt, orc, npair, n_per_bunch, monkeypatch):
+    """Sizes around every boundary of the pass (a quad of 4 particles, a chunk of 256 / 512 pairs, a tile of 16
+    chunks) in both variants of the pass (1 or 2 pairs per thread; MBT_NPAIR is the library's measurement knob):
+    padding slots, partial TMA chunks and partial tiles must not leak into particles, counts or moments.
+    compute-sanitizer is closed on this pool, so bounds are checked by comparison with the oracle."""
+    monkeypatch.setenv("MBT_NPAIR", str(npair))
+    cfg = W.tiny(m=2, n_per_bunch=n_per_bunch, n_bins=16, harmonic=(n_per_bunch % 2 == 1))
+    o = orc.Oracle(cfg)
+    o.track(2)
+    with mbt.Tracker(cfg) as t:
+        for _ in range(2):
+            assert_single_turn_parity(o, t, cfg)
+
+
 def test_several_turns_without_resync(mbt, orc):
     """Nine turns from each side's OWN initial distribution and no re-synchronisation: the fused ordering
     (kick at the head of the next pass) reproduces the sequential order of the paper."""
