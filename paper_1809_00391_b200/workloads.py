@@ -165,5 +165,23 @@ def tiny(m=5, n_per_bunch=37, n_bins=8, k_hist=3, seed=11, buckets=None, n_lr=2,
     return cfg
 
 
+def sampled_wake_table(n_bins, delta_s, r_ohm=0.0, l_henry=0.0, rw_amp=0.0):
+    """User-sampled short-range wake w[k] at lag k*Delta [V/C] for `wake["sr_table"]` (the
+    wake sources the paper lists beside resonators, P:l.98 "resistive-wall effects ... purely resistive and inductive
+    components", whose formulas are only in its ref. [7]).  Input generation, not the method: the tracker just
+    convolves whatever table it is given.  Textbook grid forms:
+      * pure resistance R:  V = R I, I_j = q_j / Delta        ->  w[0] += R / Delta
+      * pure inductance L:  V = L dI/dt (backward difference) ->  w[0] += L / Delta^2, w[1] -= L / Delta^2
+      * resistive-wall-like power law, amplitude synthetic:   ->  w[k] += rw_amp * (k Delta)^(-3/2), k >= 1
+    """
+    w = np.zeros(int(n_bins))
+    w[0] += r_ohm / delta_s + l_henry / delta_s**2
+    if n_bins > 1:
+        w[1] -= l_henry / delta_s**2
+        k = np.arange(1, int(n_bins))
+        w[1:] += rw_amp * (k * delta_s) ** -1.5
+    return w
+
+
 def n_particles(cfg) -> int:
     return len(cfg["fill"]["buckets"]) * cfg["fill"]["n_per_bunch"]

@@ -151,6 +151,24 @@ def test_ragged_sizes_both_kernel_variants(mbt, orc, npair, n_per_bunch, monkeyp
             assert_single_turn_parity(o, t, cfg)
 
 
+def test_user_sampled_wake_table(mbt, orc):
+    """A user-sampled short-range table (resistive + inductive + power law) beside the
+    resonators: same parity bar as the resonator-only wake."""
+    for n_lr, with_res in ((2, True), (0, False)):
+        cfg = W.tiny(m=3, n_per_bunch=2049, n_bins=64, n_lr=n_lr)
+        wk = cfg["wake"]
+        delta = (wk["tau_hi_s"] - wk["tau_lo_s"]) / wk["n_bins"]
+        wk["sr_table"] = W.sampled_wake_table(wk["n_bins"], delta, r_ohm=700.0, l_henry=3.0e-9, rw_amp=2.0e-4)
+        if not with_res:
+            wk["resonators"] = []
+        o = orc.Oracle(cfg)
+        o.track(3)
+        with mbt.Tracker(cfg) as t:
+            for _ in range(2):
+                r = assert_single_turn_parity(o, t, cfg)
+            assert np.abs(t.wake()[1]).max() > 0
+
+
 def test_several_turns_without_resync(mbt, orc):
     """Nine turns from each side's OWN initial distribution and no re-synchronisation: the fused ordering
     (kick at the head of the next pass) reproduces the sequential order of the paper."""

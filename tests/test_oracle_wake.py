@@ -286,3 +286,37 @@ def test_lr_uniform_fill_geometric_series(orc):
                 ph = float((np.longdouble(wb) * dt) % (2 * np.pi * np.longdouble(1)))
                 s += (cc * math.exp(-al * float(dt)) * complex(math.cos(ph), math.sin(ph))).real
             assert vlr[j, nb // 2] == pytest.approx(q * s, rel=1e-8, abs=1e-9 * q * abs(cc))
+
+
+def test_user_sampled_table_resistive_inductive_power_law(orc):
+    """a user-sampled short-range table (here R + L + a t^-3/2 power law) is added to the
+    resonator table and convolved like it.  Pins: with the table alone, V is the textbook grid form
+    R I_j + L (I_j - I_{j-1}) / Delta + power-law sum, written out with numpy; with a resonator as well, the sum."""
+    cfg = W.tiny(m=2, n_per_bunch=3000, n_bins=32, n_lr=0)
+    wk = cfg["wake"]
+    nb = wk["n_bins"]
+    delta = (wk["tau_hi_s"] - wk["tau_lo_s"]) / nb
+    R, L, A = 700.0, 3.0e-9, 2.0e-4
+    tbl = W.sampled_wake_table(nb, delta, r_ohm=R, l_henry=L, rw_amp=A)
+    both = W.tiny(m=2, n_per_bunch=3000, n_bins=32, n_lr=0)
+    both["wake"]["sr_table"] = tbl
+    only = W.tiny(m=2, n_per_bunch=3000, n_bins=32, n_lr=0)
+    only["wake"]["sr_table"] = tbl
+    only["wake"]["resonators"] = []
+    o_res, o_both, o_only = orc.Oracle(cfg), orc.Oracle(both), orc.Oracle(only)
+    for o in (o_res, o_both, o_only):
+        o.track(1)
+    h = o_only.histogram().astype(np.float64)
+    v_only = o_only.wake()[1]
+    for b in range(2):
+        q = h[b] * only["fill"]["charge_C"][b] / only["fill"]["n_per_bunch"]
+        cur = q / delta                                            # bin current [A]
+        want = R * cur + L * (cur - np.concatenate([[0.0], cur[:-1]])) / delta
+        for j in range(nb):
+            for k in range(j):
+                want[j] += A * ((j - k) * delta) ** -1.5 * q[k]
+        assert np.allclose(v_only[b], want, rtol=1e-12, atol=1e-12 * np.abs(want).max())
+    # identical particles in all three (the wake kick comes after the binning of turn 1): superposition
+    assert np.array_equal(o_res.histogram(), o_both.histogram())
+    v_sum = o_res.wake()[1] + v_only
+    assert np.allclose(o_both.wake()[1], v_sum, rtol=1e-12, atol=1e-12 * np.abs(v_sum).max())
