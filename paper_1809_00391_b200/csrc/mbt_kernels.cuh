@@ -167,13 +167,7 @@ __device__ __forceinline__ bool in_window(double t, uint32_t hi_nb) { return (ui
 // dif = V[kk]-V[kk-1], with V[-1] := V[0] and V[nb] := V[nb-1] (constant outer half bins).  Cell nb+1 is zero and
 // serves every particle outside the window (no kick, D11), which keeps the step branch-free.
 template <bool MAP, bool RAD, int GATHER, int NCAV, int NPAIR>
-#ifndef MBT_MINB1
-#define MBT_MINB1 3
-#endif
-#ifndef MBT_MINB2
-#define MBT_MINB2 2
-#endif
-__global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? MBT_MINB1 : MBT_MINB2) k_pass(const __grid_constant__ Args A) {
+__global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const __grid_constant__ Args A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int NP = 2 * NPAIR;                       // particles per thread and iteration
   constexpr uint32_t STRIDE = kPassThreads * NPAIR;   // pairs per CTA and iteration (one stage)
@@ -342,16 +336,12 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? MBT_MINB1 : MBT_MIN
       // S7: moments of the state after the kick
 #pragma unroll
       for (int i = 0; i < NP; ++i)
-#ifndef MBT_EXP_NOMOM
         if (live[i]) {
           st += tau[i];
           sd += del[i];
           stt = fma(tau[i], tau[i], stt);
           sdd = fma(del[i], del[i], sdd);
         }
-#else
-        ;
-#endif
       if (MAP) {
         // S1: RF cavities.  The phase is formed as the oracle forms it (product rounded, then the sum).  All fast sines
         // of the iteration are evaluated first, in ONE basic block together with the Box-Muller above, so that the
@@ -560,14 +550,10 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
     A.nout_acc[b] = 0ull;
   }
   if (A.mode != 0) return;
-#ifndef MBT_EXP_WAKE
-#define MBT_EXP_WAKE 0
-#endif
-  if (MBT_EXP_WAKE == 4) { if (tid == 0 && b == 0) { A.ctrl->kick_pending = 1u; A.ctrl->turn = n; } return; }
 
   // S6 sources: a[b][r] = sum_k q[k] exp(-lambda_r c_k).  One warp per resonator (shuffles only, no block
   // barrier); the other warps go straight to the convolution.
-  for (int r = tid >> 5; r < A.R && MBT_EXP_WAKE != 3; r += kWakeThreads / 32) {
+  for (int r = tid >> 5; r < A.R; r += kWakeThreads / 32) {
     double are = 0.0, aim = 0.0;
     for (int k = tid & 31; k < nb; k += 32) {
       const cplx e = A.Esrc[(size_t)r * nb + k];
@@ -589,7 +575,7 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   // S5: V_SR[j] = sum_{k<=j} w[j-k] q[k].  Outputs j and nb-1-j are paired so that every thread does nb+1 terms;
   // each sum runs on four interleaved accumulators (k mod 4), so that the 8-cycle DFMA latency and the
   // shared-memory loads of consecutive terms overlap.
-  if (A.w && MBT_EXP_WAKE != 1) {
+  if (A.w) {
     for (int idx = tid; idx < (nb + 1) / 2; idx += kWakeThreads) {
       const int j1 = idx, j2 = nb - 1 - idx;
 #pragma unroll
@@ -642,7 +628,7 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   const int M = A.M, R = A.R, K = A.K;
   const int lane = tid & 31;
   const int run = (M + 31) / 32;  // consecutive bunches per lane
-  for (int r = tid >> 5; r < R && MBT_EXP_WAKE != 2; r += kWakeThreads / 32) {
+  for (int r = tid >> 5; r < R; r += kWakeThreads / 32) {
     // G_n = sum_{k=1..min(K,n-1)} A_{n-k} exp(lambda (k T0 - span)): lanes take k = lane+1, lane+33, ...
     cplx G{0.0, 0.0};
     for (int k = lane + 1; k <= K && (int64_t)n - k >= 1; k += 32)
