@@ -17,7 +17,8 @@
  *   P:l.98-115 bins, wake on each bin, kick Eq.(6a)
  *   P:l.123-125 per-bunch mean / rms statistics
  *   P:l.229-237 HOM-driven coupled-bunch motion (long-range resonator wake)
- * plus the readings D1..D30 of DESIGN.md where the paper is silent.
+ *   P:l.113     first / last occupied bin (read as: the bin window follows the bunch, reading D31)
+ * plus the readings D1..D31 of DESIGN.md where the paper is silent.
  */
 #ifndef ORC_H
 #define ORC_H
@@ -47,6 +48,7 @@ typedef struct {
   int32_t n_bins; double tau_lo_s, tau_hi_s; int32_t gather_order;
   int32_t n_res; const orc_resonator *res; int32_t history_turns;
   int32_t n_table; const double *sr_table;
+  int32_t window_mode; /* 0: fixed window (reading D11); 1: window follows the bunch in whole bins (reading D31) */
 } orc_wake;
 typedef struct {
   orc_ring ring; int32_t n_cav; const orc_cavity *cav; orc_radiation rad;
@@ -66,6 +68,12 @@ int orc_get_moment_log(orc_handle *h, int64_t first_turn, int64_t n, double *out
 /* source phasors a[b][n'][r] of the last K turns, oldest first: [K][M][R_lr][2] (re, im) */
 int orc_get_lr_history(orc_handle *h, double *out);
 int orc_set_lr_history(orc_handle *h, const double *in);
+/* window shifts in bins (reading D31): s_hist[M] = window of the current histogram / wake, s_next[M] = window the
+ * next turn will bin with; both 0 in window_mode 0 */
+int orc_get_window(orc_handle *h, int32_t *s_hist, int32_t *s_next);
+int orc_set_window(orc_handle *h, const int32_t *s_hist, const int32_t *s_next);
+/* the whole-bin shift that re-centres a histogram: rint(centroid in bins - n_bins / 2), exact integer arithmetic */
+int32_t orc_window_step(int32_t n_bins, const uint32_t *hist);
 int64_t orc_turn(const orc_handle *h);
 double orc_phi_s(const orc_handle *h);
 const char *orc_last_error(void);

@@ -55,7 +55,8 @@ class Resonator(C.Structure):
 class Wake(C.Structure):
     _fields_ = [("n_bins", C.c_int32), ("tau_lo_s", C.c_double), ("tau_hi_s", C.c_double),
                 ("gather_order", C.c_int32), ("n_res", C.c_int32), ("res", C.POINTER(Resonator)),
-                ("history_turns", C.c_int32), ("n_table", C.c_int32), ("sr_table", C.POINTER(C.c_double))]
+                ("history_turns", C.c_int32), ("n_table", C.c_int32), ("sr_table", C.POINTER(C.c_double)),
+                ("window_mode", C.c_int32)]
 
 
 class Params(C.Structure):
@@ -85,6 +86,11 @@ def lib():
         L.orc_get_moment_log.argtypes = [H, C.c_int64, C.c_int64, dp]
         L.orc_get_lr_history.argtypes = [H, dp]
         L.orc_set_lr_history.argtypes = [H, dp]
+        ip = C.POINTER(C.c_int32)
+        L.orc_get_window.argtypes = [H, ip, ip]
+        L.orc_set_window.argtypes = [H, ip, ip]
+        L.orc_window_step.argtypes = [C.c_int32, C.POINTER(C.c_uint32)]
+        L.orc_window_step.restype = C.c_int32
         L.orc_turn.argtypes = [H]
         L.orc_turn.restype = C.c_int64
         L.orc_phi_s.argtypes = [H]
@@ -120,6 +126,11 @@ def philox(ctr, key):
     o = (C.c_uint32 * 4)()
     lib().orc_philox4x32_10(c, k, o)
     return [int(x) for x in o]
+
+
+def window_step(hist):
+    h = np.ascontiguousarray(hist, dtype=np.uint32)
+    return int(lib().orc_window_step(h.size, h.ctypes.data_as(C.POINTER(C.c_uint32))))
 
 
 def normal_quad(seed, c0, c1, c2, c3):
@@ -174,7 +185,7 @@ class Oracle:
         p.fill = Fill(self.M, self._bucket, self._charge, self.Np, f["sigma_tau0_s"], f["sigma_delta0"])
         p.wake = Wake(self.nb, w["tau_lo_s"], w["tau_hi_s"], w["gather_order"], nres, self._res, w["history_turns"],
                       0 if self._tbl is None else len(self._tbl),
-                      None if self._tbl is None else _dp(self._tbl))
+                      None if self._tbl is None else _dp(self._tbl), int(w.get("window_mode", 0)))
         p.seed = cfg["seed"]
         p.log_capacity_turns = int(log_capacity_turns)
         p.lr_mode = int(lr_mode)
@@ -252,6 +263,20 @@ class Oracle:
         a = np.ascontiguousarray(a, dtype=np.float64)
         if a.size:
             self._ck(self._L.orc_set_lr_history(self._h, _dp(a)))
+
+    def window(self):
+        """(s_hist[M], s_next[M]): window shifts in bins (reading D31)."""
+        a = np.zeros(self.M, dtype=np.int32)
+        b = np.zeros(self.M, dtype=np.int32)
+        ip = C.POINTER(C.c_int32)
+        self._ck(self._L.orc_get_window(self._h, a.ctypes.data_as(ip), b.ctypes.data_as(ip)))
+        return a, b
+
+    def set_window(self, s_hist, s_next):
+        a = np.ascontiguousarray(s_hist, dtype=np.int32)
+        b = np.ascontiguousarray(s_next, dtype=np.int32)
+        ip = C.POINTER(C.c_int32)
+        self._ck(self._L.orc_set_window(self._h, a.ctypes.data_as(ip), b.ctypes.data_as(ip)))
 
     def map_one(self, tau, delta, z=0.0):
         t = C.c_double(tau)

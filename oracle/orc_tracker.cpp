@@ -172,6 +172,9 @@ struct orc_handle {
   int nb = 0;
   double tau_lo = 0, tau_hi = 0;
   int gather = 1;
+  int window_mode = 0;
+  int32_t s_max = 0;                      // |shift| <= s_max keeps the window inside the bucket
+  std::vector<int32_t> s_hist, s_next;    // [M] window shift in bins: of the current histogram / of the next binning
   std::vector<Resonator> res_lr;
   int K = 0;
   uint64_t seed = 0;
@@ -206,6 +209,26 @@ namespace {
 ldbl dt_between(const orc_handle *h, int64_t dn, int ds) {
   ldbl T0 = (ldbl)h->ring.T0_s;
   return (ldbl)dn * T0 + (ldbl)ds * (T0 / (ldbl)h->ring.h);
+}
+
+// Reading D31: the window of bunch b starts at tau_lo + s Delta, s an integer number of bins
+inline double window_lo(const orc_handle *h, int32_t s) {
+  double off = (double)s * h->Delta;
+  return h->tau_lo + off;
+}
+// centre of bin k of a window shifted by s bins
+inline double bin_centre(const orc_handle *h, int32_t s, int k) { return window_lo(h, s) + ((double)k + 0.5) * h->Delta; }
+
+// whole-bin step that brings the centroid of the counts back to the middle of the window:
+// rint((sum_k (k + 1/2) c_k) / n_in - n_b / 2), half up, in exact integer arithmetic; 0 for an empty histogram
+int32_t window_step(int nb, const uint32_t *c) {
+  int64_t n_in = 0, m1 = 0;
+  for (int k = 0; k < nb; ++k) { n_in += (int64_t)c[k]; m1 += (int64_t)k * (int64_t)c[k]; }
+  if (n_in == 0) return 0;
+  int64_t num = 2 * m1 + (2 - (int64_t)nb) * n_in, den = 2 * n_in;   // floor(num / den), den > 0
+  int64_t q = num / den;
+  if ((num % den != 0) && (num < 0)) q -= 1;
+  return (int32_t)q;
 }
 
 // steps 1-3 for one particle; z is the unit normal of step 2
@@ -255,7 +278,7 @@ void bin_all(orc_handle *h) {
     for (int64_t i = 0; i < h->Np; ++i) {
       size_t p = (size_t)b * h->Np + i;
       // 4. t = (tau - tau_lo) * invDelta; in-window iff 0 <= t < n_b; j = floor(t)
-      double t = (h->tau[p] - h->tau_lo) * h->invDelta;
+      double t = (h->tau[p] - window_lo(h, h->s_hist[b])) * h->invDelta;
       h->tpos[p] = t;
       if (t >= 0.0 && t < (double)h->nb) {
         int j = (int)std::floor(t);
@@ -285,8 +308,16 @@ void one_turn(orc_handle *h) {
       map_one(h, h->tau[p], h->delta[p], z);
     }
   }
-  // 4: bins
+  // 4: bins, on the window chosen after the previous turn (reading D31); then the window of the next turn
+  h->s_hist = h->s_next;
   bin_all(h);
+  if (h->window_mode == 1)
+    for (int b = 0; b < M; ++b) {
+      int64_t s = (int64_t)h->s_hist[b] + window_step(nb, &h->hist[(size_t)b * nb]);
+      if (s > h->s_max) s = h->s_max;
+      if (s < -(int64_t)h->s_max) s = -(int64_t)h->s_max;
+      h->s_next[b] = (int32_t)s;
+    }
   // 5: short-range wake, V_SR[b][j] = sum_{k<=j} w[j-k] q[b][k], q = (Q_b/N_p) hist
   std::vector<double> q((size_t)nb);
   for (int b = 0; b < M; ++b) {
@@ -310,7 +341,7 @@ void one_turn(orc_handle *h) {
         cplx a(0.0, 0.0);
         for (int k = 0; k < nb; ++k) {
           double qk = qm * (double)h->hist[(size_t)b * nb + k];
-          a += qk * std::exp(-lam * h->centre[k]);
+          a += qk * std::exp(-lam * bin_centre(h, h->s_hist[b], k));
         }
         h->a_at(n, b, r) = a;
       }
@@ -353,7 +384,7 @@ void one_turn(orc_handle *h) {
         for (int r = 0; r < R; ++r) {
           const Resonator &rs = h->res_lr[r];
           cplx lam(-rs.alpha, rs.wbar);
-          v += std::real(rs.C * std::exp(lam * h->centre[j]) * P[(size_t)b * R + r]);
+          v += std::real(rs.C * std::exp(lam * bin_centre(h, h->s_hist[b], j)) * P[(size_t)b * R + r]);
         }
         h->Vlr[(size_t)b * nb + j] = v;
       }
@@ -443,6 +474,7 @@ int orc_create(const orc_params *p, orc_handle **out) {
   if (!(wk.tau_hi_s > wk.tau_lo_s) || !((wk.tau_hi_s - wk.tau_lo_s) < rg.T0_s / rg.h))
     return fail(ORC_EINVAL, "window must satisfy 0 < tau_hi - tau_lo < T_rf");
   if (wk.gather_order != 0 && wk.gather_order != 1) return fail(ORC_EINVAL, "gather_order must be 0 or 1");
+  if (wk.window_mode != 0 && wk.window_mode != 1) return fail(ORC_EINVAL, "window_mode must be 0 or 1");
   if (wk.n_res < 0 || (wk.n_res > 0 && !wk.res)) return fail(ORC_EINVAL, "resonator list");
   if (wk.n_table < 0 || (wk.n_table > 0 && !wk.sr_table)) return fail(ORC_EINVAL, "sr_table");
   if (p->rad.enable && (!(p->rad.damping_turns > 0) || !(p->rad.sigma_delta >= 0)))
@@ -465,6 +497,7 @@ int orc_create(const orc_params *p, orc_handle **out) {
     h->tau_lo = wk.tau_lo_s;
     h->tau_hi = wk.tau_hi_s;
     h->gather = wk.gather_order;
+    h->window_mode = wk.window_mode;
     h->seed = p->seed;
     h->lr_mode = p->lr_mode;
     h->log_cap = p->log_capacity_turns;
@@ -518,6 +551,14 @@ int orc_create(const orc_params *p, orc_handle **out) {
     h->tau.resize(N); h->delta.resize(N); h->tpos.resize(N);
     h->hist.assign((size_t)h->M * h->nb, 0u);
     h->n_out.assign(h->M, 0);
+    h->s_hist.assign(h->M, 0);
+    h->s_next.assign(h->M, 0);
+    // the shifted window [tau_lo + s Delta, tau_hi + s Delta] stays inside the bucket [-T_rf/2, T_rf/2]
+    {
+      double room = std::fmin(0.5 * h->T_rf - h->tau_hi, h->tau_lo + 0.5 * h->T_rf);   // to the nearer bucket edge
+      double smax = std::floor(room / h->Delta);
+      h->s_max = (h->window_mode && smax > 0.0) ? (int32_t)std::fmin(smax, 1.0e6) : 0;
+    }
     h->Vsr.assign((size_t)h->M * h->nb, 0.0);
     h->Vlr.assign((size_t)h->M * h->nb, 0.0);
     h->V.assign((size_t)h->M * h->nb, 0.0);
@@ -592,6 +633,26 @@ int orc_set_particles(orc_handle *h, const double *tau, const double *delta, int
   compute_moments(h);
   return 0;
 }
+
+int orc_get_window(orc_handle *h, int32_t *s_hist, int32_t *s_next) {
+  if (!h) return fail(ORC_EINVAL, "null argument");
+  if (s_hist) std::memcpy(s_hist, h->s_hist.data(), sizeof(int32_t) * h->M);
+  if (s_next) std::memcpy(s_next, h->s_next.data(), sizeof(int32_t) * h->M);
+  return 0;
+}
+
+int orc_set_window(orc_handle *h, const int32_t *s_hist, const int32_t *s_next) {
+  if (!h || !s_hist || !s_next) return fail(ORC_EINVAL, "null argument");
+  for (int b = 0; b < h->M; ++b)
+    if (std::abs(s_hist[b]) > h->s_max || std::abs(s_next[b]) > h->s_max) return fail(ORC_EINVAL, "window shift beyond the bucket");
+  std::memcpy(h->s_hist.data(), s_hist, sizeof(int32_t) * h->M);
+  std::memcpy(h->s_next.data(), s_next, sizeof(int32_t) * h->M);
+  bin_all(h);
+  compute_moments(h);
+  return 0;
+}
+
+int32_t orc_window_step(int32_t n_bins, const uint32_t *hist) { return window_step(n_bins, hist); }
 
 int orc_get_histogram(orc_handle *h, uint32_t *out) {
   if (!h || !out) return fail(ORC_EINVAL, "null argument");
