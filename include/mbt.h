@@ -77,11 +77,16 @@ typedef struct { double Rs_ohm, fr_Hz, Q; uint32_t flags; } mbt_resonator;
 /* wake: n_bins half-open bins over [tau_lo, tau_hi) around every bucket centre (D11);
  * gather_order 1 = linear between bin centres (default), 0 = nearest grid point (P:l.98);
  * history_turns K: the long-range sum covers all bunches of turns n-K..n-1 and the earlier bunches of turn n;
- * sr_table (optional, n_table samples, V/C at lag k*Delta) is ADDED to the resonator table. */
+ * sr_table (optional, n_table samples, V/C at lag k*Delta) is ADDED to the resonator table;
+ * window_mode 0: the window is fixed (D11); 1: after each binning the window of a bunch moves by
+ * rint(centroid of its counts in bins - n_bins/2) whole bins, clamped inside the bucket, and the kick of a turn uses
+ * the window its wake was built on (D31; the paper's first / last occupied bin search, P:l.113, read as a window
+ * that follows the bunch). */
 typedef struct {
   int32_t n_bins; double tau_lo_s, tau_hi_s; int32_t gather_order;
   int32_t n_res; const mbt_resonator *res; int32_t history_turns;
   int32_t n_table; const double *sr_table;
+  int32_t window_mode;
 } mbt_wake;
 
 typedef struct {
@@ -132,6 +137,11 @@ int mbt_get_moment_log(mbt_handle *h, int64_t first_turn, int64_t n, double *out
 /* long-range source phasors a[b][n'][r] of the last K turns, oldest first, [K][M][R_lr][2] (re, im) */
 int mbt_get_lr_history(mbt_handle *h, double *out);
 int mbt_set_lr_history(mbt_handle *h, const double *in);
+/* window shifts in bins (D31), HOST arrays of M int32 (either may be NULL in the getter): s_hist = window of the
+ * current histogram and wake, s_next = window the next turn bins with.  mbt_set_particles resets both to 0; when
+ * resuming, call mbt_set_window after it (it re-bins the state; |shift| beyond the bucket -> MBT_EINVAL). */
+int mbt_get_window(mbt_handle *h, int32_t *s_hist, int32_t *s_next);
+int mbt_set_window(mbt_handle *h, const int32_t *s_hist, const int32_t *s_next);
 
 /* ---- introspection ---- */
 int64_t mbt_turn(const mbt_handle *h);        /* completed turns, -1 on NULL                 */

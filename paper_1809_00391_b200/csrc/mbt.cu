@@ -112,6 +112,12 @@ struct mbt_handle {
   DevBuf<cplx> Esrc, F, g_step, g_tail, g_hist, a_cur, ring_a, ring_A, P;
   DevBuf<uint32_t> hist, hist_last;
   DevBuf<unsigned long long> nout_acc;
+  DevBuf<int32_t> s_hist, s_next;
+  DevBuf<double> lo_hist, lo_next;
+  DevBuf<cplx> shift_src, shift_wit;
+  int window_mode = 0;
+  int32_t s_max = 0;
+  double tau_lo = 0.0, Delta = 0.0;
   DevBuf<Ctrl> ctrl;
   void (*fn_map)(const Args) = nullptr;    // k_pass<true, ...> chosen for this handle's effects
   void (*fn_flush)(const Args) = nullptr;  // k_pass<false, ...>
@@ -189,6 +195,8 @@ void destroy(mbt_handle *h) {
   h->qm.release(); h->w.release(); h->Vsr.release(); h->mom_acc.release(); h->mom_last.release(); h->mom_log.release();
   h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
   h->cellSR.release(); h->cellF.release();
+  h->s_hist.release(); h->s_next.release(); h->lo_hist.release(); h->lo_next.release();
+  h->shift_src.release(); h->shift_wit.release();
   h->Esrc.release(); h->F.release(); h->g_step.release(); h->g_tail.release(); h->g_hist.release(); h->a_cur.release();
   h->ring_a.release(); h->ring_A.release(); h->P.release(); h->logtab.release();
   h->hist.release(); h->hist_last.release(); h->nout_acc.release(); h->ctrl.release();
@@ -196,6 +204,25 @@ void destroy(mbt_handle *h) {
   delete h;
 }
 
+}  // namespace
+
+namespace {
+int upload_window(mbt_handle *h, const int32_t *s_hist, const int32_t *s_next) {
+  std::vector<double> lh(h->M), ln(h->M);
+  for (int b = 0; b < h->M; ++b) {
+    double off_h = (double)s_hist[b] * h->Delta, off_n = (double)s_next[b] * h->Delta;
+    lh[b] = h->tau_lo + off_h;
+    ln[b] = h->tau_lo + off_n;
+    if (lh[b] == 0.0) lh[b] = -0.0;
+    if (ln[b] == 0.0) ln[b] = -0.0;
+  }
+  CU(cudaMemcpyAsync(h->s_hist.p, s_hist, sizeof(int32_t) * h->M, cudaMemcpyHostToDevice, h->stream));
+  CU(cudaMemcpyAsync(h->s_next.p, s_next, sizeof(int32_t) * h->M, cudaMemcpyHostToDevice, h->stream));
+  CU(cudaMemcpyAsync(h->lo_hist.p, lh.data(), sizeof(double) * h->M, cudaMemcpyHostToDevice, h->stream));
+  CU(cudaMemcpyAsync(h->lo_next.p, ln.data(), sizeof(double) * h->M, cudaMemcpyHostToDevice, h->stream));
+  CU(cudaStreamSynchronize(h->stream));  // the host vectors go out of scope
+  return 0;
+}
 }  // namespace
 
 extern "C" {
@@ -231,6 +258,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   if (!(wk.tau_hi_s > wk.tau_lo_s) || !((wk.tau_hi_s - wk.tau_lo_s) < rg.T0_s / rg.h))
     return fail(MBT_EINVAL, "window must satisfy 0 < tau_hi - tau_lo < T_rf");
   if (wk.gather_order != 0 && wk.gather_order != 1) return fail(MBT_EINVAL, "gather_order must be 0 or 1");
+  if (wk.window_mode != 0 && wk.window_mode != 1) return fail(MBT_EINVAL, "window_mode must be 0 or 1");
   if (wk.n_res < 0 || (wk.n_res > 0 && !wk.res)) return fail(MBT_EINVAL, "resonator list");
   if (wk.n_table < 0 || (wk.n_table > 0 && !wk.sr_table)) return fail(MBT_EINVAL, "sr_table");
   if (p->rad.enable && (!(p->rad.damping_turns > 0) || !(p->rad.sigma_delta >= 0)))
@@ -321,7 +349,6 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   A.drift = rg.alpha_c * rg.T0_s;
   A.nb = nb;
   A.gather = wk.gather_order;
-  A.tau_lo = (wk.tau_lo_s == 0.0) ? -0.0 : wk.tau_lo_s;  // see in_window()
   A.invDelta = (double)nb / (wk.tau_hi_s - wk.tau_lo_s);
   A.nb_d = (double)nb;
   A.invE0 = 1.0 / E0;
@@ -414,6 +441,34 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     CUH(h->cellF.upload(cf));
   }
   CUH(h->cellSR.alloc((size_t)M * (nb + 2)));
+  // ---- bunch-following window (D31): shifts in whole bins, |s| <= s_max keeps the window inside the bucket
+  h->window_mode = wk.window_mode;
+  h->tau_lo = wk.tau_lo_s;
+  h->Delta = Delta;
+  {
+    const double T_rf = rg.T0_s / (double)rg.h;
+    const double room = std::fmin(0.5 * T_rf - wk.tau_hi_s, wk.tau_lo_s + 0.5 * T_rf);  // to the nearer bucket edge
+    const double smax = std::floor(room / Delta);
+    h->s_max = (wk.window_mode && smax > 0.0) ? (int32_t)std::fmin(smax, 1.0e6) : 0;
+    std::vector<double> lo0(M, (wk.tau_lo_s == 0.0) ? -0.0 : wk.tau_lo_s);  // 0 stored as -0.0: see in_window()
+    CUH(h->lo_hist.upload(lo0));
+    CUH(h->lo_next.upload(lo0));
+    CUH(h->s_hist.alloc(M));
+    CUH(h->s_next.alloc(M));
+    if (wk.window_mode && R > 0) {
+      const int W = 2 * h->s_max + 1;
+      std::vector<cplx> ss((size_t)R * W), sw((size_t)R * W);
+      for (int r = 0; r < R; ++r)
+        for (int i = 0; i < W; ++i) {
+          const ldbl t = (ldbl)(i - h->s_max) * (ldbl)Delta;
+          const ldbl mg = expl(lr[r].alpha * t), ph = lr[r].wbar * t;
+          ss[(size_t)r * W + i] = cplx{(double)(mg * cosl(ph)), (double)(-mg * sinl(ph))};               // exp(-lambda t)
+          sw[(size_t)r * W + i] = cplx{(double)(cosl(ph) / mg), (double)(sinl(ph) / mg)};                // exp(+lambda t)
+        }
+      CUH(h->shift_src.upload(ss));
+      CUH(h->shift_wit.upload(sw));
+    }
+  }
   CUH(h->g_step.upload(g_step));
   CUH(h->g_tail.upload(g_tail));
   CUH(h->g_hist.upload(g_hist));
@@ -439,6 +494,8 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   A.cellSR = h->cellSR.p;
   A.cellF = h->cellF.p;
   A.hist = h->hist.p;
+  A.lo_hist = h->lo_hist.p;
+  A.lo_next = h->lo_next.p;
   A.mom_acc = h->mom_acc.p;
   A.nout_acc = h->nout_acc.p;
   A.ctrl = h->ctrl.p;
@@ -453,6 +510,9 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   Wa.Esrc = h->Esrc.p; Wa.g_step = h->g_step.p; Wa.g_tail = h->g_tail.p; Wa.g_hist = h->g_hist.p;
   Wa.hist = h->hist.p; Wa.hist_last = h->hist_last.p; Wa.Vsr = h->Vsr.p;
   Wa.cellSR = h->cellSR.p; Wa.gather = wk.gather_order;
+  Wa.window_mode = wk.window_mode; Wa.s_max = h->s_max; Wa.tau_lo = wk.tau_lo_s; Wa.Delta = Delta;
+  Wa.s_hist = h->s_hist.p; Wa.s_next = h->s_next.p; Wa.lo_hist = h->lo_hist.p; Wa.lo_next = h->lo_next.p;
+  Wa.shift_src = h->shift_src.p; Wa.shift_wit = h->shift_wit.p;
   Wa.a_cur = h->a_cur.p; Wa.ring_a = h->ring_a.p; Wa.ring_A = h->ring_A.p; Wa.P = h->P.p;
   Wa.mom_acc = h->mom_acc.p; Wa.nout_acc = h->nout_acc.p; Wa.mom_last = h->mom_last.p;
   Wa.mom_log = h->log_cap > 0 ? h->mom_log.p : nullptr;
@@ -638,6 +698,11 @@ int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int
     k_unpack<<<grid, 256, 0, h->stream>>>(h->scratch_a.p, h->ld, (uint32_t)h->Np, h->d_delta);
     h->launches += 2;
   }
+  {
+    std::vector<int32_t> zero(h->M, 0);
+    int rc = upload_window(h, zero.data(), zero.data());
+    if (rc) return rc;
+  }
   k_set_ctrl<<<1, 1, 0, h->stream>>>(h->ctrl.p, (uint32_t)turn, 0u);
   h->launches += 1;
   CU(cudaMemsetAsync(h->hist.p, 0, sizeof(uint32_t) * h->M * h->nb, h->stream));
@@ -649,6 +714,26 @@ int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int
   h->turn = turn;
   h->dirty = true;
   h->wake_valid = false;
+  return 0;
+}
+
+int mbt_get_window(mbt_handle *h, int32_t *s_hist, int32_t *s_next) {
+  if (!h) return fail(MBT_EINVAL, "null argument");
+  CU(cudaSetDevice(h->device));
+  if (s_hist) CU(cudaMemcpyAsync(s_hist, h->s_hist.p, sizeof(int32_t) * h->M, cudaMemcpyDeviceToHost, h->stream));
+  if (s_next) CU(cudaMemcpyAsync(s_next, h->s_next.p, sizeof(int32_t) * h->M, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_set_window(mbt_handle *h, const int32_t *s_hist, const int32_t *s_next) {
+  if (!h || !s_hist || !s_next) return fail(MBT_EINVAL, "null argument");
+  CU(cudaSetDevice(h->device));
+  for (int b = 0; b < h->M; ++b)
+    if (std::abs(s_hist[b]) > h->s_max || std::abs(s_next[b]) > h->s_max) return fail(MBT_EINVAL, "window shift beyond the bucket");
+  int rc = upload_window(h, s_hist, s_next);
+  if (rc) return rc;
+  h->dirty = true;  // counts and n_in / n_out are re-derived on the new window by the next flush
   return 0;
 }
 

@@ -79,7 +79,9 @@ struct Args {
   // S4 / S0
   int32_t nb;
   int32_t gather;
-  double tau_lo, invDelta, nb_d, invE0;
+  const double *lo_hist;  // [M] start of the window the current histogram / wake was built on (S0 reads it)
+  const double *lo_next;  // [M] start of the window this pass bins with (S4); equal to lo_hist unless window_mode 1 (D31)
+  double invDelta, nb_d, invE0;
   // wake state
   const double *Vsr;    // [M][nb]   short-range wake of the last turn [V]
   const cplx *P;        // [M][R]    long-range phasor seen by bunch b
@@ -151,7 +153,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 
 // 0 <= t < nb decided on the high word of t: nb < 2^21 is an integer, so the low word of (double)nb is zero and
 // t >= nb  <=>  hi(t) >= hi(nb) for t >= +0; a negative t (sign bit) or a NaN compares above hi(nb) as unsigned.
-// t = -0.0 cannot occur: the host stores tau_lo = 0 as -0.0, so that (-0.0) - tau_lo = +0.0 (in the window, bin 0,
+// t = -0.0 cannot occur: a window start of 0 is stored as -0.0, so that (-0.0) - lo = +0.0 (in the window, bin 0,
 // as the oracle's t >= 0 decides) and every other difference is unchanged.
 __device__ __forceinline__ bool in_window(double t, uint32_t hi_nb) { return (uint32_t)__double2hiint(t) < hi_nb; }
 
@@ -204,6 +206,10 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
     const int b = (int)blockIdx.y;
     const uint32_t p0 = blockIdx.x * A.tile_pairs;
     const uint32_t p1 = (A.ppb - p0 < A.tile_pairs) ? A.ppb : p0 + A.tile_pairs;
+
+    // window of the wake being applied (S0) and window this pass bins with (S4); the flush pass re-bins on the former
+    const double lo_old = A.lo_hist[b];
+    const double lo_new = MAP ? A.lo_next[b] : lo_old;
 
     // chunk k of the tile = pairs [p0 + k STRIDE, + STRIDE) clipped to p1; it lives in stage k % kStages
     const uint32_t n_it = (p1 - p0 + STRIDE - 1u) / STRIDE;
@@ -316,7 +322,7 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
       bool in[NP];
 #pragma unroll
       for (int i = 0; i < NP; ++i) {
-        t[i] = __dmul_rn(__dsub_rn(tau[i], A.tau_lo), A.invDelta);
+        t[i] = __dmul_rn(__dsub_rn(tau[i], lo_old), A.invDelta);
         in[i] = live[i] && in_window(t[i], hi_nb);
         int kk;
         double f;
@@ -406,7 +412,7 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
           del[i] -= A.loss;
           if (RAD) del[i] = fma(del[i], A.one_minus_DE, z[i]);  // S2 (z already scaled by sigma_delta sqrt(2 D_E))
           tau[i] = fma(A.drift, del[i], tau[i]);                // S3
-          t[i] = __dmul_rn(__dsub_rn(tau[i], A.tau_lo), A.invDelta);  // S4
+          t[i] = __dmul_rn(__dsub_rn(tau[i], lo_new), A.invDelta);  // S4
           in[i] = live[i] && in_window(t[i], hi_nb);
         }
       }
@@ -478,6 +484,13 @@ struct WakeArgs {
   double *Vsr;             // [M][nb]
   WakeCell *cellSR;        // [M][nb+2] gather cells of Vsr (what the pass stages)
   int32_t gather;          // 1 linear, 0 nearest grid point
+  // bunch-following window (D31); window_mode 0: the arrays below keep their initial values
+  int32_t window_mode, s_max;
+  double tau_lo, Delta;
+  int32_t *s_hist, *s_next;   // [M] window shift in bins: of this turn's histogram / of the next binning
+  double *lo_hist, *lo_next;  // [M] tau_lo + s Delta (0 stored as -0.0, see in_window())
+  const cplx *shift_src;      // [R][2 s_max + 1] exp(-lambda_r s Delta), s = -s_max..s_max
+  const cplx *shift_wit;      // [R][2 s_max + 1] exp(+lambda_r s Delta)
   cplx *a_cur;             // [M][R]   source phasors of this turn
   cplx *ring_a;            // [K+1][M][R] slot n % (K+1)
   cplx *ring_A;            // [K+1][R]    per-turn aggregates, slot n % (K+1)
@@ -510,6 +523,7 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   double *sw = smem_d + A.nb;  // [nb] wake table
   double *sv = smem_d + 2 * A.nb;  // [nb] V_SR of this bunch
   __shared__ bool s_last;
+  __shared__ unsigned long long s_cnt[kWakeThreads / 32][2];
 
   const int tid = threadIdx.x;
   const int b = blockIdx.x;
@@ -519,14 +533,49 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
 
   // counts -> charges; keep a copy of the counts; clear the accumulator for the next pass
   const double qm = A.qm[b];
+  const bool follow = A.mode == 0 && A.window_mode == 1;
+  const int32_t s_used = follow ? A.s_next[b] : 0;   // the window the pass binned this turn with
+  unsigned long long n_in = 0ull, m1 = 0ull;         // sum c_k, sum k c_k
   for (int j = tid; j < nb; j += kWakeThreads) {
     const uint32_t c = A.hist[(size_t)b * nb + j];
     A.hist_last[(size_t)b * nb + j] = c;
     A.hist[(size_t)b * nb + j] = 0u;
     sq[j] = qm * (double)c;
+    n_in += c;
+    m1 += (unsigned long long)j * c;
     if (A.mode == 0 && A.w) sw[j] = A.w[j];
   }
+  if (follow) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      n_in += __shfl_down_sync(0xffffffffu, n_in, o);
+      m1 += __shfl_down_sync(0xffffffffu, m1, o);
+    }
+    if ((tid & 31) == 0) { s_cnt[tid >> 5][0] = n_in; s_cnt[tid >> 5][1] = m1; }
+  }
   __syncthreads();
+  if (follow && tid == 0) {
+    // D31: the window moves by rint(centroid in bins - nb/2) whole bins (half up), exact integer arithmetic
+    long long N = 0, S1 = 0;
+#pragma unroll
+    for (int w = 0; w < kWakeThreads / 32; ++w) { N += (long long)s_cnt[w][0]; S1 += (long long)s_cnt[w][1]; }
+    long long step = 0;
+    if (N > 0) {
+      const long long num = 2 * S1 + (2 - (long long)nb) * N, den = 2 * N;
+      step = num / den;
+      if (num % den != 0 && num < 0) step -= 1;
+    }
+    long long s_new = (long long)s_used + step;
+    s_new = s_new > A.s_max ? A.s_max : (s_new < -(long long)A.s_max ? -(long long)A.s_max : s_new);
+    double lo_h = __dadd_rn(A.tau_lo, __dmul_rn((double)s_used, A.Delta));
+    double lo_n = __dadd_rn(A.tau_lo, __dmul_rn((double)s_new, A.Delta));
+    if (lo_h == 0.0) lo_h = -0.0;
+    if (lo_n == 0.0) lo_n = -0.0;
+    A.s_hist[b] = s_used;
+    A.lo_hist[b] = lo_h;
+    A.s_next[b] = (int32_t)s_new;
+    A.lo_next[b] = lo_n;
+  }
   // S7: close the moments the pass gathered (state after turn n_done's kick)
   // by the last thread of the CTA: its warp has no convolution work unless nb > 448, so this serial stretch
   // (a division, two square roots) runs beside the convolution instead of ahead of it
@@ -566,7 +615,8 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
       aim += __shfl_xor_sync(0xffffffffu, aim, o);
     }
     if ((tid & 31) == 0) {
-      const cplx a{are, aim};
+      cplx a{are, aim};
+      if (follow) a = cmul(a, A.shift_src[(size_t)r * (2 * A.s_max + 1) + (s_used + A.s_max)]);  // bin centres at their own window
       A.a_cur[(size_t)b * A.R + r] = a;
       A.ring_a[((size_t)(n % (uint32_t)(A.K + 1)) * A.M + b) * A.R + r] = a;
     }
@@ -686,7 +736,8 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
       for (int u = 0; u < 4; ++u) {
         const int j = j0 + u;
         if (j < j_hi) {
-          A.P[(size_t)j * R + r] = Pj;
+          // the phasor as bunch j's own window sees it: the pass expands Re[cellF_r P], cellF built on the unshifted grid
+          A.P[(size_t)j * R + r] = follow ? cmul(Pj, A.shift_wit[(size_t)r * (2 * A.s_max + 1) + (__ldcg(&A.s_hist[j]) + A.s_max)]) : Pj;
           if (j + 1 < M) Pj = cmul(cadd(Pj, a[u]), gs[u]);
         }
       }

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libmbt.so")
 # every symbol include/mbt.h declares (tests check that the library exports all of them)
 SYMBOLS = [
     "mbt_create", "mbt_track", "mbt_moments", "mbt_destroy", "mbt_get_particles", "mbt_set_particles",
-    "mbt_get_histogram", "mbt_get_wake", "mbt_get_moment_log", "mbt_get_lr_history", "mbt_set_lr_history",
+    "mbt_get_histogram", "mbt_get_wake", "mbt_get_moment_log", "mbt_get_lr_history", "mbt_set_lr_history", "mbt_get_window", "mbt_set_window",
     "mbt_turn", "mbt_phi_s", "mbt_particle_stride", "mbt_device_pointers", "mbt_launch_count",
     "mbt_last_track_seconds", "mbt_track_profiled", "mbt_philox_selftest", "mbt_normal_selftest", "mbt_last_error", "mbt_version",
 ]
@@ -48,7 +48,8 @@ class Resonator(C.Structure):
 class Wake(C.Structure):
     _fields_ = [("n_bins", C.c_int32), ("tau_lo_s", C.c_double), ("tau_hi_s", C.c_double),
                 ("gather_order", C.c_int32), ("n_res", C.c_int32), ("res", C.POINTER(Resonator)),
-                ("history_turns", C.c_int32), ("n_table", C.c_int32), ("sr_table", C.POINTER(C.c_double))]
+                ("history_turns", C.c_int32), ("n_table", C.c_int32), ("sr_table", C.POINTER(C.c_double)),
+                ("window_mode", C.c_int32)]
 
 
 class Params(C.Structure):
@@ -98,6 +99,8 @@ def lib():
         L.mbt_last_track_seconds.argtypes = [H]
         L.mbt_last_track_seconds.restype = C.c_double
         L.mbt_track_profiled.argtypes = [H, C.c_int64, dp, dp]
+        L.mbt_get_window.argtypes = [H, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        L.mbt_set_window.argtypes = [H, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.mbt_philox_selftest.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.mbt_normal_selftest.argtypes = [C.c_uint64, C.c_int64, C.POINTER(C.c_uint32), dp]
         L.mbt_last_error.restype = C.c_char_p
@@ -152,7 +155,8 @@ def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None
     p.rad = Radiation(**cfg["radiation"])
     p.fill = Fill(m, bucket, charge, int(f["n_per_bunch"]), f["sigma_tau0_s"], f["sigma_delta0"])
     p.wake = Wake(int(w["n_bins"]), w["tau_lo_s"], w["tau_hi_s"], int(w["gather_order"]), nres, res,
-                  int(w["history_turns"]), 0 if tbl is None else len(tbl), None if tbl is None else _dp(tbl))
+                  int(w["history_turns"]), 0 if tbl is None else len(tbl), None if tbl is None else _dp(tbl),
+                  int(w.get("window_mode", 0)))
     p.seed = int(cfg["seed"])
     p.log_capacity_turns = int(log_capacity_turns)
     p.d_tau = d_tau
@@ -271,6 +275,20 @@ class Tracker:
         a = np.ascontiguousarray(a, dtype=np.float64)
         if a.size:
             _ck(self._L.mbt_set_lr_history(self._h, _dp(a)))
+
+    def window(self):
+        """(s_hist[M], s_next[M]): window shifts in bins (reading D31)."""
+        a = np.zeros(self.M, dtype=np.int32)
+        b = np.zeros(self.M, dtype=np.int32)
+        ip = C.POINTER(C.c_int32)
+        _ck(self._L.mbt_get_window(self._h, a.ctypes.data_as(ip), b.ctypes.data_as(ip)))
+        return a, b
+
+    def set_window(self, s_hist, s_next):
+        a = np.ascontiguousarray(s_hist, dtype=np.int32)
+        b = np.ascontiguousarray(s_next, dtype=np.int32)
+        ip = C.POINTER(C.c_int32)
+        _ck(self._L.mbt_set_window(self._h, a.ctypes.data_as(ip), b.ctypes.data_as(ip)))
 
     def device_pointers(self):
         t, d, ld = C.c_void_p(), C.c_void_p(), C.c_int64()

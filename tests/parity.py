@@ -30,7 +30,7 @@ def wake_error(v_gpu, v_cpu):
     return float(np.max(np.abs(v_gpu - v_cpu) / scale))
 
 
-def histogram_mismatch(h_gpu, h_cpu, tau_cpu, cfg):
+def histogram_mismatch(h_gpu, h_cpu, tau_cpu, cfg, shifts=None):
     """Counts must be bit-exact, except for particles within TOL_EDGE (bin units) of a bin edge.
 
     Returns (n_mismatching_bins, n_edge_particles).  Raises if the mismatch cannot be explained by
@@ -42,7 +42,10 @@ def histogram_mismatch(h_gpu, h_cpu, tau_cpu, cfg):
     w = cfg["wake"]
     nb = w["n_bins"]
     inv = nb / (w["tau_hi_s"] - w["tau_lo_s"])
-    t = (np.asarray(tau_cpu) - w["tau_lo_s"]) * inv
+    lo = w["tau_lo_s"]
+    if shifts is not None:
+        lo = lo + np.asarray(shifts, dtype=np.float64)[:, None] * ((w["tau_hi_s"] - w["tau_lo_s"]) / nb)
+    t = (np.asarray(tau_cpu) - lo) * inv
     edge = np.abs(t - np.rint(t)) < TOL_EDGE * np.maximum(1.0, np.abs(t))
     n_edge = int(np.count_nonzero(edge))
     if bad:
@@ -51,17 +54,19 @@ def histogram_mismatch(h_gpu, h_cpu, tau_cpu, cfg):
     return bad, n_edge
 
 
-def resume_on_gpu(o, trk):
+def resume_on_gpu(o, trk, cfg=None):
     """Upload the oracle's current state (particles, turn, long-range history) into the GPU tracker."""
     tau, delta = o.particles()
     trk.set_particles(tau, delta, o.turn)
+    if cfg is not None and cfg["wake"].get("window_mode", 0):
+        trk.set_window(*o.window())                 # after set_particles (which resets the shifts)
     trk.set_lr_history(o.lr_history())
     return tau, delta
 
 
 def assert_single_turn_parity(o, trk, cfg, turns=1, tol_particle=TOL_PARTICLE, tol_wake=TOL_WAKE):
     """Both sides advance `turns` turns from the oracle's current state; everything observable is compared."""
-    resume_on_gpu(o, trk)
+    resume_on_gpu(o, trk, cfg)
     o.track(turns)
     trk.track(turns)
     tau_c, delta_c = o.particles()
@@ -70,7 +75,10 @@ def assert_single_turn_parity(o, trk, cfg, turns=1, tol_particle=TOL_PARTICLE, t
     e_delta = particle_errors(delta_g, delta_c)
     assert e_tau <= tol_particle, "tau differs by %.3e (relative, D23)" % e_tau
     assert e_delta <= tol_particle, "delta differs by %.3e (relative, D23)" % e_delta
-    bad, n_edge = histogram_mismatch(trk.histogram(), o.histogram(), tau_c, cfg)
+    sh_c, sn_c = o.window()
+    sh_g, sn_g = trk.window()
+    assert np.array_equal(sh_c, sh_g) and np.array_equal(sn_c, sn_g), "window shifts differ (D31)"
+    bad, n_edge = histogram_mismatch(trk.histogram(), o.histogram(), tau_c, cfg, shifts=sh_c)
     tot_c, sr_c, lr_c = o.wake()
     tot_g, sr_g, lr_g = trk.wake()
     if bad == 0:

@@ -169,6 +169,40 @@ def test_user_sampled_wake_table(mbt, orc):
             assert np.abs(t.wake()[1]).max() > 0
 
 
+def test_bunch_following_window(mbt, orc):
+    """window_mode 1 (reading D31): bunches displaced from their bucket centres, every window moving in whole bins;
+    single-turn parity incl. the shifts, then ten turns without re-synchronisation."""
+    cfg = W.tiny(m=4, n_per_bunch=3001, n_bins=32, k_hist=3, n_lr=2)
+    cfg["wake"]["window_mode"] = 1
+    o = orc.Oracle(cfg)
+    tau, delta = o.particles()
+    off = np.array([[12e-12], [-20e-12], [0.0], [45e-12]])
+    o.set_particles(tau * 0.5 + off, delta, 0)
+    o.track(2)
+    with mbt.Tracker(cfg) as t:
+        for _ in range(4):
+            assert_single_turn_parity(o, t, cfg)
+        assert len(set(int(s) for s in t.window()[0])) >= 3
+        # own runs from the same displaced start, no re-synchronisation
+        o2 = orc.Oracle(cfg)
+        o2.set_particles(tau * 0.5 + off, delta, 0)
+        t.set_particles(tau * 0.5 + off, delta, 0)
+        o2.track(10)
+        t.track(10)
+        assert np.array_equal(o2.window()[0], t.window()[0]) and np.array_equal(o2.window()[1], t.window()[1])
+        assert np.array_equal(o2.histogram(), t.histogram())
+        assert particle_errors(t.particles()[1], o2.particles()[1]) <= 1e-10
+        assert wake_error(t.wake()[0], o2.wake()[0]) <= 1e-9
+        m_c, m_g = o2.moments(), t.moments()
+        assert np.array_equal(m_c[:, :2], m_g[:, :2]) and np.all(m_g[:, 1] < 0.01 * 3001)
+    # the same start in a fixed window loses the displaced tails
+    cfg0 = W.tiny(m=4, n_per_bunch=3001, n_bins=32, k_hist=3, n_lr=2)
+    with mbt.Tracker(cfg0) as t0:
+        t0.set_particles(tau * 0.5 + off, delta, 0)
+        t0.track(10)
+        assert t0.moments()[3, 1] > 0.10 * 3001          # the bunch at +45 ps, sigma 5 ps: Phi(-1) = 16 % beyond +50 ps
+
+
 def test_several_turns_without_resync(mbt, orc):
     """Nine turns from each side's OWN initial distribution and no re-synchronisation: the fused ordering
     (kick at the head of the next pass) reproduces the sequential order of the paper."""
