@@ -113,6 +113,8 @@ struct mbt_handle {
   DevBuf<uint32_t> hist, hist_last;
   DevBuf<unsigned long long> nout_acc;
   DevBuf<int32_t> s_hist, s_next;
+  DevBuf<uint32_t> rd_cnt, wr_cnt;
+  int wake_splits = 1;
   DevBuf<double> lo_hist, lo_next;
   DevBuf<cplx> shift_src, shift_wit;
   int window_mode = 0;
@@ -150,7 +152,7 @@ pass_fn select_flush(int gather) {
 
 int enqueue_turn(mbt_handle *h) {
   h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
-  k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
+  k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
   return 0;
 }
 
@@ -172,6 +174,7 @@ int flush(mbt_handle *h) {
   h->fn_flush<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
   WakeArgs wa = h->wargs;
   wa.mode = 1;
+  wa.S = 1;
   k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(wa);
   k_clear_pending<<<1, 1, 0, h->stream>>>(h->ctrl.p);
   h->launches += 3;
@@ -195,6 +198,7 @@ void destroy(mbt_handle *h) {
   h->qm.release(); h->w.release(); h->Vsr.release(); h->mom_acc.release(); h->mom_last.release(); h->mom_log.release();
   h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
   h->cellSR.release(); h->cellF.release();
+  h->rd_cnt.release(); h->wr_cnt.release();
   h->s_hist.release(); h->s_next.release(); h->lo_hist.release(); h->lo_next.release();
   h->shift_src.release(); h->shift_wit.release();
   h->Esrc.release(); h->F.release(); h->g_step.release(); h->g_tail.release(); h->g_hist.release(); h->a_cur.release();
@@ -505,6 +509,18 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   WakeArgs &Wa = h->wargs;
   memset(&Wa, 0, sizeof Wa);
   Wa.M = M; Wa.nb = nb; Wa.R = R; Wa.K = K; Wa.Np = (uint32_t)h->Np; Wa.mode = 0;
+  {  // few bunches: deal the convolution of a bunch out over S CTAs (a warp of output pairs each, <= 2 waves of CTAs)
+    const int pairs = (nb + 1) / 2;
+    int S = (pairs + 31) / 32;
+    const int room = (2 * prop.multiProcessorCount + M - 1) / M;
+    if (S > room) S = room;
+    if (S > 64) S = 64;
+    if (S < 1) S = 1;
+    h->wake_splits = S;
+  }
+  CUH(h->rd_cnt.alloc(M));
+  CUH(h->wr_cnt.alloc(M));
+  Wa.S = h->wake_splits; Wa.rd_cnt = h->rd_cnt.p; Wa.wr_cnt = h->wr_cnt.p;
   Wa.qm = h->qm.p;
   Wa.w = have_sr ? h->w.p : nullptr;
   Wa.Esrc = h->Esrc.p; Wa.g_step = h->g_step.p; Wa.g_tail = h->g_tail.p; Wa.g_hist = h->g_hist.p;
@@ -605,7 +621,7 @@ int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, dou
     CU(cudaEventRecord(ev[3 * t], h->stream));
     h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
     CU(cudaEventRecord(ev[3 * t + 1], h->stream));
-    k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
+    k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
     CU(cudaEventRecord(ev[3 * t + 2], h->stream));
   }
   CU(cudaEventRecord(h->ev1, h->stream));

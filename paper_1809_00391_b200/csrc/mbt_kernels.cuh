@@ -471,6 +471,8 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
 // ------------------------------------------------------------------ wake
 struct WakeArgs {
   int32_t M, nb, R, K;
+  int32_t S;               // CTAs per bunch (grid.y): the outputs of the convolution are dealt out over them
+  uint32_t *rd_cnt, *wr_cnt;  // [M] splits that have read the counts / written their share of V_SR (S > 1)
   uint32_t Np;
   int32_t mode;            // 0: full turn (S5, S6, bump the turn counter); 1: finalise counts and moments only
   const double *qm;        // [M]      macro-particle charge Q_b / N_p
@@ -527,6 +529,7 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
 
   const int tid = threadIdx.x;
   const int b = blockIdx.x;
+  const int split = blockIdx.y, S = A.S;  // few bunches: S CTAs share a bunch (split 0 also does the per-bunch work)
   const int nb = A.nb;
   const uint32_t n_done = A.ctrl->turn;  // completed turns; the turn being closed is n_done + 1
   const uint32_t n = n_done + 1u;
@@ -538,14 +541,23 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   unsigned long long n_in = 0ull, m1 = 0ull;         // sum c_k, sum k c_k
   for (int j = tid; j < nb; j += kWakeThreads) {
     const uint32_t c = A.hist[(size_t)b * nb + j];
-    A.hist_last[(size_t)b * nb + j] = c;
-    A.hist[(size_t)b * nb + j] = 0u;
+    if (split == 0) A.hist_last[(size_t)b * nb + j] = c;
+    if (S == 1) A.hist[(size_t)b * nb + j] = 0u;
     sq[j] = qm * (double)c;
     n_in += c;
     m1 += (unsigned long long)j * c;
     if (A.mode == 0 && A.w) sw[j] = A.w[j];
   }
-  if (follow) {
+  if (S > 1) {  // the last split to have read the counts clears them (nobody waits for anybody)
+    __syncthreads();
+    if (tid == 0) s_last = (atomicAdd(&A.rd_cnt[b], 1u) == (uint32_t)(S - 1));
+    __syncthreads();
+    if (s_last) {
+      for (int j = tid; j < nb; j += kWakeThreads) A.hist[(size_t)b * nb + j] = 0u;
+      if (tid == 0) A.rd_cnt[b] = 0u;
+    }
+  }
+  if (follow && split == 0) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       n_in += __shfl_down_sync(0xffffffffu, n_in, o);
@@ -554,7 +566,7 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
     if ((tid & 31) == 0) { s_cnt[tid >> 5][0] = n_in; s_cnt[tid >> 5][1] = m1; }
   }
   __syncthreads();
-  if (follow && tid == 0) {
+  if (follow && split == 0 && tid == 0) {
     // D31: the window moves by rint(centroid in bins - nb/2) whole bins (half up), exact integer arithmetic
     long long N = 0, S1 = 0;
 #pragma unroll
@@ -579,7 +591,7 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   // S7: close the moments the pass gathered (state after turn n_done's kick)
   // by the last thread of the CTA: its warp has no convolution work unless nb > 448, so this serial stretch
   // (a division, two square roots) runs beside the convolution instead of ahead of it
-  if (tid == kWakeThreads - 1) {
+  if (split == 0 && tid == kWakeThreads - 1) {
     const double N = (double)A.Np;
     const double s1 = A.mom_acc[b * 4 + 0], s2 = A.mom_acc[b * 4 + 1];
     const double s11 = A.mom_acc[b * 4 + 2], s22 = A.mom_acc[b * 4 + 3];
@@ -602,7 +614,7 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
 
   // S6 sources: a[b][r] = sum_k q[k] exp(-lambda_r c_k).  One warp per resonator (shuffles only, no block
   // barrier); the other warps go straight to the convolution.
-  for (int r = tid >> 5; r < A.R; r += kWakeThreads / 32) {
+  for (int r = tid >> 5; r < A.R && split == 0; r += kWakeThreads / 32) {
     double are = 0.0, aim = 0.0;
     for (int k = tid & 31; k < nb; k += 32) {
       const cplx e = A.Esrc[(size_t)r * nb + k];
@@ -625,8 +637,37 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   // S5: V_SR[j] = sum_{k<=j} w[j-k] q[k].  Outputs j and nb-1-j are paired so that every thread does nb+1 terms;
   // each sum runs on four interleaved accumulators (k mod 4), so that the 8-cycle DFMA latency and the
   // shared-memory loads of consecutive terms overlap.
-  if (A.w) {
-    for (int idx = tid; idx < (nb + 1) / 2; idx += kWakeThreads) {
+  if (A.w && S > 1) {
+    // few bunches: the chain of a single sum is what costs.  Eight lanes share an output pair, lane g takes the terms
+    // k = g mod 8 of both sums, and a shuffle reduction closes them: 32 pairs per CTA, S CTAs per bunch.
+    constexpr int KS = 8;
+    const int g = tid % KS;
+    const int pairs = (nb + 1) / 2, per_cta = (pairs + S - 1) / S;                    // output pairs of this split
+    const int rounds = (per_cta + kWakeThreads / KS - 1) / (kWakeThreads / KS);       // uniform over the CTA: the
+    for (int i = 0; i < rounds; ++i) {                                                // shuffles need every lane
+      const int idx = split + S * (tid / KS + i * (kWakeThreads / KS));
+      const bool act = idx < pairs;
+      const int j1 = act ? idx : 0, j2 = act ? nb - 1 - idx : 0;
+      double a1 = 0.0, b1 = 0.0, a2 = 0.0, b2 = 0.0;
+      int k = g;
+      for (; k + KS <= j1; k += 2 * KS) { a1 = fma(sw[j1 - k], sq[k], a1); b1 = fma(sw[j1 - k - KS], sq[k + KS], b1); }
+      if (k <= j1) a1 = fma(sw[j1 - k], sq[k], a1);
+      k = g;
+      for (; k + KS <= j2; k += 2 * KS) { a2 = fma(sw[j2 - k], sq[k], a2); b2 = fma(sw[j2 - k - KS], sq[k + KS], b2); }
+      if (k <= j2) a2 = fma(sw[j2 - k], sq[k], a2);
+      double v1 = a1 + b1, v2 = a2 + b2;
+#pragma unroll
+      for (int o = KS / 2; o > 0; o >>= 1) {
+        v1 += __shfl_xor_sync(0xffffffffu, v1, o);
+        v2 += __shfl_xor_sync(0xffffffffu, v2, o);
+      }
+      if (act && g == 0) {
+        A.Vsr[(size_t)b * nb + j1] = v1;
+        if (j2 != j1) A.Vsr[(size_t)b * nb + j2] = v2;
+      }
+    }
+  } else if (A.w) {
+    for (int idx = split + S * tid; idx < (nb + 1) / 2; idx += S * kWakeThreads) {
       const int j1 = idx, j2 = nb - 1 - idx;
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
@@ -647,7 +688,17 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
       }
     }
   } else {
-    for (int j = tid; j < nb; j += kWakeThreads) { A.Vsr[(size_t)b * nb + j] = 0.0; sv[j] = 0.0; }
+    for (int j = split + S * tid; j < nb; j += S * kWakeThreads) { A.Vsr[(size_t)b * nb + j] = 0.0; sv[j] = 0.0; }
+  }
+  if (S > 1) {  // the last split to finish gathers the bunch's V_SR and goes on alone
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) s_last = (atomicAdd(&A.wr_cnt[b], 1u) == (uint32_t)(S - 1));
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (tid == 0) A.wr_cnt[b] = 0u;
+    for (int j = tid; j < nb; j += kWakeThreads) sv[j] = __ldcg(&A.Vsr[(size_t)b * nb + j]);
   }
   __syncthreads();
   for (int k = tid; k < nb + 2; k += kWakeThreads) {
