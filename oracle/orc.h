@@ -50,10 +50,22 @@ typedef struct {
   int32_t n_table; const double *sr_table;
   int32_t window_mode; /* 0: fixed window (reading D11); 1: window follows the bunch in whole bins (reading D31) */
 } orc_wake;
+/* ---- transverse planes (P:l.73-92 Eqs.(3)-(5), l.100-107 Eq.(6b); readings T1..T8) ----
+ * One plane u in {x, y}: tune nu (Psi_0 = 2 pi nu), Twiss alpha, beta [m] (gamma = (1 + alpha^2) / beta),
+ * chromaticity xi (Eq. 3: Psi = Psi_0 (1 + xi delta)), periodic dispersion eta [m], eta' (T2: the third column of the
+ * matrix of Eq. 4 is read as the one of the periodic one-turn matrix, i.e. u - eta delta is what rotates),
+ * Eq. 5: u += sigma_u sqrt(D_exc) r1, u' = u' (1 + delta) / (1 + delta + eps) + sigma_up sqrt(D_exc) r2,
+ * initial distribution u = sigma0_u z, u' = sigma0_up z' (uncorrelated Gaussian, Philox tag 3). */
+typedef struct { double nu, alpha, beta_m, xi, eta_m, etap, sigma_u_m, sigma_up, D_exc, sigma0_u_m, sigma0_up; } orc_plane;
+/* transverse short-range wake: resonators with Rs in Ohm/m (flags ignored),
+ * W_perp(t > 0) = (w_r^2 R / (Q wbar)) exp(-a t) sin(wbar t), W_perp(0) = 0 (T7); both planes use the same list */
+typedef struct { int32_t enable; orc_plane x, y; int32_t n_res; const orc_resonator *res; } orc_transverse;
+
 typedef struct {
   orc_ring ring; int32_t n_cav; const orc_cavity *cav; orc_radiation rad;
   orc_fill fill; orc_wake wake; uint64_t seed; int64_t log_capacity_turns;
   int32_t lr_mode; /* 0: pairwise sum (THE definition); 1: O(M+K) recurrence (long runs) */
+  orc_transverse trans; /* enable = 0: longitudinal tracker only */
 } orc_params;
 
 int orc_create(const orc_params *p, orc_handle **out);
@@ -74,6 +86,16 @@ int orc_get_window(orc_handle *h, int32_t *s_hist, int32_t *s_next);
 int orc_set_window(orc_handle *h, const int32_t *s_hist, const int32_t *s_next);
 /* the whole-bin shift that re-centres a histogram: rint(centroid in bins - n_bins / 2), exact integer arithmetic */
 int32_t orc_window_step(int32_t n_bins, const uint32_t *hist);
+/* transverse state, each [M][N_p]; dipole sums S[b][k] = sum of u over the particles of bin k [m]; kick tables
+ * K[b][j] = sum_{k<j} (Q_b/N_p) S[b][k] W_perp((j-k) Delta) [V]; moments out[M][8]: mean x x' y y', rms x x' y y' */
+int orc_get_transverse(orc_handle *h, double *x, double *xp, double *y, double *yp);
+int orc_set_transverse(orc_handle *h, const double *x, const double *xp, const double *y, const double *yp);
+int orc_get_dipole(orc_handle *h, double *Sx, double *Sy);
+int orc_get_transverse_wake(orc_handle *h, double *Kx, double *Ky);
+int orc_moments_transverse(orc_handle *h, double *out);
+double orc_transverse_wake(double Rs_ohm_per_m, double fr_Hz, double Q, double t_s);
+/* Eqs. (3), (4) for one particle of one plane (no excitation): u, u' in place */
+void orc_betatron_map(const orc_plane *pl, double *u, double *up, double delta);
 int64_t orc_turn(const orc_handle *h);
 double orc_phi_s(const orc_handle *h);
 const char *orc_last_error(void);

@@ -59,10 +59,21 @@ class Wake(C.Structure):
                 ("window_mode", C.c_int32)]
 
 
+PLANE_FIELDS = ("nu", "alpha", "beta_m", "xi", "eta_m", "etap", "sigma_u_m", "sigma_up", "D_exc", "sigma0_u_m", "sigma0_up")
+
+
+class Plane(C.Structure):
+    _fields_ = [(k, C.c_double) for k in PLANE_FIELDS]
+
+
+class Transverse(C.Structure):
+    _fields_ = [("enable", C.c_int32), ("x", Plane), ("y", Plane), ("n_res", C.c_int32), ("res", C.POINTER(Resonator))]
+
+
 class Params(C.Structure):
     _fields_ = [("ring", Ring), ("n_cav", C.c_int32), ("cav", C.POINTER(Cavity)), ("rad", Radiation),
                 ("fill", Fill), ("wake", Wake), ("seed", C.c_uint64), ("log_capacity_turns", C.c_int64),
-                ("lr_mode", C.c_int32)]
+                ("lr_mode", C.c_int32), ("trans", Transverse)]
 
 
 _lib = None
@@ -91,6 +102,15 @@ def lib():
         L.orc_set_window.argtypes = [H, ip, ip]
         L.orc_window_step.argtypes = [C.c_int32, C.POINTER(C.c_uint32)]
         L.orc_window_step.restype = C.c_int32
+        L.orc_get_transverse.argtypes = [H, dp, dp, dp, dp]
+        L.orc_set_transverse.argtypes = [H, dp, dp, dp, dp]
+        L.orc_get_dipole.argtypes = [H, dp, dp]
+        L.orc_get_transverse_wake.argtypes = [H, dp, dp]
+        L.orc_moments_transverse.argtypes = [H, dp]
+        L.orc_transverse_wake.argtypes = [C.c_double] * 4
+        L.orc_transverse_wake.restype = C.c_double
+        L.orc_betatron_map.argtypes = [C.POINTER(Plane), dp, dp, C.c_double]
+        L.orc_betatron_map.restype = None
         L.orc_turn.argtypes = [H]
         L.orc_turn.restype = C.c_int64
         L.orc_phi_s.argtypes = [H]
@@ -126,6 +146,17 @@ def philox(ctr, key):
     o = (C.c_uint32 * 4)()
     lib().orc_philox4x32_10(c, k, o)
     return [int(x) for x in o]
+
+
+def transverse_wake(rs, fr, q, t):
+    return float(lib().orc_transverse_wake(rs, fr, q, t))
+
+
+def betatron_map(plane, u, up, delta):
+    pl = Plane(**{k: float(plane[k]) for k in PLANE_FIELDS})
+    a, b = C.c_double(u), C.c_double(up)
+    lib().orc_betatron_map(C.byref(pl), C.byref(a), C.byref(b), float(delta))
+    return a.value, b.value
 
 
 def window_step(hist):
@@ -189,6 +220,13 @@ class Oracle:
         p.seed = cfg["seed"]
         p.log_capacity_turns = int(log_capacity_turns)
         p.lr_mode = int(lr_mode)
+        tr = cfg.get("transverse")
+        self.transverse = bool(tr)
+        if tr:
+            self._tres = (Resonator * max(len(tr["resonators"]), 1))(
+                *[Resonator(r["Rs_ohm"], r["fr_Hz"], r["Q"], r.get("flags", 1)) for r in tr["resonators"]])
+            p.trans = Transverse(1, Plane(**{k: float(tr["x"][k]) for k in PLANE_FIELDS}),
+                                 Plane(**{k: float(tr["y"][k]) for k in PLANE_FIELDS}), len(tr["resonators"]), self._tres)
         self._h = C.c_void_p()
         self._L = L
         self._ck(L.orc_create(C.byref(p), C.byref(self._h)))
@@ -263,6 +301,31 @@ class Oracle:
         a = np.ascontiguousarray(a, dtype=np.float64)
         if a.size:
             self._ck(self._L.orc_set_lr_history(self._h, _dp(a)))
+
+    def transverse_particles(self):
+        """(x, x', y, y'), each [M][N_p]."""
+        out = [np.empty((self.M, self.Np)) for _ in range(4)]
+        self._ck(self._L.orc_get_transverse(self._h, *[_dp(a) for a in out]))
+        return out
+
+    def set_transverse(self, x, xp, y, yp):
+        a = [np.ascontiguousarray(v, dtype=np.float64) for v in (x, xp, y, yp)]
+        self._ck(self._L.orc_set_transverse(self._h, *[_dp(v) for v in a]))
+
+    def dipole(self):
+        sx, sy = np.empty((self.M, self.nb)), np.empty((self.M, self.nb))
+        self._ck(self._L.orc_get_dipole(self._h, _dp(sx), _dp(sy)))
+        return sx, sy
+
+    def transverse_wake(self):
+        kx, ky = np.empty((self.M, self.nb)), np.empty((self.M, self.nb))
+        self._ck(self._L.orc_get_transverse_wake(self._h, _dp(kx), _dp(ky)))
+        return kx, ky
+
+    def moments_transverse(self):
+        out = np.empty((self.M, 8))
+        self._ck(self._L.orc_moments_transverse(self._h, _dp(out)))
+        return out
 
     def window(self):
         """(s_hist[M], s_next[M]): window shifts in bins (reading D31)."""

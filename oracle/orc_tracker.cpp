@@ -119,7 +119,7 @@ void normal_quad(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t 
   }
 }
 
-enum { TAG_EXCITATION = 0, TAG_INITIAL = 1 };
+enum { TAG_EXCITATION = 0, TAG_INITIAL = 1, TAG_TRANSVERSE = 2, TAG_INITIAL_TRANSVERSE = 3 };
 
 // ---------------------------------------------------------------- resonator
 struct Resonator {
@@ -194,6 +194,13 @@ struct orc_handle {
   std::vector<cplx> ring_a;  // [(K+1)][M][R]: source phasors a[b][n'][r], slot n' % (K+1)
   std::vector<double> mom;   // [M][6]
   std::vector<double> log;   // [log_cap][M][6]
+  // transverse planes (readings T1..T8); all empty when tr.enable == 0
+  orc_transverse tr{};
+  std::vector<Resonator> res_tr;
+  std::vector<double> wt;                  // transverse table wt[k] = sum_r W_perp_r(k Delta), wt[0] = 0
+  std::vector<double> x, xp, y, yp;        // [M][Np]
+  std::vector<double> Sx, Sy, Kx, Ky;      // [M][nb] dipole sums [m] and kick tables [V]
+  std::vector<double> mom_tr;              // [M][8]
   // lr_mode 1 tables
   std::vector<cplx> g_step;  // [M-1][R] exp(lambda (s_{j+1}-s_j) T_rf)
   std::vector<cplx> g_hist;  // [K][R]   exp(lambda (k T0 - (s_{M-1}-s_0) T_rf)), k = 1..K
@@ -209,6 +216,28 @@ namespace {
 ldbl dt_between(const orc_handle *h, int64_t dn, int ds) {
   ldbl T0 = (ldbl)h->ring.T0_s;
   return (ldbl)dn * T0 + (ldbl)ds * (T0 / (ldbl)h->ring.h);
+}
+
+// Reading T7 (the paper defers W_perp to its ref. [7], P:l.107): textbook transverse resonator wake,
+// W_perp(t > 0) = (w_r^2 R / (Q wbar)) exp(-alpha t) sin(wbar t) [V/(C m)], R in Ohm/m, W_perp(t <= 0) = 0;
+// its time integral is R / Q = |Z_perp(0)|.
+double transverse_wake(const Resonator &r, double t) {
+  if (!(t > 0.0)) return 0.0;
+  double wr = 2.0 * PI_D * r.fr;
+  return (wr * wr * r.Rs / (r.Q * r.wbar)) * std::exp(-r.alpha * t) * std::sin(r.wbar * t);
+}
+
+// Eqs. (3), (4) for one plane (readings T2, T3): Psi = 2 pi nu (1 + xi delta); the betatron part u - eta delta,
+// u' - eta' delta is rotated by the Twiss matrix and the dispersive orbit is added back.
+void betatron_map(const orc_plane &pl, double &u, double &up, double delta) {
+  double psi = 2.0 * PI_D * pl.nu * (1.0 + pl.xi * delta);
+  double c = std::cos(psi), sn = std::sin(psi);
+  double gamma = (1.0 + pl.alpha * pl.alpha) / pl.beta_m;
+  double ub = u - pl.eta_m * delta, upb = up - pl.etap * delta;
+  double un = (c + pl.alpha * sn) * ub + pl.beta_m * sn * upb;
+  double upn = -gamma * sn * ub + (c - pl.alpha * sn) * upb;
+  u = pl.eta_m * delta + un;
+  up = pl.etap * delta + upn;
 }
 
 // Reading D31: the window of bunch b starts at tau_lo + s Delta, s an integer number of bins
@@ -232,13 +261,17 @@ int32_t window_step(int nb, const uint32_t *c) {
 }
 
 // steps 1-3 for one particle; z is the unit normal of step 2
-inline void map_one(const orc_handle *h, double &tau, double &delta, double z) {
+inline void map_one(const orc_handle *h, double &tau, double &delta, double z, double *eps_out = nullptr) {
   // 1. delta += sum_c (V_c/E0) sin(m_c w_rf tau + phi_c) - U0/E0   (terms left to right)
   const double E0 = h->ring.E0_eV;
+  double eps = 0.0;  // relative energy gain in the RF cavities this turn (the epsilon of Eqs. (1), (5))
   for (size_t c = 0; c < h->cav.size(); ++c) {
     const orc_cavity &cv = h->cav[c];
-    delta += (cv.V_volt / E0) * std::sin((double)cv.m * h->omega_rf * tau + cv.phase_rad);
+    double term = (cv.V_volt / E0) * std::sin((double)cv.m * h->omega_rf * tau + cv.phase_rad);
+    delta += term;
+    eps += term;
   }
+  if (eps_out) *eps_out = eps;
   delta -= h->ring.U0_eV / E0;
   // 2. delta = delta (1 - D_E) + sigma_delta sqrt(2 D_E) z
   if (h->rad.enable) delta = delta * (1.0 - h->D_E) + h->A_q * z;
@@ -246,7 +279,19 @@ inline void map_one(const orc_handle *h, double &tau, double &delta, double z) {
   tau += h->drift * delta;
 }
 
+void moments_of(const double *v, int64_t n, double &mean, double &rms) {
+  double sm = 0; for (int64_t i = 0; i < n; ++i) sm += v[i];
+  mean = sm / (double)n;
+  double var = 0; for (int64_t i = 0; i < n; ++i) var += (v[i] - mean) * (v[i] - mean);
+  rms = std::sqrt(var / (double)n);
+}
+
 void compute_moments(orc_handle *h) {
+  if (h->tr.enable)
+    for (int b = 0; b < h->M; ++b) {
+      const double *c[4] = {&h->x[(size_t)b * h->Np], &h->xp[(size_t)b * h->Np], &h->y[(size_t)b * h->Np], &h->yp[(size_t)b * h->Np]};
+      for (int a = 0; a < 4; ++a) moments_of(c[a], h->Np, h->mom_tr[(size_t)b * 8 + a], h->mom_tr[(size_t)b * 8 + 4 + a]);
+    }
   // 8. population mean / rms over ALL particles of the bunch, two passes (reading D22)
   for (int b = 0; b < h->M; ++b) {
     const double *t = &h->tau[(size_t)b * h->Np];
@@ -274,6 +319,8 @@ void compute_moments(orc_handle *h) {
 void bin_all(orc_handle *h) {
   std::fill(h->hist.begin(), h->hist.end(), 0u);
   std::fill(h->n_out.begin(), h->n_out.end(), (int64_t)0);
+  std::fill(h->Sx.begin(), h->Sx.end(), 0.0);
+  std::fill(h->Sy.begin(), h->Sy.end(), 0.0);
   for (int b = 0; b < h->M; ++b)
     for (int64_t i = 0; i < h->Np; ++i) {
       size_t p = (size_t)b * h->Np + i;
@@ -283,6 +330,10 @@ void bin_all(orc_handle *h) {
       if (t >= 0.0 && t < (double)h->nb) {
         int j = (int)std::floor(t);
         h->hist[(size_t)b * h->nb + j] += 1u;
+        if (h->tr.enable) {  // reading T6: q_k D_p(tau_k) of Eq. (6b) = (Q_b / N_p) * sum of the offsets in bin k
+          h->Sx[(size_t)b * h->nb + j] += h->x[p];
+          h->Sy[(size_t)b * h->nb + j] += h->y[p];
+        }
       } else {
         h->n_out[b] += 1;
       }
@@ -305,7 +356,25 @@ void one_turn(orc_handle *h) {
         if ((i & 3) == 0) normal_quad(h->seed, (uint32_t)(i >> 2), (uint32_t)b, (uint32_t)n, TAG_EXCITATION, nullptr, zq);
         z = zq[i & 3];
       }
-      map_one(h, h->tau[p], h->delta[p], z);
+      double eps = 0.0;
+      map_one(h, h->tau[p], h->delta[p], z, &eps);
+      if (h->tr.enable) {
+        // reading T1: the transverse steps of a turn follow its longitudinal map and use the updated delta
+        const double d = h->delta[p];
+        betatron_map(h->tr.x, h->x[p], h->xp[p], d);   // Eqs. (3), (4)
+        betatron_map(h->tr.y, h->y[p], h->yp[p], d);
+        if (h->rad.enable) {
+          // Eq. (5) lines 2, 3 (reading T4; the same for y): one Philox block per particle, counter (i, b, n, tag 2),
+          // its four normals are (x, x', y, y')
+          double zt[4];
+          normal_quad(h->seed, (uint32_t)i, (uint32_t)b, (uint32_t)n, TAG_TRANSVERSE, nullptr, zt);
+          const double adia = (1.0 + d) / (1.0 + d + eps);
+          h->x[p] += h->tr.x.sigma_u_m * std::sqrt(h->tr.x.D_exc) * zt[0];
+          h->xp[p] = h->xp[p] * adia + h->tr.x.sigma_up * std::sqrt(h->tr.x.D_exc) * zt[1];
+          h->y[p] += h->tr.y.sigma_u_m * std::sqrt(h->tr.y.D_exc) * zt[2];
+          h->yp[p] = h->yp[p] * adia + h->tr.y.sigma_up * std::sqrt(h->tr.y.D_exc) * zt[3];
+        }
+      }
     }
   }
   // 4: bins, on the window chosen after the previous turn (reading D31); then the window of the next turn
@@ -411,6 +480,40 @@ void one_turn(orc_handle *h) {
         }
       }
       h->delta[p] -= v / h->ring.E0_eV;
+    }
+  }
+  // 6b/7b: transverse short-range wake and kick, Eq. (6b): K[j] = sum_{k<j} (Q_b/N_p) S[k] W_perp((j-k) Delta);
+  // u' += K(tau)/E0 for in-window particles, gathered like the longitudinal wake (readings T7, T8)
+  if (h->tr.enable) {
+    for (int b = 0; b < M; ++b) {
+      double qm = h->charge[b] / (double)Np;
+      for (int j = 0; j < nb; ++j) {
+        double kx = 0.0, ky = 0.0;
+        for (int k = 0; k < j; ++k) {
+          kx += h->wt[j - k] * (qm * h->Sx[(size_t)b * nb + k]);
+          ky += h->wt[j - k] * (qm * h->Sy[(size_t)b * nb + k]);
+        }
+        h->Kx[(size_t)b * nb + j] = kx;
+        h->Ky[(size_t)b * nb + j] = ky;
+      }
+      for (int64_t i = 0; i < Np; ++i) {
+        size_t p = (size_t)b * Np + i;
+        double t = h->tpos[p];
+        if (!(t >= 0.0 && t < (double)nb)) continue;
+        const double *T[2] = {&h->Kx[(size_t)b * nb], &h->Ky[(size_t)b * nb]};
+        double v[2];
+        for (int a = 0; a < 2; ++a) {
+          if (h->gather == 0) v[a] = T[a][(int)std::floor(t)];
+          else {
+            double u = t - 0.5;
+            if (u <= 0.0) v[a] = T[a][0];
+            else if (u >= (double)(nb - 1)) v[a] = T[a][nb - 1];
+            else { int j0 = (int)std::floor(u); double f = u - (double)j0; v[a] = T[a][j0] + f * (T[a][j0 + 1] - T[a][j0]); }
+          }
+        }
+        h->xp[p] += v[0] / h->ring.E0_eV;
+        h->yp[p] += v[1] / h->ring.E0_eV;
+      }
     }
   }
   // 8: statistics
@@ -564,6 +667,32 @@ int orc_create(const orc_params *p, orc_handle **out) {
     h->V.assign((size_t)h->M * h->nb, 0.0);
     h->ring_a.assign((size_t)(h->K + 1) * h->M * (h->R() ? h->R() : 1), cplx(0, 0));
     h->mom.assign((size_t)h->M * 6, 0.0);
+    // transverse planes
+    h->tr = p->trans;
+    h->tr.res = nullptr;  // copied below
+    if (h->tr.enable) {
+      const orc_plane *pls[2] = {&h->tr.x, &h->tr.y};
+      for (const orc_plane *pl : pls)
+        if (!(pl->beta_m > 0) || !std::isfinite(pl->nu) || !std::isfinite(pl->alpha) || !(pl->D_exc >= 0) ||
+            !(pl->sigma_u_m >= 0) || !(pl->sigma_up >= 0) || !(pl->sigma0_u_m >= 0) || !(pl->sigma0_up >= 0)) {
+          delete h;
+          return fail(ORC_EINVAL, "transverse plane: need beta > 0, D_exc >= 0, sigmas >= 0");
+        }
+      if (p->trans.n_res < 0 || (p->trans.n_res > 0 && !p->trans.res)) { delete h; return fail(ORC_EINVAL, "transverse resonator list"); }
+      h->wt.assign(h->nb, 0.0);
+      for (int r = 0; r < p->trans.n_res; ++r) {
+        const orc_resonator &in = p->trans.res[r];
+        if (!(in.Q > 0.5) || !(in.fr_Hz > 0) || !std::isfinite(in.Rs_ohm)) { delete h; return fail(ORC_EINVAL, "transverse resonator: need Q > 1/2, fr > 0"); }
+        Resonator rr{in.Rs_ohm, in.fr_Hz, in.Q, in.flags, 0, 0, 0, 0, cplx()};
+        derive(rr);
+        h->res_tr.push_back(rr);
+        for (int k = 0; k < h->nb; ++k) h->wt[k] += transverse_wake(rr, (double)k * h->Delta);
+      }
+      h->x.assign(N, 0.0); h->xp.assign(N, 0.0); h->y.assign(N, 0.0); h->yp.assign(N, 0.0);
+      h->Sx.assign((size_t)h->M * h->nb, 0.0); h->Sy.assign((size_t)h->M * h->nb, 0.0);
+      h->Kx.assign((size_t)h->M * h->nb, 0.0); h->Ky.assign((size_t)h->M * h->nb, 0.0);
+      h->mom_tr.assign((size_t)h->M * 8, 0.0);
+    }
     h->log.assign((size_t)h->log_cap * h->M * 6, 0.0);
     if (h->R() > 0) {
       int R = h->R(), M = h->M, K = h->K;
@@ -589,6 +718,18 @@ int orc_create(const orc_params *p, orc_handle **out) {
         h->tau[(size_t)b * h->Np + i] = h->sigma_tau0 * zc;
         h->delta[(size_t)b * h->Np + i] = h->sigma_delta0 * zs;
       }
+    // transverse initial distribution: Philox stream 3, counter (i, b, 0, 3), four normals (x, x', y, y')
+    if (h->tr.enable)
+      for (int b = 0; b < h->M; ++b)
+        for (int64_t i = 0; i < h->Np; ++i) {
+          double z4[4];
+          normal_quad(h->seed, (uint32_t)i, (uint32_t)b, 0u, TAG_INITIAL_TRANSVERSE, nullptr, z4);
+          size_t q = (size_t)b * h->Np + i;
+          h->x[q] = h->tr.x.sigma0_u_m * z4[0];
+          h->xp[q] = h->tr.x.sigma0_up * z4[1];
+          h->y[q] = h->tr.y.sigma0_u_m * z4[2];
+          h->yp[q] = h->tr.y.sigma0_up * z4[3];
+        }
     bin_all(h);
     compute_moments(h);
   } catch (const std::bad_alloc &) {
@@ -633,6 +774,52 @@ int orc_set_particles(orc_handle *h, const double *tau, const double *delta, int
   compute_moments(h);
   return 0;
 }
+
+int orc_get_transverse(orc_handle *h, double *x, double *xp, double *y, double *yp) {
+  if (!h || !h->tr.enable || !x || !xp || !y || !yp) return fail(ORC_EINVAL, "transverse planes not enabled / null argument");
+  size_t bytes = sizeof(double) * h->x.size();
+  std::memcpy(x, h->x.data(), bytes); std::memcpy(xp, h->xp.data(), bytes);
+  std::memcpy(y, h->y.data(), bytes); std::memcpy(yp, h->yp.data(), bytes);
+  return 0;
+}
+
+int orc_set_transverse(orc_handle *h, const double *x, const double *xp, const double *y, const double *yp) {
+  if (!h || !h->tr.enable || !x || !xp || !y || !yp) return fail(ORC_EINVAL, "transverse planes not enabled / null argument");
+  size_t bytes = sizeof(double) * h->x.size();
+  std::memcpy(h->x.data(), x, bytes); std::memcpy(h->xp.data(), xp, bytes);
+  std::memcpy(h->y.data(), y, bytes); std::memcpy(h->yp.data(), yp, bytes);
+  bin_all(h);
+  compute_moments(h);
+  return 0;
+}
+
+int orc_get_dipole(orc_handle *h, double *Sx, double *Sy) {
+  if (!h || !h->tr.enable) return fail(ORC_EINVAL, "transverse planes not enabled");
+  if (Sx) std::memcpy(Sx, h->Sx.data(), sizeof(double) * h->Sx.size());
+  if (Sy) std::memcpy(Sy, h->Sy.data(), sizeof(double) * h->Sy.size());
+  return 0;
+}
+
+int orc_get_transverse_wake(orc_handle *h, double *Kx, double *Ky) {
+  if (!h || !h->tr.enable) return fail(ORC_EINVAL, "transverse planes not enabled");
+  if (Kx) std::memcpy(Kx, h->Kx.data(), sizeof(double) * h->Kx.size());
+  if (Ky) std::memcpy(Ky, h->Ky.data(), sizeof(double) * h->Ky.size());
+  return 0;
+}
+
+int orc_moments_transverse(orc_handle *h, double *out) {
+  if (!h || !h->tr.enable || !out) return fail(ORC_EINVAL, "transverse planes not enabled / null argument");
+  std::memcpy(out, h->mom_tr.data(), sizeof(double) * h->mom_tr.size());
+  return 0;
+}
+
+double orc_transverse_wake(double Rs, double fr, double Q, double t) {
+  Resonator r{Rs, fr, Q, 0u, 0, 0, 0, 0, cplx()};
+  derive(r);
+  return transverse_wake(r, t);
+}
+
+void orc_betatron_map(const orc_plane *pl, double *u, double *up, double delta) { betatron_map(*pl, *u, *up, delta); }
 
 int orc_get_window(orc_handle *h, int32_t *s_hist, int32_t *s_next) {
   if (!h) return fail(ORC_EINVAL, "null argument");

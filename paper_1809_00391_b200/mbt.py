@@ -139,6 +139,9 @@ def normal_selftest(seed, ctr):
 
 def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None, device=-1):
     """Workload dict (paper_1809_00391_b200.workloads) -> (mbt_params, keep-alive list)."""
+    if cfg.get("transverse"):
+        raise NotImplementedError("transverse planes (SURVEY.md 8(f) rank 1): the oracle is written and pinned, the CUDA path "
+                                  "is not built yet; the library has no such parameter and never falls back to the CPU")
     f, w = cfg["fill"], cfg["wake"]
     m = len(f["buckets"])
     bucket = (C.c_int32 * m)(*f["buckets"])

@@ -1,0 +1,184 @@
+"""Pins of the oracle's transverse planes (P:l.73-92 Eqs.(3)-(5), l.100-111 Eq.(6b);
+DESIGN.md readings T1..T8).  Oracle only: the CUDA path of this row is not built yet."""
+import math
+
+import numpy as np
+import pytest
+from scipy import integrate
+
+from paper_1809_00391_b200 import workloads as W
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import orc as o
+    o.build()
+    return o
+
+
+PL = dict(nu=18.2317, alpha=-0.7, beta_m=6.5, xi=1.8, eta_m=0.12, etap=-0.015, sigma_u_m=0, sigma_up=0, D_exc=0,
+          sigma0_u_m=0, sigma0_up=0)
+
+
+def _tune(series):
+    n = len(series)
+    w = np.hanning(n)
+    f = np.abs(np.fft.rfft((series - series.mean()) * w))
+    k = int(np.argmax(f[1:-1])) + 1
+    a, b, c = np.log(f[k - 1]), np.log(f[k]), np.log(f[k + 1])
+    return (k + 0.5 * (a - c) / (a - 2 * b + c)) / n
+
+
+def test_betatron_map_is_symplectic_and_has_the_chromatic_tune(orc):
+    # Jacobian determinant 1 (Eq. 4 with gamma = (1 + alpha^2) / beta) at any delta
+    for d in (0.0, 2e-3, -5e-3):
+        e = 1e-6
+        u0, p0 = orc.betatron_map(PL, 0.0, 0.0, d)
+        ux, px = orc.betatron_map(PL, e, 0.0, d)
+        uy, py = orc.betatron_map(PL, 0.0, e, d)
+        det = ((ux - u0) * (py - p0) - (uy - u0) * (px - p0)) / e**2
+        assert abs(det - 1.0) < 1e-9
+    # fractional tune of the iterated map = frac(nu (1 + xi delta)) (Eq. 3); folded at 1/2 by the real FFT
+    for d in (0.0, 3e-3):
+        u, up = 1e-4, 0.0
+        xs = np.empty(4096)
+        for i in range(xs.size):
+            u, up = orc.betatron_map(PL, u, up, d)
+            xs[i] = u
+        q = (PL["nu"] * (1.0 + PL["xi"] * d)) % 1.0
+        q = min(q, 1.0 - q)
+        assert abs(_tune(xs) - q) < 2e-5
+
+
+def test_dispersive_orbit_is_the_fixed_point_and_courant_snyder_is_conserved(orc):
+    d = 4e-3
+    u, up = orc.betatron_map(PL, PL["eta_m"] * d, PL["etap"] * d, d)      # reading T2
+    assert abs(u - PL["eta_m"] * d) < 1e-18 and abs(up - PL["etap"] * d) < 1e-19
+    g = (1 + PL["alpha"] ** 2) / PL["beta_m"]
+    u, up = 3e-4, -2e-5
+    j0 = g * u * u + 2 * PL["alpha"] * u * up + PL["beta_m"] * up * up
+    for _ in range(1000):
+        u, up = orc.betatron_map(PL, u, up, 0.0)
+    assert abs(g * u * u + 2 * PL["alpha"] * u * up + PL["beta_m"] * up * up - j0) < 1e-11 * j0
+
+
+def test_transverse_resonator_wake(orc):
+    rs, fr, q = 2.0e6, 4.0e9, 3.0
+    wr = 2 * math.pi * fr
+    assert orc.transverse_wake(rs, fr, q, 0.0) == 0.0 and orc.transverse_wake(rs, fr, q, -1e-12) == 0.0
+    h = 1e-16
+    assert abs(orc.transverse_wake(rs, fr, q, h) / h - wr * wr * rs / q) < 1e-6 * wr * wr * rs / q     # initial slope
+    al = wr / (2 * q)
+    tot = integrate.quad(lambda t: orc.transverse_wake(rs, fr, q, t), 0, 60 / al, epsabs=0, epsrel=1e-11, limit=800)[0]
+    assert abs(tot - rs / q) < 1e-8 * rs / q                               # integral = |Z_perp(0)| = R / Q
+    # Fourier transform against Z_perp(w) = (w_r / w) R / (1 + i Q (w_r / w - w / w_r)), Z_perp = -i int W e^{+i w t} dt
+    # (time dependence e^{-i w t}); Re Z_perp > 0 for w > 0
+    for w in (0.4 * wr, 1.0 * wr, 2.3 * wr):
+        re = integrate.quad(lambda t: orc.transverse_wake(rs, fr, q, t) * math.cos(w * t), 0, 60 / al, limit=2000)[0]
+        im = integrate.quad(lambda t: orc.transverse_wake(rs, fr, q, t) * math.sin(w * t), 0, 60 / al, limit=2000)[0]
+        z = -1j * complex(re, im)
+        want = (wr / w) * rs / (1 + 1j * q * (wr / w - w / wr))
+        assert abs(z - want) < 1e-6 * abs(want)
+
+
+def _cfg(n_per_bunch=400, m=2, radiation=0, n_bins=16, **tr):
+    cfg = W.tiny(m=m, n_per_bunch=n_per_bunch, n_bins=n_bins, n_lr=0, radiation=radiation)
+    cfg["wake"]["resonators"] = []                                          # no longitudinal wake: delta is the map's
+    cfg["transverse"] = W.transverse_planes(**tr)
+    return cfg
+
+
+def test_dipole_sums_and_transverse_convolution_against_numpy(orc):
+    cfg = _cfg()
+    o = orc.Oracle(cfg)
+    o.track(2)
+    tau = o.particles()[0]
+    x, xp, y, yp = o.transverse_particles()
+    w = cfg["wake"]
+    nb = w["n_bins"]
+    d = (w["tau_hi_s"] - w["tau_lo_s"]) / nb
+    sx, sy = o.dipole()
+    kx, ky = o.transverse_wake()
+    r = cfg["transverse"]["resonators"][0]
+    wt = np.array([orc.transverse_wake(r["Rs_ohm"], r["fr_Hz"], r["Q"], k * d) for k in range(nb)])
+    # the kick of the turn moved x', not x / y / tau: the sums of this turn's binning can be rebuilt from the state
+    for b in range(2):
+        t = (tau[b] - w["tau_lo_s"]) * (nb / (w["tau_hi_s"] - w["tau_lo_s"]))
+        inw = (t >= 0) & (t < nb)
+        j = np.floor(t[inw]).astype(int)
+        assert np.allclose(sx[b], np.bincount(j, weights=x[b][inw], minlength=nb), rtol=1e-12, atol=1e-20)
+        assert np.allclose(sy[b], np.bincount(j, weights=y[b][inw], minlength=nb), rtol=1e-12, atol=1e-22)
+        qm = cfg["fill"]["charge_C"][b] / cfg["fill"]["n_per_bunch"]
+        want = np.array([sum(wt[jj - k] * qm * sx[b][k] for k in range(jj)) for jj in range(nb)])   # Eq. (6b), k < j
+        assert kx[b][0] == 0.0 and np.allclose(kx[b], want, rtol=1e-12, atol=1e-12 * np.abs(want).max())
+
+
+def test_transverse_kick_is_added_to_the_mapped_angle(orc):
+    """One turn, radiation off: x' after the turn = (Eq. 4 applied with the turn's delta) + K(tau)/E0, linear gather."""
+    cfg = _cfg(n_per_bunch=300, m=1)
+    o = orc.Oracle(cfg)
+    x0, xp0, y0, yp0 = [a.copy() for a in o.transverse_particles()]
+    o.track(1)
+    tau, delta = o.particles()
+    x1, xp1, y1, yp1 = o.transverse_particles()
+    kx, ky = o.transverse_wake()
+    w = cfg["wake"]
+    nb = w["n_bins"]
+    e0 = cfg["ring"]["E0_eV"]
+    plx, ply = cfg["transverse"]["x"], cfg["transverse"]["y"]
+    for i in range(300):
+        ux, upx = orc.betatron_map(plx, x0[0, i], xp0[0, i], delta[0, i])
+        uy, upy = orc.betatron_map(ply, y0[0, i], yp0[0, i], delta[0, i])
+        assert ux == x1[0, i] and uy == y1[0, i]
+        t = (tau[0, i] - w["tau_lo_s"]) * (nb / (w["tau_hi_s"] - w["tau_lo_s"]))
+        if 0 <= t < nb:
+            u = t - 0.5
+            if u <= 0:
+                vx, vy = kx[0][0], ky[0][0]
+            elif u >= nb - 1:
+                vx, vy = kx[0][nb - 1], ky[0][nb - 1]
+            else:
+                j0 = int(math.floor(u)); f = u - j0
+                vx = kx[0][j0] + f * (kx[0][j0 + 1] - kx[0][j0]); vy = ky[0][j0] + f * (ky[0][j0 + 1] - ky[0][j0])
+            upx += vx / e0
+            upy += vy / e0
+        assert abs(upx - xp1[0, i]) <= 1e-15 * max(abs(upx), 1e-9) and abs(upy - yp1[0, i]) <= 1e-15 * max(abs(upy), 1e-10)
+    assert np.abs(kx).max() > 0
+
+
+def test_adiabatic_damping_and_equilibrium_emittance(orc):
+    """Eq. (5) lines 2, 3 (reading T4) on a ring with U0/E0 = 1e-2 (damping in a few hundred turns): without
+    excitation the emittance of a particle on the synchronous orbit decays by (1 + eps)^-1 per turn in x', i.e. at
+    the rate eps per turn; with D_exc = eps / (beta gamma) the equilibrium emittance is the configured one."""
+    cfg = _cfg(n_per_bunch=4000, m=1, radiation=1, u0_over_e0=1e-2, eta_x=0.0, xi_x=0.0, xi_y=0.0, rs_ohm_per_m=0.0)
+    cfg["ring"]["U0_eV"] = 1e-2 * cfg["ring"]["E0_eV"]
+    cfg["cavities"] = [dict(V_volt=2.5e-2 * cfg["ring"]["E0_eV"], m=1, phase_rad=math.nan)]
+    cfg["radiation"]["sigma_delta"] = 0.0
+    cfg["fill"]["sigma_tau0_s"] = 0.0
+    cfg["fill"]["sigma_delta0"] = 0.0                                       # everybody sits on (tau, delta) = (0, 0)
+    eps = 1e-2
+    # (1) no excitation
+    quiet = {k: dict(v) if isinstance(v, dict) else v for k, v in cfg.items()}
+    quiet["transverse"] = {k: (dict(v, D_exc=0.0) if k in ("x", "y") else v) for k, v in cfg["transverse"].items()}
+    o = orc.Oracle(quiet)
+    bx = cfg["transverse"]["x"]["beta_m"]
+
+    def emit(a, ap):
+        return math.sqrt(np.mean(a * a) * np.mean(ap * ap) - np.mean(a * ap) ** 2)
+    x, xp, y, yp = o.transverse_particles()
+    e0x = emit(x[0], xp[0])
+    n = 300
+    o.track(n)
+    x, xp, y, yp = o.transverse_particles()
+    rate = -math.log(emit(x[0], xp[0]) / e0x) / n
+    assert abs(rate - eps) < 0.03 * eps
+    # (2) with excitation: stays at the configured emittance (started there), +-6 %
+    o = orc.Oracle(cfg)
+    acc = []
+    for _ in range(12):
+        o.track(100)
+        x, xp, y, yp = o.transverse_particles()
+        acc.append((emit(x[0], xp[0]), emit(y[0], yp[0])))
+    ex, ey = np.mean(acc[4:], axis=0)
+    assert abs(ex / 3.0e-10 - 1) < 0.06 and abs(ey / 3.0e-12 - 1) < 0.06
+    assert abs(np.mean(x[0] ** 2) / (3.0e-10 * bx) - 1) < 0.12
