@@ -89,6 +89,17 @@ typedef struct {
   int32_t window_mode;
 } mbt_wake;
 
+/* ---- transverse planes (P:l.73-92 Eqs.(3)-(5), l.100-111 Eq.(6b); readings T1..T8)
+ * One plane u in {x, y}: tune nu (Psi_0 = 2 pi nu), Twiss alpha, beta [m] (gamma = (1 + alpha^2) / beta), chromaticity
+ * xi (Eq. 3), periodic dispersion eta [m], eta' (T2), Eq. (5): u += sigma_u sqrt(D_exc) r1,
+ * u' = u' (1 + delta) / (1 + delta + eps) + sigma_up sqrt(D_exc) r2 (only with radiation enabled); initial
+ * distribution u = sigma0_u z, u' = sigma0_up z'. */
+typedef struct { double nu, alpha, beta_m, xi, eta_m, etap, sigma_u_m, sigma_up, D_exc, sigma0_u_m, sigma0_up; } mbt_plane;
+/* transverse short-range wake of Eq. (6b): resonators with Rs in Ohm/m (flags ignored),
+ * W_perp(t > 0) = (w_r^2 R / (Q wbar)) exp(-a t) sin(wbar t), W_perp(0) = 0 (T7); the same list for both planes.
+ * enable = 0: longitudinal tracker only (none of the transverse entry points may then be called). */
+typedef struct { int32_t enable; mbt_plane x, y; int32_t n_res; const mbt_resonator *res; } mbt_transverse;
+
 typedef struct {
   mbt_ring ring;
   int32_t n_cav; const mbt_cavity *cav; /* HOST array, n_cav >= 1 */
@@ -104,6 +115,7 @@ typedef struct {
   void *stream;                 /* cudaStream_t the library enqueues on (e.g. torch's current stream);
                                    NULL -> the library creates and owns a (blocking) stream             */
   int32_t device;               /* CUDA device ordinal; -1 -> the current device                        */
+  mbt_transverse trans;         /* transverse planes; the library owns their four device arrays          */
 } mbt_params;
 
 /* Validates, allocates, builds the wake tables and draws the initial distribution on the device.
@@ -142,6 +154,19 @@ int mbt_set_lr_history(mbt_handle *h, const double *in);
  * resuming, call mbt_set_window after it (it re-bins the state; |shift| beyond the bucket -> MBT_EINVAL). */
 int mbt_get_window(mbt_handle *h, int32_t *s_hist, int32_t *s_next);
 int mbt_set_window(mbt_handle *h, const int32_t *s_hist, const int32_t *s_next);
+
+/* ---- transverse planes (HOST pointers; packed [M][N_p] for coordinates, [M][n_bins] for the bin tables) ----
+ * The transverse steps of a turn run in kernels of their own after the fused longitudinal pass: betatron map,
+ * excitation and dipole deposit (k_trans_map), dipole convolution (k_wake_tr), kick and moments (k_trans_kick); no
+ * transverse kick is ever pending. */
+int mbt_get_transverse(mbt_handle *h, double *x, double *xp, double *y, double *yp);
+int mbt_set_transverse(mbt_handle *h, const double *x, const double *xp, const double *y, const double *yp);
+/* dipole sums S[b][k] = sum of u over the particles of bin k [m] and kick tables
+ * K[b][j] = sum_{k<j} (Q_b/N_p) S[b][k] W_perp((j-k) Delta) [V] of the last tracked turn (NULL entries are skipped) */
+int mbt_get_dipole(mbt_handle *h, double *Sx, double *Sy);
+int mbt_get_transverse_wake(mbt_handle *h, double *Kx, double *Ky);
+/* out[M][8]: mean x x' y y', rms x x' y y' (population), of the current state */
+int mbt_moments_transverse(mbt_handle *h, double *out);
 
 /* ---- introspection ---- */
 int64_t mbt_turn(const mbt_handle *h);        /* completed turns, -1 on NULL                 */

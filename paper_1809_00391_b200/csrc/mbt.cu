@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "mbt_kernels.cuh"
+#include "mbt_trans.cuh"
 
 using namespace mbt;
 
@@ -114,6 +115,12 @@ struct mbt_handle {
   DevBuf<unsigned long long> nout_acc;
   DevBuf<int32_t> s_hist, s_next;
   DevBuf<uint32_t> rd_cnt, wr_cnt;
+  // transverse planes (mbt_trans.cuh); empty unless trans
+  bool trans = false;
+  TArgs targs;
+  TWakeArgs twargs;
+  int grid_tr = 0;
+  DevBuf<double> tx, txp, ty, typ, wt, Sx, Sy, Sx_last, Sy_last, Kx, Ky, mom_tr_acc, mom_tr;
   int wake_splits = 1;
   DevBuf<double> lo_hist, lo_next;
   DevBuf<cplx> shift_src, shift_wit;
@@ -150,9 +157,23 @@ pass_fn select_flush(int gather) {
   return gather ? (pass_fn)k_pass<false, false, 1, 0, NPAIR> : (pass_fn)k_pass<false, false, 0, 0, NPAIR>;
 }
 
+void enqueue_trans_map(mbt_handle *h) {
+  const size_t sm = (size_t)h->nb * 2 * sizeof(double);
+  if (h->targs.rad) k_trans_map<true><<<dim3(h->grid_tr, h->M), 256, sm, h->stream>>>(h->targs);
+  else k_trans_map<false><<<dim3(h->grid_tr, h->M), 256, sm, h->stream>>>(h->targs);
+}
+void enqueue_trans_kick(mbt_handle *h) {
+  k_wake_tr<<<h->M, 256, (size_t)h->nb * 3 * sizeof(double), h->stream>>>(h->twargs);
+  k_trans_kick<<<dim3(h->grid_tr, h->M), 256, (size_t)h->nb * 2 * sizeof(double), h->stream>>>(h->targs);
+}
+// launches per tracked turn: 2, or 5 with the transverse planes
+int launches_per_turn(const mbt_handle *h) { return h->trans ? 5 : 2; }
+
 int enqueue_turn(mbt_handle *h) {
   h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
+  if (h->trans) enqueue_trans_map(h);
   k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
+  if (h->trans) enqueue_trans_kick(h);
   return 0;
 }
 
@@ -199,6 +220,8 @@ void destroy(mbt_handle *h) {
   h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
   h->cellSR.release(); h->cellF.release();
   h->rd_cnt.release(); h->wr_cnt.release();
+  h->tx.release(); h->txp.release(); h->ty.release(); h->typ.release(); h->wt.release(); h->Sx.release(); h->Sy.release();
+  h->Sx_last.release(); h->Sy_last.release(); h->Kx.release(); h->Ky.release(); h->mom_tr_acc.release(); h->mom_tr.release();
   h->s_hist.release(); h->s_next.release(); h->lo_hist.release(); h->lo_next.release();
   h->shift_src.release(); h->shift_wit.release();
   h->Esrc.release(); h->F.release(); h->g_step.release(); h->g_tail.release(); h->g_hist.release(); h->a_cur.release();
@@ -272,6 +295,18 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   if (p->d_tau && (((uintptr_t)p->d_tau | (uintptr_t)p->d_delta) & 31u)) return fail(MBT_EINVAL, "d_tau / d_delta must be 32-byte aligned");
   for (int c = 1; c < p->n_cav; ++c)
     if (std::isnan(p->cav[c].phase_rad)) return fail(MBT_EINVAL, "only cav[0] may leave its phase open");
+  const mbt_transverse &tr = p->trans;
+  if (tr.enable) {
+    const mbt_plane *pls[2] = {&tr.x, &tr.y};
+    for (const mbt_plane *pl : pls)
+      if (!(pl->beta_m > 0) || !std::isfinite(pl->nu) || !std::isfinite(pl->alpha) || !(pl->D_exc >= 0) ||
+          !(pl->sigma_u_m >= 0) || !(pl->sigma_up >= 0) || !(pl->sigma0_u_m >= 0) || !(pl->sigma0_up >= 0))
+        return fail(MBT_EINVAL, "transverse plane: need beta > 0, D_exc >= 0, sigmas >= 0");
+    if (tr.n_res < 0 || (tr.n_res > 0 && !tr.res)) return fail(MBT_EINVAL, "transverse resonator list");
+    for (int r = 0; r < tr.n_res; ++r)
+      if (!(tr.res[r].Q > 0.5) || !(tr.res[r].fr_Hz > 0) || !std::isfinite(tr.res[r].Rs_ohm))
+        return fail(MBT_EINVAL, "transverse resonator: need Q > 1/2, fr > 0");
+  }
   int n_lr = 0;
   for (int r = 0; r < wk.n_res; ++r) {
     if (!(wk.res[r].Q > 0.5) || !(wk.res[r].fr_Hz > 0) || !std::isfinite(wk.res[r].Rs_ohm))
@@ -569,6 +604,61 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     h->launches += 1;
     CUH(cudaGetLastError());
   }
+  // ---- transverse planes (mbt_trans.cuh)
+  if (tr.enable) {
+    h->trans = true;
+    std::vector<double> wt(nb, 0.0);
+    for (int r = 0; r < tr.n_res; ++r) {
+      const Res rr = make_res(tr.res[r]);
+      const ldbl wr = 2.0L * PI_L * (ldbl)rr.fr;
+      for (int k = 1; k < nb; ++k) {  // W_perp(t > 0) = (w_r^2 R / (Q wbar)) exp(-a t) sin(wbar t), W_perp(0) = 0 (T7)
+        const ldbl t = (ldbl)((double)k * Delta);
+        wt[k] += (double)((wr * wr * (ldbl)rr.Rs / ((ldbl)rr.Q * rr.wbar)) * expl(-rr.alpha * t) * sinl(rr.wbar * t));
+      }
+    }
+    CUH(h->wt.upload(wt));
+    CUH(h->tx.alloc(N)); CUH(h->txp.alloc(N)); CUH(h->ty.alloc(N)); CUH(h->typ.alloc(N));
+    CUH(h->Sx.alloc((size_t)M * nb)); CUH(h->Sy.alloc((size_t)M * nb));
+    CUH(h->Sx_last.alloc((size_t)M * nb)); CUH(h->Sy_last.alloc((size_t)M * nb));
+    CUH(h->Kx.alloc((size_t)M * nb)); CUH(h->Ky.alloc((size_t)M * nb));
+    CUH(h->mom_tr_acc.alloc((size_t)M * 8)); CUH(h->mom_tr.alloc((size_t)M * 8));
+    TArgs &T = h->targs;
+    memset(&T, 0, sizeof T);
+    T.tau = h->d_tau; T.delta = h->d_delta;
+    T.x = h->tx.p; T.xp = h->txp.p; T.y = h->ty.p; T.yp = h->typ.p;
+    T.ld = h->ld; T.Np = (uint32_t)h->Np; T.M = M; T.nb = nb;
+    T.tile = 8192;
+    h->grid_tr = (int)((h->Np + T.tile - 1) / T.tile);
+    const mbt_plane *pls[2] = {&tr.x, &tr.y};
+    Plane *dst[2] = {&T.px, &T.py};
+    for (int a = 0; a < 2; ++a) {
+      const mbt_plane &q = *pls[a];
+      Plane &d = *dst[a];
+      d.two_pi_nu = 2.0 * PI_D * q.nu;
+      d.xi = q.xi; d.alpha = q.alpha; d.beta = q.beta_m; d.gamma = (1.0 + q.alpha * q.alpha) / q.beta_m;
+      d.eta = q.eta_m; d.etap = q.etap;
+      d.exc_u = q.sigma_u_m * std::sqrt(q.D_exc);
+      d.exc_up = q.sigma_up * std::sqrt(q.D_exc);
+    }
+    T.rad = p->rad.enable ? 1 : 0;
+    T.keys = A.keys;
+    T.n_cav = p->n_cav;
+    for (int c = 0; c < p->n_cav; ++c) { T.cav_amp[c] = A.cav_amp[c]; T.cav_w[c] = A.cav_w[c]; T.cav_ph[c] = A.cav_ph[c]; }
+    T.drift = A.drift;
+    T.lo_next = h->lo_next.p; T.lo_hist = h->lo_hist.p;
+    T.invDelta = A.invDelta; T.nb_d = A.nb_d; T.invE0 = A.invE0; T.gather = wk.gather_order;
+    T.Sx = h->Sx.p; T.Sy = h->Sy.p; T.Kx = h->Kx.p; T.Ky = h->Ky.p;
+    T.ctrl = h->ctrl.p;
+    TWakeArgs &Tw = h->twargs;
+    memset(&Tw, 0, sizeof Tw);
+    Tw.M = M; Tw.nb = nb; Tw.qm = h->qm.p; Tw.wt = h->wt.p;
+    Tw.Sx = h->Sx.p; Tw.Sy = h->Sy.p; Tw.Sx_last = h->Sx_last.p; Tw.Sy_last = h->Sy_last.p; Tw.Kx = h->Kx.p; Tw.Ky = h->Ky.p;
+    dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)M);
+    k_init_tr<<<grid, 256, 0, h->stream>>>(h->tx.p, h->txp.p, h->ty.p, h->typ.p, h->ld, (uint32_t)h->Np, A.keys,
+                                           tr.x.sigma0_u_m, tr.x.sigma0_up, tr.y.sigma0_u_m, tr.y.sigma0_up);
+    h->launches += 1;
+    CUH(cudaGetLastError());
+  }
   CUH(cudaEventCreate(&h->ev0));
   CUH(cudaEventCreate(&h->ev1));
   CUH(cudaStreamSynchronize(h->stream));
@@ -603,7 +693,7 @@ int mbt_track(mbt_handle *h, int64_t n_turns) {
   }
   CU(cudaEventRecord(h->ev1, h->stream));
   h->timed = true;
-  h->launches += 2 * n_turns;
+  h->launches += launches_per_turn(h) * n_turns;
   h->turn += n_turns;
   h->dirty = true;
   h->wake_valid = true;
@@ -621,12 +711,14 @@ int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, dou
     CU(cudaEventRecord(ev[3 * t], h->stream));
     h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
     CU(cudaEventRecord(ev[3 * t + 1], h->stream));
+    if (h->trans) enqueue_trans_map(h);  // the transverse kernels are timed with the wake kernel
     k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
+    if (h->trans) enqueue_trans_kick(h);
     CU(cudaEventRecord(ev[3 * t + 2], h->stream));
   }
   CU(cudaEventRecord(h->ev1, h->stream));
   h->timed = true;
-  h->launches += 2 * n_turns;
+  h->launches += launches_per_turn(h) * n_turns;
   h->turn += n_turns;
   h->dirty = true;
   h->wake_valid = true;
@@ -730,6 +822,90 @@ int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int
   h->turn = turn;
   h->dirty = true;
   h->wake_valid = false;
+  return 0;
+}
+
+namespace {
+int copy_out_packed(mbt_handle *h, const double *dev, double *host) {
+  const size_t n = (size_t)h->M * h->Np;
+  if (h->ld == h->Np) {
+    CU(cudaMemcpyAsync(host, dev, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  } else {
+    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n)); }
+    dim3 grid((unsigned)((h->Np + 255) / 256 < 1024 ? (h->Np + 255) / 256 : 1024), (unsigned)h->M);
+    k_pack<<<grid, 256, 0, h->stream>>>(dev, h->ld, (uint32_t)h->Np, h->scratch_a.p);
+    h->launches += 1;
+    CU(cudaMemcpyAsync(host, h->scratch_a.p, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  }
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+int copy_in_packed(mbt_handle *h, const double *host, double *dev) {
+  const size_t n = (size_t)h->M * h->Np;
+  if (h->ld == h->Np) {
+    CU(cudaMemcpyAsync(dev, host, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  } else {
+    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n)); }
+    dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)h->M);
+    CU(cudaMemcpyAsync(h->scratch_a.p, host, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    k_unpack<<<grid, 256, 0, h->stream>>>(h->scratch_a.p, h->ld, (uint32_t)h->Np, dev);
+    h->launches += 1;
+  }
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+}  // namespace
+
+int mbt_get_transverse(mbt_handle *h, double *x, double *xp, double *y, double *yp) {
+  if (!h || !h->trans || !x || !xp || !y || !yp) return fail(MBT_EINVAL, "transverse planes not enabled / null argument");
+  CU(cudaSetDevice(h->device));
+  int rc;
+  if ((rc = copy_out_packed(h, h->tx.p, x)) || (rc = copy_out_packed(h, h->txp.p, xp)) ||
+      (rc = copy_out_packed(h, h->ty.p, y)) || (rc = copy_out_packed(h, h->typ.p, yp)))
+    return rc;
+  return 0;
+}
+
+int mbt_set_transverse(mbt_handle *h, const double *x, const double *xp, const double *y, const double *yp) {
+  if (!h || !h->trans || !x || !xp || !y || !yp) return fail(MBT_EINVAL, "transverse planes not enabled / null argument");
+  CU(cudaSetDevice(h->device));
+  int rc;
+  if ((rc = copy_in_packed(h, x, h->tx.p)) || (rc = copy_in_packed(h, xp, h->txp.p)) ||
+      (rc = copy_in_packed(h, y, h->ty.p)) || (rc = copy_in_packed(h, yp, h->typ.p)))
+    return rc;
+  return 0;
+}
+
+int mbt_get_dipole(mbt_handle *h, double *Sx, double *Sy) {
+  if (!h || !h->trans) return fail(MBT_EINVAL, "transverse planes not enabled");
+  CU(cudaSetDevice(h->device));
+  const size_t bytes = sizeof(double) * (size_t)h->M * h->nb;
+  if (Sx) CU(cudaMemcpyAsync(Sx, h->Sx_last.p, bytes, cudaMemcpyDeviceToHost, h->stream));
+  if (Sy) CU(cudaMemcpyAsync(Sy, h->Sy_last.p, bytes, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_get_transverse_wake(mbt_handle *h, double *Kx, double *Ky) {
+  if (!h || !h->trans) return fail(MBT_EINVAL, "transverse planes not enabled");
+  CU(cudaSetDevice(h->device));
+  const size_t bytes = sizeof(double) * (size_t)h->M * h->nb;
+  if (Kx) CU(cudaMemcpyAsync(Kx, h->Kx.p, bytes, cudaMemcpyDeviceToHost, h->stream));
+  if (Ky) CU(cudaMemcpyAsync(Ky, h->Ky.p, bytes, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_moments_transverse(mbt_handle *h, double *out) {
+  if (!h || !h->trans || !out) return fail(MBT_EINVAL, "transverse planes not enabled / null argument");
+  CU(cudaSetDevice(h->device));
+  CU(cudaMemsetAsync(h->mom_tr_acc.p, 0, sizeof(double) * h->M * 8, h->stream));
+  k_moments_tr<<<dim3(h->grid_tr, h->M), 256, 0, h->stream>>>(h->targs, h->mom_tr_acc.p);
+  k_close_moments_tr<<<(h->M + 127) / 128, 128, 0, h->stream>>>(h->M, (uint32_t)h->Np, h->mom_tr_acc.p, h->mom_tr.p);
+  h->launches += 2;
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(out, h->mom_tr.p, sizeof(double) * h->M * 8, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
   return 0;
 }
 

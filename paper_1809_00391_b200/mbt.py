@@ -19,6 +19,7 @@ SYMBOLS = [
     "mbt_create", "mbt_track", "mbt_moments", "mbt_destroy", "mbt_get_particles", "mbt_set_particles",
     "mbt_get_histogram", "mbt_get_wake", "mbt_get_moment_log", "mbt_get_lr_history", "mbt_set_lr_history", "mbt_get_window", "mbt_set_window",
     "mbt_turn", "mbt_phi_s", "mbt_particle_stride", "mbt_device_pointers", "mbt_launch_count",
+    "mbt_get_transverse", "mbt_set_transverse", "mbt_get_dipole", "mbt_get_transverse_wake", "mbt_moments_transverse",
     "mbt_last_track_seconds", "mbt_track_profiled", "mbt_philox_selftest", "mbt_normal_selftest", "mbt_last_error", "mbt_version",
 ]
 
@@ -52,10 +53,22 @@ class Wake(C.Structure):
                 ("window_mode", C.c_int32)]
 
 
+PLANE_FIELDS = ("nu", "alpha", "beta_m", "xi", "eta_m", "etap", "sigma_u_m", "sigma_up", "D_exc", "sigma0_u_m", "sigma0_up")
+
+
+class Plane(C.Structure):
+    _fields_ = [(k, C.c_double) for k in PLANE_FIELDS]
+
+
+class Transverse(C.Structure):
+    _fields_ = [("enable", C.c_int32), ("x", Plane), ("y", Plane), ("n_res", C.c_int32), ("res", C.POINTER(Resonator))]
+
+
 class Params(C.Structure):
     _fields_ = [("ring", Ring), ("n_cav", C.c_int32), ("cav", C.POINTER(Cavity)), ("rad", Radiation),
                 ("fill", Fill), ("wake", Wake), ("seed", C.c_uint64), ("log_capacity_turns", C.c_int64),
-                ("d_tau", C.c_void_p), ("d_delta", C.c_void_p), ("stream", C.c_void_p), ("device", C.c_int32)]
+                ("d_tau", C.c_void_p), ("d_delta", C.c_void_p), ("stream", C.c_void_p), ("device", C.c_int32),
+                ("trans", Transverse)]
 
 
 class MbtError(RuntimeError):
@@ -101,6 +114,11 @@ def lib():
         L.mbt_track_profiled.argtypes = [H, C.c_int64, dp, dp]
         L.mbt_get_window.argtypes = [H, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.mbt_set_window.argtypes = [H, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        L.mbt_get_transverse.argtypes = [H, dp, dp, dp, dp]
+        L.mbt_set_transverse.argtypes = [H, dp, dp, dp, dp]
+        L.mbt_get_dipole.argtypes = [H, dp, dp]
+        L.mbt_get_transverse_wake.argtypes = [H, dp, dp]
+        L.mbt_moments_transverse.argtypes = [H, dp]
         L.mbt_philox_selftest.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.mbt_normal_selftest.argtypes = [C.c_uint64, C.c_int64, C.POINTER(C.c_uint32), dp]
         L.mbt_last_error.restype = C.c_char_p
@@ -139,9 +157,6 @@ def normal_selftest(seed, ctr):
 
 def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None, device=-1):
     """Workload dict (paper_1809_00391_b200.workloads) -> (mbt_params, keep-alive list)."""
-    if cfg.get("transverse"):
-        raise NotImplementedError("transverse planes (SURVEY.md 8(f) rank 1): the oracle is written and pinned, the CUDA path "
-                                  "is not built yet; the library has no such parameter and never falls back to the CPU")
     f, w = cfg["fill"], cfg["wake"]
     m = len(f["buckets"])
     bucket = (C.c_int32 * m)(*f["buckets"])
@@ -166,7 +181,14 @@ def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None
     p.d_delta = d_delta
     p.stream = stream
     p.device = int(device)
-    return p, [bucket, charge, cav, res, tbl]
+    tr = cfg.get("transverse")
+    tres = None
+    if tr:
+        tres = (Resonator * max(len(tr["resonators"]), 1))(
+            *[Resonator(r["Rs_ohm"], r["fr_Hz"], r["Q"], r.get("flags", 1)) for r in tr["resonators"]])
+        p.trans = Transverse(1, Plane(**{k: float(tr["x"][k]) for k in PLANE_FIELDS}),
+                             Plane(**{k: float(tr["y"][k]) for k in PLANE_FIELDS}), len(tr["resonators"]), tres)
+    return p, [bucket, charge, cav, res, tbl, tres]
 
 
 class Tracker:
@@ -292,6 +314,33 @@ class Tracker:
         b = np.ascontiguousarray(s_next, dtype=np.int32)
         ip = C.POINTER(C.c_int32)
         _ck(self._L.mbt_set_window(self._h, a.ctypes.data_as(ip), b.ctypes.data_as(ip)))
+
+    def transverse_particles(self):
+        """(x, x', y, y'), each [M][N_p]."""
+        out = [np.empty((self.M, self.Np)) for _ in range(4)]
+        _ck(self._L.mbt_get_transverse(self._h, *[_dp(a) for a in out]))
+        return out
+
+    def set_transverse(self, x, xp, y, yp):
+        a = [np.ascontiguousarray(v, dtype=np.float64) for v in (x, xp, y, yp)]
+        if any(v.size != self.M * self.Np for v in a):
+            raise ValueError("need M*Np coordinates")
+        _ck(self._L.mbt_set_transverse(self._h, *[_dp(v) for v in a]))
+
+    def dipole(self):
+        sx, sy = np.empty((self.M, self.nb)), np.empty((self.M, self.nb))
+        _ck(self._L.mbt_get_dipole(self._h, _dp(sx), _dp(sy)))
+        return sx, sy
+
+    def transverse_wake(self):
+        kx, ky = np.empty((self.M, self.nb)), np.empty((self.M, self.nb))
+        _ck(self._L.mbt_get_transverse_wake(self._h, _dp(kx), _dp(ky)))
+        return kx, ky
+
+    def moments_transverse(self):
+        out = np.empty((self.M, 8))
+        _ck(self._L.mbt_moments_transverse(self._h, _dp(out)))
+        return out
 
     def device_pointers(self):
         t, d, ld = C.c_void_p(), C.c_void_p(), C.c_int64()

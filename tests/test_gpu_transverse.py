@@ -1,0 +1,176 @@
+"""GPU-vs-oracle parity of the transverse planes through the C ABI (P:l.73-92 Eqs.(3)-(5),
+l.100-111 Eq.(6b); readings T1..T8).  Same protocol as test_gpu_parity.py: the oracle's state is uploaded,
+both sides advance one turn, everything observable is compared:
+  coordinates (x, x', y, y') within 1e-12 relative (scale D23), dipole sums and kick tables within 1e-10 of the
+  row maximum (the wake tolerance of north_star (iii)), moments 1e-8."""
+import numpy as np
+import pytest
+
+from paper_1809_00391_b200 import workloads as W
+from parity import TOL_PARTICLE, TOL_WAKE, assert_single_turn_parity, particle_errors, wake_error
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mbt():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu-marked tests need a CUDA device")
+    from paper_1809_00391_b200 import build, mbt as _mbt
+    build.build()
+    _mbt.lib()
+    return _mbt
+
+
+def _cfg(tr=None, **kw):
+    cfg = W.tiny(**kw)
+    cfg["transverse"] = W.transverse_planes(**(tr or {}))
+    return cfg
+
+
+def assert_transverse_turn_parity(o, t, cfg, turns=1, tol=TOL_PARTICLE):
+    """Upload the oracle's 6-D state, advance both sides, compare the transverse observables; the longitudinal ones
+    go through assert_single_turn_parity (which does the tracking)."""
+    t.set_transverse(*o.transverse_particles())
+    r = assert_single_turn_parity(o, t, cfg, turns=turns)
+    names = ("x", "xp", "y", "yp")
+    for nm, g, c in zip(names, t.transverse_particles(), o.transverse_particles()):
+        e = particle_errors(g, c)
+        assert e <= tol, "%s differs by %.3e (relative, D23)" % (nm, e)
+        r["e_" + nm] = e
+    if r["hist_bad_bins"] == 0:
+        for nm, g, c in zip(("Sx", "Sy"), t.dipole(), o.dipole()):
+            r["e_" + nm] = wake_error(g, c)
+            assert r["e_" + nm] <= TOL_WAKE, "%s differs by %.3e" % (nm, r["e_" + nm])
+        for nm, g, c in zip(("Kx", "Ky"), t.transverse_wake(), o.transverse_wake()):
+            r["e_" + nm] = wake_error(g, c)
+            assert r["e_" + nm] <= TOL_WAKE, "%s differs by %.3e" % (nm, r["e_" + nm])
+    m_c, m_g = o.moments_transverse(), t.moments_transverse()
+    for k in range(4):
+        ref = np.maximum(m_c[:, 4 + k], np.abs(m_c[:, k]))
+        assert np.all(np.abs(m_g[:, k] - m_c[:, k]) <= 1e-10 * ref + 1e-300), (k, m_g[:, k], m_c[:, k])
+        assert np.all(np.abs(m_g[:, 4 + k] - m_c[:, 4 + k]) <= 1e-8 * ref + 1e-300), (k, m_g[:, 4 + k], m_c[:, 4 + k])
+    return r
+
+
+def test_transverse_initial_distribution(mbt, orc):
+    for kw in (dict(n_per_bunch=37), dict(n_per_bunch=8193, m=3), dict(n_per_bunch=1, m=2)):
+        cfg = _cfg(**kw)
+        o = orc.Oracle(cfg)
+        with mbt.Tracker(cfg) as t:
+            for g, c in zip(t.transverse_particles(), o.transverse_particles()):
+                assert particle_errors(g, c) <= TOL_PARTICLE
+            tau_g, delta_g = t.particles()
+            tau_c, delta_c = o.particles()
+            assert particle_errors(tau_g, tau_c) <= TOL_PARTICLE and particle_errors(delta_g, delta_c) <= TOL_PARTICLE
+            m_c, m_g = o.moments_transverse(), t.moments_transverse()
+            assert np.allclose(m_g[:, 4:], m_c[:, 4:], rtol=1e-8)
+
+
+VARIANTS = {
+    "default": dict(n_per_bunch=513, n_bins=16),
+    "no_radiation": dict(n_per_bunch=400, n_bins=16, radiation=0),
+    "ngp": dict(n_per_bunch=257, n_bins=16, gather=0),
+    "harmonic": dict(n_per_bunch=301, n_bins=32, harmonic=True),
+    "no_long_wake": dict(n_per_bunch=1000, n_bins=16, n_lr=0),
+    "one_particle": dict(n_per_bunch=1, m=2),
+    "ragged_tiles": dict(n_per_bunch=8193 + 5, m=2, n_bins=64),
+    "many_bins": dict(n_per_bunch=4000, m=2, n_bins=1023),
+    "twiss": dict(n_per_bunch=999, n_bins=16, tr=dict(alpha_x=-0.7, alpha_y=1.3, etap_x=-0.015, xi_x=2.5, xi_y=-1.0)),
+    "two_resonators": dict(n_per_bunch=777, n_bins=32),
+}
+
+
+@pytest.mark.parametrize("name", sorted(VARIANTS))
+def test_transverse_single_turn_parity(mbt, orc, name):
+    kw = dict(VARIANTS[name])
+    cfg = _cfg(**kw)
+    if name == "two_resonators":
+        cfg["transverse"]["resonators"].append(dict(Rs_ohm=-3.0e5, fr_Hz=1.1e10, Q=4.0, flags=1))
+    o = orc.Oracle(cfg)
+    o.track(3)
+    with mbt.Tracker(cfg) as t:
+        for _ in range(3):
+            r = assert_transverse_turn_parity(o, t, cfg)
+        print(name, r)
+
+
+def test_transverse_with_bunch_following_window(mbt, orc):
+    cfg = _cfg(m=3, n_per_bunch=3001, n_bins=32)
+    cfg["wake"]["window_mode"] = 1
+    o = orc.Oracle(cfg)
+    tau, delta = o.particles()
+    o.set_particles(tau * 0.5 + np.array([[15e-12], [-22e-12], [0.0]]), delta, 0)
+    o.track(2)
+    with mbt.Tracker(cfg) as t:
+        for _ in range(4):
+            assert_transverse_turn_parity(o, t, cfg)
+        assert len(set(int(s) for s in t.window()[0])) >= 2
+
+
+def test_transverse_several_turns_without_resync(mbt, orc):
+    """Ten turns from the common initial distribution, no re-synchronisation: the betatron phase advances by
+    ~2 pi nu per turn, so rounding differences rotate but do not grow; histograms stay identical on this seed."""
+    cfg = _cfg(m=3, n_per_bunch=5000, n_bins=32)
+    o = orc.Oracle(cfg)
+    with mbt.Tracker(cfg) as t:
+        o.track(10)
+        t.track(10)
+        assert t.turn == 10
+        for g, c in zip(t.transverse_particles(), o.transverse_particles()):
+            assert particle_errors(g, c) <= 1e-10
+        if np.array_equal(t.histogram(), o.histogram()):
+            for g, c in zip(t.transverse_wake(), o.transverse_wake()):
+                assert wake_error(g, c) <= 1e-9
+        m_c, m_g = o.moments_transverse(), t.moments_transverse()
+        assert np.allclose(m_g[:, 4:], m_c[:, 4:], rtol=1e-8)
+
+
+@pytest.mark.parametrize("name,over", [("c3", dict(n_per_bunch=30_000)), ("c4", dict(n_per_bunch=1_500))])
+def test_transverse_on_baseline_fills(mbt, orc, name, over):
+    """The transverse planes on the fill patterns of BASELINE configs c3 / c4 (reduced N_p): several CTAs per bunch,
+    363 bunches, long-range history in the longitudinal plane."""
+    cfg = W.config(name, **over)
+    cfg["transverse"] = W.transverse_planes()
+    o = orc.Oracle(cfg, lr_mode=0)
+    o.track(2)
+    with mbt.Tracker(cfg) as t:
+        r = assert_transverse_turn_parity(o, t, cfg)
+        print(name, r)
+
+
+def test_transverse_kick_changes_the_angles(mbt, orc):
+    """Not a no-op: with the transverse resonator removed the angles of the same turn differ by K(tau)/E0."""
+    cfg = _cfg(m=1, n_per_bunch=4096, n_bins=32, radiation=0)
+    cfg0 = _cfg(m=1, n_per_bunch=4096, n_bins=32, radiation=0)
+    cfg0["transverse"]["resonators"] = []
+    with mbt.Tracker(cfg) as t, mbt.Tracker(cfg0) as t0:
+        x, xp, y, yp = t.transverse_particles()
+        t.set_transverse(x + 1e-3, xp, y - 5e-4, yp)          # a dipole offset so that the sums are not noise
+        t0.set_transverse(x + 1e-3, xp, y - 5e-4, yp)
+        t.track(1)
+        t0.track(1)
+        kx, ky = t.transverse_wake()
+        assert np.abs(kx).max() > 0 and np.abs(ky).max() > 0
+        assert not t0.transverse_wake()[0].any()
+        d = t.transverse_particles()[1] - t0.transverse_particles()[1]
+        assert np.abs(d).max() > 0
+        assert np.abs(d).max() <= np.abs(kx).max() / cfg["ring"]["E0_eV"] * (1 + 1e-12)
+        assert np.array_equal(t.transverse_particles()[0], t0.transverse_particles()[0])   # the kick acts on u' only
+
+
+def test_transverse_entry_points_refuse_a_longitudinal_handle(mbt):
+    cfg = W.tiny()
+    with mbt.Tracker(cfg) as t:
+        with pytest.raises(mbt.MbtError) as e:
+            t.transverse_particles()
+        assert e.value.code == -1
+        with pytest.raises(mbt.MbtError):
+            t.moments_transverse()
+        with pytest.raises(mbt.MbtError):
+            t.dipole()
+    bad = _cfg()
+    bad["transverse"]["x"]["beta_m"] = 0.0
+    with pytest.raises(mbt.MbtError):
+        mbt.Tracker(bad)

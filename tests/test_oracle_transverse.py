@@ -1,5 +1,5 @@
 """Pins of the oracle's transverse planes (P:l.73-92 Eqs.(3)-(5), l.100-111 Eq.(6b);
-DESIGN.md readings T1..T8).  Oracle only: the CUDA path of this row is not built yet."""
+DESIGN.md readings T1..T8).  The CUDA path of this row is compared with this oracle in test_gpu_transverse.py."""
 import math
 
 import numpy as np
