@@ -117,10 +117,17 @@ struct mbt_handle {
   DevBuf<uint32_t> rd_cnt, wr_cnt;
   // transverse planes (mbt_trans.cuh); empty unless trans
   bool trans = false;
-  TArgs targs;
+  Args6 args6;
   TWakeArgs twargs;
-  int grid_tr = 0;
-  DevBuf<double> tx, txp, ty, typ, wt, Sx, Sy, Sx_last, Sy_last, Kx, Ky, mom_tr_acc, mom_tr;
+  TMomArgs tmargs;
+  int grid_tr = 0, grid_pass6 = 0, fix_bits = kFixBitsMax;
+  size_t smem_pass6 = 0;
+  void (*fn_map6)(const Args6) = nullptr;    // k_pass6<true, ...>
+  void (*fn_flush6)(const Args6) = nullptr;  // k_pass6<false, ...>
+  DevBuf<double> tx, txp, ty, typ, wt, Sov, S_last, Ktab, acc2, mom_tr_acc, mom_tr;
+  DevBuf<unsigned long long> Sfix;
+  DevBuf<FixScale> fix;
+  DevBuf<WakeCell> cellX, cellY;
   int wake_splits = 1;
   DevBuf<double> lo_hist, lo_next;
   DevBuf<cplx> shift_src, shift_wit;
@@ -157,23 +164,42 @@ pass_fn select_flush(int gather) {
   return gather ? (pass_fn)k_pass<false, false, 1, 0, NPAIR> : (pass_fn)k_pass<false, false, 0, 0, NPAIR>;
 }
 
-void enqueue_trans_map(mbt_handle *h) {
-  const size_t sm = (size_t)h->nb * 2 * sizeof(double);
-  if (h->targs.rad) k_trans_map<true><<<dim3(h->grid_tr, h->M), 256, sm, h->stream>>>(h->targs);
-  else k_trans_map<false><<<dim3(h->grid_tr, h->M), 256, sm, h->stream>>>(h->targs);
+typedef void (*pass6_fn)(const Args6);
+pass6_fn select_map6(bool rad, int gather, int n_cav) {
+#define MBT_SEL_(R, G)                                             \
+  (n_cav == 1 ? (pass6_fn)k_pass6<true, R, G, 1>                    \
+              : n_cav == 2 ? (pass6_fn)k_pass6<true, R, G, 2> : (pass6_fn)k_pass6<true, R, G, 0>)
+  if (rad) return gather ? MBT_SEL_(true, 1) : MBT_SEL_(true, 0);
+  return gather ? MBT_SEL_(false, 1) : MBT_SEL_(false, 0);
+#undef MBT_SEL_
 }
-void enqueue_trans_kick(mbt_handle *h) {
-  k_wake_tr<<<h->M, 256, (size_t)h->nb * 3 * sizeof(double), h->stream>>>(h->twargs);
-  k_trans_kick<<<dim3(h->grid_tr, h->M), 256, (size_t)h->nb * 2 * sizeof(double), h->stream>>>(h->targs);
+pass6_fn select_flush6(int gather) { return gather ? (pass6_fn)k_pass6<false, false, 1, 0> : (pass6_fn)k_pass6<false, false, 0, 0>; }
+
+// the pass of a tracked turn: the longitudinal one, or the fused 6-D one of a handle with the transverse planes
+void enqueue_pass(mbt_handle *h) {
+  if (h->trans) h->fn_map6<<<dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream>>>(h->args6);
+  else h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
 }
-// launches per tracked turn: 2, or 5 with the transverse planes
-int launches_per_turn(const mbt_handle *h) { return h->trans ? 5 : 2; }
+void enqueue_wakes(mbt_handle *h) {
+  k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
+  if (h->trans) k_wake_tr<<<h->M, 256, (size_t)h->nb * 5 * sizeof(double), h->stream>>>(h->twargs);
+}
+// launches per tracked turn: 2, or 3 with the transverse planes
+int launches_per_turn(const mbt_handle *h) { return h->trans ? 3 : 2; }
 
 int enqueue_turn(mbt_handle *h) {
-  h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
-  if (h->trans) enqueue_trans_map(h);
-  k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
-  if (h->trans) enqueue_trans_kick(h);
+  enqueue_pass(h);
+  enqueue_wakes(h);
+  return 0;
+}
+
+// scale of the fixed-point dipole sums from the transverse state in memory
+int rescale_transverse(mbt_handle *h) {
+  CU(cudaMemsetAsync(h->mom_tr_acc.p, 0, sizeof(double) * h->M * 8, h->stream));
+  k_moments_tr<<<dim3(h->grid_tr, h->M), 256, 0, h->stream>>>(h->tmargs, h->mom_tr_acc.p);
+  k_fix_scale<<<(2 * h->M + 127) / 128, 128, 0, h->stream>>>(h->M, (uint32_t)h->Np, h->fix_bits, h->mom_tr_acc.p, h->fix.p);
+  h->launches += 2;
+  CU(cudaGetLastError());
   return 0;
 }
 
@@ -192,7 +218,8 @@ int build_graph(mbt_handle *h, int turns, cudaGraphExec_t *out) {
 int flush(mbt_handle *h) {
   if (!h->dirty) return 0;
   CU(cudaSetDevice(h->device));
-  h->fn_flush<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
+  if (h->trans) h->fn_flush6<<<dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream>>>(h->args6);
+  else h->fn_flush<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
   WakeArgs wa = h->wargs;
   wa.mode = 1;
   wa.S = 1;
@@ -220,8 +247,9 @@ void destroy(mbt_handle *h) {
   h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
   h->cellSR.release(); h->cellF.release();
   h->rd_cnt.release(); h->wr_cnt.release();
-  h->tx.release(); h->txp.release(); h->ty.release(); h->typ.release(); h->wt.release(); h->Sx.release(); h->Sy.release();
-  h->Sx_last.release(); h->Sy_last.release(); h->Kx.release(); h->Ky.release(); h->mom_tr_acc.release(); h->mom_tr.release();
+  h->tx.release(); h->txp.release(); h->ty.release(); h->typ.release(); h->wt.release(); h->Sfix.release(); h->Sov.release();
+  h->S_last.release(); h->Ktab.release(); h->acc2.release(); h->fix.release(); h->cellX.release(); h->cellY.release();
+  h->mom_tr_acc.release(); h->mom_tr.release();
   h->s_hist.release(); h->s_next.release(); h->lo_hist.release(); h->lo_next.release();
   h->shift_src.release(); h->shift_wit.release();
   h->Esrc.release(); h->F.release(); h->g_step.release(); h->g_tail.release(); h->g_hist.release(); h->a_cur.release();
@@ -618,44 +646,61 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     }
     CUH(h->wt.upload(wt));
     CUH(h->tx.alloc(N)); CUH(h->txp.alloc(N)); CUH(h->ty.alloc(N)); CUH(h->typ.alloc(N));
-    CUH(h->Sx.alloc((size_t)M * nb)); CUH(h->Sy.alloc((size_t)M * nb));
-    CUH(h->Sx_last.alloc((size_t)M * nb)); CUH(h->Sy_last.alloc((size_t)M * nb));
-    CUH(h->Kx.alloc((size_t)M * nb)); CUH(h->Ky.alloc((size_t)M * nb));
+    CUH(h->Sfix.alloc((size_t)M * 2 * nb)); CUH(h->Sov.alloc((size_t)M * 2 * nb));
+    CUH(h->S_last.alloc((size_t)M * 2 * nb)); CUH(h->Ktab.alloc((size_t)M * 2 * nb));
+    CUH(h->cellX.alloc((size_t)M * (nb + 2))); CUH(h->cellY.alloc((size_t)M * (nb + 2)));
+    CUH(h->fix.alloc((size_t)M * 2)); CUH(h->acc2.alloc((size_t)M * 2));
     CUH(h->mom_tr_acc.alloc((size_t)M * 8)); CUH(h->mom_tr.alloc((size_t)M * 8));
-    TArgs &T = h->targs;
+    // bits of the fixed-point dipole sums: N_p 2^bits <= 2^62 (mbt_trans.cuh)
+    h->fix_bits = kFixBitsMax;
+    while (h->fix_bits > 20 && (double)h->Np * std::ldexp(1.0, h->fix_bits) > std::ldexp(1.0, 62)) h->fix_bits -= 1;
+    Args6 &T = h->args6;
     memset(&T, 0, sizeof T);
-    T.tau = h->d_tau; T.delta = h->d_delta;
+    T.L = A;
     T.x = h->tx.p; T.xp = h->txp.p; T.y = h->ty.p; T.yp = h->typ.p;
-    T.ld = h->ld; T.Np = (uint32_t)h->Np; T.M = M; T.nb = nb;
-    T.tile = 8192;
-    h->grid_tr = (int)((h->Np + T.tile - 1) / T.tile);
     const mbt_plane *pls[2] = {&tr.x, &tr.y};
     Plane *dst[2] = {&T.px, &T.py};
     for (int a = 0; a < 2; ++a) {
       const mbt_plane &q = *pls[a];
       Plane &d = *dst[a];
-      d.two_pi_nu = 2.0 * PI_D * q.nu;
-      d.xi = q.xi; d.alpha = q.alpha; d.beta = q.beta_m; d.gamma = (1.0 + q.alpha * q.alpha) / q.beta_m;
+      d.t_frac = q.nu - std::floor(q.nu);
+      d.t_xi = q.nu * q.xi;
+      d.alpha = q.alpha; d.beta = q.beta_m; d.gamma = (1.0 + q.alpha * q.alpha) / q.beta_m;
       d.eta = q.eta_m; d.etap = q.etap;
       d.exc_u = q.sigma_u_m * std::sqrt(q.D_exc);
       d.exc_up = q.sigma_up * std::sqrt(q.D_exc);
     }
-    T.rad = p->rad.enable ? 1 : 0;
-    T.keys = A.keys;
-    T.n_cav = p->n_cav;
-    for (int c = 0; c < p->n_cav; ++c) { T.cav_amp[c] = A.cav_amp[c]; T.cav_w[c] = A.cav_w[c]; T.cav_ph[c] = A.cav_ph[c]; }
-    T.drift = A.drift;
-    T.lo_next = h->lo_next.p; T.lo_hist = h->lo_hist.p;
-    T.invDelta = A.invDelta; T.nb_d = A.nb_d; T.invE0 = A.invE0; T.gather = wk.gather_order;
-    T.Sx = h->Sx.p; T.Sy = h->Sy.p; T.Kx = h->Kx.p; T.Ky = h->Ky.p;
-    T.ctrl = h->ctrl.p;
+    T.cellX = h->cellX.p; T.cellY = h->cellY.p;
+    T.Sfix = h->Sfix.p; T.Sov = h->Sov.p; T.fix = h->fix.p; T.acc2 = h->acc2.p;
+    h->fn_map6 = select_map6(rad_on, wk.gather_order, p->n_cav);
+    h->fn_flush6 = select_flush6(wk.gather_order);
+    h->smem_pass6 = pass6_smem_bytes(nb);
+    CUH(cudaFuncSetAttribute((const void *)h->fn_map6, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass6));
+    CUH(cudaFuncSetAttribute((const void *)h->fn_flush6, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass6));
+    CUH(cudaFuncSetAttribute(k_wake_tr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)nb * 5 * sizeof(double))));
+    {
+      int occ = 0;
+      CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)h->fn_map6, kPassThreads, h->smem_pass6));
+      if (occ < 1) occ = 1;
+      const int64_t ppb = h->ld / 2;
+      int64_t iters = 16;
+      while (iters > 1 && (int64_t)M * ((ppb + iters * kPassThreads - 1) / (iters * kPassThreads)) < 2ll * prop.multiProcessorCount * occ) iters /= 2;
+      T.tile_pairs = (uint32_t)(iters * kPassThreads);
+      h->grid_pass6 = (int)((ppb + T.tile_pairs - 1) / T.tile_pairs);
+    }
+    TMomArgs &Tm = h->tmargs;
+    Tm.x = h->tx.p; Tm.xp = h->txp.p; Tm.y = h->ty.p; Tm.yp = h->typ.p; Tm.ld = h->ld; Tm.Np = (uint32_t)h->Np; Tm.tile = 8192;
+    h->grid_tr = (int)((h->Np + Tm.tile - 1) / Tm.tile);
     TWakeArgs &Tw = h->twargs;
     memset(&Tw, 0, sizeof Tw);
-    Tw.M = M; Tw.nb = nb; Tw.qm = h->qm.p; Tw.wt = h->wt.p;
-    Tw.Sx = h->Sx.p; Tw.Sy = h->Sy.p; Tw.Sx_last = h->Sx_last.p; Tw.Sy_last = h->Sy_last.p; Tw.Kx = h->Kx.p; Tw.Ky = h->Ky.p;
+    Tw.M = M; Tw.nb = nb; Tw.gather = wk.gather_order; Tw.fix_bits = h->fix_bits; Tw.Np = (uint32_t)h->Np;
+    Tw.qm = h->qm.p; Tw.wt = h->wt.p;
+    Tw.Sfix = h->Sfix.p; Tw.Sov = h->Sov.p; Tw.fix = h->fix.p; Tw.acc2 = h->acc2.p;
+    Tw.S_last = h->S_last.p; Tw.K = h->Ktab.p; Tw.cellX = h->cellX.p; Tw.cellY = h->cellY.p;
     dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)M);
     k_init_tr<<<grid, 256, 0, h->stream>>>(h->tx.p, h->txp.p, h->ty.p, h->typ.p, h->ld, (uint32_t)h->Np, A.keys,
                                            tr.x.sigma0_u_m, tr.x.sigma0_up, tr.y.sigma0_u_m, tr.y.sigma0_up);
+    if (int rc = rescale_transverse(h)) { destroy(h); return rc; }
     h->launches += 1;
     CUH(cudaGetLastError());
   }
@@ -709,11 +754,9 @@ int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, dou
   CU(cudaEventRecord(h->ev0, h->stream));
   for (int64_t t = 0; t < n_turns; ++t) {
     CU(cudaEventRecord(ev[3 * t], h->stream));
-    h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
+    enqueue_pass(h);
     CU(cudaEventRecord(ev[3 * t + 1], h->stream));
-    if (h->trans) enqueue_trans_map(h);  // the transverse kernels are timed with the wake kernel
-    k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
-    if (h->trans) enqueue_trans_kick(h);
+    enqueue_wakes(h);
     CU(cudaEventRecord(ev[3 * t + 2], h->stream));
   }
   CU(cudaEventRecord(h->ev1, h->stream));
@@ -859,7 +902,8 @@ int copy_in_packed(mbt_handle *h, const double *host, double *dev) {
 int mbt_get_transverse(mbt_handle *h, double *x, double *xp, double *y, double *yp) {
   if (!h || !h->trans || !x || !xp || !y || !yp) return fail(MBT_EINVAL, "transverse planes not enabled / null argument");
   CU(cudaSetDevice(h->device));
-  int rc;
+  int rc = flush(h);  // the transverse kick of the last turn may be pending, like the longitudinal one
+  if (rc) return rc;
   if ((rc = copy_out_packed(h, h->tx.p, x)) || (rc = copy_out_packed(h, h->txp.p, xp)) ||
       (rc = copy_out_packed(h, h->ty.p, y)) || (rc = copy_out_packed(h, h->typ.p, yp)))
     return rc;
@@ -869,19 +913,22 @@ int mbt_get_transverse(mbt_handle *h, double *x, double *xp, double *y, double *
 int mbt_set_transverse(mbt_handle *h, const double *x, const double *xp, const double *y, const double *yp) {
   if (!h || !h->trans || !x || !xp || !y || !yp) return fail(MBT_EINVAL, "transverse planes not enabled / null argument");
   CU(cudaSetDevice(h->device));
-  int rc;
+  int rc = flush(h);
+  if (rc) return rc;
   if ((rc = copy_in_packed(h, x, h->tx.p)) || (rc = copy_in_packed(h, xp, h->txp.p)) ||
       (rc = copy_in_packed(h, y, h->ty.p)) || (rc = copy_in_packed(h, yp, h->typ.p)))
     return rc;
+  if ((rc = rescale_transverse(h))) return rc;
+  CU(cudaStreamSynchronize(h->stream));
   return 0;
 }
 
 int mbt_get_dipole(mbt_handle *h, double *Sx, double *Sy) {
   if (!h || !h->trans) return fail(MBT_EINVAL, "transverse planes not enabled");
   CU(cudaSetDevice(h->device));
-  const size_t bytes = sizeof(double) * (size_t)h->M * h->nb;
-  if (Sx) CU(cudaMemcpyAsync(Sx, h->Sx_last.p, bytes, cudaMemcpyDeviceToHost, h->stream));
-  if (Sy) CU(cudaMemcpyAsync(Sy, h->Sy_last.p, bytes, cudaMemcpyDeviceToHost, h->stream));
+  const size_t row = sizeof(double) * (size_t)h->nb;  // device layout [M][2][nb]
+  if (Sx) CU(cudaMemcpy2DAsync(Sx, row, h->S_last.p, 2 * row, row, h->M, cudaMemcpyDeviceToHost, h->stream));
+  if (Sy) CU(cudaMemcpy2DAsync(Sy, row, h->S_last.p + h->nb, 2 * row, row, h->M, cudaMemcpyDeviceToHost, h->stream));
   CU(cudaStreamSynchronize(h->stream));
   return 0;
 }
@@ -889,9 +936,9 @@ int mbt_get_dipole(mbt_handle *h, double *Sx, double *Sy) {
 int mbt_get_transverse_wake(mbt_handle *h, double *Kx, double *Ky) {
   if (!h || !h->trans) return fail(MBT_EINVAL, "transverse planes not enabled");
   CU(cudaSetDevice(h->device));
-  const size_t bytes = sizeof(double) * (size_t)h->M * h->nb;
-  if (Kx) CU(cudaMemcpyAsync(Kx, h->Kx.p, bytes, cudaMemcpyDeviceToHost, h->stream));
-  if (Ky) CU(cudaMemcpyAsync(Ky, h->Ky.p, bytes, cudaMemcpyDeviceToHost, h->stream));
+  const size_t row = sizeof(double) * (size_t)h->nb;
+  if (Kx) CU(cudaMemcpy2DAsync(Kx, row, h->Ktab.p, 2 * row, row, h->M, cudaMemcpyDeviceToHost, h->stream));
+  if (Ky) CU(cudaMemcpy2DAsync(Ky, row, h->Ktab.p + h->nb, 2 * row, row, h->M, cudaMemcpyDeviceToHost, h->stream));
   CU(cudaStreamSynchronize(h->stream));
   return 0;
 }
@@ -899,8 +946,9 @@ int mbt_get_transverse_wake(mbt_handle *h, double *Kx, double *Ky) {
 int mbt_moments_transverse(mbt_handle *h, double *out) {
   if (!h || !h->trans || !out) return fail(MBT_EINVAL, "transverse planes not enabled / null argument");
   CU(cudaSetDevice(h->device));
+  if (int rc = flush(h)) return rc;
   CU(cudaMemsetAsync(h->mom_tr_acc.p, 0, sizeof(double) * h->M * 8, h->stream));
-  k_moments_tr<<<dim3(h->grid_tr, h->M), 256, 0, h->stream>>>(h->targs, h->mom_tr_acc.p);
+  k_moments_tr<<<dim3(h->grid_tr, h->M), 256, 0, h->stream>>>(h->tmargs, h->mom_tr_acc.p);
   k_close_moments_tr<<<(h->M + 127) / 128, 128, 0, h->stream>>>(h->M, (uint32_t)h->Np, h->mom_tr_acc.p, h->mom_tr.p);
   h->launches += 2;
   CU(cudaGetLastError());

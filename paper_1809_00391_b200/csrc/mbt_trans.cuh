@@ -1,184 +1,409 @@
 // mbt_trans.cuh -- transverse planes (P:l.73-92 Eqs.(3)-(5), l.100-111 Eq.(6b); DESIGN.md
-// readings T1..T8).  First correct CUDA path of this row: the transverse steps of a turn run in kernels of their own
-// around the wake kernel, after the fused longitudinal pass (which is untouched):
+// readings T1..T8), fused with the longitudinal path: a handle with the planes enabled runs, per turn,
 //
-//   k_pass        longitudinal: kick of turn n-1, map, binning of turn n            (mbt_kernels.cuh)
-//   k_trans_map   Eqs. (3), (4) with the turn's delta, Eq. (5) lines 2-3, dipole deposit on the turn's window
-//   k_wake        longitudinal wake of turn n                                       (mbt_kernels.cuh)
-//   k_wake_tr     per bunch: K[j] = sum_{k<j} (Q_b/N_p) S[k] W_perp((j-k) Delta) for both planes
-//   k_trans_kick  u' += K(tau)/E0 (gather as the longitudinal one); no transverse kick is ever pending
+//   k_pass6    one pass over the 6-D SoA store (96 B per particle-turn): both kicks of turn n-1, the longitudinal
+//              map and the betatron map / excitation of turn n, counts and dipole sums of turn n
+//   k_wake     longitudinal wake of turn n                                        (mbt_kernels.cuh, unchanged)
+//   k_wake_tr  per bunch: K[j] = sum_{k<j} (Q_b/N_p) S[k] W_perp((j-k) Delta) for both planes, gather cells
 //
-// Not fused and not tuned yet (library sincos / log, shared-memory fp64 atomics for the dipole sums): the bar of this
-// stage is parity with the oracle.  Traffic: 80 B (map) + 56 B (kick) per particle-turn beside the pass's 32 B.
+// and, like the longitudinal kick, the transverse kick of the last tracked turn stays pending until the next pass or
+// a getter's flush pass (k_pass6<false>) applies it.
 #pragma once
 #include "mbt_kernels.cuh"
 
 namespace mbt {
 
 struct Plane {
-  double two_pi_nu, xi, alpha, beta, gamma, eta, etap;
+  double t_frac;  // nu - floor(nu): the betatron phase in turns, Psi / (2 pi) = nu (1 + xi delta), is used mod 1
+  double t_xi;    // nu xi
+  double alpha, beta, gamma, eta, etap;
   double exc_u, exc_up;  // sigma_u sqrt(D_exc), sigma_up sqrt(D_exc)
 };
 
-struct TArgs {
-  const double *tau, *delta;  // [M][ld] longitudinal store (read only here)
-  double *x, *xp, *y, *yp;    // [M][ld]
-  int64_t ld;
-  uint32_t Np;
-  int32_t M, nb;
-  uint32_t tile;              // particles per CTA
-  Plane px, py;
-  int32_t rad;
-  PhiloxKeys keys;
-  // RF gain eps of Eq. (5): sum_c amp_c sin(w_c tau_before_drift + ph_c)
-  int32_t n_cav;
-  double cav_amp[kMaxCav], cav_w[kMaxCav], cav_ph[kMaxCav];
-  double drift;
-  // binning (as the pass)
-  const double *lo_next;      // [M] window of this turn's binning (read by k_trans_map, before k_wake rotates it)
-  const double *lo_hist;      // [M] the same window after k_wake (read by k_trans_kick)
-  double invDelta, nb_d, invE0;
-  int32_t gather;
-  double *Sx, *Sy;            // [M][nb] dipole sums of the turn in flight (accumulated, consumed by k_wake_tr)
-  const double *Kx, *Ky;      // [M][nb] kick tables [V]
-  const Ctrl *ctrl;
+// Dipole sums in fixed point.  Shared memory has no native fp64 (nor 64-bit integer) atomic add -- both compile to a
+// compare-and-swap loop, measured at 6 ps per particle for two sums against 0.5 ps for the integer histogram -- so a
+// particle's offset is deposited as a 64-bit integer v = rint(u 2^kFixBits / X_max) split over two native 32-bit
+// atomics: the low word's returned old value tells the one thread whose addition wraps it, and that thread adds the
+// carry to the high word (1.7 ps per particle for both planes, measured).  X_max = 2^E >= 64 rms(u) comes from the
+// bunch's <u^2> of the turn before; a particle with |u| >= X_max (none in a Gaussian bunch) adds its offset in fp64
+// to a global table instead, so the sum is right for any input.  Integer sums do not depend on the order of
+// addition: S is reproducible bit for bit from run to run.  Rounding: 2^-kFixBits X_max per particle.
+constexpr int kFixBitsMax = 44;
+struct FixScale {
+  double inv_lsb;    // 2^fix_bits / X_max (a power of two: the scaling is exact)
+  double lsb;        // X_max / 2^fix_bits
+  uint32_t xmax_hi;  // high word of X_max; |u| < X_max  <=>  (hi(u) & 0x7fffffff) < xmax_hi
+  uint32_t pad;
 };
 
-// Eqs. (3), (4) for one plane (readings T2, T3), operation order as the oracle's
-__device__ __forceinline__ void betatron_map(const Plane &p, double &u, double &up, double d) {
-  const double psi = __dmul_rn(p.two_pi_nu, __dadd_rn(1.0, __dmul_rn(p.xi, d)));
-  double sn, c;
-  sincos(psi, &sn, &c);
-  const double ub = u - p.eta * d, upb = up - p.etap * d;
-  const double un = (c + p.alpha * sn) * ub + p.beta * sn * upb;
-  const double upn = -p.gamma * sn * ub + (c - p.alpha * sn) * upb;
-  u = p.eta * d + un;
-  up = p.etap * d + upn;
+struct Args6 {
+  Args L;                      // the longitudinal pass's arguments (mbt_kernels.cuh), same meaning
+  double *x, *xp, *y, *yp;     // [M][ld]
+  Plane px, py;
+  const WakeCell *cellX, *cellY;  // [M][nb+2] gather cells of the kick tables K_x, K_y of the last turn (k_wake_tr)
+  unsigned long long *Sfix;    // [M][2][nb] dipole sums of the turn in flight, fixed point (two's complement)
+  double *Sov;                 // [M][2][nb] ... of the particles beyond X_max
+  const FixScale *fix;         // [M][2]
+  double *acc2;                // [M][2] sum u^2 of the mapped state (the next turn's scale)
+  uint32_t tile_pairs;         // pairs per CTA
+};
+
+__host__ __device__ inline size_t pass6_smem_bytes(int nb) {
+  return (size_t)(nb + 2) * 3 * sizeof(WakeCell) + 128 * sizeof(LogTabEntry) + (size_t)(nb + 1) * 5 * sizeof(uint32_t) + 16;
 }
 
-__device__ __forceinline__ double uniform32_plain(uint32_t x) { return ((double)x + 0.5) * 0x1p-32; }
+// sin, cos of 2 pi t: q = rint(2 t), f = t - q/2 in [-1/4, 1/4] (exact), polynomials of mbt_math.cuh, sign (-1)^q
+__device__ __forceinline__ void sincos_turns(const MathTab &C, double t, double &sn, double &cs) {
+  const double qm = fma(t, 2.0, MBT_MAGIC);
+  const int q = __double2loint(qm);
+  const double f = fma(qm - MBT_MAGIC, -0.5, t), f2 = f * f;
+  const double ps = MBT_POLY7(C.sinf, MBT_SINF_I4, MBT_SINF_I5, f2), pc = MBT_POLY7(C.cosf, MBT_COSF_I4, MBT_COSF_I5, f2);
+  sn = flip_sign_if_odd(f * fma(f2, ps, C.two_pi), q);
+  cs = flip_sign_if_odd(fma(f2, pc, 1.0), q);
+}
 
-// after k_pass of turn n (tau, delta: mapped, not yet kicked by this turn's wake) and before k_wake of turn n
-template <bool RAD>
-__global__ void __launch_bounds__(256) k_trans_map(const __grid_constant__ TArgs A) {
-  extern __shared__ double s_dip[];  // [2][nb]
-  double *sSx = s_dip, *sSy = s_dip + A.nb;
-  const int b = blockIdx.y, tid = threadIdx.x;
-  for (int j = tid; j < 2 * A.nb; j += 256) s_dip[j] = 0.0;
+// Eqs. (3), (4) for one plane (readings T2, T3).  The oracle rounds Psi = 2 pi nu (1 + xi delta) at |Psi| ~ 100 rad
+// (2e-14 rad); here the phase is reduced exactly in turns first, so the two differ by that rounding (<< 1e-12).
+__device__ __forceinline__ void betatron_map(const MathTab &C, const Plane &p, double &u, double &up, double d) {
+  double sn, cs;
+  sincos_turns(C, fma(p.t_xi, d, p.t_frac), sn, cs);
+  const double ub = fma(-p.eta, d, u), upb = fma(-p.etap, d, up);
+  const double un = fma(fma(p.alpha, sn, cs), ub, (p.beta * sn) * upb);
+  const double upn = fma(fma(-p.alpha, sn, cs), upb, -((p.gamma * sn) * ub));
+  u = fma(p.eta, d, un);
+  up = fma(p.etap, d, upn);
+}
+
+// num / den for den near 1: MUFU.RCP64H seed (2^-22), two Newton steps, one residual correction (<= 1 ulp)
+__device__ __forceinline__ double div_near_one(double num, double den) {
+  double r = rcp_approx_f64(den);
+  r = fma(r, fma(-den, r, 1.0), r);
+  r = fma(r, fma(-den, r, 1.0), r);
+  const double q = num * r;
+  return fma(fma(-den, q, num), r, q);
+}
+
+// Fused 6-D pass (readings T1..T8 on top of the longitudinal S0..S7):
+//   head : kicks of turn n-1 -- longitudinal (S0) and transverse (Eq. 6b), gathered at the same bin position; S7
+//   MAP  : S1 S2 S3 of turn n, Eqs. (3), (4) with the turn's delta, Eq. (5) lines 2-3, then S4: counts and dipole sums
+// One pair of particles per thread and iteration, 96 bytes per particle-turn.  MAP = false is the flush pass.
+template <bool MAP, bool RAD, int GATHER, int NCAV>
+__global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant__ Args6 A6) {
+  const Args &A = A6.L;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int nb = A.nb;
+  WakeCell *sW = reinterpret_cast<WakeCell *>(smem_raw);       // [nb+2] longitudinal
+  WakeCell *sX = sW + (nb + 2), *sY = sX + (nb + 2);           // [nb+2] each
+  LogTabEntry *sL = reinterpret_cast<LogTabEntry *>(sY + (nb + 2));  // [128]
+  uint32_t *sH = reinterpret_cast<uint32_t *>(sL + 128);       // [nb+1] counts, bin nb is a sink
+  uint32_t *sLo = sH + (nb + 1), *sHi = sLo + 2 * (nb + 1);    // [2][nb+1] each: low / high words of the dipole sums
+  __shared__ double s_red[kPassThreads / 32][6];
+  __shared__ uint32_t s_nout[kPassThreads / 32];
+
+  const int tid = threadIdx.x, b = (int)blockIdx.y;
+  const uint32_t n = A.ctrl->turn + 1u;
+  const bool have_kick = A.ctrl->kick_pending != 0u;
+  const uint32_t hi_nb = (uint32_t)__double2hiint(A.nb_d);
+  const uint32_t p0 = blockIdx.x * A6.tile_pairs;
+  const uint32_t p1 = (A.ppb - p0 < A6.tile_pairs) ? A.ppb : p0 + A6.tile_pairs;
+  const double lo_old = A.lo_hist[b];
+  const double lo_new = MAP ? A.lo_next[b] : lo_old;
+  const FixScale fx = A6.fix[2 * b], fy = A6.fix[2 * b + 1];
+
+  if (MAP && RAD)
+    for (int i = tid; i < 128; i += kPassThreads) sL[i] = A.logtab[i];
+  for (int k = tid; k < nb + 2; k += kPassThreads) {
+    WakeCell c{0.0, 0.0}, cx{0.0, 0.0}, cy{0.0, 0.0};
+    if (have_kick) {
+      c = A.cellSR[(size_t)b * (nb + 2) + k];
+#pragma unroll 1
+      for (int r = 0; r < A.R; ++r) {
+        const CellF f = A.cellF[(size_t)r * (nb + 2) + k];
+        const cplx pb = A.P[(size_t)b * A.R + r];
+        c.mid += fma(f.mid.re, pb.re, -(f.mid.im * pb.im));
+        c.dif += fma(f.dif.re, pb.re, -(f.dif.im * pb.im));
+      }
+      cx = A6.cellX[(size_t)b * (nb + 2) + k];
+      cy = A6.cellY[(size_t)b * (nb + 2) + k];
+    }
+    sW[k] = c; sX[k] = cx; sY[k] = cy;
+  }
+  for (int k = tid; k < 5 * (nb + 1); k += kPassThreads) sH[k] = 0u;
   __syncthreads();
-  const uint32_t n = A.ctrl->turn + 1u;  // k_wake has not bumped the counter yet: the turn in flight
-  const double lo = A.lo_next[b];
-  const uint32_t i0 = blockIdx.x * A.tile, i1 = min(i0 + A.tile, A.Np);
+
+  double st = 0.0, sd = 0.0, stt = 0.0, sdd = 0.0, sxx = 0.0, syy = 0.0;
+  uint32_t nout = 0u;
   const size_t base = (size_t)b * A.ld;
-  for (uint32_t i = i0 + tid; i < i1; i += 256) {
-    const double tau = A.tau[base + i], d = A.delta[base + i];
-    double x = A.x[base + i], xp = A.xp[base + i], y = A.y[base + i], yp = A.yp[base + i];
-    betatron_map(A.px, x, xp, d);
-    betatron_map(A.py, y, yp, d);
-    if (RAD) {
-      // Eq. (5) lines 2, 3 (T4, T5): one Philox block per particle, counter (i, b, n, tag 2) -> (r_x, r_x', r_y, r_y')
-      uint32_t w0, w1, w2, w3;
-      philox4x32_10(i, (uint32_t)b, n, 2u, A.keys, w0, w1, w2, w3);
-      double z0, z1, z2, z3;
-      box_muller_accurate(uniform32_plain(w0), uniform32_plain(w1), z0, z1);
-      box_muller_accurate(uniform32_plain(w2), uniform32_plain(w3), z2, z3);
-      const double tau_old = fma(-A.drift, d, tau);  // tau before this turn's drift (to a rounding)
-      double eps = 0.0;
-      for (int c = 0; c < A.n_cav; ++c) eps += A.cav_amp[c] * sin(__dadd_rn(__dmul_rn(A.cav_w[c], tau_old), A.cav_ph[c]));
-      const double adia = (1.0 + d) / (1.0 + d + eps);
-      x += A.px.exc_u * z0;
-      xp = xp * adia + A.px.exc_up * z1;
-      y += A.py.exc_u * z2;
-      yp = yp * adia + A.py.exc_up * z3;
+  for (uint32_t p = p0 + (uint32_t)tid; p < p1; p += kPassThreads) {
+    const size_t o = base + 2u * (size_t)p;
+    const double2 t2 = *reinterpret_cast<const double2 *>(A.tau + o), d2 = *reinterpret_cast<const double2 *>(A.delta + o);
+    const double2 x2 = *reinterpret_cast<const double2 *>(A6.x + o), xp2 = *reinterpret_cast<const double2 *>(A6.xp + o);
+    const double2 y2 = *reinterpret_cast<const double2 *>(A6.y + o), yp2 = *reinterpret_cast<const double2 *>(A6.yp + o);
+    double tau[2] = {t2.x, t2.y}, del[2] = {d2.x, d2.y};
+    double x[2] = {x2.x, x2.y}, xp[2] = {xp2.x, xp2.y}, y[2] = {y2.x, y2.y}, yp[2] = {yp2.x, yp2.y};
+    const bool live[2] = {2u * p < A.Np, 2u * p + 1u < A.Np};  // the slots from N_p up to ld are padding
+    double t[2];
+    bool in[2];
+    // kicks of the previous turn (S0, Eq. 6b): t as the binning computed it
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      t[i] = __dmul_rn(__dsub_rn(tau[i], lo_old), A.invDelta);
+      in[i] = live[i] && in_window(t[i], hi_nb);
+      int kk;
+      double f;
+      if (GATHER == 1) {
+        const double km = t[i] + MBT_MAGIC;
+        kk = __double2loint(km);
+        f = t[i] - (km - MBT_MAGIC);
+      } else {
+        kk = __double2int_rd(t[i]);
+        f = 0.0;
+      }
+      kk = in[i] ? kk : nb + 1;
+      const WakeCell c = sW[kk], cx = sX[kk], cy = sY[kk];
+      del[i] = fma(-fma(f, c.dif, c.mid), A.invE0, del[i]);
+      xp[i] = fma(fma(f, cx.dif, cx.mid), A.invE0, xp[i]);
+      yp[i] = fma(fma(f, cy.dif, cy.mid), A.invE0, yp[i]);
+      if (!in[i] && live[i]) nout += 1u;
+      if (live[i]) {  // S7
+        st += tau[i];
+        sd += del[i];
+        stt = fma(tau[i], tau[i], stt);
+        sdd = fma(del[i], del[i], sdd);
+      }
     }
-    A.x[base + i] = x; A.xp[base + i] = xp; A.y[base + i] = y; A.yp[base + i] = yp;
-    // T6: dipole sums on the bins of this turn's histogram (the pass's S4 arithmetic)
-    const double t = __dmul_rn(__dsub_rn(tau, lo), A.invDelta);
-    if (t >= 0.0 && t < A.nb_d) {
-      const int j = __double2int_rd(t);
-      atomicAdd(&sSx[j], x);
-      atomicAdd(&sSy[j], y);
+    if (MAP) {
+      double z[2] = {0.0, 0.0};
+      if (RAD) {  // D8: the Philox block of the quad (p >> 1); its half (p & 1) is this pair's Box-Muller pair
+        uint32_t w0, w1, w2, w3;
+        philox4x32_10(p >> 1, (uint32_t)b, n, 0u, A.keys, w0, w1, w2, w3);
+        const bool hi_half = (p & 1u) != 0u;
+        box_muller_fast(A.mt, sL, uniform32(A.mt, hi_half ? w2 : w0), uniform32(A.mt, hi_half ? w3 : w1), A.A_q, z[0], z[1]);
+      }
+#pragma unroll
+      for (int i = 0; i < 2; ++i) {
+        // S1; eps = the particle's RF gain of this turn (the epsilon of Eq. 5, T4)
+        double eps = 0.0;
+        if (NCAV > 0) {
+#pragma unroll
+          for (int c = 0; c < NCAV; ++c) {
+            const double yv = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
+            double sv = sin_rf_fast(A.mt, yv);
+            if (__builtin_expect(!(fabs(yv) < 65536.0), 0)) sv = sin_rf_slow(yv);
+            del[i] = fma(A.cav_amp[c], sv, del[i]);
+            eps = fma(A.cav_amp[c], sv, eps);
+          }
+        } else {
+#pragma unroll 1
+          for (int c = 0; c < A.n_cav; ++c) {
+            const double yv = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
+            double sv = sin_rf_fast(A.mt, yv);
+            if (__builtin_expect(!(fabs(yv) < 65536.0), 0)) sv = sin_rf_slow(yv);
+            del[i] = fma(A.cav_amp[c], sv, del[i]);
+            eps = fma(A.cav_amp[c], sv, eps);
+          }
+        }
+        del[i] -= A.loss;
+        if (RAD) del[i] = fma(del[i], A.one_minus_DE, z[i]);  // S2
+        tau[i] = fma(A.drift, del[i], tau[i]);                // S3
+        // Eqs. (3), (4) with the turn's delta (T1)
+        betatron_map(A.mt, A6.px, x[i], xp[i], del[i]);
+        betatron_map(A.mt, A6.py, y[i], yp[i], del[i]);
+        if (RAD) {
+          // Eq. (5) lines 2, 3 (T4, T5): one Philox block per particle, counter (i, b, n, tag 2) -> (r_x, r_x', r_y, r_y')
+          uint32_t w0, w1, w2, w3;
+          philox4x32_10(2u * p + (uint32_t)i, (uint32_t)b, n, 2u, A.keys, w0, w1, w2, w3);
+          double z0, z1, z2, z3;
+          box_muller_fast(A.mt, sL, uniform32(A.mt, w0), uniform32(A.mt, w1), 1.0, z0, z1);
+          box_muller_fast(A.mt, sL, uniform32(A.mt, w2), uniform32(A.mt, w3), 1.0, z2, z3);
+          const double num = 1.0 + del[i];
+          const double adia = div_near_one(num, num + eps);
+          x[i] = fma(A6.px.exc_u, z0, x[i]);
+          xp[i] = fma(xp[i], adia, A6.px.exc_up * z1);
+          y[i] = fma(A6.py.exc_u, z2, y[i]);
+          yp[i] = fma(yp[i], adia, A6.py.exc_up * z3);
+        }
+        t[i] = __dmul_rn(__dsub_rn(tau[i], lo_new), A.invDelta);  // S4
+        in[i] = live[i] && in_window(t[i], hi_nb);
+      }
     }
+    // S4: counts, and (MAP) the dipole sums of the turn's bins (T6).  Branch-free: everything that is not in the
+    // window lands in the sink bin nb.
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const int j = in[i] ? __double2int_rd(t[i]) : nb;
+      atomicAdd(&sH[j], 1u);
+      if (MAP) {
+        if (live[i]) {
+          sxx = fma(x[i], x[i], sxx);
+          syy = fma(y[i], y[i], syy);
+        }
+        const bool okx = ((uint32_t)__double2hiint(x[i]) & 0x7FFFFFFFu) < fx.xmax_hi;
+        const bool oky = ((uint32_t)__double2hiint(y[i]) & 0x7FFFFFFFu) < fy.xmax_hi;
+        const double mx = fma(okx ? x[i] : 0.0, fx.inv_lsb, MBT_MAGIC), my = fma(oky ? y[i] : 0.0, fy.inv_lsb, MBT_MAGIC);
+        const uint32_t xl = (uint32_t)__double2loint(mx), xh = (uint32_t)(__double2hiint(mx) - 0x43380000);
+        const uint32_t yl = (uint32_t)__double2loint(my), yh = (uint32_t)(__double2hiint(my) - 0x43380000);
+        const uint32_t ox = atomicAdd(&sLo[j], xl), oy = atomicAdd(&sLo[(nb + 1) + j], yl);
+        atomicAdd(&sHi[j], xh + ((ox + xl) < xl ? 1u : 0u));
+        atomicAdd(&sHi[(nb + 1) + j], yh + ((oy + yl) < yl ? 1u : 0u));
+        if (__builtin_expect(in[i] && !(okx && oky), 0)) {  // beyond X_max: fp64, straight to the global table
+          if (!okx) atomicAdd(&A6.Sov[((size_t)b * 2) * nb + j], x[i]);
+          if (!oky) atomicAdd(&A6.Sov[((size_t)b * 2 + 1) * nb + j], y[i]);
+        }
+      }
+    }
+    if (MAP) {
+      *reinterpret_cast<double2 *>(A.tau + o) = make_double2(tau[0], tau[1]);
+      *reinterpret_cast<double2 *>(A6.x + o) = make_double2(x[0], x[1]);
+      *reinterpret_cast<double2 *>(A6.y + o) = make_double2(y[0], y[1]);
+    }
+    *reinterpret_cast<double2 *>(A.delta + o) = make_double2(del[0], del[1]);
+    *reinterpret_cast<double2 *>(A6.xp + o) = make_double2(xp[0], xp[1]);
+    *reinterpret_cast<double2 *>(A6.yp + o) = make_double2(yp[0], yp[1]);
+  }
+
+  // S7 and the scale sums: warp shuffles, then one atomic per CTA and bunch
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    st += __shfl_down_sync(0xffffffffu, st, o);
+    sd += __shfl_down_sync(0xffffffffu, sd, o);
+    stt += __shfl_down_sync(0xffffffffu, stt, o);
+    sdd += __shfl_down_sync(0xffffffffu, sdd, o);
+    sxx += __shfl_down_sync(0xffffffffu, sxx, o);
+    syy += __shfl_down_sync(0xffffffffu, syy, o);
+    nout += __shfl_down_sync(0xffffffffu, nout, o);
+  }
+  if ((tid & 31) == 0) {
+    double *r = s_red[tid >> 5];
+    r[0] = st; r[1] = sd; r[2] = stt; r[3] = sdd; r[4] = sxx; r[5] = syy;
+    s_nout[tid >> 5] = nout;
   }
   __syncthreads();
-  for (int j = tid; j < A.nb; j += 256) {
-    if (sSx[j] != 0.0) atomicAdd(&A.Sx[(size_t)b * A.nb + j], sSx[j]);
-    if (sSy[j] != 0.0) atomicAdd(&A.Sy[(size_t)b * A.nb + j], sSy[j]);
+  if (tid < 6) {
+    double s = 0.0;
+#pragma unroll
+    for (int w = 0; w < kPassThreads / 32; ++w) s += s_red[w][tid];
+    if (tid < 4) atomicAdd(&A.mom_acc[(size_t)b * 4 + tid], s);
+    else if (MAP) atomicAdd(&A6.acc2[(size_t)b * 2 + (tid - 4)], s);
+  } else if (tid == 6) {
+    uint32_t s = 0u;
+#pragma unroll
+    for (int w = 0; w < kPassThreads / 32; ++w) s += s_nout[w];
+    if (s) atomicAdd(&A.nout_acc[b], (unsigned long long)s);
+  }
+  for (int j = tid; j < nb; j += kPassThreads) {
+    const uint32_t c = sH[j];
+    if (c) atomicAdd(&A.hist[(size_t)b * nb + j], c);
+    if (MAP) {
+#pragma unroll
+      for (int a = 0; a < 2; ++a) {
+        const unsigned long long v = ((unsigned long long)sHi[a * (nb + 1) + j] << 32) | sLo[a * (nb + 1) + j];
+        if (v) atomicAdd(&A6.Sfix[((size_t)b * 2 + a) * nb + j], v);
+      }
+    }
   }
 }
 
 struct TWakeArgs {
-  int32_t M, nb;
+  int32_t M, nb, gather, fix_bits;
+  uint32_t Np;
   const double *qm;     // [M]
   const double *wt;     // [nb] transverse table wt[k] = sum_r W_perp_r(k Delta), wt[0] = 0
-  double *Sx, *Sy;      // [M][nb] in: sums of this turn; out: zero
-  double *Sx_last, *Sy_last;  // [M][nb] observable copy
-  double *Kx, *Ky;      // [M][nb] out
+  unsigned long long *Sfix;   // [M][2][nb] in: sums of this turn; out: zero
+  double *Sov;                // [M][2][nb] likewise
+  FixScale *fix;              // [M][2] in: the scale the sums were deposited with; out: the next turn's
+  double *acc2;               // [M][2] in: sum u^2 of this turn's mapped state; out: zero
+  double *S_last;             // [M][2][nb] observable copy of the sums [m]
+  double *K;                  // [M][2][nb] kick tables [V]
+  WakeCell *cellX, *cellY;    // [M][nb+2] their gather cells (as WakeCell of mbt_kernels.cuh)
 };
 
-// Eq. (6b): strictly causal sum over the earlier bins; one CTA per bunch
+// X_max = 2^E >= 64 sqrt(<u^2>) (E clamped; <u^2> = 0 or not finite: E = 0, every non-zero offset then takes the fp64 path)
+__device__ __forceinline__ FixScale make_fix_scale(double mean_sq, int fix_bits) {
+  int E = 0;
+  if (mean_sq > 0.0 && mean_sq < 1.0e300) {
+    int e2;
+    frexp(mean_sq, &e2);             // mean_sq = m 2^e2, m in [1/2, 1)  ->  rms < 2^((e2 + 1) / 2)
+    E = ((e2 + 1) >> 1) + 6;         // ceil(e2 / 2) + 6
+    E = max(-400, min(400, E));
+  }
+  FixScale f;
+  f.inv_lsb = scalbn(1.0, fix_bits - E);
+  f.lsb = scalbn(1.0, E - fix_bits);
+  f.xmax_hi = (uint32_t)__double2hiint(scalbn(1.0, E));
+  f.pad = 0u;
+  return f;
+}
+
+// Eq. (6b): strictly causal sum over the earlier bins, both planes; one CTA per bunch.  Also closes the fixed-point
+// dipole sums of the turn and chooses the next turn's scale.
 __global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeArgs A) {
-  extern __shared__ double s_w[];  // [3][nb]: wt, q Sx, q Sy
-  double *sw = s_w, *sx = s_w + A.nb, *sy = s_w + 2 * A.nb;
+  extern __shared__ double s_w[];  // [5][nb]: wt, q Sx, q Sy, Kx, Ky
   const int b = blockIdx.x, tid = threadIdx.x, nb = A.nb;
+  double *sw = s_w, *sx = s_w + nb, *sy = s_w + 2 * nb, *kx = s_w + 3 * nb, *ky = s_w + 4 * nb;
   const double qm = A.qm[b];
+  const FixScale fx = A.fix[2 * b], fy = A.fix[2 * b + 1];
+  const size_t ox = ((size_t)b * 2) * nb, oy = ox + nb;
   for (int j = tid; j < nb; j += 256) {
-    const double vx = A.Sx[(size_t)b * nb + j], vy = A.Sy[(size_t)b * nb + j];
-    A.Sx_last[(size_t)b * nb + j] = vx;
-    A.Sy_last[(size_t)b * nb + j] = vy;
-    A.Sx[(size_t)b * nb + j] = 0.0;
-    A.Sy[(size_t)b * nb + j] = 0.0;
+    const double vx = fma((double)(long long)A.Sfix[ox + j], fx.lsb, A.Sov[ox + j]);
+    const double vy = fma((double)(long long)A.Sfix[oy + j], fy.lsb, A.Sov[oy + j]);
+    A.Sfix[ox + j] = 0ull; A.Sfix[oy + j] = 0ull;
+    A.Sov[ox + j] = 0.0; A.Sov[oy + j] = 0.0;
+    A.S_last[ox + j] = vx; A.S_last[oy + j] = vy;
     sx[j] = qm * vx;
     sy[j] = qm * vy;
     sw[j] = A.wt[j];
   }
   __syncthreads();
+  if (tid < 2) {
+    A.fix[2 * b + tid] = make_fix_scale(A.acc2[2 * b + tid] / (double)A.Np, A.fix_bits);
+    A.acc2[2 * b + tid] = 0.0;
+  }
   for (int j = tid; j < nb; j += 256) {
-    double kx = 0.0, ky = 0.0;
+    double ax = 0.0, ay = 0.0;
     for (int k = 0; k < j; ++k) {
-      kx = fma(sw[j - k], sx[k], kx);
-      ky = fma(sw[j - k], sy[k], ky);
+      ax = fma(sw[j - k], sx[k], ax);
+      ay = fma(sw[j - k], sy[k], ay);
     }
-    A.Kx[(size_t)b * nb + j] = kx;
-    A.Ky[(size_t)b * nb + j] = ky;
+    kx[j] = ax; ky[j] = ay;
+    A.K[ox + j] = ax;
+    A.K[oy + j] = ay;
+  }
+  __syncthreads();
+  for (int k = tid; k < nb + 2; k += 256) {
+    WakeCell cx{0.0, 0.0}, cy{0.0, 0.0};
+    if (A.gather == 1) {
+      if (k <= nb) {
+        const int lo = k > 0 ? k - 1 : 0, hi = k < nb ? k : nb - 1;
+        cx.mid = 0.5 * (kx[lo] + kx[hi]); cx.dif = kx[hi] - kx[lo];
+        cy.mid = 0.5 * (ky[lo] + ky[hi]); cy.dif = ky[hi] - ky[lo];
+      }
+    } else if (k < nb) {
+      cx.mid = kx[k];
+      cy.mid = ky[k];
+    }
+    A.cellX[(size_t)b * (nb + 2) + k] = cx;
+    A.cellY[(size_t)b * (nb + 2) + k] = cy;
   }
 }
 
-// after k_wake and k_wake_tr of turn n: u' += K(tau)/E0 for in-window particles (T7, T8)
-__global__ void __launch_bounds__(256) k_trans_kick(const __grid_constant__ TArgs A) {
-  extern __shared__ double s_k[];  // [2][nb]
-  double *sKx = s_k, *sKy = s_k + A.nb;
-  const int b = blockIdx.y, tid = threadIdx.x, nb = A.nb;
-  for (int j = tid; j < nb; j += 256) { sKx[j] = A.Kx[(size_t)b * nb + j]; sKy[j] = A.Ky[(size_t)b * nb + j]; }
-  __syncthreads();
-  const double lo = A.lo_hist[b];
-  const uint32_t i0 = blockIdx.x * A.tile, i1 = min(i0 + A.tile, A.Np);
-  const size_t base = (size_t)b * A.ld;
-  for (uint32_t i = i0 + tid; i < i1; i += 256) {
-    const double t = __dmul_rn(__dsub_rn(A.tau[base + i], lo), A.invDelta);
-    if (!(t >= 0.0 && t < A.nb_d)) continue;
-    double vx, vy;
-    if (A.gather == 0) {
-      const int j = __double2int_rd(t);
-      vx = sKx[j]; vy = sKy[j];
-    } else {
-      const double u = t - 0.5;
-      if (u <= 0.0) { vx = sKx[0]; vy = sKy[0]; }
-      else if (u >= (double)(nb - 1)) { vx = sKx[nb - 1]; vy = sKy[nb - 1]; }
-      else {
-        const int j0 = __double2int_rd(u);
-        const double f = u - (double)j0;
-        vx = sKx[j0] + f * (sKx[j0 + 1] - sKx[j0]);
-        vy = sKy[j0] + f * (sKy[j0 + 1] - sKy[j0]);
-      }
-    }
-    A.xp[base + i] += vx * A.invE0;
-    A.yp[base + i] += vy * A.invE0;
-  }
+// scale of the fixed-point dipole sums from the state in memory (create, mbt_set_transverse): acc[M][8] of k_moments_tr
+__global__ void k_fix_scale(int M, uint32_t Np, int fix_bits, const double *acc, FixScale *fix) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= 2 * M) return;
+  const int b = i >> 1, a = i & 1;
+  fix[i] = make_fix_scale(acc[b * 8 + 4 + 2 * a] / (double)Np, fix_bits);
 }
 
 // sums for mbt_moments_transverse: out[M][8] += (sum x, x', y, y', sum x^2, x'^2, y^2, y'^2)
-__global__ void __launch_bounds__(256) k_moments_tr(const __grid_constant__ TArgs A, double *acc) {
+__device__ __forceinline__ double uniform32_plain(uint32_t x) { return ((double)x + 0.5) * 0x1p-32; }
+
+struct TMomArgs {
+  const double *x, *xp, *y, *yp;
+  int64_t ld;
+  uint32_t Np, tile;
+};
+__global__ void __launch_bounds__(256) k_moments_tr(const TMomArgs A, double *acc) {
   __shared__ double s_red[8][8];
   const int b = blockIdx.y, tid = threadIdx.x;
   const uint32_t i0 = blockIdx.x * A.tile, i1 = min(i0 + A.tile, A.Np);
