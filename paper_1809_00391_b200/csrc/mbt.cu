@@ -674,7 +674,10 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     T.Sfix = h->Sfix.p; T.Sov = h->Sov.p; T.fix = h->fix.p; T.acc2 = h->acc2.p;
     h->fn_map6 = select_map6(rad_on, wk.gather_order, p->n_cav);
     h->fn_flush6 = select_flush6(wk.gather_order);
-    h->smem_pass6 = pass6_smem_bytes(nb);
+    // three stages in flight if two CTAs then still fit an SM, else two
+    T.stages = (2 * (pass6_smem_bytes(nb, 3) + 1024) <= (size_t)prop.sharedMemPerMultiprocessor) ? 3 : 2;
+    if (const char *e = getenv("MBT_STAGES6")) T.stages = std::min(kMaxStages6, std::max(2, atoi(e)));  // measurement knob
+    h->smem_pass6 = pass6_smem_bytes(nb, T.stages);
     CUH(cudaFuncSetAttribute((const void *)h->fn_map6, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass6));
     CUH(cudaFuncSetAttribute((const void *)h->fn_flush6, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass6));
     CUH(cudaFuncSetAttribute(k_wake_tr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)nb * 5 * sizeof(double))));

@@ -46,10 +46,17 @@ struct Args6 {
   const FixScale *fix;         // [M][2]
   double *acc2;                // [M][2] sum u^2 of the mapped state (the next turn's scale)
   uint32_t tile_pairs;         // pairs per CTA
+  int32_t stages;              // shared-memory stages of the particle stream (2..kMaxStages6)
 };
 
-__host__ __device__ inline size_t pass6_smem_bytes(int nb) {
-  return (size_t)(nb + 2) * 3 * sizeof(WakeCell) + 128 * sizeof(LogTabEntry) + (size_t)(nb + 1) * 5 * sizeof(uint32_t) + 16;
+// Particle staging as in k_pass: `stages` shared-memory stages of kPassThreads pairs x six arrays (24 KB each), filled
+// by cp.async.bulk stages-1 iterations ahead; full[stage] completes on the bytes, empty[stage] on one arrival per warp.
+constexpr int kMaxStages6 = 4;
+constexpr uint32_t kBlock6 = kPassThreads * 16u;   // bytes of one array's block in a stage
+constexpr uint32_t kStage6 = 6u * kBlock6;
+__host__ __device__ inline size_t pass6_smem_bytes(int nb, int stages) {
+  return (size_t)stages * kStage6 + (size_t)(nb + 2) * 3 * sizeof(WakeCell) + 128 * sizeof(LogTabEntry) +
+         (size_t)(nb + 1) * 5 * sizeof(uint32_t) + 16;
 }
 
 // sin, cos of 2 pi t: q = rint(2 t), f = t - q/2 in [-1/4, 1/4] (exact), polynomials of mbt_math.cuh, sign (-1)^q
@@ -92,15 +99,23 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
   const Args &A = A6.L;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nb = A.nb;
-  WakeCell *sW = reinterpret_cast<WakeCell *>(smem_raw);       // [nb+2] longitudinal
+  const uint32_t nst = (uint32_t)A6.stages;
+  WakeCell *sW = reinterpret_cast<WakeCell *>(smem_raw + (size_t)nst * kStage6);  // [nb+2] longitudinal
   WakeCell *sX = sW + (nb + 2), *sY = sX + (nb + 2);           // [nb+2] each
   LogTabEntry *sL = reinterpret_cast<LogTabEntry *>(sY + (nb + 2));  // [128]
   uint32_t *sH = reinterpret_cast<uint32_t *>(sL + 128);       // [nb+1] counts, bin nb is a sink
   uint32_t *sLo = sH + (nb + 1), *sHi = sLo + 2 * (nb + 1);    // [2][nb+1] each: low / high words of the dipole sums
   __shared__ double s_red[kPassThreads / 32][6];
   __shared__ uint32_t s_nout[kPassThreads / 32];
+  __shared__ __align__(8) uint64_t s_bar[2 * kMaxStages6];  // full[], then empty[]
+  constexpr uint32_t NWARP = kPassThreads / 32;
 
-  const int tid = threadIdx.x, b = (int)blockIdx.y;
+  const int tid = threadIdx.x, b = (int)blockIdx.y, lane = tid & 31;
+  if (tid < (int)nst) {
+    mbar_init(smem_u32(&s_bar[tid]), 1u);
+    mbar_init(smem_u32(&s_bar[kMaxStages6 + tid]), NWARP);
+  }
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   const uint32_t n = A.ctrl->turn + 1u;
   const bool have_kick = A.ctrl->kick_pending != 0u;
   const uint32_t hi_nb = (uint32_t)__double2hiint(A.nb_d);
@@ -109,6 +124,23 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
   const double lo_old = A.lo_hist[b];
   const double lo_new = MAP ? A.lo_next[b] : lo_old;
   const FixScale fx = A6.fix[2 * b], fy = A6.fix[2 * b + 1];
+  const size_t base = (size_t)b * A.ld;
+  const uint32_t n_it = (p1 - p0 + kPassThreads - 1u) / kPassThreads;
+  const uint32_t stage0 = smem_u32(smem_raw), full0 = smem_u32(&s_bar[0]), empty0 = smem_u32(&s_bar[kMaxStages6]);
+  const double *gsrc[6] = {A.tau + base, A.delta + base, A6.x + base, A6.xp + base, A6.y + base, A6.yp + base};
+  auto issue = [&](uint32_t k) {  // fill the stage of chunk k once every warp has released it
+    const uint32_t stage = k % nst;
+    if (k >= nst) mbar_wait(empty0 + stage * 8u, ((k / nst) + 1u) & 1u);
+    const uint32_t pc = p0 + k * kPassThreads;
+    const uint32_t bytes = ((p1 - pc < (uint32_t)kPassThreads) ? p1 - pc : (uint32_t)kPassThreads) * 16u;
+    const uint32_t bar = full0 + stage * 8u, dst = stage0 + stage * kStage6;
+    mbar_expect_tx(bar, 6u * bytes);
+#pragma unroll
+    for (int a = 0; a < 6; ++a) bulk_g2s(dst + a * kBlock6, gsrc[a] + 2u * (size_t)pc, bytes, bar);
+  };
+  __syncthreads();  // barriers initialised
+  if (tid == 0)
+    for (uint32_t k = 0; k + 1u < nst && k < n_it; ++k) issue(k);
 
   if (MAP && RAD)
     for (int i = tid; i < 128; i += kPassThreads) sL[i] = A.logtab[i];
@@ -133,12 +165,32 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
 
   double st = 0.0, sd = 0.0, stt = 0.0, sdd = 0.0, sxx = 0.0, syy = 0.0;
   uint32_t nout = 0u;
-  const size_t base = (size_t)b * A.ld;
-  for (uint32_t p = p0 + (uint32_t)tid; p < p1; p += kPassThreads) {
+  // the producer role rotates over the warps: lane 0 of warp w issues the chunks c = w mod NWARP, c >= nst - 1
+  uint32_t next_issue = ~0u;
+  if (lane == 0) {
+    uint32_t c = (uint32_t)(tid >> 5);
+    while (c + 1u < nst) c += NWARP;
+    if (c < n_it) next_issue = c;
+  }
+  uint32_t stage = 0u, parity = 0u, p = p0 + (uint32_t)tid;
+  for (uint32_t k = 0; k < n_it; ++k, p += kPassThreads) {
+    const bool active = p < p1;  // the last chunk of a tile may be ragged
+    mbar_wait(full0 + stage * 8u, parity);
+    const uint32_t slot = stage0 + stage * kStage6 + (uint32_t)tid * 16u;
+    double2 t2 = make_double2(0.0, 0.0), d2 = t2, x2 = t2, xp2 = t2, y2 = t2, yp2 = t2;
+    if (active) {
+      t2 = lds_double2(slot); d2 = lds_double2(slot + kBlock6); x2 = lds_double2(slot + 2u * kBlock6);
+      xp2 = lds_double2(slot + 3u * kBlock6); y2 = lds_double2(slot + 4u * kBlock6); yp2 = lds_double2(slot + 5u * kBlock6);
+    }
+    __syncwarp();  // every lane of the warp has read the stage
+    if (lane == 0) mbar_arrive(empty0 + stage * 8u);
+    if (k + nst - 1u == next_issue) {
+      issue(next_issue);
+      next_issue = (next_issue + NWARP < n_it) ? next_issue + NWARP : ~0u;
+    }
+    if (++stage == nst) { stage = 0u; parity ^= 1u; }
+    if (!active) continue;
     const size_t o = base + 2u * (size_t)p;
-    const double2 t2 = *reinterpret_cast<const double2 *>(A.tau + o), d2 = *reinterpret_cast<const double2 *>(A.delta + o);
-    const double2 x2 = *reinterpret_cast<const double2 *>(A6.x + o), xp2 = *reinterpret_cast<const double2 *>(A6.xp + o);
-    const double2 y2 = *reinterpret_cast<const double2 *>(A6.y + o), yp2 = *reinterpret_cast<const double2 *>(A6.yp + o);
     double tau[2] = {t2.x, t2.y}, del[2] = {d2.x, d2.y};
     double x[2] = {x2.x, x2.y}, xp[2] = {xp2.x, xp2.y}, y[2] = {y2.x, y2.y}, yp[2] = {yp2.x, yp2.y};
     const bool live[2] = {2u * p < A.Np, 2u * p + 1u < A.Np};  // the slots from N_p up to ld are padding
