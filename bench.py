@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the fused per-turn hot path (macro-particle-turns/s) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c4] [--impl mbt|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c4] [--transverse] [--impl mbt|reference]
 
 A "step" is one tracked turn of the whole hot path over every macro-particle of the
 workload.  The workload at N = 1 is BASELINE.json configs[3] ("c4": 363 bunches x 1e5 macro-particles, the
@@ -11,6 +11,9 @@ store (581 MB) is larger than the 126 MB L2, so no L2 flush is needed between st
 N > 1: the path does not shard without a per-turn exchange that BASELINE north_star rules out ("no sharding, no
 collectives"), so every rank tracks an independent replica of the workload (a parameter-scan replica; DESIGN.md
 "Multi-GPU": replicas only) and `value` is the sum over ranks divided by the slowest rank's device time.
+
+--transverse adds the transverse planes to the workload: 6-D state, 96 B per particle-turn,
+the dominant kernel is then the fused 6-D pass k_pass6.  The default line is the longitudinal one BASELINE.json names.
 
 --impl reference times the CPU oracle (oracle/, test infrastructure) on this host's cores, on a bounded sample.
 """
@@ -31,6 +34,15 @@ if ROOT not in sys.path:
 
 METRIC = "macro-particle-turns/s"
 BYTES_PER_PARTICLE_TURN = 32.0  # tau, delta read once and written once per turn, fp64
+BYTES_PER_PARTICLE_TURN_6D = 96.0  # with the transverse planes: six fp64 coordinates
+
+
+def _config(args, **over):
+    from paper_1809_00391_b200 import workloads as W
+    cfg = W.config(args.config, **over)
+    if args.transverse:
+        cfg["transverse"] = W.transverse_planes()
+    return cfg
 
 
 def _peaks():
@@ -97,16 +109,16 @@ class ClockSampler:
         return out
 
 
-def _oracle_sample(cfg_name, budget_s, n_steps):
+def _oracle_sample(args, budget_s, n_steps):
     """Bounded sample of the workload for the CPU oracle: same fill pattern, wake sources, bins and history;
     N_p reduced so that n_steps turns take about budget_s seconds (the oracle runs ~1e7 particle-turns/s/core)."""
     from paper_1809_00391_b200 import workloads as W
-    full = W.config(cfg_name)
+    full = W.config(args.config)
     m = len(full["fill"]["buckets"])
     np_full = full["fill"]["n_per_bunch"]
-    per_step = budget_s / max(n_steps, 1) * 8.0e6
+    per_step = budget_s / max(n_steps, 1) * (2.0e6 if args.transverse else 8.0e6)
     np_s = int(max(500, min(np_full, per_step / m)))
-    return W.config(cfg_name, n_per_bunch=np_s), np_s, m
+    return _config(args, n_per_bunch=np_s), np_s, m
 
 
 def run_reference(args):
@@ -115,7 +127,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     from oracle import orc
-    cfg, np_s, m = _oracle_sample(args.config, 120.0, args.steps + args.warmup)
+    cfg, np_s, m = _oracle_sample(args, 120.0, args.steps + args.warmup)
     o = orc.Oracle(cfg, lr_mode=1)
     o.track(args.warmup)
     t0 = time.perf_counter()
@@ -127,7 +139,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": "particle-turns/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": _workload_name(args.config), "l2": "n/a (CPU)"},
+        "config": {"workload": _workload_name(args), "l2": "n/a (CPU)"},
         "cpu_baseline": {"value": val, "unit": "particle-turns/s", "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": "particle-turns/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -141,13 +153,17 @@ def W_np(name):
     return W.config(name)["fill"]["n_per_bunch"]
 
 
-def _workload_name(name):
+def _workload_name(args):
     from paper_1809_00391_b200 import workloads as W
+    name = args.config
     c = W.config(name)
     f, w = c["fill"], c["wake"]
-    return "%s: %d bunches x %d macro-particles, %d bins, %d resonators (%d long-range, %d-turn history), fp64 SoA" % (
+    s = "%s: %d bunches x %d macro-particles, %d bins, %d resonators (%d long-range, %d-turn history), fp64 SoA" % (
         name, len(f["buckets"]), f["n_per_bunch"], w["n_bins"], len(w["resonators"]),
         sum(1 for r in w["resonators"] if r["flags"] & 2), w["history_turns"])
+    if args.transverse:
+        s += " + transverse planes (6-D state, one transverse broadband resonator)"
+    return s
 
 
 def run_mbt(args):
@@ -165,8 +181,9 @@ def run_mbt(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     build.build()
-    cfg = W.config(args.config)
+    cfg = _config(args)
     n_part = W.n_particles(cfg)
+    bytes_pt = BYTES_PER_PARTICLE_TURN_6D if args.transverse else BYTES_PER_PARTICLE_TURN
     K, Wm = args.steps, args.warmup
 
     def barrier():
@@ -198,15 +215,16 @@ def run_mbt(args):
     pass_s, wake_s = trk.track_profiled(min(K, 2000))
     kp = min(K, 2000)
     peak, peak_src = _peaks()
-    achieved = BYTES_PER_PARTICLE_TURN * n_part / (pass_s / kp) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_pass<true>", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    achieved = bytes_pt * n_part / (pass_s / kp) / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_pass6<true>" if args.transverse else "k_pass<true>", "achieved": achieved,
+                "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": BYTES_PER_PARTICLE_TURN * n_part,
+                "algorithmic_bytes_per_launch": bytes_pt * n_part,
                 "pass_ms": pass_s / kp * 1e3, "wake_ms": wake_s / kp * 1e3,
                 "pass_share_of_step": pass_s / (pass_s + wake_s)}
     # DRAM bytes of one launch from the committed `ncu --set full` capture of this workload (profiles/traffic_<cfg>.txt)
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic_%s.txt" % args.config)) as f:
+        with open(os.path.join(ROOT, "profiles", "traffic_%s%s.txt" % (args.config, "t" if args.transverse else ""))) as f:
             for ln in f:
                 if ln.startswith("dram_bytes_per_launch"):
                     roofline["traffic"] = float(ln.split()[1])
@@ -226,8 +244,12 @@ def run_mbt(args):
                                     h_delta.numpy().reshape(len(cfg["fill"]["buckets"]), ld))
         out = np.empty((K, t2.M, 6))
         barrier()
+        tr0 = t2.transverse_particles() if args.transverse else None
+        barrier()
         t0 = time.perf_counter()
         t2.set_particles(tau0, delta0, 0)          # H2D of the whole state (pinned host memory)
+        if tr0 is not None:
+            t2.set_transverse(*tr0)                # ... and of the four transverse coordinates (pageable host memory)
         t2.track(K)
         out = t2.moment_log(1, K)                  # D2H of the per-turn statistics
         torch.cuda.synchronize()
@@ -237,7 +259,7 @@ def run_mbt(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t.item())
         e2e = {"value": world * n_part * K / dt, "unit": "particle-turns/s",
-               "h2d_bytes_per_step": 16.0 * n_part / K, "d2h_bytes_per_step": float(out.nbytes) / K,
+               "h2d_bytes_per_step": (48.0 if args.transverse else 16.0) * n_part / K, "d2h_bytes_per_step": float(out.nbytes) / K,
                "what": "mbt_set_particles (pinned host -> device) + mbt_track(K) + mbt_get_moment_log (device -> host), wall clock"}
         assert np.isfinite(out).all()
         t2.close()
@@ -262,11 +284,11 @@ def run_mbt(args):
             "metric": METRIC, "value": value, "unit": "particle-turns/s", "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": sec / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": _workload_name(args.config), "parallelism": "replicas x%d" % world,
-                       "l2": "particle store larger than L2, no flush needed" if 16 * n_part > 126e6 else
+            "config": {"workload": _workload_name(args), "parallelism": "replicas x%d" % world,
+                       "l2": "particle store larger than L2, no flush needed" if (bytes_pt / 2) * n_part > 126e6 else
                              "particle store fits L2 (latency-bound config, not an HBM roofline)"},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-            "algorithmic_GBps_whole_step": BYTES_PER_PARTICLE_TURN * value / world / 1e9,
+            "algorithmic_GBps_whole_step": bytes_pt * value / world / 1e9,
         }
         print(json.dumps(line))
     if world > 1:
@@ -280,6 +302,7 @@ def main():
     ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--config", default="c4")
+    ap.add_argument("--transverse", action="store_true")
     ap.add_argument("--impl", default="mbt", choices=["mbt", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
