@@ -29,6 +29,9 @@ struct Plane {
 // to a global table instead, so the sum is right for any input.  Integer sums do not depend on the order of
 // addition: S is reproducible bit for bit from run to run.  Rounding: 2^-kFixBits X_max per particle.
 constexpr int kFixBitsMax = 44;
+#ifndef MBT_LOCK6
+#define MBT_LOCK6 2  // particles whose angle polynomials run in lock step in k_pass6 (1 or 2; 2 measured 2 % faster at c4)
+#endif
 struct FixScale {
   double inv_lsb;    // 2^fix_bits / X_max (a power of two: the scaling is exact)
   double lsb;        // X_max / 2^fix_bits
@@ -74,6 +77,31 @@ __device__ __forceinline__ void sincos_turns(const MathTab &C, double t, double 
 __device__ __forceinline__ void betatron_map(const MathTab &C, const Plane &p, double &u, double &up, double d) {
   double sn, cs;
   sincos_turns(C, fma(p.t_xi, d, p.t_frac), sn, cs);
+  const double ub = fma(-p.eta, d, u), upb = fma(-p.etap, d, up);
+  const double un = fma(fma(p.alpha, sn, cs), ub, (p.beta * sn) * upb);
+  const double upn = fma(fma(-p.alpha, sn, cs), upb, -((p.gamma * sn) * ub));
+  u = fma(p.eta, d, un);
+  up = fma(p.etap, d, upn);
+}
+
+// the same in two halves around the polynomial evaluation, so that the caller can run the chains of several angles in
+// lock step (horner7_lockstep): head = phase reduction, tail = sin / cos and the matrix of Eq. (4)
+struct AngState {
+  double f, f2;
+  int q;
+};
+__device__ __forceinline__ AngState turns_head(double t) {
+  const double qm = fma(t, 2.0, MBT_MAGIC);
+  AngState S;
+  S.q = __double2loint(qm);
+  S.f = fma(qm - MBT_MAGIC, -0.5, t);
+  S.f2 = S.f * S.f;
+  return S;
+}
+__device__ __forceinline__ void betatron_tail(const MathTab &C, const Plane &p, const AngState &S, double ps, double pc, double &u,
+                                              double &up, double d) {
+  const double sn = flip_sign_if_odd(S.f * fma(S.f2, ps, C.two_pi), S.q);
+  const double cs = flip_sign_if_odd(fma(S.f2, pc, 1.0), S.q);
   const double ub = fma(-p.eta, d, u), upb = fma(-p.etap, d, up);
   const double un = fma(fma(p.alpha, sn, cs), ub, (p.beta * sn) * upb);
   const double upn = fma(fma(-p.alpha, sn, cs), upb, -((p.gamma * sn) * ub));
@@ -232,10 +260,11 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
         const bool hi_half = (p & 1u) != 0u;
         box_muller_fast(A.mt, sL, uniform32(A.mt, hi_half ? w2 : w0), uniform32(A.mt, hi_half ? w3 : w1), A.A_q, z[0], z[1]);
       }
+      double eps[2];
 #pragma unroll
       for (int i = 0; i < 2; ++i) {
         // S1; eps = the particle's RF gain of this turn (the epsilon of Eq. 5, T4)
-        double eps = 0.0;
+        eps[i] = 0.0;
         if (NCAV > 0) {
 #pragma unroll
           for (int c = 0; c < NCAV; ++c) {
@@ -243,7 +272,7 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
             double sv = sin_rf_fast(A.mt, yv);
             if (__builtin_expect(!(fabs(yv) < 65536.0), 0)) sv = sin_rf_slow(yv);
             del[i] = fma(A.cav_amp[c], sv, del[i]);
-            eps = fma(A.cav_amp[c], sv, eps);
+            eps[i] = fma(A.cav_amp[c], sv, eps[i]);
           }
         } else {
 #pragma unroll 1
@@ -252,29 +281,63 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
             double sv = sin_rf_fast(A.mt, yv);
             if (__builtin_expect(!(fabs(yv) < 65536.0), 0)) sv = sin_rf_slow(yv);
             del[i] = fma(A.cav_amp[c], sv, del[i]);
-            eps = fma(A.cav_amp[c], sv, eps);
+            eps[i] = fma(A.cav_amp[c], sv, eps[i]);
           }
         }
         del[i] -= A.loss;
         if (RAD) del[i] = fma(del[i], A.one_minus_DE, z[i]);  // S2
         tau[i] = fma(A.drift, del[i], tau[i]);                // S3
-        // Eqs. (3), (4) with the turn's delta (T1)
-        betatron_map(A.mt, A6.px, x[i], xp[i], del[i]);
-        betatron_map(A.mt, A6.py, y[i], yp[i], del[i]);
-        if (RAD) {
-          // Eq. (5) lines 2, 3 (T4, T5): one Philox block per particle, counter (i, b, n, tag 2) -> (r_x, r_x', r_y, r_y')
-          uint32_t w0, w1, w2, w3;
-          philox4x32_10(2u * p + (uint32_t)i, (uint32_t)b, n, 2u, A.keys, w0, w1, w2, w3);
-          double z0, z1, z2, z3;
-          box_muller_fast(A.mt, sL, uniform32(A.mt, w0), uniform32(A.mt, w1), 1.0, z0, z1);
-          box_muller_fast(A.mt, sL, uniform32(A.mt, w2), uniform32(A.mt, w3), 1.0, z2, z3);
-          const double num = 1.0 + del[i];
-          const double adia = div_near_one(num, num + eps);
-          x[i] = fma(A6.px.exc_u, z0, x[i]);
-          xp[i] = fma(xp[i], adia, A6.px.exc_up * z1);
-          y[i] = fma(A6.py.exc_u, z2, y[i]);
-          yp[i] = fma(yp[i], adia, A6.py.exc_up * z3);
+      }
+      // Eqs. (3), (4) with the turn's delta (T1) and Eq. (5) lines 2, 3 (T4, T5: one Philox block per particle, counter
+      // (i, b, n, tag 2) -> (r_x, r_x', r_y, r_y')).  The sin / cos polynomials of a particle's four angles (two
+      // betatron phases, two Box-Muller angles) are the same two polynomials: evaluated in lock step, LOCK particles
+      // at a time, so that 8 LOCK independent DFMA chains are in flight.
+      constexpr int LOCK = MBT_LOCK6;
+#pragma unroll
+      for (int i0 = 0; i0 < 2; i0 += LOCK) {
+        constexpr int NA = (RAD ? 4 : 2) * LOCK;
+        AngState ang[2 * LOCK];
+        BmState bm[2 * LOCK];
+        double f2[NA], ps[NA], pc[NA];
+        const double dummy[1] = {0.0};
+        double dummy_p[1];
+#pragma unroll
+        for (int l = 0; l < LOCK; ++l) {
+          const int i = i0 + l;
+          ang[2 * l] = turns_head(fma(A6.px.t_xi, del[i], A6.px.t_frac));
+          ang[2 * l + 1] = turns_head(fma(A6.py.t_xi, del[i], A6.py.t_frac));
+          f2[2 * l] = ang[2 * l].f2;
+          f2[2 * l + 1] = ang[2 * l + 1].f2;
+          if (RAD) {
+            uint32_t w0, w1, w2, w3;
+            philox4x32_10(2u * p + (uint32_t)i, (uint32_t)b, n, 2u, A.keys, w0, w1, w2, w3);
+            bm[2 * l] = box_muller_head(A.mt, sL, uniform32(A.mt, w0), uniform32(A.mt, w1), 1.0);
+            bm[2 * l + 1] = box_muller_head(A.mt, sL, uniform32(A.mt, w2), uniform32(A.mt, w3), 1.0);
+            f2[2 * LOCK + 2 * l] = bm[2 * l].f2;
+            f2[2 * LOCK + 2 * l + 1] = bm[2 * l + 1].f2;
+          }
         }
+        horner7_lockstep<0, NA>(A.mt, dummy, dummy_p, f2, ps, pc);
+#pragma unroll
+        for (int l = 0; l < LOCK; ++l) {
+          const int i = i0 + l;
+          betatron_tail(A.mt, A6.px, ang[2 * l], ps[2 * l], pc[2 * l], x[i], xp[i], del[i]);
+          betatron_tail(A.mt, A6.py, ang[2 * l + 1], ps[2 * l + 1], pc[2 * l + 1], y[i], yp[i], del[i]);
+          if (RAD) {
+            double z0, z1, z2, z3;
+            box_muller_tail(A.mt, bm[2 * l], ps[2 * LOCK + 2 * l], pc[2 * LOCK + 2 * l], z0, z1);
+            box_muller_tail(A.mt, bm[2 * l + 1], ps[2 * LOCK + 2 * l + 1], pc[2 * LOCK + 2 * l + 1], z2, z3);
+            const double num = 1.0 + del[i];
+            const double adia = div_near_one(num, num + eps[i]);
+            x[i] = fma(A6.px.exc_u, z0, x[i]);
+            xp[i] = fma(xp[i], adia, A6.px.exc_up * z1);
+            y[i] = fma(A6.py.exc_u, z2, y[i]);
+            yp[i] = fma(yp[i], adia, A6.py.exc_up * z3);
+          }
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < 2; ++i) {
         t[i] = __dmul_rn(__dsub_rn(tau[i], lo_new), A.invDelta);  // S4
         in[i] = live[i] && in_window(t[i], hi_nb);
       }
