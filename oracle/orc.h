@@ -59,7 +59,13 @@ typedef struct {
 typedef struct { double nu, alpha, beta_m, xi, eta_m, etap, sigma_u_m, sigma_up, D_exc, sigma0_u_m, sigma0_up; } orc_plane;
 /* transverse short-range wake: resonators with Rs in Ohm/m (flags ignored),
  * W_perp(t > 0) = (w_r^2 R / (Q wbar)) exp(-a t) sin(wbar t), W_perp(0) = 0 (T7); both planes use the same list */
-typedef struct { int32_t enable; orc_plane x, y; int32_t n_res; const orc_resonator *res; } orc_transverse;
+/* long-range resistive-wall kick on the transverse planes (P:l.117-119; readings W1..W5): after
+ * the wake kicks and the statistics of turn n, every particle of bunch b gets
+ *   du' = (1/E0) sum_{(b',n') in H_rw(b,n)} Q_b' ubar_{b',n'} A_u / sqrt((n-n') T0 + (s_b - s_b') T_rf),
+ * ubar the mean offset of ALL particles of bunch b' at the end of turn n', H_rw = the passages of the last rw_turns turns
+ * (all bunches) and the earlier bunches of this turn; A_u = rw_amp_x, rw_amp_y [V s^(1/2) / (C m)]; rw_turns = 0: off */
+typedef struct { int32_t enable; orc_plane x, y; int32_t n_res; const orc_resonator *res;
+                 double rw_amp_x, rw_amp_y; int32_t rw_turns; } orc_transverse;
 
 typedef struct {
   orc_ring ring; int32_t n_cav; const orc_cavity *cav; orc_radiation rad;
@@ -94,6 +100,11 @@ int orc_get_dipole(orc_handle *h, double *Sx, double *Sy);
 int orc_get_transverse_wake(orc_handle *h, double *Kx, double *Ky);
 int orc_moments_transverse(orc_handle *h, double *out);
 double orc_transverse_wake(double Rs_ohm_per_m, double fr_Hz, double Q, double t_s);
+/* resistive-wall kick of the last turn per bunch [V] (kx[M], ky[M]); source strengths Q_b ubar [C m] of the last
+ * rw_turns turns, oldest first: [rw_turns][M][2] (x, y) */
+int orc_get_rw_kick(orc_handle *h, double *kx, double *ky);
+int orc_get_rw_history(orc_handle *h, double *out);
+int orc_set_rw_history(orc_handle *h, const double *in);
 /* Eqs. (3), (4) for one particle of one plane (no excitation): u, u' in place */
 void orc_betatron_map(const orc_plane *pl, double *u, double *up, double delta);
 int64_t orc_turn(const orc_handle *h);

@@ -67,7 +67,8 @@ class Plane(C.Structure):
 
 
 class Transverse(C.Structure):
-    _fields_ = [("enable", C.c_int32), ("x", Plane), ("y", Plane), ("n_res", C.c_int32), ("res", C.POINTER(Resonator))]
+    _fields_ = [("enable", C.c_int32), ("x", Plane), ("y", Plane), ("n_res", C.c_int32), ("res", C.POINTER(Resonator)),
+                ("rw_amp_x", C.c_double), ("rw_amp_y", C.c_double), ("rw_turns", C.c_int32)]
 
 
 class Params(C.Structure):
@@ -107,6 +108,9 @@ def lib():
         L.orc_get_dipole.argtypes = [H, dp, dp]
         L.orc_get_transverse_wake.argtypes = [H, dp, dp]
         L.orc_moments_transverse.argtypes = [H, dp]
+        L.orc_get_rw_kick.argtypes = [H, dp, dp]
+        L.orc_get_rw_history.argtypes = [H, dp]
+        L.orc_set_rw_history.argtypes = [H, dp]
         L.orc_transverse_wake.argtypes = [C.c_double] * 4
         L.orc_transverse_wake.restype = C.c_double
         L.orc_betatron_map.argtypes = [C.POINTER(Plane), dp, dp, C.c_double]
@@ -222,11 +226,14 @@ class Oracle:
         p.lr_mode = int(lr_mode)
         tr = cfg.get("transverse")
         self.transverse = bool(tr)
+        self.K_rw = 0
         if tr:
             self._tres = (Resonator * max(len(tr["resonators"]), 1))(
                 *[Resonator(r["Rs_ohm"], r["fr_Hz"], r["Q"], r.get("flags", 1)) for r in tr["resonators"]])
             p.trans = Transverse(1, Plane(**{k: float(tr["x"][k]) for k in PLANE_FIELDS}),
-                                 Plane(**{k: float(tr["y"][k]) for k in PLANE_FIELDS}), len(tr["resonators"]), self._tres)
+                                 Plane(**{k: float(tr["y"][k]) for k in PLANE_FIELDS}), len(tr["resonators"]), self._tres,
+                                 float(tr.get("rw_amp_x", 0.0)), float(tr.get("rw_amp_y", 0.0)), int(tr.get("rw_turns", 0)))
+            self.K_rw = int(tr.get("rw_turns", 0))
         self._h = C.c_void_p()
         self._L = L
         self._ck(L.orc_create(C.byref(p), C.byref(self._h)))
@@ -321,6 +328,23 @@ class Oracle:
         kx, ky = np.empty((self.M, self.nb)), np.empty((self.M, self.nb))
         self._ck(self._L.orc_get_transverse_wake(self._h, _dp(kx), _dp(ky)))
         return kx, ky
+
+    def rw_kick(self):
+        """(kx[M], ky[M]): resistive-wall kick of the last turn [V]."""
+        kx, ky = np.zeros(self.M), np.zeros(self.M)
+        self._ck(self._L.orc_get_rw_kick(self._h, _dp(kx), _dp(ky)))
+        return kx, ky
+
+    def rw_history(self):
+        out = np.zeros((self.K_rw, self.M, 2))
+        if out.size:
+            self._ck(self._L.orc_get_rw_history(self._h, _dp(out)))
+        return out
+
+    def set_rw_history(self, a):
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        if a.size:
+            self._ck(self._L.orc_set_rw_history(self._h, _dp(a)))
 
     def moments_transverse(self):
         out = np.empty((self.M, 8))

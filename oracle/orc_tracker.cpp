@@ -201,6 +201,11 @@ struct orc_handle {
   std::vector<double> x, xp, y, yp;        // [M][Np]
   std::vector<double> Sx, Sy, Kx, Ky;      // [M][nb] dipole sums [m] and kick tables [V]
   std::vector<double> mom_tr;              // [M][8]
+  // long-range resistive wall (readings W1..W5)
+  int Krw = 0;
+  std::vector<double> ring_g;              // [(Krw+1)][M][2] source strengths Q_b ubar_{b,n'} [C m], slot n' % (Krw+1)
+  std::vector<double> rw_kick;             // [M][2] kick of the last turn [V]
+  double &g_at(int64_t n, int b, int a) { return ring_g[((size_t)(n % (Krw + 1)) * M + b) * 2 + a]; }
   // lr_mode 1 tables
   std::vector<cplx> g_step;  // [M-1][R] exp(lambda (s_{j+1}-s_j) T_rf)
   std::vector<cplx> g_hist;  // [K][R]   exp(lambda (k T0 - (s_{M-1}-s_0) T_rf)), k = 1..K
@@ -518,6 +523,34 @@ void one_turn(orc_handle *h) {
   }
   // 8: statistics
   compute_moments(h);
+  // 9: long-range resistive-wall kick on the transverse planes (P:l.117-119; readings W1..W5), "launched only when wake
+  // potential effects are calculated for all the bunches and the statistics have been updated": the sources are the
+  // bunch centroids of the statistics just taken, this turn's for the bunches ahead and the last Krw turns' for all;
+  // W_rw(t) = A / sqrt(t) (W2); every particle of the bunch gets the same kick, in the window or not (W4)
+  if (h->tr.enable && h->Krw > 0) {
+    for (int b = 0; b < M; ++b) {
+      h->g_at(n, b, 0) = h->charge[b] * h->mom_tr[(size_t)b * 8 + 0];
+      h->g_at(n, b, 1) = h->charge[b] * h->mom_tr[(size_t)b * 8 + 2];
+    }
+    const double amp[2] = {h->tr.rw_amp_x, h->tr.rw_amp_y};
+    for (int b = 0; b < M; ++b) {
+      double sum[2] = {0.0, 0.0};
+      for (int64_t np = std::max<int64_t>(1, n - h->Krw); np <= n; ++np)
+        for (int bp = 0; bp < M; ++bp) {
+          if (np == n && h->bucket[bp] >= h->bucket[b]) continue;          // this turn: only the bunches ahead (W5)
+          double dt = (double)dt_between(h, n - np, h->bucket[b] - h->bucket[bp]);
+          double wgt = 1.0 / std::sqrt(dt);
+          for (int a = 0; a < 2; ++a) sum[a] += h->g_at(np, bp, a) * wgt;
+        }
+      for (int a = 0; a < 2; ++a) h->rw_kick[(size_t)b * 2 + a] = amp[a] * sum[a];
+      const double kx = h->rw_kick[(size_t)b * 2] / h->ring.E0_eV, ky = h->rw_kick[(size_t)b * 2 + 1] / h->ring.E0_eV;
+      for (int64_t i = 0; i < Np; ++i) {
+        h->xp[(size_t)b * Np + i] += kx;
+        h->yp[(size_t)b * Np + i] += ky;
+      }
+    }
+    compute_moments(h);  // the observable moments describe the state after the kick
+  }
   h->turn = n;
   if (n - 1 < h->log_cap) std::memcpy(&h->log[(size_t)(n - 1) * M * 6], h->mom.data(), sizeof(double) * M * 6);
 }
@@ -692,6 +725,13 @@ int orc_create(const orc_params *p, orc_handle **out) {
       h->Sx.assign((size_t)h->M * h->nb, 0.0); h->Sy.assign((size_t)h->M * h->nb, 0.0);
       h->Kx.assign((size_t)h->M * h->nb, 0.0); h->Ky.assign((size_t)h->M * h->nb, 0.0);
       h->mom_tr.assign((size_t)h->M * 8, 0.0);
+      if (p->trans.rw_turns < 0 || p->trans.rw_turns > 100000 || !std::isfinite(p->trans.rw_amp_x) || !std::isfinite(p->trans.rw_amp_y)) {
+        delete h;
+        return fail(ORC_EINVAL, "resistive wall: need 0 <= rw_turns <= 100000, finite amplitudes");
+      }
+      h->Krw = p->trans.rw_turns;
+      h->ring_g.assign((size_t)(h->Krw + 1) * h->M * 2, 0.0);
+      h->rw_kick.assign((size_t)h->M * 2, 0.0);
     }
     h->log.assign((size_t)h->log_cap * h->M * 6, 0.0);
     if (h->R() > 0) {
@@ -810,6 +850,37 @@ int orc_get_transverse_wake(orc_handle *h, double *Kx, double *Ky) {
 int orc_moments_transverse(orc_handle *h, double *out) {
   if (!h || !h->tr.enable || !out) return fail(ORC_EINVAL, "transverse planes not enabled / null argument");
   std::memcpy(out, h->mom_tr.data(), sizeof(double) * h->mom_tr.size());
+  return 0;
+}
+
+int orc_get_rw_kick(orc_handle *h, double *kx, double *ky) {
+  if (!h || !h->tr.enable) return fail(ORC_EINVAL, "transverse planes not enabled");
+  for (int b = 0; b < h->M; ++b) {
+    if (kx) kx[b] = h->rw_kick[(size_t)b * 2];
+    if (ky) ky[b] = h->rw_kick[(size_t)b * 2 + 1];
+  }
+  return 0;
+}
+
+// oldest first: row k holds turn (turn - Krw + 1 + k); turns < 1 are zero
+int orc_get_rw_history(orc_handle *h, double *out) {
+  if (!h || !h->tr.enable || !out) return fail(ORC_EINVAL, "transverse planes not enabled / null argument");
+  for (int k = 0; k < h->Krw; ++k) {
+    int64_t np = h->turn - h->Krw + 1 + k;
+    for (int b = 0; b < h->M; ++b)
+      for (int a = 0; a < 2; ++a) out[((size_t)k * h->M + b) * 2 + a] = np >= 1 ? h->g_at(np, b, a) : 0.0;
+  }
+  return 0;
+}
+
+int orc_set_rw_history(orc_handle *h, const double *in) {
+  if (!h || !h->tr.enable || !in) return fail(ORC_EINVAL, "transverse planes not enabled / null argument");
+  for (int k = 0; k < h->Krw; ++k) {
+    int64_t np = h->turn - h->Krw + 1 + k;
+    if (np < 1) continue;
+    for (int b = 0; b < h->M; ++b)
+      for (int a = 0; a < 2; ++a) h->g_at(np, b, a) = in[((size_t)k * h->M + b) * 2 + a];
+  }
   return 0;
 }
 
