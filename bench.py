@@ -41,7 +41,7 @@ def _config(args, **over):
     from paper_1809_00391_b200 import workloads as W
     cfg = W.config(args.config, **over)
     if args.transverse:
-        cfg["transverse"] = W.transverse_planes()
+        cfg["transverse"] = W.transverse_planes(rw_amp_x=2.0e9, rw_amp_y=1.0e9, rw_turns=args.rw_turns)
     return cfg
 
 
@@ -163,6 +163,8 @@ def _workload_name(args):
         sum(1 for r in w["resonators"] if r["flags"] & 2), w["history_turns"])
     if args.transverse:
         s += " + transverse planes (6-D state, one transverse broadband resonator)"
+        if args.rw_turns:
+            s += " + long-range resistive-wall kick (%d-turn history)" % args.rw_turns
     return s
 
 
@@ -303,6 +305,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--config", default="c4")
     ap.add_argument("--transverse", action="store_true")
+    ap.add_argument("--rw-turns", type=int, default=0, help="with --transverse: resistive-wall history depth (0: off)")
     ap.add_argument("--impl", default="mbt", choices=["mbt", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

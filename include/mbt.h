@@ -98,7 +98,13 @@ typedef struct { double nu, alpha, beta_m, xi, eta_m, etap, sigma_u_m, sigma_up,
 /* transverse short-range wake of Eq. (6b): resonators with Rs in Ohm/m (flags ignored),
  * W_perp(t > 0) = (w_r^2 R / (Q wbar)) exp(-a t) sin(wbar t), W_perp(0) = 0 (T7); the same list for both planes.
  * enable = 0: longitudinal tracker only (none of the transverse entry points may then be called). */
-typedef struct { int32_t enable; mbt_plane x, y; int32_t n_res; const mbt_resonator *res; } mbt_transverse;
+/* Long-range resistive-wall kick on the transverse planes (P:l.117-119; DESIGN.md readings
+ * W1..W5): after the wake kicks of turn n every particle of bunch b gets
+ *   du' = (1/E0) sum_{(b',n')} Q_b' ubar_{b',n'} A_u / sqrt((n-n') T0 + (s_b - s_b') T_rf)
+ * over the passages of the last rw_turns turns (all bunches) and the bunches ahead in this turn, ubar = the mean offset of
+ * all particles of the bunch at the end of its turn; A_u = rw_amp_x, rw_amp_y [V s^(1/2) / (C m)]; rw_turns = 0: off. */
+typedef struct { int32_t enable; mbt_plane x, y; int32_t n_res; const mbt_resonator *res;
+                 double rw_amp_x, rw_amp_y; int32_t rw_turns; } mbt_transverse;
 
 typedef struct {
   mbt_ring ring;
@@ -158,13 +164,21 @@ int mbt_set_window(mbt_handle *h, const int32_t *s_hist, const int32_t *s_next);
 /* ---- transverse planes (HOST pointers; packed [M][N_p] for coordinates, [M][n_bins] for the bin tables) ----
  * The transverse steps of a turn run in kernels of their own after the fused longitudinal pass: betatron map,
  * excitation and dipole deposit (k_trans_map), dipole convolution (k_wake_tr), kick and moments (k_trans_kick); no
- * transverse kick is ever pending. */
+ * transverse kick is ever pending.
+ * (Superseded: the transverse steps are fused into the 6-D pass k_pass6; like the longitudinal kick, the transverse
+ * kicks of the last tracked turn stay pending inside the library and every getter applies them first.) */
 int mbt_get_transverse(mbt_handle *h, double *x, double *xp, double *y, double *yp);
 int mbt_set_transverse(mbt_handle *h, const double *x, const double *xp, const double *y, const double *yp);
 /* dipole sums S[b][k] = sum of u over the particles of bin k [m] and kick tables
  * K[b][j] = sum_{k<j} (Q_b/N_p) S[b][k] W_perp((j-k) Delta) [V] of the last tracked turn (NULL entries are skipped) */
 int mbt_get_dipole(mbt_handle *h, double *Sx, double *Sy);
 int mbt_get_transverse_wake(mbt_handle *h, double *Kx, double *Ky);
+/* resistive-wall kick of the last tracked turn per bunch [V] (kx[M], ky[M]; NULL entries are skipped); source strengths
+ * Q_b ubar [C m] of the last rw_turns turns, oldest first: [rw_turns][M][2] (x, y) -- get / set as the long-range
+ * history (set after mbt_set_particles, which fixes the turn the rows refer to) */
+int mbt_get_rw_kick(mbt_handle *h, double *kx, double *ky);
+int mbt_get_rw_history(mbt_handle *h, double *out);
+int mbt_set_rw_history(mbt_handle *h, const double *in);
 /* out[M][8]: mean x x' y y', rms x x' y y' (population), of the current state */
 int mbt_moments_transverse(mbt_handle *h, double *out);
 

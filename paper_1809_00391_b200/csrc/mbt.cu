@@ -128,6 +128,10 @@ struct mbt_handle {
   DevBuf<unsigned long long> Sfix;
   DevBuf<FixScale> fix;
   DevBuf<WakeCell> cellX, cellY;
+  int Krw = 0;                 // resistive-wall history depth (0: off)
+  RwArgs rwargs;
+  DevBuf<double> ring_g, rw, wrw;
+  DevBuf<int32_t> d_bucket;
   int wake_splits = 1;
   DevBuf<double> lo_hist, lo_next;
   DevBuf<cplx> shift_src, shift_wit;
@@ -183,9 +187,10 @@ void enqueue_pass(mbt_handle *h) {
 void enqueue_wakes(mbt_handle *h) {
   k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
   if (h->trans) k_wake_tr<<<h->M, 256, (size_t)h->nb * 5 * sizeof(double), h->stream>>>(h->twargs);
+  if (h->Krw > 0) k_rw<<<h->M, 256, 0, h->stream>>>(h->rwargs);
 }
-// launches per tracked turn: 2, or 3 with the transverse planes
-int launches_per_turn(const mbt_handle *h) { return h->trans ? 3 : 2; }
+// launches per tracked turn: 2; 3 with the transverse planes; 4 with their resistive-wall kick
+int launches_per_turn(const mbt_handle *h) { return h->trans ? (h->Krw > 0 ? 4 : 3) : 2; }
 
 int enqueue_turn(mbt_handle *h) {
   enqueue_pass(h);
@@ -250,6 +255,7 @@ void destroy(mbt_handle *h) {
   h->tx.release(); h->txp.release(); h->ty.release(); h->typ.release(); h->wt.release(); h->Sfix.release(); h->Sov.release();
   h->S_last.release(); h->Ktab.release(); h->acc2.release(); h->fix.release(); h->cellX.release(); h->cellY.release();
   h->mom_tr_acc.release(); h->mom_tr.release();
+  h->ring_g.release(); h->rw.release(); h->wrw.release(); h->d_bucket.release();
   h->s_hist.release(); h->s_next.release(); h->lo_hist.release(); h->lo_next.release();
   h->shift_src.release(); h->shift_wit.release();
   h->Esrc.release(); h->F.release(); h->g_step.release(); h->g_tail.release(); h->g_hist.release(); h->a_cur.release();
@@ -331,6 +337,8 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
           !(pl->sigma_u_m >= 0) || !(pl->sigma_up >= 0) || !(pl->sigma0_u_m >= 0) || !(pl->sigma0_up >= 0))
         return fail(MBT_EINVAL, "transverse plane: need beta > 0, D_exc >= 0, sigmas >= 0");
     if (tr.n_res < 0 || (tr.n_res > 0 && !tr.res)) return fail(MBT_EINVAL, "transverse resonator list");
+    if (tr.rw_turns < 0 || tr.rw_turns > 100000 || !std::isfinite(tr.rw_amp_x) || !std::isfinite(tr.rw_amp_y))
+      return fail(MBT_EINVAL, "resistive wall: need 0 <= rw_turns <= 100000, finite amplitudes");
     for (int r = 0; r < tr.n_res; ++r)
       if (!(tr.res[r].Q > 0.5) || !(tr.res[r].fr_Hz > 0) || !std::isfinite(tr.res[r].Rs_ohm))
         return fail(MBT_EINVAL, "transverse resonator: need Q > 1/2, fr > 0");
@@ -646,7 +654,22 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     }
     CUH(h->wt.upload(wt));
     CUH(h->tx.alloc(N)); CUH(h->txp.alloc(N)); CUH(h->ty.alloc(N)); CUH(h->typ.alloc(N));
-    CUH(h->Sfix.alloc((size_t)M * 2 * nb)); CUH(h->Sov.alloc((size_t)M * 2 * nb));
+    CUH(h->Sfix.alloc((size_t)M * 2 * (nb + 1))); CUH(h->Sov.alloc((size_t)M * 2 * (nb + 1)));
+    // long-range resistive wall (W1..W5): source ring, kick per bunch, weights (d T_rf)^-1/2 by bucket distance d
+    h->Krw = tr.rw_turns;
+    CUH(h->ring_g.alloc((size_t)(h->Krw + 1) * M * 2));
+    CUH(h->rw.alloc((size_t)M * 2));
+    {
+      std::vector<double> wr((size_t)(h->Krw + 1) * rg.h, 0.0);
+      for (size_t d = 1; d < wr.size(); ++d)
+        wr[d] = (double)(1.0L / sqrtl((ldbl)d * ((ldbl)rg.T0_s / (ldbl)rg.h)));
+      CUH(h->wrw.upload(wr));
+      CUH(h->d_bucket.upload(std::vector<int32_t>(fl.bucket, fl.bucket + M)));
+    }
+    RwArgs &Rw = h->rwargs;
+    memset(&Rw, 0, sizeof Rw);
+    Rw.M = M; Rw.Krw = h->Krw; Rw.h = rg.h; Rw.bucket = h->d_bucket.p; Rw.ring_g = h->ring_g.p; Rw.wrw = h->wrw.p;
+    Rw.amp[0] = tr.rw_amp_x; Rw.amp[1] = tr.rw_amp_y; Rw.rw = h->rw.p; Rw.ctrl = h->ctrl.p;
     CUH(h->S_last.alloc((size_t)M * 2 * nb)); CUH(h->Ktab.alloc((size_t)M * 2 * nb));
     CUH(h->cellX.alloc((size_t)M * (nb + 2))); CUH(h->cellY.alloc((size_t)M * (nb + 2)));
     CUH(h->fix.alloc((size_t)M * 2)); CUH(h->acc2.alloc((size_t)M * 2));
@@ -671,7 +694,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
       d.exc_up = q.sigma_up * std::sqrt(q.D_exc);
     }
     T.cellX = h->cellX.p; T.cellY = h->cellY.p;
-    T.Sfix = h->Sfix.p; T.Sov = h->Sov.p; T.fix = h->fix.p; T.acc2 = h->acc2.p;
+    T.Sfix = h->Sfix.p; T.Sov = h->Sov.p; T.fix = h->fix.p; T.acc2 = h->acc2.p; T.rw = h->rw.p;
     h->fn_map6 = select_map6(rad_on, wk.gather_order, p->n_cav);
     h->fn_flush6 = select_flush6(wk.gather_order);
     // three stages in flight if two CTAs then still fit an SM, else two
@@ -700,6 +723,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     Tw.qm = h->qm.p; Tw.wt = h->wt.p;
     Tw.Sfix = h->Sfix.p; Tw.Sov = h->Sov.p; Tw.fix = h->fix.p; Tw.acc2 = h->acc2.p;
     Tw.S_last = h->S_last.p; Tw.K = h->Ktab.p; Tw.cellX = h->cellX.p; Tw.cellY = h->cellY.p;
+    Tw.Krw = h->Krw; Tw.ring_g = h->ring_g.p; Tw.ctrl = h->ctrl.p;
     dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)M);
     k_init_tr<<<grid, 256, 0, h->stream>>>(h->tx.p, h->txp.p, h->ty.p, h->typ.p, h->ld, (uint32_t)h->Np, A.keys,
                                            tr.x.sigma0_u_m, tr.x.sigma0_up, tr.y.sigma0_u_m, tr.y.sigma0_up);
@@ -942,6 +966,49 @@ int mbt_get_transverse_wake(mbt_handle *h, double *Kx, double *Ky) {
   const size_t row = sizeof(double) * (size_t)h->nb;
   if (Kx) CU(cudaMemcpy2DAsync(Kx, row, h->Ktab.p, 2 * row, row, h->M, cudaMemcpyDeviceToHost, h->stream));
   if (Ky) CU(cudaMemcpy2DAsync(Ky, row, h->Ktab.p + h->nb, 2 * row, row, h->M, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_get_rw_kick(mbt_handle *h, double *kx, double *ky) {
+  if (!h || !h->trans) return fail(MBT_EINVAL, "transverse planes not enabled");
+  CU(cudaSetDevice(h->device));
+  std::vector<double> v((size_t)h->M * 2);
+  CU(cudaMemcpyAsync(v.data(), h->rw.p, sizeof(double) * v.size(), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  for (int b = 0; b < h->M; ++b) {
+    if (kx) kx[b] = v[(size_t)b * 2];
+    if (ky) ky[b] = v[(size_t)b * 2 + 1];
+  }
+  return 0;
+}
+
+// rows oldest first: row k = turn (turn - Krw + 1 + k), zero for turns < 1; ring slot of turn n' = n' % (Krw + 1)
+int mbt_get_rw_history(mbt_handle *h, double *out) {
+  if (!h || !h->trans || !out) return fail(MBT_EINVAL, "transverse planes not enabled / null argument");
+  CU(cudaSetDevice(h->device));
+  const size_t row = (size_t)h->M * 2;
+  std::vector<double> ring((size_t)(h->Krw + 1) * row);
+  CU(cudaMemcpyAsync(ring.data(), h->ring_g.p, sizeof(double) * ring.size(), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  for (int k = 0; k < h->Krw; ++k) {
+    const int64_t np = h->turn - h->Krw + 1 + k;
+    for (size_t i = 0; i < row; ++i) out[(size_t)k * row + i] = np >= 1 ? ring[(size_t)(np % (h->Krw + 1)) * row + i] : 0.0;
+  }
+  return 0;
+}
+
+int mbt_set_rw_history(mbt_handle *h, const double *in) {
+  if (!h || !h->trans || !in) return fail(MBT_EINVAL, "transverse planes not enabled / null argument");
+  CU(cudaSetDevice(h->device));
+  const size_t row = (size_t)h->M * 2;
+  std::vector<double> ring((size_t)(h->Krw + 1) * row, 0.0);
+  for (int k = 0; k < h->Krw; ++k) {
+    const int64_t np = h->turn - h->Krw + 1 + k;
+    if (np < 1) continue;
+    for (size_t i = 0; i < row; ++i) ring[(size_t)(np % (h->Krw + 1)) * row + i] = in[(size_t)k * row + i];
+  }
+  CU(cudaMemcpyAsync(h->ring_g.p, ring.data(), sizeof(double) * ring.size(), cudaMemcpyHostToDevice, h->stream));
   CU(cudaStreamSynchronize(h->stream));
   return 0;
 }

@@ -44,8 +44,10 @@ struct Args6 {
   double *x, *xp, *y, *yp;     // [M][ld]
   Plane px, py;
   const WakeCell *cellX, *cellY;  // [M][nb+2] gather cells of the kick tables K_x, K_y of the last turn (k_wake_tr)
-  unsigned long long *Sfix;    // [M][2][nb] dipole sums of the turn in flight, fixed point (two's complement)
-  double *Sov;                 // [M][2][nb] ... of the particles beyond X_max
+  unsigned long long *Sfix;    // [M][2][nb+1] dipole sums of the turn in flight, fixed point (two's complement);
+                               //              entry nb: the particles outside the window (for the bunch centroid)
+  double *Sov;                 // [M][2][nb+1] ... of the particles beyond X_max
+  const double *rw;            // [M][2] long-range resistive-wall kick of the last turn [V] (zeros without it)
   const FixScale *fix;         // [M][2]
   double *acc2;                // [M][2] sum u^2 of the mapped state (the next turn's scale)
   uint32_t tile_pairs;         // pairs per CTA
@@ -185,6 +187,8 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
       }
       cx = A6.cellX[(size_t)b * (nb + 2) + k];
       cy = A6.cellY[(size_t)b * (nb + 2) + k];
+      cx.mid += A6.rw[2 * b];      // the resistive-wall kick is the same for every particle of the bunch (W4),
+      cy.mid += A6.rw[2 * b + 1];  // cell nb+1 (outside the window) included
     }
     sW[k] = c; sX[k] = cx; sY[k] = cy;
   }
@@ -355,15 +359,16 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
         }
         const bool okx = ((uint32_t)__double2hiint(x[i]) & 0x7FFFFFFFu) < fx.xmax_hi;
         const bool oky = ((uint32_t)__double2hiint(y[i]) & 0x7FFFFFFFu) < fy.xmax_hi;
-        const double mx = fma(okx ? x[i] : 0.0, fx.inv_lsb, MBT_MAGIC), my = fma(oky ? y[i] : 0.0, fy.inv_lsb, MBT_MAGIC);
+        const double mx = fma(okx && live[i] ? x[i] : 0.0, fx.inv_lsb, MBT_MAGIC);  // a padding slot deposits zero
+        const double my = fma(oky && live[i] ? y[i] : 0.0, fy.inv_lsb, MBT_MAGIC);
         const uint32_t xl = (uint32_t)__double2loint(mx), xh = (uint32_t)(__double2hiint(mx) - 0x43380000);
         const uint32_t yl = (uint32_t)__double2loint(my), yh = (uint32_t)(__double2hiint(my) - 0x43380000);
         const uint32_t ox = atomicAdd(&sLo[j], xl), oy = atomicAdd(&sLo[(nb + 1) + j], yl);
         atomicAdd(&sHi[j], xh + ((ox + xl) < xl ? 1u : 0u));
         atomicAdd(&sHi[(nb + 1) + j], yh + ((oy + yl) < yl ? 1u : 0u));
-        if (__builtin_expect(in[i] && !(okx && oky), 0)) {  // beyond X_max: fp64, straight to the global table
-          if (!okx) atomicAdd(&A6.Sov[((size_t)b * 2) * nb + j], x[i]);
-          if (!oky) atomicAdd(&A6.Sov[((size_t)b * 2 + 1) * nb + j], y[i]);
+        if (__builtin_expect(live[i] && !(okx && oky), 0)) {  // beyond X_max: fp64, straight to the global table
+          if (!okx) atomicAdd(&A6.Sov[((size_t)b * 2) * (nb + 1) + j], x[i]);
+          if (!oky) atomicAdd(&A6.Sov[((size_t)b * 2 + 1) * (nb + 1) + j], y[i]);
         }
       }
     }
@@ -406,14 +411,14 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
     for (int w = 0; w < kPassThreads / 32; ++w) s += s_nout[w];
     if (s) atomicAdd(&A.nout_acc[b], (unsigned long long)s);
   }
-  for (int j = tid; j < nb; j += kPassThreads) {
+  for (int j = tid; j < nb + 1; j += kPassThreads) {
     const uint32_t c = sH[j];
-    if (c) atomicAdd(&A.hist[(size_t)b * nb + j], c);
+    if (c && j < nb) atomicAdd(&A.hist[(size_t)b * nb + j], c);
     if (MAP) {
 #pragma unroll
       for (int a = 0; a < 2; ++a) {
         const unsigned long long v = ((unsigned long long)sHi[a * (nb + 1) + j] << 32) | sLo[a * (nb + 1) + j];
-        if (v) atomicAdd(&A6.Sfix[((size_t)b * 2 + a) * nb + j], v);
+        if (v) atomicAdd(&A6.Sfix[((size_t)b * 2 + a) * (nb + 1) + j], v);
       }
     }
   }
@@ -424,8 +429,11 @@ struct TWakeArgs {
   uint32_t Np;
   const double *qm;     // [M]
   const double *wt;     // [nb] transverse table wt[k] = sum_r W_perp_r(k Delta), wt[0] = 0
-  unsigned long long *Sfix;   // [M][2][nb] in: sums of this turn; out: zero
-  double *Sov;                // [M][2][nb] likewise
+  unsigned long long *Sfix;   // [M][2][nb+1] in: sums of this turn (entry nb: outside the window); out: zero
+  double *Sov;                // [M][2][nb+1] likewise
+  int32_t Krw;                // resistive-wall history depth in turns (0: off)
+  double *ring_g;             // [Krw+1][M][2] source strengths Q_b ubar [C m], slot = turn % (Krw+1)
+  const Ctrl *ctrl;
   FixScale *fix;              // [M][2] in: the scale the sums were deposited with; out: the next turn's
   double *acc2;               // [M][2] in: sum u^2 of this turn's mapped state; out: zero
   double *S_last;             // [M][2][nb] observable copy of the sums [m]
@@ -458,16 +466,42 @@ __global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeAr
   double *sw = s_w, *sx = s_w + nb, *sy = s_w + 2 * nb, *kx = s_w + 3 * nb, *ky = s_w + 4 * nb;
   const double qm = A.qm[b];
   const FixScale fx = A.fix[2 * b], fy = A.fix[2 * b + 1];
-  const size_t ox = ((size_t)b * 2) * nb, oy = ox + nb;
-  for (int j = tid; j < nb; j += 256) {
-    const double vx = fma((double)(long long)A.Sfix[ox + j], fx.lsb, A.Sov[ox + j]);
-    const double vy = fma((double)(long long)A.Sfix[oy + j], fy.lsb, A.Sov[oy + j]);
-    A.Sfix[ox + j] = 0ull; A.Sfix[oy + j] = 0ull;
-    A.Sov[ox + j] = 0.0; A.Sov[oy + j] = 0.0;
-    A.S_last[ox + j] = vx; A.S_last[oy + j] = vy;
-    sx[j] = qm * vx;
-    sy[j] = qm * vy;
-    sw[j] = A.wt[j];
+  const size_t ox = ((size_t)b * 2) * nb, oy = ox + nb;                  // S_last, K: [M][2][nb]
+  const size_t fxo = ((size_t)b * 2) * (nb + 1), fyo = fxo + (nb + 1);   // Sfix, Sov: [M][2][nb+1]
+  long long tix = 0, tiy = 0;   // integer totals over the bins and the sink: exact, so the centroid is reproducible
+  double tox = 0.0, toy = 0.0;
+  for (int j = tid; j < nb + 1; j += 256) {
+    const long long ix = (long long)A.Sfix[fxo + j], iy = (long long)A.Sfix[fyo + j];
+    const double ovx = A.Sov[fxo + j], ovy = A.Sov[fyo + j];
+    A.Sfix[fxo + j] = 0ull; A.Sfix[fyo + j] = 0ull;
+    A.Sov[fxo + j] = 0.0; A.Sov[fyo + j] = 0.0;
+    tix += ix; tiy += iy; tox += ovx; toy += ovy;
+    if (j < nb) {
+      const double vx = fma((double)ix, fx.lsb, ovx), vy = fma((double)iy, fy.lsb, ovy);
+      A.S_last[ox + j] = vx; A.S_last[oy + j] = vy;
+      sx[j] = qm * vx;
+      sy[j] = qm * vy;
+      sw[j] = A.wt[j];
+    }
+  }
+  if (A.Krw > 0) {  // W3: source strength of this bunch and turn, Q_b ubar = (Q_b / N_p) sum of the offsets of all particles
+    __shared__ long long s_ti[8][2];
+    __shared__ double s_to[8][2];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      tix += __shfl_down_sync(0xffffffffu, tix, o); tiy += __shfl_down_sync(0xffffffffu, tiy, o);
+      tox += __shfl_down_sync(0xffffffffu, tox, o); toy += __shfl_down_sync(0xffffffffu, toy, o);
+    }
+    if ((tid & 31) == 0) { s_ti[tid >> 5][0] = tix; s_ti[tid >> 5][1] = tiy; s_to[tid >> 5][0] = tox; s_to[tid >> 5][1] = toy; }
+    __syncthreads();
+    if (tid < 2) {
+      long long ti = 0;
+      double to = 0.0;
+      for (int w = 0; w < 8; ++w) { ti += s_ti[w][tid]; to += s_to[w][tid]; }
+      const double total = fma((double)ti, tid == 0 ? fx.lsb : fy.lsb, to);
+      const uint32_t n = A.ctrl->turn;  // k_wake has closed the turn
+      A.ring_g[((size_t)(n % (uint32_t)(A.Krw + 1)) * A.M + b) * 2 + tid] = qm * total;
+    }
   }
   __syncthreads();
   if (tid < 2) {
@@ -499,6 +533,48 @@ __global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeAr
     }
     A.cellX[(size_t)b * (nb + 2) + k] = cx;
     A.cellY[(size_t)b * (nb + 2) + k] = cy;
+  }
+}
+
+// Long-range resistive-wall kick (readings W1..W5): one CTA per bunch b sums the sources of the last Krw turns (all
+// bunches) and of this turn's bunches ahead, weight wrw[d] = (d T_rf)^-1/2 at the bucket distance
+// d = (n - n') h + (s_b - s_b'); fixed summation order (reproducible).  Runs after k_wake_tr of the same turn.
+struct RwArgs {
+  int32_t M, Krw, h;
+  const int32_t *bucket;  // [M]
+  const double *ring_g;   // [Krw+1][M][2]
+  const double *wrw;      // [(Krw+1) h] weight at bucket distance d (entry 0 unused)
+  double amp[2];
+  double *rw;             // [M][2] out [V]
+  const Ctrl *ctrl;
+};
+__global__ void __launch_bounds__(256) k_rw(const __grid_constant__ RwArgs A) {
+  __shared__ double s_red[8][2];
+  const int b = blockIdx.x, tid = threadIdx.x;
+  const uint32_t n = A.ctrl->turn;
+  const int sb = A.bucket[b];
+  double sx = 0.0, sy = 0.0;
+  for (int idx = tid; idx < (A.Krw + 1) * A.M; idx += 256) {
+    const int k = idx / A.M, bp = idx - k * A.M;  // source: turn n - k, bunch bp
+    if ((uint32_t)k >= n) continue;                 // nothing before turn 1
+    const int d = k * A.h + (sb - A.bucket[bp]);
+    if (d <= 0) continue;                           // this turn: only the bunches ahead
+    const double w = A.wrw[d];
+    const double *g = A.ring_g + ((size_t)((n - (uint32_t)k) % (uint32_t)(A.Krw + 1)) * A.M + bp) * 2;
+    sx = fma(g[0], w, sx);
+    sy = fma(g[1], w, sy);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    sx += __shfl_down_sync(0xffffffffu, sx, o);
+    sy += __shfl_down_sync(0xffffffffu, sy, o);
+  }
+  if ((tid & 31) == 0) { s_red[tid >> 5][0] = sx; s_red[tid >> 5][1] = sy; }
+  __syncthreads();
+  if (tid < 2) {
+    double t = 0.0;
+    for (int w = 0; w < 8; ++w) t += s_red[w][tid];
+    A.rw[2 * b + tid] = A.amp[tid] * t;
   }
 }
 

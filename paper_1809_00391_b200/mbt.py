@@ -20,6 +20,7 @@ SYMBOLS = [
     "mbt_get_histogram", "mbt_get_wake", "mbt_get_moment_log", "mbt_get_lr_history", "mbt_set_lr_history", "mbt_get_window", "mbt_set_window",
     "mbt_turn", "mbt_phi_s", "mbt_particle_stride", "mbt_device_pointers", "mbt_launch_count",
     "mbt_get_transverse", "mbt_set_transverse", "mbt_get_dipole", "mbt_get_transverse_wake", "mbt_moments_transverse",
+    "mbt_get_rw_kick", "mbt_get_rw_history", "mbt_set_rw_history",
     "mbt_last_track_seconds", "mbt_track_profiled", "mbt_philox_selftest", "mbt_normal_selftest", "mbt_last_error", "mbt_version",
 ]
 
@@ -61,7 +62,8 @@ class Plane(C.Structure):
 
 
 class Transverse(C.Structure):
-    _fields_ = [("enable", C.c_int32), ("x", Plane), ("y", Plane), ("n_res", C.c_int32), ("res", C.POINTER(Resonator))]
+    _fields_ = [("enable", C.c_int32), ("x", Plane), ("y", Plane), ("n_res", C.c_int32), ("res", C.POINTER(Resonator)),
+                ("rw_amp_x", C.c_double), ("rw_amp_y", C.c_double), ("rw_turns", C.c_int32)]
 
 
 class Params(C.Structure):
@@ -119,6 +121,9 @@ def lib():
         L.mbt_get_dipole.argtypes = [H, dp, dp]
         L.mbt_get_transverse_wake.argtypes = [H, dp, dp]
         L.mbt_moments_transverse.argtypes = [H, dp]
+        L.mbt_get_rw_kick.argtypes = [H, dp, dp]
+        L.mbt_get_rw_history.argtypes = [H, dp]
+        L.mbt_set_rw_history.argtypes = [H, dp]
         L.mbt_philox_selftest.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.mbt_normal_selftest.argtypes = [C.c_uint64, C.c_int64, C.POINTER(C.c_uint32), dp]
         L.mbt_last_error.restype = C.c_char_p
@@ -187,7 +192,8 @@ def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None
         tres = (Resonator * max(len(tr["resonators"]), 1))(
             *[Resonator(r["Rs_ohm"], r["fr_Hz"], r["Q"], r.get("flags", 1)) for r in tr["resonators"]])
         p.trans = Transverse(1, Plane(**{k: float(tr["x"][k]) for k in PLANE_FIELDS}),
-                             Plane(**{k: float(tr["y"][k]) for k in PLANE_FIELDS}), len(tr["resonators"]), tres)
+                             Plane(**{k: float(tr["y"][k]) for k in PLANE_FIELDS}), len(tr["resonators"]), tres,
+                             float(tr.get("rw_amp_x", 0.0)), float(tr.get("rw_amp_y", 0.0)), int(tr.get("rw_turns", 0)))
     return p, [bucket, charge, cav, res, tbl, tres]
 
 
@@ -203,6 +209,7 @@ class Tracker:
         self.nb = int(w["n_bins"])
         self.R_lr = sum(1 for r in w["resonators"] if r["flags"] & 2)
         self.K = int(w["history_turns"]) if self.R_lr else 0
+        self.K_rw = int((cfg.get("transverse") or {}).get("rw_turns", 0))
         p, self._keep = make_params(cfg, log_capacity_turns, d_tau, d_delta, stream, device)
         self._h = C.c_void_p()
         self._L = L
@@ -336,6 +343,23 @@ class Tracker:
         kx, ky = np.empty((self.M, self.nb)), np.empty((self.M, self.nb))
         _ck(self._L.mbt_get_transverse_wake(self._h, _dp(kx), _dp(ky)))
         return kx, ky
+
+    def rw_kick(self):
+        """(kx[M], ky[M]): resistive-wall kick of the last tracked turn [V]."""
+        kx, ky = np.zeros(self.M), np.zeros(self.M)
+        _ck(self._L.mbt_get_rw_kick(self._h, _dp(kx), _dp(ky)))
+        return kx, ky
+
+    def rw_history(self):
+        out = np.zeros((self.K_rw, self.M, 2))
+        if out.size:
+            _ck(self._L.mbt_get_rw_history(self._h, _dp(out)))
+        return out
+
+    def set_rw_history(self, a):
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        if a.size:
+            _ck(self._L.mbt_set_rw_history(self._h, _dp(a)))
 
     def moments_transverse(self):
         out = np.empty((self.M, 8))

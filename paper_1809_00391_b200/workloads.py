@@ -167,12 +167,13 @@ def tiny(m=5, n_per_bunch=37, n_bins=8, k_hist=3, seed=11, buckets=None, n_lr=2,
 
 def transverse_planes(nu_x=18.2, nu_y=5.3, beta_x=8.0, beta_y=4.0, alpha_x=0.0, alpha_y=0.0, xi_x=1.0, xi_y=1.0,
                       eta_x=0.1, etap_x=0.0, emit_x=3.0e-10, emit_y=3.0e-12, u0_over_e0=2.5e-4, rs_ohm_per_m=1.0e6,
-                      fr_hz=5.0e9, q=1.0):
+                      fr_hz=5.0e9, q=1.0, rw_amp_x=0.0, rw_amp_y=0.0, rw_turns=0):
     """Synthetic transverse-plane parameters (inputs only) for cfg["transverse"].
     sigma_u = sqrt(emit beta), sigma_up = sqrt(emit gamma); D_exc = (U0/E0) / (beta gamma), the value for which
     the excitation of Eq. (5) balances its adiabatic damping at the emittance `emit` (reading T4); the
     initial distribution is the equilibrium one (uncorrelated, alpha = 0 by default); one broadband transverse
-    resonator for both planes."""
+    resonator for both planes.  rw_*: long-range resistive-wall kick (readings W1..W5), W_rw(t) = rw_amp / sqrt(t)
+    [V/(C m)] with a synthetic amplitude, history of rw_turns turns (0: off)."""
     def plane(nu, a, b, xi, eta, etap, emit):
         g = (1.0 + a * a) / b
         return dict(nu=nu, alpha=a, beta_m=b, xi=xi, eta_m=eta, etap=etap, sigma_u_m=math.sqrt(emit * b),
@@ -180,7 +181,8 @@ def transverse_planes(nu_x=18.2, nu_y=5.3, beta_x=8.0, beta_y=4.0, alpha_x=0.0, 
                     sigma0_up=math.sqrt(emit * g))
     return dict(x=plane(nu_x, alpha_x, beta_x, xi_x, eta_x, etap_x, emit_x),
                 y=plane(nu_y, alpha_y, beta_y, xi_y, 0.0, 0.0, emit_y),
-                resonators=[dict(Rs_ohm=rs_ohm_per_m, fr_Hz=fr_hz, Q=q, flags=FLAG_SR)])
+                resonators=[dict(Rs_ohm=rs_ohm_per_m, fr_Hz=fr_hz, Q=q, flags=FLAG_SR)],
+                rw_amp_x=float(rw_amp_x), rw_amp_y=float(rw_amp_y), rw_turns=int(rw_turns))
 
 
 def sampled_wake_table(n_bins, delta_s, r_ohm=0.0, l_henry=0.0, rw_amp=0.0):

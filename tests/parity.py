@@ -64,9 +64,11 @@ def resume_on_gpu(o, trk, cfg=None):
     return tau, delta
 
 
-def assert_single_turn_parity(o, trk, cfg, turns=1, tol_particle=TOL_PARTICLE, tol_wake=TOL_WAKE):
+def assert_single_turn_parity(o, trk, cfg, turns=1, tol_particle=TOL_PARTICLE, tol_wake=TOL_WAKE, after_resume=None):
     """Both sides advance `turns` turns from the oracle's current state; everything observable is compared."""
     resume_on_gpu(o, trk, cfg)
+    if after_resume is not None:
+        after_resume(trk)
     o.track(turns)
     trk.track(turns)
     tau_c, delta_c = o.particles()

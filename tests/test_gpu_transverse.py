@@ -33,7 +33,17 @@ def assert_transverse_turn_parity(o, t, cfg, turns=1, tol=TOL_PARTICLE):
     """Upload the oracle's 6-D state, advance both sides, compare the transverse observables; the longitudinal ones
     go through assert_single_turn_parity (which does the tracking)."""
     t.set_transverse(*o.transverse_particles())
-    r = assert_single_turn_parity(o, t, cfg, turns=turns)
+    hist_rw = o.rw_history()
+
+    def more(trk):                               # after mbt_set_particles has fixed the turn the rows refer to
+        trk.set_rw_history(hist_rw)
+    r = assert_single_turn_parity(o, t, cfg, turns=turns, after_resume=more)
+    if o.K_rw:
+        for nm, g, c in zip(("rw_x", "rw_y"), t.rw_kick(), o.rw_kick()):
+            scale = np.abs(c).max()
+            r["e_" + nm] = float(np.abs(g - c).max() / scale) if scale > 0 else float(np.abs(g).max())
+            assert r["e_" + nm] <= TOL_WAKE, "%s differs by %.3e" % (nm, r["e_" + nm])
+        assert np.allclose(t.rw_history(), o.rw_history(), rtol=1e-10, atol=1e-12 * np.abs(o.rw_history()).max())
     names = ("x", "xp", "y", "yp")
     for nm, g, c in zip(names, t.transverse_particles(), o.transverse_particles()):
         e = particle_errors(g, c)
@@ -94,6 +104,63 @@ def test_transverse_single_turn_parity(mbt, orc, name):
         for _ in range(3):
             r = assert_transverse_turn_parity(o, t, cfg)
         print(name, r)
+
+
+RW_VARIANTS = {
+    "five_bunches": dict(m=5, n_per_bunch=513, n_bins=16, rw=dict(rw_turns=3)),
+    "one_bunch_deep": dict(m=1, n_per_bunch=300, n_bins=16, rw=dict(rw_turns=40)),
+    "no_radiation_ngp": dict(m=4, n_per_bunch=257, n_bins=16, radiation=0, gather=0, rw=dict(rw_turns=2)),
+    "x_only": dict(m=3, n_per_bunch=999, n_bins=32, rw=dict(rw_turns=5, rw_amp_y=0.0)),
+    "ragged_tiles": dict(m=2, n_per_bunch=8193 + 7, n_bins=64, rw=dict(rw_turns=1)),
+}
+
+
+@pytest.mark.parametrize("name", sorted(RW_VARIANTS))
+def test_resistive_wall_single_turn_parity(mbt, orc, name):
+    """Long-range resistive-wall kick (readings W1..W5): the kick per bunch, the source history and, through x' and y',
+    its application to every particle; bunches displaced so that the centroids are not noise, a few particles parked
+    outside the bin window (they are kicked too, W4)."""
+    kw = dict(RW_VARIANTS[name])
+    rw = dict(rw_amp_x=2.0e9, rw_amp_y=-0.7e9)
+    rw.update(kw.pop("rw"))
+    cfg = _cfg(**kw)
+    cfg["transverse"].update(rw)
+    o = orc.Oracle(cfg)
+    m, n_p = len(cfg["fill"]["buckets"]), cfg["fill"]["n_per_bunch"]
+    tau, delta = o.particles()
+    tau = tau.copy()
+    tau[:, : min(3, n_p // 4)] = 90e-12
+    o.set_particles(tau, delta, 0)
+    x, xp, y, yp = o.transverse_particles()
+    off = (1.0e-3 * (1 + np.arange(m)) * (-1.0) ** np.arange(m))[:, None]
+    o.set_transverse(x + off, xp, y - 0.3 * off, yp)
+    o.track(3)
+    with mbt.Tracker(cfg) as t:
+        for _ in range(4):
+            r = assert_transverse_turn_parity(o, t, cfg)
+        assert np.abs(t.rw_kick()[0]).max() > 0
+        print(name, r)
+
+
+def test_resistive_wall_on_the_c4_fill_and_without_resync(mbt, orc):
+    """363 bunches, 20-turn resistive-wall history (7260 sources per bunch and turn), then eight turns on its own."""
+    cfg = W.config("c4", n_per_bunch=256)
+    cfg["transverse"] = W.transverse_planes()
+    cfg["transverse"].update(rw_amp_x=2.0e9, rw_amp_y=1.0e9, rw_turns=20)
+    o = orc.Oracle(cfg, lr_mode=0)
+    x, xp, y, yp = o.transverse_particles()
+    off = 1.0e-3 * np.sin(2 * np.pi * 5 * np.arange(363) / 363)[:, None]
+    o.set_transverse(x + off, xp, y + 0.5 * off, yp)
+    o.track(2)
+    with mbt.Tracker(cfg) as t:
+        r = assert_transverse_turn_parity(o, t, cfg)
+        print(r)
+        o.track(8)
+        t.track(8)
+        for g, c in zip(t.transverse_particles(), o.transverse_particles()):
+            assert particle_errors(g, c) <= 1e-10
+        for g, c in zip(t.rw_kick(), o.rw_kick()):
+            assert np.abs(g - c).max() <= 1e-9 * np.abs(c).max()
 
 
 def test_transverse_with_bunch_following_window(mbt, orc):
