@@ -102,6 +102,10 @@ int orc_moments_transverse(orc_handle *h, double *out);
 double orc_transverse_wake(double Rs_ohm_per_m, double fr_Hz, double Q, double t_s);
 /* resistive-wall kick of the last turn per bunch [V] (kx[M], ky[M]); source strengths Q_b ubar [C m] of the last
  * rw_turns turns, oldest first: [rw_turns][M][2] (x, y) */
+/* per-turn log of the transverse statistics (P:l.123: "mean values and the RMS values ... of each bunch", turn by turn):
+ * out[n][M][4] = mean x, mean y, rms x, rms y of the state at the end of turns first_turn .. first_turn+n-1 (the kicks
+ * act on u' only, so these are the offsets after the turn's map and excitation); capacity = log_capacity_turns */
+int orc_get_transverse_log(orc_handle *h, int64_t first_turn, int64_t n, double *out);
 int orc_get_rw_kick(orc_handle *h, double *kx, double *ky);
 int orc_get_rw_history(orc_handle *h, double *out);
 int orc_set_rw_history(orc_handle *h, const double *in);

@@ -108,6 +108,7 @@ def lib():
         L.orc_get_dipole.argtypes = [H, dp, dp]
         L.orc_get_transverse_wake.argtypes = [H, dp, dp]
         L.orc_moments_transverse.argtypes = [H, dp]
+        L.orc_get_transverse_log.argtypes = [H, C.c_int64, C.c_int64, dp]
         L.orc_get_rw_kick.argtypes = [H, dp, dp]
         L.orc_get_rw_history.argtypes = [H, dp]
         L.orc_set_rw_history.argtypes = [H, dp]
@@ -328,6 +329,12 @@ class Oracle:
         kx, ky = np.empty((self.M, self.nb)), np.empty((self.M, self.nb))
         self._ck(self._L.orc_get_transverse_wake(self._h, _dp(kx), _dp(ky)))
         return kx, ky
+
+    def transverse_log(self, first_turn, n):
+        """[n][M][4]: mean x, mean y, rms x, rms y at the end of each turn."""
+        out = np.empty((n, self.M, 4))
+        self._ck(self._L.orc_get_transverse_log(self._h, int(first_turn), int(n), _dp(out)))
+        return out
 
     def rw_kick(self):
         """(kx[M], ky[M]): resistive-wall kick of the last turn [V]."""

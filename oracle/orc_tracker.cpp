@@ -201,6 +201,7 @@ struct orc_handle {
   std::vector<double> x, xp, y, yp;        // [M][Np]
   std::vector<double> Sx, Sy, Kx, Ky;      // [M][nb] dipole sums [m] and kick tables [V]
   std::vector<double> mom_tr;              // [M][8]
+  std::vector<double> log_tr;              // [log_cap][M][4] mean x, mean y, rms x, rms y per turn
   // long-range resistive wall (readings W1..W5)
   int Krw = 0;
   std::vector<double> ring_g;              // [(Krw+1)][M][2] source strengths Q_b ubar_{b,n'} [C m], slot n' % (Krw+1)
@@ -553,6 +554,10 @@ void one_turn(orc_handle *h) {
   }
   h->turn = n;
   if (n - 1 < h->log_cap) std::memcpy(&h->log[(size_t)(n - 1) * M * 6], h->mom.data(), sizeof(double) * M * 6);
+  if (h->tr.enable && n - 1 < h->log_cap)
+    for (int b = 0; b < M; ++b)
+      for (int a = 0; a < 4; ++a)   // mom_tr: mean x x' y y', rms x x' y y'  ->  mean x, mean y, rms x, rms y
+        h->log_tr[((size_t)(n - 1) * M + b) * 4 + a] = h->mom_tr[(size_t)b * 8 + (a < 2 ? 2 * a : 4 + 2 * (a - 2))];
 }
 
 }  // namespace
@@ -734,6 +739,7 @@ int orc_create(const orc_params *p, orc_handle **out) {
       h->rw_kick.assign((size_t)h->M * 2, 0.0);
     }
     h->log.assign((size_t)h->log_cap * h->M * 6, 0.0);
+    if (h->tr.enable) h->log_tr.assign((size_t)h->log_cap * h->M * 4, 0.0);
     if (h->R() > 0) {
       int R = h->R(), M = h->M, K = h->K;
       h->g_step.assign((size_t)M * R, cplx(0, 0));
@@ -850,6 +856,13 @@ int orc_get_transverse_wake(orc_handle *h, double *Kx, double *Ky) {
 int orc_moments_transverse(orc_handle *h, double *out) {
   if (!h || !h->tr.enable || !out) return fail(ORC_EINVAL, "transverse planes not enabled / null argument");
   std::memcpy(out, h->mom_tr.data(), sizeof(double) * h->mom_tr.size());
+  return 0;
+}
+
+int orc_get_transverse_log(orc_handle *h, int64_t first_turn, int64_t n, double *out) {
+  if (!h || !h->tr.enable || !out || first_turn < 1 || n < 0) return fail(ORC_EINVAL, "bad argument");
+  if (first_turn - 1 + n > h->log_cap || first_turn - 1 + n > h->turn) return fail(ORC_ESTATE, "turns not in the log");
+  std::memcpy(out, &h->log_tr[(size_t)(first_turn - 1) * h->M * 4], sizeof(double) * (size_t)n * h->M * 4);
   return 0;
 }
 

@@ -130,7 +130,7 @@ struct mbt_handle {
   DevBuf<WakeCell> cellX, cellY;
   int Krw = 0;                 // resistive-wall history depth (0: off)
   RwArgs rwargs;
-  DevBuf<double> ring_g, rw, wrw;
+  DevBuf<double> ring_g, rw, wrw, log_tr;
   DevBuf<int32_t> d_bucket;
   int wake_splits = 1;
   DevBuf<double> lo_hist, lo_next;
@@ -255,7 +255,7 @@ void destroy(mbt_handle *h) {
   h->tx.release(); h->txp.release(); h->ty.release(); h->typ.release(); h->wt.release(); h->Sfix.release(); h->Sov.release();
   h->S_last.release(); h->Ktab.release(); h->acc2.release(); h->fix.release(); h->cellX.release(); h->cellY.release();
   h->mom_tr_acc.release(); h->mom_tr.release();
-  h->ring_g.release(); h->rw.release(); h->wrw.release(); h->d_bucket.release();
+  h->ring_g.release(); h->rw.release(); h->wrw.release(); h->d_bucket.release(); h->log_tr.release();
   h->s_hist.release(); h->s_next.release(); h->lo_hist.release(); h->lo_next.release();
   h->shift_src.release(); h->shift_wit.release();
   h->Esrc.release(); h->F.release(); h->g_step.release(); h->g_tail.release(); h->g_hist.release(); h->a_cur.release();
@@ -724,6 +724,9 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     Tw.Sfix = h->Sfix.p; Tw.Sov = h->Sov.p; Tw.fix = h->fix.p; Tw.acc2 = h->acc2.p;
     Tw.S_last = h->S_last.p; Tw.K = h->Ktab.p; Tw.cellX = h->cellX.p; Tw.cellY = h->cellY.p;
     Tw.Krw = h->Krw; Tw.ring_g = h->ring_g.p; Tw.ctrl = h->ctrl.p;
+    if (h->log_cap > 0) CUH(h->log_tr.alloc((size_t)h->log_cap * M * 4));
+    Tw.log_tr = h->log_cap > 0 ? h->log_tr.p : nullptr;
+    Tw.log_cap = h->log_cap;
     dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)M);
     k_init_tr<<<grid, 256, 0, h->stream>>>(h->tx.p, h->txp.p, h->ty.p, h->typ.p, h->ld, (uint32_t)h->Np, A.keys,
                                            tr.x.sigma0_u_m, tr.x.sigma0_up, tr.y.sigma0_u_m, tr.y.sigma0_up);
@@ -966,6 +969,17 @@ int mbt_get_transverse_wake(mbt_handle *h, double *Kx, double *Ky) {
   const size_t row = sizeof(double) * (size_t)h->nb;
   if (Kx) CU(cudaMemcpy2DAsync(Kx, row, h->Ktab.p, 2 * row, row, h->M, cudaMemcpyDeviceToHost, h->stream));
   if (Ky) CU(cudaMemcpy2DAsync(Ky, row, h->Ktab.p + h->nb, 2 * row, row, h->M, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int mbt_get_transverse_log(mbt_handle *h, int64_t first_turn, int64_t n, double *out) {
+  if (!h || !h->trans || !out || first_turn < 1 || n < 0) return fail(MBT_EINVAL, "bad argument");
+  if (first_turn - 1 + n > h->log_cap || first_turn - 1 + n > h->turn) return fail(MBT_ESTATE, "turns not in the log");
+  CU(cudaSetDevice(h->device));
+  if (n == 0) return 0;
+  CU(cudaMemcpyAsync(out, h->log_tr.p + (size_t)(first_turn - 1) * h->M * 4, sizeof(double) * (size_t)n * h->M * 4,
+                     cudaMemcpyDeviceToHost, h->stream));
   CU(cudaStreamSynchronize(h->stream));
   return 0;
 }

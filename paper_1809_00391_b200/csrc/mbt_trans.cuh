@@ -431,6 +431,8 @@ struct TWakeArgs {
   const double *wt;     // [nb] transverse table wt[k] = sum_r W_perp_r(k Delta), wt[0] = 0
   unsigned long long *Sfix;   // [M][2][nb+1] in: sums of this turn (entry nb: outside the window); out: zero
   double *Sov;                // [M][2][nb+1] likewise
+  double *log_tr;             // [log_cap][M][4] mean x, mean y, rms x, rms y per turn, or nullptr
+  int64_t log_cap;
   int32_t Krw;                // resistive-wall history depth in turns (0: off)
   double *ring_g;             // [Krw+1][M][2] source strengths Q_b ubar [C m], slot = turn % (Krw+1)
   const Ctrl *ctrl;
@@ -484,7 +486,8 @@ __global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeAr
       sw[j] = A.wt[j];
     }
   }
-  if (A.Krw > 0) {  // W3: source strength of this bunch and turn, Q_b ubar = (Q_b / N_p) sum of the offsets of all particles
+  // centroid of the bunch (all particles): per-turn log, and W3: source strength Q_b ubar = (Q_b / N_p) sum of offsets
+  if (A.Krw > 0 || A.log_tr) {
     __shared__ long long s_ti[8][2];
     __shared__ double s_to[8][2];
 #pragma unroll
@@ -500,7 +503,13 @@ __global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeAr
       for (int w = 0; w < 8; ++w) { ti += s_ti[w][tid]; to += s_to[w][tid]; }
       const double total = fma((double)ti, tid == 0 ? fx.lsb : fy.lsb, to);
       const uint32_t n = A.ctrl->turn;  // k_wake has closed the turn
-      A.ring_g[((size_t)(n % (uint32_t)(A.Krw + 1)) * A.M + b) * 2 + tid] = qm * total;
+      if (A.Krw > 0) A.ring_g[((size_t)(n % (uint32_t)(A.Krw + 1)) * A.M + b) * 2 + tid] = qm * total;
+      if (A.log_tr && n >= 1u && (int64_t)n <= A.log_cap) {
+        const double iN = 1.0 / (double)A.Np, mean = total * iN;
+        double *row = A.log_tr + ((size_t)(n - 1u) * A.M + b) * 4;
+        row[tid] = mean;
+        row[2 + tid] = sqrt(fmax(A.acc2[2 * b + tid] * iN - mean * mean, 0.0));  // acc2 is reset further down
+      }
     }
   }
   __syncthreads();

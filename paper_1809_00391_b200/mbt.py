@@ -20,7 +20,7 @@ SYMBOLS = [
     "mbt_get_histogram", "mbt_get_wake", "mbt_get_moment_log", "mbt_get_lr_history", "mbt_set_lr_history", "mbt_get_window", "mbt_set_window",
     "mbt_turn", "mbt_phi_s", "mbt_particle_stride", "mbt_device_pointers", "mbt_launch_count",
     "mbt_get_transverse", "mbt_set_transverse", "mbt_get_dipole", "mbt_get_transverse_wake", "mbt_moments_transverse",
-    "mbt_get_rw_kick", "mbt_get_rw_history", "mbt_set_rw_history",
+    "mbt_get_rw_kick", "mbt_get_rw_history", "mbt_set_rw_history", "mbt_get_transverse_log",
     "mbt_last_track_seconds", "mbt_track_profiled", "mbt_philox_selftest", "mbt_normal_selftest", "mbt_last_error", "mbt_version",
 ]
 
@@ -121,6 +121,7 @@ def lib():
         L.mbt_get_dipole.argtypes = [H, dp, dp]
         L.mbt_get_transverse_wake.argtypes = [H, dp, dp]
         L.mbt_moments_transverse.argtypes = [H, dp]
+        L.mbt_get_transverse_log.argtypes = [H, C.c_int64, C.c_int64, dp]
         L.mbt_get_rw_kick.argtypes = [H, dp, dp]
         L.mbt_get_rw_history.argtypes = [H, dp]
         L.mbt_set_rw_history.argtypes = [H, dp]
@@ -343,6 +344,12 @@ class Tracker:
         kx, ky = np.empty((self.M, self.nb)), np.empty((self.M, self.nb))
         _ck(self._L.mbt_get_transverse_wake(self._h, _dp(kx), _dp(ky)))
         return kx, ky
+
+    def transverse_log(self, first_turn, n):
+        """[n][M][4]: mean x, mean y, rms x, rms y at the end of each turn."""
+        out = np.empty((n, self.M, 4))
+        _ck(self._L.mbt_get_transverse_log(self._h, int(first_turn), int(n), _dp(out)))
+        return out
 
     def rw_kick(self):
         """(kx[M], ky[M]): resistive-wall kick of the last tracked turn [V]."""

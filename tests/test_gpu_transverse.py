@@ -207,6 +207,27 @@ def test_transverse_on_baseline_fills(mbt, orc, name, over):
         print(name, r)
 
 
+def test_transverse_log_matches_oracle(mbt, orc):
+    """Per-turn log of mean / rms x, y (P:l.123) from the pass's own sums, twelve turns without re-synchronisation; one
+    bunch displaced by 20 sigma (mean >> rms: the single-pass variance must survive the cancellation)."""
+    cfg = _cfg(m=3, n_per_bunch=9001, n_bins=32)
+    cfg["transverse"].update(rw_amp_x=2.0e9, rw_amp_y=-0.7e9, rw_turns=2)
+    o = orc.Oracle(cfg, log_capacity_turns=12)
+    with mbt.Tracker(cfg, log_capacity_turns=12) as t:
+        x, xp, y, yp = o.transverse_particles()
+        off = np.array([[1.0e-3], [0.0], [-2.0e-4]])
+        o.set_transverse(x + off, xp, y - off, yp)
+        t.set_transverse(x + off, xp, y - off, yp)
+        o.track(12)
+        t.track(12)
+        lc, lg = o.transverse_log(1, 12), t.transverse_log(1, 12)
+        sig = lc[:, :, 2:]
+        assert np.all(np.abs(lg[:, :, :2] - lc[:, :, :2]) <= 1e-9 * np.maximum(sig, np.abs(lc[:, :, :2])))
+        assert np.all(np.abs(lg[:, :, 2:] - lc[:, :, 2:]) <= 1e-7 * sig)
+        with pytest.raises(mbt.MbtError):
+            t.transverse_log(5, 9)
+
+
 def test_transverse_kick_changes_the_angles(mbt, orc):
     """Not a no-op: with the transverse resonator removed the angles of the same turn differ by K(tau)/E0."""
     cfg = _cfg(m=1, n_per_bunch=4096, n_bins=32, radiation=0)

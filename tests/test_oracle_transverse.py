@@ -268,3 +268,17 @@ def test_coherent_tune_shift_of_the_dipole_mode(orc):
     want = -cfg["transverse"]["x"]["beta_m"] * k / (4 * math.pi)
     assert 1e-4 < abs(want) < 6e-4
     assert abs((q1 - q0) / want - 1) < 0.08, (q1 - q0, want)
+
+
+def test_transverse_log_rows_are_the_statistics_of_each_turn(orc):
+    cfg = _cfg(n_per_bunch=300, m=2, radiation=1)
+    o = orc.Oracle(cfg, log_capacity_turns=6)
+    rows = []
+    for _ in range(6):
+        o.track(1)
+        x, xp, y, yp = o.transverse_particles()
+        rows.append(np.stack([x.mean(axis=1), y.mean(axis=1), x.std(axis=1), y.std(axis=1)], axis=1))   # numpy, not the oracle
+    log = o.transverse_log(1, 6)
+    assert np.allclose(log, np.array(rows), rtol=1e-12, atol=1e-20)
+    with pytest.raises(Exception):
+        o.transverse_log(3, 5)
