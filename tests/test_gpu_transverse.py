@@ -207,6 +207,38 @@ def test_transverse_on_baseline_fills(mbt, orc, name, over):
         print(name, r)
 
 
+def test_resistive_wall_growth_rate_long_run(mbt, orc):
+    """Long run (north_star (iii): fitted growth rates within 5 %): the resistive-wall coupled-bunch instability of 22
+    equally spaced bunches (the configuration pinned against linear theory in tests/test_oracle_rw.py, here with 64
+    macro-particles per bunch), 1200 turns in one mbt_track call, growth of mode 19 fitted from the per-turn centroid log
+    on both sides."""
+    import math
+    M, K, turns, n_p = 22, 30, 1200, 64
+    cfg = W.tiny(m=M, n_per_bunch=n_p, n_bins=16, n_lr=0, radiation=0, buckets=list(range(0, 484, 22)))
+    cfg["wake"]["resonators"] = []
+    cfg["fill"]["charge_C"] = [1.0e-9] * M
+    tr = W.transverse_planes(xi_x=0.0, xi_y=0.0, eta_x=0.0, rw_amp_x=3.0e10, rw_amp_y=0.0, rw_turns=K)
+    tr["resonators"] = []
+    cfg["transverse"] = tr
+    nu, beta = tr["x"]["nu"], tr["x"]["beta_m"]
+    b = np.arange(M)
+    a0 = 1.0e-3 * np.exp(2j * np.pi * (19 - nu) * b / M)
+    rates = []
+    o = orc.Oracle(cfg, log_capacity_turns=turns)
+    with mbt.Tracker(cfg, log_capacity_turns=turns) as t:
+        x, xp, y, yp = o.transverse_particles()
+        start = (x + (math.sqrt(beta) * a0.real)[:, None], xp + (a0.imag / math.sqrt(beta))[:, None], y, yp)
+        for side in (o, t):
+            side.set_transverse(*start)
+            side.track(turns)
+            cx = side.transverse_log(1, turns)[:, :, 0]                       # [turns][M] centroids
+            amp = np.abs(cx @ np.exp(-2j * np.pi * (19 - nu) * b / M))
+            n = np.arange(turns)
+            rates.append(np.polyfit(n[300:], np.log(amp[300:]), 1)[0])
+    assert rates[0] > 5e-4                                                     # it does grow
+    assert abs(rates[1] / rates[0] - 1) < 0.05, rates
+
+
 def test_transverse_log_matches_oracle(mbt, orc):
     """Per-turn log of mean / rms x, y (P:l.123) from the pass's own sums, twelve turns without re-synchronisation; one
     bunch displaced by 20 sigma (mean >> rms: the single-pass variance must survive the cancellation)."""
