@@ -162,11 +162,12 @@ int mbt_get_window(mbt_handle *h, int32_t *s_hist, int32_t *s_next);
 int mbt_set_window(mbt_handle *h, const int32_t *s_hist, const int32_t *s_next);
 
 /* ---- transverse planes (HOST pointers; packed [M][N_p] for coordinates, [M][n_bins] for the bin tables) ----
- * The transverse steps of a turn run in kernels of their own after the fused longitudinal pass: betatron map,
- * excitation and dipole deposit (k_trans_map), dipole convolution (k_wake_tr), kick and moments (k_trans_kick); no
- * transverse kick is ever pending.
- * (Superseded: the transverse steps are fused into the 6-D pass k_pass6; like the longitudinal kick, the transverse
- * kicks of the last tracked turn stay pending inside the library and every getter applies them first.) */
+ * The transverse steps of a turn are fused into the 6-D pass (k_pass6: betatron map, excitation, dipole deposit, and the
+ * transverse kicks of the turn before); k_wake_tr convolves the dipole sums (Eq. 6b), k_rw sums the resistive-wall
+ * sources.  Like the longitudinal kick, the transverse kicks of the last tracked turn stay pending inside the library;
+ * every getter applies them first, so what is observed is the state after the turn's kicks (as in the oracle).
+ * All of these return MBT_EINVAL on a handle created without trans.enable.  mbt_set_transverse replaces the four
+ * coordinates of every particle (the longitudinal state, the turn counter and the histories stay). */
 int mbt_get_transverse(mbt_handle *h, double *x, double *xp, double *y, double *yp);
 int mbt_set_transverse(mbt_handle *h, const double *x, const double *xp, const double *y, const double *yp);
 /* dipole sums S[b][k] = sum of u over the particles of bin k [m] and kick tables
