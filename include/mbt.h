@@ -12,6 +12,11 @@
  *   S6  long-range resonator wake        P:l.229-237                 (D14)
  *   S0  wake kick  delta -= V(tau)/E0    P:l.102 Eq.(6a), l.115      (D9, D12)
  *   S7  per-bunch mean / rms             P:l.123-125                 (D22)
+ * and, on a handle created with trans.enable:
+ *   T   betatron map with chromaticity and dispersion   P:l.73-81 Eqs.(3), (4)     (T1-T3)
+ *       transverse damping / excitation                 P:l.83-92 Eq.(5) lines 2-3 (T4, T5)
+ *       per-bin dipole sums, transverse wake kick       P:l.100-111 Eq.(6b)        (T6-T8)
+ *   W   long-range resistive-wall kick                  P:l.117-119                (W1-W5)
  *
  * Every step runs in CUDA kernels on the device; there is NO CPU fallback.  All
  * parameter structs are plain old data; every array passed to mbt_create is a
