@@ -697,6 +697,13 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     T.Sfix = h->Sfix.p; T.Sov = h->Sov.p; T.fix = h->fix.p; T.acc2 = h->acc2.p; T.rw = h->rw.p;
     h->fn_map6 = select_map6(rad_on, wk.gather_order, p->n_cav);
     h->fn_flush6 = select_flush6(wk.gather_order);
+    if (pass6_smem_bytes(nb, 2) > (size_t)prop.sharedMemPerBlockOptin) {
+      char buf[160];
+      snprintf(buf, sizeof buf, "transverse planes: n_bins = %d needs %zu bytes of shared memory per CTA (limit %zu)", nb,
+               pass6_smem_bytes(nb, 2), (size_t)prop.sharedMemPerBlockOptin);
+      destroy(h);
+      return fail(MBT_EINVAL, buf);
+    }
     // three stages in flight if two CTAs then still fit an SM, else two
     T.stages = (2 * (pass6_smem_bytes(nb, 3) + 1024) <= (size_t)prop.sharedMemPerMultiprocessor) ? 3 : 2;
     if (const char *e = getenv("MBT_STAGES6")) T.stages = std::min(kMaxStages6, std::max(2, atoi(e)));  // measurement knob

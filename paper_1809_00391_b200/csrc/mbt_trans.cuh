@@ -517,12 +517,24 @@ __global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeAr
     A.fix[2 * b + tid] = make_fix_scale(A.acc2[2 * b + tid] / (double)A.Np, A.fix_bits);
     A.acc2[2 * b + tid] = 0.0;
   }
-  for (int j = tid; j < nb; j += 256) {
-    double ax = 0.0, ay = 0.0;
-    for (int k = 0; k < j; ++k) {
-      ax = fma(sw[j - k], sx[k], ax);
-      ay = fma(sw[j - k], sy[k], ay);
+  // outputs dealt out so that a thread's two outputs (j, nb-1-j) cost nb-1 terms together; four accumulators per
+  // plane keep the dependent DFMA chains (8 cycles each) and the shared-memory loads overlapped
+  for (int jj = tid; jj < nb; jj += 256) {
+    const int j = (jj & 1) ? nb - 1 - (jj >> 1) : (jj >> 1);
+    double ax0 = 0.0, ax1 = 0.0, ax2 = 0.0, ax3 = 0.0, ay0 = 0.0, ay1 = 0.0, ay2 = 0.0, ay3 = 0.0;
+    int k = 0;
+    for (; k + 4 <= j; k += 4) {
+      const double w0 = sw[j - k], w1 = sw[j - k - 1], w2 = sw[j - k - 2], w3 = sw[j - k - 3];
+      ax0 = fma(w0, sx[k], ax0); ay0 = fma(w0, sy[k], ay0);
+      ax1 = fma(w1, sx[k + 1], ax1); ay1 = fma(w1, sy[k + 1], ay1);
+      ax2 = fma(w2, sx[k + 2], ax2); ay2 = fma(w2, sy[k + 2], ay2);
+      ax3 = fma(w3, sx[k + 3], ax3); ay3 = fma(w3, sy[k + 3], ay3);
     }
+    for (; k < j; ++k) {
+      ax0 = fma(sw[j - k], sx[k], ax0);
+      ay0 = fma(sw[j - k], sy[k], ay0);
+    }
+    const double ax = (ax0 + ax1) + (ax2 + ax3), ay = (ay0 + ay1) + (ay2 + ay3);
     kx[j] = ax; ky[j] = ay;
     A.K[ox + j] = ax;
     A.K[oy + j] = ay;

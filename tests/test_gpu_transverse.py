@@ -280,6 +280,46 @@ def test_transverse_kick_changes_the_angles(mbt, orc):
         assert np.array_equal(t.transverse_particles()[0], t0.transverse_particles()[0])   # the kick acts on u' only
 
 
+def test_transverse_edge_cases(mbt, orc):
+    """Degenerate inputs of the 6-D pass: everybody outside the bin window (no dipole sums, no wake kick, the
+    resistive-wall kick still reaches every particle); offsets far beyond the fixed-point range X_max = 64 rms (the
+    fp64 overflow path of the dipole sums) and a bunch sitting exactly on the axis (<u^2> = 0)."""
+    # (1) all particles outside the window
+    cfg = _cfg(m=3, n_per_bunch=500, n_bins=16)
+    cfg["transverse"].update(rw_amp_x=2.0e9, rw_amp_y=1.0e9, rw_turns=2)
+    o = orc.Oracle(cfg)
+    tau, delta = o.particles()
+    o.set_particles(tau + 120e-12, delta * 0.0, 0)
+    x, xp, y, yp = o.transverse_particles()
+    o.set_transverse(x + 1e-3, xp, y - 1e-3, yp)
+    o.track(2)
+    with mbt.Tracker(cfg) as t:
+        for _ in range(2):
+            r = assert_transverse_turn_parity(o, t, cfg)
+        assert np.all(t.moments()[:, 0] == 0) and not t.dipole()[0].any() and not t.transverse_wake()[0].any()
+        assert np.abs(t.rw_kick()[0]).max() > 0
+    # (2) outliers beyond X_max and an on-axis bunch
+    cfg = _cfg(m=3, n_per_bunch=2049, n_bins=32)
+    o = orc.Oracle(cfg)
+    x, xp, y, yp = [a.copy() for a in o.transverse_particles()]
+    x[0, ::97] = 0.5                               # 1e4 sigma_x: far outside 64 rms of the rest ... but they raise the rms
+    x[0, 5] = 40.0                                 # ... and this one is beyond 64 rms whatever the others do
+    y[0, 7] = -3.0
+    x[1, :] = 0.0; xp[1, :] = 0.0; y[1, :] = 0.0; yp[1, :] = 0.0
+    o.set_transverse(x, xp, y, yp)
+    o.track(1)
+    with mbt.Tracker(cfg) as t:
+        for _ in range(3):
+            r = assert_transverse_turn_parity(o, t, cfg)
+        sx, sy = t.dipole()
+        assert np.abs(sx[0]).max() > 1.0 and np.abs(sy[0]).max() > 0.5    # the outliers are in the sums
+    # (3) too many bins for the 6-D pass's shared memory: a clean error, not a launch failure
+    big = _cfg(m=1, n_per_bunch=64, n_bins=4000)
+    with pytest.raises(mbt.MbtError) as e:
+        mbt.Tracker(big)
+    assert e.value.code == -1 and "shared memory" in str(e.value)
+
+
 def test_transverse_entry_points_refuse_a_longitudinal_handle(mbt):
     cfg = W.tiny()
     with mbt.Tracker(cfg) as t:
@@ -290,6 +330,14 @@ def test_transverse_entry_points_refuse_a_longitudinal_handle(mbt):
             t.moments_transverse()
         with pytest.raises(mbt.MbtError):
             t.dipole()
+        with pytest.raises(mbt.MbtError):
+            t.rw_kick()
+        with pytest.raises(mbt.MbtError):
+            t.transverse_log(1, 0)
+    bad = _cfg()
+    bad["transverse"]["rw_turns"] = -2
+    with pytest.raises(mbt.MbtError):
+        mbt.Tracker(bad)
     bad = _cfg()
     bad["transverse"]["x"]["beta_m"] = 0.0
     with pytest.raises(mbt.MbtError):
