@@ -186,7 +186,7 @@ void enqueue_pass(mbt_handle *h) {
 }
 void enqueue_wakes(mbt_handle *h) {
   k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
-  if (h->trans) k_wake_tr<<<h->M, 256, (size_t)h->nb * 5 * sizeof(double), h->stream>>>(h->twargs);
+  if (h->trans) k_wake_tr<<<h->M, 256, wake_tr_smem_bytes(h->nb), h->stream>>>(h->twargs);
   if (h->Krw > 0) k_rw<<<h->M, 256, 0, h->stream>>>(h->rwargs);
 }
 // launches per tracked turn: 2; 3 with the transverse planes; 4 with their resistive-wall kick
@@ -710,7 +710,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     h->smem_pass6 = pass6_smem_bytes(nb, T.stages);
     CUH(cudaFuncSetAttribute((const void *)h->fn_map6, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass6));
     CUH(cudaFuncSetAttribute((const void *)h->fn_flush6, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass6));
-    CUH(cudaFuncSetAttribute(k_wake_tr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)nb * 5 * sizeof(double))));
+    CUH(cudaFuncSetAttribute(k_wake_tr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wake_tr_smem_bytes(nb)));
     {
       int occ = 0;
       CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)h->fn_map6, kPassThreads, h->smem_pass6));
