@@ -610,15 +610,22 @@ __global__ void __launch_bounds__(256) k_rw(const __grid_constant__ RwArgs A) {
   const uint32_t n = A.ctrl->turn;
   const int sb = A.bucket[b];
   double sx = 0.0, sy = 0.0;
-  for (int idx = tid; idx < (A.Krw + 1) * A.M; idx += 256) {
-    const int k = idx / A.M, bp = idx - k * A.M;  // source: turn n - k, bunch bp
-    if ((uint32_t)k >= n) continue;                 // nothing before turn 1
-    const int d = k * A.h + (sb - A.bucket[bp]);
-    if (d <= 0) continue;                           // this turn: only the bunches ahead
-    const double w = A.wrw[d];
-    const double *g = A.ring_g + ((size_t)((n - (uint32_t)k) % (uint32_t)(A.Krw + 1)) * A.M + bp) * 2;
-    sx = fma(g[0], w, sx);
-    sy = fma(g[1], w, sy);
+  // a thread keeps its source bunches bp (their bucket distance within a turn in a register) and walks the turns back;
+  // the loads of one turn do not depend on the previous one's, so they overlap
+  const int kmax = min(A.Krw, (int)min(n - 1u, (uint32_t)A.Krw));  // nothing before turn 1
+  for (int bp = tid; bp < A.M; bp += 256) {
+    const int ds = sb - A.bucket[bp];
+    const double2 *g = reinterpret_cast<const double2 *>(A.ring_g) + bp;
+    uint32_t slot = n % (uint32_t)(A.Krw + 1);
+#pragma unroll 4
+    for (int k = 0; k <= kmax; ++k) {  // source: turn n - k, bunch bp, bucket distance d
+      const int d = k * A.h + ds;
+      const double w = d > 0 ? A.wrw[d] : 0.0;          // this turn (k = 0): only the bunches ahead
+      const double2 gv = g[(size_t)slot * A.M];
+      sx = fma(gv.x, w, sx);
+      sy = fma(gv.y, w, sy);
+      slot = slot == 0u ? (uint32_t)A.Krw : slot - 1u;
+    }
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
