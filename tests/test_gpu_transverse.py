@@ -280,6 +280,42 @@ def test_transverse_kick_changes_the_angles(mbt, orc):
         assert np.array_equal(t.transverse_particles()[0], t0.transverse_particles()[0])   # the kick acts on u' only
 
 
+def test_transverse_full_size_c4(mbt, orc):
+    """The workload `bench.py --transverse --rw-turns 20` times (363 x 1e5 particles, 6-D, resistive wall), in its launch
+    configuration: initial distribution and one tracked turn element by element against the oracle, then properties
+    that hold at any size."""
+    cfg = W.config("c4")
+    cfg["transverse"] = W.transverse_planes(rw_amp_x=2.0e9, rw_amp_y=1.0e9, rw_turns=20)
+    o = orc.Oracle(cfg, lr_mode=1)
+    with mbt.Tracker(cfg) as t:
+        for g, c in zip(t.transverse_particles(), o.transverse_particles()):
+            assert particle_errors(g, c) <= TOL_PARTICLE
+        del g, c
+        o.track(1); t.track(1)
+        errs = {}
+        for nm, g, c in zip(("x", "xp", "y", "yp"), t.transverse_particles(), o.transverse_particles()):
+            errs[nm] = particle_errors(g, c)
+        del g, c
+        tau_c, delta_c = o.particles()
+        tau_g, delta_g = t.particles()
+        errs["tau"], errs["delta"] = particle_errors(tau_g, tau_c), particle_errors(delta_g, delta_c)
+        print(errs)
+        assert max(errs.values()) <= TOL_PARTICLE, errs
+        if np.array_equal(t.histogram(), o.histogram()):
+            for g, c in zip(t.dipole() + t.transverse_wake(), o.dipole() + o.transverse_wake()):
+                assert wake_error(g, c) <= TOL_WAKE
+        for g, c in zip(t.rw_kick(), o.rw_kick()):
+            assert np.abs(g - c).max() <= TOL_WAKE * np.abs(c).max()
+        # the dipole sums are fixed-point integers: a second handle reproduces them bit for bit
+        sx1, sy1 = t.dipole()
+    with mbt.Tracker(cfg) as t2:
+        t2.track(1)
+        sx2, sy2 = t2.dipole()
+        assert np.array_equal(sx1, sx2) and np.array_equal(sy1, sy2)
+        m = t2.moments()
+        assert np.all(t2.histogram().sum(axis=1) == m[:, 0]) and np.all(m[:, 0] + m[:, 1] == cfg["fill"]["n_per_bunch"])
+
+
 def test_three_cavities_and_lost_particles(mbt, orc):
     """The generic cavity loop (more than two cavities) of both passes, and particles far off the bucket (the
     large-argument branch of the RF sine, |phase| >= 2^16 rad) in the 6-D pass; NaN offsets stay NaN and do not crash."""
