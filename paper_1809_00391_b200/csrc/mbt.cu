@@ -873,6 +873,10 @@ int mbt_get_particles(mbt_handle *h, double *tau, double *delta) {
 int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int64_t turn) {
   if (!h || !tau || !delta || turn < 0 || turn > 0xFFFFFFFFll) return fail(MBT_EINVAL, "bad argument");
   CU(cudaSetDevice(h->device));
+  if (h->trans) {  // a pending transverse kick belongs to x', y', which this call does not replace: apply it first
+    int rc = flush(h);
+    if (rc) return rc;
+  }
   const size_t n = (size_t)h->M * h->Np;
   if (h->ld == h->Np) {
     CU(cudaMemcpyAsync(h->d_tau, tau, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
@@ -898,6 +902,7 @@ int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int
   CU(cudaMemsetAsync(h->nout_acc.p, 0, sizeof(unsigned long long) * h->M, h->stream));
   CU(cudaMemsetAsync(h->ring_a.p, 0, sizeof(cplx) * (h->ring_a.n ? h->ring_a.n : 1), h->stream));
   CU(cudaMemsetAsync(h->ring_A.p, 0, sizeof(cplx) * (h->ring_A.n ? h->ring_A.n : 1), h->stream));
+  if (h->trans) CU(cudaMemsetAsync(h->ring_g.p, 0, sizeof(double) * (h->ring_g.n ? h->ring_g.n : 1), h->stream));
   CU(cudaStreamSynchronize(h->stream));
   h->turn = turn;
   h->dirty = true;

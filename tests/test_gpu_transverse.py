@@ -355,6 +355,24 @@ def test_three_cavities_and_lost_particles(mbt, orc):
         assert np.array_equal(t.histogram(), o.histogram())
 
 
+def test_set_particles_keeps_a_pending_transverse_kick(mbt):
+    """mbt_set_particles replaces tau and delta only: the transverse kick still pending from the last tracked turn must
+    reach x', y' first (it is not the caller's to lose)."""
+    cfg = _cfg(m=2, n_per_bunch=3000, n_bins=32)
+    cfg["transverse"].update(rw_amp_x=2.0e9, rw_amp_y=1.0e9, rw_turns=2)
+    with mbt.Tracker(cfg) as a, mbt.Tracker(cfg) as b:
+        for t in (a, b):
+            x, xp, y, yp = t.transverse_particles()
+            t.set_transverse(x + 1e-3, xp, y - 1e-3, yp)
+            t.track(2)
+        tau, delta = a.particles()                 # flushes the pending kicks of `a`
+        ra = a.transverse_particles()
+        b.set_particles(tau, delta, 2)             # no getter in between
+        rb = b.transverse_particles()
+        for u, v in zip(ra, rb):
+            assert np.array_equal(u, v)
+
+
 def test_transverse_edge_cases(mbt, orc):
     """Degenerate inputs of the 6-D pass: everybody outside the bin window (no dipole sums, no wake kick, the
     resistive-wall kick still reaches every particle); offsets far beyond the fixed-point range X_max = 64 rms (the
