@@ -132,6 +132,9 @@ struct mbt_handle {
   RwArgs rwargs;
   DevBuf<double> ring_g, rw, wrw, log_tr;
   DevBuf<int32_t> d_bucket;
+  DevBuf<uint32_t> turn_tr;
+  cudaStream_t stream2 = nullptr;          // side stream: k_wake_tr and k_rw run beside k_wake (fork / join by events)
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   int wake_splits = 1;
   DevBuf<double> lo_hist, lo_next;
   DevBuf<cplx> shift_src, shift_wit;
@@ -184,10 +187,19 @@ void enqueue_pass(mbt_handle *h) {
   if (h->trans) h->fn_map6<<<dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream>>>(h->args6);
   else h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
 }
+// the wake kernels of a turn: k_wake on the handle's stream; the transverse ones (independent of it: they read what the
+// pass wrote, and the next pass waits for both) on the side stream.  Under stream capture this becomes a fork and a join
+// in the graph.
 void enqueue_wakes(mbt_handle *h) {
+  if (h->trans) {
+    cudaEventRecord(h->ev_fork, h->stream);
+    cudaStreamWaitEvent(h->stream2, h->ev_fork, 0);
+    k_wake_tr<<<h->M, 256, wake_tr_smem_bytes(h->nb), h->stream2>>>(h->twargs);
+    if (h->Krw > 0) k_rw<<<h->M, 256, 0, h->stream2>>>(h->rwargs);
+    cudaEventRecord(h->ev_join, h->stream2);
+  }
   k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
-  if (h->trans) k_wake_tr<<<h->M, 256, wake_tr_smem_bytes(h->nb), h->stream>>>(h->twargs);
-  if (h->Krw > 0) k_rw<<<h->M, 256, 0, h->stream>>>(h->rwargs);
+  if (h->trans) cudaStreamWaitEvent(h->stream, h->ev_join, 0);
 }
 // launches per tracked turn: 2; 3 with the transverse planes; 4 with their resistive-wall kick
 int launches_per_turn(const mbt_handle *h) { return h->trans ? (h->Krw > 0 ? 4 : 3) : 2; }
@@ -242,6 +254,9 @@ void destroy(mbt_handle *h) {
   if (h->stream) cudaStreamSynchronize(h->stream);
   if (h->graph1) cudaGraphExecDestroy(h->graph1);
   if (h->graphU) cudaGraphExecDestroy(h->graphU);
+  if (h->stream2) { cudaStreamSynchronize(h->stream2); cudaStreamDestroy(h->stream2); }
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  if (h->ev_join) cudaEventDestroy(h->ev_join);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
   if (h->own_particles) {
@@ -255,7 +270,7 @@ void destroy(mbt_handle *h) {
   h->tx.release(); h->txp.release(); h->ty.release(); h->typ.release(); h->wt.release(); h->Sfix.release(); h->Sov.release();
   h->S_last.release(); h->Ktab.release(); h->acc2.release(); h->fix.release(); h->cellX.release(); h->cellY.release();
   h->mom_tr_acc.release(); h->mom_tr.release();
-  h->ring_g.release(); h->rw.release(); h->wrw.release(); h->d_bucket.release(); h->log_tr.release();
+  h->ring_g.release(); h->rw.release(); h->wrw.release(); h->d_bucket.release(); h->log_tr.release(); h->turn_tr.release();
   h->s_hist.release(); h->s_next.release(); h->lo_hist.release(); h->lo_next.release();
   h->shift_src.release(); h->shift_wit.release();
   h->Esrc.release(); h->F.release(); h->g_step.release(); h->g_tail.release(); h->g_hist.release(); h->a_cur.release();
@@ -669,7 +684,11 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     RwArgs &Rw = h->rwargs;
     memset(&Rw, 0, sizeof Rw);
     Rw.M = M; Rw.Krw = h->Krw; Rw.h = rg.h; Rw.bucket = h->d_bucket.p; Rw.ring_g = h->ring_g.p; Rw.wrw = h->wrw.p;
-    Rw.amp[0] = tr.rw_amp_x; Rw.amp[1] = tr.rw_amp_y; Rw.rw = h->rw.p; Rw.ctrl = h->ctrl.p;
+    CUH(h->turn_tr.alloc(1));
+    CUH(cudaStreamCreateWithFlags(&h->stream2, cudaStreamNonBlocking));
+    CUH(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+    CUH(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
+    Rw.amp[0] = tr.rw_amp_x; Rw.amp[1] = tr.rw_amp_y; Rw.rw = h->rw.p; Rw.turn_tr = h->turn_tr.p;
     CUH(h->S_last.alloc((size_t)M * 2 * nb)); CUH(h->Ktab.alloc((size_t)M * 2 * nb));
     CUH(h->cellX.alloc((size_t)M * (nb + 2))); CUH(h->cellY.alloc((size_t)M * (nb + 2)));
     CUH(h->fix.alloc((size_t)M * 2)); CUH(h->acc2.alloc((size_t)M * 2));
@@ -694,7 +713,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
       d.exc_up = q.sigma_up * std::sqrt(q.D_exc);
     }
     T.cellX = h->cellX.p; T.cellY = h->cellY.p;
-    T.Sfix = h->Sfix.p; T.Sov = h->Sov.p; T.fix = h->fix.p; T.acc2 = h->acc2.p; T.rw = h->rw.p;
+    T.Sfix = h->Sfix.p; T.Sov = h->Sov.p; T.fix = h->fix.p; T.acc2 = h->acc2.p; T.rw = h->rw.p; T.turn_tr = h->turn_tr.p;
     h->fn_map6 = select_map6(rad_on, wk.gather_order, p->n_cav);
     h->fn_flush6 = select_flush6(wk.gather_order);
     if (pass6_smem_bytes(nb, 2) > (size_t)prop.sharedMemPerBlockOptin) {
@@ -730,7 +749,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     Tw.qm = h->qm.p; Tw.wt = h->wt.p;
     Tw.Sfix = h->Sfix.p; Tw.Sov = h->Sov.p; Tw.fix = h->fix.p; Tw.acc2 = h->acc2.p;
     Tw.S_last = h->S_last.p; Tw.K = h->Ktab.p; Tw.cellX = h->cellX.p; Tw.cellY = h->cellY.p;
-    Tw.Krw = h->Krw; Tw.ring_g = h->ring_g.p; Tw.ctrl = h->ctrl.p;
+    Tw.Krw = h->Krw; Tw.ring_g = h->ring_g.p; Tw.turn_tr = h->turn_tr.p;
     if (h->log_cap > 0) CUH(h->log_tr.alloc((size_t)h->log_cap * M * 4));
     Tw.log_tr = h->log_cap > 0 ? h->log_tr.p : nullptr;
     Tw.log_cap = h->log_cap;

@@ -50,6 +50,8 @@ struct Args6 {
   const double *rw;            // [M][2] long-range resistive-wall kick of the last turn [V] (zeros without it)
   const FixScale *fix;         // [M][2]
   double *acc2;                // [M][2] sum u^2 of the mapped state (the next turn's scale)
+  uint32_t *turn_tr;           // the turn this pass tracks, for k_wake_tr / k_rw: they run beside k_wake, which bumps
+                               // ctrl->turn, so they must not read that word
   uint32_t tile_pairs;         // pairs per CTA
   int32_t stages;              // shared-memory stages of the particle stream (2..kMaxStages6)
 };
@@ -149,6 +151,7 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
   const uint32_t n = A.ctrl->turn + 1u;
   const bool have_kick = A.ctrl->kick_pending != 0u;
   const uint32_t hi_nb = (uint32_t)__double2hiint(A.nb_d);
+  if (MAP && tid == 0 && blockIdx.x == 0 && b == 0) *A6.turn_tr = n;
   const uint32_t p0 = blockIdx.x * A6.tile_pairs;
   const uint32_t p1 = (A.ppb - p0 < A6.tile_pairs) ? A.ppb : p0 + A6.tile_pairs;
   const double lo_old = A.lo_hist[b];
@@ -435,7 +438,7 @@ struct TWakeArgs {
   int64_t log_cap;
   int32_t Krw;                // resistive-wall history depth in turns (0: off)
   double *ring_g;             // [Krw+1][M][2] source strengths Q_b ubar [C m], slot = turn % (Krw+1)
-  const Ctrl *ctrl;
+  const uint32_t *turn_tr;    // the turn being closed (written by the pass; ctrl->turn is k_wake's to bump, beside us)
   FixScale *fix;              // [M][2] in: the scale the sums were deposited with; out: the next turn's
   double *acc2;               // [M][2] in: sum u^2 of this turn's mapped state; out: zero
   double *S_last;             // [M][2][nb] observable copy of the sums [m]
@@ -516,7 +519,7 @@ __global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeAr
       double to = 0.0;
       for (int w = 0; w < 8; ++w) { ti += s_ti[w][tid]; to += s_to[w][tid]; }
       const double total = fma((double)ti, tid == 0 ? fx.lsb : fy.lsb, to);
-      const uint32_t n = A.ctrl->turn;  // k_wake has closed the turn
+      const uint32_t n = *A.turn_tr;
       if (A.Krw > 0) A.ring_g[((size_t)(n % (uint32_t)(A.Krw + 1)) * A.M + b) * 2 + tid] = qm * total;
       if (A.log_tr && n >= 1u && (int64_t)n <= A.log_cap) {
         const double iN = 1.0 / (double)A.Np, mean = total * iN;
@@ -594,7 +597,8 @@ __global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeAr
 
 // Long-range resistive-wall kick (readings W1..W5): one CTA per bunch b sums the sources of the last Krw turns (all
 // bunches) and of this turn's bunches ahead, weight wrw[d] = (d T_rf)^-1/2 at the bucket distance
-// d = (n - n') h + (s_b - s_b'); fixed summation order (reproducible).  Runs after k_wake_tr of the same turn.
+// d = (n - n') h + (s_b - s_b'); fixed summation order (reproducible).  Runs after k_wake_tr of the same turn, on the
+// library's side stream beside k_wake.
 struct RwArgs {
   int32_t M, Krw, h;
   const int32_t *bucket;  // [M]
@@ -602,12 +606,12 @@ struct RwArgs {
   const double *wrw;      // [(Krw+1) h] weight at bucket distance d (entry 0 unused)
   double amp[2];
   double *rw;             // [M][2] out [V]
-  const Ctrl *ctrl;
+  const uint32_t *turn_tr;
 };
 __global__ void __launch_bounds__(256) k_rw(const __grid_constant__ RwArgs A) {
   __shared__ double s_red[8][2];
   const int b = blockIdx.x, tid = threadIdx.x;
-  const uint32_t n = A.ctrl->turn;
+  const uint32_t n = *A.turn_tr;
   const int sb = A.bucket[b];
   double sx = 0.0, sy = 0.0;
   // a thread keeps its source bunches bp (their bucket distance within a turn in a register) and walks the turns back;
