@@ -15,6 +15,11 @@
 //   6. long-range resonator wake         P:l.229-237 (formula: reading D14)
 //   7. wake kick                         P:l.102 Eq.(6a) (reading D9: delta -= V/E0)
 //   8. per-bunch mean / rms              P:l.123-125
+// and, with trans.enable (readings T1..T8, W1..W5):
+//   3b. betatron map, excitation         P:l.73-92 Eqs.(3)-(5), after the longitudinal map (T1)
+//   4b. per-bin dipole sums              P:l.104-111 (T6)
+//   6b/7b. transverse wake and kick      P:l.100-107 Eq.(6b) (T7, T8)
+//   9. long-range resistive-wall kick    P:l.117-119 (W1..W5), after the statistics of step 8
 //
 // PINS (tests/test_oracle_*.py, all run without a GPU):
 //   philox4x32_10   Random123 known-answer vectors + cuRAND's host-callable Philox header
@@ -29,6 +34,13 @@
 //                   lr_mode 1 (recurrence) against lr_mode 0 (definition)
 //   whole loop      coupled-bunch growth rate vs the analytic uniform-fill formula, Eq.(7)
 //   moments (8)     numpy mean / std
+//   transverse      symplecticity, chromatic tune, dispersive fixed point, Courant-Snyder invariant; W_perp against
+//                   its Lorentzian impedance; dipole sums vs numpy.bincount, Eq.(6b) written out; kick factor of a
+//                   displaced Gaussian bunch from the impedance; coherent tune shift of the dipole line; adiabatic
+//                   damping rate and equilibrium emittance (tests/test_oracle_transverse.py)
+//   resistive wall  partial sums of k^-1/2 for a frozen offset, contiguous distance sum for a uniform fill, pairwise
+//                   brute force, coupled-bunch growth / damping rates vs first-order theory (tests/test_oracle_rw.py)
+// No function of this file is "parity unpinned".
 #include "orc.h"
 
 #include <cmath>
