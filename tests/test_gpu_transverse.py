@@ -355,6 +355,31 @@ def test_three_cavities_and_lost_particles(mbt, orc):
         assert np.array_equal(t.histogram(), o.histogram())
 
 
+def test_transverse_on_a_caller_owned_stream(mbt, orc):
+    """The caller's stream (a torch stream) with the library's side stream forked off it: 40 turns through the
+    graph-replayed path (unrolled graph + single-turn graphs), twice, against the oracle; two handles on two streams at
+    the same time do not disturb each other."""
+    import torch
+    cfg = _cfg(m=3, n_per_bunch=2500, n_bins=32)
+    cfg["transverse"].update(rw_amp_x=2.0e9, rw_amp_y=1.0e9, rw_turns=3)
+    o = orc.Oracle(cfg, log_capacity_turns=80)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    with mbt.Tracker(cfg, log_capacity_turns=80, stream=s1.cuda_stream) as a, \
+            mbt.Tracker(cfg, log_capacity_turns=80, stream=s2.cuda_stream) as b:
+        for _ in range(2):
+            a.track(40); b.track(40)
+            o.track(40)
+        lc = o.transverse_log(1, 80)
+        for t in (a, b):
+            lg = t.transverse_log(1, 80)
+            assert np.all(np.abs(lg[:, :, :2] - lc[:, :, :2]) <= 1e-8 * lc[:, :, 2:])
+            for g, c in zip(t.transverse_particles(), o.transverse_particles()):
+                assert particle_errors(g, c) <= 1e-9
+        assert np.array_equal(a.dipole()[0], b.dipole()[0])        # fixed-point sums: identical bit for bit
+        for u, v in zip(a.transverse_particles(), b.transverse_particles()):
+            assert np.array_equal(u, v)
+
+
 def test_set_particles_keeps_a_pending_transverse_kick(mbt):
     """mbt_set_particles replaces tau and delta only: the transverse kick still pending from the last tracked turn must
     reach x', y' first (it is not the caller's to lose)."""
