@@ -171,6 +171,42 @@ pass_fn select_flush(int gather) {
   return gather ? (pass_fn)k_pass<false, false, 1, 0, NPAIR> : (pass_fn)k_pass<false, false, 0, 0, NPAIR>;
 }
 
+// Tiles of a pass: pairs per CTA (a multiple of `stride`, the pairs a CTA advances per iteration) and tiles per bunch.
+// Large workloads: the grid runs in waves of `slots` resident CTAs, and what a launch costs beyond its traffic is the
+// last, partly filled wave and the per-CTA prologue (gather cells, barriers) and epilogue (count flush).  Measured at c4
+// (k_pass: 7 ragged tiles of 16 iterations -> 4 even tiles of 25: 0.2063 -> 0.1958 ms; 3, 5, 6, 7 even tiles 0.199 ..
+// 0.204; k_pass6: 13 ragged tiles of 16 -> 4 even tiles of 49: 0.864 -> 0.832 ms, 22 tiles of 9: 0.879).  So: even tiles
+// (the last one at least 3/4 of the others), at least 8 iterations each, at least two waves of CTAs, and among those
+// the tile count that minimises ceil(w) / w (1 + 1 / iterations), w = tiles M / slots the number of waves and one
+// iteration's worth of per-CTA work.  Small workloads: ~16 iterations per CTA, halved until the grid fills two waves.
+// MBT_TILE_ITERS overrides (measurement knob).
+void choose_tiles(int64_t ppb, int64_t stride, int M, int slots, uint32_t *tile_pairs, int *tiles) {
+  const int64_t total = (ppb + stride - 1) / stride;  // iterations per bunch
+  int64_t iters = 0;
+  if (const char *e = getenv("MBT_TILE_ITERS")) iters = atoi(e) > 0 ? atoi(e) : 0;
+  if (iters == 0) {
+    double best = 1.0e30;
+    for (int64_t n = 1; n <= total; ++n) {
+      const int64_t it = (total + n - 1) / n;
+      if (it < 8) break;
+      const int64_t n_eff = (total + it - 1) / it, last = total - (n_eff - 1) * it;
+      if (n_eff * M < 2ll * slots) continue;
+      if (n_eff > 1 && 4 * last < 3 * it) continue;
+      const double w = (double)(n_eff * M) / (double)slots, cost = std::ceil(w) / w * (1.0 + 1.0 / (double)it);
+      if (cost < best) { best = cost; iters = it; }
+    }
+  }
+  if (iters == 0) {
+    iters = 16;
+    while (iters > 1 && (int64_t)M * ((ppb + iters * stride - 1) / (iters * stride)) < 2ll * slots) iters /= 2;
+  }
+  *tile_pairs = (uint32_t)(iters * stride);
+  *tiles = (int)((ppb + iters * stride - 1) / (iters * stride));
+  if (getenv("MBT_DEBUG"))
+    fprintf(stderr, "mbt: choose_tiles ppb %lld stride %lld M %d slots %d -> %lld iterations, %d tiles\n", (long long)ppb,
+            (long long)stride, M, slots, (long long)iters, *tiles);
+}
+
 typedef void (*pass6_fn)(const Args6);
 pass6_fn select_map6(bool rad, int gather, int n_cav) {
 #define MBT_SEL_(R, G)                                             \
@@ -634,17 +670,12 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   CUH(cudaFuncSetAttribute((const void *)h->fn_map, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
   CUH(cudaFuncSetAttribute((const void *)h->fn_flush, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
   CUH(cudaFuncSetAttribute(k_wake, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_wake));
-  // tiles: ~16 iterations per CTA; fewer when the whole grid would not fill two waves of the device
+  // tiles (choose_tiles)
   {
     int occ = 0;
     CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)h->fn_map, kPassThreads, h->smem_pass));
     if (occ < 1) occ = 1;
-    const int64_t stride = (int64_t)kPassThreads * h->npair, ppb = h->ld / 2;
-    int64_t iters = 16;
-    if (const char *e = getenv("MBT_TILE_ITERS")) iters = atoi(e) > 0 ? atoi(e) : 16;  // measurement knob
-    while (iters > 1 && (int64_t)M * ((ppb + iters * stride - 1) / (iters * stride)) < 2ll * prop.multiProcessorCount * occ) iters /= 2;
-    A.tile_pairs = (uint32_t)(iters * stride);
-    h->grid_pass = (int)((ppb + A.tile_pairs - 1) / A.tile_pairs);
+    choose_tiles(h->ld / 2, (int64_t)kPassThreads * h->npair, M, prop.multiProcessorCount * occ, &A.tile_pairs, &h->grid_pass);
   }
 
   // ---- initial distribution (D20) on the device
@@ -734,11 +765,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
       int occ = 0;
       CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)h->fn_map6, kPassThreads, h->smem_pass6));
       if (occ < 1) occ = 1;
-      const int64_t ppb = h->ld / 2;
-      int64_t iters = 16;
-      while (iters > 1 && (int64_t)M * ((ppb + iters * kPassThreads - 1) / (iters * kPassThreads)) < 2ll * prop.multiProcessorCount * occ) iters /= 2;
-      T.tile_pairs = (uint32_t)(iters * kPassThreads);
-      h->grid_pass6 = (int)((ppb + T.tile_pairs - 1) / T.tile_pairs);
+      choose_tiles(h->ld / 2, kPassThreads, M, prop.multiProcessorCount * occ, &T.tile_pairs, &h->grid_pass6);
     }
     TMomArgs &Tm = h->tmargs;
     Tm.x = h->tx.p; Tm.xp = h->txp.p; Tm.y = h->ty.p; Tm.yp = h->typ.p; Tm.ld = h->ld; Tm.Np = (uint32_t)h->Np; Tm.tile = 8192;
