@@ -176,10 +176,10 @@ pass_fn select_flush(int gather) {
 // last, partly filled wave and the per-CTA prologue (gather cells, barriers) and epilogue (count flush).  Measured at c4
 // (k_pass: 7 ragged tiles of 16 iterations -> 4 even tiles of 25: 0.2063 -> 0.1958 ms; 3, 5, 6, 7 even tiles 0.199 ..
 // 0.204; k_pass6: 13 ragged tiles of 16 -> 4 even tiles of 49: 0.864 -> 0.832 ms, 22 tiles of 9: 0.879).  So: even tiles
-// (the last one at least 3/4 of the others), at least 8 iterations each, at least two waves of CTAs, and among those
-// the tile count that minimises ceil(w) / w (1 + 1 / iterations), w = tiles M / slots the number of waves and one
-// iteration's worth of per-CTA work.  Small workloads: ~16 iterations per CTA, halved until the grid fills two waves.
-// MBT_TILE_ITERS overrides (measurement knob).
+// (the last one at least 3/4 of the others) and among those the tile count that minimises
+// ceil(w) / w (1 + 1 / iterations), w = tiles M / slots the number of waves, one iteration's worth of per-CTA work.
+// The same rule serves the small workloads, where it settles just under one wave (c2, one bunch of 1e6: 391 CTAs of
+// 5 iterations instead of 977 of 2: pass 23.7 -> 18.6 us).  MBT_TILE_ITERS overrides (measurement knob).
 void choose_tiles(int64_t ppb, int64_t stride, int M, int slots, uint32_t *tile_pairs, int *tiles) {
   const int64_t total = (ppb + stride - 1) / stride;  // iterations per bunch
   int64_t iters = 0;
@@ -188,9 +188,8 @@ void choose_tiles(int64_t ppb, int64_t stride, int M, int slots, uint32_t *tile_
     double best = 1.0e30;
     for (int64_t n = 1; n <= total; ++n) {
       const int64_t it = (total + n - 1) / n;
-      if (it < 8) break;
       const int64_t n_eff = (total + it - 1) / it, last = total - (n_eff - 1) * it;
-      if (n_eff * M < 2ll * slots) continue;
+      if (n_eff != n) continue;  // the same tiling as a smaller n
       if (n_eff > 1 && 4 * last < 3 * it) continue;
       const double w = (double)(n_eff * M) / (double)slots, cost = std::ceil(w) / w * (1.0 + 1.0 / (double)it);
       if (cost < best) { best = cost; iters = it; }
