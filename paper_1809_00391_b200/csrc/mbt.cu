@@ -145,6 +145,9 @@ struct mbt_handle {
   void (*fn_map)(const Args) = nullptr;    // k_pass<true, ...> chosen for this handle's effects
   void (*fn_flush)(const Args) = nullptr;  // k_pass<false, ...>
   int npair = 1;
+  int pdl = 1;  // bit 0: the pass, bit 1: k_wake launched as a programmatic dependent (longitudinal handles; MBT_PDL sets it).
+                // Measured, us per turn, graph replay: pass only c1 10.8 -> 10.0, c3 16.6 -> 16.0, c4 223.9 -> 222.8; k_wake as
+                // well helps c1 (9.1) but costs c2 and c3 (26.8, 19.3): its resident CTAs are in the way of the pass's tail
   DevBuf<LogTabEntry> logtab;
   cudaGraphExec_t graph1 = nullptr, graphU = nullptr;
   int unroll = 16;
@@ -218,8 +221,25 @@ pass6_fn select_map6(bool rad, int gather, int n_cav) {
 pass6_fn select_flush6(int gather) { return gather ? (pass6_fn)k_pass6<false, false, 1, 0> : (pass6_fn)k_pass6<false, false, 0, 0>; }
 
 // the pass of a tracked turn: the longitudinal one, or the fused 6-D one of a handle with the transverse planes
+// launch as a programmatic dependent of the kernel before it on the stream (mbt_kernels.cuh, griddepcontrol)
+template <typename ArgT>
+void launch_dependent(void (*fn)(const ArgT), dim3 grid, int threads, size_t smem, cudaStream_t st, const ArgT &a) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(threads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, fn, a);
+}
+
 void enqueue_pass(mbt_handle *h) {
   if (h->trans) h->fn_map6<<<dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream>>>(h->args6);
+  else if (h->pdl & 1) launch_dependent(h->fn_map, dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream, h->args);
   else h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
 }
 // the wake kernels of a turn: k_wake on the handle's stream; the transverse ones (independent of it: they read what the
@@ -233,7 +253,10 @@ void enqueue_wakes(mbt_handle *h) {
     if (h->Krw > 0) k_rw<<<h->M, 256, 0, h->stream2>>>(h->rwargs);
     cudaEventRecord(h->ev_join, h->stream2);
   }
-  k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
+  if ((h->pdl & 2) && !h->trans)
+    launch_dependent<WakeArgs>(k_wake, dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream, h->wargs);
+  else
+    k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
   if (h->trans) cudaStreamWaitEvent(h->stream, h->ev_join, 0);
 }
 // launches per tracked turn: 2; 3 with the transverse planes; 4 with their resistive-wall kick
@@ -659,6 +682,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   // ---- launch shapes: one resident wave of CTAs, each owning a contiguous run of pairs
   // two pairs per thread (twice the independent arithmetic per warp, 2 CTAs/SM) pay off except for small
   // two-cavity workloads, where the four sine chains per thread cost more registers than they hide latency
+  if (const char *e = getenv("MBT_PDL")) h->pdl = atoi(e) & 3;  // measurement knob
   h->npair = kDefaultNPair ? kDefaultNPair : ((p->n_cav == 1 || (int64_t)M * h->Np >= 10000000ll) ? 2 : 1);
   if (const char *e = getenv("MBT_NPAIR")) h->npair = (atoi(e) == 2) ? 2 : 1;  // measurement knob
   const bool rad_on = p->rad.enable != 0;

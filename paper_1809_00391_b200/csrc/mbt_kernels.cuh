@@ -113,6 +113,12 @@ __host__ __device__ inline size_t pass_smem_bytes(int nb, int npair) {
          128 * sizeof(LogTabEntry) + 16;
 }
 
+// ---- programmatic dependent launch (PTX griddepcontrol; no-ops in a kernel launched without the attribute).  The pass and
+// k_wake of a turn are launched as a chain of programmatic dependents: a kernel may become resident while its
+// predecessor is still running, does what does not depend on it, and waits before it touches the predecessor's output.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- mbarrier / bulk-copy primitives (PTX; SASS: SYNCS / UBLKCP)
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -185,8 +191,6 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
 
   const int tid = threadIdx.x;
   const int lane = tid & 31;
-  const uint32_t n = A.ctrl->turn + 1u;  // the turn this pass tracks (Philox counter word, D24)
-  const bool have_kick = A.ctrl->kick_pending != 0u;
   const int nb = A.nb;
   const uint32_t hi_nb = (uint32_t)__double2hiint(A.nb_d);
   if (tid < kStages) {
@@ -207,10 +211,6 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
     const uint32_t p0 = blockIdx.x * A.tile_pairs;
     const uint32_t p1 = (A.ppb - p0 < A.tile_pairs) ? A.ppb : p0 + A.tile_pairs;
 
-    // window of the wake being applied (S0) and window this pass bins with (S4); the flush pass re-bins on the former
-    const double lo_old = A.lo_hist[b];
-    const double lo_new = MAP ? A.lo_next[b] : lo_old;
-
     // chunk k of the tile = pairs [p0 + k STRIDE, + STRIDE) clipped to p1; it lives in stage k % kStages
     const uint32_t n_it = (p1 - p0 + STRIDE - 1u) / STRIDE;
     const double2 *gT = reinterpret_cast<const double2 *>(A.tau + (size_t)b * A.ld);
@@ -227,6 +227,17 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
     };
     if (tid == 0)
       for (uint32_t k = 0; k + 1u < (uint32_t)kStages && k < n_it; ++k) issue(k);
+
+    // Everything above is independent of the wake kernel before this pass (barriers, log table, the first particle
+    // stages: the particles were last written by the pass before it, which that wake kernel waited for); its output --
+    // the control words, the gather cells, the phasors, the windows -- is read from here on.
+    griddep_launch_dependents();  // the wake kernel after this pass may become resident; it waits for this grid itself
+    griddep_wait();
+    const uint32_t n = A.ctrl->turn + 1u;  // the turn this pass tracks (Philox counter word, D24)
+    const bool have_kick = A.ctrl->kick_pending != 0u;
+    // window of the wake being applied (S0) and window this pass bins with (S4); the flush pass re-bins on the former
+    const double lo_old = A.lo_hist[b];
+    const double lo_new = MAP ? A.lo_next[b] : lo_old;
 
     // stage the gather cells of bunch b's wake: cellSR + sum_r Re[cellF_r P[b][r]] (S6 expansion); clear the counts
     for (int k = tid; k < nb + 2; k += kPassThreads) {
@@ -531,6 +542,8 @@ __global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ W
   const int b = blockIdx.x;
   const int split = blockIdx.y, S = A.S;  // few bunches: S CTAs share a bunch (split 0 also does the per-bunch work)
   const int nb = A.nb;
+  griddep_wait();               // the pass of this turn is complete (counts, moment sums)
+  griddep_launch_dependents();  // the next pass may become resident: it stages what does not depend on this kernel
   const uint32_t n_done = A.ctrl->turn;  // completed turns; the turn being closed is n_done + 1
   const uint32_t n = n_done + 1u;
 
