@@ -72,7 +72,9 @@ class ClockSampler:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
                                           "--format=csv,noheader,nounits", "-lms", "25"],
                                          stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
-            time.sleep(0.3)
+            t_end = time.time() + 5.0          # nvidia-smi needs a moment before its first line: wait for it, so that
+            while time.time() < t_end and os.path.getsize(self.path) == 0:   # the samples fall inside the timed region
+                time.sleep(0.02)
         except Exception:
             self.proc = None
 
