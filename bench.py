@@ -208,6 +208,7 @@ def run_mbt(args):
     barrier()
     sec = trk.last_track_seconds()
     launches = trk.launch_count - l0
+    clocks = sampler.stop() if rank == 0 else None   # sampled during the timed region only
     if world > 1:
         t = torch.tensor([sec], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -221,7 +222,6 @@ def run_mbt(args):
     time.sleep(pause_s)
     pass_s, wake_s = trk.track_profiled(min(K, 2000))
     kp = min(K, 2000)
-    clocks = sampler.stop() if rank == 0 else None   # sampled over both timed regions (graph run, per-kernel run)
     peak, peak_src = _peaks()
     achieved = bytes_pt * n_part / (pass_s / kp) / 1e9
     roofline = {"bound": "hbm", "kernel": "k_pass6<true>" if args.transverse else "k_pass<true>", "achieved": achieved,
