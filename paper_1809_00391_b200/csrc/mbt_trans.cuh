@@ -4,8 +4,11 @@
 //   k_pass6    one pass over the 6-D SoA store (96 B per particle-turn): both kicks of turn n-1, the longitudinal
 //              map and the betatron map / excitation of turn n, counts and dipole sums of turn n
 //   k_wake     longitudinal wake of turn n                                        (mbt_kernels.cuh, unchanged)
-//   k_wake_tr  per bunch: K[j] = sum_{k<j} (Q_b/N_p) S[k] W_perp((j-k) Delta) for both planes, gather cells
+//   k_wake_tr  per bunch: K[j] = sum_{k<j} (Q_b/N_p) S[k] W_perp((j-k) Delta) for both planes, gather cells, bunch
+//              centroids (per-turn log; source ring of the resistive wall), scale of the next turn's dipole sums
+//   k_rw       long-range resistive-wall kick per bunch (readings W1..W5), if enabled
 //
+// k_wake_tr and k_rw run on a side stream beside k_wake (they read only what the pass wrote; the next pass joins both),
 // and, like the longitudinal kick, the transverse kick of the last tracked turn stays pending until the next pass or
 // a getter's flush pass (k_pass6<false>) applies it.
 #pragma once
