@@ -777,8 +777,9 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
       destroy(h);
       return fail(MBT_EINVAL, buf);
     }
-    // three stages in flight if two CTAs then still fit an SM, else two
-    T.stages = (2 * (pass6_smem_bytes(nb, 3) + 1024) <= (size_t)prop.sharedMemPerMultiprocessor) ? 3 : 2;
+    // two stages (48 KB) in flight per CTA: three measured the same to 1 % (c4 0.839 vs 0.834 ms, c5 2.41 vs 2.37), four
+    // cost a CTA per SM
+    T.stages = 2;
     if (const char *e = getenv("MBT_STAGES6")) T.stages = std::min(kMaxStages6, std::max(2, atoi(e)));  // measurement knob
     h->smem_pass6 = pass6_smem_bytes(nb, T.stages);
     CUH(cudaFuncSetAttribute((const void *)h->fn_map6, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass6));
