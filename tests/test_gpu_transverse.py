@@ -316,6 +316,26 @@ def test_transverse_full_size_c4(mbt, orc):
         assert np.all(t2.histogram().sum(axis=1) == m[:, 0]) and np.all(m[:, 0] + m[:, 1] == cfg["fill"]["n_per_bunch"])
 
 
+def test_many_particles_per_bunch_fewer_fixed_point_bits(mbt, orc):
+    """N_p > 2^18 per bunch: the fixed-point dipole sums give up bits so that N_p 2^bits stays below 2^62 (here 43,
+    and 41 for the million-particle bunch of c2); sums, kicks and coordinates keep their tolerances."""
+    cfg = _cfg(m=1, n_per_bunch=300_001, n_bins=64)
+    o = orc.Oracle(cfg)
+    x, xp, y, yp = o.transverse_particles()
+    o.set_transverse(x + 2.0e-4, xp, y - 1.0e-5, yp)
+    o.track(1)
+    with mbt.Tracker(cfg) as t:
+        r = assert_transverse_turn_parity(o, t, cfg)
+        print(r)
+    cfg = W.config("c2")
+    cfg["transverse"] = W.transverse_planes()
+    o = orc.Oracle(cfg)
+    o.track(1)
+    with mbt.Tracker(cfg) as t:
+        r = assert_transverse_turn_parity(o, t, cfg)
+        print(r)
+
+
 def test_three_cavities_and_lost_particles(mbt, orc):
     """The generic cavity loop (more than two cavities) of both passes, and particles far off the bucket (the
     large-argument branch of the RF sine, |phase| >= 2^16 rad) in the 6-D pass; NaN offsets stay NaN and do not crash."""
