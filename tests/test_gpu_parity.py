@@ -151,6 +151,30 @@ def test_ragged_sizes_both_kernel_variants(mbt, orc, npair, n_per_bunch, monkeyp
             assert_single_turn_parity(o, t, cfg)
 
 
+@pytest.mark.parametrize("n_per_bunch", [3 * 1024 + 1, 7 * 1024 - 3, 6 * 1024, 5000])
+def test_multi_iteration_tiles_with_ragged_ends(mbt, orc, n_per_bunch, monkeypatch):
+    """Tiles of three iterations forced (MBT_TILE_ITERS, the library's measurement knob; small workloads otherwise get
+    one-iteration tiles): full tiles, a last tile with fewer iterations and a last chunk that is partly filled, in both
+    pass variants and in the 6-D pass."""
+    monkeypatch.setenv("MBT_TILE_ITERS", "3")
+    for npair in (1, 2):
+        monkeypatch.setenv("MBT_NPAIR", str(npair))
+        cfg = W.tiny(m=2, n_per_bunch=n_per_bunch, n_bins=16)
+        o = orc.Oracle(cfg)
+        o.track(2)
+        with mbt.Tracker(cfg) as t:
+            assert_single_turn_parity(o, t, cfg)
+    cfg = W.tiny(m=2, n_per_bunch=n_per_bunch, n_bins=16)
+    cfg["transverse"] = W.transverse_planes()
+    o = orc.Oracle(cfg)
+    o.track(2)
+    with mbt.Tracker(cfg) as t:
+        t.set_transverse(*o.transverse_particles())
+        assert_single_turn_parity(o, t, cfg)
+        for g, c in zip(t.transverse_particles(), o.transverse_particles()):
+            assert particle_errors(g, c) <= TOL_PARTICLE
+
+
 def test_user_sampled_wake_table(mbt, orc):
     """A user-sampled short-range table (resistive + inductive + power law) beside the
     resonators: same parity bar as the resonator-only wake."""
