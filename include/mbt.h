@@ -196,6 +196,11 @@ int mbt_moments_transverse(mbt_handle *h, double *out);
 int64_t mbt_turn(const mbt_handle *h);        /* completed turns, -1 on NULL                 */
 double mbt_phi_s(const mbt_handle *h);        /* synchronous phase of cav[0] [rad]           */
 int64_t mbt_particle_stride(int64_t n_per_bunch); /* ld of the device arrays                 */
+/* The tiling a pass would get (host logic only, no device needed): a bunch of pairs_per_bunch particle pairs, CTAs that
+ * advance `stride` pairs per iteration, M bunches, `slots` CTAs resident on the device at once.  Even tiles (the last
+ * at least 3/4 of the others) and, among those, the count that minimises ceil(w)/w (1 + 1/iterations), w = tiles M /
+ * slots.  Writes pairs per tile and tiles per bunch; MBT_EINVAL on non-positive arguments. */
+int mbt_plan_tiles(int64_t pairs_per_bunch, int64_t stride, int32_t M, int32_t slots, uint32_t *tile_pairs, int32_t *tiles);
 /* DEVICE pointers of the particle store (for zero-copy wrapping, e.g. torch.from_blob-like views) */
 int mbt_device_pointers(mbt_handle *h, void **d_tau, void **d_delta, int64_t *ld);
 /* kernels launched by this handle so far (bench.py's gpu_launches) */

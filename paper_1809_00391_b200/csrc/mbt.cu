@@ -364,6 +364,13 @@ extern "C" {
 const char *mbt_last_error(void) { return g_err.c_str(); }
 const char *mbt_version(void) { return "mbt-b200 0.1 (sm_100a)"; }
 int64_t mbt_particle_stride(int64_t n) { return n < 0 ? -1 : (n + 3) / 4 * 4; }
+int mbt_plan_tiles(int64_t ppb, int64_t stride, int32_t M, int32_t slots, uint32_t *tile_pairs, int32_t *tiles) {
+  if (ppb < 1 || stride < 1 || M < 1 || slots < 1 || !tile_pairs || !tiles) return fail(MBT_EINVAL, "bad argument");
+  int n = 0;
+  choose_tiles(ppb, stride, M, slots, tile_pairs, &n);
+  *tiles = n;
+  return 0;
+}
 int64_t mbt_turn(const mbt_handle *h) { return h ? h->turn : -1; }
 double mbt_phi_s(const mbt_handle *h) { return h ? h->phi_s : NAN; }
 int64_t mbt_launch_count(const mbt_handle *h) { return h ? h->launches : -1; }

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libmbt.so")
 SYMBOLS = [
     "mbt_create", "mbt_track", "mbt_moments", "mbt_destroy", "mbt_get_particles", "mbt_set_particles",
     "mbt_get_histogram", "mbt_get_wake", "mbt_get_moment_log", "mbt_get_lr_history", "mbt_set_lr_history", "mbt_get_window", "mbt_set_window",
-    "mbt_turn", "mbt_phi_s", "mbt_particle_stride", "mbt_device_pointers", "mbt_launch_count",
+    "mbt_turn", "mbt_phi_s", "mbt_particle_stride", "mbt_plan_tiles", "mbt_device_pointers", "mbt_launch_count",
     "mbt_get_transverse", "mbt_set_transverse", "mbt_get_dipole", "mbt_get_transverse_wake", "mbt_moments_transverse",
     "mbt_get_rw_kick", "mbt_get_rw_history", "mbt_set_rw_history", "mbt_get_transverse_log",
     "mbt_last_track_seconds", "mbt_track_profiled", "mbt_philox_selftest", "mbt_normal_selftest", "mbt_last_error", "mbt_version",
@@ -108,6 +108,7 @@ def lib():
         L.mbt_phi_s.restype = C.c_double
         L.mbt_particle_stride.argtypes = [C.c_int64]
         L.mbt_particle_stride.restype = C.c_int64
+        L.mbt_plan_tiles.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.c_int32, C.POINTER(C.c_uint32), C.POINTER(C.c_int32)]
         L.mbt_device_pointers.argtypes = [H, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
         L.mbt_launch_count.argtypes = [H]
         L.mbt_launch_count.restype = C.c_int64
@@ -144,6 +145,13 @@ def _ck(rc):
 
 def particle_stride(n_per_bunch: int) -> int:
     return int(lib().mbt_particle_stride(int(n_per_bunch)))
+
+
+def plan_tiles(pairs_per_bunch, stride, n_bunches, slots):
+    """(pairs per tile, tiles per bunch) a pass would get (host logic, no device needed)."""
+    tp, nt = C.c_uint32(), C.c_int32()
+    _ck(lib().mbt_plan_tiles(int(pairs_per_bunch), int(stride), int(n_bunches), int(slots), C.byref(tp), C.byref(nt)))
+    return tp.value, nt.value
 
 
 def philox_selftest(ctr, key):

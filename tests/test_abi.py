@@ -102,3 +102,34 @@ def test_workloads_match_baseline_configs():
     assert len(W.config("c5")["cavities"]) == 2 and len(W.config("c5")["wake"]["resonators"]) == 4
     # seeded: two calls give identical inputs
     assert W.config("c4") == W.config("c4")
+
+
+def test_pass_tiling_host_logic(monkeypatch):
+    """mbt_plan_tiles (no device needed): the tilings of the BASELINE workloads on a B200 (148 SMs x 2 or 3 resident CTAs)
+    and the properties every tiling has: it covers the bunch, tiles are whole iterations, the last tile is at least
+    3/4 of the others."""
+    from paper_1809_00391_b200 import build, mbt
+    build.build()
+    monkeypatch.delenv("MBT_TILE_ITERS", raising=False)
+    assert mbt.plan_tiles(50_000, 512, 363, 296) == (25 * 512, 4)          # c4, k_pass two pairs per thread: 4.9 waves
+    assert mbt.plan_tiles(100_000, 512, 484, 296) == (66 * 512, 3)         # c5
+    assert mbt.plan_tiles(50_000, 256, 363, 296) == (49 * 256, 4)          # c4, k_pass6
+    assert mbt.plan_tiles(500_000, 256, 1, 444) == (5 * 256, 391)          # c2: just under one wave
+    assert mbt.plan_tiles(5_000, 512, 1, 296) == (512, 10)                 # c1: one iteration per CTA
+    import random
+    rng = random.Random(3)
+    for _ in range(300):
+        ppb = rng.randint(1, 400_000)
+        stride = rng.choice([256, 512])
+        m = rng.choice([1, 2, 3, 22, 121, 363, 484, 1000])
+        slots = rng.choice([148, 296, 444])
+        tp, nt = mbt.plan_tiles(ppb, stride, m, slots)
+        assert tp % stride == 0 and tp > 0 and nt >= 1
+        assert nt * tp >= ppb > (nt - 1) * tp                                # covers the bunch, no empty tile
+        it = tp // stride
+        last = -(-(ppb - (nt - 1) * tp) // stride)
+        assert nt == 1 or 4 * last >= 3 * it
+    monkeypatch.setenv("MBT_TILE_ITERS", "16")
+    assert mbt.plan_tiles(50_000, 512, 363, 296) == (16 * 512, 7)           # the measurement knob
+    with pytest.raises(mbt.MbtError):
+        mbt.plan_tiles(0, 512, 1, 296)
