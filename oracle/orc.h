@@ -82,6 +82,9 @@ int orc_get_particles(orc_handle *h, double *tau, double *delta);
 int orc_set_particles(orc_handle *h, const double *tau, const double *delta, int64_t turn);
 int orc_get_histogram(orc_handle *h, uint32_t *out /* [M][n_bins] */);
 int orc_get_wake(orc_handle *h, double *total, double *sr_only, double *lr_only /* each [M][n_bins] or NULL */);
+/* steps 5, 6 of the turn just completed for OTHER counts hist[M][n_bins] of that turn (history of the turns before as
+ * held by the handle; the handle is not changed); with the oracle's own counts: orc_get_wake()'s tables bit for bit */
+int orc_wake_from_counts(orc_handle *h, const uint32_t *hist, double *total, double *sr_only, double *lr_only);
 int orc_get_moment_log(orc_handle *h, int64_t first_turn, int64_t n, double *out /* [n][M][6] */);
 /* source phasors a[b][n'][r] of the last K turns, oldest first: [K][M][R_lr][2] (re, im) */
 int orc_get_lr_history(orc_handle *h, double *out);

@@ -95,6 +95,7 @@ def lib():
         L.orc_set_particles.argtypes = [H, dp, dp, C.c_int64]
         L.orc_get_histogram.argtypes = [H, C.POINTER(C.c_uint32)]
         L.orc_get_wake.argtypes = [H, dp, dp, dp]
+        L.orc_wake_from_counts.argtypes = [H, C.POINTER(C.c_uint32), dp, dp, dp]
         L.orc_get_moment_log.argtypes = [H, C.c_int64, C.c_int64, dp]
         L.orc_get_lr_history.argtypes = [H, dp]
         L.orc_set_lr_history.argtypes = [H, dp]
@@ -292,6 +293,16 @@ class Oracle:
         sr = np.empty_like(tot)
         lr = np.empty_like(tot)
         self._ck(self._L.orc_get_wake(self._h, _dp(tot), _dp(sr), _dp(lr)))
+        return tot, sr, lr
+
+    def wake_from_counts(self, hist):
+        """(total, sr, lr) of the turn just completed for other counts of that turn (steps 5, 6; state unchanged)."""
+        hist = np.ascontiguousarray(hist, dtype=np.uint32)
+        assert hist.shape == (self.M, self.nb)
+        tot = np.empty((self.M, self.nb))
+        sr = np.empty_like(tot)
+        lr = np.empty_like(tot)
+        self._ck(self._L.orc_wake_from_counts(self._h, hist.ctypes.data_as(C.POINTER(C.c_uint32)), _dp(tot), _dp(sr), _dp(lr)))
         return tot, sr, lr
 
     def moment_log(self, first_turn, n):

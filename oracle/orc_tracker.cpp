@@ -358,8 +358,89 @@ void bin_all(orc_handle *h) {
     }
 }
 
-void one_turn(orc_handle *h) {
+// steps 5 and 6 of turn n for the counts `hist` [M][nb] (on the windows s_hist): V_SR and V_LR on the bins.
+// commit = true (the tracked turn): the source phasors of the counts enter the history ring (and, lr_mode 1, the
+// per-turn aggregate); commit = false (orc_wake_from_counts): the handle is left untouched.
+void build_wake(orc_handle *h, int64_t n, const uint32_t *hist, bool commit, double *Vsr, double *Vlr) {
   const int M = h->M, nb = h->nb, R = h->R(), K = h->K;
+  const int64_t Np = h->Np;
+  // 5: short-range wake, V_SR[b][j] = sum_{k<=j} w[j-k] q[b][k], q = (Q_b/N_p) hist
+  std::vector<double> q((size_t)nb);
+  for (int b = 0; b < M; ++b) {
+    double qm = h->charge[b] / (double)Np;
+    for (int k = 0; k < nb; ++k) q[k] = qm * (double)hist[(size_t)b * nb + k];
+    double *Vs = &Vsr[(size_t)b * nb];
+    if (h->have_sr)
+      orc_sr_convolve(nb, h->w.data(), q.data(), Vs);
+    else
+      for (int j = 0; j < nb; ++j) Vs[j] = 0.0;
+  }
+  // 6: long-range resonator wake
+  std::fill(Vlr, Vlr + (size_t)M * nb, 0.0);
+  if (R > 0) {
+    // source phasors a[b][n][r] = sum_k q[b][k] exp(-lambda_r c_k)
+    std::vector<cplx> a_n((size_t)M * R);
+    for (int b = 0; b < M; ++b) {
+      double qm = h->charge[b] / (double)Np;
+      for (int r = 0; r < R; ++r) {
+        const Resonator &rs = h->res_lr[r];
+        cplx lam(-rs.alpha, rs.wbar);
+        cplx a(0.0, 0.0);
+        for (int k = 0; k < nb; ++k) {
+          double qk = qm * (double)hist[(size_t)b * nb + k];
+          a += qk * std::exp(-lam * bin_centre(h, h->s_hist[b], k));
+        }
+        a_n[(size_t)b * R + r] = a;
+        if (commit) h->a_at(n, b, r) = a;
+      }
+    }
+    std::vector<cplx> P((size_t)M * R, cplx(0, 0));
+    if (h->lr_mode == 0) {
+      // THE definition: pairwise sum over H(b,n)
+      for (int b = 0; b < M; ++b)
+        for (int r = 0; r < R; ++r) {
+          const Resonator &rs = h->res_lr[r];
+          cplx acc(0, 0);
+          int64_t first = (n - K > 1) ? (n - K) : 1;
+          for (int64_t np = first; np <= n - 1; ++np)
+            for (int bp = 0; bp < M; ++bp)
+              acc += h->a_at(np, bp, r) * exp_lambda(rs, dt_between(h, n - np, h->bucket[b] - h->bucket[bp]));
+          for (int bp = 0; bp < M; ++bp)
+            if (h->bucket[bp] < h->bucket[b])
+              acc += a_n[(size_t)bp * R + r] * exp_lambda(rs, dt_between(h, 0, h->bucket[b] - h->bucket[bp]));
+          P[(size_t)b * R + r] = acc;
+        }
+    } else {
+      // equivalent O(M+K) form (DESIGN.md "LR recurrence"); only decaying factors occur
+      for (int r = 0; r < R; ++r) {
+        cplx G(0, 0);
+        for (int k = 1; k <= K && n - k >= 1; ++k)
+          G += h->ring_A[(size_t)((n - k) % (K + 1)) * R + r] * h->g_hist[(size_t)(k - 1) * R + r];
+        cplx Pj = G, own(0, 0);
+        for (int j = 0; j < M; ++j) {
+          P[(size_t)j * R + r] = Pj;
+          own += a_n[(size_t)j * R + r] * h->g_tail[(size_t)j * R + r];
+          if (j + 1 < M) Pj = (Pj + a_n[(size_t)j * R + r]) * h->g_step[(size_t)j * R + r];
+        }
+        if (commit) h->ring_A[(size_t)(n % (K + 1)) * R + r] = own;
+      }
+    }
+    // V_LR[b][j] = sum_r Re[C_r exp(lambda_r c_j) P[b][r]]
+    for (int b = 0; b < M; ++b)
+      for (int j = 0; j < nb; ++j) {
+        double v = 0.0;
+        for (int r = 0; r < R; ++r) {
+          const Resonator &rs = h->res_lr[r];
+          cplx lam(-rs.alpha, rs.wbar);
+          v += std::real(rs.C * std::exp(lam * bin_centre(h, h->s_hist[b], j)) * P[(size_t)b * R + r]);
+        }
+        Vlr[(size_t)b * nb + j] = v;
+      }
+  }
+}
+
+void one_turn(orc_handle *h) {
+  const int M = h->M, nb = h->nb;
   const int64_t Np = h->Np;
   const int64_t n = h->turn + 1;
   // 1-3: single-particle map
@@ -405,77 +486,8 @@ void one_turn(orc_handle *h) {
       if (s < -(int64_t)h->s_max) s = -(int64_t)h->s_max;
       h->s_next[b] = (int32_t)s;
     }
-  // 5: short-range wake, V_SR[b][j] = sum_{k<=j} w[j-k] q[b][k], q = (Q_b/N_p) hist
-  std::vector<double> q((size_t)nb);
-  for (int b = 0; b < M; ++b) {
-    double qm = h->charge[b] / (double)Np;
-    for (int k = 0; k < nb; ++k) q[k] = qm * (double)h->hist[(size_t)b * nb + k];
-    double *Vs = &h->Vsr[(size_t)b * nb];
-    if (h->have_sr)
-      orc_sr_convolve(nb, h->w.data(), q.data(), Vs);
-    else
-      for (int j = 0; j < nb; ++j) Vs[j] = 0.0;
-  }
-  // 6: long-range resonator wake
-  std::fill(h->Vlr.begin(), h->Vlr.end(), 0.0);
-  if (R > 0) {
-    // source phasors a[b][n][r] = sum_k q[b][k] exp(-lambda_r c_k)
-    for (int b = 0; b < M; ++b) {
-      double qm = h->charge[b] / (double)Np;
-      for (int r = 0; r < R; ++r) {
-        const Resonator &rs = h->res_lr[r];
-        cplx lam(-rs.alpha, rs.wbar);
-        cplx a(0.0, 0.0);
-        for (int k = 0; k < nb; ++k) {
-          double qk = qm * (double)h->hist[(size_t)b * nb + k];
-          a += qk * std::exp(-lam * bin_centre(h, h->s_hist[b], k));
-        }
-        h->a_at(n, b, r) = a;
-      }
-    }
-    std::vector<cplx> P((size_t)M * R, cplx(0, 0));
-    if (h->lr_mode == 0) {
-      // THE definition: pairwise sum over H(b,n)
-      for (int b = 0; b < M; ++b)
-        for (int r = 0; r < R; ++r) {
-          const Resonator &rs = h->res_lr[r];
-          cplx acc(0, 0);
-          int64_t first = (n - K > 1) ? (n - K) : 1;
-          for (int64_t np = first; np <= n - 1; ++np)
-            for (int bp = 0; bp < M; ++bp)
-              acc += h->a_at(np, bp, r) * exp_lambda(rs, dt_between(h, n - np, h->bucket[b] - h->bucket[bp]));
-          for (int bp = 0; bp < M; ++bp)
-            if (h->bucket[bp] < h->bucket[b])
-              acc += h->a_at(n, bp, r) * exp_lambda(rs, dt_between(h, 0, h->bucket[b] - h->bucket[bp]));
-          P[(size_t)b * R + r] = acc;
-        }
-    } else {
-      // equivalent O(M+K) form (DESIGN.md "LR recurrence"); only decaying factors occur
-      for (int r = 0; r < R; ++r) {
-        cplx G(0, 0);
-        for (int k = 1; k <= K && n - k >= 1; ++k)
-          G += h->ring_A[(size_t)((n - k) % (K + 1)) * R + r] * h->g_hist[(size_t)(k - 1) * R + r];
-        cplx Pj = G, own(0, 0);
-        for (int j = 0; j < M; ++j) {
-          P[(size_t)j * R + r] = Pj;
-          own += h->a_at(n, j, r) * h->g_tail[(size_t)j * R + r];
-          if (j + 1 < M) Pj = (Pj + h->a_at(n, j, r)) * h->g_step[(size_t)j * R + r];
-        }
-        h->ring_A[(size_t)(n % (K + 1)) * R + r] = own;
-      }
-    }
-    // V_LR[b][j] = sum_r Re[C_r exp(lambda_r c_j) P[b][r]]
-    for (int b = 0; b < M; ++b)
-      for (int j = 0; j < nb; ++j) {
-        double v = 0.0;
-        for (int r = 0; r < R; ++r) {
-          const Resonator &rs = h->res_lr[r];
-          cplx lam(-rs.alpha, rs.wbar);
-          v += std::real(rs.C * std::exp(lam * bin_centre(h, h->s_hist[b], j)) * P[(size_t)b * R + r]);
-        }
-        h->Vlr[(size_t)b * nb + j] = v;
-      }
-  }
+  // 5, 6: wake potentials of this turn's counts (build_wake above); the source phasors enter the history ring
+  build_wake(h, n, h->hist.data(), true, h->Vsr.data(), h->Vlr.data());
   for (size_t x = 0; x < h->V.size(); ++x) h->V[x] = h->Vsr[x] + h->Vlr[x];
   // 7: wake kick on in-window particles, delta -= v/E0 (reading D9)
   for (int b = 0; b < M; ++b) {
@@ -949,6 +961,25 @@ int orc_get_wake(orc_handle *h, double *total, double *sr, double *lr) {
   if (total) std::memcpy(total, h->V.data(), bytes);
   if (sr) std::memcpy(sr, h->Vsr.data(), bytes);
   if (lr) std::memcpy(lr, h->Vlr.data(), bytes);
+  return 0;
+}
+
+// Steps 5 and 6 of the turn just completed, evaluated for OTHER counts of that turn (hist[M][n_bins], on the current
+// windows) with the history the handle holds for the turns before; nothing in the handle changes.  With the oracle's
+// own counts it returns orc_get_wake()'s tables bit for bit (same code path, build_wake).  The parity tests use it when
+// the CUDA path's counts differ from the oracle's by edge-adjacent particles (north_star (ii)): the wake is then
+// compared on the CUDA path's own counts instead of being skipped.
+int orc_wake_from_counts(orc_handle *h, const uint32_t *hist, double *total, double *sr, double *lr) {
+  if (!h || !hist) return fail(ORC_EINVAL, "null argument");
+  if (h->turn < 1) return fail(ORC_ESTATE, "no tracked turn");
+  const size_t n = (size_t)h->M * h->nb;
+  std::vector<double> vs(n), vl(n);
+  build_wake(h, h->turn, hist, false, vs.data(), vl.data());
+  for (size_t x = 0; x < n; ++x) {
+    if (total) total[x] = vs[x] + vl[x];
+    if (sr) sr[x] = vs[x];
+    if (lr) lr[x] = vl[x];
+  }
   return 0;
 }
 

@@ -239,6 +239,46 @@ def test_pin_e_lr_wake_against_pairwise_brute_force(orc, lr_mode):
         assert np.allclose(vlr, want, rtol=0, atol=1e-10 * scale)
 
 
+@pytest.mark.parametrize("lr_mode", [0, 1])
+def test_wake_from_counts_own_counts_bit_equal_other_counts_brute_force(orc, lr_mode):
+    """orc_wake_from_counts (steps 5, 6 for other counts of the turn just completed): with the oracle's own counts it
+    is orc_get_wake bit for bit and leaves the state alone; with counts moved between bins it equals the written-out
+    short-range sum and the physical pairwise long-range sum (no phasors) of those counts."""
+    cfg = W.tiny(m=5, n_per_bunch=37, n_bins=8, k_hist=3, n_lr=2)
+    o = orc.Oracle(cfg, lr_mode=lr_mode)
+    lr_res = [r for r in cfg["wake"]["resonators"] if r["flags"] & W.FLAG_LR]
+    sr_res = [r for r in cfg["wake"]["resonators"] if r["flags"] & W.FLAG_SR]
+    wk = cfg["wake"]
+    nb = wk["n_bins"]
+    d = (wk["tau_hi_s"] - wk["tau_lo_s"]) / nb
+    w = np.array([sum(orc.resonator_wake(r["Rs_ohm"], r["fr_Hz"], r["Q"], k * d) for r in sr_res) for k in range(nb)])
+    hists = {}
+    for n in range(1, 7):
+        o.track(1)
+        hists[n] = o.histogram()
+        before = [x.copy() for x in o.wake()] + [o.lr_history().copy()]
+        same = o.wake_from_counts(hists[n])
+        for a, b in zip(same, before[:3]):
+            assert np.array_equal(a, b)
+        # move one particle of every bunch to the neighbouring bin (what an edge-adjacent particle does)
+        other = hists[n].copy()
+        for b in range(other.shape[0]):
+            k = int(np.argmax(other[b]))
+            other[b, k] -= 1
+            other[b, (k + 1) % nb] += 1
+        tot, sr, lr = o.wake_from_counts(other)
+        q = np.array(cfg["fill"]["charge_C"])[:, None] / cfg["fill"]["n_per_bunch"] * other
+        want_sr = np.array([[sum(w[j - k] * q[b, k] for k in range(j + 1)) for j in range(nb)] for b in range(len(q))])
+        assert np.allclose(sr, want_sr, rtol=1e-13, atol=0)
+        want_lr = _lr_brute_force(orc, cfg, {**hists, n: other}, n, lr_res)
+        assert np.allclose(lr, want_lr, rtol=0, atol=1e-10 * np.abs(want_lr).max())
+        assert np.array_equal(tot, sr + lr)
+        assert not np.array_equal(lr[1:], before[2][1:]) and not np.array_equal(sr, before[1])
+        after = [x.copy() for x in o.wake()] + [o.lr_history().copy()]
+        for a, b in zip(after, before):
+            assert np.array_equal(a, b)                       # the handle is unchanged
+
+
 def test_lr_recurrence_equals_definition_long_history(orc):
     cfg = W.tiny(m=5, n_per_bunch=101, n_bins=16, k_hist=6, n_lr=3, harmonic=True)
     a = orc.Oracle(cfg, lr_mode=0)
