@@ -141,7 +141,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": "particle-turns/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": _workload_name(args), "l2": "n/a (CPU)"},
+        "config": _config_keys(args, 1),
         "cpu_baseline": {"value": val, "unit": "particle-turns/s", "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": "particle-turns/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -153,6 +153,15 @@ def run_reference(args):
 def W_np(name):
     from paper_1809_00391_b200 import workloads as W
     return W.config(name)["fill"]["n_per_bunch"]
+
+
+def _config_keys(args, world):
+    """`config` of the JSON line: the same keys and values in both arms (they describe the workload, not the arm)."""
+    from paper_1809_00391_b200 import workloads as W
+    state = (BYTES_PER_PARTICLE_TURN_6D if args.transverse else BYTES_PER_PARTICLE_TURN) / 2 * W.n_particles(W.config(args.config))
+    return {"workload": _workload_name(args), "parallelism": "replicas x%d" % world,
+            "l2": "particle store larger than L2, no flush needed" if state > 126e6 else
+                  "particle store fits L2 (latency-bound config, not an HBM roofline)"}
 
 
 def _workload_name(args):
@@ -196,7 +205,9 @@ def run_mbt(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    trk = mbt.Tracker(cfg, log_capacity_turns=0, device=local)
+    tuning = {k: v for k, v in (("turn_mode", args.turn_mode), ("tile_iters", args.tile_iters),
+                                ("pairs_per_thread", args.pairs_per_thread), ("pdl", args.pdl), ("verbose", args.verbose)) if v}
+    trk = mbt.Tracker(cfg, log_capacity_turns=0, device=local, tuning=tuning)
     trk.track(Wm)
     trk.moments()
     sampler = ClockSampler(local)
@@ -224,9 +235,11 @@ def run_mbt(args):
     kp = min(K, 2000)
     peak, peak_src = _peaks()
     achieved = bytes_pt * n_part / (pass_s / kp) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_pass6<true>" if args.transverse else "k_pass<true>", "achieved": achieved,
-                "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+    one_launch = trk.launches_per_turn == 1
+    roofline = {"bound": "hbm", "kernel": "k_pass6<true>" if args.transverse else
+                ("k_pass<true> (one launch per turn: pass + wake of the bunches it completes)" if one_launch else "k_pass<true>"),
+                "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "traffic_source": None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": bytes_pt * n_part,
                 "pass_ms": pass_s / kp * 1e3, "wake_ms": wake_s / kp * 1e3,
                 "pass_share_of_step": pass_s / (pass_s + wake_s),
@@ -238,8 +251,37 @@ def run_mbt(args):
             for ln in f:
                 if ln.startswith("dram_bytes_per_launch"):
                     roofline["traffic"] = float(ln.split()[1])
+                    roofline["traffic_source"] = ("profiles/%s: dram__bytes_read.sum + dram__bytes_write.sum of one launch from the "
+                                                  "committed `ncu --set full` capture named there (not measured in this run)" %
+                                                  os.path.basename(f.name))
     except Exception:
         pass
+
+    # the sustained state: the config's full number of turns (what a real run sees: after ~0.1 s of this load the board
+    # sits at its power cap), bounded in wall time; then, without a pause, the per-kernel timing in that same state
+    sustained = None
+    if args.sustained:
+        T = int(min(cfg["n_turns"], max(K, args.sustained_seconds / (sec / K))))
+        samp2 = ClockSampler(local)
+        if rank == 0:
+            samp2.start()
+        barrier()
+        trk.track(T)
+        barrier()
+        sec_s = trk.last_track_seconds()
+        kp2 = min(T, 1000)
+        pass_s2, wake_s2 = trk.track_profiled(kp2)
+        clocks2 = samp2.stop() if rank == 0 else None
+        if world > 1:
+            t = torch.tensor([sec_s], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            sec_s = float(t.item())
+        sustained = {"steps": T, "value": world * n_part * T / sec_s, "ms_per_step": sec_s / T * 1e3,
+                     "pass_ms": pass_s2 / kp2 * 1e3, "wake_ms": wake_s2 / kp2 * 1e3,
+                     "frac": bytes_pt * n_part / (pass_s2 / kp2) / 1e9 / peak,
+                     "whole_step_frac": bytes_pt * n_part / (sec_s / T) / 1e9 / peak, "clocks": clocks2,
+                     "what": "mbt_track(%d) of the config's %d turns, graph replay, CUDA events; then %d event-bracketed turns "
+                             "with no pause (pass_ms, frac: the dominant kernel in the power-capped state)" % (T, cfg["n_turns"], kp2)}
     trk.close()
 
     # end to end through the C ABI with HOST buffers: upload the particle state from pinned host memory, track K
@@ -249,7 +291,7 @@ def run_mbt(args):
         ld = n_part // len(cfg["fill"]["buckets"])
         h_tau = torch.empty(n_part, dtype=torch.float64).pin_memory()
         h_delta = torch.empty(n_part, dtype=torch.float64).pin_memory()
-        t2 = mbt.Tracker(cfg, log_capacity_turns=K, device=local)
+        t2 = mbt.Tracker(cfg, log_capacity_turns=K, device=local, tuning=tuning)
         tau0, delta0 = t2.particles(h_tau.numpy().reshape(len(cfg["fill"]["buckets"]), ld),
                                     h_delta.numpy().reshape(len(cfg["fill"]["buckets"]), ld))
         out = np.empty((K, t2.M, 6))
@@ -294,10 +336,9 @@ def run_mbt(args):
             "metric": METRIC, "value": value, "unit": "particle-turns/s", "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": sec / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": _workload_name(args), "parallelism": "replicas x%d" % world,
-                       "l2": "particle store larger than L2, no flush needed" if (bytes_pt / 2) * n_part > 126e6 else
-                             "particle store fits L2 (latency-bound config, not an HBM roofline)"},
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "config": _config_keys(args, world),
+            "roofline": roofline, "sustained": sustained, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+            "clocks": clocks, "tuning": tuning or "library's choice",
             "algorithmic_GBps_whole_step": bytes_pt * value / world / 1e9,
         }
         print(json.dumps(line))
@@ -316,6 +357,13 @@ def main():
     ap.add_argument("--rw-turns", type=int, default=0, help="with --transverse: resistive-wall history depth (0: off)")
     ap.add_argument("--impl", default="mbt", choices=["mbt", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sustained", dest="sustained", action="store_false", help="skip the full-length sustained run")
+    ap.add_argument("--sustained-seconds", type=float, default=8.0, help="device-time bound of the sustained run")
+    ap.add_argument("--turn-mode", type=int, default=0, help="mbt_tuning.turn_mode (0: the library's choice)")
+    ap.add_argument("--tile-iters", type=int, default=0, help="mbt_tuning.tile_iters")
+    ap.add_argument("--pairs-per-thread", type=int, default=0, help="mbt_tuning.pairs_per_thread")
+    ap.add_argument("--pdl", type=int, default=0, help="mbt_tuning.pdl")
+    ap.add_argument("--verbose", type=int, default=0)
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

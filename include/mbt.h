@@ -111,6 +111,21 @@ typedef struct { double nu, alpha, beta_m, xi, eta_m, etap, sigma_u_m, sigma_up,
 typedef struct { int32_t enable; mbt_plane x, y; int32_t n_res; const mbt_resonator *res;
                  double rw_amp_x, rw_amp_y; int32_t rw_turns; } mbt_transverse;
 
+/* Kernel-selection knobs (measurement and test aid; they change how the path is launched, never what it computes).
+ * Every member: 0 = the library's choice.  All-zero (what a zero-initialised mbt_params carries) is the production setting.
+ *   tile_iters        iterations of 256 * pairs_per_thread particle pairs a pass CTA runs (> 0 fixes the tile size)
+ *   pairs_per_thread  1 or 2 particle pairs advanced per thread and iteration of the longitudinal pass
+ *   pdl               programmatic dependent launch: 1 off, 2 the pass only, 3 the pass and the wake kernel
+ *   stages6           shared-memory stages of the 6-D pass (2..4)
+ *   turn_mode         1: a turn is two launches (k_pass, k_wake); 2: one launch (the last pass CTA of a bunch builds that
+ *                     bunch's wake, the last CTA of the grid closes the turn); 3: the chip-resident persistent kernel
+ *                     (whole mbt_track in one cooperative launch; MBT_EINVAL if the particle store does not fit on chip)
+ *   verbose           1: print the chosen launch shapes to stderr at create */
+typedef struct {
+  int32_t tile_iters, pairs_per_thread, pdl, stages6, turn_mode, verbose;
+  int32_t reserved[2]; /* must be 0 */
+} mbt_tuning;
+
 typedef struct {
   mbt_ring ring;
   int32_t n_cav; const mbt_cavity *cav; /* HOST array, n_cav >= 1 */
@@ -127,17 +142,25 @@ typedef struct {
                                    NULL -> the library creates and owns a (blocking) stream             */
   int32_t device;               /* CUDA device ordinal; -1 -> the current device                        */
   mbt_transverse trans;         /* transverse planes; the library owns their four device arrays          */
+  mbt_tuning tuning;            /* kernel-selection knobs; all zero = the library's choice               */
 } mbt_params;
 
-/* Validates, allocates, builds the wake tables and draws the initial distribution on the device.
+/* Validates, allocates, builds the wake tables and draws the initial distribution on the device (P:l.37: the user chooses
+ * the effects included -- radiation, harmonic cavities, short- and long-range wakes are each switched by a zero count or
+ * flag; P:l.39: the particles then live on the GPU for the whole run; D20: seeded Gaussian start).
  * On failure *out is NULL. */
 int mbt_create(const mbt_params *p, mbt_handle **out);
 
-/* Enqueues n_turns turns on the handle's stream (asynchronous; the turn counter is cumulative and must stay
- * below 2^32 because it is a Philox counter word). */
+/* The per-turn loop of P:l.47-51 (Fig. 2) for n_turns turns: per turn S1 (P:l.63-67 Eq. 1, l.94), S2 (P:l.83-92 Eq. 5
+ * line 1), S3 (P:l.67-71 Eq. 2), S4 (P:l.98, l.109-111), S5 (P:l.98, l.107), S6 (P:l.229-237), S0 (P:l.102 Eq. 6a, l.115),
+ * S7 (P:l.123-125); with trans.enable also P:l.73-92 Eqs. (3)-(5), l.100-111 Eq. (6b), l.117-119.  Nothing returns to the
+ * host inside the loop (the paper's host "controls the flow", P:l.39; here a CUDA graph, or one persistent kernel, does).
+ * Enqueues on the handle's stream (asynchronous; the turn counter is cumulative and must stay below 2^32 because it is
+ * a Philox counter word). */
 int mbt_track(mbt_handle *h, int64_t n_turns);
 
-/* Per-bunch statistics of the current state into HOST memory, out[M][6]:
+/* P:l.123-125 ("statistical information of the bunches ... mean and standard deviation"), the longitudinal pair:
+ * per-bunch statistics of the current state into HOST memory, out[M][6]:
  * n_in, n_out, mean_tau, mean_delta, rms_tau, rms_delta (population rms over all N_p particles, D22).
  * Synchronises the stream. */
 int mbt_moments(mbt_handle *h, double *out);
@@ -146,21 +169,25 @@ int mbt_moments(mbt_handle *h, double *out);
 int mbt_destroy(mbt_handle *h);
 
 /* ---- state access used by the parity tests (HOST pointers, packed [M][N_p]; each call synchronises) ---- */
+/* the coordinates tau, delta of P:l.55-61 after the last tracked turn's wake kick (P:l.102 Eq. 6a) */
 int mbt_get_particles(mbt_handle *h, double *tau, double *delta);
 /* Upload coordinates and set the turn counter; the pending kick, the wake and the long-range history are
  * cleared (call mbt_set_lr_history AFTER this call when resuming in the middle of a run). */
 int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int64_t turn);
-/* counts of the current state, out[M][n_bins] */
+/* per-bin particle counts (P:l.109-111: "number of particles in each bin") of the current state, out[M][n_bins] */
 int mbt_get_histogram(mbt_handle *h, uint32_t *out);
-/* wake potential [V] on the bin centres built by the last tracked turn; each of total / sr_only / lr_only is
+/* V(tau_j) of P:l.102-107 on the bin centres: the short-range convolution (P:l.98) and the long-range resonator sum
+ * (P:l.229-237; D14) built by the last tracked turn [V]; each of total / sr_only / lr_only is
  * [M][n_bins] or NULL.  All zero before the first turn and after mbt_set_particles. */
 int mbt_get_wake(mbt_handle *h, double *total, double *sr_only, double *lr_only);
-/* per-turn statistics of turns first_turn .. first_turn+n-1 (1-based), out[n][M][6]; needs log_capacity_turns */
+/* P:l.123: the statistics "at every turn" -- kept on the device instead of copied to the host each turn: per-turn
+ * statistics of turns first_turn .. first_turn+n-1 (1-based), out[n][M][6]; needs log_capacity_turns */
 int mbt_get_moment_log(mbt_handle *h, int64_t first_turn, int64_t n, double *out);
-/* long-range source phasors a[b][n'][r] of the last K turns, oldest first, [K][M][R_lr][2] (re, im) */
+/* the history the long-range sum of P:l.229-237 runs over (D14; the resonator analogue of P:l.117 "information about
+ * previous bunches"): source phasors a[b][n'][r] of the last K turns, oldest first, [K][M][R_lr][2] (re, im) */
 int mbt_get_lr_history(mbt_handle *h, double *out);
 int mbt_set_lr_history(mbt_handle *h, const double *in);
-/* window shifts in bins (D31), HOST arrays of M int32 (either may be NULL in the getter): s_hist = window of the
+/* P:l.113 (first / last occupied bin, read as a window that follows the bunch, D31): window shifts in bins, HOST arrays of M int32 (either may be NULL in the getter): s_hist = window of the
  * current histogram and wake, s_next = window the next turn bins with.  mbt_set_particles resets both to 0; when
  * resuming, call mbt_set_window after it (it re-bins the state; |shift| beyond the bucket -> MBT_EINVAL). */
 int mbt_get_window(mbt_handle *h, int32_t *s_hist, int32_t *s_next);
@@ -199,12 +226,22 @@ int64_t mbt_particle_stride(int64_t n_per_bunch); /* ld of the device arrays    
 /* The tiling a pass would get (host logic only, no device needed): a bunch of pairs_per_bunch particle pairs, CTAs that
  * advance `stride` pairs per iteration, M bunches, `slots` CTAs resident on the device at once.  Even tiles (the last
  * at least 3/4 of the others) and, among those, the count that minimises ceil(w)/w (1 + 1/iterations), w = tiles M /
- * slots.  Writes pairs per tile and tiles per bunch; MBT_EINVAL on non-positive arguments. */
-int mbt_plan_tiles(int64_t pairs_per_bunch, int64_t stride, int32_t M, int32_t slots, uint32_t *tile_pairs, int32_t *tiles);
-/* DEVICE pointers of the particle store (for zero-copy wrapping, e.g. torch.from_blob-like views) */
+ * slots; tile_iters > 0 fixes the iterations per tile instead (mbt_tuning.tile_iters).  Writes pairs per tile and tiles
+ * per bunch; MBT_EINVAL on non-positive arguments. */
+int mbt_plan_tiles(int64_t pairs_per_bunch, int64_t stride, int32_t M, int32_t slots, int32_t tile_iters,
+                   uint32_t *tile_pairs, int32_t *tiles);
+/* DEVICE pointers of the particle store (for zero-copy wrapping, e.g. torch.from_blob-like views); applies a pending kick
+ * first.  The library cannot see writes through these pointers (or into caller-owned d_tau / d_delta): after changing
+ * coordinates in place call mbt_invalidate(), else mbt_moments / mbt_get_histogram return the statistics of the state the
+ * library last closed.  (In-place writes never touch the wake, the history or the turn counter.) */
 int mbt_device_pointers(mbt_handle *h, void **d_tau, void **d_delta, int64_t *ld);
+/* The particle store was modified behind the library's back: the next getter re-derives counts and moments from memory. */
+int mbt_invalidate(mbt_handle *h);
 /* kernels launched by this handle so far (bench.py's gpu_launches) */
 int64_t mbt_launch_count(const mbt_handle *h);
+/* kernel launches per tracked turn of this handle: 1 (one-launch turn), 2 (k_pass, k_wake), 3 / 4 with the transverse
+ * planes (+ k_wake_tr, + k_rw); -1 on NULL */
+int mbt_launches_per_turn(const mbt_handle *h);
 /* Seconds of device time of the most recent mbt_track call, measured with CUDA events recorded on the handle's
  * stream around the enqueued turns; synchronises.  Negative on error. */
 double mbt_last_track_seconds(mbt_handle *h);

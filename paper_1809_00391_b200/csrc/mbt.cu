@@ -20,6 +20,11 @@ namespace {
 
 thread_local std::string g_err;
 
+// mbt_tuning.turn_mode 0: two launches per turn.  The one-launch turn is complete and parity-tested, but measured slower on
+// every BASELINE workload: a bunch's wake costs its closing CTA ~15 us of latency-bound work during
+// which it holds one of the pass's 296 CTA slots (c4: 0.238 vs 0.218 ms per turn).
+constexpr bool kFusedTurnDefault = false;
+
 int fail(int code, const std::string &msg) {
   g_err = msg;
   return code;
@@ -65,20 +70,24 @@ cplx exp_lambda(const Res &r, ldbl t) {
   return cplx{(double)(mag * cosl(ph)), (double)(mag * sinl(ph))};
 }
 
+// Device buffer.  Zero-filling and uploads are enqueued on the HANDLE's stream -- the stream every kernel and copy of the
+// handle runs on -- so that they are ordered against them also when the caller's stream is a non-blocking one (the legacy
+// default stream, which cudaMemset / cudaMemcpy use, is not ordered against such streams).  cudaMemcpyAsync from pageable
+// host memory returns once the source has been staged, so the host vector may go out of scope after the call.
 template <class T>
 struct DevBuf {
   T *p = nullptr;
   size_t n = 0;
-  cudaError_t alloc(size_t count) {
+  cudaError_t alloc(size_t count, cudaStream_t st) {
     n = count;
     if (count == 0) count = 1;
     cudaError_t e = cudaMalloc((void **)&p, count * sizeof(T));
-    if (e == cudaSuccess) e = cudaMemset(p, 0, count * sizeof(T));
+    if (e == cudaSuccess) e = cudaMemsetAsync(p, 0, count * sizeof(T), st);
     return e;
   }
-  cudaError_t upload(const std::vector<T> &v) {
-    cudaError_t e = alloc(v.size());
-    if (e == cudaSuccess && !v.empty()) e = cudaMemcpy(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+  cudaError_t upload(const std::vector<T> &v, cudaStream_t st) {
+    cudaError_t e = alloc(v.size(), st);
+    if (e == cudaSuccess && !v.empty()) e = cudaMemcpyAsync(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, st);
     return e;
   }
   void release() {
@@ -93,13 +102,14 @@ struct mbt_handle {
   int device = 0;
   cudaStream_t stream = nullptr;
   bool own_stream = false;
-  int M = 0, nb = 0, R = 0, K = 0;
+  int M = 0, nb = 0, R = 0, K = 0, slots = 2;  // slots of the long-range rings: K + 1, at least 2
   int64_t Np = 0, ld = 0;
   bool own_particles = false;
   double *d_tau = nullptr, *d_delta = nullptr;
   double phi_s = 0.0;
   int64_t turn = 0;        // host mirror of ctrl.turn
   bool dirty = true;       // observable quantities (pending kick, moments, counts) need a flush
+  bool pointers_out = false;  // mbt_device_pointers has handed the store out: in-place writes are possible from now on
   bool wake_valid = false; // a tracked turn has built a wake since create / set_particles
   int64_t launches = 0;
   int64_t log_cap = 0;
@@ -142,10 +152,14 @@ struct mbt_handle {
   int32_t s_max = 0;
   double tau_lo = 0.0, Delta = 0.0;
   DevBuf<Ctrl> ctrl;
-  void (*fn_map)(const Args) = nullptr;    // k_pass<true, ...> chosen for this handle's effects
-  void (*fn_flush)(const Args) = nullptr;  // k_pass<false, ...>
+  void (*fn_map)(const Args, const WakeArgs) = nullptr;    // k_pass<true, ...> chosen for this handle's effects
+  void (*fn_flush)(const Args, const WakeArgs) = nullptr;  // k_pass<false, ...>
+  bool fused = false;  // a turn is ONE launch: the pass's last CTA of a bunch builds the bunch's wake (mbt_tuning.turn_mode 2)
+  DevBuf<uint32_t> bunch_done;
+  DevBuf<uint32_t> a_ready, bunch_ready, agg_ready;
+  DevBuf<cplx> gd;
   int npair = 1;
-  int pdl = 1;  // bit 0: the pass, bit 1: k_wake launched as a programmatic dependent (longitudinal handles; MBT_PDL sets it).
+  int pdl = 1;  // bit 0: the pass, bit 1: k_wake launched as a programmatic dependent (longitudinal handles; mbt_tuning.pdl sets it).
                 // Measured, us per turn, graph replay: pass only c1 10.8 -> 10.0, c3 16.6 -> 16.0, c4 223.9 -> 222.8; k_wake as
                 // well helps c1 (9.1) but costs c2 and c3 (26.8, 19.3): its resident CTAs are in the way of the pass's tail
   DevBuf<LogTabEntry> logtab;
@@ -158,7 +172,7 @@ struct mbt_handle {
 namespace {
 
 // ---- the instantiations of the fused pass and their selection at create time
-typedef void (*pass_fn)(const Args);
+typedef void (*pass_fn)(const Args, const WakeArgs);
 
 template <int NPAIR>
 pass_fn select_map(bool rad, int gather, int n_cav) {
@@ -182,11 +196,10 @@ pass_fn select_flush(int gather) {
 // (the last one at least 3/4 of the others) and among those the tile count that minimises
 // ceil(w) / w (1 + 1 / iterations), w = tiles M / slots the number of waves, one iteration's worth of per-CTA work.
 // The same rule serves the small workloads, where it settles just under one wave (c2, one bunch of 1e6: 391 CTAs of
-// 5 iterations instead of 977 of 2: pass 23.7 -> 18.6 us).  MBT_TILE_ITERS overrides (measurement knob).
-void choose_tiles(int64_t ppb, int64_t stride, int M, int slots, uint32_t *tile_pairs, int *tiles) {
+// 5 iterations instead of 977 of 2: pass 23.7 -> 18.6 us).  tile_iters > 0 (mbt_tuning.tile_iters) fixes the iterations.
+void choose_tiles(int64_t ppb, int64_t stride, int M, int slots, int tile_iters, bool verbose, uint32_t *tile_pairs, int *tiles) {
   const int64_t total = (ppb + stride - 1) / stride;  // iterations per bunch
-  int64_t iters = 0;
-  if (const char *e = getenv("MBT_TILE_ITERS")) iters = atoi(e) > 0 ? atoi(e) : 0;
+  int64_t iters = tile_iters > 0 ? tile_iters : 0;
   if (iters == 0) {
     double best = 1.0e30;
     for (int64_t n = 1; n <= total; ++n) {
@@ -204,7 +217,7 @@ void choose_tiles(int64_t ppb, int64_t stride, int M, int slots, uint32_t *tile_
   }
   *tile_pairs = (uint32_t)(iters * stride);
   *tiles = (int)((ppb + iters * stride - 1) / (iters * stride));
-  if (getenv("MBT_DEBUG"))
+  if (verbose)
     fprintf(stderr, "mbt: choose_tiles ppb %lld stride %lld M %d slots %d -> %lld iterations, %d tiles\n", (long long)ppb,
             (long long)stride, M, slots, (long long)iters, *tiles);
 }
@@ -220,10 +233,9 @@ pass6_fn select_map6(bool rad, int gather, int n_cav) {
 }
 pass6_fn select_flush6(int gather) { return gather ? (pass6_fn)k_pass6<false, false, 1, 0> : (pass6_fn)k_pass6<false, false, 0, 0>; }
 
-// the pass of a tracked turn: the longitudinal one, or the fused 6-D one of a handle with the transverse planes
 // launch as a programmatic dependent of the kernel before it on the stream (mbt_kernels.cuh, griddepcontrol)
-template <typename ArgT>
-void launch_dependent(void (*fn)(const ArgT), dim3 grid, int threads, size_t smem, cudaStream_t st, const ArgT &a) {
+template <typename... KArgs, typename... Vals>
+cudaError_t launch_dependent(void (*fn)(KArgs...), dim3 grid, int threads, size_t smem, cudaStream_t st, const Vals &...a) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = grid;
   cfg.blockDim = dim3(threads);
@@ -234,38 +246,55 @@ void launch_dependent(void (*fn)(const ArgT), dim3 grid, int threads, size_t sme
   at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, fn, a);
+  return cudaLaunchKernelEx(&cfg, fn, a...);
 }
 
-void enqueue_pass(mbt_handle *h) {
-  if (h->trans) h->fn_map6<<<dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream>>>(h->args6);
-  else if (h->pdl & 1) launch_dependent(h->fn_map, dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream, h->args);
-  else h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
+// the pass of a tracked turn: the longitudinal one, or the fused 6-D one of a handle with the transverse planes.
+// Every enqueue_* returns the first launch error (a bad configuration shows up here, not at a later synchronise).
+cudaError_t enqueue_pass(mbt_handle *h) {
+  if (h->trans) {
+    h->fn_map6<<<dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream>>>(h->args6);
+    return cudaGetLastError();
+  }
+  if (h->pdl & 1)
+    return launch_dependent(h->fn_map, dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream, h->args, h->wargs);
+  h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args, h->wargs);
+  return cudaGetLastError();
 }
 // the wake kernels of a turn: k_wake on the handle's stream; the transverse ones (independent of it: they read what the
 // pass wrote, and the next pass waits for both) on the side stream.  Under stream capture this becomes a fork and a join
-// in the graph.
-void enqueue_wakes(mbt_handle *h) {
+// in the graph.  In the one-launch turn there is nothing to enqueue: the pass has built the wakes.
+cudaError_t enqueue_wakes(mbt_handle *h) {
+  if (h->fused) return cudaSuccess;
+  cudaError_t e = cudaSuccess;
+#define MBT_E_(call) do { if (e == cudaSuccess) e = (call); } while (0)
   if (h->trans) {
-    cudaEventRecord(h->ev_fork, h->stream);
-    cudaStreamWaitEvent(h->stream2, h->ev_fork, 0);
+    MBT_E_(cudaEventRecord(h->ev_fork, h->stream));
+    MBT_E_(cudaStreamWaitEvent(h->stream2, h->ev_fork, 0));
     k_wake_tr<<<h->M, 256, wake_tr_smem_bytes(h->nb), h->stream2>>>(h->twargs);
-    if (h->Krw > 0) k_rw<<<h->M, 256, 0, h->stream2>>>(h->rwargs);
-    cudaEventRecord(h->ev_join, h->stream2);
+    MBT_E_(cudaGetLastError());
+    if (h->Krw > 0) {
+      k_rw<<<h->M, 256, 0, h->stream2>>>(h->rwargs);
+      MBT_E_(cudaGetLastError());
+    }
+    MBT_E_(cudaEventRecord(h->ev_join, h->stream2));
   }
-  if ((h->pdl & 2) && !h->trans)
-    launch_dependent<WakeArgs>(k_wake, dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream, h->wargs);
-  else
+  if ((h->pdl & 2) && !h->trans) {
+    MBT_E_(launch_dependent(k_wake, dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream, h->wargs));
+  } else {
     k_wake<<<dim3(h->M, h->wake_splits), kWakeThreads, h->smem_wake, h->stream>>>(h->wargs);
-  if (h->trans) cudaStreamWaitEvent(h->stream, h->ev_join, 0);
+    MBT_E_(cudaGetLastError());
+  }
+  if (h->trans) MBT_E_(cudaStreamWaitEvent(h->stream, h->ev_join, 0));
+#undef MBT_E_
+  return e;
 }
-// launches per tracked turn: 2; 3 with the transverse planes; 4 with their resistive-wall kick
-int launches_per_turn(const mbt_handle *h) { return h->trans ? (h->Krw > 0 ? 4 : 3) : 2; }
+// launches per tracked turn: 1 in the one-launch turn, else 2; 3 with the transverse planes; 4 with their resistive-wall kick
+int launches_per_turn(const mbt_handle *h) { return h->fused ? 1 : h->trans ? (h->Krw > 0 ? 4 : 3) : 2; }
 
-int enqueue_turn(mbt_handle *h) {
-  enqueue_pass(h);
-  enqueue_wakes(h);
-  return 0;
+cudaError_t enqueue_turn(mbt_handle *h) {
+  cudaError_t e = enqueue_pass(h);
+  return e == cudaSuccess ? enqueue_wakes(h) : e;
 }
 
 // scale of the fixed-point dipole sums from the transverse state in memory
@@ -281,8 +310,14 @@ int rescale_transverse(mbt_handle *h) {
 int build_graph(mbt_handle *h, int turns, cudaGraphExec_t *out) {
   cudaGraph_t g = nullptr;
   CU(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
-  for (int t = 0; t < turns; ++t) enqueue_turn(h);
-  CU(cudaStreamEndCapture(h->stream, &g));
+  cudaError_t le = cudaSuccess;
+  for (int t = 0; t < turns && le == cudaSuccess; ++t) le = enqueue_turn(h);
+  cudaError_t ce = cudaStreamEndCapture(h->stream, &g);  // always end the capture, also after a failed launch
+  if (le != cudaSuccess || ce != cudaSuccess) {
+    if (g) cudaGraphDestroy(g);
+    cudaGetLastError();
+    return fail(MBT_ECUDA, std::string("capturing a turn failed: ") + cudaGetErrorString(le != cudaSuccess ? le : ce));
+  }
   cudaError_t e = cudaGraphInstantiate(out, g, 0);
   cudaGraphDestroy(g);
   CU(e);
@@ -293,16 +328,19 @@ int build_graph(mbt_handle *h, int turns, cudaGraphExec_t *out) {
 int flush(mbt_handle *h) {
   if (!h->dirty) return 0;
   CU(cudaSetDevice(h->device));
-  if (h->trans) h->fn_flush6<<<dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream>>>(h->args6);
-  else h->fn_flush<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args);
   WakeArgs wa = h->wargs;
   wa.mode = 1;
   wa.S = 1;
-  k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(wa);
-  k_clear_pending<<<1, 1, 0, h->stream>>>(h->ctrl.p);
-  h->launches += 3;
+  if (h->trans) h->fn_flush6<<<dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream>>>(h->args6);
+  else h->fn_flush<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args, wa);
   CU(cudaGetLastError());
-  h->dirty = false;
+  k_wake<<<h->M, kWakeThreads, h->smem_wake, h->stream>>>(wa);
+  CU(cudaGetLastError());
+  k_clear_pending<<<1, 1, 0, h->stream>>>(h->ctrl.p);
+  CU(cudaGetLastError());
+  h->launches += 3;
+  // a handle on caller-owned buffers stays dirty: the caller may write the coordinates in place at any time (mbt.h)
+  h->dirty = !h->own_particles || h->pointers_out;
   return 0;
 }
 
@@ -324,7 +362,8 @@ void destroy(mbt_handle *h) {
   h->qm.release(); h->w.release(); h->Vsr.release(); h->mom_acc.release(); h->mom_last.release(); h->mom_log.release();
   h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
   h->cellSR.release(); h->cellF.release();
-  h->rd_cnt.release(); h->wr_cnt.release();
+  h->rd_cnt.release(); h->wr_cnt.release(); h->bunch_done.release();
+  h->a_ready.release(); h->bunch_ready.release(); h->agg_ready.release(); h->gd.release();
   h->tx.release(); h->txp.release(); h->ty.release(); h->typ.release(); h->wt.release(); h->Sfix.release(); h->Sov.release();
   h->S_last.release(); h->Ktab.release(); h->acc2.release(); h->fix.release(); h->cellX.release(); h->cellY.release();
   h->mom_tr_acc.release(); h->mom_tr.release();
@@ -364,16 +403,18 @@ extern "C" {
 const char *mbt_last_error(void) { return g_err.c_str(); }
 const char *mbt_version(void) { return "mbt-b200 0.1 (sm_100a)"; }
 int64_t mbt_particle_stride(int64_t n) { return n < 0 ? -1 : (n + 3) / 4 * 4; }
-int mbt_plan_tiles(int64_t ppb, int64_t stride, int32_t M, int32_t slots, uint32_t *tile_pairs, int32_t *tiles) {
-  if (ppb < 1 || stride < 1 || M < 1 || slots < 1 || !tile_pairs || !tiles) return fail(MBT_EINVAL, "bad argument");
+int mbt_plan_tiles(int64_t ppb, int64_t stride, int32_t M, int32_t slots, int32_t tile_iters, uint32_t *tile_pairs,
+                   int32_t *tiles) {
+  if (ppb < 1 || stride < 1 || M < 1 || slots < 1 || tile_iters < 0 || !tile_pairs || !tiles) return fail(MBT_EINVAL, "bad argument");
   int n = 0;
-  choose_tiles(ppb, stride, M, slots, tile_pairs, &n);
+  choose_tiles(ppb, stride, M, slots, tile_iters, false, tile_pairs, &n);
   *tiles = n;
   return 0;
 }
 int64_t mbt_turn(const mbt_handle *h) { return h ? h->turn : -1; }
 double mbt_phi_s(const mbt_handle *h) { return h ? h->phi_s : NAN; }
 int64_t mbt_launch_count(const mbt_handle *h) { return h ? h->launches : -1; }
+int mbt_launches_per_turn(const mbt_handle *h) { return h ? launches_per_turn(h) : -1; }
 
 int mbt_create(const mbt_params *p, mbt_handle **out) {
   if (!p || !out) return fail(MBT_EINVAL, "null argument");
@@ -423,6 +464,11 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
       if (!(tr.res[r].Q > 0.5) || !(tr.res[r].fr_Hz > 0) || !std::isfinite(tr.res[r].Rs_ohm))
         return fail(MBT_EINVAL, "transverse resonator: need Q > 1/2, fr > 0");
   }
+  const mbt_tuning &tn = p->tuning;
+  if (tn.tile_iters < 0 || tn.pairs_per_thread < 0 || tn.pairs_per_thread > 2 || tn.pdl < 0 || tn.pdl > 3 || tn.stages6 < 0 ||
+      (tn.stages6 != 0 && (tn.stages6 < 2 || tn.stages6 > kMaxStages6)) || tn.turn_mode < 0 || tn.turn_mode > 3 ||
+      tn.verbose < 0 || tn.reserved[0] != 0 || tn.reserved[1] != 0)
+    return fail(MBT_EINVAL, "tuning: a member is out of range (see mbt_tuning in mbt.h; all zero = the library's choice)");
   int n_lr = 0;
   for (int r = 0; r < wk.n_res; ++r) {
     if (!(wk.res[r].Q > 0.5) || !(wk.res[r].fr_Hz > 0) || !std::isfinite(wk.res[r].Rs_ohm))
@@ -573,10 +619,10 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     CUH(cudaMalloc((void **)&h->d_tau, N * sizeof(double)));
     CUH(cudaMalloc((void **)&h->d_delta, N * sizeof(double)));
   }
-  CUH(h->qm.upload(qm));
-  if (have_sr) CUH(h->w.upload(w));
-  CUH(h->Esrc.upload(Esrc));
-  CUH(h->F.upload(F));
+  CUH(h->qm.upload(qm, h->stream));
+  if (have_sr) CUH(h->w.upload(w, h->stream));
+  CUH(h->Esrc.upload(Esrc, h->stream));
+  CUH(h->F.upload(F, h->stream));
   {  // gather cells of the constant tables F_r (same cell definition as k_wake applies to V_SR)
     std::vector<CellF> cf((size_t)(R ? R : 1) * (nb + 2), CellF{cplx{0, 0}, cplx{0, 0}});
     for (int r = 0; r < R; ++r)
@@ -593,9 +639,9 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
         }
         cf[(size_t)r * (nb + 2) + k] = c;
       }
-    CUH(h->cellF.upload(cf));
+    CUH(h->cellF.upload(cf, h->stream));
   }
-  CUH(h->cellSR.alloc((size_t)M * (nb + 2)));
+  CUH(h->cellSR.alloc((size_t)M * (nb + 2), h->stream));
   // ---- bunch-following window (D31): shifts in whole bins, |s| <= s_max keeps the window inside the bucket
   h->window_mode = wk.window_mode;
   h->tau_lo = wk.tau_lo_s;
@@ -606,10 +652,10 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     const double smax = std::floor(room / Delta);
     h->s_max = (wk.window_mode && smax > 0.0) ? (int32_t)std::fmin(smax, 1.0e6) : 0;
     std::vector<double> lo0(M, (wk.tau_lo_s == 0.0) ? -0.0 : wk.tau_lo_s);  // 0 stored as -0.0: see in_window()
-    CUH(h->lo_hist.upload(lo0));
-    CUH(h->lo_next.upload(lo0));
-    CUH(h->s_hist.alloc(M));
-    CUH(h->s_next.alloc(M));
+    CUH(h->lo_hist.upload(lo0, h->stream));
+    CUH(h->lo_next.upload(lo0, h->stream));
+    CUH(h->s_hist.alloc(M, h->stream));
+    CUH(h->s_next.alloc(M, h->stream));
     if (wk.window_mode && R > 0) {
       const int W = 2 * h->s_max + 1;
       std::vector<cplx> ss((size_t)R * W), sw((size_t)R * W);
@@ -620,26 +666,37 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
           ss[(size_t)r * W + i] = cplx{(double)(mg * cosl(ph)), (double)(-mg * sinl(ph))};               // exp(-lambda t)
           sw[(size_t)r * W + i] = cplx{(double)(cosl(ph) / mg), (double)(sinl(ph) / mg)};                // exp(+lambda t)
         }
-      CUH(h->shift_src.upload(ss));
-      CUH(h->shift_wit.upload(sw));
+      CUH(h->shift_src.upload(ss, h->stream));
+      CUH(h->shift_wit.upload(sw, h->stream));
     }
   }
-  CUH(h->g_step.upload(g_step));
-  CUH(h->g_tail.upload(g_tail));
-  CUH(h->g_hist.upload(g_hist));
-  CUH(h->Vsr.alloc((size_t)M * nb));
-  CUH(h->a_cur.alloc((size_t)M * (R ? R : 1)));
-  CUH(h->ring_a.alloc((size_t)(K + 1) * M * (R ? R : 1)));
-  CUH(h->ring_A.alloc((size_t)(K + 1) * (R ? R : 1)));
-  CUH(h->P.alloc((size_t)M * (R ? R : 1)));
-  CUH(h->hist.alloc((size_t)M * nb));
-  CUH(h->hist_last.alloc((size_t)M * nb));
-  CUH(h->mom_acc.alloc((size_t)M * 4));
-  CUH(h->nout_acc.alloc((size_t)M));
-  CUH(h->mom_last.alloc((size_t)M * 6));
-  if (h->log_cap > 0) CUH(h->mom_log.alloc((size_t)h->log_cap * M * 6));
-  CUH(h->ctrl.alloc(1));
-  CUH(h->logtab.upload(std::vector<LogTabEntry>(kLogTabHost, kLogTabHost + 128)));
+  CUH(h->g_step.upload(g_step, h->stream));
+  CUH(h->g_tail.upload(g_tail, h->stream));
+  CUH(h->g_hist.upload(g_hist, h->stream));
+  {  // exp(lambda_r d T_rf) over the bucket distance d (one-launch turn: the per-bunch phasor gather)
+    std::vector<cplx> gd((size_t)(R ? R : 1) * rg.h, cplx{1.0, 0.0});
+    for (int r = 0; r < R; ++r)
+      for (int d = 0; d < rg.h; ++d) gd[(size_t)r * rg.h + d] = exp_lambda(lr[r], (ldbl)d * Trf);
+    CUH(h->gd.upload(gd, h->stream));
+    CUH(h->d_bucket.upload(std::vector<int32_t>(fl.bucket, fl.bucket + M), h->stream));
+    CUH(h->a_ready.alloc((size_t)M * (R ? R : 1), h->stream));
+    CUH(h->bunch_ready.alloc(M, h->stream));
+    CUH(h->agg_ready.alloc(1, h->stream));
+  }
+  CUH(h->Vsr.alloc((size_t)M * nb, h->stream));
+  CUH(h->a_cur.alloc((size_t)M * (R ? R : 1), h->stream));
+  h->slots = K + 1 < 2 ? 2 : K + 1;
+  CUH(h->ring_a.alloc((size_t)h->slots * M * (R ? R : 1), h->stream));
+  CUH(h->ring_A.alloc((size_t)h->slots * (R ? R : 1), h->stream));
+  CUH(h->P.alloc((size_t)M * (R ? R : 1), h->stream));
+  CUH(h->hist.alloc((size_t)M * nb, h->stream));
+  CUH(h->hist_last.alloc((size_t)M * nb, h->stream));
+  CUH(h->mom_acc.alloc((size_t)M * 4, h->stream));
+  CUH(h->nout_acc.alloc((size_t)M, h->stream));
+  CUH(h->mom_last.alloc((size_t)M * 6, h->stream));
+  if (h->log_cap > 0) CUH(h->mom_log.alloc((size_t)h->log_cap * M * 6, h->stream));
+  CUH(h->ctrl.alloc(1, h->stream));
+  CUH(h->logtab.upload(std::vector<LogTabEntry>(kLogTabHost, kLogTabHost + 128), h->stream));
 
   A.tau = h->d_tau;
   A.delta = h->d_delta;
@@ -669,8 +726,8 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     if (S < 1) S = 1;
     h->wake_splits = S;
   }
-  CUH(h->rd_cnt.alloc(M));
-  CUH(h->wr_cnt.alloc(M));
+  CUH(h->rd_cnt.alloc(M, h->stream));
+  CUH(h->wr_cnt.alloc(M, h->stream));
   Wa.S = h->wake_splits; Wa.rd_cnt = h->rd_cnt.p; Wa.wr_cnt = h->wr_cnt.p;
   Wa.qm = h->qm.p;
   Wa.w = have_sr ? h->w.p : nullptr;
@@ -685,28 +742,66 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   Wa.mom_log = h->log_cap > 0 ? h->mom_log.p : nullptr;
   Wa.log_cap = h->log_cap;
   Wa.ctrl = h->ctrl.p;
+  Wa.h = rg.h; Wa.slots = h->slots; Wa.bucket = h->d_bucket.p; Wa.gd = h->gd.p;
+  Wa.a_ready = h->a_ready.p; Wa.bunch_ready = h->bunch_ready.p; Wa.agg_ready = h->agg_ready.p;
 
   // ---- launch shapes: one resident wave of CTAs, each owning a contiguous run of pairs
   // two pairs per thread (twice the independent arithmetic per warp, 2 CTAs/SM) pay off except for small
   // two-cavity workloads, where the four sine chains per thread cost more registers than they hide latency
-  if (const char *e = getenv("MBT_PDL")) h->pdl = atoi(e) & 3;  // measurement knob
+  if (tn.pdl) h->pdl = tn.pdl == 1 ? 0 : tn.pdl == 2 ? 1 : 3;  // mbt_tuning.pdl: 1 off, 2 the pass, 3 the pass and k_wake
   h->npair = kDefaultNPair ? kDefaultNPair : ((p->n_cav == 1 || (int64_t)M * h->Np >= 10000000ll) ? 2 : 1);
-  if (const char *e = getenv("MBT_NPAIR")) h->npair = (atoi(e) == 2) ? 2 : 1;  // measurement knob
+  if (tn.pairs_per_thread) h->npair = tn.pairs_per_thread;
   const bool rad_on = p->rad.enable != 0;
   h->fn_map = h->npair == 2 ? select_map<2>(rad_on, wk.gather_order, p->n_cav) : select_map<1>(rad_on, wk.gather_order, p->n_cav);
   h->fn_flush = h->npair == 2 ? select_flush<2>(wk.gather_order) : select_flush<1>(wk.gather_order);
   h->smem_pass = pass_smem_bytes(nb, h->npair);
-  h->smem_wake = (size_t)nb * 3 * sizeof(double);
+  // k_wake: the convolution's shared memory + the staged source factors (if <= 64 KB), or the scan's staged operands (if
+  // the scan runs and they fit in 96 KB).  Kept small: every CTA of the launch should be resident at once.
+  {
+    size_t need = wake_smem_bytes(nb, M);
+    const size_t stage_e = (size_t)R * nb * sizeof(cplx) + 16;
+    if (R > 0 && stage_e <= 64u * 1024u) need += stage_e;
+    // one CTA per bunch: the per-bunch phasor gather replaces the scan.  A bunch's CTA waits only for CTAs of a lower
+    // index, which were dispatched before it: no deadlock whether or not all M CTAs are resident at once (they are up to
+    // 3 x 148 bunches: __launch_bounds__(256, 3) and the carve-out below)
+    CUH(cudaFuncSetAttribute(k_wake, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
+    const bool gather = h->wake_splits == 1;
+    if (!gather && scan_smem_bytes(M, R) <= 96u * 1024u) need = std::max(need, scan_smem_bytes(M, R));
+    h->smem_wake = need;
+    Wa.gather_P = gather ? 1 : 0;
+  }
+  Wa.smem_wake_bytes = (uint32_t)h->smem_wake;
+  Wa.smem_pass_bytes = (uint32_t)h->smem_pass;
   CUH(cudaFuncSetAttribute((const void *)h->fn_map, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
   CUH(cudaFuncSetAttribute((const void *)h->fn_flush, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass));
   CUH(cudaFuncSetAttribute(k_wake, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_wake));
+  // all CTAs of k_wake should be resident at once: with the default carve-out only two per SM were (the third of an SM
+  // started when the first had finished: 15 us later)
+  CUH(cudaFuncSetAttribute(k_wake, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
   // tiles (choose_tiles)
   {
     int occ = 0;
     CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)h->fn_map, kPassThreads, h->smem_pass));
     if (occ < 1) occ = 1;
-    choose_tiles(h->ld / 2, (int64_t)kPassThreads * h->npair, M, prop.multiProcessorCount * occ, &A.tile_pairs, &h->grid_pass);
+    choose_tiles(h->ld / 2, (int64_t)kPassThreads * h->npair, M, prop.multiProcessorCount * occ, tn.tile_iters, tn.verbose != 0,
+                 &A.tile_pairs, &h->grid_pass);
   }
+
+  // ---- one launch per turn (mbt_tuning.turn_mode): the last pass CTA of a bunch builds the bunch's wake in the (drained)
+  // particle stages, the last CTA of the grid closes the turn.  Not with the transverse planes (their wake kernels run
+  // beside k_wake on a side stream).
+  CUH(h->bunch_done.alloc(M, h->stream));
+  A.bunch_done = h->bunch_done.p;
+  h->fused = !tr.enable && (tn.turn_mode == 2 || (tn.turn_mode == 0 && kFusedTurnDefault));
+  if (tn.turn_mode == 2 && tr.enable) {
+    destroy(h);
+    return fail(MBT_EINVAL, "tuning.turn_mode 2 (one launch per turn) is not available with the transverse planes");
+  }
+  if (h->fused && h->smem_pass < wake_smem_bytes(nb, M)) h->fused = false;  // cannot happen for nb <= MBT_MAX_BINS
+  A.fused = h->fused ? 1 : 0;
+  if (tn.verbose)
+    fprintf(stderr, "mbt: %s, %d pair(s) per thread, grid %d x %d, %zu B shared memory per CTA, pdl %d\n",
+            h->fused ? "one launch per turn" : "two launches per turn", h->npair, h->grid_pass, M, h->smem_pass, h->pdl);
 
   // ---- initial distribution (D20) on the device
   {
@@ -728,32 +823,31 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
         wt[k] += (double)((wr * wr * (ldbl)rr.Rs / ((ldbl)rr.Q * rr.wbar)) * expl(-rr.alpha * t) * sinl(rr.wbar * t));
       }
     }
-    CUH(h->wt.upload(wt));
-    CUH(h->tx.alloc(N)); CUH(h->txp.alloc(N)); CUH(h->ty.alloc(N)); CUH(h->typ.alloc(N));
-    CUH(h->Sfix.alloc((size_t)M * 2 * (nb + 1))); CUH(h->Sov.alloc((size_t)M * 2 * (nb + 1)));
+    CUH(h->wt.upload(wt, h->stream));
+    CUH(h->tx.alloc(N, h->stream)); CUH(h->txp.alloc(N, h->stream)); CUH(h->ty.alloc(N, h->stream)); CUH(h->typ.alloc(N, h->stream));
+    CUH(h->Sfix.alloc((size_t)M * 2 * (nb + 1), h->stream)); CUH(h->Sov.alloc((size_t)M * 2 * (nb + 1), h->stream));
     // long-range resistive wall (W1..W5): source ring, kick per bunch, weights (d T_rf)^-1/2 by bucket distance d
     h->Krw = tr.rw_turns;
-    CUH(h->ring_g.alloc((size_t)(h->Krw + 1) * M * 2));
-    CUH(h->rw.alloc((size_t)M * 2));
+    CUH(h->ring_g.alloc((size_t)(h->Krw + 1) * M * 2, h->stream));
+    CUH(h->rw.alloc((size_t)M * 2, h->stream));
     {
       std::vector<double> wr((size_t)(h->Krw + 1) * rg.h, 0.0);
       for (size_t d = 1; d < wr.size(); ++d)
         wr[d] = (double)(1.0L / sqrtl((ldbl)d * ((ldbl)rg.T0_s / (ldbl)rg.h)));
-      CUH(h->wrw.upload(wr));
-      CUH(h->d_bucket.upload(std::vector<int32_t>(fl.bucket, fl.bucket + M)));
+      CUH(h->wrw.upload(wr, h->stream));
     }
     RwArgs &Rw = h->rwargs;
     memset(&Rw, 0, sizeof Rw);
     Rw.M = M; Rw.Krw = h->Krw; Rw.h = rg.h; Rw.bucket = h->d_bucket.p; Rw.ring_g = h->ring_g.p; Rw.wrw = h->wrw.p;
-    CUH(h->turn_tr.alloc(1));
+    CUH(h->turn_tr.alloc(1, h->stream));
     CUH(cudaStreamCreateWithFlags(&h->stream2, cudaStreamNonBlocking));
     CUH(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
     CUH(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
     Rw.amp[0] = tr.rw_amp_x; Rw.amp[1] = tr.rw_amp_y; Rw.rw = h->rw.p; Rw.turn_tr = h->turn_tr.p;
-    CUH(h->S_last.alloc((size_t)M * 2 * nb)); CUH(h->Ktab.alloc((size_t)M * 2 * nb));
-    CUH(h->cellX.alloc((size_t)M * (nb + 2))); CUH(h->cellY.alloc((size_t)M * (nb + 2)));
-    CUH(h->fix.alloc((size_t)M * 2)); CUH(h->acc2.alloc((size_t)M * 2));
-    CUH(h->mom_tr_acc.alloc((size_t)M * 8)); CUH(h->mom_tr.alloc((size_t)M * 8));
+    CUH(h->S_last.alloc((size_t)M * 2 * nb, h->stream)); CUH(h->Ktab.alloc((size_t)M * 2 * nb, h->stream));
+    CUH(h->cellX.alloc((size_t)M * (nb + 2), h->stream)); CUH(h->cellY.alloc((size_t)M * (nb + 2), h->stream));
+    CUH(h->fix.alloc((size_t)M * 2, h->stream)); CUH(h->acc2.alloc((size_t)M * 2, h->stream));
+    CUH(h->mom_tr_acc.alloc((size_t)M * 8, h->stream)); CUH(h->mom_tr.alloc((size_t)M * 8, h->stream));
     // bits of the fixed-point dipole sums: N_p 2^bits <= 2^62 (mbt_trans.cuh)
     h->fix_bits = kFixBitsMax;
     while (h->fix_bits > 20 && (double)h->Np * std::ldexp(1.0, h->fix_bits) > std::ldexp(1.0, 62)) h->fix_bits -= 1;
@@ -786,8 +880,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     }
     // two stages (48 KB) in flight per CTA: three measured the same to 1 % (c4 0.839 vs 0.834 ms, c5 2.41 vs 2.37), four
     // cost a CTA per SM
-    T.stages = 2;
-    if (const char *e = getenv("MBT_STAGES6")) T.stages = std::min(kMaxStages6, std::max(2, atoi(e)));  // measurement knob
+    T.stages = tn.stages6 ? tn.stages6 : 2;
     h->smem_pass6 = pass6_smem_bytes(nb, T.stages);
     CUH(cudaFuncSetAttribute((const void *)h->fn_map6, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass6));
     CUH(cudaFuncSetAttribute((const void *)h->fn_flush6, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pass6));
@@ -796,7 +889,8 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
       int occ = 0;
       CUH(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)h->fn_map6, kPassThreads, h->smem_pass6));
       if (occ < 1) occ = 1;
-      choose_tiles(h->ld / 2, kPassThreads, M, prop.multiProcessorCount * occ, &T.tile_pairs, &h->grid_pass6);
+      choose_tiles(h->ld / 2, kPassThreads, M, prop.multiProcessorCount * occ, tn.tile_iters, tn.verbose != 0, &T.tile_pairs,
+                   &h->grid_pass6);
     }
     TMomArgs &Tm = h->tmargs;
     Tm.x = h->tx.p; Tm.xp = h->txp.p; Tm.y = h->ty.p; Tm.yp = h->typ.p; Tm.ld = h->ld; Tm.Np = (uint32_t)h->Np; Tm.tile = 8192;
@@ -808,7 +902,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     Tw.Sfix = h->Sfix.p; Tw.Sov = h->Sov.p; Tw.fix = h->fix.p; Tw.acc2 = h->acc2.p;
     Tw.S_last = h->S_last.p; Tw.K = h->Ktab.p; Tw.cellX = h->cellX.p; Tw.cellY = h->cellY.p;
     Tw.Krw = h->Krw; Tw.ring_g = h->ring_g.p; Tw.turn_tr = h->turn_tr.p;
-    if (h->log_cap > 0) CUH(h->log_tr.alloc((size_t)h->log_cap * M * 4));
+    if (h->log_cap > 0) CUH(h->log_tr.alloc((size_t)h->log_cap * M * 4, h->stream));
     Tw.log_tr = h->log_cap > 0 ? h->log_tr.p : nullptr;
     Tw.log_cap = h->log_cap;
     dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)M);
@@ -863,22 +957,27 @@ int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, dou
   if (!h || n_turns < 1 || n_turns > 65536 || !pass_seconds || !wake_seconds) return fail(MBT_EINVAL, "bad argument");
   if (h->turn + n_turns > 0xFFFFFFFFll) return fail(MBT_EINVAL, "turn counter would exceed 2^32");
   CU(cudaSetDevice(h->device));
-  std::vector<cudaEvent_t> ev((size_t)n_turns * 3, nullptr);
+  struct Events {  // destroyed on every exit path
+    std::vector<cudaEvent_t> v;
+    ~Events() { for (cudaEvent_t e : v) if (e) cudaEventDestroy(e); }
+  } evs;
+  evs.v.assign((size_t)n_turns * 3, nullptr);
+  std::vector<cudaEvent_t> &ev = evs.v;
   for (auto &e : ev) CU(cudaEventCreate(&e));
   CU(cudaEventRecord(h->ev0, h->stream));
   for (int64_t t = 0; t < n_turns; ++t) {
     CU(cudaEventRecord(ev[3 * t], h->stream));
-    enqueue_pass(h);
+    CU(enqueue_pass(h));
     CU(cudaEventRecord(ev[3 * t + 1], h->stream));
-    enqueue_wakes(h);
+    CU(enqueue_wakes(h));
     CU(cudaEventRecord(ev[3 * t + 2], h->stream));
+    h->launches += launches_per_turn(h);
+    h->turn += 1;
+    h->dirty = true;
+    h->wake_valid = true;
   }
   CU(cudaEventRecord(h->ev1, h->stream));
   h->timed = true;
-  h->launches += launches_per_turn(h) * n_turns;
-  h->turn += n_turns;
-  h->dirty = true;
-  h->wake_valid = true;
   CU(cudaStreamSynchronize(h->stream));
   double ps = 0.0, ws = 0.0;
   for (int64_t t = 0; t < n_turns; ++t) {
@@ -888,7 +987,6 @@ int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, dou
     ps += (double)a * 1e-3;
     ws += (double)b * 1e-3;
   }
-  for (auto &e : ev) cudaEventDestroy(e);
   *pass_seconds = ps;
   *wake_seconds = ws;
   return 0;
@@ -923,6 +1021,14 @@ int mbt_device_pointers(mbt_handle *h, void **d_tau, void **d_delta, int64_t *ld
   if (d_tau) *d_tau = h->d_tau;
   if (d_delta) *d_delta = h->d_delta;
   if (ld) *ld = h->ld;
+  h->pointers_out = true;  // in-place writes are possible from now on: every later getter re-derives counts and moments
+  h->dirty = true;
+  return 0;
+}
+
+int mbt_invalidate(mbt_handle *h) {
+  if (!h) return fail(MBT_EINVAL, "null argument");
+  h->dirty = true;
   return 0;
 }
 
@@ -935,7 +1041,7 @@ int mbt_get_particles(mbt_handle *h, double *tau, double *delta) {
     CU(cudaMemcpyAsync(tau, h->d_tau, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CU(cudaMemcpyAsync(delta, h->d_delta, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   } else {
-    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n)); }
+    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n, h->stream)); }
     dim3 grid((unsigned)((h->Np + 255) / 256 < 1024 ? (h->Np + 255) / 256 : 1024), (unsigned)h->M);
     k_pack<<<grid, 256, 0, h->stream>>>(h->d_tau, h->ld, (uint32_t)h->Np, h->scratch_a.p);
     CU(cudaMemcpyAsync(tau, h->scratch_a.p, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
@@ -959,7 +1065,7 @@ int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int
     CU(cudaMemcpyAsync(h->d_tau, tau, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(h->d_delta, delta, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
   } else {
-    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n)); }
+    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n, h->stream)); }
     dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)h->M);
     CU(cudaMemcpyAsync(h->scratch_a.p, tau, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     k_unpack<<<grid, 256, 0, h->stream>>>(h->scratch_a.p, h->ld, (uint32_t)h->Np, h->d_tau);
@@ -972,7 +1078,9 @@ int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int
     int rc = upload_window(h, zero.data(), zero.data());
     if (rc) return rc;
   }
-  k_set_ctrl<<<1, 1, 0, h->stream>>>(h->ctrl.p, (uint32_t)turn, 0u);
+  k_set_ctrl<<<1, 256, 0, h->stream>>>(h->ctrl.p, (uint32_t)turn, 0u, h->a_ready.p, h->M * (h->R ? h->R : 1), h->bunch_ready.p, h->M,
+                                       h->agg_ready.p, h->bunch_done.p);
+  CU(cudaGetLastError());
   h->launches += 1;
   CU(cudaMemsetAsync(h->hist.p, 0, sizeof(uint32_t) * h->M * h->nb, h->stream));
   CU(cudaMemsetAsync(h->mom_acc.p, 0, sizeof(double) * h->M * 4, h->stream));
@@ -993,7 +1101,7 @@ int copy_out_packed(mbt_handle *h, const double *dev, double *host) {
   if (h->ld == h->Np) {
     CU(cudaMemcpyAsync(host, dev, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   } else {
-    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n)); }
+    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n, h->stream)); }
     dim3 grid((unsigned)((h->Np + 255) / 256 < 1024 ? (h->Np + 255) / 256 : 1024), (unsigned)h->M);
     k_pack<<<grid, 256, 0, h->stream>>>(dev, h->ld, (uint32_t)h->Np, h->scratch_a.p);
     h->launches += 1;
@@ -1007,7 +1115,7 @@ int copy_in_packed(mbt_handle *h, const double *host, double *dev) {
   if (h->ld == h->Np) {
     CU(cudaMemcpyAsync(dev, host, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
   } else {
-    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n)); }
+    if (h->scratch_a.n < n) { h->scratch_a.release(); CU(h->scratch_a.alloc(n, h->stream)); }
     dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)h->M);
     CU(cudaMemcpyAsync(h->scratch_a.p, host, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     k_unpack<<<grid, 256, 0, h->stream>>>(h->scratch_a.p, h->ld, (uint32_t)h->Np, dev);
@@ -1169,7 +1277,7 @@ int mbt_get_wake(mbt_handle *h, double *total, double *sr, double *lr) {
     if (lr) memset(lr, 0, n * sizeof(double));
     return 0;
   }
-  if (h->scratch_b.n < 3 * n) { h->scratch_b.release(); CU(h->scratch_b.alloc(3 * n)); }
+  if (h->scratch_b.n < 3 * n) { h->scratch_b.release(); CU(h->scratch_b.alloc(3 * n, h->stream)); }
   double *dt = h->scratch_b.p, *ds = dt + n, *dl = ds + n;
   k_eval_wake<<<h->M, 256, 0, h->stream>>>(h->M, h->nb, h->R, h->Vsr.p, h->P.p, h->F.p, dt, ds, dl);
   h->launches += 1;
@@ -1197,7 +1305,7 @@ int mbt_get_lr_history(mbt_handle *h, double *out) {
   CU(cudaSetDevice(h->device));
   const int M = h->M, R = h->R, K = h->K;
   if (R == 0 || K == 0) return 0;
-  std::vector<cplx> ring((size_t)(K + 1) * M * R);
+  std::vector<cplx> ring((size_t)h->slots * M * R);
   CU(cudaMemcpyAsync(ring.data(), h->ring_a.p, ring.size() * sizeof(cplx), cudaMemcpyDeviceToHost, h->stream));
   CU(cudaStreamSynchronize(h->stream));
   for (int k = 0; k < K; ++k) {
@@ -1205,7 +1313,7 @@ int mbt_get_lr_history(mbt_handle *h, double *out) {
     for (int b = 0; b < M; ++b)
       for (int r = 0; r < R; ++r) {
         cplx a{0.0, 0.0};
-        if (t >= 1) a = ring[((size_t)(t % (K + 1)) * M + b) * R + r];
+        if (t >= 1) a = ring[((size_t)(t % h->slots) * M + b) * R + r];
         double *o = &out[(((size_t)k * M + b) * R + r) * 2];
         o[0] = a.re;
         o[1] = a.im;
@@ -1219,18 +1327,18 @@ int mbt_set_lr_history(mbt_handle *h, const double *in) {
   CU(cudaSetDevice(h->device));
   const int M = h->M, R = h->R, K = h->K;
   if (R == 0 || K == 0) return 0;
-  std::vector<cplx> ring((size_t)(K + 1) * M * R, cplx{0.0, 0.0});
+  std::vector<cplx> ring((size_t)h->slots * M * R, cplx{0.0, 0.0});
   for (int k = 0; k < K; ++k) {
     const int64_t t = h->turn - K + 1 + k;
     if (t < 1) continue;
     for (int b = 0; b < M; ++b)
       for (int r = 0; r < R; ++r) {
         const double *i2 = &in[(((size_t)k * M + b) * R + r) * 2];
-        ring[((size_t)(t % (K + 1)) * M + b) * R + r] = cplx{i2[0], i2[1]};
+        ring[((size_t)(t % h->slots) * M + b) * R + r] = cplx{i2[0], i2[1]};
       }
   }
   CU(cudaMemcpyAsync(h->ring_a.p, ring.data(), ring.size() * sizeof(cplx), cudaMemcpyHostToDevice, h->stream));
-  k_aggregate_history<<<K + 1, 32, 0, h->stream>>>(M, R, K, h->ring_a.p, h->g_tail.p, h->ring_A.p);
+  k_aggregate_history<<<h->slots, 32, 0, h->stream>>>(M, R, K, h->ring_a.p, h->g_tail.p, h->ring_A.p);
   h->launches += 1;
   CU(cudaGetLastError());
   CU(cudaStreamSynchronize(h->stream));

@@ -21,6 +21,7 @@ namespace mbt {
 
 constexpr int kPassThreads = 256;
 constexpr int kWakeThreads = 256;
+static_assert(kWakeThreads == kPassThreads, "the one-launch turn runs wake_body in a pass CTA");
 constexpr int kMaxCav = 8;
 constexpr int kMaxLR = 8;
 constexpr int kDefaultNPair = 0;  // pairs per thread and iteration of the pass: 1, 2, or 0 = chosen from the workload at create
@@ -95,6 +96,9 @@ struct Args {
   Ctrl *ctrl;
   const LogTabEntry *logtab;  // [128] device copy of the log table
   MathTab mt;
+  // one-launch turn (mbt_tuning.turn_mode 2): the last CTA of a bunch to finish builds that bunch's wake (wake_body)
+  int32_t fused;              // 1: this launch is a whole turn; its predecessor in the stream is the pass before it
+  uint32_t *bunch_done;       // [M] pass CTAs of the bunch that have flushed their counts and moment sums
 };
 
 // Particle staging: a CTA owns kStages shared-memory stages of kPassThreads*NPAIR pairs (tau block, then delta
@@ -163,6 +167,543 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 // as the oracle's t >= 0 decides) and every other difference is unchanged.
 __device__ __forceinline__ bool in_window(double t, uint32_t hi_nb) { return (uint32_t)__double2hiint(t) < hi_nb; }
 
+// ------------------------------------------------------------------ wake
+struct WakeArgs {
+  int32_t M, nb, R, K;
+  int32_t S;               // CTAs per bunch (grid.y): the outputs of the convolution are dealt out over them
+  uint32_t *rd_cnt, *wr_cnt;  // [M] splits that have read the counts / written their share of V_SR (S > 1)
+  uint32_t Np;
+  int32_t mode;            // 0: full turn (S5, S6, bump the turn counter); 1: finalise counts and moments only
+  const double *qm;        // [M]      macro-particle charge Q_b / N_p
+  const double *w;         // [nb]     short-range table w_k = W(k Delta); nullptr: none
+  const cplx *Esrc;        // [R][nb]  exp(-lambda_r c_k)
+  const cplx *g_step;      // [M][R]   exp(lambda_r (s_{j+1}-s_j) T_rf), j < M-1
+  const cplx *g_tail;      // [M][R]   exp(lambda_r (s_{M-1}-s_j) T_rf)
+  const cplx *g_hist;      // [K][R]   exp(lambda_r (k T0 - (s_{M-1}-s_0) T_rf)), k = 1..K
+  uint32_t *hist;          // [M][nb]  in: counts of this turn; out: zero
+  uint32_t *hist_last;     // [M][nb]  out: counts of this turn
+  double *Vsr;             // [M][nb]
+  WakeCell *cellSR;        // [M][nb+2] gather cells of Vsr (what the pass stages)
+  int32_t gather;          // 1 linear, 0 nearest grid point
+  // bunch-following window (D31); window_mode 0: the arrays below keep their initial values
+  int32_t window_mode, s_max;
+  double tau_lo, Delta;
+  int32_t *s_hist, *s_next;   // [M] window shift in bins: of this turn's histogram / of the next binning
+  double *lo_hist, *lo_next;  // [M] tau_lo + s Delta (0 stored as -0.0, see in_window())
+  const cplx *shift_src;      // [R][2 s_max + 1] exp(-lambda_r s Delta), s = -s_max..s_max
+  const cplx *shift_wit;      // [R][2 s_max + 1] exp(+lambda_r s Delta)
+  cplx *a_cur;             // [M][R]   source phasors of this turn
+  cplx *ring_a;            // [K+1][M][R] slot n % (K+1)
+  cplx *ring_A;            // [K+1][R]    per-turn aggregates, slot n % (K+1)
+  cplx *P;                 // [M][R]
+  double *mom_acc;         // [M][4]  in: sums gathered by the pass; out: zero
+  unsigned long long *nout_acc;  // [M]
+  double *mom_last;        // [M][6]
+  double *mom_log;         // [cap][M][6] or nullptr
+  int64_t log_cap;
+  Ctrl *ctrl;
+  uint32_t smem_wake_bytes, smem_pass_bytes;  // dynamic shared memory of a k_wake launch / of a pass launch (one-launch turn)
+  // one-launch turn: per-bunch phasor gather instead of the scan (wake_body<false, true>)
+  int32_t gather_P;           // k_wake with one CTA per bunch: per-bunch phasor gather (all CTAs resident) instead of the scan
+  int32_t h, slots;           // harmonic number; slots of ring_a / ring_A (K + 1, at least 2)
+  const int32_t *bucket;      // [M]
+  const cplx *gd;             // [R][h] exp(lambda_r d T_rf), d = 0 .. h-1 (bucket distance)
+  uint32_t *a_ready;          // [M][R] turn whose source phasor a[b][r] is in ring_a (release / acquire)
+  uint32_t *bunch_ready;      // [M]    turn whose wake (cells, phasor P, windows, cleared counts) of bunch b is complete
+  uint32_t *agg_ready;        // [1]    turn whose aggregate A_n is in ring_A
+};
+
+// L2 load of a complex number written earlier in this kernel by another CTA (never through a stale L1 line)
+__device__ __forceinline__ cplx __ldcg_cplx(const cplx *p) {
+  const double2 v = __ldcg(reinterpret_cast<const double2 *>(p));
+  return cplx{v.x, v.y};
+}
+
+// flags written by one CTA and awaited by another of the same (or the next) launch
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_u32(uint32_t *p, uint32_t v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// turn numbers are compared modulo 2^32
+__device__ __forceinline__ void wait_turn(const uint32_t *flag, uint32_t n) {
+  while ((int32_t)(ld_acquire_u32(flag) - n) < 0) {
+  }
+}
+
+// affine map x -> g x + c over the complex numbers; (first o second)(x) = second(first(x))
+struct Affine {
+  cplx g, c;
+};
+__device__ __forceinline__ Affine compose(const Affine &first, const Affine &second) {
+  return Affine{cmul(first.g, second.g), cfma(first.c, second.g, second.c)};
+}
+
+// Shared memory of wake_body: charges, V_SR, and the wake table with sixteen zeros in front and eight behind (the sliding
+// window of the register-blocked convolution runs off both ends).  The scan of the turn's last CTA stages its operands
+// (48 bytes per bunch and resonator) in the same memory if they fit into what the launch provides (`smem_bytes`).
+__host__ __device__ inline size_t wake_smem_bytes(int nb, int M) { return (size_t)(3 * nb + 24) * sizeof(double) + (size_t)M * sizeof(int32_t); }
+__host__ __device__ inline size_t scan_smem_bytes(int M, int R) { return (size_t)M * (size_t)R * 3 * sizeof(cplx); }
+
+// The wake of bunch b (and, for the CTA that finishes last, the closing of the turn).  Called by every thread of a CTA of
+// kWakeThreads threads: by k_wake (SPLIT: the S = gridDim.y CTAs of a bunch share its convolution), and by the last pass
+// CTA of a bunch in the one-launch turn (SPLIT = false).  smem_d: smem_bytes >= wake_smem_bytes(nb) of shared memory.
+// Counts and moment sums were accumulated with atomics by other CTAs, possibly of this same launch: they are read
+// through L2 (__ldcg), never through an L1 line that a neighbouring bunch's reader may have pulled in earlier.
+//
+// Everything here is latency: a bunch's wake is ~1e5 multiply-adds, but a dependent trip to L2 costs most of a
+// microsecond, and this code runs ONCE per CTA, so its instruction fetches miss too -- a first version with every loop
+// over resonators and scan elements unrolled (200 KB of SASS) ran slower than the loops it replaced.  Hence: compact loops,
+// few dependent trips to memory, a register-blocked convolution that uses every thread.
+template <bool SPLIT, bool FUSED>
+__device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const int split, double *smem_d, const uint32_t smem_bytes) {
+  constexpr int NW = kWakeThreads / 32;
+  const int nb = A.nb;
+  double *sq = smem_d;               // [nb] charge per bin
+  double *sv = smem_d + nb;          // [nb] V_SR of this bunch
+  double *sw = smem_d + 2 * nb + 16;  // [-16, nb + 8) wake table, zero outside [0, nb)
+  int32_t *sB = reinterpret_cast<int32_t *>(smem_d + 3 * nb + 24);  // [M] buckets (FUSED)
+  __shared__ bool s_last;
+  __shared__ unsigned long long s_cnt[NW][2];
+
+  const int tid = threadIdx.x;
+  const int lane = tid & 31, warp = tid >> 5;
+  const int S = SPLIT ? A.S : 1;  // few bunches: S CTAs share a bunch (split 0 also does the per-bunch work)
+  const uint32_t n_done = A.ctrl->turn;  // completed turns; the turn being closed is n_done + 1
+  const uint32_t n = n_done + 1u;
+
+  // counts -> charges; keep a copy of the counts; clear the accumulator for the next pass.  The loads of a round (counts,
+  // table, and -- if it fits -- the source factors exp(-lambda_r c_k) of all resonators, into shared memory) have no
+  // global store between them, so that they are all in flight together: one trip to L2.
+  const double qm = A.qm[b];
+  const bool follow = A.mode == 0 && A.window_mode == 1;
+  const int32_t s_used = follow ? A.s_next[b] : 0;   // the window the pass binned this turn with
+  unsigned long long n_in = 0ull, m1 = 0ull;         // sum c_k, sum k c_k
+  const bool sources = A.mode == 0 && split == 0 && A.R > 0;
+  const cplx *pE = A.Esrc;  // [R][nb] as the source sums read it: staged behind the buckets if the launch's memory holds it
+  if (sources && wake_smem_bytes(nb, A.M) + (size_t)A.R * nb * sizeof(cplx) + 16 <= (size_t)smem_bytes) {
+    cplx *sE = reinterpret_cast<cplx *>((reinterpret_cast<uintptr_t>(sB + A.M) + 15) & ~(uintptr_t)15);
+    const int nE = A.R * nb;
+#pragma unroll 4
+    for (int i = tid; i < nE; i += kWakeThreads) sE[i] = A.Esrc[i];
+    pE = sE;
+  }
+#pragma unroll 2
+  for (int j = tid; j < nb; j += kWakeThreads) {
+    const uint32_t c = __ldcg(&A.hist[(size_t)b * nb + j]);
+    if (A.mode == 0) sw[j] = A.w ? A.w[j] : 0.0;
+    sq[j] = qm * (double)c;
+    reinterpret_cast<uint32_t *>(sv)[j] = c;
+    n_in += c;
+    m1 += (unsigned long long)j * c;
+  }
+  for (int j = tid; j < nb; j += kWakeThreads) {  // the stores, from the thread's own shared-memory copy
+    const uint32_t c = reinterpret_cast<const uint32_t *>(sv)[j];
+    if (split == 0) A.hist_last[(size_t)b * nb + j] = c;
+    if (S == 1) A.hist[(size_t)b * nb + j] = 0u;
+  }
+  if (tid < 24) sw[tid < 16 ? tid - 16 : nb + tid - 16] = 0.0;
+  if (FUSED && A.mode == 0 && A.R > 0)
+    for (int j = tid; j < A.M; j += kWakeThreads) sB[j] = A.bucket[j];
+  if (S > 1) {  // the last split to have read the counts clears them (nobody waits for anybody)
+    __syncthreads();
+    if (tid == 0) s_last = (atomicAdd(&A.rd_cnt[b], 1u) == (uint32_t)(S - 1));
+    __syncthreads();
+    if (s_last) {
+      for (int j = tid; j < nb; j += kWakeThreads) A.hist[(size_t)b * nb + j] = 0u;
+      if (tid == 0) A.rd_cnt[b] = 0u;
+    }
+  }
+  if (follow && split == 0) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      n_in += __shfl_down_sync(0xffffffffu, n_in, o);
+      m1 += __shfl_down_sync(0xffffffffu, m1, o);
+    }
+    if (lane == 0) { s_cnt[warp][0] = n_in; s_cnt[warp][1] = m1; }
+  }
+  __syncthreads();
+  if (follow && split == 0 && tid == 0) {
+    // D31: the window moves by rint(centroid in bins - nb/2) whole bins (half up), exact integer arithmetic
+    long long N = 0, S1 = 0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) { N += (long long)s_cnt[w][0]; S1 += (long long)s_cnt[w][1]; }
+    long long step = 0;
+    if (N > 0) {
+      const long long num = 2 * S1 + (2 - (long long)nb) * N, den = 2 * N;
+      step = num / den;
+      if (num % den != 0 && num < 0) step -= 1;
+    }
+    long long s_new = (long long)s_used + step;
+    s_new = s_new > A.s_max ? A.s_max : (s_new < -(long long)A.s_max ? -(long long)A.s_max : s_new);
+    double lo_h = __dadd_rn(A.tau_lo, __dmul_rn((double)s_used, A.Delta));
+    double lo_n = __dadd_rn(A.tau_lo, __dmul_rn((double)s_new, A.Delta));
+    if (lo_h == 0.0) lo_h = -0.0;
+    if (lo_n == 0.0) lo_n = -0.0;
+    A.s_hist[b] = s_used;
+    A.lo_hist[b] = lo_h;
+    A.s_next[b] = (int32_t)s_new;
+    A.lo_next[b] = lo_n;
+  }
+  // S7: close the moments the pass gathered (state after turn n_done's kick): by the last thread of the CTA, beside
+  // the convolution of the others
+  if (split == 0 && tid == kWakeThreads - 1) {
+    const double N = (double)A.Np;
+    const double s1 = __ldcg(&A.mom_acc[b * 4 + 0]), s2 = __ldcg(&A.mom_acc[b * 4 + 1]);
+    const double s11 = __ldcg(&A.mom_acc[b * 4 + 2]), s22 = __ldcg(&A.mom_acc[b * 4 + 3]);
+    const double no = (double)__ldcg(&A.nout_acc[b]);
+    const double iN = 1.0 / N;
+    const double mt = s1 * iN, md = s2 * iN;
+    const double vt = fmax(s11 * iN - mt * mt, 0.0), vd = fmax(s22 * iN - md * md, 0.0);
+    double m[6] = {N - no, no, mt, md, sqrt(vt), sqrt(vd)};
+#pragma unroll
+    for (int k = 0; k < 6; ++k) A.mom_last[b * 6 + k] = m[k];
+    if (A.mom_log && n_done >= 1u && (int64_t)n_done <= A.log_cap) {
+#pragma unroll
+      for (int k = 0; k < 6; ++k) A.mom_log[((size_t)(n_done - 1u) * A.M + b) * 6 + k] = m[k];
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) A.mom_acc[b * 4 + k] = 0.0;
+    A.nout_acc[b] = 0ull;
+  }
+  if (A.mode != 0) return;
+
+  // S6 sources: a[b][r] = sum_k q[k] exp(-lambda_r c_k).  One warp per resonator, counted from the LAST warp down (the
+  // first warps carry the convolution's heaviest tasks); shuffles only, no block barrier.
+  for (int r = NW - 1 - warp; r < A.R && split == 0; r += NW) {
+    double are = 0.0, aim = 0.0;
+#pragma unroll 4
+    for (int k = lane; k < nb; k += 32) {
+      const cplx e = pE[(size_t)r * nb + k];
+      are = fma(sq[k], e.re, are);
+      aim = fma(sq[k], e.im, aim);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      are += __shfl_xor_sync(0xffffffffu, are, o);
+      aim += __shfl_xor_sync(0xffffffffu, aim, o);
+    }
+    if (lane == 0) {
+      cplx a{are, aim};
+      if (follow) a = cmul(a, A.shift_src[(size_t)r * (2 * A.s_max + 1) + (s_used + A.s_max)]);  // bin centres at their own window
+      A.a_cur[(size_t)b * A.R + r] = a;
+      A.ring_a[((size_t)(n % (uint32_t)A.slots) * A.M + b) * A.R + r] = a;
+      if (FUSED) st_release_u32(&A.a_ready[(size_t)b * A.R + r], n);  // later bunches' gathers wait for it
+    }
+  }
+
+  // S5: V_SR[j] = sum_{k<=j} w[j-k] q[k], register-blocked.  Outputs come in blocks of NO = 8 consecutive bins; block pi
+  // is paired with block J-1-pi so that every pair has nb + 8 (+-8) terms; a pair is dealt to SEG lanes of one warp, lane
+  // g taking the g-th segment of each block's k-range with the NO table values it needs in a sliding register window
+  // (per k: two shared-memory loads and NO independent DFMAs -- 2 bytes of shared-memory traffic per multiply-add, where
+  // one output per thread moves 16; the load/store unit, not the fp64 pipe, bounds this loop); a shuffle reduction over
+  // the SEG lanes closes the sums.  SEG is the largest power of two that keeps all threads of the bunch's S CTAs busy;
+  // segment lengths are odd, so that the lanes of a pair fall into different banks.
+  if (A.w) {
+    constexpr int NO = 8;
+    const int J = (nb + NO - 1) / NO, pairs = (J + 1) >> 1;
+    const int nthreads = S * kWakeThreads;
+    int seg = 1, lg = 0;
+    while (seg < 32 && 2 * seg * pairs <= nthreads) { seg <<= 1; ++lg; }
+    const int tasks = pairs << lg;
+    const int g = tid & (seg - 1);
+    for (int base = 0; base < tasks; base += nthreads) {  // uniform over the CTA: the shuffles need every lane
+      const int task = base + split * kWakeThreads + tid;
+      const bool act = task < tasks;
+      const int pi = act ? (task >> lg) : 0;
+#pragma unroll 1
+      for (int h = 0; h < 2; ++h) {
+        const int jb = h ? J - 1 - pi : pi;
+        const int j0 = NO * jb;
+        const bool skip = h && jb == pi;                      // the middle block of an odd J is its own partner
+        const int kend = (act && !skip) ? min(j0 + NO, nb) : 0;  // k in [0, kend)
+        const int len = ((kend + seg - 1) >> lg) | 1;
+        const int ka = min(g * len, kend), kb = min(ka + len, kend);
+        const double *wp = sw + (j0 - ka);  // wp[i] = w[j0 + i - ka]
+        double w[NO], a[NO];
+#pragma unroll
+        for (int i = 0; i < NO; ++i) { w[i] = wp[i]; a[i] = 0.0; }
+        // NO values of k per round: all 2 NO loads first, then NO x NO multiply-adds on static register indices (the
+        // window slides by renaming, not by moves); beyond kb the charges are taken as zero
+#pragma unroll 1
+        for (int k = ka; k < kb; k += NO) {
+          double q[NO], nw[NO];
+#pragma unroll
+          for (int t = 0; t < NO; ++t) {
+            q[t] = (k + t < kb) ? sq[k + t] : 0.0;
+            nw[t] = wp[-1 - t];  // w[j0 - k - 1 - t]
+          }
+#pragma unroll
+          for (int t = 0; t < NO; ++t)
+#pragma unroll
+            for (int i = 0; i < NO; ++i) a[i] = fma(i >= t ? w[i - t] : nw[t - i - 1], q[t], a[i]);
+#pragma unroll
+          for (int i = 0; i < NO; ++i) w[i] = nw[NO - 1 - i];
+          wp -= NO;
+        }
+        for (int o = seg >> 1; o > 0; o >>= 1) {
+#pragma unroll
+          for (int i = 0; i < NO; ++i) a[i] += __shfl_xor_sync(0xffffffffu, a[i], o);
+        }
+        if (act && g == 0 && !skip) {
+#pragma unroll
+          for (int i = 0; i < NO; ++i) {
+            const int j = j0 + i;
+            if (j < nb) {
+              A.Vsr[(size_t)b * nb + j] = a[i];
+              if (!SPLIT) sv[j] = a[i];
+            }
+          }
+        }
+      }
+    }
+  } else {
+    for (int j = split * kWakeThreads + tid; j < nb; j += S * kWakeThreads) { A.Vsr[(size_t)b * nb + j] = 0.0; sv[j] = 0.0; }
+  }
+  if (S > 1) {  // the last split to finish gathers the bunch's V_SR and goes on alone
+    __syncthreads();
+    if (tid == 0) {
+      __threadfence();
+      s_last = (atomicAdd(&A.wr_cnt[b], 1u) == (uint32_t)(S - 1));
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (tid == 0) A.wr_cnt[b] = 0u;
+    for (int j = tid; j < nb; j += kWakeThreads) sv[j] = __ldcg(&A.Vsr[(size_t)b * nb + j]);
+  }
+  __syncthreads();
+  for (int k = tid; k < nb + 2; k += kWakeThreads) {
+    WakeCell c{0.0, 0.0};
+    if (A.gather == 1) {
+      if (k <= nb) {
+        const double lo = sv[k > 0 ? k - 1 : 0], hi = sv[k < nb ? k : nb - 1];
+        c.mid = 0.5 * (lo + hi);
+        c.dif = hi - lo;
+      }
+    } else if (k < nb) {
+      c.mid = sv[k];
+    }
+    A.cellSR[(size_t)b * (nb + 2) + k] = c;
+  }
+
+  const int M = A.M, R = A.R, K = A.K;
+  if constexpr (FUSED) {
+    // S6, one-launch turn: the phasor bunch b sees, gathered by the bunch's own closing CTA as the pairwise sum itself --
+    //   P[b][r] = gd_r[s_b - s_0] sum_{k=1..min(K,n-1)} A_{n-k}[r] g_hist[k][r] + sum_{j<b} a_j[r] gd_r[s_b - s_j],
+    // gd_r[d] = exp(lambda_r d T_rf) a host table over the bucket distance (every factor decays).  The sources a_j of the
+    // bunches ahead are awaited one by one (flags a_ready, set by their closing CTAs: CTAs of a lower index, dispatched
+    // earlier, so they are resident or done -- the wait cannot deadlock); no CTA waits for the whole grid, and the scan of
+    // the two-launch turn, which ran alone on the device after the last bunch, is gone.  A resonator is dealt to
+    // NW / R warps (fixed order of summation: deterministic).
+    __shared__ cplx s_part[NW];
+    if (R > 0) {
+      const int nq = NW / R;                 // warps per resonator (R <= NW)
+      const int r = warp % R, q = warp / R;  // warps >= nq R idle
+      const int Kh = (int)min((uint32_t)K, n - 1u);
+      const int n_el = b + Kh;
+      const int sb = sB[b];
+      cplx acc{0.0, 0.0};
+      if (q < nq) {
+        const cplx *gdr = A.gd + (size_t)r * A.h;
+        const cplx g0 = gdr[sb - sB[0]];
+#pragma unroll 2
+        for (int e = q * 32 + lane; e < n_el; e += 32 * nq) {
+          if (e < b) {
+            wait_turn(&A.a_ready[(size_t)e * R + r], n);
+            acc = cfma(__ldcg_cplx(&A.ring_a[((size_t)(n % (uint32_t)A.slots) * M + e) * R + r]), gdr[sb - sB[e]], acc);
+          } else {
+            const int k = e - b + 1;
+            wait_turn(A.agg_ready, n - 1u);
+            acc = cfma(__ldcg_cplx(&A.ring_A[(size_t)((n - (uint32_t)k) % (uint32_t)A.slots) * R + r]),
+                       cmul(A.g_hist[(size_t)(k - 1) * R + r], g0), acc);
+          }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          acc.re += __shfl_xor_sync(0xffffffffu, acc.re, o);
+          acc.im += __shfl_xor_sync(0xffffffffu, acc.im, o);
+        }
+      }
+      if (lane == 0) s_part[warp] = acc;
+      __syncthreads();
+      if (tid < R) {
+        cplx Pb{0.0, 0.0};
+        for (int w = tid; w < nq * R; w += R) { Pb.re += s_part[w].re; Pb.im += s_part[w].im; }
+        // the phasor as bunch b's own window sees it: the pass expands Re[cellF_r P], cellF built on the unshifted grid
+        A.P[(size_t)b * R + tid] = follow ? cmul(Pb, A.shift_wit[(size_t)tid * (2 * A.s_max + 1) + (s_used + A.s_max)]) : Pb;
+      }
+    }
+    // the bunch is complete: publish it, take a ticket; the CTA that closes the last bunch closes the turn
+    __syncthreads();
+    if (tid == 0) {
+      __threadfence();
+      st_release_u32(&A.bunch_ready[b], n);
+      s_last = (atomicAdd(&A.ctrl->ticket, 1u) == (uint32_t)(M - 1));
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    // A_n[r] = sum_j a_j[r] exp(lambda_r (s_{M-1} - s_j) T_rf): the aggregate later turns' seeds are built from
+    if (R > 0) {
+      const int nq = NW / R, r = warp % R, q = warp / R;
+      cplx acc{0.0, 0.0};
+      if (q < nq) {
+#pragma unroll 2
+        for (int j = q * 32 + lane; j < M; j += 32 * nq)
+          acc = cfma(__ldcg_cplx(&A.ring_a[((size_t)(n % (uint32_t)A.slots) * M + j) * R + r]), A.g_tail[(size_t)j * R + r], acc);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          acc.re += __shfl_xor_sync(0xffffffffu, acc.re, o);
+          acc.im += __shfl_xor_sync(0xffffffffu, acc.im, o);
+        }
+      }
+      if (lane == 0) s_part[warp] = acc;
+      __syncthreads();
+      if (tid < R) {
+        cplx An{0.0, 0.0};
+        for (int w = tid; w < nq * R; w += R) { An.re += s_part[w].re; An.im += s_part[w].im; }
+        A.ring_A[(size_t)(n % (uint32_t)A.slots) * R + tid] = An;
+      }
+    }
+    __syncthreads();
+    if (tid == 0) {
+      __threadfence();
+      st_release_u32(A.agg_ready, n);
+      A.ctrl->ticket = 0u;
+      A.ctrl->kick_pending = 1u;
+      A.ctrl->turn = n;
+    }
+  } else {
+  // last-CTA-done election: the CTA that sees every other CTA's ticket closes the turn.  Barrier, then ONE thread's
+  // fence and ticket (the pattern of a cooperative grid barrier: the barrier orders the CTA's writes before the fence).
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    s_last = (atomicAdd(&A.ctrl->ticket, 1u) == (uint32_t)(A.M - 1));
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+
+  // S6: P_0 = G_n (history seed), P_{j+1} = (P_j + a_j) g_j -- an inclusive scan of affine maps over the fill
+  // pattern; every factor is exp(lambda * positive time), |g| < 1.  One WARP per resonator, all resonators at once,
+  // shuffles only (no block barrier inside): this tail runs alone on the device, so its latency is the turn's.  Its
+  // operands -- a, g_step, g_tail of every bunch and resonator -- are first staged in shared memory by ALL threads (one
+  // trip to L2 instead of one per four bunches of a lane's run) if the launch's shared memory holds them.
+  const int total = M * R;
+  const cplx *pa = A.a_cur, *pgs = A.g_step, *pgt = A.g_tail;
+  const bool staged = scan_smem_bytes(M, R) <= (size_t)smem_bytes;
+  if (staged) {
+    cplx *sa = reinterpret_cast<cplx *>(smem_d), *sgs = sa + total, *sgt = sgs + total;
+#pragma unroll 2
+    for (int i = tid; i < total; i += kWakeThreads) {
+      sa[i] = __ldcg_cplx(&A.a_cur[i]);
+      sgs[i] = A.g_step[i];
+      sgt[i] = A.g_tail[i];
+    }
+    pa = sa; pgs = sgs; pgt = sgt;
+    __syncthreads();
+  }
+  const int run = (M + 31) / 32;  // consecutive bunches per lane
+  for (int r = warp; r < R; r += NW) {
+    // G_n = sum_{k=1..min(K,n-1)} A_{n-k} exp(lambda (k T0 - span)): lanes take k = lane+1, lane+33, ...
+    cplx G{0.0, 0.0};
+    for (int k = lane + 1; k <= K && (int64_t)n - k >= 1; k += 32)
+      G = cfma(__ldcg_cplx(&A.ring_A[(size_t)((n - (uint32_t)k) % (uint32_t)A.slots) * R + r]), A.g_hist[(size_t)(k - 1) * R + r], G);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      G.re += __shfl_xor_sync(0xffffffffu, G.re, o);
+      G.im += __shfl_xor_sync(0xffffffffu, G.im, o);
+    }
+    // lane-local composite of its run of bunches, and this turn's own aggregate.  The run is walked four bunches
+    // at a time with all of a chunk's loads issued before its arithmetic.
+    const int j_lo = lane * run, j_hi = min(j_lo + run, M);
+    Affine loc{cplx{1.0, 0.0}, cplx{0.0, 0.0}};
+    cplx own{0.0, 0.0};
+    for (int j0 = j_lo; j0 < j_hi; j0 += 4) {
+      cplx a[4], gt[4], gs[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int j = min(j0 + u, M - 1);
+        a[u] = staged ? pa[(size_t)j * R + r] : __ldcg_cplx(&pa[(size_t)j * R + r]);
+        gt[u] = pgt[(size_t)j * R + r];
+        gs[u] = pgs[(size_t)j * R + r];
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int j = j0 + u;
+        if (j < j_hi) {
+          own = cfma(a[u], gt[u], own);
+          if (j + 1 < M) loc = compose(loc, Affine{gs[u], cmul(a[u], gs[u])});
+        }
+      }
+    }
+    // inclusive warp scan of the lane composites (Kogge-Stone on shuffles), then the exclusive prefix applied to G
+    Affine inc = loc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      Affine up;
+      up.g.re = __shfl_up_sync(0xffffffffu, inc.g.re, o); up.g.im = __shfl_up_sync(0xffffffffu, inc.g.im, o);
+      up.c.re = __shfl_up_sync(0xffffffffu, inc.c.re, o); up.c.im = __shfl_up_sync(0xffffffffu, inc.c.im, o);
+      if (lane >= o) inc = compose(up, inc);
+    }
+    Affine pre;
+    pre.g.re = __shfl_up_sync(0xffffffffu, inc.g.re, 1); pre.g.im = __shfl_up_sync(0xffffffffu, inc.g.im, 1);
+    pre.c.re = __shfl_up_sync(0xffffffffu, inc.c.re, 1); pre.c.im = __shfl_up_sync(0xffffffffu, inc.c.im, 1);
+    cplx Pj = (lane > 0) ? cfma(pre.g, G, pre.c) : G;
+    for (int j0 = j_lo; j0 < j_hi; j0 += 4) {
+      cplx a[4], gs[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int j = min(j0 + u, M - 1);
+        a[u] = staged ? pa[(size_t)j * R + r] : __ldcg_cplx(&pa[(size_t)j * R + r]);
+        gs[u] = pgs[(size_t)j * R + r];
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int j = j0 + u;
+        if (j < j_hi) {
+          // the phasor as bunch j's own window sees it: the pass expands Re[cellF_r P], cellF built on the unshifted grid
+          A.P[(size_t)j * R + r] = follow ? cmul(Pj, A.shift_wit[(size_t)r * (2 * A.s_max + 1) + (__ldcg(&A.s_hist[j]) + A.s_max)]) : Pj;
+          if (j + 1 < M) Pj = cmul(cadd(Pj, a[u]), gs[u]);
+        }
+      }
+    }
+    // A_n = sum_j a_j exp(lambda (s_{M-1}-s_j) T_rf)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      own.re += __shfl_xor_sync(0xffffffffu, own.re, o);
+      own.im += __shfl_xor_sync(0xffffffffu, own.im, o);
+    }
+    if (lane == 0) A.ring_A[(size_t)(n % (uint32_t)A.slots) * R + r] = own;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    A.ctrl->ticket = 0u;
+    A.ctrl->kick_pending = 1u;
+    A.ctrl->turn = n;
+  }
+  }  // !FUSED
+}
+
+__global__ void __launch_bounds__(kWakeThreads, 3) k_wake(const __grid_constant__ WakeArgs A) {
+  extern __shared__ double smem_wake[];
+  griddep_wait();               // the pass of this turn is complete (counts, moment sums)
+  griddep_launch_dependents();  // the next pass may become resident: it stages what does not depend on this kernel
+  if (A.S > 1) wake_body<true, false>(A, (int)blockIdx.x, (int)blockIdx.y, smem_wake, A.smem_wake_bytes);
+  else if (A.gather_P) wake_body<false, true>(A, (int)blockIdx.x, 0, smem_wake, A.smem_wake_bytes);
+  else wake_body<false, false>(A, (int)blockIdx.x, 0, smem_wake, A.smem_wake_bytes);
+}
+// out of line in the pass, so that its registers are not the hot loop's
+__device__ __noinline__ void wake_bunch_fused(const WakeArgs &A, int b, double *smem_d) {
+  wake_body<false, true>(A, b, 0, smem_d, A.smem_pass_bytes);
+}
+
+
 // ------------------------------------------------------------------ fused particle pass
 // MAP = true : S0 S7 | S1 S2 S3 | S4      (a tracked turn)
 // MAP = false: S0 S7 |          | S4      (flush of the pending kick before the state is observed)
@@ -175,7 +716,8 @@ __device__ __forceinline__ bool in_window(double t, uint32_t hi_nb) { return (ui
 // dif = V[kk]-V[kk-1], with V[-1] := V[0] and V[nb] := V[nb-1] (constant outer half bins).  Cell nb+1 is zero and
 // serves every particle outside the window (no kick, D11), which keeps the step branch-free.
 template <bool MAP, bool RAD, int GATHER, int NCAV, int NPAIR>
-__global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const __grid_constant__ Args A) {
+__global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const __grid_constant__ Args A,
+                                                                             const __grid_constant__ WakeArgs Wk) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int NP = 2 * NPAIR;                       // particles per thread and iteration
   constexpr uint32_t STRIDE = kPassThreads * NPAIR;   // pairs per CTA and iteration (one stage)
@@ -225,14 +767,18 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
       bulk_g2s(dst, gT + pc, bytes, bar);
       bulk_g2s(dst + STRIDE * 16u, gD + pc, bytes, bar);
     };
-    if (tid == 0)
+    const bool fused = MAP && A.fused != 0;
+    if (tid == 0 && !fused)
       for (uint32_t k = 0; k + 1u < (uint32_t)kStages && k < n_it; ++k) issue(k);
 
     // Everything above is independent of the wake kernel before this pass (barriers, log table, the first particle
     // stages: the particles were last written by the pass before it, which that wake kernel waited for); its output --
-    // the control words, the gather cells, the phasors, the windows -- is read from here on.
-    griddep_launch_dependents();  // the wake kernel after this pass may become resident; it waits for this grid itself
+    // the control words, the gather cells, the phasors, the windows -- is read from here on.  In the one-launch turn the
+    // predecessor is the pass before, which wrote the particles: the first stages are issued after the wait.
+    griddep_launch_dependents();  // the kernel after this pass may become resident; it waits for this grid itself
     griddep_wait();
+    if (tid == 0 && fused)
+      for (uint32_t k = 0; k + 1u < (uint32_t)kStages && k < n_it; ++k) issue(k);
     const uint32_t n = A.ctrl->turn + 1u;  // the turn this pass tracks (Philox counter word, D24)
     const bool have_kick = A.ctrl->kick_pending != 0u;
     // window of the wake being applied (S0) and window this pass bins with (S4); the flush pass re-bins on the former
@@ -476,349 +1022,29 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
       const uint32_t c = sH[j];
       if (c) atomicAdd(&A.hist[(size_t)b * nb + j], c);
     }
-  }
-}
-
-// ------------------------------------------------------------------ wake
-struct WakeArgs {
-  int32_t M, nb, R, K;
-  int32_t S;               // CTAs per bunch (grid.y): the outputs of the convolution are dealt out over them
-  uint32_t *rd_cnt, *wr_cnt;  // [M] splits that have read the counts / written their share of V_SR (S > 1)
-  uint32_t Np;
-  int32_t mode;            // 0: full turn (S5, S6, bump the turn counter); 1: finalise counts and moments only
-  const double *qm;        // [M]      macro-particle charge Q_b / N_p
-  const double *w;         // [nb]     short-range table w_k = W(k Delta); nullptr: none
-  const cplx *Esrc;        // [R][nb]  exp(-lambda_r c_k)
-  const cplx *g_step;      // [M][R]   exp(lambda_r (s_{j+1}-s_j) T_rf), j < M-1
-  const cplx *g_tail;      // [M][R]   exp(lambda_r (s_{M-1}-s_j) T_rf)
-  const cplx *g_hist;      // [K][R]   exp(lambda_r (k T0 - (s_{M-1}-s_0) T_rf)), k = 1..K
-  uint32_t *hist;          // [M][nb]  in: counts of this turn; out: zero
-  uint32_t *hist_last;     // [M][nb]  out: counts of this turn
-  double *Vsr;             // [M][nb]
-  WakeCell *cellSR;        // [M][nb+2] gather cells of Vsr (what the pass stages)
-  int32_t gather;          // 1 linear, 0 nearest grid point
-  // bunch-following window (D31); window_mode 0: the arrays below keep their initial values
-  int32_t window_mode, s_max;
-  double tau_lo, Delta;
-  int32_t *s_hist, *s_next;   // [M] window shift in bins: of this turn's histogram / of the next binning
-  double *lo_hist, *lo_next;  // [M] tau_lo + s Delta (0 stored as -0.0, see in_window())
-  const cplx *shift_src;      // [R][2 s_max + 1] exp(-lambda_r s Delta), s = -s_max..s_max
-  const cplx *shift_wit;      // [R][2 s_max + 1] exp(+lambda_r s Delta)
-  cplx *a_cur;             // [M][R]   source phasors of this turn
-  cplx *ring_a;            // [K+1][M][R] slot n % (K+1)
-  cplx *ring_A;            // [K+1][R]    per-turn aggregates, slot n % (K+1)
-  cplx *P;                 // [M][R]
-  double *mom_acc;         // [M][4]  in: sums gathered by the pass; out: zero
-  unsigned long long *nout_acc;  // [M]
-  double *mom_last;        // [M][6]
-  double *mom_log;         // [cap][M][6] or nullptr
-  int64_t log_cap;
-  Ctrl *ctrl;
-};
-
-// L2 load of a complex number written earlier in this kernel by another CTA (never through a stale L1 line)
-__device__ __forceinline__ cplx __ldcg_cplx(const cplx *p) {
-  const double2 v = __ldcg(reinterpret_cast<const double2 *>(p));
-  return cplx{v.x, v.y};
-}
-
-// affine map x -> g x + c over the complex numbers; (first o second)(x) = second(first(x))
-struct Affine {
-  cplx g, c;
-};
-__device__ __forceinline__ Affine compose(const Affine &first, const Affine &second) {
-  return Affine{cmul(first.g, second.g), cfma(first.c, second.g, second.c)};
-}
-
-__global__ void __launch_bounds__(kWakeThreads) k_wake(const __grid_constant__ WakeArgs A) {
-  extern __shared__ double smem_d[];
-  double *sq = smem_d;         // [nb] charge per bin
-  double *sw = smem_d + A.nb;  // [nb] wake table
-  double *sv = smem_d + 2 * A.nb;  // [nb] V_SR of this bunch
-  __shared__ bool s_last;
-  __shared__ unsigned long long s_cnt[kWakeThreads / 32][2];
-
-  const int tid = threadIdx.x;
-  const int b = blockIdx.x;
-  const int split = blockIdx.y, S = A.S;  // few bunches: S CTAs share a bunch (split 0 also does the per-bunch work)
-  const int nb = A.nb;
-  griddep_wait();               // the pass of this turn is complete (counts, moment sums)
-  griddep_launch_dependents();  // the next pass may become resident: it stages what does not depend on this kernel
-  const uint32_t n_done = A.ctrl->turn;  // completed turns; the turn being closed is n_done + 1
-  const uint32_t n = n_done + 1u;
-
-  // counts -> charges; keep a copy of the counts; clear the accumulator for the next pass
-  const double qm = A.qm[b];
-  const bool follow = A.mode == 0 && A.window_mode == 1;
-  const int32_t s_used = follow ? A.s_next[b] : 0;   // the window the pass binned this turn with
-  unsigned long long n_in = 0ull, m1 = 0ull;         // sum c_k, sum k c_k
-  for (int j = tid; j < nb; j += kWakeThreads) {
-    const uint32_t c = A.hist[(size_t)b * nb + j];
-    if (split == 0) A.hist_last[(size_t)b * nb + j] = c;
-    if (S == 1) A.hist[(size_t)b * nb + j] = 0u;
-    sq[j] = qm * (double)c;
-    n_in += c;
-    m1 += (unsigned long long)j * c;
-    if (A.mode == 0 && A.w) sw[j] = A.w[j];
-  }
-  if (S > 1) {  // the last split to have read the counts clears them (nobody waits for anybody)
-    __syncthreads();
-    if (tid == 0) s_last = (atomicAdd(&A.rd_cnt[b], 1u) == (uint32_t)(S - 1));
-    __syncthreads();
-    if (s_last) {
-      for (int j = tid; j < nb; j += kWakeThreads) A.hist[(size_t)b * nb + j] = 0u;
-      if (tid == 0) A.rd_cnt[b] = 0u;
-    }
-  }
-  if (follow && split == 0) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      n_in += __shfl_down_sync(0xffffffffu, n_in, o);
-      m1 += __shfl_down_sync(0xffffffffu, m1, o);
-    }
-    if ((tid & 31) == 0) { s_cnt[tid >> 5][0] = n_in; s_cnt[tid >> 5][1] = m1; }
-  }
-  __syncthreads();
-  if (follow && split == 0 && tid == 0) {
-    // D31: the window moves by rint(centroid in bins - nb/2) whole bins (half up), exact integer arithmetic
-    long long N = 0, S1 = 0;
-#pragma unroll
-    for (int w = 0; w < kWakeThreads / 32; ++w) { N += (long long)s_cnt[w][0]; S1 += (long long)s_cnt[w][1]; }
-    long long step = 0;
-    if (N > 0) {
-      const long long num = 2 * S1 + (2 - (long long)nb) * N, den = 2 * N;
-      step = num / den;
-      if (num % den != 0 && num < 0) step -= 1;
-    }
-    long long s_new = (long long)s_used + step;
-    s_new = s_new > A.s_max ? A.s_max : (s_new < -(long long)A.s_max ? -(long long)A.s_max : s_new);
-    double lo_h = __dadd_rn(A.tau_lo, __dmul_rn((double)s_used, A.Delta));
-    double lo_n = __dadd_rn(A.tau_lo, __dmul_rn((double)s_new, A.Delta));
-    if (lo_h == 0.0) lo_h = -0.0;
-    if (lo_n == 0.0) lo_n = -0.0;
-    A.s_hist[b] = s_used;
-    A.lo_hist[b] = lo_h;
-    A.s_next[b] = (int32_t)s_new;
-    A.lo_next[b] = lo_n;
-  }
-  // S7: close the moments the pass gathered (state after turn n_done's kick)
-  // by the last thread of the CTA: its warp has no convolution work unless nb > 448, so this serial stretch
-  // (a division, two square roots) runs beside the convolution instead of ahead of it
-  if (split == 0 && tid == kWakeThreads - 1) {
-    const double N = (double)A.Np;
-    const double s1 = A.mom_acc[b * 4 + 0], s2 = A.mom_acc[b * 4 + 1];
-    const double s11 = A.mom_acc[b * 4 + 2], s22 = A.mom_acc[b * 4 + 3];
-    const double no = (double)A.nout_acc[b];
-    const double iN = 1.0 / N;
-    const double mt = s1 * iN, md = s2 * iN;
-    const double vt = fmax(s11 * iN - mt * mt, 0.0), vd = fmax(s22 * iN - md * md, 0.0);
-    double m[6] = {N - no, no, mt, md, sqrt(vt), sqrt(vd)};
-#pragma unroll
-    for (int k = 0; k < 6; ++k) A.mom_last[b * 6 + k] = m[k];
-    if (A.mom_log && n_done >= 1u && (int64_t)n_done <= A.log_cap) {
-#pragma unroll
-      for (int k = 0; k < 6; ++k) A.mom_log[((size_t)(n_done - 1u) * A.M + b) * 6 + k] = m[k];
-    }
-#pragma unroll
-    for (int k = 0; k < 4; ++k) A.mom_acc[b * 4 + k] = 0.0;
-    A.nout_acc[b] = 0ull;
-  }
-  if (A.mode != 0) return;
-
-  // S6 sources: a[b][r] = sum_k q[k] exp(-lambda_r c_k).  One warp per resonator (shuffles only, no block
-  // barrier); the other warps go straight to the convolution.
-  for (int r = tid >> 5; r < A.R && split == 0; r += kWakeThreads / 32) {
-    double are = 0.0, aim = 0.0;
-    for (int k = tid & 31; k < nb; k += 32) {
-      const cplx e = A.Esrc[(size_t)r * nb + k];
-      are = fma(sq[k], e.re, are);
-      aim = fma(sq[k], e.im, aim);
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      are += __shfl_xor_sync(0xffffffffu, are, o);
-      aim += __shfl_xor_sync(0xffffffffu, aim, o);
-    }
-    if ((tid & 31) == 0) {
-      cplx a{are, aim};
-      if (follow) a = cmul(a, A.shift_src[(size_t)r * (2 * A.s_max + 1) + (s_used + A.s_max)]);  // bin centres at their own window
-      A.a_cur[(size_t)b * A.R + r] = a;
-      A.ring_a[((size_t)(n % (uint32_t)(A.K + 1)) * A.M + b) * A.R + r] = a;
-    }
-  }
-
-  // S5: V_SR[j] = sum_{k<=j} w[j-k] q[k].  Outputs j and nb-1-j are paired so that every thread does nb+1 terms;
-  // each sum runs on four interleaved accumulators (k mod 4), so that the 8-cycle DFMA latency and the
-  // shared-memory loads of consecutive terms overlap.
-  if (A.w && S > 1) {
-    // few bunches: the chain of a single sum is what costs.  Eight lanes share an output pair, lane g takes the terms
-    // k = g mod 8 of both sums, and a shuffle reduction closes them: 32 pairs per CTA, S CTAs per bunch.
-    constexpr int KS = 8;
-    const int g = tid % KS;
-    const int pairs = (nb + 1) / 2, per_cta = (pairs + S - 1) / S;                    // output pairs of this split
-    const int rounds = (per_cta + kWakeThreads / KS - 1) / (kWakeThreads / KS);       // uniform over the CTA: the
-    for (int i = 0; i < rounds; ++i) {                                                // shuffles need every lane
-      const int idx = split + S * (tid / KS + i * (kWakeThreads / KS));
-      const bool act = idx < pairs;
-      const int j1 = act ? idx : 0, j2 = act ? nb - 1 - idx : 0;
-      double a1 = 0.0, b1 = 0.0, a2 = 0.0, b2 = 0.0;
-      int k = g;
-      for (; k + KS <= j1; k += 2 * KS) { a1 = fma(sw[j1 - k], sq[k], a1); b1 = fma(sw[j1 - k - KS], sq[k + KS], b1); }
-      if (k <= j1) a1 = fma(sw[j1 - k], sq[k], a1);
-      k = g;
-      for (; k + KS <= j2; k += 2 * KS) { a2 = fma(sw[j2 - k], sq[k], a2); b2 = fma(sw[j2 - k - KS], sq[k + KS], b2); }
-      if (k <= j2) a2 = fma(sw[j2 - k], sq[k], a2);
-      double v1 = a1 + b1, v2 = a2 + b2;
-#pragma unroll
-      for (int o = KS / 2; o > 0; o >>= 1) {
-        v1 += __shfl_xor_sync(0xffffffffu, v1, o);
-        v2 += __shfl_xor_sync(0xffffffffu, v2, o);
+    if (MAP) {
+      if (!fused) return;
+      // One-launch turn: the CTA that completes bunch b (every other CTA of the bunch has flushed its counts and sums:
+      // barrier, one thread's fence, then the counter) builds the bunch's wake while other bunches still stream -- S5, the
+      // S6 source, the gather cells, the closing of S7, and the phasor P[b] gathered from the sources of the bunches ahead
+      // (wake_body<false, true>) -- in the shared memory of the particle stages, which are drained; the CTA that completes
+      // the last bunch adds up the turn's aggregate and bumps the turn.  Who may touch what, when: hist[b], mom_acc[b],
+      // cellSR[b], Vsr[b], P[b] and the windows of bunch b are written here only after ALL pass CTAs of bunch b are done
+      // with them (they read the cells and P[b] in their prologue); ring_A and the control words only after all CTAs of
+      // the grid are (the grid-wide ticket in wake_body); the next launch reads all of it after its griddepcontrol.wait,
+      // i.e. after this grid has completed.
+      __shared__ bool s_mine;
+      __syncthreads();
+      if (tid == 0) {
+        __threadfence();
+        s_mine = (atomicAdd(&A.bunch_done[b], 1u) == gridDim.x - 1u);
+        if (s_mine) A.bunch_done[b] = 0u;
       }
-      if (act && g == 0) {
-        A.Vsr[(size_t)b * nb + j1] = v1;
-        if (j2 != j1) A.Vsr[(size_t)b * nb + j2] = v2;
-      }
+      __syncthreads();
+      if (!s_mine) return;
+      __threadfence();
+      wake_bunch_fused(Wk, b, reinterpret_cast<double *>(smem_raw));
     }
-  } else if (A.w) {
-    for (int idx = split + S * tid; idx < (nb + 1) / 2; idx += S * kWakeThreads) {
-      const int j1 = idx, j2 = nb - 1 - idx;
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int j = h ? j2 : j1;
-        if (h && j2 == j1) break;
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-        int k = 0;
-        for (; k + 3 <= j; k += 4) {
-          a0 = fma(sw[j - k], sq[k], a0);
-          a1 = fma(sw[j - k - 1], sq[k + 1], a1);
-          a2 = fma(sw[j - k - 2], sq[k + 2], a2);
-          a3 = fma(sw[j - k - 3], sq[k + 3], a3);
-        }
-        for (; k <= j; ++k) a0 = fma(sw[j - k], sq[k], a0);
-        const double v = (a0 + a1) + (a2 + a3);
-        A.Vsr[(size_t)b * nb + j] = v;
-        sv[j] = v;
-      }
-    }
-  } else {
-    for (int j = split + S * tid; j < nb; j += S * kWakeThreads) { A.Vsr[(size_t)b * nb + j] = 0.0; sv[j] = 0.0; }
-  }
-  if (S > 1) {  // the last split to finish gathers the bunch's V_SR and goes on alone
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) s_last = (atomicAdd(&A.wr_cnt[b], 1u) == (uint32_t)(S - 1));
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    if (tid == 0) A.wr_cnt[b] = 0u;
-    for (int j = tid; j < nb; j += kWakeThreads) sv[j] = __ldcg(&A.Vsr[(size_t)b * nb + j]);
-  }
-  __syncthreads();
-  for (int k = tid; k < nb + 2; k += kWakeThreads) {
-    WakeCell c{0.0, 0.0};
-    if (A.gather == 1) {
-      if (k <= nb) {
-        const double lo = sv[k > 0 ? k - 1 : 0], hi = sv[k < nb ? k : nb - 1];
-        c.mid = 0.5 * (lo + hi);
-        c.dif = hi - lo;
-      }
-    } else if (k < nb) {
-      c.mid = sv[k];
-    }
-    A.cellSR[(size_t)b * (nb + 2) + k] = c;
-  }
-
-  // last-CTA-done election: the CTA that sees every other CTA's ticket closes the turn
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) s_last = (atomicAdd(&A.ctrl->ticket, 1u) == (uint32_t)(A.M - 1));
-  __syncthreads();
-  if (!s_last) return;
-  __threadfence();
-
-  // S6: P_0 = G_n (history seed), P_{j+1} = (P_j + a_j) g_j -- an inclusive scan of affine maps over the fill
-  // pattern; every factor is exp(lambda * positive time), |g| < 1.  One WARP per resonator, all resonators at once,
-  // shuffles only (no block barrier inside): this tail runs alone on the device, so its latency is the turn's.
-  const int M = A.M, R = A.R, K = A.K;
-  const int lane = tid & 31;
-  const int run = (M + 31) / 32;  // consecutive bunches per lane
-  for (int r = tid >> 5; r < R; r += kWakeThreads / 32) {
-    // G_n = sum_{k=1..min(K,n-1)} A_{n-k} exp(lambda (k T0 - span)): lanes take k = lane+1, lane+33, ...
-    cplx G{0.0, 0.0};
-    for (int k = lane + 1; k <= K && (int64_t)n - k >= 1; k += 32)
-      G = cfma(__ldcg_cplx(&A.ring_A[(size_t)((n - (uint32_t)k) % (uint32_t)(K + 1)) * R + r]), A.g_hist[(size_t)(k - 1) * R + r], G);
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      G.re += __shfl_xor_sync(0xffffffffu, G.re, o);
-      G.im += __shfl_xor_sync(0xffffffffu, G.im, o);
-    }
-    // lane-local composite of its run of bunches, and this turn's own aggregate.  The run is walked four bunches
-    // at a time with all of a chunk's loads issued before its arithmetic: each chunk costs one L2 round trip.
-    const int j_lo = lane * run, j_hi = min(j_lo + run, M);
-    Affine loc{cplx{1.0, 0.0}, cplx{0.0, 0.0}};
-    cplx own{0.0, 0.0};
-    for (int j0 = j_lo; j0 < j_hi; j0 += 4) {
-      cplx a[4], gt[4], gs[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int j = min(j0 + u, M - 1);
-        a[u] = __ldcg_cplx(&A.a_cur[(size_t)j * R + r]);
-        gt[u] = A.g_tail[(size_t)j * R + r];
-        gs[u] = A.g_step[(size_t)j * R + r];
-      }
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int j = j0 + u;
-        if (j < j_hi) {
-          own = cfma(a[u], gt[u], own);
-          if (j + 1 < M) loc = compose(loc, Affine{gs[u], cmul(a[u], gs[u])});
-        }
-      }
-    }
-    // inclusive warp scan of the lane composites (Kogge-Stone on shuffles), then the exclusive prefix applied to G
-    Affine inc = loc;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      Affine up;
-      up.g.re = __shfl_up_sync(0xffffffffu, inc.g.re, o); up.g.im = __shfl_up_sync(0xffffffffu, inc.g.im, o);
-      up.c.re = __shfl_up_sync(0xffffffffu, inc.c.re, o); up.c.im = __shfl_up_sync(0xffffffffu, inc.c.im, o);
-      if (lane >= o) inc = compose(up, inc);
-    }
-    Affine pre;
-    pre.g.re = __shfl_up_sync(0xffffffffu, inc.g.re, 1); pre.g.im = __shfl_up_sync(0xffffffffu, inc.g.im, 1);
-    pre.c.re = __shfl_up_sync(0xffffffffu, inc.c.re, 1); pre.c.im = __shfl_up_sync(0xffffffffu, inc.c.im, 1);
-    cplx Pj = (lane > 0) ? cfma(pre.g, G, pre.c) : G;
-    for (int j0 = j_lo; j0 < j_hi; j0 += 4) {
-      cplx a[4], gs[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int j = min(j0 + u, M - 1);
-        a[u] = __ldcg_cplx(&A.a_cur[(size_t)j * R + r]);
-        gs[u] = A.g_step[(size_t)j * R + r];
-      }
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int j = j0 + u;
-        if (j < j_hi) {
-          // the phasor as bunch j's own window sees it: the pass expands Re[cellF_r P], cellF built on the unshifted grid
-          A.P[(size_t)j * R + r] = follow ? cmul(Pj, A.shift_wit[(size_t)r * (2 * A.s_max + 1) + (__ldcg(&A.s_hist[j]) + A.s_max)]) : Pj;
-          if (j + 1 < M) Pj = cmul(cadd(Pj, a[u]), gs[u]);
-        }
-      }
-    }
-    // A_n = sum_j a_j exp(lambda (s_{M-1}-s_j) T_rf)
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      own.re += __shfl_xor_sync(0xffffffffu, own.re, o);
-      own.im += __shfl_xor_sync(0xffffffffu, own.im, o);
-    }
-    if (lane == 0) A.ring_A[(size_t)(n % (uint32_t)(K + 1)) * R + r] = own;
-  }
-  __syncthreads();
-  if (tid == 0) {
-    A.ctrl->ticket = 0u;
-    A.ctrl->kick_pending = 1u;
-    A.ctrl->turn = n;
   }
 }
 
@@ -882,10 +1108,17 @@ __global__ void k_aggregate_history(int M, int R, int K, const cplx *ring_a, con
   ring_A[(size_t)slot * R + r] = acc;
 }
 
-__global__ void k_set_ctrl(Ctrl *c, uint32_t turn, uint32_t pending) {
-  c->turn = turn;
-  c->ticket = 0u;
-  c->kick_pending = pending;
+// set the turn counter; every flag of the one-launch turn says "complete through `turn`"
+__global__ void k_set_ctrl(Ctrl *c, uint32_t turn, uint32_t pending, uint32_t *a_ready, int n_a, uint32_t *bunch_ready, int M,
+                           uint32_t *agg_ready, uint32_t *bunch_done) {
+  for (int i = threadIdx.x; i < n_a; i += blockDim.x) a_ready[i] = turn;
+  for (int i = threadIdx.x; i < M; i += blockDim.x) { bunch_ready[i] = turn; bunch_done[i] = 0u; }
+  if (threadIdx.x == 0) {
+    *agg_ready = turn;
+    c->turn = turn;
+    c->ticket = 0u;
+    c->kick_pending = pending;
+  }
 }
 __global__ void k_clear_pending(Ctrl *c) { c->kick_pending = 0u; }
 

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libmbt.so")
 SYMBOLS = [
     "mbt_create", "mbt_track", "mbt_moments", "mbt_destroy", "mbt_get_particles", "mbt_set_particles",
     "mbt_get_histogram", "mbt_get_wake", "mbt_get_moment_log", "mbt_get_lr_history", "mbt_set_lr_history", "mbt_get_window", "mbt_set_window",
-    "mbt_turn", "mbt_phi_s", "mbt_particle_stride", "mbt_plan_tiles", "mbt_device_pointers", "mbt_launch_count",
+    "mbt_turn", "mbt_phi_s", "mbt_particle_stride", "mbt_plan_tiles", "mbt_device_pointers", "mbt_invalidate", "mbt_launch_count", "mbt_launches_per_turn",
     "mbt_get_transverse", "mbt_set_transverse", "mbt_get_dipole", "mbt_get_transverse_wake", "mbt_moments_transverse",
     "mbt_get_rw_kick", "mbt_get_rw_history", "mbt_set_rw_history", "mbt_get_transverse_log",
     "mbt_last_track_seconds", "mbt_track_profiled", "mbt_philox_selftest", "mbt_normal_selftest", "mbt_last_error", "mbt_version",
@@ -66,11 +66,18 @@ class Transverse(C.Structure):
                 ("rw_amp_x", C.c_double), ("rw_amp_y", C.c_double), ("rw_turns", C.c_int32)]
 
 
+TUNING_FIELDS = ("tile_iters", "pairs_per_thread", "pdl", "stages6", "turn_mode", "verbose")
+
+
+class Tuning(C.Structure):
+    _fields_ = [(k, C.c_int32) for k in TUNING_FIELDS] + [("reserved", C.c_int32 * 2)]
+
+
 class Params(C.Structure):
     _fields_ = [("ring", Ring), ("n_cav", C.c_int32), ("cav", C.POINTER(Cavity)), ("rad", Radiation),
                 ("fill", Fill), ("wake", Wake), ("seed", C.c_uint64), ("log_capacity_turns", C.c_int64),
                 ("d_tau", C.c_void_p), ("d_delta", C.c_void_p), ("stream", C.c_void_p), ("device", C.c_int32),
-                ("trans", Transverse)]
+                ("trans", Transverse), ("tuning", Tuning)]
 
 
 class MbtError(RuntimeError):
@@ -108,7 +115,9 @@ def lib():
         L.mbt_phi_s.restype = C.c_double
         L.mbt_particle_stride.argtypes = [C.c_int64]
         L.mbt_particle_stride.restype = C.c_int64
-        L.mbt_plan_tiles.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.c_int32, C.POINTER(C.c_uint32), C.POINTER(C.c_int32)]
+        L.mbt_plan_tiles.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_uint32), C.POINTER(C.c_int32)]
+        L.mbt_invalidate.argtypes = [H]
+        L.mbt_launches_per_turn.argtypes = [H]
         L.mbt_device_pointers.argtypes = [H, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
         L.mbt_launch_count.argtypes = [H]
         L.mbt_launch_count.restype = C.c_int64
@@ -147,10 +156,11 @@ def particle_stride(n_per_bunch: int) -> int:
     return int(lib().mbt_particle_stride(int(n_per_bunch)))
 
 
-def plan_tiles(pairs_per_bunch, stride, n_bunches, slots):
+def plan_tiles(pairs_per_bunch, stride, n_bunches, slots, tile_iters=0):
     """(pairs per tile, tiles per bunch) a pass would get (host logic, no device needed)."""
     tp, nt = C.c_uint32(), C.c_int32()
-    _ck(lib().mbt_plan_tiles(int(pairs_per_bunch), int(stride), int(n_bunches), int(slots), C.byref(tp), C.byref(nt)))
+    _ck(lib().mbt_plan_tiles(int(pairs_per_bunch), int(stride), int(n_bunches), int(slots), int(tile_iters), C.byref(tp),
+                             C.byref(nt)))
     return tp.value, nt.value
 
 
@@ -169,8 +179,9 @@ def normal_selftest(seed, ctr):
     return out
 
 
-def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None, device=-1):
-    """Workload dict (paper_1809_00391_b200.workloads) -> (mbt_params, keep-alive list)."""
+def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None, device=-1, tuning=None):
+    """Workload dict (paper_1809_00391_b200.workloads) -> (mbt_params, keep-alive list).
+    tuning: dict of mbt_tuning members (mbt.h), e.g. dict(turn_mode=1); omitted members are 0 = the library's choice."""
     f, w = cfg["fill"], cfg["wake"]
     m = len(f["buckets"])
     bucket = (C.c_int32 * m)(*f["buckets"])
@@ -195,6 +206,10 @@ def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None
     p.d_delta = d_delta
     p.stream = stream
     p.device = int(device)
+    for k, v in (tuning or {}).items():
+        if k not in TUNING_FIELDS:
+            raise KeyError(k)
+        setattr(p.tuning, k, int(v))
     tr = cfg.get("transverse")
     tres = None
     if tr:
@@ -210,7 +225,7 @@ class Tracker:
     """One mbt_handle.  `d_tau` / `d_delta` / `stream` are raw device pointers / cudaStream_t values (ints),
     e.g. ``tensor.data_ptr()`` and ``torch.cuda.current_stream().cuda_stream``."""
 
-    def __init__(self, cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None, device=-1):
+    def __init__(self, cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None, device=-1, tuning=None):
         L = lib()
         f, w = cfg["fill"], cfg["wake"]
         self.M = len(f["buckets"])
@@ -219,7 +234,7 @@ class Tracker:
         self.R_lr = sum(1 for r in w["resonators"] if r["flags"] & 2)
         self.K = int(w["history_turns"]) if self.R_lr else 0
         self.K_rw = int((cfg.get("transverse") or {}).get("rw_turns", 0))
-        p, self._keep = make_params(cfg, log_capacity_turns, d_tau, d_delta, stream, device)
+        p, self._keep = make_params(cfg, log_capacity_turns, d_tau, d_delta, stream, device, tuning)
         self._h = C.c_void_p()
         self._L = L
         _ck(L.mbt_create(C.byref(p), C.byref(self._h)))
@@ -248,6 +263,10 @@ class Tracker:
     @property
     def phi_s(self):
         return float(self._L.mbt_phi_s(self._h))
+
+    @property
+    def launches_per_turn(self):
+        return int(self._L.mbt_launches_per_turn(self._h))
 
     @property
     def launch_count(self):
@@ -380,6 +399,10 @@ class Tracker:
         out = np.empty((self.M, 8))
         _ck(self._L.mbt_moments_transverse(self._h, _dp(out)))
         return out
+
+    def invalidate(self):
+        """The particle store was written in place (through device_pointers or caller-owned buffers)."""
+        _ck(self._L.mbt_invalidate(self._h))
 
     def device_pointers(self):
         t, d, ld = C.c_void_p(), C.c_void_p(), C.c_int64()

@@ -60,11 +60,12 @@ def test_struct_layout_matches_header(tmp_path):
 #include <stddef.h>
 #include "mbt.h"
 int main(void) {
-  printf("%zu %zu %zu %zu %zu %zu %zu\\n", sizeof(mbt_ring), sizeof(mbt_cavity), sizeof(mbt_radiation), sizeof(mbt_fill),
-         sizeof(mbt_resonator), sizeof(mbt_wake), sizeof(mbt_params));
-  printf("%zu %zu %zu %zu %zu %zu %zu %zu\\n", offsetof(mbt_params, cav), offsetof(mbt_params, rad), offsetof(mbt_params, fill),
+  printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n", sizeof(mbt_ring), sizeof(mbt_cavity), sizeof(mbt_radiation), sizeof(mbt_fill),
+         sizeof(mbt_resonator), sizeof(mbt_wake), sizeof(mbt_params), sizeof(mbt_tuning), sizeof(mbt_transverse), sizeof(mbt_plane));
+  printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n", offsetof(mbt_params, cav), offsetof(mbt_params, rad), offsetof(mbt_params, fill),
          offsetof(mbt_params, wake), offsetof(mbt_params, seed), offsetof(mbt_params, d_tau), offsetof(mbt_params, stream),
-         offsetof(mbt_params, device));
+         offsetof(mbt_params, device), offsetof(mbt_params, trans), offsetof(mbt_params, tuning),
+         offsetof(mbt_tuning, pairs_per_thread), offsetof(mbt_tuning, turn_mode), offsetof(mbt_tuning, reserved));
   return 0;
 }''')
     exe = tmp_path / "probe"
@@ -72,10 +73,12 @@ int main(void) {
     a, b = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.strip().splitlines()
     sizes = [int(x) for x in a.split()]
     offs = [int(x) for x in b.split()]
-    assert sizes == [ctypes.sizeof(c) for c in (mbt.Ring, mbt.Cavity, mbt.Radiation, mbt.Fill, mbt.Resonator, mbt.Wake, mbt.Params)]
-    P = mbt.Params
+    assert sizes == [ctypes.sizeof(c) for c in (mbt.Ring, mbt.Cavity, mbt.Radiation, mbt.Fill, mbt.Resonator, mbt.Wake, mbt.Params,
+                                                mbt.Tuning, mbt.Transverse, mbt.Plane)]
+    P, T = mbt.Params, mbt.Tuning
     assert offs == [P.cav.offset, P.rad.offset, P.fill.offset, P.wake.offset, P.seed.offset, P.d_tau.offset,
-                    P.stream.offset, P.device.offset]
+                    P.stream.offset, P.device.offset, P.trans.offset, P.tuning.offset,
+                    T.pairs_per_thread.offset, T.turn_mode.offset, T.reserved.offset]
 
 
 def test_make_params_marshalling():
@@ -86,6 +89,11 @@ def test_make_params_marshalling():
     assert p.wake.n_res == 3 and p.wake.res[2].fr_Hz == 2.1e9 and p.wake.res[0].flags == 1
     assert p.wake.history_turns == 20 and p.log_capacity_turns == 7 and p.seed == 4
     assert np.isnan(p.cav[0].phase_rad)
+    assert all(getattr(p.tuning, k) == 0 for k in mbt.TUNING_FIELDS) and list(p.tuning.reserved) == [0, 0]
+    p, keep = mbt.make_params(cfg, tuning=dict(turn_mode=1, tile_iters=3))
+    assert p.tuning.turn_mode == 1 and p.tuning.tile_iters == 3 and p.tuning.pdl == 0
+    with pytest.raises(KeyError):
+        mbt.make_params(cfg, tuning=dict(no_such_knob=1))
 
 
 def test_workloads_match_baseline_configs():
@@ -104,13 +112,12 @@ def test_workloads_match_baseline_configs():
     assert W.config("c4") == W.config("c4")
 
 
-def test_pass_tiling_host_logic(monkeypatch):
+def test_pass_tiling_host_logic():
     """mbt_plan_tiles (no device needed): the tilings of the BASELINE workloads on a B200 (148 SMs x 2 or 3 resident CTAs)
     and the properties every tiling has: it covers the bunch, tiles are whole iterations, the last tile is at least
     3/4 of the others."""
     from paper_1809_00391_b200 import build, mbt
     build.build()
-    monkeypatch.delenv("MBT_TILE_ITERS", raising=False)
     assert mbt.plan_tiles(50_000, 512, 363, 296) == (25 * 512, 4)          # c4, k_pass two pairs per thread: 4.9 waves
     assert mbt.plan_tiles(100_000, 512, 484, 296) == (66 * 512, 3)         # c5
     assert mbt.plan_tiles(50_000, 256, 363, 296) == (49 * 256, 4)          # c4, k_pass6
@@ -129,7 +136,6 @@ def test_pass_tiling_host_logic(monkeypatch):
         it = tp // stride
         last = -(-(ppb - (nt - 1) * tp) // stride)
         assert nt == 1 or 4 * last >= 3 * it
-    monkeypatch.setenv("MBT_TILE_ITERS", "16")
-    assert mbt.plan_tiles(50_000, 512, 363, 296) == (16 * 512, 7)           # the measurement knob
+    assert mbt.plan_tiles(50_000, 512, 363, 296, tile_iters=16) == (16 * 512, 7)   # mbt_tuning.tile_iters
     with pytest.raises(mbt.MbtError):
         mbt.plan_tiles(0, 512, 1, 296)
