@@ -156,7 +156,9 @@ def test_pin_c_equilibrium_energy_spread(orc):
 
 
 def test_excitation_stream_layout(orc):
-    """Particle i of bunch b at turn n uses Philox counter (i>>1, b, n, 0): z_c if i even, z_s if odd."""
+    """Particle i of bunch b at turn n uses Philox counter (i>>2, b, n, 0) (reading D8: one block serves four consecutive
+    particles): words (x0, x1) make the Box-Muller pair of particles 4j, 4j+1, (x2, x3) that of 4j+2, 4j+3; the even particle
+    of a pair takes z_c, the odd one z_s."""
     cfg = _bare(5, 1)
     cfg["fill"]["buckets"] = [0, 7]
     cfg["fill"]["charge_C"] = [1e-9, 1e-9]
