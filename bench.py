@@ -179,6 +179,60 @@ def _workload_name(args):
     return s
 
 
+def run_sharded(args):
+    """--sharded: the opt-in bunch-sharded path: the fill's bunches are split over the ranks, one
+    all-gather of the source phasors per turn (NCCL; none at N = 1).  STRONG scaling: the workload is fixed.  Not the
+    default line (BASELINE north_star fixes one GPU, no collectives); at N = 1 it measures what the host-driven turn
+    (three launches and a host round trip per turn, no graph) costs against mbt_track."""
+    import torch
+    import torch.distributed as dist
+    from paper_1809_00391_b200 import build, sharded, workloads as W
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    build.build()
+    cfg = _config(args)
+    n_part = W.n_particles(cfg)
+    K, Wm = args.steps, args.warmup
+    trk = sharded.ShardedTracker(cfg, rank=rank, world=world, device=local)
+    trk.track(Wm)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(trk.stream)
+    trk.track(K)
+    e1.record(trk.stream)
+    torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3
+    if world > 1:
+        t = torch.tensor([sec], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        sec = float(t.item())
+    m = trk.tracker.moments()
+    assert np_isfinite(m)
+    if rank == 0:
+        line = {"metric": METRIC, "value": n_part * K / sec, "unit": "particle-turns/s", "n_gpus": world, "steps": K, "warmup": Wm,
+                "ms_per_step": sec / K * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+                "data": "synthetic", "config": dict(_config_keys(args, world), parallelism="bunch-sharded x%d" % world),
+                "roofline": None, "gpu_launches": int(4 * K),
+                "note": "opt-in sharded path: mbt_shard_turn_begin / all_gather_into_tensor / mbt_shard_turn_end per turn"}
+        print(json.dumps(line))
+    trk.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def np_isfinite(a):
+    import numpy as np
+    return bool(np.isfinite(a).all())
+
+
 def run_mbt(args):
     import numpy as np
     import torch
@@ -364,11 +418,14 @@ def main():
     ap.add_argument("--pairs-per-thread", type=int, default=0, help="mbt_tuning.pairs_per_thread")
     ap.add_argument("--pdl", type=int, default=0, help="mbt_tuning.pdl")
     ap.add_argument("--verbose", type=int, default=0)
+    ap.add_argument("--sharded", action="store_true", help="opt-in bunch-sharded path (strong scaling; see run_sharded)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.sharded:
+        return run_sharded(args)
     return run_mbt(args)
 
 

@@ -126,6 +126,20 @@ typedef struct {
   int32_t reserved[2]; /* must be 0 */
 } mbt_tuning;
 
+/* Bunch sharding over several devices (the paper's own outlook, P:l.253: "splitting the bunches
+ * among multiple GPUs").  Opt-in; the default path is one device (BASELINE north_star).  fill / bucket / charge_C describe
+ * the WHOLE fill on every rank; the handle of `rank` owns the contiguous bunches mbt_shard_range() gives it (chunks of
+ * ceil(n_bunches / world)): particles, counts, short-range wakes and moments of a bunch never leave its owner.  The only
+ * coupling is the long-range sum: every turn each rank needs the source phasors a[b][r] of all bunches.  A turn is
+ *     mbt_shard_turn_begin(h)   the pass and the first half of the wakes; this rank's rows of d_exchange are written
+ *     all-gather of d_exchange  the CALLER's collective (e.g. torch.distributed.all_gather_into_tensor over NCCL, on
+ *                               the handle's stream): equal chunks of ceil(n_bunches / world) * R_lr complex doubles, rank order
+ *     mbt_shard_turn_end(h)     the phasor of every local bunch from the sources of ALL bunches ahead of it; turn closed
+ * d_exchange: caller-owned DEVICE buffer of mbt_shard_exchange_doubles() doubles, 16-byte aligned (may be NULL without
+ * long-range resonators).  Getters, setters and mbt_moments work on the rank's own bunches ([n_local][...]);
+ * mbt_get / set_lr_history carry all n_bunches rows on every rank.  mbt_track returns MBT_ESTATE on a sharded handle. */
+typedef struct { int32_t enable, rank, world; void *d_exchange; } mbt_shard;
+
 typedef struct {
   mbt_ring ring;
   int32_t n_cav; const mbt_cavity *cav; /* HOST array, n_cav >= 1 */
@@ -143,6 +157,7 @@ typedef struct {
   int32_t device;               /* CUDA device ordinal; -1 -> the current device                        */
   mbt_transverse trans;         /* transverse planes; the library owns their four device arrays          */
   mbt_tuning tuning;            /* kernel-selection knobs; all zero = the library's choice               */
+  mbt_shard shard;              /* bunch sharding over several devices; enable = 0: one device            */
 } mbt_params;
 
 /* Validates, allocates, builds the wake tables and draws the initial distribution on the device (P:l.37: the user chooses
@@ -235,6 +250,13 @@ int mbt_plan_tiles(int64_t pairs_per_bunch, int64_t stride, int32_t M, int32_t s
  * coordinates in place call mbt_invalidate(), else mbt_moments / mbt_get_histogram return the statistics of the state the
  * library last closed.  (In-place writes never touch the wake, the history or the turn counter.) */
 int mbt_device_pointers(mbt_handle *h, void **d_tau, void **d_delta, int64_t *ld);
+/* ---- bunch sharding (mbt_shard above); the first two are host-only ---- */
+/* the bunches rank owns: first index and count (count may be 0 for the last ranks; mbt_create refuses such a rank) */
+int mbt_shard_range(int32_t n_bunches, int32_t world, int32_t rank, int32_t *first, int32_t *count);
+/* doubles in the exchange buffer: world * ceil(n_bunches / world) * n_lr * 2; -1 on bad arguments */
+int64_t mbt_shard_exchange_doubles(int32_t n_bunches, int32_t world, int32_t n_lr);
+int mbt_shard_turn_begin(mbt_handle *h);
+int mbt_shard_turn_end(mbt_handle *h);
 /* The particle store was modified behind the library's back: the next getter re-derives counts and moments from memory. */
 int mbt_invalidate(mbt_handle *h);
 /* kernels launched by this handle so far (bench.py's gpu_launches) */

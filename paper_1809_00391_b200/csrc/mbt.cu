@@ -102,6 +102,11 @@ struct mbt_handle {
   int device = 0;
   cudaStream_t stream = nullptr;
   bool own_stream = false;
+  int Mg = 0, b0 = 0;        // bunches of the whole fill, global index of this handle's first one (Mg = M, b0 = 0 unless sharded)
+  bool sharded = false;
+  int shard_rank = 0, shard_world = 1, shard_chunk = 0;
+  int shard_phase = 0;       // 0: between turns; 1: mbt_shard_turn_begin done, the exchange is the caller's move
+  cplx *xbuf = nullptr;      // caller-owned exchange buffer [world * chunk][R]
   int M = 0, nb = 0, R = 0, K = 0, slots = 2;  // slots of the long-range rings: K + 1, at least 2
   int64_t Np = 0, ld = 0;
   bool own_particles = false;
@@ -464,6 +469,12 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
       if (!(tr.res[r].Q > 0.5) || !(tr.res[r].fr_Hz > 0) || !std::isfinite(tr.res[r].Rs_ohm))
         return fail(MBT_EINVAL, "transverse resonator: need Q > 1/2, fr > 0");
   }
+  const mbt_shard &sh = p->shard;
+  if (sh.enable) {
+    if (sh.world < 1 || sh.rank < 0 || sh.rank >= sh.world) return fail(MBT_EINVAL, "shard: need 0 <= rank < world");
+    if (p->trans.enable) return fail(MBT_EINVAL, "shard: not available with the transverse planes");
+    if (sh.world > fl.n_bunches) return fail(MBT_EINVAL, "shard: more ranks than bunches");
+  }
   const mbt_tuning &tn = p->tuning;
   if (tn.tile_iters < 0 || tn.pairs_per_thread < 0 || tn.pairs_per_thread > 2 || tn.pdl < 0 || tn.pdl > 3 || tn.stages6 < 0 ||
       (tn.stages6 != 0 && (tn.stages6 < 2 || tn.stages6 > kMaxStages6)) || tn.turn_mode < 0 || tn.turn_mode > 3 ||
@@ -497,7 +508,24 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     }
     h->own_stream = true;
   }
-  const int M = h->M = fl.n_bunches;
+  // bunch sharding (S:8(f) rank 4): this handle owns the contiguous bunches [b0, b0 + M) of the fill's Mg
+  const int Mg = h->Mg = fl.n_bunches;
+  {
+    int first = 0, count = Mg;
+    if (sh.enable) {
+      h->sharded = true;
+      h->shard_rank = sh.rank;
+      h->shard_world = sh.world;
+      h->shard_chunk = (Mg + sh.world - 1) / sh.world;
+      first = sh.rank * h->shard_chunk;
+      count = std::max(0, std::min(h->shard_chunk, Mg - first));
+      if (count == 0) { destroy(h); return fail(MBT_EINVAL, "shard: this rank owns no bunch (use fewer ranks)"); }
+    }
+    h->b0 = first;
+    h->M = count;
+  }
+  const int M = h->M, b0 = h->b0;
+  const int32_t *bucket_g = fl.bucket;   // the whole fill (long-range sums run over it)
   const int nb = h->nb = wk.n_bins;
   const int R = h->R = n_lr;
   const int K = h->K = n_lr ? wk.history_turns : 0;
@@ -585,7 +613,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     have_sr = true;
     for (int k = 0; k < nb && k < wk.n_table; ++k) w[k] += wk.sr_table[k];
   }
-  std::vector<cplx> Esrc((size_t)R * nb), F((size_t)R * nb), g_step((size_t)M * (R ? R : 1)), g_tail((size_t)M * (R ? R : 1)),
+  std::vector<cplx> Esrc((size_t)R * nb), F((size_t)R * nb), g_step((size_t)Mg * (R ? R : 1)), g_tail((size_t)Mg * (R ? R : 1)),
       g_hist((size_t)(K ? K : 1) * (R ? R : 1));
   const ldbl T0 = (ldbl)rg.T0_s, Trf = T0 / (ldbl)rg.h;
   for (int r = 0; r < R; ++r) {
@@ -599,15 +627,15 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
       F[(size_t)r * nb + k] = cplx{(double)((ldbl)Cr[r].re * ere - (ldbl)Cr[r].im * eim),
                                    (double)((ldbl)Cr[r].re * eim + (ldbl)Cr[r].im * ere)};
     }
-    const int span = fl.bucket[M - 1] - fl.bucket[0];
-    for (int j = 0; j < M; ++j) {
-      if (j + 1 < M) g_step[(size_t)j * R + r] = exp_lambda(lr[r], (ldbl)(fl.bucket[j + 1] - fl.bucket[j]) * Trf);
-      g_tail[(size_t)j * R + r] = exp_lambda(lr[r], (ldbl)(fl.bucket[M - 1] - fl.bucket[j]) * Trf);
+    const int span = bucket_g[Mg - 1] - bucket_g[0];
+    for (int j = 0; j < Mg; ++j) {
+      if (j + 1 < Mg) g_step[(size_t)j * R + r] = exp_lambda(lr[r], (ldbl)(bucket_g[j + 1] - bucket_g[j]) * Trf);
+      g_tail[(size_t)j * R + r] = exp_lambda(lr[r], (ldbl)(bucket_g[Mg - 1] - bucket_g[j]) * Trf);
     }
     for (int k = 1; k <= K; ++k) g_hist[(size_t)(k - 1) * R + r] = exp_lambda(lr[r], (ldbl)k * T0 - (ldbl)span * Trf);
   }
   std::vector<double> qm(M);
-  for (int b = 0; b < M; ++b) qm[b] = fl.charge_C[b] / (double)h->Np;
+  for (int b = 0; b < M; ++b) qm[b] = fl.charge_C[b0 + b] / (double)h->Np;
 
   // ---- device memory
   const size_t N = (size_t)M * (size_t)h->ld;
@@ -678,15 +706,15 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     for (int r = 0; r < R; ++r)
       for (int d = 0; d < rg.h; ++d) gd[(size_t)r * rg.h + d] = exp_lambda(lr[r], (ldbl)d * Trf);
     CUH(h->gd.upload(gd, h->stream));
-    CUH(h->d_bucket.upload(std::vector<int32_t>(fl.bucket, fl.bucket + M), h->stream));
-    CUH(h->a_ready.alloc((size_t)M * (R ? R : 1), h->stream));
+    CUH(h->d_bucket.upload(std::vector<int32_t>(bucket_g, bucket_g + Mg), h->stream));
+    CUH(h->a_ready.alloc((size_t)Mg * (R ? R : 1), h->stream));
     CUH(h->bunch_ready.alloc(M, h->stream));
     CUH(h->agg_ready.alloc(1, h->stream));
   }
   CUH(h->Vsr.alloc((size_t)M * nb, h->stream));
   CUH(h->a_cur.alloc((size_t)M * (R ? R : 1), h->stream));
   h->slots = K + 1 < 2 ? 2 : K + 1;
-  CUH(h->ring_a.alloc((size_t)h->slots * M * (R ? R : 1), h->stream));
+  CUH(h->ring_a.alloc((size_t)h->slots * Mg * (R ? R : 1), h->stream));
   CUH(h->ring_A.alloc((size_t)h->slots * (R ? R : 1), h->stream));
   CUH(h->P.alloc((size_t)M * (R ? R : 1), h->stream));
   CUH(h->hist.alloc((size_t)M * nb, h->stream));
@@ -723,7 +751,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     const int room = (2 * prop.multiProcessorCount + M - 1) / M;
     if (S > room) S = room;
     if (S > 64) S = 64;
-    if (S < 1) S = 1;
+    if (S < 1 || sh.enable) S = 1;  // a sharded handle runs the per-bunch phasor gather: one CTA per bunch
     h->wake_splits = S;
   }
   CUH(h->rd_cnt.alloc(M, h->stream));
@@ -742,6 +770,11 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   Wa.mom_log = h->log_cap > 0 ? h->mom_log.p : nullptr;
   Wa.log_cap = h->log_cap;
   Wa.ctrl = h->ctrl.p;
+  if (sh.enable && R > 0) {
+    if (!sh.d_exchange || ((uintptr_t)sh.d_exchange & 15u)) { destroy(h); return fail(MBT_EINVAL, "shard: d_exchange must be a 16-byte aligned device buffer (mbt_shard_exchange_doubles)"); }
+    h->xbuf = (cplx *)sh.d_exchange;
+  }
+  Wa.Mg = Mg; Wa.b0 = b0; Wa.part = 0; Wa.xbuf = h->xbuf;
   Wa.h = rg.h; Wa.slots = h->slots; Wa.bucket = h->d_bucket.p; Wa.gd = h->gd.p;
   Wa.a_ready = h->a_ready.p; Wa.bunch_ready = h->bunch_ready.p; Wa.agg_ready = h->agg_ready.p;
 
@@ -758,7 +791,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   // k_wake: the convolution's shared memory + the staged source factors (if <= 64 KB), or the scan's staged operands (if
   // the scan runs and they fit in 96 KB).  Kept small: every CTA of the launch should be resident at once.
   {
-    size_t need = wake_smem_bytes(nb, M);
+    size_t need = wake_smem_bytes(nb, Mg);
     const size_t stage_e = (size_t)R * nb * sizeof(cplx) + 16;
     if (R > 0 && stage_e <= 64u * 1024u) need += stage_e;
     // one CTA per bunch: the per-bunch phasor gather replaces the scan.  A bunch's CTA waits only for CTAs of a lower
@@ -792,12 +825,13 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   // beside k_wake on a side stream).
   CUH(h->bunch_done.alloc(M, h->stream));
   A.bunch_done = h->bunch_done.p;
-  h->fused = !tr.enable && (tn.turn_mode == 2 || (tn.turn_mode == 0 && kFusedTurnDefault));
+  A.b0 = b0;
+  h->fused = !tr.enable && !sh.enable && (tn.turn_mode == 2 || (tn.turn_mode == 0 && kFusedTurnDefault));
   if (tn.turn_mode == 2 && tr.enable) {
     destroy(h);
     return fail(MBT_EINVAL, "tuning.turn_mode 2 (one launch per turn) is not available with the transverse planes");
   }
-  if (h->fused && h->smem_pass < wake_smem_bytes(nb, M)) h->fused = false;  // cannot happen for nb <= MBT_MAX_BINS
+  if (h->fused && h->smem_pass < wake_smem_bytes(nb, Mg)) h->fused = false;  // cannot happen for nb <= MBT_MAX_BINS
   A.fused = h->fused ? 1 : 0;
   if (tn.verbose)
     fprintf(stderr, "mbt: %s, %d pair(s) per thread, grid %d x %d, %zu B shared memory per CTA, pdl %d\n",
@@ -806,7 +840,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   // ---- initial distribution (D20) on the device
   {
     dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)M);
-    k_init<<<grid, 256, 0, h->stream>>>(h->d_tau, h->d_delta, h->ld, (uint32_t)h->Np, M, A.keys, fl.sigma_tau0_s,
+    k_init<<<grid, 256, 0, h->stream>>>(h->d_tau, h->d_delta, h->ld, (uint32_t)h->Np, M, b0, A.keys, fl.sigma_tau0_s,
                                          fl.sigma_delta0);
     h->launches += 1;
     CUH(cudaGetLastError());
@@ -924,6 +958,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
 int mbt_track(mbt_handle *h, int64_t n_turns) {
   if (!h || n_turns < 0) return fail(MBT_EINVAL, "bad argument");
   if (h->turn + n_turns > 0xFFFFFFFFll) return fail(MBT_EINVAL, "turn counter would exceed 2^32");
+  if (h->sharded) return fail(MBT_ESTATE, "a sharded handle advances by mbt_shard_turn_begin / (all-gather) / mbt_shard_turn_end");
   CU(cudaSetDevice(h->device));
   if (n_turns == 0) return 0;
   if (!h->graph1) {
@@ -956,6 +991,7 @@ int mbt_track(mbt_handle *h, int64_t n_turns) {
 int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, double *wake_seconds) {
   if (!h || n_turns < 1 || n_turns > 65536 || !pass_seconds || !wake_seconds) return fail(MBT_EINVAL, "bad argument");
   if (h->turn + n_turns > 0xFFFFFFFFll) return fail(MBT_EINVAL, "turn counter would exceed 2^32");
+  if (h->sharded) return fail(MBT_ESTATE, "not available on a sharded handle");
   CU(cudaSetDevice(h->device));
   struct Events {  // destroyed on every exit path
     std::vector<cudaEvent_t> v;
@@ -1026,6 +1062,66 @@ int mbt_device_pointers(mbt_handle *h, void **d_tau, void **d_delta, int64_t *ld
   return 0;
 }
 
+int mbt_shard_range(int32_t n_bunches, int32_t world, int32_t rank, int32_t *first, int32_t *count) {
+  if (n_bunches < 1 || world < 1 || rank < 0 || rank >= world || !first || !count) return fail(MBT_EINVAL, "bad argument");
+  const int chunk = (n_bunches + world - 1) / world;
+  *first = std::min(rank * chunk, n_bunches);
+  *count = std::max(0, std::min(chunk, n_bunches - rank * chunk));
+  return 0;
+}
+
+int64_t mbt_shard_exchange_doubles(int32_t n_bunches, int32_t world, int32_t n_lr) {
+  if (n_bunches < 1 || world < 1 || n_lr < 0) return -1;
+  const int64_t chunk = (n_bunches + world - 1) / world;
+  return (int64_t)world * chunk * n_lr * 2;
+}
+
+int mbt_shard_turn_begin(mbt_handle *h) {
+  if (!h) return fail(MBT_EINVAL, "null argument");
+  if (!h->sharded) return fail(MBT_ESTATE, "not a sharded handle");
+  if (h->shard_phase != 0) return fail(MBT_ESTATE, "mbt_shard_turn_end has not closed the turn before");
+  if (h->turn + 1 > 0xFFFFFFFFll) return fail(MBT_EINVAL, "turn counter would exceed 2^32");
+  CU(cudaSetDevice(h->device));
+  // the pass over this rank's bunches, then the first half of their wakes: counts, S5, gather cells, moments, and the S6
+  // sources into this rank's rows of the exchange buffer
+  h->fn_map<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args, h->wargs);
+  CU(cudaGetLastError());
+  WakeArgs wa = h->wargs;
+  wa.part = 1;
+  k_wake<<<dim3(h->M, 1), kWakeThreads, h->smem_wake, h->stream>>>(wa);
+  CU(cudaGetLastError());
+  h->launches += 2;
+  h->shard_phase = 1;
+  h->dirty = true;
+  return 0;
+}
+
+int mbt_shard_turn_end(mbt_handle *h) {
+  if (!h) return fail(MBT_EINVAL, "null argument");
+  if (!h->sharded) return fail(MBT_ESTATE, "not a sharded handle");
+  if (h->shard_phase != 1) return fail(MBT_ESTATE, "mbt_shard_turn_begin first");
+  CU(cudaSetDevice(h->device));
+  // the exchange buffer now holds the sources of ALL bunches: into the history ring, flags raised; then the second half
+  // of the wakes of this rank's bunches (phasor gather over all bunches ahead, on any rank) and the closing of the turn
+  if (h->R > 0) {
+    const int rows = h->Mg;
+    k_shard_scatter<<<(rows * h->R + 255) / 256, 256, 0, h->stream>>>(h->xbuf, rows, h->R, h->Mg, h->slots, h->ctrl.p, h->ring_a.p,
+                                                                      h->a_ready.p);
+    CU(cudaGetLastError());
+    h->launches += 1;
+  }
+  WakeArgs wa = h->wargs;
+  wa.part = 2;
+  k_wake<<<dim3(h->M, 1), kWakeThreads, h->smem_wake, h->stream>>>(wa);
+  CU(cudaGetLastError());
+  h->launches += 1;
+  h->shard_phase = 0;
+  h->turn += 1;
+  h->dirty = true;
+  h->wake_valid = true;
+  return 0;
+}
+
 int mbt_invalidate(mbt_handle *h) {
   if (!h) return fail(MBT_EINVAL, "null argument");
   h->dirty = true;
@@ -1078,7 +1174,7 @@ int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int
     int rc = upload_window(h, zero.data(), zero.data());
     if (rc) return rc;
   }
-  k_set_ctrl<<<1, 256, 0, h->stream>>>(h->ctrl.p, (uint32_t)turn, 0u, h->a_ready.p, h->M * (h->R ? h->R : 1), h->bunch_ready.p, h->M,
+  k_set_ctrl<<<1, 256, 0, h->stream>>>(h->ctrl.p, (uint32_t)turn, 0u, h->a_ready.p, h->Mg * (h->R ? h->R : 1), h->bunch_ready.p, h->M,
                                        h->agg_ready.p, h->bunch_done.p);
   CU(cudaGetLastError());
   h->launches += 1;
@@ -1303,7 +1399,7 @@ int mbt_get_moment_log(mbt_handle *h, int64_t first_turn, int64_t n, double *out
 int mbt_get_lr_history(mbt_handle *h, double *out) {
   if (!h || !out) return fail(MBT_EINVAL, "null argument");
   CU(cudaSetDevice(h->device));
-  const int M = h->M, R = h->R, K = h->K;
+  const int M = h->Mg, R = h->R, K = h->K;  // rows of the whole fill (a sharded handle holds them all)
   if (R == 0 || K == 0) return 0;
   std::vector<cplx> ring((size_t)h->slots * M * R);
   CU(cudaMemcpyAsync(ring.data(), h->ring_a.p, ring.size() * sizeof(cplx), cudaMemcpyDeviceToHost, h->stream));
@@ -1325,7 +1421,7 @@ int mbt_get_lr_history(mbt_handle *h, double *out) {
 int mbt_set_lr_history(mbt_handle *h, const double *in) {
   if (!h || !in) return fail(MBT_EINVAL, "null argument");
   CU(cudaSetDevice(h->device));
-  const int M = h->M, R = h->R, K = h->K;
+  const int M = h->Mg, R = h->R, K = h->K;  // rows of the whole fill (a sharded handle holds them all)
   if (R == 0 || K == 0) return 0;
   std::vector<cplx> ring((size_t)h->slots * M * R, cplx{0.0, 0.0});
   for (int k = 0; k < K; ++k) {

@@ -98,6 +98,7 @@ struct Args {
   MathTab mt;
   // one-launch turn (mbt_tuning.turn_mode 2): the last CTA of a bunch to finish builds that bunch's wake (wake_body)
   int32_t fused;              // 1: this launch is a whole turn; its predecessor in the stream is the pass before it
+  int32_t b0;                 // global index of the handle's first bunch (Philox counter word; 0 unless sharded)
   uint32_t *bunch_done;       // [M] pass CTAs of the bunch that have flushed their counts and moment sums
 };
 
@@ -204,6 +205,9 @@ struct WakeArgs {
   Ctrl *ctrl;
   uint32_t smem_wake_bytes, smem_pass_bytes;  // dynamic shared memory of a k_wake launch / of a pass launch (one-launch turn)
   // one-launch turn: per-bunch phasor gather instead of the scan (wake_body<false, true>)
+  int32_t part;               // 0: the whole wake; sharded handle: 1 = up to the gather cells, 2 = phasor gather and close
+  int32_t Mg, b0;             // bunches of the whole fill and index of this handle's first one (Mg = M, b0 = 0 unless sharded)
+  cplx *xbuf;                 // sharded: [Mg padded][R] exchange buffer of the turn's source phasors (else nullptr)
   int32_t gather_P;           // k_wake with one CTA per bunch: per-bunch phasor gather (all CTAs resident) instead of the scan
   int32_t h, slots;           // harmonic number; slots of ring_a / ring_A (K + 1, at least 2)
   const int32_t *bucket;      // [M]
@@ -259,7 +263,7 @@ __host__ __device__ inline size_t scan_smem_bytes(int M, int R) { return (size_t
 // over resonators and scan elements unrolled (200 KB of SASS) ran slower than the loops it replaced.  Hence: compact loops,
 // few dependent trips to memory, a register-blocked convolution that uses every thread.
 template <bool SPLIT, bool FUSED>
-__device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const int split, double *smem_d, const uint32_t smem_bytes) {
+__device__ __forceinline__ bool wake_first(const WakeArgs &A, const int b, const int split, double *smem_d, const uint32_t smem_bytes) {
   constexpr int NW = kWakeThreads / 32;
   const int nb = A.nb;
   double *sq = smem_d;               // [nb] charge per bin
@@ -284,8 +288,8 @@ __device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const 
   unsigned long long n_in = 0ull, m1 = 0ull;         // sum c_k, sum k c_k
   const bool sources = A.mode == 0 && split == 0 && A.R > 0;
   const cplx *pE = A.Esrc;  // [R][nb] as the source sums read it: staged behind the buckets if the launch's memory holds it
-  if (sources && wake_smem_bytes(nb, A.M) + (size_t)A.R * nb * sizeof(cplx) + 16 <= (size_t)smem_bytes) {
-    cplx *sE = reinterpret_cast<cplx *>((reinterpret_cast<uintptr_t>(sB + A.M) + 15) & ~(uintptr_t)15);
+  if (sources && wake_smem_bytes(nb, A.Mg) + (size_t)A.R * nb * sizeof(cplx) + 16 <= (size_t)smem_bytes) {
+    cplx *sE = reinterpret_cast<cplx *>((reinterpret_cast<uintptr_t>(sB + A.Mg) + 15) & ~(uintptr_t)15);
     const int nE = A.R * nb;
 #pragma unroll 4
     for (int i = tid; i < nE; i += kWakeThreads) sE[i] = A.Esrc[i];
@@ -307,7 +311,7 @@ __device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const 
   }
   if (tid < 24) sw[tid < 16 ? tid - 16 : nb + tid - 16] = 0.0;
   if (FUSED && A.mode == 0 && A.R > 0)
-    for (int j = tid; j < A.M; j += kWakeThreads) sB[j] = A.bucket[j];
+    for (int j = tid; j < A.Mg; j += kWakeThreads) sB[j] = A.bucket[j];
   if (S > 1) {  // the last split to have read the counts clears them (nobody waits for anybody)
     __syncthreads();
     if (tid == 0) s_last = (atomicAdd(&A.rd_cnt[b], 1u) == (uint32_t)(S - 1));
@@ -369,7 +373,7 @@ __device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const 
     for (int k = 0; k < 4; ++k) A.mom_acc[b * 4 + k] = 0.0;
     A.nout_acc[b] = 0ull;
   }
-  if (A.mode != 0) return;
+  if (A.mode != 0) return false;
 
   // S6 sources: a[b][r] = sum_k q[k] exp(-lambda_r c_k).  One warp per resonator, counted from the LAST warp down (the
   // first warps carry the convolution's heaviest tasks); shuffles only, no block barrier.
@@ -390,8 +394,9 @@ __device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const 
       cplx a{are, aim};
       if (follow) a = cmul(a, A.shift_src[(size_t)r * (2 * A.s_max + 1) + (s_used + A.s_max)]);  // bin centres at their own window
       A.a_cur[(size_t)b * A.R + r] = a;
-      A.ring_a[((size_t)(n % (uint32_t)A.slots) * A.M + b) * A.R + r] = a;
-      if (FUSED) st_release_u32(&A.a_ready[(size_t)b * A.R + r], n);  // later bunches' gathers wait for it
+      A.ring_a[((size_t)(n % (uint32_t)A.slots) * A.Mg + (A.b0 + b)) * A.R + r] = a;  // rows by the GLOBAL bunch index
+      if (A.xbuf) A.xbuf[(size_t)(A.b0 + b) * A.R + r] = a;                          // sharded: this rank's rows of the exchange
+      if (FUSED) st_release_u32(&A.a_ready[(size_t)(A.b0 + b) * A.R + r], n);        // later bunches' gathers wait for it
     }
   }
 
@@ -470,7 +475,7 @@ __device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const 
       s_last = (atomicAdd(&A.wr_cnt[b], 1u) == (uint32_t)(S - 1));
     }
     __syncthreads();
-    if (!s_last) return;
+    if (!s_last) return false;
     __threadfence();
     if (tid == 0) A.wr_cnt[b] = 0u;
     for (int j = tid; j < nb; j += kWakeThreads) sv[j] = __ldcg(&A.Vsr[(size_t)b * nb + j]);
@@ -489,7 +494,23 @@ __device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const 
     }
     A.cellSR[(size_t)b * (nb + 2) + k] = c;
   }
+  return true;
+}
 
+// The second half of a bunch's wake: the phasor P[b] and the closing of the turn.  FUSED (one CTA per bunch): the
+// per-bunch gather; else the last-CTA scan.  Needs the buckets in shared memory (FUSED; staged by wake_first, or by
+// wake_body for a sharded handle's second phase).
+template <bool FUSED>
+__device__ __forceinline__ void wake_second(const WakeArgs &A, const int b, double *smem_d, const uint32_t smem_bytes) {
+  constexpr int NW = kWakeThreads / 32;
+  const int nb = A.nb;
+  int32_t *sB = reinterpret_cast<int32_t *>(smem_d + 3 * nb + 24);  // [Mg] buckets (FUSED)
+  __shared__ bool s_last;
+  const int tid = threadIdx.x;
+  const int lane = tid & 31, warp = tid >> 5;
+  const uint32_t n = A.ctrl->turn + 1u;  // the turn being closed
+  const bool follow = A.mode == 0 && A.window_mode == 1;
+  const int32_t s_used = follow ? A.s_hist[b] : 0;  // the window this turn's counts were taken on (set by wake_first)
   const int M = A.M, R = A.R, K = A.K;
   if constexpr (FUSED) {
     // S6, one-launch turn: the phasor bunch b sees, gathered by the bunch's own closing CTA as the pairwise sum itself --
@@ -504,19 +525,20 @@ __device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const 
       const int nq = NW / R;                 // warps per resonator (R <= NW)
       const int r = warp % R, q = warp / R;  // warps >= nq R idle
       const int Kh = (int)min((uint32_t)K, n - 1u);
-      const int n_el = b + Kh;
-      const int sb = sB[b];
+      const int bg = A.b0 + b;               // global index of the bunch: the bunches ahead are 0 .. bg-1, on any rank
+      const int n_el = bg + Kh;
+      const int sb = sB[bg];
       cplx acc{0.0, 0.0};
       if (q < nq) {
         const cplx *gdr = A.gd + (size_t)r * A.h;
         const cplx g0 = gdr[sb - sB[0]];
 #pragma unroll 2
         for (int e = q * 32 + lane; e < n_el; e += 32 * nq) {
-          if (e < b) {
+          if (e < bg) {
             wait_turn(&A.a_ready[(size_t)e * R + r], n);
-            acc = cfma(__ldcg_cplx(&A.ring_a[((size_t)(n % (uint32_t)A.slots) * M + e) * R + r]), gdr[sb - sB[e]], acc);
+            acc = cfma(__ldcg_cplx(&A.ring_a[((size_t)(n % (uint32_t)A.slots) * A.Mg + e) * R + r]), gdr[sb - sB[e]], acc);
           } else {
-            const int k = e - b + 1;
+            const int k = e - bg + 1;
             wait_turn(A.agg_ready, n - 1u);
             acc = cfma(__ldcg_cplx(&A.ring_A[(size_t)((n - (uint32_t)k) % (uint32_t)A.slots) * R + r]),
                        cmul(A.g_hist[(size_t)(k - 1) * R + r], g0), acc);
@@ -553,8 +575,8 @@ __device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const 
       cplx acc{0.0, 0.0};
       if (q < nq) {
 #pragma unroll 2
-        for (int j = q * 32 + lane; j < M; j += 32 * nq)
-          acc = cfma(__ldcg_cplx(&A.ring_a[((size_t)(n % (uint32_t)A.slots) * M + j) * R + r]), A.g_tail[(size_t)j * R + r], acc);
+        for (int j = q * 32 + lane; j < A.Mg; j += 32 * nq)
+          acc = cfma(__ldcg_cplx(&A.ring_a[((size_t)(n % (uint32_t)A.slots) * A.Mg + j) * R + r]), A.g_tail[(size_t)j * R + r], acc);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
           acc.re += __shfl_xor_sync(0xffffffffu, acc.re, o);
@@ -688,6 +710,23 @@ __device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const 
     A.ctrl->turn = n;
   }
   }  // !FUSED
+}
+
+
+// The wake of bunch b: wake_first, then wake_second.  A sharded handle (mbt_params.shard) runs the two halves as two
+// launches around the exchange of the source phasors: part 1 stops after the gather cells (the sources of the other
+// ranks' bunches are not here yet), part 2 starts at the phasor gather.
+template <bool SPLIT, bool FUSED>
+__device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const int split, double *smem_d, const uint32_t smem_bytes) {
+  if (FUSED && A.part == 2) {
+    int32_t *sB = reinterpret_cast<int32_t *>(smem_d + 3 * A.nb + 24);
+    for (int j = threadIdx.x; j < A.Mg; j += kWakeThreads) sB[j] = A.bucket[j];
+    __syncthreads();
+  } else {
+    if (!wake_first<SPLIT, FUSED>(A, b, split, smem_d, smem_bytes)) return;
+    if (FUSED && A.part == 1) return;
+  }
+  wake_second<FUSED>(A, b, smem_d, smem_bytes);
 }
 
 __global__ void __launch_bounds__(kWakeThreads, 3) k_wake(const __grid_constant__ WakeArgs A) {
@@ -865,7 +904,7 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
           // one Philox block serves FOUR consecutive particles (D8): counter (particle >> 2, bunch, turn, tag 0);
           // its words (x0, x1) give the Box-Muller pair of particles 4j, 4j+1, (x2, x3) that of 4j+2, 4j+3; the even
           // particle of a pair takes z_c, the odd one z_s.  A thread that owns the whole quad (NPAIR = 2) calls it once.
-          if (q == 0 || NPAIR == 1) philox4x32_10(pq >> 1, (uint32_t)b, n, 0u, A.keys, xs[0], xs[1], xs[2], xs[3]);
+          if (q == 0 || NPAIR == 1) philox4x32_10(pq >> 1, (uint32_t)(b + A.b0), n, 0u, A.keys, xs[0], xs[1], xs[2], xs[3]);
           const bool hi_half = (NPAIR == 2) ? (q == 1) : ((pq & 1u) != 0u);  // with NPAIR = 2 the thread's first pair is even
           const double u1 = uniform32(A.mt, hi_half ? xs[2] : xs[0]), u2 = uniform32(A.mt, hi_half ? xs[3] : xs[1]);
           if (NCAV > 0) bm[q] = box_muller_head(A.mt, sL, u1, u2, A.A_q);  // polynomials: lock step with S1's
@@ -1068,14 +1107,14 @@ __global__ void k_eval_wake(int M, int nb, int R, const double *Vsr, const cplx 
 }
 
 // initial distribution (D20): Philox stream tag 1, counter (i, b, 0, 1); tau = sigma_tau0 z_c, delta = sigma_delta0 z_s
-__global__ void k_init(double *tau, double *delta, int64_t ld, uint32_t Np, int M, PhiloxKeys keys, double s_tau,
+__global__ void k_init(double *tau, double *delta, int64_t ld, uint32_t Np, int M, int b0, PhiloxKeys keys, double s_tau,
                        double s_delta) {
   const int b = blockIdx.y;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < (uint32_t)ld; i += gridDim.x * blockDim.x) {
     double t = 0.0, d = 0.0;
     if (i < Np) {
       uint32_t x0, x1, x2, x3;
-      philox4x32_10(i, (uint32_t)b, 0u, 1u, keys, x0, x1, x2, x3);
+      philox4x32_10(i, (uint32_t)(b + b0), 0u, 1u, keys, x0, x1, x2, x3);
       double zc, zs;
       box_muller_accurate(uniform52(x0, x1), uniform52(x2, x3), zc, zs);
       t = s_tau * zc;
@@ -1121,6 +1160,18 @@ __global__ void k_set_ctrl(Ctrl *c, uint32_t turn, uint32_t pending, uint32_t *a
   }
 }
 __global__ void k_clear_pending(Ctrl *c) { c->kick_pending = 0u; }
+
+// Sharded handle, after the all-gather of the exchange buffer: the source phasors of ALL bunches of the turn being closed
+// go into the history ring (so that every rank holds the whole history), and their flags are raised, so that the phasor
+// gather of the second half of the wake finds them like sources of its own launch.
+__global__ void k_shard_scatter(const cplx *xbuf, int n_rows, int R, int Mg, int slots, const Ctrl *ctrl, cplx *ring_a, uint32_t *a_ready) {
+  const uint32_t n = ctrl->turn + 1u;
+  cplx *dst = ring_a + (size_t)(n % (uint32_t)slots) * Mg * R;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_rows * R; i += gridDim.x * blockDim.x) {
+    dst[i] = xbuf[i];
+    a_ready[i] = n;
+  }
+}
 
 __global__ void k_philox_selftest(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, PhiloxKeys keys, uint32_t *out) {
   uint32_t x0, x1, x2, x3;

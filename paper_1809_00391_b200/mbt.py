@@ -18,7 +18,8 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libmbt.so")
 SYMBOLS = [
     "mbt_create", "mbt_track", "mbt_moments", "mbt_destroy", "mbt_get_particles", "mbt_set_particles",
     "mbt_get_histogram", "mbt_get_wake", "mbt_get_moment_log", "mbt_get_lr_history", "mbt_set_lr_history", "mbt_get_window", "mbt_set_window",
-    "mbt_turn", "mbt_phi_s", "mbt_particle_stride", "mbt_plan_tiles", "mbt_device_pointers", "mbt_invalidate", "mbt_launch_count", "mbt_launches_per_turn",
+    "mbt_turn", "mbt_phi_s", "mbt_particle_stride", "mbt_plan_tiles", "mbt_device_pointers", "mbt_invalidate", "mbt_shard_range", "mbt_shard_exchange_doubles", "mbt_shard_turn_begin", "mbt_shard_turn_end",
+    "mbt_launch_count", "mbt_launches_per_turn",
     "mbt_get_transverse", "mbt_set_transverse", "mbt_get_dipole", "mbt_get_transverse_wake", "mbt_moments_transverse",
     "mbt_get_rw_kick", "mbt_get_rw_history", "mbt_set_rw_history", "mbt_get_transverse_log",
     "mbt_last_track_seconds", "mbt_track_profiled", "mbt_philox_selftest", "mbt_normal_selftest", "mbt_last_error", "mbt_version",
@@ -73,11 +74,15 @@ class Tuning(C.Structure):
     _fields_ = [(k, C.c_int32) for k in TUNING_FIELDS] + [("reserved", C.c_int32 * 2)]
 
 
+class Shard(C.Structure):
+    _fields_ = [("enable", C.c_int32), ("rank", C.c_int32), ("world", C.c_int32), ("d_exchange", C.c_void_p)]
+
+
 class Params(C.Structure):
     _fields_ = [("ring", Ring), ("n_cav", C.c_int32), ("cav", C.POINTER(Cavity)), ("rad", Radiation),
                 ("fill", Fill), ("wake", Wake), ("seed", C.c_uint64), ("log_capacity_turns", C.c_int64),
                 ("d_tau", C.c_void_p), ("d_delta", C.c_void_p), ("stream", C.c_void_p), ("device", C.c_int32),
-                ("trans", Transverse), ("tuning", Tuning)]
+                ("trans", Transverse), ("tuning", Tuning), ("shard", Shard)]
 
 
 class MbtError(RuntimeError):
@@ -117,6 +122,11 @@ def lib():
         L.mbt_particle_stride.restype = C.c_int64
         L.mbt_plan_tiles.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_uint32), C.POINTER(C.c_int32)]
         L.mbt_invalidate.argtypes = [H]
+        L.mbt_shard_range.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        L.mbt_shard_exchange_doubles.argtypes = [C.c_int32, C.c_int32, C.c_int32]
+        L.mbt_shard_exchange_doubles.restype = C.c_int64
+        L.mbt_shard_turn_begin.argtypes = [H]
+        L.mbt_shard_turn_end.argtypes = [H]
         L.mbt_launches_per_turn.argtypes = [H]
         L.mbt_device_pointers.argtypes = [H, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
         L.mbt_launch_count.argtypes = [H]
@@ -164,6 +174,18 @@ def plan_tiles(pairs_per_bunch, stride, n_bunches, slots, tile_iters=0):
     return tp.value, nt.value
 
 
+def shard_range(n_bunches, world, rank):
+    """(first, count): the contiguous bunches `rank` of `world` owns (host logic, no device needed)."""
+    a, b = C.c_int32(), C.c_int32()
+    _ck(lib().mbt_shard_range(int(n_bunches), int(world), int(rank), C.byref(a), C.byref(b)))
+    return a.value, b.value
+
+
+def shard_exchange_doubles(n_bunches, world, n_lr):
+    """Doubles in the exchange buffer of a sharded handle: world * ceil(n_bunches / world) * n_lr * 2."""
+    return int(lib().mbt_shard_exchange_doubles(int(n_bunches), int(world), int(n_lr)))
+
+
 def philox_selftest(ctr, key):
     c = (C.c_uint32 * 4)(*ctr)
     k = (C.c_uint32 * 2)(*key)
@@ -179,7 +201,7 @@ def normal_selftest(seed, ctr):
     return out
 
 
-def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None, device=-1, tuning=None):
+def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None, device=-1, tuning=None, shard=None):
     """Workload dict (paper_1809_00391_b200.workloads) -> (mbt_params, keep-alive list).
     tuning: dict of mbt_tuning members (mbt.h), e.g. dict(turn_mode=1); omitted members are 0 = the library's choice."""
     f, w = cfg["fill"], cfg["wake"]
@@ -210,6 +232,8 @@ def make_params(cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None
         if k not in TUNING_FIELDS:
             raise KeyError(k)
         setattr(p.tuning, k, int(v))
+    if shard:
+        p.shard = Shard(1, int(shard["rank"]), int(shard["world"]), shard.get("d_exchange"))
     tr = cfg.get("transverse")
     tres = None
     if tr:
@@ -225,16 +249,19 @@ class Tracker:
     """One mbt_handle.  `d_tau` / `d_delta` / `stream` are raw device pointers / cudaStream_t values (ints),
     e.g. ``tensor.data_ptr()`` and ``torch.cuda.current_stream().cuda_stream``."""
 
-    def __init__(self, cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None, device=-1, tuning=None):
+    def __init__(self, cfg, log_capacity_turns=0, d_tau=None, d_delta=None, stream=None, device=-1, tuning=None, shard=None):
+        """shard: dict(rank=, world=, d_exchange=device pointer) makes this the handle of one rank of a bunch-sharded run
+        (mbt_shard in mbt.h); self.M is then the number of bunches this rank owns, self.Mg that of the whole fill."""
         L = lib()
         f, w = cfg["fill"], cfg["wake"]
-        self.M = len(f["buckets"])
+        self.Mg = len(f["buckets"])
+        self.first_bunch, self.M = shard_range(self.Mg, shard["world"], shard["rank"]) if shard else (0, self.Mg)
         self.Np = int(f["n_per_bunch"])
         self.nb = int(w["n_bins"])
         self.R_lr = sum(1 for r in w["resonators"] if r["flags"] & 2)
         self.K = int(w["history_turns"]) if self.R_lr else 0
         self.K_rw = int((cfg.get("transverse") or {}).get("rw_turns", 0))
-        p, self._keep = make_params(cfg, log_capacity_turns, d_tau, d_delta, stream, device, tuning)
+        p, self._keep = make_params(cfg, log_capacity_turns, d_tau, d_delta, stream, device, tuning, shard)
         self._h = C.c_void_p()
         self._L = L
         _ck(L.mbt_create(C.byref(p), C.byref(self._h)))
@@ -325,8 +352,14 @@ class Tracker:
         _ck(self._L.mbt_get_moment_log(self._h, int(first_turn), int(n), _dp(out)))
         return out
 
+    def shard_turn_begin(self):
+        _ck(self._L.mbt_shard_turn_begin(self._h))
+
+    def shard_turn_end(self):
+        _ck(self._L.mbt_shard_turn_end(self._h))
+
     def lr_history(self):
-        out = np.zeros((max(self.K, 0), self.M, max(self.R_lr, 0), 2))
+        out = np.zeros((max(self.K, 0), self.Mg, max(self.R_lr, 0), 2))
         if out.size:
             _ck(self._L.mbt_get_lr_history(self._h, _dp(out)))
         return out
