@@ -824,17 +824,35 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
     const double lo_old = A.lo_hist[b];
     const double lo_new = MAP ? A.lo_next[b] : lo_old;
 
-    // stage the gather cells of bunch b's wake: cellSR + sum_r Re[cellF_r P[b][r]] (S6 expansion); clear the counts
+    // stage the gather cells of bunch b's wake: cellSR + sum_r Re[cellF_r P[b][r]] (S6 expansion); clear the counts.
+    // All loads of a cell -- its short-range part and, for up to four resonators, the table cell and the phasor -- are
+    // issued before the first of them is used: one trip to L2 per cell, where a loop over the resonators made 1 + R_lr
+    // dependent ones (c4: 3 per CTA prologue, 4.9 waves of CTAs per pass).
     for (int k = tid; k < nb + 2; k += kPassThreads) {
       WakeCell c{0.0, 0.0};
       if (have_kick) {
+        constexpr int RU = 4;
+        CellF f[RU];
+        cplx pb[RU];
         c = A.cellSR[(size_t)b * (nb + 2) + k];
+#pragma unroll
+        for (int r = 0; r < RU; ++r)
+          if (r < A.R) {
+            f[r] = A.cellF[(size_t)r * (nb + 2) + k];
+            pb[r] = A.P[(size_t)b * A.R + r];
+          }
+#pragma unroll
+        for (int r = 0; r < RU; ++r)
+          if (r < A.R) {
+            c.mid += fma(f[r].mid.re, pb[r].re, -(f[r].mid.im * pb[r].im));
+            c.dif += fma(f[r].dif.re, pb[r].re, -(f[r].dif.im * pb[r].im));
+          }
 #pragma unroll 1
-        for (int r = 0; r < A.R; ++r) {
-          const CellF f = A.cellF[(size_t)r * (nb + 2) + k];
-          const cplx pb = A.P[(size_t)b * A.R + r];
-          c.mid += fma(f.mid.re, pb.re, -(f.mid.im * pb.im));
-          c.dif += fma(f.dif.re, pb.re, -(f.dif.im * pb.im));
+        for (int r = RU; r < A.R; ++r) {
+          const CellF fr = A.cellF[(size_t)r * (nb + 2) + k];
+          const cplx pr = A.P[(size_t)b * A.R + r];
+          c.mid += fma(fr.mid.re, pr.re, -(fr.mid.im * pr.im));
+          c.dif += fma(fr.dif.re, pr.re, -(fr.dif.im * pr.im));
         }
       }
       sW[k] = c;
