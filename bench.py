@@ -260,7 +260,7 @@ def run_mbt(args):
         torch.cuda.synchronize()
 
     tuning = {k: v for k, v in (("turn_mode", args.turn_mode), ("tile_iters", args.tile_iters),
-                                ("pairs_per_thread", args.pairs_per_thread), ("pdl", args.pdl), ("verbose", args.verbose)) if v}
+                                ("pairs_per_thread", args.pairs_per_thread), ("pdl", args.pdl), ("verbose", args.verbose), ("per_bunch_start", args.per_bunch_start)) if v}
     trk = mbt.Tracker(cfg, log_capacity_turns=0, device=local, tuning=tuning)
     trk.track(Wm)
     trk.moments()
@@ -418,6 +418,7 @@ def main():
     ap.add_argument("--pairs-per-thread", type=int, default=0, help="mbt_tuning.pairs_per_thread")
     ap.add_argument("--pdl", type=int, default=0, help="mbt_tuning.pdl")
     ap.add_argument("--verbose", type=int, default=0)
+    ap.add_argument("--per-bunch-start", type=int, default=0, help="mbt_tuning.per_bunch_start")
     ap.add_argument("--sharded", action="store_true", help="opt-in bunch-sharded path (strong scaling; see run_sharded)")
     args = ap.parse_args()
     if args.warmup < 3:

@@ -120,10 +120,12 @@ typedef struct { int32_t enable; mbt_plane x, y; int32_t n_res; const mbt_resona
  *   turn_mode         1: a turn is two launches (k_pass, k_wake); 2: one launch (the last pass CTA of a bunch builds that
  *                     bunch's wake, the last CTA of the grid closes the turn); 3: the chip-resident persistent kernel
  *                     (whole mbt_track in one cooperative launch; MBT_EINVAL if the particle store does not fit on chip)
- *   verbose           1: print the chosen launch shapes to stderr at create */
+ *   verbose           1: print the chosen launch shapes to stderr at create
+ *   per_bunch_start   1: every pass CTA waits for the whole wake kernel before it (griddepcontrol.wait); 2 (= the library's
+ *                     choice where one k_wake CTA serves a bunch): it waits for its own bunch's wake only */
 typedef struct {
-  int32_t tile_iters, pairs_per_thread, pdl, stages6, turn_mode, verbose;
-  int32_t reserved[2]; /* must be 0 */
+  int32_t tile_iters, pairs_per_thread, pdl, stages6, turn_mode, verbose, per_bunch_start;
+  int32_t reserved[1]; /* must be 0 */
 } mbt_tuning;
 
 /* Bunch sharding over several devices (the paper's own outlook, P:l.253: "splitting the bunches

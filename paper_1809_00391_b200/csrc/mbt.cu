@@ -161,7 +161,7 @@ struct mbt_handle {
   void (*fn_flush)(const Args, const WakeArgs) = nullptr;  // k_pass<false, ...>
   bool fused = false;  // a turn is ONE launch: the pass's last CTA of a bunch builds the bunch's wake (mbt_tuning.turn_mode 2)
   DevBuf<uint32_t> bunch_done;
-  DevBuf<uint32_t> a_ready, bunch_ready, agg_ready;
+  DevBuf<uint32_t> a_ready, bunch_ready, agg_ready, tile_turn;
   DevBuf<cplx> gd;
   int npair = 1;
   int pdl = 1;  // bit 0: the pass, bit 1: k_wake launched as a programmatic dependent (longitudinal handles; mbt_tuning.pdl sets it).
@@ -368,7 +368,7 @@ void destroy(mbt_handle *h) {
   h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
   h->cellSR.release(); h->cellF.release();
   h->rd_cnt.release(); h->wr_cnt.release(); h->bunch_done.release();
-  h->a_ready.release(); h->bunch_ready.release(); h->agg_ready.release(); h->gd.release();
+  h->a_ready.release(); h->bunch_ready.release(); h->agg_ready.release(); h->gd.release(); h->tile_turn.release();
   h->tx.release(); h->txp.release(); h->ty.release(); h->typ.release(); h->wt.release(); h->Sfix.release(); h->Sov.release();
   h->S_last.release(); h->Ktab.release(); h->acc2.release(); h->fix.release(); h->cellX.release(); h->cellY.release();
   h->mom_tr_acc.release(); h->mom_tr.release();
@@ -478,7 +478,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   const mbt_tuning &tn = p->tuning;
   if (tn.tile_iters < 0 || tn.pairs_per_thread < 0 || tn.pairs_per_thread > 2 || tn.pdl < 0 || tn.pdl > 3 || tn.stages6 < 0 ||
       (tn.stages6 != 0 && (tn.stages6 < 2 || tn.stages6 > kMaxStages6)) || tn.turn_mode < 0 || tn.turn_mode > 3 ||
-      tn.verbose < 0 || tn.reserved[0] != 0 || tn.reserved[1] != 0)
+      tn.verbose < 0 || tn.per_bunch_start < 0 || tn.per_bunch_start > 2 || tn.reserved[0] != 0)
     return fail(MBT_EINVAL, "tuning: a member is out of range (see mbt_tuning in mbt.h; all zero = the library's choice)");
   int n_lr = 0;
   for (int r = 0; r < wk.n_res; ++r) {
@@ -826,6 +826,11 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   CUH(h->bunch_done.alloc(M, h->stream));
   A.bunch_done = h->bunch_done.p;
   A.b0 = b0;
+  CUH(h->tile_turn.alloc((size_t)M * h->grid_pass, h->stream));
+  A.tile_turn = h->tile_turn.p;
+  A.bunch_ready = h->bunch_ready.p;
+  // a pass CTA starts on its own bunch's wake (one k_wake CTA per bunch publishes bunch_ready) instead of on the whole grid
+  A.flag_wait = (!tr.enable && !sh.enable && h->wargs.gather_P && tn.per_bunch_start != 1) ? 1 : 0;
   h->fused = !tr.enable && !sh.enable && (tn.turn_mode == 2 || (tn.turn_mode == 0 && kFusedTurnDefault));
   if (tn.turn_mode == 2 && tr.enable) {
     destroy(h);
@@ -833,6 +838,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   }
   if (h->fused && h->smem_pass < wake_smem_bytes(nb, Mg)) h->fused = false;  // cannot happen for nb <= MBT_MAX_BINS
   A.fused = h->fused ? 1 : 0;
+  if (h->fused) A.flag_wait = 0;  // the one-launch turn waits for its predecessor grid (it wrote the particles)
   if (tn.verbose)
     fprintf(stderr, "mbt: %s, %d pair(s) per thread, grid %d x %d, %zu B shared memory per CTA, pdl %d\n",
             h->fused ? "one launch per turn" : "two launches per turn", h->npair, h->grid_pass, M, h->smem_pass, h->pdl);
@@ -1175,7 +1181,7 @@ int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int
     if (rc) return rc;
   }
   k_set_ctrl<<<1, 256, 0, h->stream>>>(h->ctrl.p, (uint32_t)turn, 0u, h->a_ready.p, h->Mg * (h->R ? h->R : 1), h->bunch_ready.p, h->M,
-                                       h->agg_ready.p, h->bunch_done.p);
+                                       h->agg_ready.p, h->bunch_done.p, h->tile_turn.p, h->M * h->grid_pass);
   CU(cudaGetLastError());
   h->launches += 1;
   CU(cudaMemsetAsync(h->hist.p, 0, sizeof(uint32_t) * h->M * h->nb, h->stream));

@@ -43,7 +43,7 @@ struct Ctrl {
   uint32_t turn;          // completed turns
   uint32_t ticket;        // CTAs of k_wake that have finished (last-CTA-done election)
   uint32_t kick_pending;  // 1: the wake of turn `turn` has not been applied to delta yet
-  uint32_t pad;
+  uint32_t kick_base;     // the turn at which no kick was pending last (create, mbt_set_particles, a getter's flush)
 };
 
 // gather cell k of a wake grid V[0..nb) (D12): linear gather: the particle with rint(t) = k sits between the centres
@@ -99,6 +99,10 @@ struct Args {
   // one-launch turn (mbt_tuning.turn_mode 2): the last CTA of a bunch to finish builds that bunch's wake (wake_body)
   int32_t fused;              // 1: this launch is a whole turn; its predecessor in the stream is the pass before it
   int32_t b0;                 // global index of the handle's first bunch (Philox counter word; 0 unless sharded)
+  // per-bunch start (two-launch turn, one k_wake CTA per bunch): a pass CTA waits for ITS bunch's wake, not for the grid
+  int32_t flag_wait;
+  const uint32_t *bunch_ready;  // [M] turn whose wake of bunch b is complete (k_wake, release)
+  uint32_t *tile_turn;          // [M][tiles] completed turns of the tile: written by the tile's own CTA, read by its next one
   uint32_t *bunch_done;       // [M] pass CTAs of the bunch that have flushed their counts and moment sums
 };
 
@@ -815,14 +819,32 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
     // the control words, the gather cells, the phasors, the windows -- is read from here on.  In the one-launch turn the
     // predecessor is the pass before, which wrote the particles: the first stages are issued after the wait.
     griddep_launch_dependents();  // the kernel after this pass may become resident; it waits for this grid itself
-    griddep_wait();
+    // What this CTA needs of the wake kernel before it is the wake of ITS bunch: with one k_wake CTA per bunch
+    // (flag_wait) it waits for bunch_ready[b] instead of the whole grid -- the CTAs of the first bunches stream while the
+    // wakes of the last ones, and the closing of the turn, are still under way.  The turn number cannot then come from
+    // the control word (the closing CTA may not have bumped it yet): the tile's own CTA of the pass before left it in
+    // tile_turn (that pass is complete: the wake kernel in between waited for it).  A wait that reads a stale flag just
+    // keeps waiting; everything the wake kernel wrote is read through L2 below (__ldcg), never through an L1 line.
+    __shared__ uint32_t s_turn;
+    const bool by_flag = MAP && A.flag_wait != 0;
+    if (by_flag) {
+      if (tid == 0) {
+        const uint32_t done = __ldcg(&A.tile_turn[(size_t)b * gridDim.x + blockIdx.x]);
+        wait_turn(&A.bunch_ready[b], done);
+        s_turn = done;
+      }
+      __syncthreads();
+    } else {
+      griddep_wait();
+    }
     if (tid == 0 && fused)
       for (uint32_t k = 0; k + 1u < (uint32_t)kStages && k < n_it; ++k) issue(k);
-    const uint32_t n = A.ctrl->turn + 1u;  // the turn this pass tracks (Philox counter word, D24)
-    const bool have_kick = A.ctrl->kick_pending != 0u;
+    const uint32_t n_done = by_flag ? s_turn : A.ctrl->turn;
+    const uint32_t n = n_done + 1u;  // the turn this pass tracks (Philox counter word, D24)
+    const bool have_kick = by_flag ? (n_done != A.ctrl->kick_base) : (A.ctrl->kick_pending != 0u);
     // window of the wake being applied (S0) and window this pass bins with (S4); the flush pass re-bins on the former
-    const double lo_old = A.lo_hist[b];
-    const double lo_new = MAP ? A.lo_next[b] : lo_old;
+    const double lo_old = __ldcg(&A.lo_hist[b]);
+    const double lo_new = MAP ? __ldcg(&A.lo_next[b]) : lo_old;
 
     // stage the gather cells of bunch b's wake: cellSR + sum_r Re[cellF_r P[b][r]] (S6 expansion); clear the counts.
     // All loads of a cell -- its short-range part and, for up to four resonators, the table cell and the phasor -- are
@@ -834,12 +856,15 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
         constexpr int RU = 4;
         CellF f[RU];
         cplx pb[RU];
-        c = A.cellSR[(size_t)b * (nb + 2) + k];
+        {
+          const double2 v = __ldcg(reinterpret_cast<const double2 *>(&A.cellSR[(size_t)b * (nb + 2) + k]));
+          c.mid = v.x; c.dif = v.y;
+        }
 #pragma unroll
         for (int r = 0; r < RU; ++r)
           if (r < A.R) {
             f[r] = A.cellF[(size_t)r * (nb + 2) + k];
-            pb[r] = A.P[(size_t)b * A.R + r];
+            pb[r] = __ldcg_cplx(&A.P[(size_t)b * A.R + r]);
           }
 #pragma unroll
         for (int r = 0; r < RU; ++r)
@@ -850,7 +875,7 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
 #pragma unroll 1
         for (int r = RU; r < A.R; ++r) {
           const CellF fr = A.cellF[(size_t)r * (nb + 2) + k];
-          const cplx pr = A.P[(size_t)b * A.R + r];
+          const cplx pr = __ldcg_cplx(&A.P[(size_t)b * A.R + r]);
           c.mid += fma(fr.mid.re, pr.re, -(fr.mid.im * pr.im));
           c.dif += fma(fr.dif.re, pr.re, -(fr.dif.im * pr.im));
         }
@@ -1080,6 +1105,7 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
       if (c) atomicAdd(&A.hist[(size_t)b * nb + j], c);
     }
     if (MAP) {
+      if (tid == 0 && A.tile_turn) A.tile_turn[(size_t)b * gridDim.x + blockIdx.x] = n;
       if (!fused) return;
       // One-launch turn: the CTA that completes bunch b (every other CTA of the bunch has flushed its counts and sums:
       // barrier, one thread's fence, then the counter) builds the bunch's wake while other bunches still stream -- S5, the
@@ -1167,7 +1193,8 @@ __global__ void k_aggregate_history(int M, int R, int K, const cplx *ring_a, con
 
 // set the turn counter; every flag of the one-launch turn says "complete through `turn`"
 __global__ void k_set_ctrl(Ctrl *c, uint32_t turn, uint32_t pending, uint32_t *a_ready, int n_a, uint32_t *bunch_ready, int M,
-                           uint32_t *agg_ready, uint32_t *bunch_done) {
+                           uint32_t *agg_ready, uint32_t *bunch_done, uint32_t *tile_turn, int n_tiles) {
+  for (int i = threadIdx.x; i < n_tiles; i += blockDim.x) tile_turn[i] = turn;
   for (int i = threadIdx.x; i < n_a; i += blockDim.x) a_ready[i] = turn;
   for (int i = threadIdx.x; i < M; i += blockDim.x) { bunch_ready[i] = turn; bunch_done[i] = 0u; }
   if (threadIdx.x == 0) {
@@ -1175,9 +1202,13 @@ __global__ void k_set_ctrl(Ctrl *c, uint32_t turn, uint32_t pending, uint32_t *a
     c->turn = turn;
     c->ticket = 0u;
     c->kick_pending = pending;
+    c->kick_base = turn;
   }
 }
-__global__ void k_clear_pending(Ctrl *c) { c->kick_pending = 0u; }
+__global__ void k_clear_pending(Ctrl *c) {
+  c->kick_pending = 0u;
+  c->kick_base = c->turn;
+}
 
 // Sharded handle, after the all-gather of the exchange buffer: the source phasors of ALL bunches of the turn being closed
 // go into the history ring (so that every rank holds the whole history), and their flags are raised, so that the phasor

@@ -67,11 +67,11 @@ class Transverse(C.Structure):
                 ("rw_amp_x", C.c_double), ("rw_amp_y", C.c_double), ("rw_turns", C.c_int32)]
 
 
-TUNING_FIELDS = ("tile_iters", "pairs_per_thread", "pdl", "stages6", "turn_mode", "verbose")
+TUNING_FIELDS = ("tile_iters", "pairs_per_thread", "pdl", "stages6", "turn_mode", "verbose", "per_bunch_start")
 
 
 class Tuning(C.Structure):
-    _fields_ = [(k, C.c_int32) for k in TUNING_FIELDS] + [("reserved", C.c_int32 * 2)]
+    _fields_ = [(k, C.c_int32) for k in TUNING_FIELDS] + [("reserved", C.c_int32 * 1)]
 
 
 class Shard(C.Structure):

@@ -89,7 +89,7 @@ def test_make_params_marshalling():
     assert p.wake.n_res == 3 and p.wake.res[2].fr_Hz == 2.1e9 and p.wake.res[0].flags == 1
     assert p.wake.history_turns == 20 and p.log_capacity_turns == 7 and p.seed == 4
     assert np.isnan(p.cav[0].phase_rad)
-    assert all(getattr(p.tuning, k) == 0 for k in mbt.TUNING_FIELDS) and list(p.tuning.reserved) == [0, 0]
+    assert all(getattr(p.tuning, k) == 0 for k in mbt.TUNING_FIELDS) and list(p.tuning.reserved) == [0]
     p, keep = mbt.make_params(cfg, tuning=dict(turn_mode=1, tile_iters=3))
     assert p.tuning.turn_mode == 1 and p.tuning.tile_iters == 3 and p.tuning.pdl == 0
     with pytest.raises(KeyError):
