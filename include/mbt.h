@@ -122,7 +122,8 @@ typedef struct { int32_t enable; mbt_plane x, y; int32_t n_res; const mbt_resona
  *                     (whole mbt_track in one cooperative launch; MBT_EINVAL if the particle store does not fit on chip)
  *   verbose           1: print the chosen launch shapes to stderr at create
  *   per_bunch_start   1: every pass CTA waits for the whole wake kernel before it (griddepcontrol.wait); 2 (= the library's
- *                     choice where one k_wake CTA serves a bunch): it waits for its own bunch's wake only */
+ *                     choice where one k_wake CTA serves a bunch): it waits for its own bunch's wake only, and the wake
+ *                     kernel's CTA of a bunch for that bunch's pass CTAs only; 3: the former without the latter */
 typedef struct {
   int32_t tile_iters, pairs_per_thread, pdl, stages6, turn_mode, verbose, per_bunch_start;
   int32_t reserved[1]; /* must be 0 */

@@ -336,6 +336,7 @@ int flush(mbt_handle *h) {
   WakeArgs wa = h->wargs;
   wa.mode = 1;
   wa.S = 1;
+  wa.bunch_wait = 0;
   if (h->trans) h->fn_flush6<<<dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream>>>(h->args6);
   else h->fn_flush<<<dim3(h->grid_pass, h->M), kPassThreads, h->smem_pass, h->stream>>>(h->args, wa);
   CU(cudaGetLastError());
@@ -478,7 +479,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   const mbt_tuning &tn = p->tuning;
   if (tn.tile_iters < 0 || tn.pairs_per_thread < 0 || tn.pairs_per_thread > 2 || tn.pdl < 0 || tn.pdl > 3 || tn.stages6 < 0 ||
       (tn.stages6 != 0 && (tn.stages6 < 2 || tn.stages6 > kMaxStages6)) || tn.turn_mode < 0 || tn.turn_mode > 3 ||
-      tn.verbose < 0 || tn.per_bunch_start < 0 || tn.per_bunch_start > 2 || tn.reserved[0] != 0)
+      tn.verbose < 0 || tn.per_bunch_start < 0 || tn.per_bunch_start > 3 || tn.reserved[0] != 0)
     return fail(MBT_EINVAL, "tuning: a member is out of range (see mbt_tuning in mbt.h; all zero = the library's choice)");
   int n_lr = 0;
   for (int r = 0; r < wk.n_res; ++r) {
@@ -839,6 +840,14 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   if (h->fused && h->smem_pass < wake_smem_bytes(nb, Mg)) h->fused = false;  // cannot happen for nb <= MBT_MAX_BINS
   A.fused = h->fused ? 1 : 0;
   if (h->fused) A.flag_wait = 0;  // the one-launch turn waits for its predecessor grid (it wrote the particles)
+  // ... and the wake kernel's CTA of a bunch starts on its own bunch's pass CTAs (launched as a programmatic dependent)
+  if (A.flag_wait && tn.per_bunch_start != 3) {
+    A.count_done = 1;
+    h->wargs.bunch_wait = 1;
+    h->wargs.tiles = h->grid_pass;
+    h->wargs.bunch_done = h->bunch_done.p;
+    if (!tn.pdl) h->pdl |= 2;
+  }
   if (tn.verbose)
     fprintf(stderr, "mbt: %s, %d pair(s) per thread, grid %d x %d, %zu B shared memory per CTA, pdl %d\n",
             h->fused ? "one launch per turn" : "two launches per turn", h->npair, h->grid_pass, M, h->smem_pass, h->pdl);

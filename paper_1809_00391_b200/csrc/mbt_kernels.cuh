@@ -41,9 +41,11 @@ __host__ __device__ __forceinline__ cplx cfma(cplx a, cplx b, cplx c) {
 // device-resident control words (so that a captured CUDA graph replays without parameter updates)
 struct Ctrl {
   uint32_t turn;          // completed turns
-  uint32_t ticket;        // CTAs of k_wake that have finished (last-CTA-done election)
+  uint32_t ticket[2];     // CTAs that have closed their bunch in the turn of this parity (last-CTA-done election; two
+                          // slots: the first CTAs of a turn's wake kernel may overlap the last ones of the turn before)
   uint32_t kick_pending;  // 1: the wake of turn `turn` has not been applied to delta yet
   uint32_t kick_base;     // the turn at which no kick was pending last (create, mbt_set_particles, a getter's flush)
+  uint32_t pad[3];
 };
 
 // gather cell k of a wake grid V[0..nb) (D12): linear gather: the particle with rint(t) = k sits between the centres
@@ -101,6 +103,7 @@ struct Args {
   int32_t b0;                 // global index of the handle's first bunch (Philox counter word; 0 unless sharded)
   // per-bunch start (two-launch turn, one k_wake CTA per bunch): a pass CTA waits for ITS bunch's wake, not for the grid
   int32_t flag_wait;
+  int32_t count_done;           // 1: count this CTA in bunch_done[b] when it has flushed (the wake kernel's CTA of the bunch waits for it)
   const uint32_t *bunch_ready;  // [M] turn whose wake of bunch b is complete (k_wake, release)
   uint32_t *tile_turn;          // [M][tiles] completed turns of the tile: written by the tile's own CTA, read by its next one
   uint32_t *bunch_done;       // [M] pass CTAs of the bunch that have flushed their counts and moment sums
@@ -209,6 +212,8 @@ struct WakeArgs {
   Ctrl *ctrl;
   uint32_t smem_wake_bytes, smem_pass_bytes;  // dynamic shared memory of a k_wake launch / of a pass launch (one-launch turn)
   // one-launch turn: per-bunch phasor gather instead of the scan (wake_body<false, true>)
+  int32_t bunch_wait, tiles;  // 1: a CTA waits for the `tiles` pass CTAs of ITS bunch (bunch_done) instead of the pass's grid
+  uint32_t *bunch_done;       // [M] (the pass counts, this kernel's CTA of the bunch resets)
   int32_t part;               // 0: the whole wake; sharded handle: 1 = up to the gather cells, 2 = phasor gather and close
   int32_t Mg, b0;             // bunches of the whole fill and index of this handle's first one (Mg = M, b0 = 0 unless sharded)
   cplx *xbuf;                 // sharded: [Mg padded][R] exchange buffer of the turn's source phasors (else nullptr)
@@ -280,7 +285,9 @@ __device__ __forceinline__ bool wake_first(const WakeArgs &A, const int b, const
   const int tid = threadIdx.x;
   const int lane = tid & 31, warp = tid >> 5;
   const int S = SPLIT ? A.S : 1;  // few bunches: S CTAs share a bunch (split 0 also does the per-bunch work)
-  const uint32_t n_done = A.ctrl->turn;  // completed turns; the turn being closed is n_done + 1
+  // completed turns; the turn being closed is n_done + 1.  One CTA per bunch: from the bunch's own flag (what this bunch's
+  // CTA of the turn before published -- the control word may still be waiting for that turn's closing CTA)
+  const uint32_t n_done = FUSED ? __ldcg(&A.bunch_ready[b]) : A.ctrl->turn;
   const uint32_t n = n_done + 1u;
 
   // counts -> charges; keep a copy of the counts; clear the accumulator for the next pass.  The loads of a round (counts,
@@ -512,7 +519,7 @@ __device__ __forceinline__ void wake_second(const WakeArgs &A, const int b, doub
   __shared__ bool s_last;
   const int tid = threadIdx.x;
   const int lane = tid & 31, warp = tid >> 5;
-  const uint32_t n = A.ctrl->turn + 1u;  // the turn being closed
+  const uint32_t n = (FUSED ? __ldcg(&A.bunch_ready[b]) : A.ctrl->turn) + 1u;  // the turn being closed
   const bool follow = A.mode == 0 && A.window_mode == 1;
   const int32_t s_used = follow ? A.s_hist[b] : 0;  // the window this turn's counts were taken on (set by wake_first)
   const int M = A.M, R = A.R, K = A.K;
@@ -568,7 +575,7 @@ __device__ __forceinline__ void wake_second(const WakeArgs &A, const int b, doub
     if (tid == 0) {
       __threadfence();
       st_release_u32(&A.bunch_ready[b], n);
-      s_last = (atomicAdd(&A.ctrl->ticket, 1u) == (uint32_t)(M - 1));
+      s_last = (atomicAdd(&A.ctrl->ticket[n & 1u], 1u) == (uint32_t)(M - 1));
     }
     __syncthreads();
     if (!s_last) return;
@@ -599,7 +606,7 @@ __device__ __forceinline__ void wake_second(const WakeArgs &A, const int b, doub
     if (tid == 0) {
       __threadfence();
       st_release_u32(A.agg_ready, n);
-      A.ctrl->ticket = 0u;
+      A.ctrl->ticket[n & 1u] = 0u;
       A.ctrl->kick_pending = 1u;
       A.ctrl->turn = n;
     }
@@ -609,7 +616,7 @@ __device__ __forceinline__ void wake_second(const WakeArgs &A, const int b, doub
   __syncthreads();
   if (tid == 0) {
     __threadfence();
-    s_last = (atomicAdd(&A.ctrl->ticket, 1u) == (uint32_t)(A.M - 1));
+    s_last = (atomicAdd(&A.ctrl->ticket[n & 1u], 1u) == (uint32_t)(A.M - 1));
   }
   __syncthreads();
   if (!s_last) return;
@@ -709,7 +716,7 @@ __device__ __forceinline__ void wake_second(const WakeArgs &A, const int b, doub
   }
   __syncthreads();
   if (tid == 0) {
-    A.ctrl->ticket = 0u;
+    A.ctrl->ticket[n & 1u] = 0u;
     A.ctrl->kick_pending = 1u;
     A.ctrl->turn = n;
   }
@@ -735,7 +742,20 @@ __device__ __forceinline__ void wake_body(const WakeArgs &A, const int b, const 
 
 __global__ void __launch_bounds__(kWakeThreads, 3) k_wake(const __grid_constant__ WakeArgs A) {
   extern __shared__ double smem_wake[];
-  griddep_wait();               // the pass of this turn is complete (counts, moment sums)
+  // The pass of this turn is complete (counts, moment sums) -- or, with bunch_wait (one CTA per bunch, launched as a
+  // programmatic dependent of the pass): the pass CTAs of THIS bunch are.  CTAs that become resident during the pass's last
+  // wave then build the wakes of the bunches that are long complete, and the next pass -- whose CTAs wait for their own
+  // bunch's wake -- finds them ready when it starts.
+  if (A.bunch_wait) {
+    if (threadIdx.x == 0) {
+      while (ld_acquire_u32(&A.bunch_done[blockIdx.x]) < (uint32_t)A.tiles) {
+      }
+      A.bunch_done[blockIdx.x] = 0u;
+    }
+    __syncthreads();
+  } else {
+    griddep_wait();
+  }
   griddep_launch_dependents();  // the next pass may become resident: it stages what does not depend on this kernel
   if (A.S > 1) wake_body<true, false>(A, (int)blockIdx.x, (int)blockIdx.y, smem_wake, A.smem_wake_bytes);
   else if (A.gather_P) wake_body<false, true>(A, (int)blockIdx.x, 0, smem_wake, A.smem_wake_bytes);
@@ -1106,7 +1126,7 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
     }
     if (MAP) {
       if (tid == 0 && A.tile_turn) A.tile_turn[(size_t)b * gridDim.x + blockIdx.x] = n;
-      if (!fused) return;
+      if (!fused && !A.count_done) return;
       // One-launch turn: the CTA that completes bunch b (every other CTA of the bunch has flushed its counts and sums:
       // barrier, one thread's fence, then the counter) builds the bunch's wake while other bunches still stream -- S5, the
       // S6 source, the gather cells, the closing of S7, and the phasor P[b] gathered from the sources of the bunches ahead
@@ -1120,7 +1140,7 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
       __syncthreads();
       if (tid == 0) {
         __threadfence();
-        s_mine = (atomicAdd(&A.bunch_done[b], 1u) == gridDim.x - 1u);
+        s_mine = (atomicAdd(&A.bunch_done[b], 1u) == gridDim.x - 1u) && fused;
         if (s_mine) A.bunch_done[b] = 0u;
       }
       __syncthreads();
@@ -1200,7 +1220,7 @@ __global__ void k_set_ctrl(Ctrl *c, uint32_t turn, uint32_t pending, uint32_t *a
   if (threadIdx.x == 0) {
     *agg_ready = turn;
     c->turn = turn;
-    c->ticket = 0u;
+    c->ticket[0] = c->ticket[1] = 0u;
     c->kick_pending = pending;
     c->kick_base = turn;
   }
