@@ -1138,9 +1138,16 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
       // i.e. after this grid has completed.
       __shared__ bool s_mine;
       __syncthreads();
+      if (!fused) {  // two-launch turn, wake kernel starting per bunch: release this CTA's counts and sums, count it, done
+        if (tid == 0) {
+          __threadfence();
+          atomicAdd(&A.bunch_done[b], 1u);  // result unused: a reduction, nobody waits for its round trip
+        }
+        return;
+      }
       if (tid == 0) {
         __threadfence();
-        s_mine = (atomicAdd(&A.bunch_done[b], 1u) == gridDim.x - 1u) && fused;
+        s_mine = (atomicAdd(&A.bunch_done[b], 1u) == gridDim.x - 1u);
         if (s_mine) A.bunch_done[b] = 0u;
       }
       __syncthreads();
