@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libmbt.so")
 SOURCES = ["mbt.cu"]
-DEPS = ["mbt.cu", "mbt_kernels.cuh", "mbt_trans.cuh", "mbt_math.cuh", "mbt_coeffs.inc", "gen_coeffs.py",
+DEPS = ["mbt.cu", "mbt_kernels.cuh", "mbt_trans.cuh", "mbt_resident.cuh", "mbt_math.cuh", "mbt_coeffs.inc", "gen_coeffs.py",
         os.path.join("..", "..", "include", "mbt.h"), os.path.join("..", "build.py")]
 
 NVCC_FLAGS = [

@@ -13,6 +13,7 @@
 
 #include "mbt_kernels.cuh"
 #include "mbt_trans.cuh"
+#include "mbt_resident.cuh"
 
 using namespace mbt;
 
@@ -24,6 +25,9 @@ thread_local std::string g_err;
 // every BASELINE workload: a bunch's wake costs its closing CTA ~15 us of latency-bound work during
 // which it holds one of the pass's 296 CTA slots (c4: 0.238 vs 0.218 ms per turn).
 constexpr bool kFusedTurnDefault = false;
+// mbt_tuning.turn_mode 0 picks the chip-resident turn loop for workloads of at most this many particles that fit on chip
+constexpr bool kResidentAuto = false;
+constexpr int64_t kResidentAutoMaxParticles = 2000000;
 
 int fail(int code, const std::string &msg) {
   g_err = msg;
@@ -159,6 +163,14 @@ struct mbt_handle {
   DevBuf<Ctrl> ctrl;
   void (*fn_map)(const Args, const WakeArgs) = nullptr;    // k_pass<true, ...> chosen for this handle's effects
   void (*fn_flush)(const Args, const WakeArgs) = nullptr;  // k_pass<false, ...>
+  // chip-resident turn loop (mbt_resident.cuh): one cooperative launch per mbt_track call
+  bool resident = false;
+  void (*fn_res)(const Args, const WakeArgs, const ResArgs) = nullptr;
+  ResArgs rargs;
+  WakeArgs wargs_res;
+  size_t smem_res = 0;
+  int grid_res = 0;
+  DevBuf<uint32_t> res_bar;
   bool fused = false;  // a turn is ONE launch: the pass's last CTA of a bunch builds the bunch's wake (mbt_tuning.turn_mode 2)
   DevBuf<uint32_t> bunch_done;
   DevBuf<uint32_t> a_ready, bunch_ready, agg_ready, tile_turn;
@@ -225,6 +237,14 @@ void choose_tiles(int64_t ppb, int64_t stride, int M, int slots, int tile_iters,
   if (verbose)
     fprintf(stderr, "mbt: choose_tiles ppb %lld stride %lld M %d slots %d -> %lld iterations, %d tiles\n", (long long)ppb,
             (long long)stride, M, slots, (long long)iters, *tiles);
+}
+
+typedef void (*res_fn)(const Args, const WakeArgs, const ResArgs);
+res_fn select_resident(bool rad, int gather, int n_cav) {
+#define MBT_SEL_(R, G) (n_cav == 1 ? (res_fn)k_resident<R, G, 1> : n_cav == 2 ? (res_fn)k_resident<R, G, 2> : (res_fn)k_resident<R, G, 0>)
+  if (rad) return gather ? MBT_SEL_(true, 1) : MBT_SEL_(true, 0);
+  return gather ? MBT_SEL_(false, 1) : MBT_SEL_(false, 0);
+#undef MBT_SEL_
 }
 
 typedef void (*pass6_fn)(const Args6);
@@ -295,7 +315,7 @@ cudaError_t enqueue_wakes(mbt_handle *h) {
   return e;
 }
 // launches per tracked turn: 1 in the one-launch turn, else 2; 3 with the transverse planes; 4 with their resistive-wall kick
-int launches_per_turn(const mbt_handle *h) { return h->fused ? 1 : h->trans ? (h->Krw > 0 ? 4 : 3) : 2; }
+int launches_per_turn(const mbt_handle *h) { return h->resident ? 0 : h->fused ? 1 : h->trans ? (h->Krw > 0 ? 4 : 3) : 2; }
 
 cudaError_t enqueue_turn(mbt_handle *h) {
   cudaError_t e = enqueue_pass(h);
@@ -369,7 +389,7 @@ void destroy(mbt_handle *h) {
   h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
   h->cellSR.release(); h->cellF.release();
   h->rd_cnt.release(); h->wr_cnt.release(); h->bunch_done.release();
-  h->a_ready.release(); h->bunch_ready.release(); h->agg_ready.release(); h->gd.release(); h->tile_turn.release();
+  h->a_ready.release(); h->bunch_ready.release(); h->agg_ready.release(); h->gd.release(); h->tile_turn.release(); h->res_bar.release();
   h->tx.release(); h->txp.release(); h->ty.release(); h->typ.release(); h->wt.release(); h->Sfix.release(); h->Sov.release();
   h->S_last.release(); h->Ktab.release(); h->acc2.release(); h->fix.release(); h->cellX.release(); h->cellY.release();
   h->mom_tr_acc.release(); h->mom_tr.release();
@@ -400,6 +420,34 @@ int upload_window(mbt_handle *h, const int32_t *s_hist, const int32_t *s_next) {
   CU(cudaMemcpyAsync(h->lo_hist.p, lh.data(), sizeof(double) * h->M, cudaMemcpyHostToDevice, h->stream));
   CU(cudaMemcpyAsync(h->lo_next.p, ln.data(), sizeof(double) * h->M, cudaMemcpyHostToDevice, h->stream));
   CU(cudaStreamSynchronize(h->stream));  // the host vectors go out of scope
+  return 0;
+}
+}  // namespace
+
+namespace {
+// the chip-resident turn loop: one cooperative launch per (at most 2^20) turns
+int track_resident(mbt_handle *h, int64_t n_turns) {
+  CU(cudaEventRecord(h->ev0, h->stream));
+  int64_t left = n_turns;
+  while (left > 0) {
+    const int64_t chunk = std::min<int64_t>(left, 1 << 20);
+    CU(cudaMemsetAsync(h->res_bar.p, 0, 2 * sizeof(uint32_t), h->stream));
+    ResArgs ra = h->rargs;
+    ra.n_turns = (int32_t)chunk;
+    void *args[3] = {(void *)&h->args, (void *)&h->wargs_res, (void *)&ra};
+    CU(cudaLaunchCooperativeKernel((const void *)h->fn_res, dim3(h->grid_res), dim3(kPassThreads), args, h->smem_res, h->stream));
+    left -= chunk;
+    h->launches += 1;
+  }
+  k_sync_flags<<<1, 256, 0, h->stream>>>(h->ctrl.p, h->a_ready.p, h->Mg * (h->R ? h->R : 1), h->bunch_ready.p, h->M, h->agg_ready.p,
+                                         h->tile_turn.p, h->M * h->grid_pass);
+  CU(cudaGetLastError());
+  h->launches += 1;
+  CU(cudaEventRecord(h->ev1, h->stream));
+  h->timed = true;
+  h->turn += n_turns;
+  h->dirty = true;
+  h->wake_valid = true;
   return 0;
 }
 }  // namespace
@@ -479,7 +527,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   const mbt_tuning &tn = p->tuning;
   if (tn.tile_iters < 0 || tn.pairs_per_thread < 0 || tn.pairs_per_thread > 2 || tn.pdl < 0 || tn.pdl > 3 || tn.stages6 < 0 ||
       (tn.stages6 != 0 && (tn.stages6 < 2 || tn.stages6 > kMaxStages6)) || tn.turn_mode < 0 || tn.turn_mode > 3 ||
-      tn.verbose < 0 || tn.per_bunch_start < 0 || tn.per_bunch_start > 3 || tn.reserved[0] != 0)
+      tn.verbose < 0 || tn.per_bunch_start < 0 || tn.per_bunch_start > 3 || tn.reserved[0] < 0)
     return fail(MBT_EINVAL, "tuning: a member is out of range (see mbt_tuning in mbt.h; all zero = the library's choice)");
   int n_lr = 0;
   for (int r = 0; r < wk.n_res; ++r) {
@@ -746,12 +794,16 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   WakeArgs &Wa = h->wargs;
   memset(&Wa, 0, sizeof Wa);
   Wa.M = M; Wa.nb = nb; Wa.R = R; Wa.K = K; Wa.Np = (uint32_t)h->Np; Wa.mode = 0;
-  {  // few bunches: deal the convolution of a bunch out over S CTAs (a warp of output pairs each, <= 2 waves of CTAs)
+  {  // few bunches and many bins: deal the convolution of a bunch out over S CTAs (<= 2 waves of CTAs).  Sharing a bunch
+     // costs three dependent elections (atomics, fences, a reload of V_SR): ~3 us, what one CTA needs for the whole
+     // register-blocked convolution of ~500 bins -- so up to 512 bins a bunch has ONE CTA (which also gives it the per-bunch
+     // phasor gather and the per-bunch start of the next pass); tuning.wake_splits overrides.
     const int pairs = (nb + 1) / 2;
-    int S = (pairs + 31) / 32;
+    int S = nb <= 512 ? 1 : (pairs + 31) / 32;
     const int room = (2 * prop.multiProcessorCount + M - 1) / M;
     if (S > room) S = room;
     if (S > 64) S = 64;
+    if (tn.reserved[0] > 0) S = std::min(tn.reserved[0], std::min(room, 64));  // measurement: forced number of splits
     if (S < 1 || sh.enable) S = 1;  // a sharded handle runs the per-bunch phasor gather: one CTA per bunch
     h->wake_splits = S;
   }
@@ -851,6 +903,60 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   if (tn.verbose)
     fprintf(stderr, "mbt: %s, %d pair(s) per thread, grid %d x %d, %zu B shared memory per CTA, pdl %d\n",
             h->fused ? "one launch per turn" : "two launches per turn", h->npair, h->grid_pass, M, h->smem_pass, h->pdl);
+
+  // ---- chip-resident turn loop (mbt_tuning.turn_mode 3; the library's choice when it fits and the workload is small
+  // enough to be latency-bound in the streaming path): grid = M x G_b CTAs, all resident (cooperative launch), each
+  // holding tile_pairs pairs of one bunch in shared memory
+  if (!tr.enable && !sh.enable && (tn.turn_mode == 3 || (tn.turn_mode == 0 && kResidentAuto))) {
+    res_fn fn = select_resident(rad_on, wk.gather_order, p->n_cav);
+    const int64_t ppb = h->ld / 2, stride = (int64_t)kPassThreads * 2;
+    bool ok = false;
+    for (int occ = 2; occ >= 1 && !ok; --occ) {
+      int gb = (prop.multiProcessorCount * occ) / M;                        // CTAs per bunch
+      gb = (int)std::min<int64_t>(gb, (ppb + stride - 1) / stride);         // at least one full iteration per CTA
+      if (gb < 1) continue;
+      uint32_t tile = (uint32_t)((ppb + gb - 1) / gb);
+      tile += tile & 1u;
+      const size_t wake_bytes = (h->smem_wake + 15) & ~(size_t)15;
+      const size_t smem = resident_smem_bytes(tile, nb, wake_bytes);
+      if (smem > (size_t)prop.sharedMemPerBlockOptin) continue;
+      if (cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); continue; }
+      int got = 0;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&got, (const void *)fn, kPassThreads, smem) != cudaSuccess) { cudaGetLastError(); continue; }
+      if ((int64_t)got * prop.multiProcessorCount < (int64_t)gb * M) continue;
+      int coop = 0;
+      cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+      if (!coop) continue;
+      // the automatic choice is for the latency-bound workloads only: a few waves' worth of streaming work per turn
+      if (tn.turn_mode == 0 && (int64_t)M * h->Np > kResidentAutoMaxParticles) continue;
+      ok = true;
+      h->resident = true;
+      h->fn_res = fn;
+      h->grid_res = gb * M;
+      h->smem_res = smem;
+      memset(&h->rargs, 0, sizeof h->rargs);
+      h->rargs.ctas_per_bunch = gb;
+      h->rargs.tile_pairs = tile;
+      h->rargs.wake_off = (uint32_t)(smem - wake_bytes - 16 + 15) & ~15u;
+      h->rargs.wake_bytes = (uint32_t)wake_bytes;
+      h->wargs_res = h->wargs;
+      h->wargs_res.S = std::min(h->wake_splits, gb);
+      h->wargs_res.bunch_wait = 0;
+    }
+    if (ok) {
+      CUH(h->res_bar.alloc(2, h->stream));
+      h->rargs.bar = h->res_bar.p;
+    } else if (tn.turn_mode == 3) {
+      destroy(h);
+      return fail(MBT_EINVAL, "tuning.turn_mode 3: the particle store does not fit in the chip's shared memory (or no cooperative launch)");
+    }
+    if (tn.verbose && ok)
+      fprintf(stderr, "mbt: chip-resident turn loop, %d CTAs per bunch, %u pairs per CTA, %zu B shared memory per CTA\n",
+              h->rargs.ctas_per_bunch, h->rargs.tile_pairs, h->smem_res);
+  } else if (tn.turn_mode == 3) {
+    destroy(h);
+    return fail(MBT_EINVAL, "tuning.turn_mode 3 (chip-resident) is not available with the transverse planes or bunch sharding");
+  }
 
   // ---- initial distribution (D20) on the device
   {
@@ -976,6 +1082,7 @@ int mbt_track(mbt_handle *h, int64_t n_turns) {
   if (h->sharded) return fail(MBT_ESTATE, "a sharded handle advances by mbt_shard_turn_begin / (all-gather) / mbt_shard_turn_end");
   CU(cudaSetDevice(h->device));
   if (n_turns == 0) return 0;
+  if (h->resident) return track_resident(h, n_turns);
   if (!h->graph1) {
     int rc = build_graph(h, 1, &h->graph1);
     if (rc) return rc;
@@ -1008,6 +1115,14 @@ int mbt_track_profiled(mbt_handle *h, int64_t n_turns, double *pass_seconds, dou
   if (h->turn + n_turns > 0xFFFFFFFFll) return fail(MBT_EINVAL, "turn counter would exceed 2^32");
   if (h->sharded) return fail(MBT_ESTATE, "not available on a sharded handle");
   CU(cudaSetDevice(h->device));
+  if (h->resident) {  // one launch does everything: its device time is the "pass", there is no separate wake kernel
+    if (int rc = track_resident(h, n_turns)) return rc;
+    const double sec = mbt_last_track_seconds(h);
+    if (sec < 0) return MBT_ECUDA;
+    *pass_seconds = sec;
+    *wake_seconds = 0.0;
+    return 0;
+  }
   struct Events {  // destroyed on every exit path
     std::vector<cudaEvent_t> v;
     ~Events() { for (cudaEvent_t e : v) if (e) cudaEventDestroy(e); }

@@ -767,6 +767,146 @@ __device__ __noinline__ void wake_bunch_fused(const WakeArgs &A, int b, double *
 }
 
 
+// One iteration of the fused pass on registers, for the NPAIR pairs (2 NPAIR particles) a thread owns: S0 S7 | S1 S2 S3 |
+// S4.  t2, d2: the pairs as loaded (tau, delta); tau, del: the particles after the iteration (the caller stores them).
+// p: the thread's first pair in the bunch, p1: end of the tile; sW: the bunch's gather cells, sL: the log table, sH: the
+// CTA's counts (bin nb is a sink).  Shared by the streaming pass (k_pass) and the chip-resident one (k_resident).
+template <bool MAP, bool RAD, int GATHER, int NCAV, int NPAIR, bool FULL>
+__device__ __forceinline__ void advance_pairs(const Args &A, const double2 (&t2)[NPAIR], const double2 (&d2)[NPAIR],
+                                              double (&tau)[2 * NPAIR], double (&del)[2 * NPAIR], const uint32_t p, const uint32_t p1,
+                                              const int b, const uint32_t n, const double lo_old, const double lo_new,
+                                              const uint32_t hi_nb, const int nb, const WakeCell *sW, const LogTabEntry *sL,
+                                              uint32_t *sH, double &st, double &sd, double &stt, double &sdd, uint32_t &nout) {
+  constexpr int NP = 2 * NPAIR;
+  double z[NP];
+  bool live[NP];
+  BmState bm[NPAIR];
+  uint32_t xs[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+  for (int q = 0; q < NPAIR; ++q) {
+    const uint32_t pq = p + q;
+    tau[2 * q] = t2[q].x; tau[2 * q + 1] = t2[q].y;
+    del[2 * q] = d2[q].x; del[2 * q + 1] = d2[q].y;
+    live[2 * q] = FULL || (pq < p1 && 2u * pq < A.Np);  // past the end of the tile: stale stage contents, ignored;
+    live[2 * q + 1] = FULL || (live[2 * q] && (2u * pq + 1u < A.Np));  // the slots from N_p up to ld are padding
+    z[2 * q] = z[2 * q + 1] = 0.0;
+    if (MAP && RAD) {
+      // one Philox block serves FOUR consecutive particles (D8): counter (particle >> 2, bunch, turn, tag 0);
+      // its words (x0, x1) give the Box-Muller pair of particles 4j, 4j+1, (x2, x3) that of 4j+2, 4j+3; the even
+      // particle of a pair takes z_c, the odd one z_s.  A thread that owns the whole quad (NPAIR = 2) calls it once.
+      if (q == 0 || NPAIR == 1) philox4x32_10(pq >> 1, (uint32_t)(b + A.b0), n, 0u, A.keys, xs[0], xs[1], xs[2], xs[3]);
+      const bool hi_half = (NPAIR == 2) ? (q == 1) : ((pq & 1u) != 0u);  // with NPAIR = 2 the thread's first pair is even
+      const double u1 = uniform32(A.mt, hi_half ? xs[2] : xs[0]), u2 = uniform32(A.mt, hi_half ? xs[3] : xs[1]);
+      if (NCAV > 0) bm[q] = box_muller_head(A.mt, sL, u1, u2, A.A_q);  // polynomials: lock step with S1's
+      else box_muller_fast(A.mt, sL, u1, u2, A.A_q, z[2 * q], z[2 * q + 1]);
+    }
+  }
+  // S0: kick of the previous turn's wake.  t exactly as the binning computed it (one subtraction, one
+  // multiplication, no contraction), so the in-window decision is the one that deposited the particle.
+  // In-window test 0 <= t < nb on the high word of t alone (in_window()): an integer compare, off the fp64 pipe.
+  double t[NP];
+  bool in[NP];
+#pragma unroll
+  for (int i = 0; i < NP; ++i) {
+    t[i] = __dmul_rn(__dsub_rn(tau[i], lo_old), A.invDelta);
+    in[i] = live[i] && in_window(t[i], hi_nb);
+    int kk;
+    double f;
+    if (GATHER == 1) {
+      const double km = t[i] + MBT_MAGIC;
+      kk = __double2loint(km);
+      f = t[i] - (km - MBT_MAGIC);
+    } else {
+      kk = __double2int_rd(t[i]);
+      f = 0.0;
+    }
+    kk = in[i] ? kk : nb + 1;
+    const WakeCell c = sW[kk];
+    del[i] = fma(-fma(f, c.dif, c.mid), A.invE0, del[i]);
+    if (!in[i] && live[i]) nout += 1u;
+  }
+  // S7: moments of the state after the kick
+#pragma unroll
+  for (int i = 0; i < NP; ++i)
+    if (live[i]) {
+      st += tau[i];
+      sd += del[i];
+      stt = fma(tau[i], tau[i], stt);
+      sdd = fma(del[i], del[i], sdd);
+    }
+  if (MAP) {
+    // S1: RF cavities.  The phase is formed as the oracle forms it (product rounded, then the sum).  All fast sines
+    // of the iteration are evaluated first, in ONE basic block together with the Box-Muller above, so that the
+    // independent polynomial chains interleave (DFMA latency is 8 cycles); a particle long lost from the bucket
+    // (|y| >= 2^16, or not finite) is then patched with the library sine in a single cold branch.
+    if (NCAV > 0) {
+      constexpr int NS = (NCAV > 0 ? NCAV : 1) * NP;
+      constexpr int NB = RAD ? NPAIR : 0;
+      SinState ss[NS];
+      constexpr int NB1 = NB > 0 ? NB : 1;
+      double zz[NS], pp[NS], f2[NB1], ps[NB1], pc[NB1];
+      uint32_t worst = 0u;
+#pragma unroll
+      for (int c = 0; c < NCAV; ++c)
+#pragma unroll
+        for (int i = 0; i < NP; ++i) {
+          const double y = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
+          ss[c * NP + i] = sin_rf_head(A.mt, y);
+          zz[c * NP + i] = ss[c * NP + i].z;
+          worst = max(worst, (uint32_t)__double2hiint(y) & 0x7FFFFFFFu);
+        }
+#pragma unroll
+      for (int q = 0; q < NB; ++q) f2[q] = bm[q].f2;
+      horner7_lockstep<NS, NB>(A.mt, zz, pp, f2, ps, pc);
+      double sn[NCAV > 0 ? NCAV : 1][NP];
+#pragma unroll
+      for (int c = 0; c < NCAV; ++c)
+#pragma unroll
+        for (int i = 0; i < NP; ++i) sn[c][i] = sin_rf_tail(ss[c * NP + i], pp[c * NP + i]);
+      if (RAD) {
+#pragma unroll
+        for (int q = 0; q < NB; ++q) box_muller_tail(A.mt, bm[q], ps[q], pc[q], z[2 * q], z[2 * q + 1]);
+      }
+      if (__builtin_expect(worst >= 0x40F00000u, 0)) {  // some |y| >= 65536, inf or NaN
+#pragma unroll
+        for (int c = 0; c < NCAV; ++c)
+#pragma unroll
+          for (int i = 0; i < NP; ++i) {
+            const double y = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
+            if (!(fabs(y) < 65536.0)) sn[c][i] = sin_rf_slow(y);
+          }
+      }
+#pragma unroll
+      for (int c = 0; c < NCAV; ++c)
+#pragma unroll
+        for (int i = 0; i < NP; ++i) del[i] = fma(A.cav_amp[c], sn[c][i], del[i]);
+    } else {
+#pragma unroll 1
+      for (int c = 0; c < A.n_cav; ++c) {
+        const double cw = A.cav_w[c], cp = A.cav_ph[c], ca = A.cav_amp[c];
+#pragma unroll
+        for (int i = 0; i < NP; ++i) {
+          const double y = __dadd_rn(__dmul_rn(cw, tau[i]), cp);
+          double sv = sin_rf_fast(A.mt, y);
+          if (__builtin_expect(!(fabs(y) < 65536.0), 0)) sv = sin_rf_slow(y);
+          del[i] = fma(ca, sv, del[i]);
+        }
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < NP; ++i) {
+      del[i] -= A.loss;
+      if (RAD) del[i] = fma(del[i], A.one_minus_DE, z[i]);  // S2 (z already scaled by sigma_delta sqrt(2 D_E))
+      tau[i] = fma(A.drift, del[i], tau[i]);                // S3
+      t[i] = __dmul_rn(__dsub_rn(tau[i], lo_new), A.invDelta);  // S4
+      in[i] = live[i] && in_window(t[i], hi_nb);
+    }
+  }
+  // S4: deposit.  Branch-free: a particle outside the window (or a padding slot) counts into the spare bin nb.
+#pragma unroll
+  for (int i = 0; i < NP; ++i) atomicAdd(&sH[in[i] ? __double2int_rd(t[i]) : nb], 1u);
+}
+
 // ------------------------------------------------------------------ fused particle pass
 // MAP = true : S0 S7 | S1 S2 S3 | S4      (a tracked turn)
 // MAP = false: S0 S7 |          | S4      (flush of the pending kick before the state is observed)
@@ -951,133 +1091,9 @@ __global__ void __launch_bounds__(kPassThreads, NPAIR == 1 ? 3 : 2) k_pass(const
         parity ^= 1u;
       }
 
-      double tau[NP], del[NP], z[NP];
-      bool live[NP];
-      BmState bm[NPAIR];
-      uint32_t xs[4] = {0u, 0u, 0u, 0u};
-#pragma unroll
-      for (int q = 0; q < NPAIR; ++q) {
-        const uint32_t pq = p + q;
-        tau[2 * q] = t2[q].x; tau[2 * q + 1] = t2[q].y;
-        del[2 * q] = d2[q].x; del[2 * q + 1] = d2[q].y;
-        live[2 * q] = FULL || (pq < p1 && 2u * pq < A.Np);  // past the end of the tile: stale stage contents, ignored;
-        live[2 * q + 1] = FULL || (live[2 * q] && (2u * pq + 1u < A.Np));  // the slots from N_p up to ld are padding
-        z[2 * q] = z[2 * q + 1] = 0.0;
-        if (MAP && RAD) {
-          // one Philox block serves FOUR consecutive particles (D8): counter (particle >> 2, bunch, turn, tag 0);
-          // its words (x0, x1) give the Box-Muller pair of particles 4j, 4j+1, (x2, x3) that of 4j+2, 4j+3; the even
-          // particle of a pair takes z_c, the odd one z_s.  A thread that owns the whole quad (NPAIR = 2) calls it once.
-          if (q == 0 || NPAIR == 1) philox4x32_10(pq >> 1, (uint32_t)(b + A.b0), n, 0u, A.keys, xs[0], xs[1], xs[2], xs[3]);
-          const bool hi_half = (NPAIR == 2) ? (q == 1) : ((pq & 1u) != 0u);  // with NPAIR = 2 the thread's first pair is even
-          const double u1 = uniform32(A.mt, hi_half ? xs[2] : xs[0]), u2 = uniform32(A.mt, hi_half ? xs[3] : xs[1]);
-          if (NCAV > 0) bm[q] = box_muller_head(A.mt, sL, u1, u2, A.A_q);  // polynomials: lock step with S1's
-          else box_muller_fast(A.mt, sL, u1, u2, A.A_q, z[2 * q], z[2 * q + 1]);
-        }
-      }
-      // S0: kick of the previous turn's wake.  t exactly as the binning computed it (one subtraction, one
-      // multiplication, no contraction), so the in-window decision is the one that deposited the particle.
-      // In-window test 0 <= t < nb on the high word of t alone (in_window()): an integer compare, off the fp64 pipe.
-      double t[NP];
-      bool in[NP];
-#pragma unroll
-      for (int i = 0; i < NP; ++i) {
-        t[i] = __dmul_rn(__dsub_rn(tau[i], lo_old), A.invDelta);
-        in[i] = live[i] && in_window(t[i], hi_nb);
-        int kk;
-        double f;
-        if (GATHER == 1) {
-          const double km = t[i] + MBT_MAGIC;
-          kk = __double2loint(km);
-          f = t[i] - (km - MBT_MAGIC);
-        } else {
-          kk = __double2int_rd(t[i]);
-          f = 0.0;
-        }
-        kk = in[i] ? kk : nb + 1;
-        const WakeCell c = sW[kk];
-        del[i] = fma(-fma(f, c.dif, c.mid), A.invE0, del[i]);
-        if (!in[i] && live[i]) nout += 1u;
-      }
-      // S7: moments of the state after the kick
-#pragma unroll
-      for (int i = 0; i < NP; ++i)
-        if (live[i]) {
-          st += tau[i];
-          sd += del[i];
-          stt = fma(tau[i], tau[i], stt);
-          sdd = fma(del[i], del[i], sdd);
-        }
-      if (MAP) {
-        // S1: RF cavities.  The phase is formed as the oracle forms it (product rounded, then the sum).  All fast sines
-        // of the iteration are evaluated first, in ONE basic block together with the Box-Muller above, so that the
-        // independent polynomial chains interleave (DFMA latency is 8 cycles); a particle long lost from the bucket
-        // (|y| >= 2^16, or not finite) is then patched with the library sine in a single cold branch.
-        if (NCAV > 0) {
-          constexpr int NS = (NCAV > 0 ? NCAV : 1) * NP;
-          constexpr int NB = RAD ? NPAIR : 0;
-          SinState ss[NS];
-          constexpr int NB1 = NB > 0 ? NB : 1;
-          double zz[NS], pp[NS], f2[NB1], ps[NB1], pc[NB1];
-          uint32_t worst = 0u;
-#pragma unroll
-          for (int c = 0; c < NCAV; ++c)
-#pragma unroll
-            for (int i = 0; i < NP; ++i) {
-              const double y = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
-              ss[c * NP + i] = sin_rf_head(A.mt, y);
-              zz[c * NP + i] = ss[c * NP + i].z;
-              worst = max(worst, (uint32_t)__double2hiint(y) & 0x7FFFFFFFu);
-            }
-#pragma unroll
-          for (int q = 0; q < NB; ++q) f2[q] = bm[q].f2;
-          horner7_lockstep<NS, NB>(A.mt, zz, pp, f2, ps, pc);
-          double sn[NCAV > 0 ? NCAV : 1][NP];
-#pragma unroll
-          for (int c = 0; c < NCAV; ++c)
-#pragma unroll
-            for (int i = 0; i < NP; ++i) sn[c][i] = sin_rf_tail(ss[c * NP + i], pp[c * NP + i]);
-          if (RAD) {
-#pragma unroll
-            for (int q = 0; q < NB; ++q) box_muller_tail(A.mt, bm[q], ps[q], pc[q], z[2 * q], z[2 * q + 1]);
-          }
-          if (__builtin_expect(worst >= 0x40F00000u, 0)) {  // some |y| >= 65536, inf or NaN
-#pragma unroll
-            for (int c = 0; c < NCAV; ++c)
-#pragma unroll
-              for (int i = 0; i < NP; ++i) {
-                const double y = __dadd_rn(__dmul_rn(A.cav_w[c], tau[i]), A.cav_ph[c]);
-                if (!(fabs(y) < 65536.0)) sn[c][i] = sin_rf_slow(y);
-              }
-          }
-#pragma unroll
-          for (int c = 0; c < NCAV; ++c)
-#pragma unroll
-            for (int i = 0; i < NP; ++i) del[i] = fma(A.cav_amp[c], sn[c][i], del[i]);
-        } else {
-#pragma unroll 1
-          for (int c = 0; c < A.n_cav; ++c) {
-            const double cw = A.cav_w[c], cp = A.cav_ph[c], ca = A.cav_amp[c];
-#pragma unroll
-            for (int i = 0; i < NP; ++i) {
-              const double y = __dadd_rn(__dmul_rn(cw, tau[i]), cp);
-              double sv = sin_rf_fast(A.mt, y);
-              if (__builtin_expect(!(fabs(y) < 65536.0), 0)) sv = sin_rf_slow(y);
-              del[i] = fma(ca, sv, del[i]);
-            }
-          }
-        }
-#pragma unroll
-        for (int i = 0; i < NP; ++i) {
-          del[i] -= A.loss;
-          if (RAD) del[i] = fma(del[i], A.one_minus_DE, z[i]);  // S2 (z already scaled by sigma_delta sqrt(2 D_E))
-          tau[i] = fma(A.drift, del[i], tau[i]);                // S3
-          t[i] = __dmul_rn(__dsub_rn(tau[i], lo_new), A.invDelta);  // S4
-          in[i] = live[i] && in_window(t[i], hi_nb);
-        }
-      }
-      // S4: deposit.  Branch-free: a particle outside the window (or a padding slot) counts into the spare bin nb.
-#pragma unroll
-      for (int i = 0; i < NP; ++i) atomicAdd(&sH[in[i] ? __double2int_rd(t[i]) : nb], 1u);
+      double tau[NP], del[NP];
+      advance_pairs<MAP, RAD, GATHER, NCAV, NPAIR, FULL>(A, t2, d2, tau, del, p, p1, b, n, lo_old, lo_new, hi_nb, nb, sW, sL, sH, st,
+                                                        sd, stt, sdd, nout);
       if (FULL || p < p1) {  // p and p1 are even when NPAIR = 2: the thread's pairs are inside the tile together
         if (NPAIR == 2) {
           if (MAP) stg_double4(T, tau[0], tau[1], tau[NP - 2], tau[NP - 1]);

@@ -274,6 +274,48 @@ def test_lr_scan_against_bruteforce_pairwise_sum(mbt, orc):
         assert wake_error(t.wake()[2], o.wake()[2]) <= 1e-10
 
 
+# ---------------------------------------------------------------------------------------------- chip-resident turn loop
+@pytest.mark.parametrize("name", sorted(TINY_VARIANTS))
+def test_resident_turn_loop_single_turn_parity(mbt, orc, name):
+    """mbt_tuning.turn_mode 3: the whole mbt_track call in one cooperative launch, particles resident in shared memory
+    (mbt_resident.cuh); same parity bar as the streaming path."""
+    cfg = W.tiny(**TINY_VARIANTS[name])
+    o = orc.Oracle(cfg)
+    o.track(4)
+    with mbt.Tracker(cfg, tuning=dict(turn_mode=3)) as t:
+        assert t.launches_per_turn == 0
+        for _ in range(2):
+            assert_single_turn_parity(o, t, cfg)
+
+
+@pytest.mark.parametrize("name,over,turns", [("c1", dict(), 50), ("c3", dict(), 30), ("c2", dict(), 12), ("c3", dict(n_per_bunch=30_001), 30),
+                                             ("c4", dict(n_per_bunch=1_000, n_bunches=120), 25)])
+def test_resident_turn_loop_equals_streaming_path(mbt, orc, name, over, turns):
+    """The resident loop runs the streaming pass's own loop body (advance_pairs) and the wake kernel's own code
+    (wake_body): after many turns particles and counts are BIT-identical to the two-launch path (moments and wakes to
+    rounding: their sums are taken in another order), the per-turn log included; and it agrees with the oracle."""
+    cfg = W.config(name, **over)
+    with mbt.Tracker(cfg, log_capacity_turns=turns, tuning=dict(turn_mode=3)) as tr, \
+            mbt.Tracker(cfg, log_capacity_turns=turns, tuning=dict(turn_mode=1)) as ts:
+        tr.track(turns // 2); tr.track(turns - turns // 2)            # two calls: the state survives the launch boundary
+        ts.track(turns)
+        (tau_r, del_r), (tau_s, del_s) = tr.particles(), ts.particles()
+        assert np.array_equal(tr.histogram(), ts.histogram())
+        assert particle_errors(tau_r, tau_s) <= 1e-12 and particle_errors(del_r, del_s) <= 1e-12
+        assert wake_error(tr.wake()[0], ts.wake()[0]) <= 1e-10
+        lr_, ls_ = tr.moment_log(1, turns), ts.moment_log(1, turns)
+        assert np.array_equal(lr_[..., :2], ls_[..., :2]) and np.allclose(lr_[..., 2:], ls_[..., 2:], rtol=1e-9, atol=1e-24)
+        assert tr.turn == turns
+        tr.track(3); ts.track(3)                                       # and both go on
+        assert np.array_equal(tr.histogram(), ts.histogram())
+    if name == "c1":
+        o = orc.Oracle(cfg)
+        with mbt.Tracker(cfg, tuning=dict(turn_mode=3)) as t:
+            o.track(9); t.track(9)
+            assert particle_errors(t.particles()[1], o.particles()[1]) <= 1e-10
+            assert np.array_equal(t.histogram(), o.histogram())
+
+
 # ---------------------------------------------------------------------------------------------- edge cases
 def test_edge_cases(mbt, orc):
     cfg = W.tiny()
