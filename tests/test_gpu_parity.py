@@ -316,6 +316,27 @@ def test_resident_turn_loop_equals_streaming_path(mbt, orc, name, over, turns):
             assert np.array_equal(t.histogram(), o.histogram())
 
 
+@pytest.mark.parametrize("name,over,turns", [("c4", dict(n_per_bunch=600), 600), ("c5", dict(n_per_bunch=1_000), 200),
+                                             ("c4", dict(n_per_bunch=20_000), 100), ("c3", dict(n_per_bunch=5_000), 500),
+                                             ("c1", dict(), 500)])
+def test_per_bunch_start_equals_grid_waits(mbt, name, over, turns):
+    """The sequencing of DESIGN.md 7.1 (a pass CTA waits for its own bunch's wake, a wake CTA for its own bunch's pass
+    CTAs) changes WHEN things run, not what is computed: against the same library with grid-wide waits
+    (per_bunch_start = 1) particles and counts are bit-identical after hundreds of short turns -- short turns, many
+    bunches: the regime where consecutive kernels overlap most -- and so is every turn of the moment log's counts."""
+    cfg = W.config(name, **over)
+    with mbt.Tracker(cfg, log_capacity_turns=turns, tuning=dict(per_bunch_start=2)) as ta, \
+            mbt.Tracker(cfg, log_capacity_turns=turns, tuning=dict(per_bunch_start=1)) as tb:
+        for n in (turns // 3, 1, turns - turns // 3 - 1):        # several calls: graph of 16, single turns, remainders
+            ta.track(n); tb.track(n)
+        (tau_a, del_a), (tau_b, del_b) = ta.particles(), tb.particles()
+        assert np.array_equal(tau_a, tau_b) and np.array_equal(del_a, del_b)
+        assert np.array_equal(ta.histogram(), tb.histogram())
+        la, lb = ta.moment_log(1, turns), tb.moment_log(1, turns)
+        assert np.array_equal(la[..., :2], lb[..., :2]) and np.allclose(la[..., 2:], lb[..., 2:], rtol=1e-9, atol=1e-24)
+        assert np.allclose(ta.lr_history(), tb.lr_history(), rtol=1e-12, atol=1e-300)
+
+
 # ---------------------------------------------------------------------------------------------- edge cases
 def test_edge_cases(mbt, orc):
     cfg = W.tiny()
