@@ -180,8 +180,12 @@ struct mbt_handle {
                 // Measured, us per turn, graph replay: pass only c1 10.8 -> 10.0, c3 16.6 -> 16.0, c4 223.9 -> 222.8; k_wake as
                 // well helps c1 (9.1) but costs c2 and c3 (26.8, 19.3): its resident CTAs are in the way of the pass's tail
   DevBuf<LogTabEntry> logtab;
-  cudaGraphExec_t graph1 = nullptr, graphU = nullptr;
-  int unroll = 16;
+  // captured graphs of 1, 2, 4, ... 64 turns, built on demand: a run is replayed largest first.  Inside a graph the kernels
+  // are chained as programmatic dependents; BETWEEN two graph launches the dependency is a full one (the wake kernel's
+  // latency is exposed there), so few, long graphs: 300 turns are 4 x 64 + 32 + 8 + 4 (7 boundaries, where graphs of 16
+  // and single turns made 30).
+  static constexpr int kGraphLevels = 7;
+  cudaGraphExec_t graphs[kGraphLevels] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
 };
@@ -374,8 +378,8 @@ void destroy(mbt_handle *h) {
   if (!h) return;
   cudaSetDevice(h->device);
   if (h->stream) cudaStreamSynchronize(h->stream);
-  if (h->graph1) cudaGraphExecDestroy(h->graph1);
-  if (h->graphU) cudaGraphExecDestroy(h->graphU);
+  for (cudaGraphExec_t g : h->graphs)
+    if (g) cudaGraphExecDestroy(g);
   if (h->stream2) { cudaStreamSynchronize(h->stream2); cudaStreamDestroy(h->stream2); }
   if (h->ev_fork) cudaEventDestroy(h->ev_fork);
   if (h->ev_join) cudaEventDestroy(h->ev_join);
@@ -1083,24 +1087,20 @@ int mbt_track(mbt_handle *h, int64_t n_turns) {
   CU(cudaSetDevice(h->device));
   if (n_turns == 0) return 0;
   if (h->resident) return track_resident(h, n_turns);
-  if (!h->graph1) {
-    int rc = build_graph(h, 1, &h->graph1);
-    if (rc) return rc;
-  }
-  if (n_turns >= h->unroll && !h->graphU) {
-    int rc = build_graph(h, h->unroll, &h->graphU);
-    if (rc) return rc;
-  }
+  for (int lv = mbt_handle::kGraphLevels - 1; lv >= 0; --lv)  // build what this call needs before the timed region
+    if (((n_turns >> lv) & 1) || (lv == mbt_handle::kGraphLevels - 1 && (n_turns >> lv)))
+      if (!h->graphs[lv]) {
+        int rc = build_graph(h, 1 << lv, &h->graphs[lv]);
+        if (rc) return rc;
+      }
   CU(cudaEventRecord(h->ev0, h->stream));
   int64_t left = n_turns;
-  while (left >= h->unroll) {
-    CU(cudaGraphLaunch(h->graphU, h->stream));
-    left -= h->unroll;
-  }
-  while (left > 0) {
-    CU(cudaGraphLaunch(h->graph1, h->stream));
-    left -= 1;
-  }
+  for (int lv = mbt_handle::kGraphLevels - 1; lv >= 0; --lv)
+    while (left >= (1ll << lv)) {
+      CU(cudaGraphLaunch(h->graphs[lv], h->stream));
+      left -= 1ll << lv;
+      if (lv < mbt_handle::kGraphLevels - 1) break;  // every smaller size at most once
+    }
   CU(cudaEventRecord(h->ev1, h->stream));
   h->timed = true;
   h->launches += launches_per_turn(h) * n_turns;

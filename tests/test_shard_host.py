@@ -75,7 +75,10 @@ def test_gloo_world2_exchange_rebuilds_single_rank_phasors(m, n_lr):
     import torch.multiprocessing as mp
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    port = 29500 + (os.getpid() + m) % 2000
+    import socket
+    with socket.socket() as sk:                                   # a free port of this host
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
     procs = [ctx.Process(target=_rank_main, args=(r, 2, port, m, n_lr, q)) for r in range(2)]
     for p in procs:
         p.start()
