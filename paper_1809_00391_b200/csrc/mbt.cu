@@ -173,7 +173,10 @@ struct mbt_handle {
   DevBuf<uint32_t> res_bar;
   bool fused = false;  // a turn is ONE launch: the pass's last CTA of a bunch builds the bunch's wake (mbt_tuning.turn_mode 2)
   DevBuf<uint32_t> bunch_done;
-  DevBuf<uint32_t> a_ready, bunch_ready, agg_ready, tile_turn;
+  DevBuf<uint32_t> a_ready, bunch_ready, agg_ready, tile_turn, tr_ready, rw_ready;
+  size_t smem_wake6 = 0;
+  DevBuf<uint32_t> bunch_done_tr;
+  bool pipe6 = false;  // 6-D turn as one chain of programmatic dependents with per-bunch flags
   DevBuf<cplx> gd;
   int npair = 1;
   int pdl = 1;  // bit 0: the pass, bit 1: k_wake launched as a programmatic dependent (longitudinal handles; mbt_tuning.pdl sets it).
@@ -282,6 +285,7 @@ cudaError_t launch_dependent(void (*fn)(KArgs...), dim3 grid, int threads, size_
 // Every enqueue_* returns the first launch error (a bad configuration shows up here, not at a later synchronise).
 cudaError_t enqueue_pass(mbt_handle *h) {
   if (h->trans) {
+    if (h->pipe6) return launch_dependent(h->fn_map6, dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream, h->args6);
     h->fn_map6<<<dim3(h->grid_pass6, h->M), kPassThreads, h->smem_pass6, h->stream>>>(h->args6);
     return cudaGetLastError();
   }
@@ -297,6 +301,11 @@ cudaError_t enqueue_wakes(mbt_handle *h) {
   if (h->fused) return cudaSuccess;
   cudaError_t e = cudaSuccess;
 #define MBT_E_(call) do { if (e == cudaSuccess) e = (call); } while (0)
+  if (h->pipe6) {  // one stream, every kernel a programmatic dependent of the one before; per-bunch flags order the data
+    MBT_E_(launch_dependent(k_wake6, dim3(h->M, 2), kWakeThreads, h->smem_wake6, h->stream, h->wargs, h->twargs));
+    if (h->Krw > 0) MBT_E_(launch_dependent(k_rw, dim3(h->M), 256, (size_t)0, h->stream, h->rwargs));
+    return e;
+  }
   if (h->trans) {
     MBT_E_(cudaEventRecord(h->ev_fork, h->stream));
     MBT_E_(cudaStreamWaitEvent(h->stream2, h->ev_fork, 0));
@@ -319,7 +328,7 @@ cudaError_t enqueue_wakes(mbt_handle *h) {
   return e;
 }
 // launches per tracked turn: 1 in the one-launch turn, else 2; 3 with the transverse planes; 4 with their resistive-wall kick
-int launches_per_turn(const mbt_handle *h) { return h->resident ? 0 : h->fused ? 1 : h->trans ? (h->Krw > 0 ? 4 : 3) : 2; }
+int launches_per_turn(const mbt_handle *h) { return h->resident ? 0 : h->fused ? 1 : h->trans ? (h->pipe6 ? (h->Krw > 0 ? 3 : 2) : (h->Krw > 0 ? 4 : 3)) : 2; }
 
 cudaError_t enqueue_turn(mbt_handle *h) {
   cudaError_t e = enqueue_pass(h);
@@ -393,7 +402,7 @@ void destroy(mbt_handle *h) {
   h->scratch_a.release(); h->scratch_b.release(); h->scratch_c.release();
   h->cellSR.release(); h->cellF.release();
   h->rd_cnt.release(); h->wr_cnt.release(); h->bunch_done.release();
-  h->a_ready.release(); h->bunch_ready.release(); h->agg_ready.release(); h->gd.release(); h->tile_turn.release(); h->res_bar.release();
+  h->a_ready.release(); h->bunch_ready.release(); h->agg_ready.release(); h->gd.release(); h->tile_turn.release(); h->res_bar.release(); h->tr_ready.release(); h->rw_ready.release(); h->bunch_done_tr.release();
   h->tx.release(); h->txp.release(); h->ty.release(); h->typ.release(); h->wt.release(); h->Sfix.release(); h->Sov.release();
   h->S_last.release(); h->Ktab.release(); h->acc2.release(); h->fix.release(); h->cellX.release(); h->cellY.release();
   h->mom_tr_acc.release(); h->mom_tr.release();
@@ -444,7 +453,7 @@ int track_resident(mbt_handle *h, int64_t n_turns) {
     h->launches += 1;
   }
   k_sync_flags<<<1, 256, 0, h->stream>>>(h->ctrl.p, h->a_ready.p, h->Mg * (h->R ? h->R : 1), h->bunch_ready.p, h->M, h->agg_ready.p,
-                                         h->tile_turn.p, h->M * h->grid_pass);
+                                         h->tile_turn.p, (int)h->tile_turn.n);
   CU(cudaGetLastError());
   h->launches += 1;
   CU(cudaEventRecord(h->ev1, h->stream));
@@ -1051,6 +1060,28 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
       choose_tiles(h->ld / 2, kPassThreads, M, prop.multiProcessorCount * occ, tn.tile_iters, tn.verbose != 0, &T.tile_pairs,
                    &h->grid_pass6);
     }
+    // per-bunch sequencing of the 6-D turn (as the longitudinal one): one k_wake CTA per bunch, launches chained
+    CUH(h->tr_ready.alloc(M, h->stream));
+    CUH(h->rw_ready.alloc(M, h->stream));
+    CUH(h->bunch_done_tr.alloc(M, h->stream));
+    h->pipe6 = h->wargs.gather_P && tn.per_bunch_start != 1 && tn.pdl != 1;
+    if (h->pipe6) {
+      h->tile_turn.release();
+      CUH(h->tile_turn.alloc((size_t)M * h->grid_pass6, h->stream));
+      T.L.tile_turn = h->tile_turn.p;
+      T.L.bunch_ready = h->bunch_ready.p;
+      T.L.flag_wait = 1;
+      T.L.count_done = 1;
+      T.tr_ready = h->tr_ready.p;
+      T.rw_ready = h->Krw > 0 ? h->rw_ready.p : nullptr;
+      T.bunch_done_tr = h->bunch_done_tr.p;
+      h->smem_wake6 = std::max(h->smem_wake, wake_tr_smem_bytes(nb));
+      CUH(cudaFuncSetAttribute(k_wake6, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_wake6));
+      CUH(cudaFuncSetAttribute(k_wake6, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
+      h->wargs.bunch_wait = 1;
+      h->wargs.tiles = h->grid_pass6;
+      h->wargs.bunch_done = h->bunch_done.p;
+    }
     TMomArgs &Tm = h->tmargs;
     Tm.x = h->tx.p; Tm.xp = h->txp.p; Tm.y = h->ty.p; Tm.yp = h->typ.p; Tm.ld = h->ld; Tm.Np = (uint32_t)h->Np; Tm.tile = 8192;
     h->grid_tr = (int)((h->Np + Tm.tile - 1) / Tm.tile);
@@ -1064,6 +1095,8 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     if (h->log_cap > 0) CUH(h->log_tr.alloc((size_t)h->log_cap * M * 4, h->stream));
     Tw.log_tr = h->log_cap > 0 ? h->log_tr.p : nullptr;
     Tw.log_cap = h->log_cap;
+    Tw.tr_ready = h->tr_ready.p; Tw.use_flags = h->pipe6 ? 1 : 0; Tw.bunch_done_tr = h->bunch_done_tr.p;
+    h->rwargs.rw_ready = h->rw_ready.p; h->rwargs.tr_ready = h->tr_ready.p; h->rwargs.use_flags = h->pipe6 ? 1 : 0;
     dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)M);
     k_init_tr<<<grid, 256, 0, h->stream>>>(h->tx.p, h->txp.p, h->ty.p, h->typ.p, h->ld, (uint32_t)h->Np, A.keys,
                                            tr.x.sigma0_u_m, tr.x.sigma0_up, tr.y.sigma0_u_m, tr.y.sigma0_up);
@@ -1305,7 +1338,8 @@ int mbt_set_particles(mbt_handle *h, const double *tau, const double *delta, int
     if (rc) return rc;
   }
   k_set_ctrl<<<1, 256, 0, h->stream>>>(h->ctrl.p, (uint32_t)turn, 0u, h->a_ready.p, h->Mg * (h->R ? h->R : 1), h->bunch_ready.p, h->M,
-                                       h->agg_ready.p, h->bunch_done.p, h->tile_turn.p, h->M * h->grid_pass);
+                                       h->agg_ready.p, h->bunch_done.p, h->tile_turn.p, (int)h->tile_turn.n);
+  if (h->trans) k_set_flags_tr<<<1, 256, 0, h->stream>>>(h->tr_ready.p, h->rw_ready.p, h->bunch_done_tr.p, h->M, (uint32_t)turn);
   CU(cudaGetLastError());
   h->launches += 1;
   CU(cudaMemsetAsync(h->hist.p, 0, sizeof(uint32_t) * h->M * h->nb, h->stream));

@@ -55,6 +55,9 @@ struct Args6 {
   double *acc2;                // [M][2] sum u^2 of the mapped state (the next turn's scale)
   uint32_t *turn_tr;           // the turn this pass tracks, for k_wake_tr / k_rw: they run beside k_wake, which bumps
                                // ctrl->turn, so they must not read that word
+  uint32_t *bunch_done_tr;     // [M] second completion count (the transverse side of k_wake6 resets it), or nullptr
+  const uint32_t *tr_ready;    // [M] turn whose transverse kick tables of bunch b are complete (k_wake_tr), or nullptr
+  const uint32_t *rw_ready;    // [M] ... whose resistive-wall kick is (k_rw), or nullptr (no resistive wall / grid-wide waits)
   uint32_t tile_pairs;         // pairs per CTA
   int32_t stages;              // shared-memory stages of the particle stream (2..kMaxStages6)
 };
@@ -151,15 +154,9 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
     mbar_init(smem_u32(&s_bar[kMaxStages6 + tid]), NWARP);
   }
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  const uint32_t n = A.ctrl->turn + 1u;
-  const bool have_kick = A.ctrl->kick_pending != 0u;
   const uint32_t hi_nb = (uint32_t)__double2hiint(A.nb_d);
-  if (MAP && tid == 0 && blockIdx.x == 0 && b == 0) *A6.turn_tr = n;
   const uint32_t p0 = blockIdx.x * A6.tile_pairs;
   const uint32_t p1 = (A.ppb - p0 < A6.tile_pairs) ? A.ppb : p0 + A6.tile_pairs;
-  const double lo_old = A.lo_hist[b];
-  const double lo_new = MAP ? A.lo_next[b] : lo_old;
-  const FixScale fx = A6.fix[2 * b], fy = A6.fix[2 * b + 1];
   const size_t base = (size_t)b * A.ld;
   const uint32_t n_it = (p1 - p0 + kPassThreads - 1u) / kPassThreads;
   const uint32_t stage0 = smem_u32(smem_raw), full0 = smem_u32(&s_bar[0]), empty0 = smem_u32(&s_bar[kMaxStages6]);
@@ -177,24 +174,57 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
   __syncthreads();  // barriers initialised
   if (tid == 0)
     for (uint32_t k = 0; k + 1u < nst && k < n_it; ++k) issue(k);
+  // Sequencing as in k_pass: with flag_wait the kernels of a 6-D turn are a chain of programmatic
+  // dependents on one stream, and this CTA waits for the wakes of ITS bunch -- longitudinal (bunch_ready), transverse
+  // (tr_ready) and resistive wall (rw_ready) -- instead of the grids before it; the turn number comes from the tile's own
+  // CTA of the pass before.  (The particle stages above were written by that pass, which is complete: the wake kernels
+  // between it and this launch let their dependents in only after they had seen their bunch's pass CTAs counted.)
+  __shared__ uint32_t s_turn;
+  const bool by_flag = MAP && A.flag_wait != 0;
+  griddep_launch_dependents();
+  if (by_flag) {
+    if (tid == 0) {
+      const uint32_t done = __ldcg(&A.tile_turn[(size_t)b * gridDim.x + blockIdx.x]);
+      wait_turn(&A.bunch_ready[b], done);
+      wait_turn(&A6.tr_ready[b], done);
+      if (A6.rw_ready) wait_turn(&A6.rw_ready[b], done);
+      s_turn = done;
+    }
+    __syncthreads();
+  }
+  const uint32_t n_done = by_flag ? s_turn : A.ctrl->turn;
+  const uint32_t n = n_done + 1u;
+  const bool have_kick = by_flag ? (n_done != A.ctrl->kick_base) : (A.ctrl->kick_pending != 0u);
+  if (MAP && tid == 0 && blockIdx.x == 0 && b == 0) *A6.turn_tr = n;
+  const double lo_old = __ldcg(&A.lo_hist[b]);
+  const double lo_new = MAP ? __ldcg(&A.lo_next[b]) : lo_old;
+  FixScale fx, fy;  // (written by k_wake_tr of the turn before: through L2)
+  fx.inv_lsb = __ldcg(&A6.fix[2 * b].inv_lsb); fx.lsb = __ldcg(&A6.fix[2 * b].lsb); fx.xmax_hi = __ldcg(&A6.fix[2 * b].xmax_hi); fx.pad = 0u;
+  fy.inv_lsb = __ldcg(&A6.fix[2 * b + 1].inv_lsb); fy.lsb = __ldcg(&A6.fix[2 * b + 1].lsb); fy.xmax_hi = __ldcg(&A6.fix[2 * b + 1].xmax_hi); fy.pad = 0u;
 
   if (MAP && RAD)
     for (int i = tid; i < 128; i += kPassThreads) sL[i] = A.logtab[i];
   for (int k = tid; k < nb + 2; k += kPassThreads) {
     WakeCell c{0.0, 0.0}, cx{0.0, 0.0}, cy{0.0, 0.0};
     if (have_kick) {
-      c = A.cellSR[(size_t)b * (nb + 2) + k];
+      {
+        const double2 v = __ldcg(reinterpret_cast<const double2 *>(&A.cellSR[(size_t)b * (nb + 2) + k]));
+        c.mid = v.x; c.dif = v.y;
+      }
 #pragma unroll 1
       for (int r = 0; r < A.R; ++r) {
         const CellF f = A.cellF[(size_t)r * (nb + 2) + k];
-        const cplx pb = A.P[(size_t)b * A.R + r];
+        const cplx pb = __ldcg_cplx(&A.P[(size_t)b * A.R + r]);
         c.mid += fma(f.mid.re, pb.re, -(f.mid.im * pb.im));
         c.dif += fma(f.dif.re, pb.re, -(f.dif.im * pb.im));
       }
-      cx = A6.cellX[(size_t)b * (nb + 2) + k];
-      cy = A6.cellY[(size_t)b * (nb + 2) + k];
-      cx.mid += A6.rw[2 * b];      // the resistive-wall kick is the same for every particle of the bunch (W4),
-      cy.mid += A6.rw[2 * b + 1];  // cell nb+1 (outside the window) included
+      {
+        const double2 vx = __ldcg(reinterpret_cast<const double2 *>(&A6.cellX[(size_t)b * (nb + 2) + k]));
+        const double2 vy = __ldcg(reinterpret_cast<const double2 *>(&A6.cellY[(size_t)b * (nb + 2) + k]));
+        cx.mid = vx.x; cx.dif = vx.y; cy.mid = vy.x; cy.dif = vy.y;
+      }
+      cx.mid += __ldcg(&A6.rw[2 * b]);      // the resistive-wall kick is the same for every particle of the bunch (W4),
+      cy.mid += __ldcg(&A6.rw[2 * b + 1]);  // cell nb+1 (outside the window) included
     }
     sW[k] = c; sX[k] = cx; sY[k] = cy;
   }
@@ -428,6 +458,17 @@ __global__ void __launch_bounds__(kPassThreads, 2) k_pass6(const __grid_constant
       }
     }
   }
+  if (MAP) {
+    if (tid == 0 && A.tile_turn) A.tile_turn[(size_t)b * gridDim.x + blockIdx.x] = n;
+    if (A.count_done) {  // release this CTA's counts and sums and count it: the wake kernels' CTAs of the bunch wait for it
+      __syncthreads();
+      if (tid == 0) {
+        __threadfence();
+        atomicAdd(&A.bunch_done[b], 1u);
+        if (A6.bunch_done_tr) atomicAdd(&A6.bunch_done_tr[b], 1u);
+      }
+    }
+  }
 }
 
 struct TWakeArgs {
@@ -447,6 +488,9 @@ struct TWakeArgs {
   double *S_last;             // [M][2][nb] observable copy of the sums [m]
   double *K;                  // [M][2][nb] kick tables [V]
   WakeCell *cellX, *cellY;    // [M][nb+2] their gather cells (as WakeCell of mbt_kernels.cuh)
+  uint32_t *tr_ready;         // [M] per-bunch sequencing: turn whose tables of bunch b are complete; the turn
+  int32_t use_flags;          //     being closed is then tr_ready[b] + 1 (turn_tr may already belong to the next pass)
+  uint32_t *bunch_done_tr;    // [M] pass CTAs of the bunch counted for the transverse side of k_wake6
 };
 
 // X_max = 2^E >= 64 sqrt(<u^2>) (E clamped; <u^2> = 0 or not finite: E = 0, every non-zero offset then takes the fp64 path)
@@ -478,20 +522,24 @@ __host__ __device__ inline size_t wake_tr_smem_bytes(int nb) {
 
 // Eq. (6b): strictly causal sum over the earlier bins, both planes; one CTA per bunch.  Also closes the fixed-point
 // dipole sums of the turn and chooses the next turn's scale.
-__global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeArgs A) {
-  extern __shared__ double s_w[];  // [5][nb]: wt, q Sx, q Sy, Kx, Ky; then the padded table [nb+8] and the partial sums
+// s_w: wake_tr_smem_bytes(nb) of shared memory: [5][nb]: wt, q Sx, q Sy, Kx, Ky; then the padded table [nb+8] and the
+// partial sums.  Called by every thread of a 256-thread CTA: by k_wake_tr, or by the y = 1 CTAs of k_wake6.
+__device__ __forceinline__ void wake_tr_body(const TWakeArgs &A, const int b, double *s_w) {
   double *swp = s_w + 5 * A.nb;    // swp[3 + l] = wt[l]; zero for the lags -3..0 below and up to 4 beyond the table
-  const int b = blockIdx.x, tid = threadIdx.x, nb = A.nb;
+  const int tid = threadIdx.x, nb = A.nb;
   double *sw = s_w, *sx = s_w + nb, *sy = s_w + 2 * nb, *kx = s_w + 3 * nb, *ky = s_w + 4 * nb;
+  const uint32_t n_turn = A.use_flags ? __ldcg(&A.tr_ready[b]) + 1u : *A.turn_tr;
   const double qm = A.qm[b];
-  const FixScale fx = A.fix[2 * b], fy = A.fix[2 * b + 1];
+  FixScale fx, fy;  // the scale this turn's sums were deposited with: written by this bunch's CTA of the turn before (L2)
+  fx.inv_lsb = __ldcg(&A.fix[2 * b].inv_lsb); fx.lsb = __ldcg(&A.fix[2 * b].lsb); fx.xmax_hi = 0u; fx.pad = 0u;
+  fy.inv_lsb = __ldcg(&A.fix[2 * b + 1].inv_lsb); fy.lsb = __ldcg(&A.fix[2 * b + 1].lsb); fy.xmax_hi = 0u; fy.pad = 0u;
   const size_t ox = ((size_t)b * 2) * nb, oy = ox + nb;                  // S_last, K: [M][2][nb]
   const size_t fxo = ((size_t)b * 2) * (nb + 1), fyo = fxo + (nb + 1);   // Sfix, Sov: [M][2][nb+1]
   long long tix = 0, tiy = 0;   // integer totals over the bins and the sink: exact, so the centroid is reproducible
   double tox = 0.0, toy = 0.0;
   for (int j = tid; j < nb + 1; j += 256) {
-    const long long ix = (long long)A.Sfix[fxo + j], iy = (long long)A.Sfix[fyo + j];
-    const double ovx = A.Sov[fxo + j], ovy = A.Sov[fyo + j];
+    const long long ix = (long long)__ldcg(&A.Sfix[fxo + j]), iy = (long long)__ldcg(&A.Sfix[fyo + j]);  // accumulated by atomics: L2
+    const double ovx = __ldcg(&A.Sov[fxo + j]), ovy = __ldcg(&A.Sov[fyo + j]);
     A.Sfix[fxo + j] = 0ull; A.Sfix[fyo + j] = 0ull;
     A.Sov[fxo + j] = 0.0; A.Sov[fyo + j] = 0.0;
     tix += ix; tiy += iy; tox += ovx; toy += ovy;
@@ -522,19 +570,19 @@ __global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeAr
       double to = 0.0;
       for (int w = 0; w < 8; ++w) { ti += s_ti[w][tid]; to += s_to[w][tid]; }
       const double total = fma((double)ti, tid == 0 ? fx.lsb : fy.lsb, to);
-      const uint32_t n = *A.turn_tr;
+      const uint32_t n = n_turn;
       if (A.Krw > 0) A.ring_g[((size_t)(n % (uint32_t)(A.Krw + 1)) * A.M + b) * 2 + tid] = qm * total;
       if (A.log_tr && n >= 1u && (int64_t)n <= A.log_cap) {
         const double iN = 1.0 / (double)A.Np, mean = total * iN;
         double *row = A.log_tr + ((size_t)(n - 1u) * A.M + b) * 4;
         row[tid] = mean;
-        row[2 + tid] = sqrt(fmax(A.acc2[2 * b + tid] * iN - mean * mean, 0.0));  // acc2 is reset further down
+        row[2 + tid] = sqrt(fmax(__ldcg(&A.acc2[2 * b + tid]) * iN - mean * mean, 0.0));  // acc2 is reset further down
       }
     }
   }
   __syncthreads();
   if (tid < 2) {
-    A.fix[2 * b + tid] = make_fix_scale(A.acc2[2 * b + tid] / (double)A.Np, A.fix_bits);
+    A.fix[2 * b + tid] = make_fix_scale(__ldcg(&A.acc2[2 * b + tid]) / (double)A.Np, A.fix_bits);
     A.acc2[2 * b + tid] = 0.0;
   }
   // Toeplitz sums, register-blocked (the plain loop is shared-memory-bandwidth bound: 12 wavefronts per 8 MACs): a
@@ -596,6 +644,37 @@ __global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeAr
     A.cellX[(size_t)b * (nb + 2) + k] = cx;
     A.cellY[(size_t)b * (nb + 2) + k] = cy;
   }
+  if (A.use_flags) {  // the bunch's tables, scale and source strength are written: publish them
+    __syncthreads();
+    if (tid == 0) {
+      __threadfence();
+      st_release_u32(&A.tr_ready[b], n_turn);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256) k_wake_tr(const __grid_constant__ TWakeArgs A) {
+  extern __shared__ double s_wtr[];
+  wake_tr_body(A, (int)blockIdx.x, s_wtr);
+}
+
+// Per-bunch sequencing of the 6-D turn: ONE wake kernel, grid (M, 2), launched as a programmatic dependent
+// of the pass -- CTA (b, 0) builds the longitudinal wake of bunch b (wake_body), CTA (b, 1) its transverse kick tables
+// (wake_tr_body) -- each as soon as the pass CTAs of ITS bunch are counted (two counters: each side resets its own).
+// CTAs that become resident during the pass's last wave work on bunches that completed long before.
+__global__ void __launch_bounds__(256, 3) k_wake6(const __grid_constant__ WakeArgs A, const __grid_constant__ TWakeArgs T) {
+  extern __shared__ double smem_w6[];
+  const int b = (int)blockIdx.x;
+  uint32_t *cnt = blockIdx.y == 0 ? A.bunch_done : T.bunch_done_tr;
+  if (threadIdx.x == 0) {
+    while (ld_acquire_u32(&cnt[b]) < (uint32_t)A.tiles) {
+    }
+    cnt[b] = 0u;
+  }
+  __syncthreads();
+  griddep_launch_dependents();  // k_rw or the next pass may come in: their CTAs wait for the flags of their own bunch
+  if (blockIdx.y == 0) wake_body<false, true>(A, b, 0, smem_w6, A.smem_wake_bytes);
+  else wake_tr_body(T, b, smem_w6);
 }
 
 // Long-range resistive-wall kick (readings W1..W5): one CTA per bunch b sums the sources of the last Krw turns (all
@@ -610,11 +689,17 @@ struct RwArgs {
   double amp[2];
   double *rw;             // [M][2] out [V]
   const uint32_t *turn_tr;
+  const uint32_t *tr_ready;  // [M] (k_wake6's transverse side)
+  uint32_t *rw_ready;     // [M] per-bunch sequencing: turn whose kick of bunch b is complete (the turn summed is rw_ready[b] + 1)
+  int32_t use_flags;
 };
 __global__ void __launch_bounds__(256) k_rw(const __grid_constant__ RwArgs A) {
   __shared__ double s_red[8][2];
   const int b = blockIdx.x, tid = threadIdx.x;
-  const uint32_t n = *A.turn_tr;
+  griddep_launch_dependents();  // the next pass may come in: its CTAs wait for rw_ready
+  // per-bunch sequencing: this turn's sources are those of the bunches AHEAD (W5); each is awaited through its tr_ready
+  // flag below (CTAs of k_wake6, all resident or done before this kernel was let in); earlier turns are long complete
+  const uint32_t n = A.use_flags ? __ldcg(&A.rw_ready[b]) + 1u : *A.turn_tr;
   const int sb = A.bucket[b];
   double sx = 0.0, sy = 0.0;
   // a thread keeps its source bunches bp (their bucket distance within a turn in a register) and walks the turns back;
@@ -622,13 +707,14 @@ __global__ void __launch_bounds__(256) k_rw(const __grid_constant__ RwArgs A) {
   const int kmax = min(A.Krw, (int)min(n - 1u, (uint32_t)A.Krw));  // nothing before turn 1
   for (int bp = tid; bp < A.M; bp += 256) {
     const int ds = sb - A.bucket[bp];
+    if (A.use_flags && ds > 0) wait_turn(&A.tr_ready[bp], n);
     const double2 *g = reinterpret_cast<const double2 *>(A.ring_g) + bp;
     uint32_t slot = n % (uint32_t)(A.Krw + 1);
 #pragma unroll 4
     for (int k = 0; k <= kmax; ++k) {  // source: turn n - k, bunch bp, bucket distance d
       const int d = k * A.h + ds;
       const double w = d > 0 ? A.wrw[d] : 0.0;          // this turn (k = 0): only the bunches ahead
-      const double2 gv = g[(size_t)slot * A.M];
+      const double2 gv = __ldcg(&g[(size_t)slot * A.M]);
       sx = fma(gv.x, w, sx);
       sy = fma(gv.y, w, sy);
       slot = slot == 0u ? (uint32_t)A.Krw : slot - 1u;
@@ -646,6 +732,18 @@ __global__ void __launch_bounds__(256) k_rw(const __grid_constant__ RwArgs A) {
     for (int w = 0; w < 8; ++w) t += s_red[w][tid];
     A.rw[2 * b + tid] = A.amp[tid] * t;
   }
+  if (A.use_flags) {
+    __syncthreads();
+    if (tid == 0) {
+      __threadfence();
+      st_release_u32(&A.rw_ready[b], n);
+    }
+  }
+}
+
+// per-bunch sequencing flags of the transverse wake kernels: "complete through `turn`"
+__global__ void k_set_flags_tr(uint32_t *tr_ready, uint32_t *rw_ready, uint32_t *bunch_done_tr, int M, uint32_t turn) {
+  for (int i = threadIdx.x; i < M; i += blockDim.x) { tr_ready[i] = turn; rw_ready[i] = turn; bunch_done_tr[i] = 0u; }
 }
 
 // scale of the fixed-point dipole sums from the state in memory (create, mbt_set_transverse): acc[M][8] of k_moments_tr
