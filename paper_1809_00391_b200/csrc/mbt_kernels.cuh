@@ -258,7 +258,21 @@ __device__ __forceinline__ Affine compose(const Affine &first, const Affine &sec
 // Shared memory of wake_body: charges, V_SR, and the wake table with sixteen zeros in front and eight behind (the sliding
 // window of the register-blocked convolution runs off both ends).  The scan of the turn's last CTA stages its operands
 // (48 bytes per bunch and resonator) in the same memory if they fit into what the launch provides (`smem_bytes`).
-__host__ __device__ inline size_t wake_smem_bytes(int nb, int M) { return (size_t)(3 * nb + 24) * sizeof(double) + (size_t)M * sizeof(int32_t); }
+// Up to this many bins the one CTA of a bunch convolves on the fp64 tensor path (wake_first).  Measured, same session, us
+// per turn: c1 (200 bins) 9.81 -> 9.53; c3 (500 bins) 18.9 -> 20.6 -- a column group's accumulator is a chain of n_b / 32
+// dependent DMMAs, and their latency, not their number, is what a single CTA pays -- so the limit sits between.
+constexpr int kDmmaMaxBins = 320;
+__host__ __device__ inline size_t wake_part_bytes(int nb) {  // per-warp partial sums of the tensor-core convolution
+  return nb <= kDmmaMaxBins ? (size_t)(kWakeThreads / 32) * 64 * ((nb + 63) / 64) * sizeof(double) + 16 : 0;
+}
+__host__ __device__ inline size_t wake_smem_bytes(int nb, int M) {
+  return (size_t)(3 * nb + 24) * sizeof(double) + (size_t)M * sizeof(int32_t) + wake_part_bytes(nb);
+}
+// D += A B, A 8x4 (row-major: lane holds A[lane >> 2][lane & 3]), B 4x8 (lane holds B[lane & 3][lane >> 2]),
+// D 8x8 (lane holds D[lane >> 2][2 (lane & 3) + {0, 1}]), all fp64 (SASS: DMMA)
+__device__ __forceinline__ void dmma_8x8x4(double &d0, double &d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
 __host__ __device__ inline size_t scan_smem_bytes(int M, int R) { return (size_t)M * (size_t)R * 3 * sizeof(cplx); }
 
 // The wake of bunch b (and, for the CTA that finishes last, the closing of the turn).  Called by every thread of a CTA of
@@ -300,7 +314,7 @@ __device__ __forceinline__ bool wake_first(const WakeArgs &A, const int b, const
   const bool sources = A.mode == 0 && split == 0 && A.R > 0;
   const cplx *pE = A.Esrc;  // [R][nb] as the source sums read it: staged behind the buckets if the launch's memory holds it
   if (sources && wake_smem_bytes(nb, A.Mg) + (size_t)A.R * nb * sizeof(cplx) + 16 <= (size_t)smem_bytes) {
-    cplx *sE = reinterpret_cast<cplx *>((reinterpret_cast<uintptr_t>(sB + A.Mg) + 15) & ~(uintptr_t)15);
+    cplx *sE = reinterpret_cast<cplx *>(((reinterpret_cast<uintptr_t>(sB + A.Mg) + 15) & ~(uintptr_t)15) + wake_part_bytes(nb));
     const int nE = A.R * nb;
 #pragma unroll 4
     for (int i = tid; i < nE; i += kWakeThreads) sE[i] = A.Esrc[i];
@@ -418,7 +432,54 @@ __device__ __forceinline__ bool wake_first(const WakeArgs &A, const int b, const
   // one output per thread moves 16; the load/store unit, not the fp64 pipe, bounds this loop); a shuffle reduction over
   // the SEG lanes closes the sums.  SEG is the largest power of two that keeps all threads of the bunch's S CTAs busy;
   // segment lengths are odd, so that the lanes of a pair fall into different banks.
-  if (A.w) {
+  if (A.w && !SPLIT && nb <= kDmmaMaxBins) {
+    // One CTA per bunch, up to kDmmaMaxBins bins: the convolution as a dense fp64 contraction on the tensor path (north_star (3)).
+    // With j = 8a + alpha, k = 8(a - d) + beta:  V[alpha][a] = sum_d sum_beta W_d[alpha][beta] Q_d[beta][a],
+    // W_d[alpha][beta] = w[8d + alpha - beta] (an 8x8 Toeplitz block, zero outside the table: causality is the zero
+    // padding in front of it), Q_d[beta][a] = q[8(a - d) + beta]: for every block diagonal d an (8x8)(8 x n_b/8) product,
+    // n_b^2 / 2 multiply-adds in all, none wasted.  mma.m8n8k4 tiles: 8 columns a per tile (a column group g), two k-steps
+    // of four beta.  Warp w takes the diagonals d = w mod 8 for ALL column groups (equal work; the A fragment of a
+    // diagonal serves every group) with one accumulator pair per group; the eight partial results are added in shared
+    // memory in warp order (reproducible).  ~30 DMMA per warp where the DFMA loop issued 640 per thread.
+    const int G = (nb + 63) >> 6;
+    double *part = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(sB + A.Mg) + 15) & ~(uintptr_t)15);  // [NW][64 G]
+    const int al = lane >> 2, k4 = lane & 3;
+    constexpr int GMAX = (kDmmaMaxBins + 63) / 64;
+    double c[GMAX][2];
+#pragma unroll
+    for (int g = 0; g < GMAX; ++g) c[g][0] = c[g][1] = 0.0;
+    for (int d = warp; 8 * d < nb + 7; d += NW) {
+#pragma unroll
+      for (int ks = 0; ks < 2; ++ks) {
+        const int beta = 4 * ks + k4;
+        const int wi = 8 * d + al - beta;                      // >= -7: the zeros in front of the table
+        const double av = wi < nb ? sw[wi] : 0.0;
+#pragma unroll
+        for (int g = 0; g < GMAX; ++g) {
+          if (g < G && 8 * g + 7 >= d) {                       // warp-uniform
+            const int a = 8 * g + al;
+            const int qi = 8 * (a - d) + beta;
+            const double bv = (a >= d && qi < nb) ? sq[qi] : 0.0;
+            dmma_8x8x4(c[g][0], c[g][1], av, bv);
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int g = 0; g < GMAX; ++g)
+      if (g < G) {
+        part[(size_t)warp * 64 * G + (8 * g + 2 * k4) * 8 + al] = c[g][0];
+        part[(size_t)warp * 64 * G + (8 * g + 2 * k4 + 1) * 8 + al] = c[g][1];
+      }
+    __syncthreads();
+    for (int j = tid; j < nb; j += kWakeThreads) {
+      double v = 0.0;
+#pragma unroll
+      for (int w = 0; w < NW; ++w) v += part[(size_t)w * 64 * G + j];
+      A.Vsr[(size_t)b * nb + j] = v;
+      sv[j] = v;
+    }
+  } else if (A.w) {
     constexpr int NO = 8;
     const int J = (nb + NO - 1) / NO, pairs = (J + 1) >> 1;
     const int nthreads = S * kWakeThreads;
