@@ -259,7 +259,7 @@ __device__ __forceinline__ Affine compose(const Affine &first, const Affine &sec
 // window of the register-blocked convolution runs off both ends).  The scan of the turn's last CTA stages its operands
 // (48 bytes per bunch and resonator) in the same memory if they fit into what the launch provides (`smem_bytes`).
 // Up to this many bins the one CTA of a bunch convolves on the fp64 tensor path (wake_first).  Measured, same session, us
-// per turn: c1 (200 bins) 9.81 -> 9.53; c3 (500 bins) 18.9 -> 20.6 -- a column group's accumulator is a chain of n_b / 32
+// per turn: c1 (200 bins) 9.81 -> 9.27; c3 (500 bins) 18.9 -> 20.2 -- a column group's accumulator is a chain of n_b / 32
 // dependent DMMAs, and their latency, not their number, is what a single CTA pays -- so the limit sits between.
 constexpr int kDmmaMaxBins = 320;
 __host__ __device__ inline size_t wake_part_bytes(int nb) {  // per-warp partial sums of the tensor-core convolution
@@ -439,38 +439,40 @@ __device__ __forceinline__ bool wake_first(const WakeArgs &A, const int b, const
     // padding in front of it), Q_d[beta][a] = q[8(a - d) + beta]: for every block diagonal d an (8x8)(8 x n_b/8) product,
     // n_b^2 / 2 multiply-adds in all, none wasted.  mma.m8n8k4 tiles: 8 columns a per tile (a column group g), two k-steps
     // of four beta.  Warp w takes the diagonals d = w mod 8 for ALL column groups (equal work; the A fragment of a
-    // diagonal serves every group) with one accumulator pair per group; the eight partial results are added in shared
-    // memory in warp order (reproducible).  ~30 DMMA per warp where the DFMA loop issued 640 per thread.
+    // diagonal serves every group), an accumulator pair per group and k-step (independent chains); the eight partial
+    // results are added in shared memory in warp order (reproducible).  ~30 DMMA per warp where the DFMA loop issued 640 per thread.
     const int G = (nb + 63) >> 6;
     double *part = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(sB + A.Mg) + 15) & ~(uintptr_t)15);  // [NW][64 G]
     const int al = lane >> 2, k4 = lane & 3;
-    constexpr int GMAX = (kDmmaMaxBins + 63) / 64;
-    double c[GMAX][2];
+    // column groups four at a time, the two k-steps on accumulators of their own: 8 independent DMMA chains in flight
+    for (int g0 = 0; g0 < G; g0 += 4) {
+      double c[4][2][2];
 #pragma unroll
-    for (int g = 0; g < GMAX; ++g) c[g][0] = c[g][1] = 0.0;
-    for (int d = warp; 8 * d < nb + 7; d += NW) {
+      for (int g = 0; g < 4; ++g) c[g][0][0] = c[g][0][1] = c[g][1][0] = c[g][1][1] = 0.0;
+      for (int d = warp; 8 * d < nb + 7 && d <= 8 * (g0 + 3) + 7; d += NW) {
 #pragma unroll
-      for (int ks = 0; ks < 2; ++ks) {
-        const int beta = 4 * ks + k4;
-        const int wi = 8 * d + al - beta;                      // >= -7: the zeros in front of the table
-        const double av = wi < nb ? sw[wi] : 0.0;
+        for (int ks = 0; ks < 2; ++ks) {
+          const int beta = 4 * ks + k4;
+          const int wi = 8 * d + al - beta;                    // >= -7: the zeros in front of the table
+          const double av = wi < nb ? sw[wi] : 0.0;
 #pragma unroll
-        for (int g = 0; g < GMAX; ++g) {
-          if (g < G && 8 * g + 7 >= d) {                       // warp-uniform
-            const int a = 8 * g + al;
-            const int qi = 8 * (a - d) + beta;
-            const double bv = (a >= d && qi < nb) ? sq[qi] : 0.0;
-            dmma_8x8x4(c[g][0], c[g][1], av, bv);
+          for (int g = 0; g < 4; ++g) {
+            if (g0 + g < G && 8 * (g0 + g) + 7 >= d) {         // warp-uniform
+              const int a = 8 * (g0 + g) + al;
+              const int qi = 8 * (a - d) + beta;
+              const double bv = (a >= d && qi < nb) ? sq[qi] : 0.0;
+              dmma_8x8x4(c[g][ks][0], c[g][ks][1], av, bv);
+            }
           }
         }
       }
-    }
 #pragma unroll
-    for (int g = 0; g < GMAX; ++g)
-      if (g < G) {
-        part[(size_t)warp * 64 * G + (8 * g + 2 * k4) * 8 + al] = c[g][0];
-        part[(size_t)warp * 64 * G + (8 * g + 2 * k4 + 1) * 8 + al] = c[g][1];
-      }
+      for (int g = 0; g < 4; ++g)
+        if (g0 + g < G) {
+          part[(size_t)warp * 64 * G + (8 * (g0 + g) + 2 * k4) * 8 + al] = c[g][0][0] + c[g][1][0];
+          part[(size_t)warp * 64 * G + (8 * (g0 + g) + 2 * k4 + 1) * 8 + al] = c[g][0][1] + c[g][1][1];
+        }
+    }
     __syncthreads();
     for (int j = tid; j < nb; j += kWakeThreads) {
       double v = 0.0;
