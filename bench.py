@@ -297,8 +297,13 @@ def run_mbt(args):
                 "algorithmic_bytes_per_launch": bytes_pt * n_part,
                 "pass_ms": pass_s / kp * 1e3, "wake_ms": wake_s / kp * 1e3,
                 "pass_share_of_step": pass_s / (pass_s + wake_s),
+                "whole_step_frac": bytes_pt * n_part / (sec / K) / 1e9 / peak,
                 "timing": "CUDA events around each launch, %d turns of plain launches, started %.1f s after the graph-replayed "
-                          "timed region (same idle start for both; the board is power-capped after ~0.1 s of load)" % (kp, pause_s)}
+                          "timed region (same idle start for both; the board is power-capped after ~0.1 s of load).  pass_ms is the kernel ALONE: "
+                          "events between the launches serialise them, whereas in the graph-replayed step (ms_per_step) the wake kernel "
+                          "runs beside the tail of its pass and the head of the next one (per-bunch flags, DESIGN.md 7.1) -- so the step "
+                          "can be shorter than pass_ms + wake_ms, and even than pass_ms; whole_step_frac = algorithmic bytes / "
+                          "ms_per_step / peak" % (kp, pause_s)}
     # DRAM bytes of one launch from the committed `ncu --set full` capture of this workload (profiles/traffic_<cfg>.txt)
     try:
         with open(os.path.join(ROOT, "profiles", "traffic_%s%s.txt" % (args.config, "t" if args.transverse else ""))) as f:
