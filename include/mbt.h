@@ -237,6 +237,40 @@ int mbt_set_rw_history(mbt_handle *h, const double *in);
 /* out[M][8]: mean x x' y y', rms x x' y y' (population), of the current state */
 int mbt_moments_transverse(mbt_handle *h, double *out);
 
+/* ---- statistics without any device allocation ----
+ * P:l.123-125 (per-bunch mean and standard deviation of the coordinates), the same sums mbt_moments_transverse forms, as
+ * a free-standing call on the CALLER's device arrays that never allocates.
+ *
+ * Who needs it.  The handle-based calls keep their partial sums in memory mbt_create took from cudaMalloc.  Two kinds of
+ * caller cannot work that way: (1) a monitor that samples the beam on a second stream while mbt_track runs -- cudaMalloc
+ * and cudaFree serialise against all work in flight on the device, so an allocating call would stall the very run it
+ * watches; (2) a host that has given all of HBM to its own pool (a caching allocator, a run sized to the card), where a
+ * cudaMalloc issued from inside a library may fail.  Here the partial sums live in a fixed array compiled into the library
+ * (MBT_NOALLOC_MAX_BUNCHES * 8 doubles = 64 KiB, held by every GPU that loads libmbt.so until the process exits); the
+ * call issues one memset and two kernel launches and calls neither cudaMalloc nor cudaFree nor any allocating routine.
+ *
+ * Arguments.  d_x, d_xp, d_y, d_yp: DEVICE arrays [n_bunches][ld] of doubles, the first n_per_bunch entries of each row
+ * are summed (ld >= n_per_bunch; any four coordinate arrays will do, e.g. tau, delta twice).  d_out: DEVICE array
+ * [n_bunches][8], written with mean x, x', y, y', then population rms x, x', y, y' -- the layout of
+ * mbt_moments_transverse.  stream: the cudaStream_t to enqueue on (NULL = the default stream).  The call is
+ * asynchronous: d_out is complete when the stream reaches that point.  All pointers belong to the device that is current
+ * at the call; the caller keeps ownership of all of them.
+ *
+ * Limits and errors.  n_bunches > MBT_NOALLOC_MAX_BUNCHES, n_bunches < 1, n_per_bunch outside 1 .. 2^32-1, ld <
+ * n_per_bunch or a NULL pointer: MBT_EINVAL, nothing enqueued, text in mbt_last_error().  CUDA failures: MBT_ECUDA.
+ *
+ * First call on a device.  It looks up where the fixed array sits on that device (once; later calls reuse the answer).
+ * That look-up can make the CUDA runtime load the library's code onto the device, so make the first call per device
+ * early, before beginning any stream capture.
+ *
+ * Sharing.  There is ONE array per device, shared by every call from every thread and stream, and it keeps the sums of
+ * the last call.  Each call zeroes the rows it uses before accumulating, so calls that follow one another on one stream
+ * are independent.  Calls that can overlap on the GPU (different streams without an ordering between them, or host
+ * threads enqueueing on different streams) race on the array and give wrong statistics: order them, or keep to one stream. */
+#define MBT_NOALLOC_MAX_BUNCHES 1024
+int mbt_bunch_stats_noalloc(const double *d_x, const double *d_xp, const double *d_y, const double *d_yp,
+                            int32_t n_bunches, int64_t n_per_bunch, int64_t ld, double *d_out, void *stream);
+
 /* ---- introspection ---- */
 int64_t mbt_turn(const mbt_handle *h);        /* completed turns, -1 on NULL                 */
 double mbt_phi_s(const mbt_handle *h);        /* synchronous phase of cav[0] [rad]           */

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1640,3 +1641,70 @@ int mbt_normal_selftest(uint64_t seed, int64_t n, const uint32_t *ctr, double *o
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// mbt_bunch_stats_noalloc: the per-bunch statistics of P:l.123-125 for callers that must not allocate device memory.
+//
+// The handle-based statistics calls keep their per-bunch partial sums in a buffer mbt_create obtained with cudaMalloc.
+// Some users of this library cannot afford that: a monitoring hook that runs beside a long mbt_track on a second stream
+// (cudaMalloc and cudaFree serialise against everything in flight on the device, so an allocating call would stall the
+// tracking stream it is meant to watch), and hosts that have handed all of HBM to a pool of their own (a framework's
+// caching allocator, a run sized to the card) where a cudaMalloc from inside a library can simply fail.  For them the
+// partial sums of this entry point live in the fixed array below, which is part of the library image: every GPU that
+// loads libmbt.so carries its 64 KiB until the process exits, and nothing is allocated or freed at call time.
+//
+// g_stats_scratch is a __device__ symbol.  In host code its name is only the host-side shadow of that symbol, NOT a
+// device address -- handing `g_stats_scratch` itself to a kernel would fault (or, on a system whose GPU can reach host
+// memory, quietly sum into the wrong place).  The device address is asked for once per device with
+// cudaGetSymbolAddress, with that device current, and that pointer is what the kernels get.
+static __device__ __align__(256) double g_stats_scratch[MBT_NOALLOC_MAX_BUNCHES * 8];
+
+namespace {
+constexpr int kNoallocMaxDevices = 64;
+double *g_stats_scratch_addr[kNoallocMaxDevices];  // device address of g_stats_scratch on device d; nullptr = not looked up
+std::mutex g_stats_scratch_mutex;
+
+// First call on a device: resolve the array's address there.  The look-up may make the CUDA runtime load this library's
+// module onto the device, which is why the header asks for the first call to be made outside any stream capture.
+int stats_scratch_on_current_device(double **out) {
+  int dev = -1;
+  CU(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNoallocMaxDevices) return fail(MBT_EINVAL, "mbt_bunch_stats_noalloc: device ordinal beyond 63");
+  std::lock_guard<std::mutex> lock(g_stats_scratch_mutex);
+  if (!g_stats_scratch_addr[dev]) {
+    double *p = nullptr;
+    CU(cudaGetSymbolAddress((void **)&p, g_stats_scratch));
+    if (!p) return fail(MBT_ECUDA, "mbt_bunch_stats_noalloc: cudaGetSymbolAddress returned a null address");
+    g_stats_scratch_addr[dev] = p;
+  }
+  *out = g_stats_scratch_addr[dev];
+  return 0;
+}
+}  // namespace
+
+extern "C" int mbt_bunch_stats_noalloc(const double *d_x, const double *d_xp, const double *d_y, const double *d_yp,
+                                       int32_t n_bunches, int64_t n_per_bunch, int64_t ld, double *d_out, void *stream) {
+  if (!d_x || !d_xp || !d_y || !d_yp || !d_out) return fail(MBT_EINVAL, "mbt_bunch_stats_noalloc: null argument");
+  if (n_bunches < 1) return fail(MBT_EINVAL, "mbt_bunch_stats_noalloc: n_bunches must be at least 1");
+  if (n_bunches > MBT_NOALLOC_MAX_BUNCHES) {
+    char buf[192];
+    snprintf(buf, sizeof buf, "mbt_bunch_stats_noalloc: %d bunches exceed the fixed scratch array (MBT_NOALLOC_MAX_BUNCHES = %d); "
+             "split the call or use mbt_moments_transverse", (int)n_bunches, (int)MBT_NOALLOC_MAX_BUNCHES);
+    return fail(MBT_EINVAL, buf);
+  }
+  if (n_per_bunch < 1 || n_per_bunch > 0xFFFFFFFFll) return fail(MBT_EINVAL, "mbt_bunch_stats_noalloc: n_per_bunch must be in 1 .. 2^32-1");
+  if (ld < n_per_bunch) return fail(MBT_EINVAL, "mbt_bunch_stats_noalloc: ld is smaller than n_per_bunch");
+  double *acc = nullptr;
+  if (int rc = stats_scratch_on_current_device(&acc)) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  TMomArgs A;
+  A.x = d_x; A.xp = d_xp; A.y = d_y; A.yp = d_yp; A.ld = ld; A.Np = (uint32_t)n_per_bunch; A.tile = 8192;
+  const int grid_x = (int)((n_per_bunch + A.tile - 1) / A.tile);
+  // The array still holds the sums of whoever called last (on this device, from any thread or stream): the rows this
+  // call accumulates into must start from zero.  A memset of existing memory allocates nothing.
+  CU(cudaMemsetAsync(acc, 0, sizeof(double) * (size_t)n_bunches * 8, st));
+  k_moments_tr<<<dim3(grid_x, n_bunches), 256, 0, st>>>(A, acc);
+  k_close_moments_tr<<<(n_bunches + 127) / 128, 128, 0, st>>>(n_bunches, (uint32_t)n_per_bunch, acc, d_out);
+  CU(cudaGetLastError());
+  return 0;
+}

@@ -22,6 +22,7 @@ SYMBOLS = [
     "mbt_launch_count", "mbt_launches_per_turn",
     "mbt_get_transverse", "mbt_set_transverse", "mbt_get_dipole", "mbt_get_transverse_wake", "mbt_moments_transverse",
     "mbt_get_rw_kick", "mbt_get_rw_history", "mbt_set_rw_history", "mbt_get_transverse_log",
+    "mbt_bunch_stats_noalloc",
     "mbt_last_track_seconds", "mbt_track_profiled", "mbt_philox_selftest", "mbt_normal_selftest", "mbt_last_error", "mbt_version",
 ]
 
@@ -147,6 +148,8 @@ def lib():
         L.mbt_set_rw_history.argtypes = [H, dp]
         L.mbt_philox_selftest.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.mbt_normal_selftest.argtypes = [C.c_uint64, C.c_int64, C.POINTER(C.c_uint32), dp]
+        L.mbt_bunch_stats_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_int64,
+                                              C.c_void_p, C.c_void_p]
         L.mbt_last_error.restype = C.c_char_p
         L.mbt_version.restype = C.c_char_p
         _lib = L
@@ -184,6 +187,19 @@ def shard_range(n_bunches, world, rank):
 def shard_exchange_doubles(n_bunches, world, n_lr):
     """Doubles in the exchange buffer of a sharded handle: world * ceil(n_bunches / world) * n_lr * 2."""
     return int(lib().mbt_shard_exchange_doubles(int(n_bunches), int(world), int(n_lr)))
+
+
+NOALLOC_MAX_BUNCHES = 1024  # MBT_NOALLOC_MAX_BUNCHES of include/mbt.h
+
+
+def bunch_stats_noalloc(d_x, d_xp, d_y, d_yp, n_bunches, n_per_bunch, ld, d_out, stream=0):
+    """mbt_bunch_stats_noalloc: per-bunch mean / rms of four DEVICE arrays [n_bunches][ld] into the DEVICE array
+    d_out[n_bunches][8], for callers that may not allocate device memory (a monitor beside a running mbt_track, a host
+    whose own pool holds all of HBM): the partial sums live in a fixed 64 KiB array inside the library.  All pointer
+    arguments are integer device addresses (e.g. ``tensor.data_ptr()``), `stream` a cudaStream_t as an integer.
+    Asynchronous on `stream`; at most NOALLOC_MAX_BUNCHES bunches; calls overlapping on the GPU race (include/mbt.h)."""
+    _ck(lib().mbt_bunch_stats_noalloc(C.c_void_p(d_x), C.c_void_p(d_xp), C.c_void_p(d_y), C.c_void_p(d_yp), int(n_bunches),
+                                      int(n_per_bunch), int(ld), C.c_void_p(d_out), C.c_void_p(stream)))
 
 
 def philox_selftest(ctr, key):
