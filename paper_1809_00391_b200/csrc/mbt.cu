@@ -328,8 +328,12 @@ cudaError_t enqueue_wakes(mbt_handle *h) {
 #undef MBT_E_
   return e;
 }
-// launches per tracked turn: 1 in the one-launch turn, else 2; 3 with the transverse planes; 4 with their resistive-wall kick
-int launches_per_turn(const mbt_handle *h) { return h->resident ? 0 : h->fused ? 1 : h->trans ? (h->pipe6 ? (h->Krw > 0 ? 3 : 2) : (h->Krw > 0 ? 4 : 3)) : 2; }
+// launches per tracked turn: 1 in the one-launch turn, else 2; 3 with the transverse planes; 4 with their resistive-wall kick;
+// a sharded handle: pass, first half of the wakes, (with long-range resonators) the scatter of the gathered sources, second half
+int launches_per_turn(const mbt_handle *h) {
+  if (h->sharded) return h->R > 0 ? 4 : 3;
+  return h->resident ? 0 : h->fused ? 1 : h->trans ? (h->pipe6 ? (h->Krw > 0 ? 3 : 2) : (h->Krw > 0 ? 4 : 3)) : 2;
+}
 
 cudaError_t enqueue_turn(mbt_handle *h) {
   cudaError_t e = enqueue_pass(h);
@@ -997,7 +1001,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     CUH(h->Sfix.alloc((size_t)M * 2 * (nb + 1), h->stream)); CUH(h->Sov.alloc((size_t)M * 2 * (nb + 1), h->stream));
     // long-range resistive wall (W1..W5): source ring, kick per bunch, weights (d T_rf)^-1/2 by bucket distance d
     h->Krw = tr.rw_turns;
-    CUH(h->ring_g.alloc((size_t)(h->Krw + 1) * M * 2, h->stream));
+    CUH(h->ring_g.alloc((size_t)(h->Krw + 2) * M * 2, h->stream));  // Krw + 1 slots are read per turn, one spare (TWakeArgs)
     CUH(h->rw.alloc((size_t)M * 2, h->stream));
     {
       std::vector<double> wr((size_t)(h->Krw + 1) * rg.h, 0.0);
@@ -1097,6 +1101,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     Tw.log_tr = h->log_cap > 0 ? h->log_tr.p : nullptr;
     Tw.log_cap = h->log_cap;
     Tw.tr_ready = h->tr_ready.p; Tw.use_flags = h->pipe6 ? 1 : 0; Tw.bunch_done_tr = h->bunch_done_tr.p;
+    Tw.rw_ready = h->rw_ready.p;
     h->rwargs.rw_ready = h->rw_ready.p; h->rwargs.tr_ready = h->tr_ready.p; h->rwargs.use_flags = h->pipe6 ? 1 : 0;
     dim3 grid((unsigned)((h->ld + 255) / 256 < 1024 ? (h->ld + 255) / 256 : 1024), (unsigned)M);
     k_init_tr<<<grid, 256, 0, h->stream>>>(h->tx.p, h->txp.p, h->ty.p, h->typ.p, h->ld, (uint32_t)h->Np, A.keys,
@@ -1455,17 +1460,17 @@ int mbt_get_rw_kick(mbt_handle *h, double *kx, double *ky) {
   return 0;
 }
 
-// rows oldest first: row k = turn (turn - Krw + 1 + k), zero for turns < 1; ring slot of turn n' = n' % (Krw + 1)
+// rows oldest first: row k = turn (turn - Krw + 1 + k), zero for turns < 1; ring slot of turn n' = n' % (Krw + 2)
 int mbt_get_rw_history(mbt_handle *h, double *out) {
   if (!h || !h->trans || !out) return fail(MBT_EINVAL, "transverse planes not enabled / null argument");
   CU(cudaSetDevice(h->device));
   const size_t row = (size_t)h->M * 2;
-  std::vector<double> ring((size_t)(h->Krw + 1) * row);
+  std::vector<double> ring((size_t)(h->Krw + 2) * row);
   CU(cudaMemcpyAsync(ring.data(), h->ring_g.p, sizeof(double) * ring.size(), cudaMemcpyDeviceToHost, h->stream));
   CU(cudaStreamSynchronize(h->stream));
   for (int k = 0; k < h->Krw; ++k) {
     const int64_t np = h->turn - h->Krw + 1 + k;
-    for (size_t i = 0; i < row; ++i) out[(size_t)k * row + i] = np >= 1 ? ring[(size_t)(np % (h->Krw + 1)) * row + i] : 0.0;
+    for (size_t i = 0; i < row; ++i) out[(size_t)k * row + i] = np >= 1 ? ring[(size_t)(np % (h->Krw + 2)) * row + i] : 0.0;
   }
   return 0;
 }
@@ -1474,11 +1479,11 @@ int mbt_set_rw_history(mbt_handle *h, const double *in) {
   if (!h || !h->trans || !in) return fail(MBT_EINVAL, "transverse planes not enabled / null argument");
   CU(cudaSetDevice(h->device));
   const size_t row = (size_t)h->M * 2;
-  std::vector<double> ring((size_t)(h->Krw + 1) * row, 0.0);
+  std::vector<double> ring((size_t)(h->Krw + 2) * row, 0.0);
   for (int k = 0; k < h->Krw; ++k) {
     const int64_t np = h->turn - h->Krw + 1 + k;
     if (np < 1) continue;
-    for (size_t i = 0; i < row; ++i) ring[(size_t)(np % (h->Krw + 1)) * row + i] = in[(size_t)k * row + i];
+    for (size_t i = 0; i < row; ++i) ring[(size_t)(np % (h->Krw + 2)) * row + i] = in[(size_t)k * row + i];
   }
   CU(cudaMemcpyAsync(h->ring_g.p, ring.data(), sizeof(double) * ring.size(), cudaMemcpyHostToDevice, h->stream));
   CU(cudaStreamSynchronize(h->stream));

@@ -481,7 +481,9 @@ struct TWakeArgs {
   double *log_tr;             // [log_cap][M][4] mean x, mean y, rms x, rms y per turn, or nullptr
   int64_t log_cap;
   int32_t Krw;                // resistive-wall history depth in turns (0: off)
-  double *ring_g;             // [Krw+1][M][2] source strengths Q_b ubar [C m], slot = turn % (Krw+1)
+  double *ring_g;             // [Krw+2][M][2] source strengths Q_b ubar [C m], slot = turn % (Krw+2): k_rw of a turn reads
+                              // Krw+1 slots; the spare one is what the next turn writes while trailing bunches still read
+  const uint32_t *rw_ready;   // [M] (k_rw's flags) awaited before a ring_g slot is overwritten; used with use_flags only
   const uint32_t *turn_tr;    // the turn being closed (written by the pass; ctrl->turn is k_wake's to bump, beside us)
   FixScale *fix;              // [M][2] in: the scale the sums were deposited with; out: the next turn's
   double *acc2;               // [M][2] in: sum u^2 of this turn's mapped state; out: zero
@@ -564,6 +566,12 @@ __device__ __forceinline__ void wake_tr_body(const TWakeArgs &A, const int b, do
       tox += __shfl_down_sync(0xffffffffu, tox, o); toy += __shfl_down_sync(0xffffffffu, toy, o);
     }
     if ((tid & 31) == 0) { s_ti[tid >> 5][0] = tix; s_ti[tid >> 5][1] = tiy; s_to[tid >> 5][0] = tox; s_to[tid >> 5][1] = toy; }
+    // The slot of turn n last held turn n - Krw - 2, whose last readers are the k_rw CTAs of turn n - 2 (they sum the turns
+    // n - 2 - Krw .. n - 2).  With the per-bunch flags nothing else orders a trailing bunch's k_rw CTA against this write
+    // (a leading bunch runs ahead by design), so wait for every bunch's rw_ready >= n - 2: two turns of slack, true on
+    // arrival in practice, and those CTAs belong to a launch four kernels back (resident or done: no deadlock).
+    if (A.use_flags && A.Krw > 0)
+      for (int bp = tid; bp < A.M; bp += 256) wait_turn(&A.rw_ready[bp], n_turn - 2u);
     __syncthreads();
     if (tid < 2) {
       long long ti = 0;
@@ -571,7 +579,7 @@ __device__ __forceinline__ void wake_tr_body(const TWakeArgs &A, const int b, do
       for (int w = 0; w < 8; ++w) { ti += s_ti[w][tid]; to += s_to[w][tid]; }
       const double total = fma((double)ti, tid == 0 ? fx.lsb : fy.lsb, to);
       const uint32_t n = n_turn;
-      if (A.Krw > 0) A.ring_g[((size_t)(n % (uint32_t)(A.Krw + 1)) * A.M + b) * 2 + tid] = qm * total;
+      if (A.Krw > 0) A.ring_g[((size_t)(n % (uint32_t)(A.Krw + 2)) * A.M + b) * 2 + tid] = qm * total;
       if (A.log_tr && n >= 1u && (int64_t)n <= A.log_cap) {
         const double iN = 1.0 / (double)A.Np, mean = total * iN;
         double *row = A.log_tr + ((size_t)(n - 1u) * A.M + b) * 4;
@@ -684,7 +692,7 @@ __global__ void __launch_bounds__(256, 3) k_wake6(const __grid_constant__ WakeAr
 struct RwArgs {
   int32_t M, Krw, h;
   const int32_t *bucket;  // [M]
-  const double *ring_g;   // [Krw+1][M][2]
+  const double *ring_g;   // [Krw+2][M][2], slot = turn % (Krw+2)
   const double *wrw;      // [(Krw+1) h] weight at bucket distance d (entry 0 unused)
   double amp[2];
   double *rw;             // [M][2] out [V]
@@ -698,7 +706,9 @@ __global__ void __launch_bounds__(256) k_rw(const __grid_constant__ RwArgs A) {
   const int b = blockIdx.x, tid = threadIdx.x;
   griddep_launch_dependents();  // the next pass may come in: its CTAs wait for rw_ready
   // per-bunch sequencing: this turn's sources are those of the bunches AHEAD (W5); each is awaited through its tr_ready
-  // flag below (CTAs of k_wake6, all resident or done before this kernel was let in); earlier turns are long complete
+  // flag below (CTAs of k_wake6, all resident or done before this kernel was let in).  The sources of the turns before
+  // come from every bunch, also the trailing ones, whose k_wake6 CTA of turn n - 1 no launch boundary orders against
+  // this CTA: they are awaited as tr_ready >= n - 1 (true on arrival in practice).
   const uint32_t n = A.use_flags ? __ldcg(&A.rw_ready[b]) + 1u : *A.turn_tr;
   const int sb = A.bucket[b];
   double sx = 0.0, sy = 0.0;
@@ -707,9 +717,9 @@ __global__ void __launch_bounds__(256) k_rw(const __grid_constant__ RwArgs A) {
   const int kmax = min(A.Krw, (int)min(n - 1u, (uint32_t)A.Krw));  // nothing before turn 1
   for (int bp = tid; bp < A.M; bp += 256) {
     const int ds = sb - A.bucket[bp];
-    if (A.use_flags && ds > 0) wait_turn(&A.tr_ready[bp], n);
+    if (A.use_flags) wait_turn(&A.tr_ready[bp], ds > 0 ? n : n - 1u);
     const double2 *g = reinterpret_cast<const double2 *>(A.ring_g) + bp;
-    uint32_t slot = n % (uint32_t)(A.Krw + 1);
+    uint32_t slot = n % (uint32_t)(A.Krw + 2);
 #pragma unroll 4
     for (int k = 0; k <= kmax; ++k) {  // source: turn n - k, bunch bp, bucket distance d
       const int d = k * A.h + ds;
@@ -717,7 +727,7 @@ __global__ void __launch_bounds__(256) k_rw(const __grid_constant__ RwArgs A) {
       const double2 gv = __ldcg(&g[(size_t)slot * A.M]);
       sx = fma(gv.x, w, sx);
       sy = fma(gv.y, w, sy);
-      slot = slot == 0u ? (uint32_t)A.Krw : slot - 1u;
+      slot = slot == 0u ? (uint32_t)A.Krw + 1u : slot - 1u;
     }
   }
 #pragma unroll

@@ -239,6 +239,31 @@ def test_resistive_wall_growth_rate_long_run(mbt, orc):
     assert abs(rates[1] / rates[0] - 1) < 0.05, rates
 
 
+@pytest.mark.parametrize("rw_turns,m,npb", [(1, 5, 64), (2, 5, 33), (1, 40, 16), (3, 7, 64)])
+def test_resistive_wall_ring_under_per_bunch_sequencing(mbt, rw_turns, m, npb):
+    """The source ring of the resistive-wall kick (ring_g) under the per-bunch flags of DESIGN.md 7.1: a leading bunch may
+    start its next turn while the k_rw CTA of a trailing bunch still sums this one, so the slot the next turn writes must
+    not be one this turn reads (the ring has rw_turns + 2 slots and the writer waits for the readers of two turns back).
+    Tiny bunches, short histories and hundreds of turns are where kernels of consecutive turns overlap most; the run
+    must equal, bit for bit, the same library with grid-wide waits (per_bunch_start = 1)."""
+    turns = 400
+    buckets = sorted(set(int(b) for b in np.linspace(0, 482, m)))
+    cfg = _cfg(tr=dict(rw_amp_x=2.0e9, rw_amp_y=1.0e9, rw_turns=rw_turns), m=len(buckets), buckets=buckets, n_per_bunch=npb,
+               n_bins=8)
+    with mbt.Tracker(cfg, log_capacity_turns=turns, tuning=dict(per_bunch_start=2)) as ta, \
+            mbt.Tracker(cfg, log_capacity_turns=turns, tuning=dict(per_bunch_start=1)) as tb:
+        for n in (turns // 3, 1, turns - turns // 3 - 1):
+            ta.track(n); tb.track(n)
+        for a, b in zip(ta.transverse_particles(), tb.transverse_particles()):
+            assert np.array_equal(a, b)
+        assert np.array_equal(ta.rw_history(), tb.rw_history())
+        for a, b in zip(ta.rw_kick(), tb.rw_kick()):
+            assert np.array_equal(a, b)
+        la, lb = ta.transverse_log(1, turns), tb.transverse_log(1, turns)
+        assert np.array_equal(la[..., :2], lb[..., :2])                  # centroids: from the exact integer totals
+        assert np.allclose(la[..., 2:], lb[..., 2:], rtol=1e-9, atol=0)  # rms: sums of squares added by fp64 atomics
+
+
 def test_transverse_log_matches_oracle(mbt, orc):
     """Per-turn log of mean / rms x, y (P:l.123) from the pass's own sums, twelve turns without re-synchronisation; one
     bunch displaced by 20 sigma (mean >> rms: the single-pass variance must survive the cancellation)."""
