@@ -183,7 +183,7 @@ def run_sharded(args):
     """--sharded: the opt-in bunch-sharded path: the fill's bunches are split over the ranks, one
     all-gather of the source phasors per turn (NCCL; none at N = 1).  STRONG scaling: the workload is fixed.  Not the
     default line (BASELINE north_star fixes one GPU, no collectives); at N = 1 it measures what the host-driven turn
-    (three launches and a host round trip per turn, no graph) costs against mbt_track."""
+    (three or four plain launches per turn enqueued by the host, no graph) costs against mbt_track."""
     import torch
     import torch.distributed as dist
     from paper_1809_00391_b200 import build, sharded, workloads as W
@@ -204,9 +204,11 @@ def run_sharded(args):
         dist.barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
+    l0 = trk.tracker.launch_count
     e0.record(trk.stream)
     trk.track(K)
     e1.record(trk.stream)
+    launches = trk.tracker.launch_count - l0     # what the handle counted: 3 per turn, 4 with long-range resonators
     torch.cuda.synchronize()
     sec = e0.elapsed_time(e1) * 1e-3
     if world > 1:
@@ -219,7 +221,7 @@ def run_sharded(args):
         line = {"metric": METRIC, "value": n_part * K / sec, "unit": "particle-turns/s", "n_gpus": world, "steps": K, "warmup": Wm,
                 "ms_per_step": sec / K * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
                 "data": "synthetic", "config": dict(_config_keys(args, world), parallelism="bunch-sharded x%d" % world),
-                "roofline": None, "gpu_launches": int(4 * K),
+                "roofline": None, "gpu_launches": int(launches),
                 "note": "opt-in sharded path: mbt_shard_turn_begin / all_gather_into_tensor / mbt_shard_turn_end per turn"}
         print(json.dumps(line))
     trk.close()

@@ -299,7 +299,9 @@ int mbt_invalidate(mbt_handle *h);
 /* kernels launched by this handle so far (bench.py's gpu_launches) */
 int64_t mbt_launch_count(const mbt_handle *h);
 /* kernel launches per tracked turn of this handle: 1 (one-launch turn), 2 (k_pass, k_wake), 3 / 4 with the transverse
- * planes (+ k_wake_tr, + k_rw); 0 for the chip-resident turn loop (one launch per mbt_track call); -1 on NULL */
+ * planes (+ k_wake_tr, + k_rw); a sharded handle: 3, or 4 with long-range resonators (mbt_shard_turn_begin: pass, first half
+ * of the wakes; mbt_shard_turn_end: scatter of the gathered sources, second half); 0 for the chip-resident turn loop (one
+ * launch per mbt_track call); -1 on NULL */
 int mbt_launches_per_turn(const mbt_handle *h);
 /* Seconds of device time of the most recent mbt_track call, measured with CUDA events recorded on the handle's
  * stream around the enqueued turns; synchronises.  Negative on error. */

@@ -545,7 +545,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   const mbt_tuning &tn = p->tuning;
   if (tn.tile_iters < 0 || tn.pairs_per_thread < 0 || tn.pairs_per_thread > 2 || tn.pdl < 0 || tn.pdl > 3 || tn.stages6 < 0 ||
       (tn.stages6 != 0 && (tn.stages6 < 2 || tn.stages6 > kMaxStages6)) || tn.turn_mode < 0 || tn.turn_mode > 3 ||
-      tn.verbose < 0 || tn.per_bunch_start < 0 || tn.per_bunch_start > 3 || tn.reserved[0] < 0)
+      tn.verbose < 0 || tn.per_bunch_start < 0 || tn.per_bunch_start > 3 || tn.reserved[0] != 0)
     return fail(MBT_EINVAL, "tuning: a member is out of range (see mbt_tuning in mbt.h; all zero = the library's choice)");
   int n_lr = 0;
   for (int r = 0; r < wk.n_res; ++r) {

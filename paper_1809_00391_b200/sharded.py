@@ -5,6 +5,10 @@ kernels; this module allocates the exchange buffer (a torch tensor), and per tur
     mbt_shard_turn_begin  ->  all_gather_into_tensor(exchange)  ->  mbt_shard_turn_end
 
 on one CUDA stream.  The default path of the repository is one GPU (BASELINE north_star: "no sharding, no collectives").
+
+Validation status: the turn halves are checked on one GPU with the all-gather EMULATED by copies (tests/test_gpu_sharded.py)
+and the partition / layout logic over two gloo ranks on CPU (tests/test_shard_host.py).  The in-place NCCL
+all_gather_into_tensor below has not yet run on more than one GPU (no multi-GPU box was available to this build).
 """
 from __future__ import annotations
 
@@ -36,10 +40,13 @@ class ShardedTracker:
         m = len(cfg["fill"]["buckets"])
         self.rows, self.per_rank, total = exchange_layout(m, self.world, n_lr)
         assert total == mbt.shard_exchange_doubles(m, self.world, n_lr)
-        self.exchange = torch.zeros(max(total, 2), dtype=torch.float64, device=self.device)
+        self.stream = torch.cuda.Stream(self.device)   # the library's kernels and the collective are ordered on this stream
+        # The exchange buffer is zero-filled ON that stream: torch streams do not wait for the default stream, so a fill
+        # enqueued there could land after the first turn's source phasors had been written.
+        with torch.cuda.stream(self.stream):
+            self.exchange = torch.zeros(max(total, 2), dtype=torch.float64, device=self.device)
         self._own = self.exchange[self.rank * self.per_rank:(self.rank + 1) * self.per_rank]
         self._all_gather = all_gather   # test hook: a callable(exchange tensor, own slice) replacing the collective
-        self.stream = torch.cuda.Stream(self.device)   # the library's kernels and the collective are ordered on this stream
         self.tracker = mbt.Tracker(cfg, log_capacity_turns=log_capacity_turns, stream=self.stream.cuda_stream, device=device,
                                    shard=dict(rank=self.rank, world=self.world, d_exchange=self.exchange.data_ptr() if n_lr else None))
         self.n_lr = n_lr

@@ -96,6 +96,18 @@ def test_make_params_marshalling():
         mbt.make_params(cfg, tuning=dict(no_such_knob=1))
 
 
+def test_create_refuses_nonzero_reserved_tuning_word(libpath):
+    """mbt.h: mbt_tuning.reserved "must be 0" -- any other value is MBT_EINVAL at validation, before a device is touched."""
+    from paper_1809_00391_b200 import mbt
+    L = mbt.lib()
+    for bad in (1, -1):
+        p, keep = mbt.make_params(W.config("c1"))
+        p.tuning.reserved[0] = bad
+        h = ctypes.c_void_p()
+        assert L.mbt_create(ctypes.byref(p), ctypes.byref(h)) == -1 and not h.value
+        assert b"tuning" in L.mbt_last_error()
+
+
 def test_workloads_match_baseline_configs():
     shapes = {"c1": (1, 10_000, 200, 0, 1000), "c2": (1, 1_000_000, 1000, 0, 10_000), "c3": (3, 100_000, 500, 10, 20_000),
               "c4": (363, 100_000, 300, 20, 10_000), "c5": (484, 200_000, 500, 50, 5_000)}
