@@ -40,6 +40,9 @@
 //                   damping rate and equilibrium emittance (tests/test_oracle_transverse.py)
 //   resistive wall  partial sums of k^-1/2 for a frozen offset, contiguous distance sum for a uniform fill, pairwise
 //                   brute force, coupled-bunch growth / damping rates vs first-order theory (tests/test_oracle_rw.py)
+//   history setters  orc_set_lr_history (rebuilds the per-turn aggregates ring_A) and orc_set_rw_history: checkpoint /
+//                   resume into a fresh oracle is bit-identical to the uninterrupted run, both lr_modes, and is not
+//                   when either setter is left out (tests/test_oracle_resume.py)
 // No function of this file is "parity unpinned".
 #include "orc.h"
 
