@@ -117,7 +117,7 @@ def test_single_turn_parity_tiny(mbt, orc, name, turn_mode):
             assert_single_turn_parity(o, t, cfg)
 
 
-@pytest.mark.parametrize("turn_mode", [0, 1])    # the library's choice (one launch per turn) / two launches per turn
+@pytest.mark.parametrize("turn_mode", [0, 1])    # the library's choice (today: two launches per turn) / two launches, spelled out
 @pytest.mark.parametrize("name,over", [
     ("c1", dict()),
     ("c2", dict()),                       # full size: 1e6 particles, the tiling bench.py --config c2 times

@@ -63,11 +63,14 @@ class Ranks:
         ws = [t.wake() for t in self.t]
         return [np.concatenate([w[k] for w in ws]) for k in range(3)]
 
-    def resume(self, o):
+    def resume(self, o, window=False):
         tau, delta = o.particles()
         for t in self.t:
             sl = slice(t.first_bunch, t.first_bunch + t.M)
             t.set_particles(tau[sl], delta[sl], o.turn)
+            if window:                                           # after set_particles, which resets the shifts; own bunches only
+                s_hist, s_next = o.window()
+                t.set_window(s_hist[sl], s_next[sl])
             t.set_lr_history(o.lr_history())                     # every rank holds the whole history
         return tau, delta
 
@@ -103,6 +106,54 @@ def test_sharded_single_turns_match_oracle(mbt, orc, world, kw):
                 assert t.lr_history().shape == hist_c.shape
                 if hist_c.size:
                     assert np.allclose(t.lr_history(), hist_c, rtol=0, atol=1e-10 * np.abs(hist_c).max())
+    finally:
+        R.close()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_sharded_with_bunch_following_window(mbt, orc, world):
+    """mbt_shard with window_mode = 1 (reading D31): every bunch displaced differently, so the per-bunch window shifts
+    differ across the ranks' bunches.  The shift of a bunch's window multiplies its long-range SOURCE phasor (indexed by the
+    rank's LOCAL bunch) and the phasor it WITNESSES, which is summed over ring rows and ready-flags indexed by the GLOBAL
+    bunch -- the local / global mix this test walks through.  Single turns from the oracle's state incl. its windows, then
+    turns without re-synchronisation; launches_per_turn of a sharded handle is 4 with long-range resonators."""
+    cfg = W.tiny(m=5, n_per_bunch=1501, n_bins=32, k_hist=3, n_lr=2)
+    cfg["wake"]["window_mode"] = 1
+    o = orc.Oracle(cfg, lr_mode=0)
+    tau0, delta0 = o.particles()
+    off = np.array([[12e-12], [-20e-12], [0.0], [30e-12], [-8e-12]])
+    o.set_particles(tau0 * 0.5 + off, delta0, 0)
+    o.track(4)
+    R = Ranks(mbt, cfg, world)
+    try:
+        assert all(t.launches_per_turn == 4 for t in R.t)
+        for _ in range(3):
+            R.resume(o, window=True)
+            o.track(1)
+            R.track(1)
+            tau_c, delta_c = o.particles()
+            tau_g, delta_g = R.particles()
+            assert particle_errors(tau_g, tau_c) <= TOL_PARTICLE and particle_errors(delta_g, delta_c) <= TOL_PARTICLE
+            sh_c, sn_c = o.window()
+            sh_g = np.concatenate([t.window()[0] for t in R.t]); sn_g = np.concatenate([t.window()[1] for t in R.t])
+            assert np.array_equal(sh_c, sh_g) and np.array_equal(sn_c, sn_g)
+            bad, _ = histogram_mismatch(R.gather("histogram"), o.histogram(), tau_c, cfg, shifts=sh_c)
+            assert bad == 0
+            for g, c in zip(R.wake(), o.wake()):
+                assert wake_error(g, c) <= 1e-10
+        assert len(set(int(s) for s in o.window()[0])) >= 3      # the windows really sit in different places
+        # own runs from the same displaced start, no re-synchronisation
+        o2 = orc.Oracle(cfg, lr_mode=0)
+        o2.set_particles(tau0 * 0.5 + off, delta0, 0)
+        for t in R.t:
+            sl = slice(t.first_bunch, t.first_bunch + t.M)
+            t.set_particles((tau0 * 0.5 + off)[sl], delta0[sl], 0)
+        o2.track(8)
+        R.track(8)
+        assert np.array_equal(np.concatenate([t.window()[0] for t in R.t]), o2.window()[0])
+        assert np.array_equal(R.gather("histogram"), o2.histogram())
+        assert particle_errors(R.particles()[1], o2.particles()[1]) <= 1e-10
+        assert wake_error(R.wake()[0], o2.wake()[0]) <= 1e-9
     finally:
         R.close()
 
