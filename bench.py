@@ -88,7 +88,7 @@ class ClockSampler:
             self.proc.wait(timeout=5)
         except Exception:
             self.proc.kill()
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         try:
             with open(self.path) as f:
                 for line in f:
@@ -99,6 +99,10 @@ class ClockSampler:
                         sm.append(float(c[1])); mx.append(float(c[2]))
                     except ValueError:
                         continue
+                    try:
+                        pw.append(float(c[3]))          # board power draw [W]
+                    except ValueError:
+                        pass
                     for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
                         if v.lower().startswith("active"):
                             reasons.add(name)
@@ -108,6 +112,9 @@ class ClockSampler:
         if sm:
             sm.sort()
             out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        if pw:
+            pw.sort()
+            out.update(power_w=pw[len(pw) // 2])        # median of the samples taken during the region
         return out
 
 
@@ -341,6 +348,10 @@ def run_mbt(args):
                      "pass_ms": pass_s2 / kp2 * 1e3, "wake_ms": wake_s2 / kp2 * 1e3,
                      "frac": bytes_pt * n_part / (pass_s2 / kp2) / 1e9 / peak,
                      "whole_step_frac": bytes_pt * n_part / (sec_s / T) / 1e9 / peak, "clocks": clocks2,
+                     # energy: median board power of rank 0's GPU over the region x the time of a turn / particles of a turn
+                     "power_w_median": (clocks2 or {}).get("power_w"),
+                     "joules_per_particle_turn": ((clocks2["power_w"] * (sec_s / T) / n_part)
+                                                  if clocks2 and clocks2.get("power_w") else None),
                      "what": "mbt_track(%d) of the config's %d turns, graph replay, CUDA events; then %d event-bracketed turns "
                              "with no pause (pass_ms, frac: the dominant kernel in the power-capped state)" % (T, cfg["n_turns"], kp2)}
     trk.close()

@@ -224,13 +224,13 @@ int mbt_set_transverse(mbt_handle *h, const double *x, const double *xp, const d
  * K[b][j] = sum_{k<j} (Q_b/N_p) S[b][k] W_perp((j-k) Delta) [V] of the last tracked turn (NULL entries are skipped) */
 int mbt_get_dipole(mbt_handle *h, double *Sx, double *Sy);
 int mbt_get_transverse_wake(mbt_handle *h, double *Kx, double *Ky);
-/* resistive-wall kick of the last tracked turn per bunch [V] (kx[M], ky[M]; NULL entries are skipped); source strengths
- * Q_b ubar [C m] of the last rw_turns turns, oldest first: [rw_turns][M][2] (x, y) -- get / set as the long-range
- * history (set after mbt_set_particles, which fixes the turn the rows refer to) */
 /* per-turn log of the transverse statistics (P:l.123), kept on the device when log_capacity_turns > 0:
  * out[n][M][4] = mean x, mean y, rms x, rms y of the state at the end of turns first_turn .. first_turn+n-1 (from the
  * pass's own sums: no extra pass over the particles).  MBT_ESTATE if the turns are not in the log. */
 int mbt_get_transverse_log(mbt_handle *h, int64_t first_turn, int64_t n, double *out);
+/* resistive-wall kick of the last tracked turn per bunch [V] (kx[M], ky[M]; NULL entries are skipped); source strengths
+ * Q_b ubar [C m] of the last rw_turns turns, oldest first: [rw_turns][M][2] (x, y) -- get / set as the long-range
+ * history (set after mbt_set_particles, which fixes the turn the rows refer to) */
 int mbt_get_rw_kick(mbt_handle *h, double *kx, double *ky);
 int mbt_get_rw_history(mbt_handle *h, double *out);
 int mbt_set_rw_history(mbt_handle *h, const double *in);

@@ -22,13 +22,9 @@ namespace {
 
 thread_local std::string g_err;
 
-// mbt_tuning.turn_mode 0: two launches per turn.  The one-launch turn is complete and parity-tested, but measured slower on
-// every BASELINE workload: a bunch's wake costs its closing CTA ~15 us of latency-bound work during
-// which it holds one of the pass's 296 CTA slots (c4: 0.238 vs 0.218 ms per turn).
-constexpr bool kFusedTurnDefault = false;
-// mbt_tuning.turn_mode 0 picks the chip-resident turn loop for workloads of at most this many particles that fit on chip
-constexpr bool kResidentAuto = false;
-constexpr int64_t kResidentAutoMaxParticles = 2000000;
+// mbt_tuning.turn_mode 0 (the library's choice) is always two launches per turn.  The one-launch turn (turn_mode 2) and the
+// chip-resident turn loop (turn_mode 3) are complete and parity-tested, but measured slower on every BASELINE workload
+// (DESIGN.md sections 7.5, 7.6; e.g. c4: 0.238 vs 0.218 ms per turn), so neither is ever picked automatically.
 
 int fail(int code, const std::string &msg) {
   g_err = msg;
@@ -902,7 +898,7 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
   A.bunch_ready = h->bunch_ready.p;
   // a pass CTA starts on its own bunch's wake (one k_wake CTA per bunch publishes bunch_ready) instead of on the whole grid
   A.flag_wait = (!tr.enable && !sh.enable && h->wargs.gather_P && tn.per_bunch_start != 1) ? 1 : 0;
-  h->fused = !tr.enable && !sh.enable && (tn.turn_mode == 2 || (tn.turn_mode == 0 && kFusedTurnDefault));
+  h->fused = !tr.enable && !sh.enable && tn.turn_mode == 2;
   if (tn.turn_mode == 2 && tr.enable) {
     destroy(h);
     return fail(MBT_EINVAL, "tuning.turn_mode 2 (one launch per turn) is not available with the transverse planes");
@@ -922,10 +918,9 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
     fprintf(stderr, "mbt: %s, %d pair(s) per thread, grid %d x %d, %zu B shared memory per CTA, pdl %d\n",
             h->fused ? "one launch per turn" : "two launches per turn", h->npair, h->grid_pass, M, h->smem_pass, h->pdl);
 
-  // ---- chip-resident turn loop (mbt_tuning.turn_mode 3; the library's choice when it fits and the workload is small
-  // enough to be latency-bound in the streaming path): grid = M x G_b CTAs, all resident (cooperative launch), each
-  // holding tile_pairs pairs of one bunch in shared memory
-  if (!tr.enable && !sh.enable && (tn.turn_mode == 3 || (tn.turn_mode == 0 && kResidentAuto))) {
+  // ---- chip-resident turn loop (mbt_tuning.turn_mode 3 only): grid = M x G_b CTAs, all resident (cooperative launch),
+  // each holding tile_pairs pairs of one bunch in shared memory
+  if (!tr.enable && !sh.enable && tn.turn_mode == 3) {
     res_fn fn = select_resident(rad_on, wk.gather_order, p->n_cav);
     const int64_t ppb = h->ld / 2, stride = (int64_t)kPassThreads * 2;
     bool ok = false;
@@ -945,8 +940,6 @@ int mbt_create(const mbt_params *p, mbt_handle **out) {
       int coop = 0;
       cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
       if (!coop) continue;
-      // the automatic choice is for the latency-bound workloads only: a few waves' worth of streaming work per turn
-      if (tn.turn_mode == 0 && (int64_t)M * h->Np > kResidentAutoMaxParticles) continue;
       ok = true;
       h->resident = true;
       h->fn_res = fn;

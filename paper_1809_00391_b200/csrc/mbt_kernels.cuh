@@ -3,8 +3,10 @@
 // One turn = two launches:
 //   k_pass  the fused particle pass (S0 kick of the previous turn, S7 moments, S1 RF, S2 radiation,
 //           S3 drift, S4 binning), one read and one write of the SoA fp64 particle store;
-//   k_wake  per bunch: counts -> charges, S5 Toeplitz short-range convolution, S6 source phasors; the
-//           last CTA to finish runs the S6 in-turn phasor scan over the fill pattern and the history ring.
+//   k_wake  per bunch: counts -> charges, S5 Toeplitz short-range convolution, S6 source phasors, and (the default,
+//           one CTA per bunch) the bunch's own phasor gathered from the sources of the bunches ahead and the history
+//           ring, as soon as those are flagged ready; where a bunch is split over several CTAs the last CTA to finish
+//           runs the S6 in-turn phasor scan over the fill pattern instead.
 // The long-range part of the wake is kept as ONE complex number per (bunch, resonator) and expanded onto the
 // bins when a CTA of the next pass stages the bunch's wake grid in shared memory.
 //
@@ -639,6 +641,9 @@ __device__ __forceinline__ void wake_second(const WakeArgs &A, const int b, doub
       __threadfence();
       st_release_u32(&A.bunch_ready[b], n);
       s_last = (atomicAdd(&A.ctrl->ticket[n & 1u], 1u) == (uint32_t)(M - 1));
+      // All M tickets of turn n are taken: the counter goes back to zero at once, before anything this CTA publishes can
+      // let turn n + 2 (the next user of this word) advance -- not after the release of agg_ready, as it used to.
+      if (s_last) A.ctrl->ticket[n & 1u] = 0u;
     }
     __syncthreads();
     if (!s_last) return;
@@ -669,7 +674,6 @@ __device__ __forceinline__ void wake_second(const WakeArgs &A, const int b, doub
     if (tid == 0) {
       __threadfence();
       st_release_u32(A.agg_ready, n);
-      A.ctrl->ticket[n & 1u] = 0u;
       A.ctrl->kick_pending = 1u;
       A.ctrl->turn = n;
     }
